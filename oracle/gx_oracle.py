@@ -1,0 +1,148 @@
+"""ctypes wrapper around oracle/gx_oracle.c (plain C, gcc -O2 -ffp-contract=off, OpenMP over environments).
+
+TEST INFRASTRUCTURE, NOT PRODUCT -- see the header of gx_oracle.c.  Argument marshalling only; every
+step of the definition (N0-N10) is in the C file.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gx_oracle.c")
+_LIB = os.path.join(_HERE, "libgx_oracle.so")
+BACKGROUND_ID = 0xFFFFFFFF
+FLAG_FULL_SCAN = 1
+
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle (building the checker is not using it)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        cmd = ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-std=c11", "-Wall", "-Wextra",
+               "-shared", "-fPIC", "-o", tmp, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Mesh(C.Structure):
+    _fields_ = [("positions", C.c_void_p), ("colors", C.c_void_p), ("indices", C.c_void_p),
+                ("nv", C.c_uint32), ("nt", C.c_uint32)]
+
+
+class _Camera(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float),
+                ("znear", C.c_float), ("zfar", C.c_float)]
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+        _lib.gx_oracle_render.restype = C.c_int
+        _lib.gx_oracle_raster_soup.restype = C.c_int
+        _lib.gx_oracle_vertex_stage.restype = C.c_int
+    return _lib
+
+
+def _p(a: Optional[np.ndarray]):
+    return None if a is None else C.c_void_p(a.ctypes.data)
+
+
+def _meshes(meshes):
+    keep = []
+    arr = (_Mesh * max(1, len(meshes)))()
+    for i, m in enumerate(meshes):
+        pos = np.ascontiguousarray(m.positions, np.float32)
+        col = np.ascontiguousarray(m.colors, np.uint8)
+        idx = np.ascontiguousarray(m.indices, np.uint32)
+        keep += [pos, col, idx]
+        arr[i] = _Mesh(pos.ctypes.data, col.ctypes.data, idx.ctypes.data, pos.shape[0], idx.shape[0])
+    return arr, keep
+
+
+def _camera(W, H, fx, fy, znear, zfar):
+    return _Camera(int(W), int(H), float(fx), float(fy), float(znear), float(zfar))
+
+
+def render(wl, n_threads: Optional[int] = None, want_sub: bool = False, want_count: bool = False,
+           full_scan: bool = False):
+    """Render a workload (any object with the fields of gen.Workload).  Returns dict(rgb, depth, id[, sub, count])."""
+    lib = _load()
+    N, K, W, H = wl.N, wl.K, wl.width, wl.height
+    sm, k1 = _meshes(wl.static_meshes)
+    dm, k2 = _meshes(wl.dyn_meshes)
+    cam = _camera(W, H, wl.fx, wl.fy, wl.znear, wl.zfar)
+    env_scene = np.ascontiguousarray(wl.env_scene, np.int32)
+    cam_pose = np.ascontiguousarray(wl.cam_pose, np.float32)
+    inst_mesh = np.ascontiguousarray(wl.inst_mesh, np.int32)
+    inst_xform = np.ascontiguousarray(wl.inst_xform, np.float32)
+    rgb = np.empty((N, H, W, 3), np.uint8)
+    depth = np.empty((N, H, W), np.float32)
+    ids = np.empty((N, H, W), np.uint32)
+    sub = np.empty((N, H, W), np.uint8) if want_sub else None
+    cnt = np.empty((N, H, W), np.uint32) if want_count else None
+    if n_threads is None:
+        n_threads = len(os.sched_getaffinity(0))
+    rc = lib.gx_oracle_render(sm, C.c_int32(len(wl.static_meshes)), dm, C.c_int32(len(wl.dyn_meshes)), C.byref(cam),
+                              C.c_int32(N), C.c_int32(K), _p(env_scene), _p(cam_pose), _p(inst_mesh), _p(inst_xform),
+                              _p(rgb), _p(depth), _p(ids), _p(sub), _p(cnt),
+                              C.c_int32(FLAG_FULL_SCAN if full_scan else 0), C.c_int32(int(n_threads)))
+    if rc != 0:
+        raise RuntimeError(f"gx_oracle_render failed: {rc}")
+    out = dict(rgb=rgb, depth=depth, id=ids)
+    if want_sub:
+        out["sub"] = sub
+    if want_count:
+        out["count"] = cnt
+    return out
+
+
+def raster_soup(W, H, fx, fy, znear, zfar, verts: np.ndarray, ids: Sequence[int], want_count=False,
+                full_scan=False):
+    """N4-N9 on a camera-space soup: verts [nt,3,6] = (xc, yc, w, r, g, b); ids [nt]."""
+    lib = _load()
+    verts = np.ascontiguousarray(verts, np.float32)
+    nt = verts.shape[0]
+    assert verts.shape == (nt, 3, 6)
+    ids = np.ascontiguousarray(ids, np.uint32)
+    assert ids.shape == (nt,)
+    cam = _camera(W, H, fx, fy, znear, zfar)
+    rgb = np.empty((H, W, 3), np.uint8)
+    depth = np.empty((H, W), np.float32)
+    oid = np.empty((H, W), np.uint32)
+    sub = np.empty((H, W), np.uint8)
+    cnt = np.empty((H, W), np.uint32) if want_count else None
+    rc = lib.gx_oracle_raster_soup(C.byref(cam), _p(verts), _p(ids), C.c_uint32(nt), _p(rgb), _p(depth), _p(oid),
+                                   _p(sub), _p(cnt), C.c_int32(FLAG_FULL_SCAN if full_scan else 0))
+    if rc != 0:
+        raise RuntimeError(f"gx_oracle_raster_soup failed: {rc}")
+    out = dict(rgb=rgb, depth=depth, id=oid, sub=sub)
+    if want_count:
+        out["count"] = cnt
+    return out
+
+
+def vertex_stage(W, H, fx, fy, znear, zfar, cam_pose, xform, positions):
+    """N1-N3 + N5 per vertex.  Returns dict(xc, yc, w, q, Xi, Yi, inside)."""
+    lib = _load()
+    cam = _camera(W, H, fx, fy, znear, zfar)
+    cam_pose = np.ascontiguousarray(cam_pose, np.float32).reshape(16)
+    xf = None if xform is None else np.ascontiguousarray(xform, np.float32).reshape(16)
+    pos = np.ascontiguousarray(positions, np.float32)
+    nv = pos.shape[0]
+    o = dict(xc=np.empty(nv, np.float32), yc=np.empty(nv, np.float32), w=np.empty(nv, np.float32),
+             q=np.empty(nv, np.float32), Xi=np.empty(nv, np.int32), Yi=np.empty(nv, np.int32),
+             inside=np.empty(nv, np.uint8))
+    rc = lib.gx_oracle_vertex_stage(C.byref(cam), _p(cam_pose), _p(xf), _p(pos), C.c_uint32(nv), _p(o["xc"]),
+                                    _p(o["yc"]), _p(o["w"]), _p(o["q"]), _p(o["Xi"]), _p(o["Yi"]), _p(o["inside"]))
+    if rc != 0:
+        raise RuntimeError(f"gx_oracle_vertex_stage failed: {rc}")
+    return o

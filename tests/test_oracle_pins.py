@@ -1,0 +1,557 @@
+"""Pins of the CPU oracle against what the mathematics fixes (run with -m "not gpu").
+
+The paper prints no worked rendering example (PAPER.md:91,141 give only the problem statement), so the
+pins are closed forms, exact brute force, double-precision ray casting and invariants, chosen so that a
+dropped term, wrong sign/index or transposed operand in oracle/gx_oracle.c fails at least one of them.
+Nothing here retypes the oracle's formulas: expected values come from hand derivations
+(tests/golden/), exact integer/rational geometry, numpy float64 linear algebra, or ray casting.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2306_07552_b200 import gen
+
+BG = 0xFFFFFFFF
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _pose(name):
+    C = np.eye(4, dtype=np.float32)
+    if name == "T":
+        C[:3, 3] = [1, 2, 3]
+    elif name == "Y90":
+        C[:3, :3] = np.array([[0, 0, 1], [0, 1, 0], [-1, 0, 0]], np.float32)
+    return C
+
+
+# --------------------------------------------------------------------------------------------
+# N1-N5 vertex stage
+# --------------------------------------------------------------------------------------------
+
+def test_vertex_closed_form(oracle_mod):
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "vertex_closed_form.txt")) if l.strip() and l[0] != "#"]
+    assert len(rows) >= 10
+    for pose, px, py, pz, X, Y, w in rows:
+        o = oracle_mod.vertex_stage(64, 64, 1.0, 1.0, 0.1, 20.0, _pose(pose), None,
+                                    np.array([[float(px), float(py), float(pz)]], np.float32))
+        assert o["inside"][0] == 1
+        assert (int(o["Xi"][0]), int(o["Yi"][0]), float(o["w"][0])) == (int(X), int(Y), float(w)), (pose, px, py, pz)
+
+
+def test_vertex_instance_closed_form(oracle_mod):
+    # object-to-world = uniform scale 2 then translate (0,0,-6): object point (0.5,0.5,1) -> world (1,1,-4)
+    M = np.eye(4, dtype=np.float32)
+    M[:3, :3] *= 2
+    M[:3, 3] = [0, 0, -6]
+    o = oracle_mod.vertex_stage(64, 64, 1.0, 1.0, 0.1, 20.0, _pose("I"), M, np.array([[0.5, 0.5, 1.0]], np.float32))
+    assert (int(o["Xi"][0]), int(o["Yi"][0]), float(o["w"][0])) == (8192 + 2048, 8192 - 2048, 4.0)
+    # non-symmetric object matrix: a transposed operand would map x->z: M = rot +90 about Y then translate
+    M = np.array([[0, 0, 1, 0], [0, 1, 0, 0], [-1, 0, 0, -4], [0, 0, 0, 1]], np.float32)
+    # object (1,0,2) -> world (2,0,-1-4) = (2,0,-5)?  row2: -1*1 + 0 + 0*2 - 4 = -5 ; row0: 2
+    o = oracle_mod.vertex_stage(64, 64, 1.0, 1.0, 0.1, 20.0, _pose("T"), M, np.array([[1.0, 0.0, 2.0]], np.float32))
+    # camera at (1,2,3): rel = (1,-2,-8): X = (1/8)*8192+8192 = 9216, Y = (2/8)*8192+8192 = 10240, w = 8
+    assert (int(o["Xi"][0]), int(o["Yi"][0]), float(o["w"][0])) == (9216, 10240, 8.0)
+
+
+def test_vertex_vs_float64(oracle_mod):
+    rng = np.random.default_rng(7)
+    W, H, fx, fy = 128, 64, 0.5, 1.0   # non-square on purpose: swapping W/H or fx/fy must fail
+    for trial in range(20):
+        wl_pose = gen._cam_pose(rng.uniform(-3, 3, (1, 3)), rng.uniform(0, 6.28, 1), rng.uniform(-1, 1, 1))[0]
+        A = rng.normal(size=(3, 3))
+        M = np.eye(4)
+        M[:3, :3] = A
+        M[:3, 3] = rng.uniform(-2, 2, 3)
+        pos = rng.uniform(-6, 6, (400, 3)).astype(np.float32)
+        o = oracle_mod.vertex_stage(W, H, fx, fy, 0.1, 50.0, wl_pose.astype(np.float32), M.astype(np.float32), pos)
+        C64 = wl_pose.astype(np.float32).astype(np.float64)
+        M64 = M.astype(np.float32).astype(np.float64)
+        pc = (np.linalg.inv(C64) @ M64 @ np.concatenate([pos.astype(np.float64), np.ones((400, 1))], 1).T).T
+        w = -pc[:, 2]
+        sel = (w > 0.5) & (np.abs(pc[:, 0] / w) < 4) & (np.abs(pc[:, 1] / w) < 4)
+        if sel.sum() < 20:
+            continue   # geometry seen edge-on in this trial
+        assert np.all(o["inside"][sel] == 1) and np.all(o["inside"][w < 0.0999] == 0)
+        Xpix = (fx * pc[:, 0] / w * 0.5 + 0.5) * W       # pixel units, x right
+        Ypix = (0.5 - 0.5 * fy * pc[:, 1] / w) * H       # row 0 at the top
+        assert np.max(np.abs(o["Xi"][sel] - 256 * Xpix[sel])) <= 0.51
+        assert np.max(np.abs(o["Yi"][sel] - 256 * Ypix[sel])) <= 0.51
+        assert np.allclose(o["w"][sel], w[sel], rtol=1e-5)
+        assert np.allclose(o["q"][sel], 1 / w[sel], rtol=1e-5)
+
+
+# --------------------------------------------------------------------------------------------
+# helpers: camera-space soups whose snapped coordinates are known by construction
+# --------------------------------------------------------------------------------------------
+
+def _soup_from_snapped(XY, W, H, w=2.0, colors=None):
+    """Triangles given by snapped integer corners XY [nt,3,2] (1/256 px) at constant view depth w (a
+    power of two): xc = (X - hw) * w / hw is exact in binary32, so N5 reproduces X exactly."""
+    XY = np.asarray(XY, np.float64)
+    nt = XY.shape[0]
+    hw, hh = 128.0 * W, 128.0 * H
+    v = np.zeros((nt, 3, 6), np.float32)
+    v[:, :, 0] = (XY[:, :, 0] - hw) * w / hw
+    v[:, :, 1] = -(XY[:, :, 1] - hh) * w / hh
+    v[:, :, 2] = w
+    v[:, :, 3:] = 200.0 if colors is None else colors
+    return v
+
+
+def _covered_exact(tri, px, py):
+    """Top-left rule from its geometric meaning, in exact integer arithmetic: the pixel centre displaced
+    infinitesimally to the right and (to second order) downwards, p + (eps, eps^2), is strictly inside
+    the triangle.  Orientation-free: all three edge functions must have the sign of the area."""
+    (x0, y0), (x1, y1), (x2, y2) = [(int(a), int(b)) for a, b in tri]
+    area = (x1 - x0) * (y2 - y0) - (y1 - y0) * (x2 - x0)
+    if area == 0:
+        return False
+    s = 1 if area > 0 else -1
+    S = 1 << 80  # eps = 2^-80: |perturbation| < 2^-40 << 1 = smallest non-zero |integer edge value|
+    for (ax, ay), (bx, by) in (((x0, y0), (x1, y1)), ((x1, y1), (x2, y2)), ((x2, y2), (x0, y0))):
+        # edge function scaled by S^2 at (px + 1/S, py + 1/S^2)
+        e = ((bx - ax) * ((py - ay) * S * S + 1) - (by - ay) * ((px - ax) * S * S + S))
+        if e * s <= 0:
+            return False
+    return True
+
+
+# --------------------------------------------------------------------------------------------
+# N6 coverage
+# --------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("diag", [0, 1])
+@pytest.mark.parametrize("flip", [0, 1])
+def test_quad_closed_form(oracle_mod, diag, flip):
+    W = H = 16
+    offs = [0, 1, 127, 128, 129, 255]
+    for ox0 in offs:
+        for ox1 in offs:
+            for oy0, oy1 in ((0, 128), (129, 255), (128, 127), (1, 129)):
+                Xlo, Xhi = 256 * 3 + ox0, 256 * 9 + ox1
+                Ylo, Yhi = 256 * 2 + oy0, 256 * 12 + oy1
+                a, b, c, d = (Xlo, Ylo), (Xhi, Ylo), (Xhi, Yhi), (Xlo, Yhi)
+                tris = [[a, b, c], [a, c, d]] if diag == 0 else [[a, b, d], [b, c, d]]
+                if flip:
+                    tris = [[t[0], t[2], t[1]] for t in tris]
+                o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, _soup_from_snapped(tris, W, H), [0, 1],
+                                           want_count=True)
+                cx = 256 * np.arange(W) + 128
+                cy = 256 * np.arange(H) + 128
+                exp = ((cy[:, None] >= Ylo) & (cy[:, None] < Yhi)) & ((cx[None, :] >= Xlo) & (cx[None, :] < Xhi))
+                assert np.array_equal(o["count"], exp.astype(np.uint32)), (ox0, ox1, oy0, oy1)
+                assert np.array_equal(o["id"] != BG, exp)
+                assert np.all(o["depth"][exp] == 2.0) and np.all(o["depth"][~exp] == 0.0)
+
+
+def test_bruteforce_exact_integers(oracle_mod):
+    """Coverage count and winning id against exact big-integer evaluation; vertices on a 64-unit lattice
+    so that edges and vertices pass through pixel centres all the time; all triangles at the same depth,
+    so by N9 the winner is the lowest id among the covering triangles."""
+    rng = np.random.default_rng(11)
+    W, H = 12, 10
+    for trial in range(12):
+        nt = 12
+        XY = rng.integers(-8, 60, (nt, 3, 2)) * 64
+        XY[:, :, 1] = np.minimum(XY[:, :, 1], 48 * 64)
+        if trial % 3 == 0:  # axis-aligned and degenerate cases
+            XY[::4, 1, 1] = XY[::4, 0, 1]
+            XY[1::8, 2] = XY[1::8, 1]
+        ids = rng.permutation(nt).astype(np.uint32) + 5
+        o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, _soup_from_snapped(XY, W, H), ids, want_count=True)
+        cnt = np.zeros((H, W), np.uint32)
+        win = np.full((H, W), BG, np.uint32)
+        for j in range(H):
+            for i in range(W):
+                for t in range(nt):
+                    if _covered_exact(XY[t], 256 * i + 128, 256 * j + 128):
+                        cnt[j, i] += 1
+                        win[j, i] = min(win[j, i], ids[t])
+        assert cnt.max() >= 3 and (cnt == 0).any()
+        assert np.array_equal(o["count"], cnt)
+        assert np.array_equal(o["id"], win)
+
+
+def test_watertight_grid_exactly_once(oracle_mod):
+    """A triangulated surface with shared vertices, random diagonals and random windings, in perspective
+    (varying depth), larger than the screen: every pixel is covered by exactly one triangle."""
+    rng = np.random.default_rng(3)
+    W, H = 48, 40
+    n = 30
+    gx, gy = np.meshgrid(np.linspace(-1.6, 1.6, n + 1), np.linspace(-1.6, 1.6, n + 1), indexing="ij")
+    for trial in range(4):
+        jx = gx + rng.uniform(-0.02, 0.02, gx.shape)
+        jy = gy + rng.uniform(-0.02, 0.02, gy.shape)
+        w = 1.0 + rng.uniform(0, 3.0) * (gx + 2) + rng.uniform(-0.2, 0.2, gx.shape)   # tilted, bumpy
+        P = np.stack([jx * w, jy * w, w], -1)    # camera space (x = ndc*w for fx=1)
+        tris = []
+        for i in range(n):
+            for j in range(n):
+                a, b, c, d = P[i, j], P[i + 1, j], P[i + 1, j + 1], P[i, j + 1]
+                pair = ([a, b, c], [a, c, d]) if rng.random() < 0.5 else ([a, b, d], [b, c, d])
+                for t in pair:
+                    if rng.random() < 0.5:
+                        t = [t[0], t[2], t[1]]
+                    k = rng.integers(0, 3)
+                    tris.append(t[k:] + t[:k])
+        v = np.zeros((len(tris), 3, 6), np.float32)
+        v[:, :, :3] = np.array(tris)
+        v[:, :, 3:] = 100
+        o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 100.0, v, np.arange(len(tris)), want_count=True)
+        assert np.all(o["count"] == 1)
+
+
+def test_rotation_and_winding_leave_coverage_unchanged(oracle_mod):
+    rng = np.random.default_rng(5)
+    W = H = 24
+    XY = rng.integers(-2 * 256, 26 * 256, (60, 3, 2))
+    base = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, _soup_from_snapped(XY, W, H), np.arange(60), want_count=True)
+    for perm in ([1, 2, 0], [2, 0, 1], [0, 2, 1], [2, 1, 0]):
+        o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, _soup_from_snapped(XY[:, perm], W, H), np.arange(60),
+                                   want_count=True)
+        # (the winning id may change: with areas > 2^24 the depth of a w=2 triangle rounds to 2 -/+ 1 ulp
+        # depending on the order of the three terms of N7, so only coverage is invariant)
+        assert np.array_equal(o["count"], base["count"])
+        assert np.array_equal(o["id"] != BG, base["id"] != BG)
+
+
+def test_full_scan_equals_bbox(oracle_mod):
+    wl = gen.make_config(0)
+    a = oracle_mod.render(wl, want_count=True)
+    b = oracle_mod.render(wl, want_count=True, full_scan=True)
+    for k in ("rgb", "depth", "id", "count"):
+        assert np.array_equal(a[k], b[k]), k
+
+
+# --------------------------------------------------------------------------------------------
+# ray casting in float64 (independent of snapping, edge functions and the clip)
+# --------------------------------------------------------------------------------------------
+
+def _raycast(tri_cam, col, W, H, fx, fy, znear, zfar):
+    """Nearest hit per pixel-centre ray, Moeller-Trumbore in float64, camera space, unsnapped geometry.
+    tri_cam [nt,3,3] (x, y, z) with the camera looking along -z.  Returns id [-1 none], depth w, rgb."""
+    j, i = np.meshgrid(np.arange(H), np.arange(W), indexing="ij")
+    d = np.stack([((i + 0.5) / W * 2 - 1) / fx, (1 - (j + 0.5) / H * 2) / fy, -np.ones_like(i, float)], -1).reshape(-1, 3)
+    best = np.full(d.shape[0], np.inf)
+    bid = np.full(d.shape[0], -1)
+    brgb = np.zeros((d.shape[0], 3))
+    second = np.full(d.shape[0], np.inf)
+    edge = np.zeros(d.shape[0], bool)
+    for t in range(tri_cam.shape[0]):
+        v0, v1, v2 = tri_cam[t]
+        e1, e2 = v1 - v0, v2 - v0
+        pv = np.cross(d, e2)
+        det = pv @ e1
+        ok = np.abs(det) > 1e-14
+        inv = np.where(ok, 1.0 / np.where(ok, det, 1), 0)
+        tv = -v0
+        u = (pv @ tv) * inv
+        qv = np.cross(tv, e1)
+        vv = (d @ qv) * inv
+        tt = (e2 @ qv) * inv        # ray parameter = w because d_z = -1
+        hit = ok & (u >= 0) & (vv >= 0) & (u + vv <= 1) & (tt >= znear) & (tt <= zfar)
+        near_edge = ok & (np.minimum(np.minimum(u, vv), 1 - u - vv) > -0.02) & (np.minimum(np.minimum(u, vv), 1 - u - vv) < 0.02)
+        edge |= near_edge
+        closer = hit & (tt < best)
+        second = np.where(closer, best, np.where(hit & (tt < second), tt, second))
+        best = np.where(closer, tt, best)
+        bid = np.where(closer, t, bid)
+        wgt = np.stack([1 - u - vv, u, vv], -1)
+        brgb = np.where(closer[:, None], wgt @ col[t].astype(float), brgb)
+    return (bid.reshape(H, W), best.reshape(H, W), brgb.reshape(H, W, 3), second.reshape(H, W), edge.reshape(H, W))
+
+
+def _rel_inv_w_gradient(tri_cam, rid, rw, W, H, fx, fy):
+    """|gradient of 1/w with respect to pixel coordinates| * w for the triangle hit at each pixel.
+    Plane n.P = d and ray P = w*(xn/fx, yn/fy, -1) give 1/w = n.dir/d, affine in the pixel position."""
+    v0, v1, v2 = tri_cam[:, 0], tri_cam[:, 1], tri_cam[:, 2]
+    nrm = np.cross(v1 - v0, v2 - v0)
+    d = np.einsum("ij,ij->i", nrm, v0)
+    with np.errstate(divide="ignore", invalid="ignore"):
+        gx = nrm[:, 0] * (2.0 / (W * fx)) / d
+        gy = -nrm[:, 1] * (2.0 / (H * fy)) / d
+    t = np.maximum(rid, 0)
+    return np.hypot(gx[t], gy[t]) * np.where(np.isfinite(rw), rw, 0.0)
+
+
+def _camera_space_triangles(wl, n):
+    """float64 camera-space corners and colours of every triangle of env n, in triangle-id order."""
+    C = wl.cam_pose[n].reshape(4, 4).astype(np.float64)
+    Vm = np.linalg.inv(C)
+    tris, cols = [], []
+    parts = [(wl.static_meshes[wl.env_scene[n]], np.eye(4))]
+    for k in range(wl.K):
+        if wl.inst_mesh[n, k] >= 0:
+            parts.append((wl.dyn_meshes[wl.inst_mesh[n, k]], wl.inst_xform[n, k].reshape(4, 4).astype(np.float64)))
+    for m, M in parts:
+        p = np.concatenate([m.positions.astype(np.float64), np.ones((m.nv, 1))], 1) @ (Vm @ M).T
+        tris.append(p[:, :3][m.indices.astype(np.int64)])
+        cols.append(m.colors[m.indices.astype(np.int64)])
+    return np.concatenate(tris), np.concatenate(cols)
+
+
+def test_whole_image_vs_raycast_config0(oracle_mod):
+    """End-to-end check of conventions (handedness, row order, FoV, near clip, id numbering, instance
+    transforms, perspective-correct depth and colour) on config 0."""
+    wl = gen.make_config(0)
+    o = oracle_mod.render(wl)
+    n_unclipped = n_clipped = 0
+    for n in range(wl.N):
+        tri, col = _camera_space_triangles(wl, n)
+        rid, rw, rrgb, second, edge = _raycast(tri, col, wl.width, wl.height, wl.fx, wl.fy, wl.znear, wl.zfar)
+        oid = o["id"][n].astype(np.int64)
+        oid[oid == BG] = -1
+        same = oid == rid
+        assert same.mean() >= 0.99, same.mean()
+        # every disagreement sits next to a projected edge (snapping moves edges by < 1/256 px) or at a
+        # near-tie of two surfaces
+        bad = ~same
+        assert np.all(edge[bad] | (np.abs(second[bad] - rw[bad]) < 1e-3 * rw[bad]))
+        hit = same & (rid >= 0)
+        rel = np.abs(o["depth"][n][hit] - rw[hit]) / rw[hit]
+        # Snapping moves each vertex by <= sqrt(2)/512 px.  Inside a triangle that is the same as
+        # evaluating the unsnapped affine function 1/w at a point moved by a convex combination of the
+        # three shifts, so |d(depth)/depth| <= |grad_px(1/w)| * w * sqrt(2)/512 (+ float32 rounding).
+        # A near-clipped triangle lies in the same plane with its new vertices on the old edges, so the
+        # same bound holds for it.
+        g = _rel_inv_w_gradient(tri, rid, rw, wl.width, wl.height, wl.fx, wl.fy)[hit]
+        unclipped = (-tri[:, :, 2]).min(axis=1)[rid[hit]] >= wl.znear
+        bound = g * (np.sqrt(2.0) / 512.0) * 1.02 + 2e-6
+        n_unclipped += int(unclipped.sum())
+        n_clipped += int((~unclipped).sum())
+        assert np.all(rel <= bound), float((rel / bound).max())
+        dc = np.abs(o["rgb"][n][hit].astype(float) - rrgb[hit])
+        assert np.quantile(dc, 0.99) <= 1.0 and dc.max() <= 6.0, (np.quantile(dc, 0.99), dc.max())
+        assert np.all(o["depth"][n][rid < 0][same[rid < 0]] == 0.0)
+    assert n_unclipped > 20 and n_clipped > 1000   # both kinds of triangle are exercised (config 0 is mostly clipped)
+
+
+# --------------------------------------------------------------------------------------------
+# N4 near clip
+# --------------------------------------------------------------------------------------------
+
+def _floor_soup(n_cells, rng=None):
+    """A horizontal floor 1.2 m below the camera from 2 m behind it to 6 m ahead, as an n x n grid."""
+    xs = np.linspace(-8, 8, n_cells + 1)   # wide enough to span the 90-degree FoV out to w = 6
+    zs = np.linspace(2, -6, n_cells + 1)   # camera space z; w = -z
+    tris = []
+    for i in range(n_cells):
+        for j in range(n_cells):
+            a = (xs[i], -1.2, zs[j]); b = (xs[i + 1], -1.2, zs[j]); c = (xs[i + 1], -1.2, zs[j + 1]); d = (xs[i], -1.2, zs[j + 1])
+            tris += [[a, b, c], [a, c, d]]
+    t = np.array(tris)
+    v = np.zeros((t.shape[0], 3, 6), np.float32)
+    v[:, :, 0] = t[:, :, 0]; v[:, :, 1] = t[:, :, 1]; v[:, :, 2] = -t[:, :, 2]
+    v[:, :, 3:] = 128
+    return v
+
+
+def test_near_clip_invariants(oracle_mod):
+    W = H = 64
+    znear = 0.5
+    coarse = oracle_mod.raster_soup(W, H, 1.0, 1.0, znear, 20.0, _floor_soup(1), np.arange(2), want_count=True)
+    fine = oracle_mod.raster_soup(W, H, 1.0, 1.0, znear, 20.0, _floor_soup(37), np.arange(2 * 37 * 37), want_count=True)
+    # the floor plane y=-1.2 seen by a level camera: pixel row j sees it at w = 1.2 / tan(angle below horizon)
+    yndc = 1 - (np.arange(H) + 0.5) / H * 2
+    with np.errstate(divide="ignore"):
+        w_row = np.where(yndc < 0, 1.2 / -yndc, np.inf)
+    vis = (w_row >= znear * 1.05) & (w_row <= 5.9)
+    gone = (w_row < znear * 0.95) | ~np.isfinite(w_row)
+    for o in (coarse, fine):
+        assert o["count"].max() == 1                      # clipped pieces never overlap or double-cover
+        assert np.all(o["count"][vis] == 1)               # exactly once where the plane is in front of the near plane
+        assert np.all(o["count"][gone] == 0)              # nothing from behind the near plane
+        d = o["depth"][o["id"] != BG]
+        assert d.min() >= znear * (1 - 1e-6)
+        rows = np.nonzero(vis)[0]
+        assert np.allclose(o["depth"][rows, :], w_row[rows, None], rtol=2e-3)
+    diff = np.nonzero((coarse["count"] != fine["count"]).any(1))[0]
+    assert np.all(np.abs(w_row[diff] - znear) < 0.1 * znear)   # tessellation only matters at the clip line
+
+
+def test_near_clip_keeps_shared_edges_watertight(oracle_mod):
+    rng = np.random.default_rng(9)
+    W = H = 48
+    znear = 0.4
+    n = 14
+    # bumpy tilted sheet that dives through the near plane; shared vertices; random rotation of corners
+    gx, gz = np.meshgrid(np.linspace(-3, 3, n + 1), np.linspace(1.0, -5.0, n + 1), indexing="ij")
+    # (height jitter kept below the grazing slope 0.6/5 so the sheet never folds over itself in the view)
+    y = -0.6 + 0.15 * gx + rng.uniform(-0.01, 0.01, gx.shape)
+    P = np.stack([gx + rng.uniform(-0.05, 0.05, gx.shape), y, gz + rng.uniform(-0.05, 0.05, gx.shape)], -1)
+    tris = []
+    for i in range(n):
+        for j in range(n):
+            a, b, c, d = P[i, j], P[i + 1, j], P[i + 1, j + 1], P[i, j + 1]
+            for t in (([a, b, c], [a, c, d]) if rng.random() < 0.5 else ([a, b, d], [b, c, d])):
+                k = rng.integers(0, 3)
+                t = t[k:] + t[:k]
+                tris.append(t if rng.random() < 0.5 else [t[0], t[2], t[1]])
+    t = np.array(tris)
+    v = np.zeros((t.shape[0], 3, 6), np.float32)
+    v[:, :, 0] = t[:, :, 0]; v[:, :, 1] = t[:, :, 1]; v[:, :, 2] = -t[:, :, 2]
+    v[:, :, 3:] = 50
+    o = oracle_mod.raster_soup(W, H, 1.0, 1.0, znear, 50.0, v, np.arange(t.shape[0]), want_count=True)
+    assert o["count"].max() == 1
+    rid, rw, _, _, edge = _raycast(t, np.zeros((t.shape[0], 3, 3)), W, H, 1.0, 1.0, znear, 50.0)
+    far_from_border = np.zeros_like(edge)
+    # interior of the sheet well in front of the near plane must be covered exactly once
+    inside = (rid >= 0) & (rw > znear * 1.1)
+    # ignore the outer silhouette of the sheet: erode by one pixel
+    er = inside.copy()
+    er[1:, :] &= inside[:-1, :]; er[:-1, :] &= inside[1:, :]; er[:, 1:] &= inside[:, :-1]; er[:, :-1] &= inside[:, 1:]
+    assert er.sum() > 200
+    assert np.all(o["count"][er] == 1)
+    assert np.all(o["count"][(rid < 0) & ~_dilate(rid >= 0)] == 0)
+
+
+def _dilate(m):
+    d = m.copy()
+    d[1:, :] |= m[:-1, :]; d[:-1, :] |= m[1:, :]; d[:, 1:] |= m[:, :-1]; d[:, :-1] |= m[:, 1:]
+    return d
+
+
+# --------------------------------------------------------------------------------------------
+# N7 depth, N8 colour, far plane
+# --------------------------------------------------------------------------------------------
+
+def test_depth_exact_for_power_of_two(oracle_mod):
+    W = H = 32
+    for w in (0.5, 1.0, 4.0, 16.0):
+        XY = [[(256 * 4 + 3, 256 * 5 + 77), (256 * 19 + 200, 256 * 6 + 1), (256 * 9 + 128, 256 * 20 + 130)]]
+        o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, _soup_from_snapped(XY, W, H, w=w), [0])
+        cov = o["id"] == 0
+        assert cov.sum() > 50
+        assert np.all(o["depth"][cov] == np.float32(w))
+
+
+def test_depth_and_far_plane_tilted(oracle_mod):
+    # one big triangle receding from w=1 (bottom) to w=40 (top); zfar=10 cuts it
+    W = H = 64
+    v = np.zeros((1, 3, 6), np.float32)
+    v[0, 0, :3] = (-3 * 1, -0.9 * 1, 1)
+    v[0, 1, :3] = (3 * 1, -0.9 * 1, 1)
+    v[0, 2, :3] = (0.0, 0.9 * 40, 40)
+    v[0, :, 3:] = 255
+    o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 10.0, v, [7])
+    tri = np.array([[[-3, -0.9, -1], [3, -0.9, -1], [0, 36.0, -40]]], float)
+    rid, rw, _, _, edge = _raycast(tri, np.zeros((1, 3, 3)), W, H, 1.0, 1.0, 0.1, 1e9)
+    hit = (o["id"] == 7)
+    assert hit.sum() > 100
+    assert np.all(o["depth"][hit] <= 10.0)
+    inner = (rid == 0) & ~edge
+    assert np.all(hit[inner & (rw < 9.99)]) and not np.any(hit[inner & (rw > 10.01)])
+    # snapping bound on the relative depth error (see test_whole_image_vs_raycast_config0)
+    sel = hit & inner
+    g = _rel_inv_w_gradient(tri, rid, rw, W, H, 1.0, 1.0)[sel]
+    rel = np.abs(o["depth"][sel] - rw[sel]) / rw[sel]
+    assert np.all(rel <= g * (np.sqrt(2.0) / 512.0) * 1.02 + 2e-6), float(rel.max())
+
+
+def test_colour_constant_and_affine(oracle_mod):
+    W = H = 32
+    XY = np.array([[(256 * 2, 256 * 2), (256 * 30, 256 * 3), (256 * 10, 256 * 29)]])
+    col = np.zeros((1, 3, 3), np.float32)
+    col[0, :, :] = (13, 250, 97)
+    o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, _soup_from_snapped(XY, W, H, colors=col), [0])
+    cov = o["id"] == 0
+    assert np.all(o["rgb"][cov] == np.array([13, 250, 97], np.uint8))
+    assert np.all(o["rgb"][~cov] == 0)
+    # fronto-parallel -> perspective-correct interpolation reduces to affine barycentric interpolation
+    col[0] = [[255, 0, 10], [0, 255, 20], [0, 0, 250]]
+    o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, _soup_from_snapped(XY, W, H, w=4.0, colors=col), [0])
+    T = np.array([[XY[0, 0, 0], XY[0, 1, 0], XY[0, 2, 0]], [XY[0, 0, 1], XY[0, 1, 1], XY[0, 2, 1]], [1, 1, 1]], float)
+    for j in range(H):
+        for i in range(W):
+            if cov[j, i]:
+                lam = np.linalg.solve(T, np.array([256 * i + 128, 256 * j + 128, 1.0]))
+                exp = lam @ col[0].astype(float)
+                assert np.all(np.abs(o["rgb"][j, i].astype(float) - exp) <= 0.5 + 1e-3), (i, j)
+
+
+def test_colour_perspective_correct(oracle_mod):
+    # receding triangle with a colour ramp along depth: screen-space-linear interpolation would be far off
+    W = H = 64
+    tri = np.array([[[-2, -1, -1], [2, -1, -1], [0, 8.0, -16]]], float)
+    col = np.array([[[255, 0, 0], [255, 0, 0], [0, 255, 0]]], float)
+    v = np.zeros((1, 3, 6), np.float32)
+    v[0, :, 0] = tri[0, :, 0]; v[0, :, 1] = tri[0, :, 1]; v[0, :, 2] = -tri[0, :, 2]; v[0, :, 3:] = col[0]
+    o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 100.0, v, [0])
+    rid, rw, rrgb, _, edge = _raycast(tri, col, W, H, 1.0, 1.0, 0.1, 100.0)
+    sel = (o["id"] == 0) & (rid == 0) & ~edge
+    assert sel.sum() > 300
+    assert np.max(np.abs(o["rgb"][sel].astype(float) - rrgb[sel])) <= 1.0
+    assert np.ptp(o["rgb"][sel][:, 1].astype(int)) > 100   # the ramp is actually exercised
+
+
+# --------------------------------------------------------------------------------------------
+# N9 resolve
+# --------------------------------------------------------------------------------------------
+
+def test_processing_order_does_not_matter(oracle_mod):
+    wl = gen.make_config(0)
+    tri, col = _camera_space_triangles(wl, 1)
+    v = np.zeros((tri.shape[0], 3, 6), np.float32)
+    v[:, :, 0] = tri[:, :, 0]; v[:, :, 1] = tri[:, :, 1]; v[:, :, 2] = -tri[:, :, 2]; v[:, :, 3:] = col
+    # add exact duplicates so that exact depth ties exist
+    v = np.concatenate([v, v[:40]])
+    ids = np.arange(v.shape[0], dtype=np.uint32)
+    base = oracle_mod.raster_soup(64, 64, 1.0, 1.0, 0.1, 20.0, v, ids)
+    rng = np.random.default_rng(1)
+    for _ in range(3):
+        p = rng.permutation(v.shape[0])
+        o = oracle_mod.raster_soup(64, 64, 1.0, 1.0, 0.1, 20.0, v[p], ids[p])
+        for k in ("rgb", "depth", "id", "sub"):
+            assert np.array_equal(o[k], base[k]), k
+    assert not np.any((base["id"] >= tri.shape[0]) & (base["id"] != BG))   # of two coincident triangles the lower id wins
+    # permuting the ids changes only pixels with an exact depth tie (here: the duplicated triangles)
+    ids2 = ids.copy()
+    ids2[:40], ids2[tri.shape[0]:] = ids[tri.shape[0]:], ids[:40]
+    o = oracle_mod.raster_soup(64, 64, 1.0, 1.0, 0.1, 20.0, v, ids2)
+    assert np.array_equal(o["depth"], base["depth"]) and np.array_equal(o["rgb"], base["rgb"])
+    assert np.array_equal(o["id"], base["id"])   # winner is still the lower of the two ids {i, i+nt}
+
+
+def test_coincident_triangles_lowest_id(oracle_mod):
+    XY = np.array([[(100, 100), (7000, 300), (2000, 6000)]] * 3)
+    for ids in ([5, 3, 9], [9, 5, 3], [3, 9, 5]):
+        o = oracle_mod.raster_soup(32, 32, 1.0, 1.0, 0.1, 20.0, _soup_from_snapped(XY, 32, 32), ids)
+        assert set(np.unique(o["id"])) == {3, BG}
+
+
+# --------------------------------------------------------------------------------------------
+# batch entry point: ids, instance slots, env independence
+# --------------------------------------------------------------------------------------------
+
+def test_render_ids_and_empty_slots(oracle_mod):
+    wl = gen.make_config(0)
+    full = oracle_mod.render(wl)
+    ns = wl.static_meshes[0].nt
+    assert full["id"][full["id"] != BG].max() < ns + 24
+    assert (full["id"][full["id"] != BG] >= ns).any()      # cubes are visible somewhere
+    # emptying slot 0 renumbers slot 1's triangles down by 12 and removes slot 0's fragments
+    wl2 = wl.subset(np.arange(wl.N))
+    wl2.inst_mesh = wl.inst_mesh.copy()
+    wl2.inst_mesh[:, 0] = -1
+    o2 = oracle_mod.render(wl2)
+    was1 = (full["id"] >= ns + 12) & (full["id"] != BG)
+    assert np.array_equal(o2["id"][was1], full["id"][was1] - 12)
+    assert not np.any((o2["id"] >= ns + 12) & (o2["id"] != BG))
+    # environments are independent: a subset renders to the same rows
+    sub = oracle_mod.render(wl.subset([2, 0]))
+    for k in ("rgb", "depth", "id"):
+        assert np.array_equal(sub[k][0], full[k][2]) and np.array_equal(sub[k][1], full[k][0])
+    # threads do not change anything
+    one = oracle_mod.render(wl, n_threads=1)
+    for k in ("rgb", "depth", "id"):
+        assert np.array_equal(one[k], full[k])
+
+
+def test_generators_are_subset_reproducible():
+    a = gen.make_config(1, n_envs=6)
+    b = gen.make_config(1, env_ids=[4, 1])
+    assert np.array_equal(b.cam_pose, a.cam_pose[[4, 1]]) and np.array_equal(b.inst_xform, a.inst_xform[[4, 1]])
+    assert a.static_meshes[0].nt == 50_000 and [m.nt for m in a.dyn_meshes] == [980, 400, 400, 400, 400, 400]
+    assert a.K == 25 and np.all(a.tris_per_env() == 71_600)
