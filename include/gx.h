@@ -1,0 +1,133 @@
+/*
+ * gx.h -- C ABI of the B200-native batch RGBD rasteriser.
+ *
+ * The operation is the rendering hot path of Galactic's simulation step: "A single ... renderer instance
+ * renders all environments, sharing GPU memory assets across environments. Scene graph updates are
+ * communicated from our physics simulation to the ... renderer ... The renderer outputs a single batch
+ * observation per camera sensor, essentially a stack of images from each environment in GPU memory. This is
+ * directly consumed by PyTorch GPU-based batch DNN inference, without ever copying pixels to the CPU."
+ * (section 3.1).  Sensor: 128x128 RGBD, 90-degree FoV head camera (section 4.1).
+ * The paper is silent on the per-pixel arithmetic; it is fixed by DESIGN.md section 3 (readings N0-N10).
+ *
+ * Conventions (N0): right-handed world, +Y up; the camera looks along its local -Z with +X right
+ * and +Y up; all 4x4 matrices are row-major with points as columns; image row 0 is the top row; pixel
+ * (col i, row j) has its centre at (i + 0.5, j + 0.5).
+ *
+ * Threading: one call in flight per handle; distinct handles are independent.  No exception crosses this
+ * boundary; every entry point returns 0 or a negative GX_ERR_* code and gx_last_error() holds a
+ * thread-local message for the last failure.
+ */
+#ifndef GX_H_
+#define GX_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GX_OK 0
+#define GX_ERR_INVALID_ARG (-1) /* null pointer, bad size, bad camera */
+#define GX_ERR_CUDA (-2)        /* a CUDA runtime call failed; message has the CUDA error string */
+#define GX_ERR_OOM (-3)         /* host or device allocation failed */
+#define GX_ERR_UNSUPPORTED (-4) /* valid request outside what this build supports (see gx_render_batch) */
+
+#define GX_BACKGROUND_ID 0xFFFFFFFFu
+#define GX_MAX_INSTANCES 254 /* K, instance slots per environment */
+
+typedef struct GxScene GxScene; /* opaque; owns the device copies of all meshes and all scratch memory */
+
+/* One indexed triangle mesh in HOST memory.  Read only during gx_create_scene. */
+typedef struct {
+    const float *positions;  /* [nv*3] float32, object space (static meshes: world space), metres */
+    const uint8_t *colors;   /* [nv*3] uint8 RGB per vertex */
+    const uint32_t *indices; /* [nt*3] uint32 vertex indices, each < nv */
+    uint32_t nv, nt;
+} GxMesh;
+
+/* Pinhole camera shared by all environments of a call. */
+typedef struct {
+    int32_t width, height; /* pixels; multiples of 16; width*height <= 16384 in this build */
+    float fx, fy;          /* NDC focal lengths: fy = 1/tan(fovy/2), fx = fy*height/width; 90 deg square: 1 */
+    float znear, zfar;     /* metres, 0 < znear < zfar; fragments with view depth > zfar are dropped */
+} GxCamera;
+
+/*
+ * gx_create_scene -- upload the shared assets once ("sharing GPU memory assets across
+ * environments").  static_meshes[s] is the static indoor mesh of scene s (world space); dyn_meshes[m] are
+ * the movable-object and robot-link meshes placed per environment by instance transforms.  Every mesh is
+ * split into clusters of 256 consecutive triangles, each with its own AABB (frustum-culled per
+ * environment); triangle order, and therefore triangle ids, are preserved.
+ *   All mesh arrays are HOST pointers and are copied: the caller may free them on return.
+ *   cuda_device: ordinal of the device that will own the scene.  *out receives the handle.
+ * Errors: INVALID_ARG (null pointers, n_static <= 0, n_dyn < 0, an index >= nv, empty mesh with non-null
+ * arrays is allowed), OOM, CUDA.
+ */
+int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh *dyn_meshes, int32_t n_dyn,
+                    int32_t cuda_device, GxScene **out);
+
+/*
+ * gx_render_batch -- rasterise RGBD (and optionally triangle ids) for N independent environments.
+ * Per pixel: among all post-clip, post-snap triangles of the environment whose integer edge functions
+ * cover the pixel centre under the top-left rule and whose depth is <= zfar, the one with the smallest
+ * (depth, triangle id, clip sub-index); DESIGN.md section 3 gives every arithmetic step.
+ *
+ * All array arguments are DEVICE pointers on the scene's device, caller-owned, 16-byte aligned:
+ *   env_scene  [N]       int32   static mesh of each environment, in [0, n_static)
+ *   cam_pose   [N,16]    float32 camera-to-world, row-major, rigid
+ *   inst_mesh  [N,K]     int32   dynamic mesh id in [0, n_dyn), or -1 for an empty slot (may be NULL if K == 0)
+ *   inst_xform [N,K,16]  float32 object-to-world, row-major, affine (bottom row ignored)
+ *   rgb_out    [N,H,W,3] uint8   may be NULL (depth-only); background (0,0,0)
+ *   depth_out  [N,H,W]   float32 planar view-space depth in metres; background 0.0f
+ *   id_out     [N,H,W]   uint32  may be NULL; winning triangle id, background GX_BACKGROUND_ID.
+ *                                id = j for static triangle j; T_static + sum of nt over earlier non-empty
+ *                                slots + j for triangle j of instance slot k.
+ *   cuda_stream: a cudaStream_t (NULL = legacy default stream).
+ * The call only enqueues work on the stream and returns; outputs are valid in stream order (the zero-copy
+ * hand-off of PAPER.md:91).  Scratch inside the handle grows on demand; growing may synchronise the device,
+ * steady state does not.  Same inputs give bit-identical outputs, independent of how N is sharded.
+ * NaN/Inf inputs and out-of-range env_scene/inst_mesh values are precondition violations: the image is
+ * undefined, but no out-of-bounds write occurs for in-range ids.
+ * Errors: INVALID_ARG (null handle/camera/required pointer, N <= 0, K < 0, K > GX_MAX_INSTANCES, width or
+ * height not a positive multiple of 16, znear <= 0, zfar <= znear), UNSUPPORTED (width*height > 16384),
+ * OOM, CUDA.
+ */
+int gx_render_batch(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K, const int32_t *env_scene,
+                    const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,
+                    float *depth_out, uint32_t *id_out, void *cuda_stream);
+
+/*
+ * gx_render_batch_host -- the same operation with every array argument in HOST memory (pageable or
+ * pinned): copies the inputs to the device, renders, copies the outputs back and synchronises the stream
+ * before returning.  This is the end-to-end entry point bench.py times for its "e2e" figure.
+ */
+int gx_render_batch_host(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K, const int32_t *env_scene,
+                         const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform,
+                         uint8_t *rgb_out, float *depth_out, uint32_t *id_out);
+
+/*
+ * gx_set_option -- tuning / verification switches of a handle.  Unknown names return INVALID_ARG.
+ *   "cull"  0|1  (default 1): per-environment frustum culling of clusters (K1).  Culling is
+ *                conservative: the images with 0 and 1 are bit-identical (tested).
+ */
+int gx_set_option(GxScene *scene, const char *name, int64_t value);
+
+/*
+ * gx_get_stat -- counters of the most recent gx_render_batch on this handle; synchronises the stream the
+ * call ran on.  Names: "clusters_tested", "clusters_drawn", "triangles_in" (triangles of drawn clusters),
+ * "triangles_raster" (survived clip, zero-area and pixel-centre bounding-box rejection), "fragments"
+ * (pixel-centre hits before the depth test), "launches" (kernels launched by the call).
+ * Unknown names return INVALID_ARG; *out receives the value.
+ */
+int gx_get_stat(GxScene *scene, const char *name, int64_t *out);
+
+/* gx_destroy -- free the handle and everything it owns.  NULL is allowed. */
+void gx_destroy(GxScene *scene);
+
+/* gx_last_error -- thread-local, NUL-terminated message for the last non-zero return on this thread. */
+const char *gx_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GX_H_ */

@@ -1,0 +1,147 @@
+"""Thin ctypes binding over libgx.so (include/gx.h): same names, argument marshalling only.
+
+Every step of the render path runs in the CUDA kernels of csrc/; there is no CPU fallback.  If the
+library is missing, import of this module's functions raises.  PyTorch is used by callers for device
+memory and streams only; this module accepts anything with `.data_ptr()` (torch tensors), raw integer
+addresses, or numpy arrays (host entry point only).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgx.so")
+
+GX_OK, GX_ERR_INVALID_ARG, GX_ERR_CUDA, GX_ERR_OOM, GX_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
+GX_BACKGROUND_ID = 0xFFFFFFFF
+EXPORTS = ("gx_create_scene", "gx_render_batch", "gx_render_batch_host", "gx_set_option", "gx_get_stat",
+           "gx_destroy", "gx_last_error")
+
+
+class GxMesh(C.Structure):
+    _fields_ = [("positions", C.c_void_p), ("colors", C.c_void_p), ("indices", C.c_void_p),
+                ("nv", C.c_uint32), ("nt", C.c_uint32)]
+
+
+class GxCamera(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float),
+                ("znear", C.c_float), ("zfar", C.c_float)]
+
+
+class GxError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"gx error {code}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libgx.so.  Fails loudly if it has not been built (python -m paper_2306_07552_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not built; run `python -m paper_2306_07552_b200.build` "
+                                    "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.gx_last_error.restype = C.c_char_p
+        L.gx_destroy.restype = None
+        for n in EXPORTS[:5]:
+            getattr(L, n).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise GxError(rc, lib().gx_last_error().decode("utf-8", "replace"))
+
+
+def _dev(a) -> Optional[C.c_void_p]:
+    if a is None:
+        return None
+    if isinstance(a, int):
+        return C.c_void_p(a)
+    if hasattr(a, "data_ptr"):
+        if not a.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return C.c_void_p(a.data_ptr())
+    raise TypeError(f"expected a device tensor or address, got {type(a)}")
+
+
+def _host(a, dtype) -> Optional[C.c_void_p]:
+    if a is None:
+        return None
+    if hasattr(a, "data_ptr"):   # CPU torch tensor (e.g. pinned)
+        return C.c_void_p(a.data_ptr())
+    assert isinstance(a, np.ndarray) and a.dtype == dtype and a.flags.c_contiguous, (type(a), dtype)
+    return C.c_void_p(a.ctypes.data)
+
+
+def _mesh_array(meshes: Sequence):
+    keep = []
+    arr = (GxMesh * max(1, len(meshes)))()
+    for i, m in enumerate(meshes):
+        pos = np.ascontiguousarray(m.positions, np.float32)
+        col = np.ascontiguousarray(m.colors, np.uint8)
+        idx = np.ascontiguousarray(m.indices, np.uint32)
+        keep += [pos, col, idx]
+        arr[i] = GxMesh(pos.ctypes.data, col.ctypes.data, idx.ctypes.data, pos.shape[0], idx.shape[0])
+    return arr, keep
+
+
+def gx_create_scene(static_meshes: Sequence, dyn_meshes: Sequence, cuda_device: int = 0) -> C.c_void_p:
+    """Meshes: objects with .positions [nv,3] f32, .colors [nv,3] u8, .indices [nt,3] u32 (host)."""
+    sm, k1 = _mesh_array(static_meshes)
+    dm, k2 = _mesh_array(dyn_meshes)
+    h = C.c_void_p()
+    _check(lib().gx_create_scene(sm, C.c_int32(len(static_meshes)), dm, C.c_int32(len(dyn_meshes)),
+                                 C.c_int32(cuda_device), C.byref(h)))
+    return h
+
+
+def gx_render_batch(scene, camera: GxCamera, N: int, K: int, env_scene, cam_pose, inst_mesh, inst_xform,
+                    rgb_out, depth_out, id_out=None, cuda_stream: int = 0) -> None:
+    """All arrays are device tensors / addresses; enqueues on cuda_stream and returns."""
+    _check(lib().gx_render_batch(scene, C.byref(camera), C.c_int32(N), C.c_int32(K), _dev(env_scene), _dev(cam_pose),
+                                 _dev(inst_mesh), _dev(inst_xform), _dev(rgb_out), _dev(depth_out), _dev(id_out),
+                                 C.c_void_p(cuda_stream)))
+
+
+def gx_render_batch_host(scene, camera: GxCamera, N: int, K: int, env_scene, cam_pose, inst_mesh, inst_xform,
+                         rgb_out, depth_out, id_out=None) -> None:
+    """All arrays are host numpy arrays (or CPU/pinned torch tensors); synchronous."""
+    _check(lib().gx_render_batch_host(scene, C.byref(camera), C.c_int32(N), C.c_int32(K),
+                                      _host(env_scene, np.int32), _host(cam_pose, np.float32),
+                                      _host(inst_mesh, np.int32), _host(inst_xform, np.float32),
+                                      _host(rgb_out, np.uint8), _host(depth_out, np.float32),
+                                      _host(id_out, np.uint32)))
+
+
+def gx_set_option(scene, name: str, value: int) -> None:
+    _check(lib().gx_set_option(scene, name.encode(), C.c_int64(value)))
+
+
+def gx_get_stat(scene, name: str) -> int:
+    v = C.c_int64()
+    _check(lib().gx_get_stat(scene, name.encode(), C.byref(v)))
+    return int(v.value)
+
+
+def gx_destroy(scene) -> None:
+    if scene:
+        lib().gx_destroy(scene)
+
+
+def gx_last_error() -> str:
+    return lib().gx_last_error().decode("utf-8", "replace")
+
+
+def camera_of(wl) -> GxCamera:
+    """GxCamera from a gen.Workload (or anything with width/height/fx/fy/znear/zfar)."""
+    return GxCamera(int(wl.width), int(wl.height), float(wl.fx), float(wl.fy), float(wl.znear), float(wl.zfar))

@@ -1,0 +1,388 @@
+// gx_api.cu -- host side of the C ABI declared in include/gx.h: scene upload (clustering), launch, errors.
+// Product code.  Nothing here includes, links or calls anything under oracle/.
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include "../../include/gx.h"
+#include "gx_kernels.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define GX_CUDA(call)                                                                              \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? GX_ERR_OOM : GX_ERR_CUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                   \
+    } while (0)
+
+struct DeviceGuard {   // make the scene's device current for the duration of a call
+    int prev = -1;
+    bool ok = false;
+    explicit DeviceGuard(int dev) {
+        if (cudaGetDevice(&prev) != cudaSuccess) return;
+        ok = prev == dev || cudaSetDevice(dev) == cudaSuccess;
+        if (prev == dev) prev = -1;
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+template <typename T>
+struct DevBuf {
+    T *p = nullptr;
+    size_t n = 0;
+    int reserve(size_t want) {   // grow only; contents are not kept
+        if (want <= n) return GX_OK;
+        if (p) cudaFree(p);
+        p = nullptr;
+        n = 0;
+        GX_CUDA(cudaMalloc(&p, want * sizeof(T)));
+        n = want;
+        return GX_OK;
+    }
+    void release() {
+        if (p) cudaFree(p);
+        p = nullptr;
+        n = 0;
+    }
+};
+
+}  // namespace
+
+struct GxScene {
+    int device = 0;
+    int num_sms = 0;
+    int n_static = 0, n_dyn = 0;
+    float4 *verts = nullptr;
+    uchar4 *tris = nullptr;
+    GxBatchDev *batches = nullptr;
+    GxClusterDev *clusters = nullptr;
+    GxMeshDev *meshes = nullptr;
+    std::vector<uint32_t> mesh_nt;      // host copy, for id-range validation
+    uint32_t max_dyn_nt = 0, max_static_nt = 0;
+    unsigned int *env_counter = nullptr;
+    unsigned long long *stats = nullptr;   // device [GX_NSTAT]
+    int opt_cull = 1;
+    int opt_stats = 0;
+    int last_launches = 0;
+    cudaStream_t last_stream = nullptr;
+    // staging for gx_render_batch_host
+    DevBuf<int32_t> h_env_scene, h_inst_mesh;
+    DevBuf<float> h_cam_pose, h_inst_xform, h_depth;
+    DevBuf<uint8_t> h_rgb;
+    DevBuf<uint32_t> h_id;
+    cudaStream_t host_stream = nullptr;
+};
+
+namespace {
+
+// Cut one mesh into clusters of GX_CLUSTER_TRIS consecutive triangles and batches of <= GX_VCAP unique
+// vertices (gx_types.h).  Vertices are copied per batch in first-use order with the colour packed into .w.
+int build_mesh(const GxMesh &m, std::vector<float4> &verts, std::vector<uchar4> &tris, std::vector<GxBatchDev> &batches,
+               std::vector<GxClusterDev> &clusters, GxMeshDev &out) {
+    out.cluster_off = (uint32_t)clusters.size();
+    out.nt = m.nt;
+    out.pad = 0;
+    std::vector<int32_t> local(m.nv, -1);
+    std::vector<uint32_t> touched;
+    touched.reserve(GX_VCAP);
+    for (uint32_t t0 = 0; t0 < m.nt; t0 += GX_CLUSTER_TRIS) {
+        const uint32_t t1 = std::min<uint32_t>(t0 + GX_CLUSTER_TRIS, m.nt);
+        GxClusterDev c;
+        c.batch_off = (uint32_t)batches.size();
+        c.nbatch = 0;
+        for (int k = 0; k < 3; ++k) { c.bmin[k] = 3.0e38f; c.bmax[k] = -3.0e38f; }
+        uint32_t t = t0;
+        while (t < t1) {
+            GxBatchDev b;
+            b.vert_off = (uint32_t)verts.size();
+            b.tri_off = (uint32_t)tris.size();
+            b.first_tri = t;
+            uint32_t nv = 0, nt = 0;
+            touched.clear();
+            for (; t < t1; ++t, ++nt) {
+                uint32_t idx[3];
+                int fresh = 0;
+                for (int k = 0; k < 3; ++k) {
+                    idx[k] = m.indices[3 * (size_t)t + k];
+                    if (idx[k] >= m.nv) return fail(GX_ERR_INVALID_ARG, "triangle %u references vertex %u >= nv %u", t, idx[k], m.nv);
+                    if (local[idx[k]] < 0 && (k < 1 || idx[k] != idx[0]) && (k < 2 || idx[k] != idx[1])) ++fresh;
+                }
+                if (nv + fresh > (uint32_t)GX_VCAP) break;
+                uchar4 li;
+                unsigned char *lp = &li.x;
+                for (int k = 0; k < 3; ++k) {
+                    if (local[idx[k]] < 0) {
+                        local[idx[k]] = (int32_t)nv++;
+                        touched.push_back(idx[k]);
+                        const float *p = m.positions + 3 * (size_t)idx[k];
+                        const uint8_t *col = m.colors + 3 * (size_t)idx[k];
+                        const uint32_t rgba = (uint32_t)col[0] | ((uint32_t)col[1] << 8) | ((uint32_t)col[2] << 16);
+                        float4 v;
+                        v.x = p[0]; v.y = p[1]; v.z = p[2];
+                        memcpy(&v.w, &rgba, 4);
+                        verts.push_back(v);
+                        for (int a = 0; a < 3; ++a) {
+                            c.bmin[a] = std::min(c.bmin[a], p[a]);
+                            c.bmax[a] = std::max(c.bmax[a], p[a]);
+                        }
+                    }
+                    lp[k] = (unsigned char)local[idx[k]];
+                }
+                li.w = 0;
+                tris.push_back(li);
+            }
+            for (uint32_t v : touched) local[v] = -1;
+            b.nv_nt = nv | (nt << 16);
+            batches.push_back(b);
+            ++c.nbatch;
+        }
+        clusters.push_back(c);
+    }
+    out.ncluster = (uint32_t)clusters.size() - out.cluster_off;
+    return GX_OK;
+}
+
+template <typename T>
+int upload(T *&dst, const std::vector<T> &src) {
+    const size_t n = std::max<size_t>(src.size(), 1);
+    GX_CUDA(cudaMalloc(&dst, n * sizeof(T)));
+    if (!src.empty()) GX_CUDA(cudaMemcpy(dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return GX_OK;
+}
+
+struct LaunchPlan {
+    int warps, minb;
+    size_t smem;
+    int grid;
+};
+
+template <int WARPS, int MINB>
+int launch(const GxScene *sc, const GxParams &P, size_t smem, cudaStream_t stream, bool stats) {
+    auto kern = stats ? gx::render_kernel<WARPS, MINB, true> : gx::render_kernel<WARPS, MINB, false>;
+    GX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 0;
+    GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem));
+    if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "kernel does not fit: %zu bytes of shared memory", smem);
+    const int grid = std::min(P.N, sc->num_sms * per_sm);
+    kern<<<grid, WARPS * 32, smem, stream>>>(P);
+    GX_CUDA(cudaGetLastError());
+    return GX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *gx_last_error(void) { return g_err; }
+
+int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh *dyn_meshes, int32_t n_dyn,
+                    int32_t cuda_device, GxScene **out) {
+    if (!out) return fail(GX_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (!static_meshes || n_static <= 0) return fail(GX_ERR_INVALID_ARG, "need at least one static mesh");
+    if (n_dyn < 0 || (n_dyn > 0 && !dyn_meshes)) return fail(GX_ERR_INVALID_ARG, "bad dynamic mesh array");
+    std::vector<float4> verts;
+    std::vector<uchar4> tris;
+    std::vector<GxBatchDev> batches;
+    std::vector<GxClusterDev> clusters;
+    std::vector<GxMeshDev> meshes;
+    GxScene *sc = new (std::nothrow) GxScene();
+    if (!sc) return fail(GX_ERR_OOM, "host allocation failed");
+    try {
+        for (int i = 0; i < n_static + n_dyn; ++i) {
+            const GxMesh &m = i < n_static ? static_meshes[i] : dyn_meshes[i - n_static];
+            if ((m.nv && (!m.positions || !m.colors)) || (m.nt && !m.indices)) {
+                delete sc;
+                return fail(GX_ERR_INVALID_ARG, "mesh %d has NULL arrays", i);
+            }
+            GxMeshDev md;
+            const int rc = build_mesh(m, verts, tris, batches, clusters, md);
+            if (rc != GX_OK) { delete sc; return rc; }
+            meshes.push_back(md);
+            sc->mesh_nt.push_back(m.nt);
+            if (i < n_static) sc->max_static_nt = std::max(sc->max_static_nt, m.nt);
+            else sc->max_dyn_nt = std::max(sc->max_dyn_nt, m.nt);
+        }
+    } catch (const std::bad_alloc &) {
+        delete sc;
+        return fail(GX_ERR_OOM, "host allocation failed while clustering");
+    }
+    if (batches.size() >= (1u << 24) || verts.size() >= 0xFFFFFFFFull || tris.size() >= 0xFFFFFFFFull) {
+        delete sc;
+        return fail(GX_ERR_UNSUPPORTED, "scene too large: %zu batches", batches.size());
+    }
+    sc->device = cuda_device;
+    sc->n_static = n_static;
+    sc->n_dyn = n_dyn;
+    DeviceGuard guard(cuda_device);
+    int rc = GX_OK;
+    if (!guard.ok) rc = fail(GX_ERR_CUDA, "cannot select CUDA device %d", cuda_device);
+    cudaDeviceProp prop;
+    if (rc == GX_OK && cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess)
+        rc = fail(GX_ERR_CUDA, "cudaGetDeviceProperties failed");
+    if (rc == GX_OK) sc->num_sms = prop.multiProcessorCount;
+    if (rc == GX_OK) rc = upload(sc->verts, verts);
+    if (rc == GX_OK) rc = upload(sc->tris, tris);
+    if (rc == GX_OK) rc = upload(sc->batches, batches);
+    if (rc == GX_OK) rc = upload(sc->clusters, clusters);
+    if (rc == GX_OK) rc = upload(sc->meshes, meshes);
+    if (rc == GX_OK) {
+        auto alloc = [&]() -> int {
+            GX_CUDA(cudaMalloc(&sc->env_counter, sizeof(unsigned int)));
+            GX_CUDA(cudaMalloc(&sc->stats, GX_NSTAT * sizeof(unsigned long long)));
+            GX_CUDA(cudaMemset(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long)));
+            return GX_OK;
+        };
+        rc = alloc();
+    }
+    if (rc != GX_OK) {
+        std::string keep = g_err;
+        gx_destroy(sc);
+        snprintf(g_err, sizeof(g_err), "%s", keep.c_str());
+        return rc;
+    }
+    *out = sc;
+    return GX_OK;
+}
+
+void gx_destroy(GxScene *sc) {
+    if (!sc) return;
+    DeviceGuard guard(sc->device);
+    cudaFree(sc->verts);
+    cudaFree(sc->tris);
+    cudaFree(sc->batches);
+    cudaFree(sc->clusters);
+    cudaFree(sc->meshes);
+    cudaFree(sc->env_counter);
+    cudaFree(sc->stats);
+    sc->h_env_scene.release(); sc->h_inst_mesh.release(); sc->h_cam_pose.release(); sc->h_inst_xform.release();
+    sc->h_depth.release(); sc->h_rgb.release(); sc->h_id.release();
+    if (sc->host_stream) cudaStreamDestroy(sc->host_stream);
+    delete sc;
+}
+
+int gx_set_option(GxScene *sc, const char *name, int64_t value) {
+    if (!sc || !name) return fail(GX_ERR_INVALID_ARG, "NULL argument");
+    if (!strcmp(name, "cull")) { sc->opt_cull = value != 0; return GX_OK; }
+    if (!strcmp(name, "stats")) { sc->opt_stats = value != 0; return GX_OK; }
+    return fail(GX_ERR_INVALID_ARG, "unknown option '%s'", name);
+}
+
+int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
+    if (!sc || !name || !out) return fail(GX_ERR_INVALID_ARG, "NULL argument");
+    if (!strcmp(name, "launches")) { *out = sc->last_launches; return GX_OK; }
+    static const char *names[GX_NSTAT] = {"clusters_tested", "clusters_drawn", "triangles_in", "triangles_raster",
+                                          "fragments"};
+    for (int k = 0; k < GX_NSTAT; ++k)
+        if (!strcmp(name, names[k])) {
+            DeviceGuard guard(sc->device);
+            unsigned long long v[GX_NSTAT];
+            GX_CUDA(cudaStreamSynchronize(sc->last_stream));
+            GX_CUDA(cudaMemcpy(v, sc->stats, sizeof(v), cudaMemcpyDeviceToHost));
+            *out = (int64_t)v[k];
+            return GX_OK;
+        }
+    return fail(GX_ERR_INVALID_ARG, "unknown stat '%s'", name);
+}
+
+int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
+                    const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,
+                    float *depth_out, uint32_t *id_out, void *cuda_stream) {
+    if (!sc || !cam) return fail(GX_ERR_INVALID_ARG, "NULL scene or camera");
+    if (N <= 0) return fail(GX_ERR_INVALID_ARG, "N must be positive, got %d", N);
+    if (K < 0 || K > GX_MAX_INSTANCES) return fail(GX_ERR_INVALID_ARG, "K must be in [0, %d], got %d", GX_MAX_INSTANCES, K);
+    if (!env_scene || !cam_pose || !depth_out) return fail(GX_ERR_INVALID_ARG, "env_scene, cam_pose and depth_out are required");
+    if (K > 0 && (!inst_mesh || !inst_xform)) return fail(GX_ERR_INVALID_ARG, "inst_mesh and inst_xform are required when K > 0");
+    if (cam->width <= 0 || cam->height <= 0 || cam->width % 16 || cam->height % 16)
+        return fail(GX_ERR_INVALID_ARG, "width and height must be positive multiples of 16, got %dx%d", cam->width, cam->height);
+    if (!(cam->znear > 0.0f) || !(cam->zfar > cam->znear)) return fail(GX_ERR_INVALID_ARG, "need 0 < znear < zfar");
+    if (!(cam->fx > 0.0f) || !(cam->fy > 0.0f)) return fail(GX_ERR_INVALID_ARG, "fx and fy must be positive");
+    if ((long long)cam->width * cam->height > 16384)
+        return fail(GX_ERR_UNSUPPORTED, "width*height = %lld exceeds 16384 (the frame must fit shared memory)",
+                    (long long)cam->width * cam->height);
+    if ((unsigned long long)sc->max_static_nt + (unsigned long long)K * sc->max_dyn_nt >= (1ull << 31))
+        return fail(GX_ERR_UNSUPPORTED, "more than 2^31 triangles per environment");
+    DeviceGuard guard(sc->device);
+    if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    GxParams P;
+    P.verts = sc->verts; P.tris = sc->tris; P.batches = sc->batches; P.clusters = sc->clusters; P.meshes = sc->meshes;
+    P.n_static = sc->n_static; P.n_dyn = sc->n_dyn;
+    P.N = N; P.K = K; P.W = cam->width; P.H = cam->height;
+    P.fx = cam->fx; P.fy = cam->fy; P.znear = cam->znear; P.zfar = cam->zfar;
+    P.env_scene = env_scene; P.cam_pose = cam_pose; P.inst_mesh = inst_mesh; P.inst_xform = inst_xform;
+    P.rgb = rgb_out; P.depth = depth_out; P.id = id_out;
+    P.env_counter = sc->env_counter; P.stats = sc->stats;
+    P.cull = sc->opt_cull;
+
+    GX_CUDA(cudaMemsetAsync(sc->env_counter, 0, sizeof(unsigned int), stream));
+    if (sc->opt_stats) GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
+    // Big frames: one 16-warp CTA per SM owns the whole frame.  Small frames (<= 64 KB of keys): 8-warp CTAs,
+    // three per SM, so that one CTA's serial phases overlap another's geometry.
+    const bool small_frame = (size_t)P.W * P.H * 8 <= 32768;
+    int rc;
+    if (small_frame) rc = launch<8, 3>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, sc->opt_stats != 0);
+    else rc = launch<16, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 16), stream, sc->opt_stats != 0);
+    if (rc != GX_OK) return rc;
+    sc->last_launches = 1;
+    sc->last_stream = stream;
+    return GX_OK;
+}
+
+int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
+                         const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,
+                         float *depth_out, uint32_t *id_out) {
+    if (!sc || !cam) return fail(GX_ERR_INVALID_ARG, "NULL scene or camera");
+    if (N <= 0 || K < 0) return fail(GX_ERR_INVALID_ARG, "bad N or K");
+    if (!env_scene || !cam_pose || !depth_out || (K > 0 && (!inst_mesh || !inst_xform)))
+        return fail(GX_ERR_INVALID_ARG, "NULL array argument");
+    if (cam->width <= 0 || cam->height <= 0) return fail(GX_ERR_INVALID_ARG, "bad camera size");
+    DeviceGuard guard(sc->device);
+    if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
+    if (!sc->host_stream) GX_CUDA(cudaStreamCreateWithFlags(&sc->host_stream, cudaStreamNonBlocking));
+    cudaStream_t st = sc->host_stream;
+    const size_t npix = (size_t)cam->width * cam->height, nk = (size_t)N * K;
+    int rc;
+    if ((rc = sc->h_env_scene.reserve(N)) || (rc = sc->h_cam_pose.reserve((size_t)N * 16)) ||
+        (rc = sc->h_inst_mesh.reserve(std::max<size_t>(nk, 1))) || (rc = sc->h_inst_xform.reserve(std::max<size_t>(nk * 16, 1))) ||
+        (rc = sc->h_depth.reserve(N * npix)) || (rgb_out && (rc = sc->h_rgb.reserve(N * npix * 3))) ||
+        (id_out && (rc = sc->h_id.reserve(N * npix))))
+        return rc;
+    GX_CUDA(cudaMemcpyAsync(sc->h_env_scene.p, env_scene, (size_t)N * 4, cudaMemcpyHostToDevice, st));
+    GX_CUDA(cudaMemcpyAsync(sc->h_cam_pose.p, cam_pose, (size_t)N * 64, cudaMemcpyHostToDevice, st));
+    if (K > 0) {
+        GX_CUDA(cudaMemcpyAsync(sc->h_inst_mesh.p, inst_mesh, nk * 4, cudaMemcpyHostToDevice, st));
+        GX_CUDA(cudaMemcpyAsync(sc->h_inst_xform.p, inst_xform, nk * 64, cudaMemcpyHostToDevice, st));
+    }
+    rc = gx_render_batch(sc, cam, N, K, sc->h_env_scene.p, sc->h_cam_pose.p, K > 0 ? sc->h_inst_mesh.p : nullptr,
+                         K > 0 ? sc->h_inst_xform.p : nullptr, rgb_out ? sc->h_rgb.p : nullptr, sc->h_depth.p,
+                         id_out ? sc->h_id.p : nullptr, st);
+    if (rc != GX_OK) return rc;
+    GX_CUDA(cudaMemcpyAsync(depth_out, sc->h_depth.p, N * npix * 4, cudaMemcpyDeviceToHost, st));
+    if (rgb_out) GX_CUDA(cudaMemcpyAsync(rgb_out, sc->h_rgb.p, N * npix * 3, cudaMemcpyDeviceToHost, st));
+    if (id_out) GX_CUDA(cudaMemcpyAsync(id_out, sc->h_id.p, N * npix * 4, cudaMemcpyDeviceToHost, st));
+    GX_CUDA(cudaStreamSynchronize(st));
+    return GX_OK;
+}
+
+}  // extern "C"
