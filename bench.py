@@ -1,0 +1,322 @@
+#!/usr/bin/env python
+"""bench.py -- rendered env-frames/s of the batch RGBD rasteriser and its HBM-roofline fraction.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl gx|reference] [--config 2]
+
+A "step" is one pass of the whole hot path (K1 cull .. K5 write) over one batch: one
+gx_render_batch call on BASELINE.json configs[2] (1024 envs, 128x128 RGBD, 4 scenes x 50k triangles, 20
+icospheres + 5 robot links per env), the configuration BASELINE.json's metric and target are quoted on.
+Inputs are seeded synthetic (paper_2306_07552_b200/gen.py) and resident in HBM before the timed region;
+outputs stay in HBM (the zero-copy hand-off of PAPER.md:91).  Multi-GPU: environments are independent, so
+every rank renders its own 1024-env batch with no collective ("weak" scaling); time is
+the max over ranks.
+
+Prints ONE JSON line (rank 0).  `value` = env-frames/s, device timed; `e2e` = the same metric through
+gx_render_batch_host with pinned HOST buffers (H2D of poses/transforms and D2H of RGBD inside the timed
+region); `roofline` = algorithmic bytes (accounting.py: culled geometry + RGBD out) / render-kernel time
+against the measured HBM copy peak; `cpu_baseline` = the CPU oracle on this box's host cores.
+
+--impl reference times the oracle itself (this tier's reference arm): each step renders a bounded sample
+of the same workload on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "rendered env-frames/sec (RGBD) at 1 B200; HBM-roofline fraction"
+UNIT = "env-frames/s"
+NOMINAL_HBM_GBS = 8000.0        # north_star divides by 8 TB/s
+FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="gx", choices=["gx", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2, the graded one)")
+    ap.add_argument("--envs", type=int, default=0, help="render only the first n environments (development)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.25)
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def load_workload(cfg: int, n_envs: int):
+    from paper_2306_07552_b200 import gen
+    wl = gen.make_config(cfg, n_envs=n_envs or None)
+    return wl
+
+
+def workload_name(cfg: int, wl) -> str:
+    from paper_2306_07552_b200 import gen
+    return f"configs[{cfg}]: {gen.CONFIG_SHAPES[cfg][0]}" + ("" if wl.N == gen.CONFIG_SHAPES[cfg][1] else f" (first {wl.N} envs)")
+
+
+def time_oracle(wl, budget_s: float = 15.0):
+    """The oracle as it stands, all host cores (OpenMP over environments), on a bounded sample: whole
+    passes over the first S environments until ~budget_s of wall time is spent."""
+    import oracle
+    oracle.build()
+    cores = len(os.sched_getaffinity(0))
+    probe = wl.subset(np.arange(min(wl.N, 4 * cores)))
+    t0 = time.perf_counter(); oracle.render(probe, n_threads=cores); dt = time.perf_counter() - t0
+    rate = probe.N / dt
+    S = int(min(wl.N, max(4 * cores, rate * budget_s)))
+    sample = wl if S == wl.N else wl.subset(np.arange(S))
+    reps = max(1, int(budget_s / max(S / rate, 1e-3)))
+    reps = min(reps, 20)
+    t0 = time.perf_counter()
+    for _ in range(reps):
+        oracle.render(sample, n_threads=cores)
+    dt = time.perf_counter() - t0
+    return {"value": S * reps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {S} of {wl.N} envs x {reps} passes, {dt:.1f} s wall, OpenMP over envs"}
+
+
+def run_reference(args):
+    """Reference arm = the CPU oracle (tier framing (4)): rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    oracle.build()
+    wl = load_workload(args.config, args.envs)
+    cores = len(os.sched_getaffinity(0))
+    probe = wl.subset(np.arange(min(wl.N, 2 * cores)))
+    t0 = time.perf_counter(); oracle.render(probe, n_threads=cores); rate = probe.N / (time.perf_counter() - t0)
+    # bound the whole run to ~2 minutes: each step renders S environments
+    S = int(min(wl.N, max(cores, rate * 120.0 / max(args.steps + args.warmup, 1))))
+    sample = wl if S == wl.N else wl.subset(np.arange(S))
+    for _ in range(args.warmup):
+        oracle.render(sample, n_threads=cores)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        oracle.render(sample, n_threads=cores)
+    dt = time.perf_counter() - t0
+    value = S * args.steps / dt
+    desc = f"first {S} of {wl.N} envs per step, OpenMP over envs"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps * (wl.N / S),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32+i64", "data": "synthetic",
+        "config": {"workload": workload_name(args.config, wl), "envs_per_step_sampled": S,
+                   "note": "ms_per_step is scaled to the full batch (N/S x the sampled step)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+def run_gx(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2306_07552_b200 import accounting, binding as gx, build as gx_build
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the render path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=dev)
+    if rank == 0:
+        gx_build.build()
+    if world > 1:
+        dist.barrier()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    wl = load_workload(args.config, args.envs)
+    N, K, H, W = wl.N, wl.K, wl.height, wl.width
+    scene = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, local)
+    cam = gx.camera_of(wl)
+    h_in = [np.ascontiguousarray(wl.env_scene, np.int32), np.ascontiguousarray(wl.cam_pose, np.float32),
+            np.ascontiguousarray(wl.inst_mesh, np.int32), np.ascontiguousarray(wl.inst_xform, np.float32)]
+    d_in = [torch.from_numpy(a).to(dev) for a in h_in]
+    rgb = None if wl.depth_only else torch.empty((N, H, W, 3), dtype=torch.uint8, device=dev)
+    depth = torch.empty((N, H, W), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def step():
+        gx.gx_render_batch(scene, cam, N, K, d_in[0], d_in[1], d_in[2] if K else None, d_in[3] if K else None,
+                           rgb, depth, None, stream)
+
+    with ClockSampler(local) as clk:
+        for _ in range(max(args.warmup, 0)):
+            step()
+        barrier()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a, b in ev:
+            flush.zero_()            # L2 flush between timed iterations (untimed)
+            a.record()
+            step()
+            b.record()
+        barrier()
+        ms = [a.elapsed_time(b) for a, b in ev]
+        # keep the GPU under load a little longer so that nvidia-smi (200 ms period) sees the render clocks
+        t_end = time.perf_counter() + max(0.0, 1.0 - 1e-3 * sum(ms))
+        while time.perf_counter() < t_end:
+            step()
+            torch.cuda.synchronize()
+    total_ms = float(sum(ms))
+    launches = gx.gx_get_stat(scene, "launches")
+    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms_max = float(t.item())
+    ms_per_step = total_ms_max / args.steps
+    value = world * N * args.steps / (total_ms_max * 1e-3)
+
+    # ---- e2e: host buffers in, host buffers out, through gx_render_batch_host -------------------------
+    e2e = None
+    if not args.no_e2e:
+        p_in = [torch.from_numpy(a).pin_memory() for a in h_in]
+        p_rgb = None if wl.depth_only else torch.empty((N, H, W, 3), dtype=torch.uint8).pin_memory()
+        p_depth = torch.empty((N, H, W), dtype=torch.float32).pin_memory()
+        n_e2e = max(3, min(args.steps, 10))
+
+        def host_step():
+            gx.gx_render_batch_host(scene, cam, N, K, p_in[0], p_in[1], p_in[2] if K else None,
+                                    p_in[3] if K else None, p_rgb, p_depth, None)
+        for _ in range(2):
+            host_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            host_step()
+        dt = time.perf_counter() - t0
+        t = torch.tensor([dt], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        h2d = sum(a.nbytes for a in h_in)
+        d2h = N * H * W * (4 if wl.depth_only else 7)
+        e2e = {"value": world * N * n_e2e / float(t.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+               "d2h_bytes_per_step": int(d2h), "steps": n_e2e,
+               "note": "gx_render_batch_host: pinned host inputs -> device, render, RGBD -> pinned host, sync"}
+        # the e2e images must be the device-path images
+        assert np.array_equal(p_depth.numpy().view(np.uint32), depth.cpu().numpy().view(np.uint32))
+
+    if rank != 0:
+        gx.gx_destroy(scene)
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline: algorithmic bytes / render-kernel time --------------------------------------------
+    peak, peak_src = measured_peak()
+    b = accounting.env_bytes(wl)
+    bytes_per_launch = float(b["total"].sum())
+    kernel_ms = total_ms / args.steps                  # one kernel per step: its duration is the step's
+    achieved = bytes_per_launch / (kernel_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "kernel": "gx::render_kernel",
+                "kernel_ms": kernel_ms, "algorithmic_bytes_per_launch": bytes_per_launch,
+                "bytes_per_env": {k: float(b[k].mean()) for k in ("cull", "geom", "out", "total")},
+                "post_cull_tris_per_env": float(b["tris"].mean()),
+                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
+    cpu = None if args.no_cpu_baseline else time_oracle(wl)
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32", "data": "synthetic",
+        "config": {"workload": workload_name(args.config, wl), "envs_per_gpu": N, "width": W, "height": H,
+                   "instances_per_env": K, "tris_per_env": float(wl.tris_per_env().mean()),
+                   "outputs": "depth f32" if wl.depth_only else "rgb u8 + depth f32",
+                   "l2": "256 MB buffer written between timed iterations (untimed)",
+                   "arithmetic": "f32 vertex stage, i32/i64 fixed-point coverage, f32 depth/colour"},
+        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches) * args.steps,
+        "roofline": roofline, "cpu_baseline": cpu,
+    }
+    print(json.dumps(out), flush=True)
+    gx.gx_destroy(scene)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gx(args)
+
+
+if __name__ == "__main__":
+    main()
