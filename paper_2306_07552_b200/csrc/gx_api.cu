@@ -78,6 +78,8 @@ struct GxScene {
     GxMeshDev *meshes = nullptr;
     std::vector<uint32_t> mesh_nt;      // host copy, for id-range validation
     uint32_t max_dyn_nt = 0, max_static_nt = 0;
+    uint32_t max_nbatch = 1;            // largest number of batches in any cluster
+    int max_smem_optin = 0;
     unsigned int *env_counter = nullptr;
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
     int opt_cull = 1;
@@ -239,7 +241,11 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
     cudaDeviceProp prop;
     if (rc == GX_OK && cudaGetDeviceProperties(&prop, cuda_device) != cudaSuccess)
         rc = fail(GX_ERR_CUDA, "cudaGetDeviceProperties failed");
-    if (rc == GX_OK) sc->num_sms = prop.multiProcessorCount;
+    if (rc == GX_OK) {
+        sc->num_sms = prop.multiProcessorCount;
+        sc->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
+        for (const GxClusterDev &c : clusters) sc->max_nbatch = std::max(sc->max_nbatch, c.nbatch);
+    }
     if (rc == GX_OK) rc = upload(sc->verts, verts);
     if (rc == GX_OK) rc = upload(sc->tris, tris);
     if (rc == GX_OK) rc = upload(sc->batches, batches);
@@ -334,15 +340,21 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     P.rgb = rgb_out; P.depth = depth_out; P.id = id_out;
     P.env_counter = sc->env_counter; P.stats = sc->stats;
     P.cull = sc->opt_cull;
+    P.cull_chunk = gx::WORK_CAP / (int)sc->max_nbatch;
 
     GX_CUDA(cudaMemsetAsync(sc->env_counter, 0, sizeof(unsigned int), stream));
     if (sc->opt_stats) GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
-    // Big frames: one 16-warp CTA per SM owns the whole frame.  Small frames (<= 64 KB of keys): 8-warp CTAs,
-    // three per SM, so that one CTA's serial phases overlap another's geometry.
+    // Small frames (<= 32 KB of keys): 8-warp CTAs, several per SM, so that one CTA's serial phases overlap
+    // another's geometry.  Big frames: one CTA per SM owns the whole frame, with as many warps as the rest of
+    // the 227 KB of shared memory holds warp-private staging for.
     const bool small_frame = (size_t)P.W * P.H * 8 <= 32768;
+    const size_t cap = (size_t)sc->max_smem_optin - 256;   // static shared memory of the kernel
+    const bool st = sc->opt_stats != 0;
     int rc;
-    if (small_frame) rc = launch<8, 3>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, sc->opt_stats != 0);
-    else rc = launch<16, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 16), stream, sc->opt_stats != 0);
+    if (small_frame) rc = launch<8, 2>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, st);
+    else if (gx::kernel_smem_bytes(P.W, P.H, K, 16) <= cap) rc = launch<16, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 16), stream, st);
+    else if (gx::kernel_smem_bytes(P.W, P.H, K, 12) <= cap) rc = launch<12, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 12), stream, st);
+    else rc = launch<8, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, st);
     if (rc != GX_OK) return rc;
     sc->last_launches = 1;
     sc->last_stream = stream;

@@ -20,8 +20,7 @@ namespace gx {
 
 constexpr unsigned long long KEY_BG = 0xFFFFFFFFFFFFFFFFull;
 constexpr int X_OUT = (int)0x80000000;   // staged X of a vertex behind the near plane
-constexpr int WORK_CAP = 2048;           // work items (batches) per cull chunk
-constexpr int CULL_CHUNK = WORK_CAP / GX_MAX_BATCH_PER_CLUSTER;  // clusters per cull chunk
+constexpr int WORK_CAP = 1024;           // work items (batches) per cull chunk; clusters per chunk = P.cull_chunk
 constexpr int SMALL_MAX_PX = 6;          // bounding boxes up to this many pixels are shaded by one lane
 constexpr int KMAX = 254;
 
@@ -165,14 +164,28 @@ struct EnvSmem {
     uint32_t *work;       // [WORK_CAP] slot << 24 | global batch index
 };
 
+// Record of a set-up "narrow" triangle (bounding-box extent < NARROW_EXT sub-pixel units in x and y, so every
+// edge value at a pixel centre of its bounding box fits int32).  Stored SoA: word k of record r at rec[k*32+r].
+enum { R_E0 = 0, R_E1, R_E2,   // E_e - bias_e at the bounding-box origin pixel (i0, j0)
+       R_D0, R_D1, R_D2,       // edge deltas: dx_e << 16 | (dy_e & 0xFFFF)
+       R_Q0, R_Q1, R_Q2,       // q = 1/w of vertices 0, 1, 2 (after orientation normalisation)
+       R_FA,                   // (float)A
+       R_ID,                   // id << 1 | sub
+       R_BB,                   // i0 | j0 << 7 | (w-1) << 14 | (h-1) << 21 | bias bits << 28
+       REC_WORDS };
+constexpr int NARROW_EXT = 30000;   // 2 * 30000 * (30000 + 3*256) < 2^31
+constexpr int FQ_CAP = 256;         // fragment queue entries per warp
+
 struct WarpSmem {
     int2 *vXY;            // [GX_VCAP] snapped position, X = X_OUT if behind the near plane
     float *vQ;            // [GX_VCAP] 1/w
-    unsigned char *surv;  // [256] batch-local indices of triangles that passed the bbox reject
-    unsigned char *clipl; // [256] ... of triangles that straddle the near plane
+    unsigned char *lst;   // [256] batch-local triangle indices: narrow survivors from the front, slow-path
+                          //       triangles (wide, or straddling the near plane) from the back
+    uint32_t *rec;        // [REC_WORDS * 32] records of the current group
+    uint32_t *fq;         // [FQ_CAP] covered fragments: r | (x - i0) << 5 | (y - j0) << 12
 };
 
-constexpr int WARP_SMEM_BYTES = GX_VCAP * 8 + GX_VCAP * 4 + 256 + 256;
+constexpr int WARP_SMEM_BYTES = GX_VCAP * 8 + GX_VCAP * 4 + 256 + REC_WORDS * 32 * 4 + FQ_CAP * 4;
 
 __host__ __device__ inline size_t env_smem_bytes(int K) {
     return (size_t)(K + 1) * 48 + (size_t)(K + 2) * 8 + (size_t)(K + 1) * 16 + (size_t)WORK_CAP * 4;
@@ -317,11 +330,195 @@ __device__ __forceinline__ int clip_near(const CamVert v[3], const float c[3][3]
 namespace gx {
 
 // ------------------------------------------------------------------------------------------------
-// K2 + K3 + K4 for one batch, by one warp
+// K2c: set-up of narrow survivors into the warp's record group.  Lanes [nrec, nrec + take) each set up one
+// triangle of lst[g .. g + take); records [0, nrec) of earlier batches stay.  Returns take.
+// ------------------------------------------------------------------------------------------------
+template <bool STATS>
+__device__ __forceinline__ int setup_fill(const WarpSmem &ws, const uchar4 *__restrict__ tris, uint32_t idb, int g,
+                                          int nsurv, int nrec, int W, int H, int lane, unsigned &n_tri) {
+    const int take = min(32 - nrec, nsurv - g);
+    const int k = lane - nrec;
+    if (k >= 0 && k < take) {
+        const int t = ws.lst[g + k];
+        const uchar4 ix = __ldg(&tris[t]);
+        const int2 a = ws.vXY[ix.x], b = ws.vXY[ix.y], c = ws.vXY[ix.z];
+        int X[3] = {a.x, b.x, c.x}, Y[3] = {a.y, b.y, c.y};
+        float q[3] = {ws.vQ[ix.x], ws.vQ[ix.y], ws.vQ[ix.z]};
+        int i0, i1, j0, j1;
+        pixel_bbox(X, Y, W, H, i0, i1, j0, j1);   // non-empty: the triangle passed K2b
+        // N6 in int32: |differences| < NARROW_EXT, so every product is < 2^30
+        int A = (X[1] - X[0]) * (Y[2] - Y[0]) - (Y[1] - Y[0]) * (X[2] - X[0]);
+        const bool degenerate = A == 0;
+        if (A < 0) {
+            A = -A;
+            int ti = X[1]; X[1] = X[2]; X[2] = ti;
+            ti = Y[1]; Y[1] = Y[2]; Y[2] = ti;
+            const float tf = q[1]; q[1] = q[2]; q[2] = tf;
+        }
+        const int px0 = (i0 << 8) + 128, py0 = (j0 << 8) + 128;
+        uint32_t bias_bits = 0;
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            const int va = (e + 1) % 3, vb = (e + 2) % 3;
+            int dx = X[vb] - X[va], dy = Y[vb] - Y[va];
+            const bool tl = (dy < 0) || (dy == 0 && dx > 0);
+            int E0 = dx * (py0 - Y[va]) - dy * (px0 - X[va]) - (tl ? 0 : 1);
+            if (degenerate) { E0 = -1; dx = 0; dy = 0; }   // covers nothing
+            bias_bits |= (tl ? 0u : 1u) << e;
+            ws.rec[(R_E0 + e) * 32 + lane] = (uint32_t)E0;
+            ws.rec[(R_D0 + e) * 32 + lane] = ((uint32_t)dx << 16) | ((uint32_t)dy & 0xFFFFu);
+            ws.rec[(R_Q0 + e) * 32 + lane] = __float_as_uint(q[e]);
+        }
+        ws.rec[R_FA * 32 + lane] = __float_as_uint((float)A);
+        ws.rec[R_ID * 32 + lane] = (idb + (uint32_t)t) << 1;
+        ws.rec[R_BB * 32 + lane] = (uint32_t)i0 | ((uint32_t)j0 << 7) | ((uint32_t)(i1 - i0) << 14) |
+                                   ((uint32_t)(j1 - j0) << 21) | (bias_bits << 28);
+        if (STATS) n_tri += degenerate ? 0u : 1u;
+    }
+    __syncwarp();
+    return take;
+}
+
+// ------------------------------------------------------------------------------------------------
+// K4b: depth (N7) and (depth, id) min (N9) for the queued fragments, one fragment per lane.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void shade_queue(const WarpSmem &ws, int qn, int W, float zfar, unsigned long long *fb,
+                                            int lane) {
+    for (int f = lane; f < qn; f += 32) {
+        const uint32_t en = ws.fq[f];
+        const int r = (int)(en & 31u), a = (int)((en >> 5) & 127u), b = (int)((en >> 12) & 127u);
+        const uint32_t bb = ws.rec[R_BB * 32 + r];
+        float fe[3], q[3];
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            const uint32_t d = ws.rec[(R_D0 + e) * 32 + r];
+            const int dx = (int)d >> 16, dy = (int)(short)(d & 0xFFFFu);
+            const int Ee = (int)ws.rec[(R_E0 + e) * 32 + r] + ((b * dx - a * dy) << 8) + (int)((bb >> (28 + e)) & 1u);
+            fe[e] = (float)Ee;
+            q[e] = __uint_as_float(ws.rec[(R_Q0 + e) * 32 + r]);
+        }
+        const float num = fmaf(fe[2], q[2], fmaf(fe[1], q[1], fe[0] * q[0]));
+        const float depth = __uint_as_float(ws.rec[R_FA * 32 + r]) / num;
+        if (depth > zfar) continue;
+        const int x = (int)(bb & 127u) + a, y = (int)((bb >> 7) & 127u) + b;
+        const unsigned long long key = ((unsigned long long)__float_as_uint(depth) << 32) | ws.rec[R_ID * 32 + r];
+        key_min(&fb[fb_index(x, y, W)], key);
+    }
+    __syncwarp();
+}
+
+// ------------------------------------------------------------------------------------------------
+// K3 + K4a: coverage of the nrec records of the warp's group.  The bounding boxes are cut into slots of 4
+// pixels of one row; the T slots of the group are dealt to the lanes in equal contiguous runs (a lane walks
+// through its run, moving to the next record when one is exhausted), so that lanes stay busy whatever the mix
+// of triangle sizes.  Covered pixels are appended to the fragment queue and shaded densely by shade_queue.
+// ------------------------------------------------------------------------------------------------
+template <bool STATS>
+__device__ __forceinline__ void raster_group(const WarpSmem &ws, int nrec, int W, float zfar, unsigned long long *fb,
+                                             int lane, unsigned &n_frag) {
+    const unsigned FULL = 0xFFFFFFFFu;
+    const unsigned lt = (1u << lane) - 1u;
+    int ns = 0;
+    if (lane < nrec) {
+        const uint32_t bb = ws.rec[R_BB * 32 + lane];
+        const int w = (int)((bb >> 14) & 127u) + 1, h = (int)((bb >> 21) & 127u) + 1;
+        ns = h * ((w + 3) >> 2);
+    }
+    int inc = ns;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int v = __shfl_up_sync(FULL, inc, d);
+        if (lane >= d) inc += v;
+    }
+    const int T = __shfl_sync(FULL, inc, 31);
+    const int Pex = inc - ns;
+    const int per = (T + 31) >> 5;
+    const int s0 = lane * per;
+    const int n = min(per, T - s0);
+    int r = 0;   // largest record index with Pex[r] <= s0
+#pragma unroll
+    for (int step = 16; step; step >>= 1) {
+        const int cand = r + step;
+        const int pc = __shfl_sync(FULL, Pex, cand);
+        if (pc <= s0) r = cand;
+    }
+    const int off = s0 - __shfl_sync(FULL, Pex, r);
+
+    int E0[3], dx[3], dy[3], w = 1, h = 1, cw = 1;
+    auto load_rec = [&](int rr) {
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            E0[e] = (int)ws.rec[(R_E0 + e) * 32 + rr];
+            const uint32_t d = ws.rec[(R_D0 + e) * 32 + rr];
+            dx[e] = (int)d >> 16;
+            dy[e] = (int)(short)(d & 0xFFFFu);
+        }
+        const uint32_t bb = ws.rec[R_BB * 32 + rr];
+        w = (int)((bb >> 14) & 127u) + 1;
+        h = (int)((bb >> 21) & 127u) + 1;
+        cw = (w + 3) >> 2;
+    };
+    load_rec(r);
+    int row = off / cw, chunk = off - row * cw;
+    int qn = 0;
+    for (int it = 0; it < per; ++it) {
+        const bool act = it < n;
+        const int a = chunk << 2;
+        unsigned m4 = 0;
+        if (act) {
+            int Ee[3], sx[3];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) {
+                Ee[e] = E0[e] + ((row * dx[e] - a * dy[e]) << 8);
+                sx[e] = -(dy[e] << 8);
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const bool c = ((Ee[0] | Ee[1] | Ee[2]) >= 0) && (a + k < w);
+                m4 |= (c ? 1u : 0u) << k;
+                Ee[0] += sx[0]; Ee[1] += sx[1]; Ee[2] += sx[2];
+            }
+        }
+        if (__any_sync(FULL, m4 != 0)) {
+            const uint32_t ebase = (uint32_t)r | ((uint32_t)a << 5) | ((uint32_t)row << 12);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const bool c = (m4 >> k) & 1u;
+                const unsigned m = __ballot_sync(FULL, c);
+                if (c) ws.fq[qn + __popc(m & lt)] = ebase + ((uint32_t)k << 5);
+                qn += __popc(m);
+            }
+        }
+        if (act) {
+            if (++chunk == cw) {
+                chunk = 0;
+                if (++row == h) {
+                    row = 0;
+                    ++r;
+                    if (it + 1 < n) load_rec(r);
+                }
+            }
+        }
+        if (qn > FQ_CAP - 128) {
+            __syncwarp();
+            if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
+            shade_queue(ws, qn, W, zfar, fb, lane);
+            qn = 0;
+        }
+    }
+    __syncwarp();
+    if (qn) {
+        if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
+        shade_queue(ws, qn, W, zfar, fb, lane);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// K2 + K3 + K4 for one batch, by one warp.  nrec (warp-uniform) = records pending in the warp's group.
 // ------------------------------------------------------------------------------------------------
 template <bool STATS>
 __device__ __forceinline__ void process_batch(const GxParams &P, const Proj &pj, uint32_t item, const EnvSmem &es,
-                                              const WarpSmem &ws, unsigned long long *fb, int lane,
+                                              const WarpSmem &ws, unsigned long long *fb, int lane, int &nrec,
                                               unsigned &n_in, unsigned &n_tri, unsigned &n_frag) {
     const uint32_t s = item >> 24;
     const GxBatchDev b = P.batches[item & 0xFFFFFFu];
@@ -347,11 +544,12 @@ __device__ __forceinline__ void process_batch(const GxParams &P, const Proj &pj,
     }
     __syncwarp();
 
-    // K2b: per triangle, near classification and the pixel-centre bounding-box reject; ballot-compact
-    int nsurv = 0, nclip = 0;
+    // K2b: per triangle, near classification and the pixel-centre bounding-box reject; ballot-compact into
+    // narrow survivors (front of lst) and slow-path triangles (back of lst)
+    int nsurv = 0, nslow = 0;
     for (int t0 = 0; t0 < nt; t0 += 32) {
         const int t = t0 + lane;
-        bool ok = false, cl = false;
+        bool ok = false, slow = false;
         if (t < nt) {
             const uchar4 ix = __ldg(&tris[t]);
             const int2 a = ws.vXY[ix.x], bb = ws.vXY[ix.y], c = ws.vXY[ix.z];
@@ -359,61 +557,76 @@ __device__ __forceinline__ void process_batch(const GxParams &P, const Proj &pj,
             if (nout == 0) {
                 const int X[3] = {a.x, bb.x, c.x}, Y[3] = {a.y, bb.y, c.y};
                 int i0, i1, j0, j1;
-                ok = pixel_bbox(X, Y, P.W, P.H, i0, i1, j0, j1);
+                if (pixel_bbox(X, Y, P.W, P.H, i0, i1, j0, j1)) {
+                    const int ext = max(max(X[0], max(X[1], X[2])) - min(X[0], min(X[1], X[2])),
+                                        max(Y[0], max(Y[1], Y[2])) - min(Y[0], min(Y[1], Y[2])));
+                    ok = ext < NARROW_EXT;
+                    slow = !ok;
+                }
             } else if (nout < 3) {
-                cl = true;
+                slow = true;
             }
         }
-        const unsigned mo = __ballot_sync(0xFFFFFFFFu, ok), mc = __ballot_sync(0xFFFFFFFFu, cl);
-        if (ok) ws.surv[nsurv + __popc(mo & lt)] = (unsigned char)t;
-        if (cl) ws.clipl[nclip + __popc(mc & lt)] = (unsigned char)t;
+        const unsigned mo = __ballot_sync(0xFFFFFFFFu, ok), mc = __ballot_sync(0xFFFFFFFFu, slow);
+        if (ok) ws.lst[nsurv + __popc(mo & lt)] = (unsigned char)t;
+        if (slow) ws.lst[255 - (nslow + __popc(mc & lt))] = (unsigned char)t;
         nsurv += __popc(mo);
-        nclip += __popc(mc);
+        nslow += __popc(mc);
     }
     __syncwarp();
 
-    // K3/K4: survivors, 32 at a time with all lanes busy
-    for (int g = 0; g < nsurv; g += 32) {
-        const bool have = g + lane < nsurv;
-        Tri tri;
-        if (have) {
-            const int t = ws.surv[g + lane];
-            const uchar4 ix = __ldg(&tris[t]);
-            const int2 a = ws.vXY[ix.x], bb = ws.vXY[ix.y], c = ws.vXY[ix.z];
-            tri.X[0] = a.x; tri.X[1] = bb.x; tri.X[2] = c.x;
-            tri.Y[0] = a.y; tri.Y[1] = bb.y; tri.Y[2] = c.y;
-            tri.q[0] = ws.vQ[ix.x]; tri.q[1] = ws.vQ[ix.y]; tri.q[2] = ws.vQ[ix.z];
-            tri.id2 = (idb + (uint32_t)t) << 1;
+    // K2c + K3 + K4: narrow survivors through the record group
+    for (int g = 0; g < nsurv;) {
+        const int take = setup_fill<STATS>(ws, tris, idb, g, nsurv, nrec, P.W, P.H, lane, n_tri);
+        g += take;
+        nrec += take;
+        if (nrec == 32) {
+            raster_group<STATS>(ws, 32, P.W, P.zfar, fb, lane, n_frag);
+            nrec = 0;
         }
-        raster_warp<STATS>(tri, have, P.W, P.H, P.zfar, fb, lane, n_tri, n_frag);
     }
 
-    // near-plane straddlers: N4 clip, then the same raster, piece by piece
-    for (int g = 0; g < nclip; g += 32) {
-        const bool have = g + lane < nclip;
+    // slow path: wide triangles (int64 edge functions) and near-plane straddlers (N4 clip), piece by piece
+    for (int g = 0; g < nslow; g += 32) {
+        const bool have = g + lane < nslow;
         CamVert cv[3];
+        Tri whole;
         int t = 0;
+        bool clipped = false;
         if (have) {
-            t = ws.clipl[g + lane];
+            t = ws.lst[255 - (g + lane)];
             const uchar4 ix = __ldg(&tris[t]);
-            const float4 p0 = __ldg(&verts[ix.x]), p1 = __ldg(&verts[ix.y]), p2 = __ldg(&verts[ix.z]);
-            cv[0] = xform(M, p0.x, p0.y, p0.z);
-            cv[1] = xform(M, p1.x, p1.y, p1.z);
-            cv[2] = xform(M, p2.x, p2.y, p2.z);
+            const int2 a = ws.vXY[ix.x], bb = ws.vXY[ix.y], c = ws.vXY[ix.z];
+            clipped = a.x == X_OUT || bb.x == X_OUT || c.x == X_OUT;
+            if (clipped) {
+                const float4 p0 = __ldg(&verts[ix.x]), p1 = __ldg(&verts[ix.y]), p2 = __ldg(&verts[ix.z]);
+                cv[0] = xform(M, p0.x, p0.y, p0.z);
+                cv[1] = xform(M, p1.x, p1.y, p1.z);
+                cv[2] = xform(M, p2.x, p2.y, p2.z);
+            } else {
+                whole.X[0] = a.x; whole.X[1] = bb.x; whole.X[2] = c.x;
+                whole.Y[0] = a.y; whole.Y[1] = bb.y; whole.Y[2] = c.y;
+                whole.q[0] = ws.vQ[ix.x]; whole.q[1] = ws.vQ[ix.y]; whole.q[2] = ws.vQ[ix.z];
+            }
         }
 #pragma unroll 1
         for (int sub = 0; sub < 2; ++sub) {
             Tri tri;
             bool h2 = false;
             if (have) {
-                CamVert o[3];
-                const int np = clip_near<false>(cv, nullptr, P.znear, sub, o, nullptr);
-                h2 = sub < np;
-                if (h2) {
+                if (clipped) {
+                    CamVert o[3];
+                    const int np = clip_near<false>(cv, nullptr, P.znear, sub, o, nullptr);
+                    h2 = sub < np;
+                    if (h2) {
 #pragma unroll
-                    for (int k = 0; k < 3; ++k) project(pj, o[k].xc, o[k].yc, o[k].w, tri.X[k], tri.Y[k], tri.q[k]);
-                    tri.id2 = ((idb + (uint32_t)t) << 1) | (unsigned)sub;
+                        for (int k = 0; k < 3; ++k) project(pj, o[k].xc, o[k].yc, o[k].w, tri.X[k], tri.Y[k], tri.q[k]);
+                    }
+                } else {
+                    h2 = sub == 0;
+                    tri = whole;
                 }
+                tri.id2 = ((idb + (uint32_t)t) << 1) | (unsigned)sub;
             }
             raster_warp<STATS>(tri, h2, P.W, P.H, P.zfar, fb, lane, n_tri, n_frag);
         }
@@ -538,8 +751,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) render_kernel(const GxParams
         unsigned char *w = p + (size_t)warp * WARP_SMEM_BYTES;
         ws.vXY = reinterpret_cast<int2 *>(w);
         ws.vQ = reinterpret_cast<float *>(w + GX_VCAP * 8);
-        ws.surv = w + GX_VCAP * 12;
-        ws.clipl = ws.surv + 256;
+        ws.lst = w + GX_VCAP * 12;
+        ws.rec = reinterpret_cast<uint32_t *>(w + GX_VCAP * 12 + 256);
+        ws.fq = ws.rec + REC_WORDS * 32;
     }
     p += (size_t)WARPS * WARP_SMEM_BYTES;
     EnvSmem es;
@@ -641,10 +855,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) render_kernel(const GxParams
 
         // ---- K1 cull + K2..K4 draw, in chunks of the environment's cluster space -------------------
         const uint32_t n_cl = es.cl_base[K + 1];
-        for (uint32_t c0 = 0; c0 < n_cl; c0 += CULL_CHUNK) {
+        int nrec = 0;
+        for (uint32_t c0 = 0; c0 < n_cl; c0 += (uint32_t)P.cull_chunk) {
             if (tid == 0) { s_work_n = 0; s_work_next = 0; }
             __syncthreads();
-            const uint32_t c1 = min(c0 + (uint32_t)CULL_CHUNK, n_cl);
+            const uint32_t c1 = min(c0 + (uint32_t)P.cull_chunk, n_cl);
             for (uint32_t g0 = c0 + warp * 32; g0 < c1; g0 += NT) {
                 const uint32_t g = g0 + lane;
                 uint32_t nb = 0, boff = 0, s = 0;
@@ -679,10 +894,15 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) render_kernel(const GxParams
                 if (lane == 0) wi = atomicAdd(&s_work_next, 1u);
                 wi = __shfl_sync(0xFFFFFFFFu, wi, 0);
                 if (wi >= n_work) break;
-                process_batch<STATS>(P, pj, es.work[wi], es, ws, fb, lane, st_in, st_tri, st_frag);
+                process_batch<STATS>(P, pj, es.work[wi], es, ws, fb, lane, nrec, st_in, st_tri, st_frag);
             }
             __syncthreads();
         }
+        if (nrec) {   // records still pending in this warp's group
+            raster_group<STATS>(ws, nrec, W, P.zfar, fb, lane, st_frag);
+            nrec = 0;
+        }
+        __syncthreads();
 
         // ---- K5a: resolve in place: key -> (depth bits, rgba) ------------------------------------
         const bool want_rgb = P.rgb != nullptr;

@@ -55,6 +55,7 @@ struct GxParams {
     unsigned int *env_counter;    // zeroed before the launch; persistent CTAs draw environments from it
     unsigned long long *stats;    // [GX_NSTAT], only touched by the STATS instantiation
     int32_t cull;
+    int32_t cull_chunk;           // clusters per cull chunk: WORK_CAP / (largest nbatch of any cluster)
 };
 
 enum { GX_STAT_CLUSTERS_TESTED = 0, GX_STAT_CLUSTERS_DRAWN, GX_STAT_TRIS_IN, GX_STAT_TRIS_RASTER,
