@@ -59,6 +59,11 @@ __device__ __forceinline__ float clip_lerp(float t, float a_in, float a_out) { r
 // contiguous run.
 __device__ __forceinline__ int fb_index(int i, int j, int W) { return j * W + (i ^ ((j & 1) << 3)); }
 
+// st.shared.u32 [addr], v if pred != 0 (a predicated store, no branch)
+__device__ __forceinline__ void sts_if(uint32_t addr, uint32_t v, uint32_t pred) {
+    asm volatile("{ .reg .pred p; setp.ne.u32 p, %2, 0; @p st.shared.u32 [%0], %1; }" ::"r"(addr), "r"(v), "r"(pred) : "memory");
+}
+
 __device__ __forceinline__ void key_min(unsigned long long *slot, unsigned long long key) {
     unsigned long long cur = *reinterpret_cast<volatile unsigned long long *>(slot);
     while (key < cur) {
@@ -166,7 +171,7 @@ struct EnvSmem {
 
 // Record of a set-up "narrow" triangle (bounding-box extent < NARROW_EXT sub-pixel units in x and y, so every
 // edge value at a pixel centre of its bounding box fits int32).  Stored SoA: word k of record r at rec[k*32+r].
-enum { R_E0 = 0, R_E1, R_E2,   // E_e - bias_e at the bounding-box origin pixel (i0, j0)
+enum { R_E0 = 0, R_E1, R_E2,   // E_e at the bounding-box origin pixel (i0, j0)
        R_D0, R_D1, R_D2,       // edge deltas: dx_e << 16 | (dy_e & 0xFFFF)
        R_Q0, R_Q1, R_Q2,       // q = 1/w of vertices 0, 1, 2 (after orientation normalisation)
        R_FA,                   // (float)A
@@ -362,7 +367,7 @@ __device__ __forceinline__ int setup_fill(const WarpSmem &ws, const uchar4 *__re
             const int va = (e + 1) % 3, vb = (e + 2) % 3;
             int dx = X[vb] - X[va], dy = Y[vb] - Y[va];
             const bool tl = (dy < 0) || (dy == 0 && dx > 0);
-            int E0 = dx * (py0 - Y[va]) - dy * (px0 - X[va]) - (tl ? 0 : 1);
+            int E0 = dx * (py0 - Y[va]) - dy * (px0 - X[va]);
             if (degenerate) { E0 = -1; dx = 0; dy = 0; }   // covers nothing
             bias_bits |= (tl ? 0u : 1u) << e;
             ws.rec[(R_E0 + e) * 32 + lane] = (uint32_t)E0;
@@ -393,7 +398,7 @@ __device__ __forceinline__ void shade_queue(const WarpSmem &ws, int qn, int W, f
         for (int e = 0; e < 3; ++e) {
             const uint32_t d = ws.rec[(R_D0 + e) * 32 + r];
             const int dx = (int)d >> 16, dy = (int)(short)(d & 0xFFFFu);
-            const int Ee = (int)ws.rec[(R_E0 + e) * 32 + r] + ((b * dx - a * dy) << 8) + (int)((bb >> (28 + e)) & 1u);
+            const int Ee = (int)ws.rec[(R_E0 + e) * 32 + r] + ((b * dx - a * dy) << 8);
             fe[e] = (float)Ee;
             q[e] = __uint_as_float(ws.rec[(R_Q0 + e) * 32 + r]);
         }
@@ -445,15 +450,15 @@ __device__ __forceinline__ void raster_group(const WarpSmem &ws, int nrec, int W
     const int off = s0 - __shfl_sync(FULL, Pex, r);
 
     int E0[3], dx[3], dy[3], w = 1, h = 1, cw = 1;
-    auto load_rec = [&](int rr) {
+    auto load_rec = [&](int rr) {   // E0 := E_e - bias_e at the origin pixel, so that "covered" is all E0 >= 0
+        const uint32_t bb = ws.rec[R_BB * 32 + rr];
 #pragma unroll
         for (int e = 0; e < 3; ++e) {
-            E0[e] = (int)ws.rec[(R_E0 + e) * 32 + rr];
+            E0[e] = (int)ws.rec[(R_E0 + e) * 32 + rr] - (int)((bb >> (28 + e)) & 1u);
             const uint32_t d = ws.rec[(R_D0 + e) * 32 + rr];
             dx[e] = (int)d >> 16;
             dy[e] = (int)(short)(d & 0xFFFFu);
         }
-        const uint32_t bb = ws.rec[R_BB * 32 + rr];
         w = (int)((bb >> 14) & 127u) + 1;
         h = (int)((bb >> 21) & 127u) + 1;
         cw = (w + 3) >> 2;
@@ -461,6 +466,7 @@ __device__ __forceinline__ void raster_group(const WarpSmem &ws, int nrec, int W
     load_rec(r);
     int row = off / cw, chunk = off - row * cw;
     int qn = 0;
+    const uint32_t fq_addr = (uint32_t)__cvta_generic_to_shared(ws.fq);
     for (int it = 0; it < per; ++it) {
         const bool act = it < n;
         const int a = chunk << 2;
@@ -479,15 +485,26 @@ __device__ __forceinline__ void raster_group(const WarpSmem &ws, int nrec, int W
                 Ee[0] += sx[0]; Ee[1] += sx[1]; Ee[2] += sx[2];
             }
         }
-        if (__any_sync(FULL, m4 != 0)) {
-            const uint32_t ebase = (uint32_t)r | ((uint32_t)a << 5) | ((uint32_t)row << 12);
+        // append the covered pixels: one warp scan of the per-lane counts, then predicated stores
+        const int cnt = __popc(m4);
+        int incl = cnt;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int v = __shfl_up_sync(FULL, incl, d);
+            if (lane >= d) incl += v;
+        }
+        const int tot = __shfl_sync(FULL, incl, 31);
+        if (tot) {
+            uint32_t en = (uint32_t)r | ((uint32_t)a << 5) | ((uint32_t)row << 12);
+            uint32_t addr = fq_addr + (uint32_t)(qn + incl - cnt) * 4u;
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
-                const bool c = (m4 >> k) & 1u;
-                const unsigned m = __ballot_sync(FULL, c);
-                if (c) ws.fq[qn + __popc(m & lt)] = ebase + ((uint32_t)k << 5);
-                qn += __popc(m);
+                const uint32_t bit = (m4 >> k) & 1u;
+                sts_if(addr, en, bit);
+                addr += bit << 2;
+                en += 32u;
             }
+            qn += tot;
         }
         if (act) {
             if (++chunk == cw) {
