@@ -10,7 +10,7 @@
 #include <vector>
 
 #include "../../include/gx.h"
-#include "gx_kernels.cuh"
+#include "gx_pipeline.cuh"
 
 namespace {
 
@@ -84,6 +84,13 @@ struct GxScene {
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
     int opt_cull = 1;
     int opt_stats = 0;
+    int last_chunk_n = 0;               // environments in the last chunk of the last two-kernel call
+    int opt_path = 0;                   // 0 = two-kernel path (geometry -> records -> raster), 1 = single kernel
+    int64_t opt_pool_slots = 0;         // narrow record slots per environment; 0 = max(4096, 4*W*H)
+    int64_t opt_pool_bytes = 0;         // record pool budget; 0 = 8 GB
+    int opt_geom_split = 0;             // geometry work units per environment; 0 = automatic
+    DevBuf<uint4> pool;                 // triangle records of one chunk of environments
+    DevBuf<uint32_t> pipe_scratch;      // counters[4] | cnt[2*chunk] | env_flag[chunk]
     int last_launches = 0;
     cudaStream_t last_stream = nullptr;
     // staging for gx_render_batch_host
@@ -190,6 +197,52 @@ int launch(const GxScene *sc, const GxParams &P, size_t smem, cudaStream_t strea
     return GX_OK;
 }
 
+
+// single-kernel path (gx_kernels.cuh): small frames (<= 32 KB of keys) use 8-warp CTAs, several per SM; big
+// frames one CTA per SM with as many warps as the rest of the 227 KB of shared memory holds staging for.
+int launch_single(const GxScene *sc, const GxParams &P, cudaStream_t stream, bool st) {
+    const int K = P.K;
+    const bool small_frame = (size_t)P.W * P.H * 8 <= 32768;
+    const size_t cap = (size_t)sc->max_smem_optin - 256;   // static shared memory of the kernel
+    if (small_frame) return launch<8, 2>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, st);
+    if (gx::kernel_smem_bytes(P.W, P.H, K, 16) <= cap) return launch<16, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 16), stream, st);
+    if (gx::kernel_smem_bytes(P.W, P.H, K, 12) <= cap) return launch<12, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 12), stream, st);
+    return launch<8, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, st);
+}
+
+template <int WARPS, int MINB>
+int launch_raster(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
+    auto kern = stats ? gx::raster_kernel<WARPS, MINB, true> : gx::raster_kernel<WARPS, MINB, false>;
+    const size_t smem = gx::raster_smem_bytes(PP.g.W, PP.g.H, WARPS);
+    GX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 0;
+    GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem));
+    if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "raster kernel does not fit: %zu bytes of shared memory", smem);
+    kern<<<std::min(PP.g.N, sc->num_sms * per_sm), WARPS * 32, smem, stream>>>(PP);
+    GX_CUDA(cudaGetLastError());
+    return GX_OK;
+}
+
+// two-kernel path (gx_pipeline.cuh): geometry kernel, then raster kernel
+int launch_pipeline(const GxScene *sc, gx::PipeParams &PP, cudaStream_t stream, bool stats) {
+    constexpr int GW = 8;
+    auto gk = stats ? gx::geom_kernel<GW, true> : gx::geom_kernel<GW, false>;
+    const size_t gsmem = gx::geom_smem_bytes(PP.g.K, GW);
+    GX_CUDA(cudaFuncSetAttribute(gk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem));
+    int per_sm = 0;
+    GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gk, GW * 32, gsmem));
+    if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "geometry kernel does not fit: %zu bytes of shared memory", gsmem);
+    const int slots = sc->num_sms * per_sm;
+    // work units per environment: enough units that the last wave of CTAs is a small part of the whole
+    int split = sc->opt_geom_split;
+    if (split <= 0) split = PP.g.N >= 8 * slots ? 1 : std::min(8, std::max(1, (8 * slots + PP.g.N - 1) / PP.g.N));
+    PP.split = split;
+    gk<<<(int)std::min<long long>((long long)PP.g.N * split, slots), GW * 32, gsmem, stream>>>(PP);
+    GX_CUDA(cudaGetLastError());
+    if ((size_t)PP.g.W * PP.g.H * 8 <= 32768) return launch_raster<16, 2>(sc, PP, stream, stats);
+    return launch_raster<32, 1>(sc, PP, stream, stats);
+}
+
 }  // namespace
 
 extern "C" {
@@ -280,6 +333,7 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->meshes);
     cudaFree(sc->env_counter);
     cudaFree(sc->stats);
+    sc->pool.release(); sc->pipe_scratch.release();
     sc->h_env_scene.release(); sc->h_inst_mesh.release(); sc->h_cam_pose.release(); sc->h_inst_xform.release();
     sc->h_depth.release(); sc->h_rgb.release(); sc->h_id.release();
     if (sc->host_stream) cudaStreamDestroy(sc->host_stream);
@@ -290,14 +344,47 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
     if (!sc || !name) return fail(GX_ERR_INVALID_ARG, "NULL argument");
     if (!strcmp(name, "cull")) { sc->opt_cull = value != 0; return GX_OK; }
     if (!strcmp(name, "stats")) { sc->opt_stats = value != 0; return GX_OK; }
+    if (!strcmp(name, "path")) {
+        if (value < 0 || value > 1) return fail(GX_ERR_INVALID_ARG, "path must be 0 or 1");
+        sc->opt_path = (int)value;
+        return GX_OK;
+    }
+    if (!strcmp(name, "pool_slots")) {
+        if (value < 0 || value > (1 << 24)) return fail(GX_ERR_INVALID_ARG, "pool_slots out of range");
+        sc->opt_pool_slots = value;
+        return GX_OK;
+    }
+    if (!strcmp(name, "pool_bytes")) {
+        if (value < 0) return fail(GX_ERR_INVALID_ARG, "pool_bytes must be >= 0");
+        sc->opt_pool_bytes = value;
+        return GX_OK;
+    }
+    if (!strcmp(name, "geom_split")) {
+        if (value < 0 || value > 64) return fail(GX_ERR_INVALID_ARG, "geom_split must be in [0, 64]");
+        sc->opt_geom_split = (int)value;
+        return GX_OK;
+    }
     return fail(GX_ERR_INVALID_ARG, "unknown option '%s'", name);
 }
 
 int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
     if (!sc || !name || !out) return fail(GX_ERR_INVALID_ARG, "NULL argument");
     if (!strcmp(name, "launches")) { *out = sc->last_launches; return GX_OK; }
+    if (!strcmp(name, "max_env_records") || !strcmp(name, "p50_env_records")) {   // last chunk of the two-kernel path
+        *out = 0;
+        if (sc->last_chunk_n <= 0) return GX_OK;
+        DeviceGuard guard(sc->device);
+        std::vector<uint32_t> cnt(2 * (size_t)sc->last_chunk_n);
+        GX_CUDA(cudaStreamSynchronize(sc->last_stream));
+        GX_CUDA(cudaMemcpy(cnt.data(), sc->pipe_scratch.p + 4, cnt.size() * 4, cudaMemcpyDeviceToHost));
+        std::vector<uint32_t> tot(sc->last_chunk_n);
+        for (int e = 0; e < sc->last_chunk_n; ++e) tot[e] = cnt[2 * e] + cnt[2 * e + 1];
+        std::sort(tot.begin(), tot.end());
+        *out = name[0] == 'm' ? tot.back() : tot[tot.size() / 2];
+        return GX_OK;
+    }
     static const char *names[GX_NSTAT] = {"clusters_tested", "clusters_drawn", "triangles_in", "triangles_raster",
-                                          "fragments"};
+                                          "fragments", "overflow_envs"};
     for (int k = 0; k < GX_NSTAT; ++k)
         if (!strcmp(name, names[k])) {
             DeviceGuard guard(sc->device);
@@ -331,6 +418,8 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
 
+    if (cam->width > 128 || cam->height > 128)
+        return fail(GX_ERR_UNSUPPORTED, "width and height must be <= 128 in this build, got %dx%d", cam->width, cam->height);
     GxParams P;
     P.verts = sc->verts; P.tris = sc->tris; P.batches = sc->batches; P.clusters = sc->clusters; P.meshes = sc->meshes;
     P.n_static = sc->n_static; P.n_dyn = sc->n_dyn;
@@ -339,27 +428,65 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     P.env_scene = env_scene; P.cam_pose = cam_pose; P.inst_mesh = inst_mesh; P.inst_xform = inst_xform;
     P.rgb = rgb_out; P.depth = depth_out; P.id = id_out;
     P.env_counter = sc->env_counter; P.stats = sc->stats;
+    P.env_filter = nullptr;
     P.cull = sc->opt_cull;
     P.cull_chunk = gx::WORK_CAP / (int)sc->max_nbatch;
 
-    GX_CUDA(cudaMemsetAsync(sc->env_counter, 0, sizeof(unsigned int), stream));
-    if (sc->opt_stats) GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
-    // Small frames (<= 32 KB of keys): 8-warp CTAs, several per SM, so that one CTA's serial phases overlap
-    // another's geometry.  Big frames: one CTA per SM owns the whole frame, with as many warps as the rest of
-    // the 227 KB of shared memory holds warp-private staging for.
-    const bool small_frame = (size_t)P.W * P.H * 8 <= 32768;
-    const size_t cap = (size_t)sc->max_smem_optin - 256;   // static shared memory of the kernel
+    GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
     const bool st = sc->opt_stats != 0;
-    int rc;
-    if (small_frame) rc = launch<8, 2>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, st);
-    else if (gx::kernel_smem_bytes(P.W, P.H, K, 16) <= cap) rc = launch<16, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 16), stream, st);
-    else if (gx::kernel_smem_bytes(P.W, P.H, K, 12) <= cap) rc = launch<12, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 12), stream, st);
-    else rc = launch<8, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, st);
-    if (rc != GX_OK) return rc;
-    sc->last_launches = 1;
     sc->last_stream = stream;
+    sc->last_chunk_n = 0;
+    if (sc->opt_path == 1) {
+        GX_CUDA(cudaMemsetAsync(sc->env_counter, 0, sizeof(unsigned int), stream));
+        const int rc = launch_single(sc, P, stream, st);
+        if (rc != GX_OK) return rc;
+        sc->last_launches = 1;
+        return GX_OK;
+    }
+
+    // ---- two-kernel path, in chunks of environments that share the record pool ----------------------
+    const int64_t npix = (int64_t)P.W * P.H;
+    const int64_t cap_n = sc->opt_pool_slots > 0 ? sc->opt_pool_slots : std::max<int64_t>(4096, 4 * npix);
+    const int64_t cap_w = std::max<int64_t>(64, cap_n / 8) & ~(int64_t)1;
+    const int64_t env_bytes = (cap_n + cap_w) * 64;
+    const int64_t budget = sc->opt_pool_bytes > 0 ? sc->opt_pool_bytes : (int64_t)8 << 30;
+    const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(N, budget / env_bytes));
+    int rc;
+    if ((rc = sc->pool.reserve((size_t)chunk * (size_t)(cap_n + cap_w) * 4)) != GX_OK) return rc;
+    if ((rc = sc->pipe_scratch.reserve(4 + 3 * (size_t)chunk)) != GX_OK) return rc;
+    int launches = 0;
+    for (int e0 = 0; e0 < N; e0 += chunk) {
+        const int n = std::min(chunk, N - e0);
+        gx::PipeParams PP;
+        PP.g = P;
+        PP.g.N = n;
+        PP.g.env_scene = env_scene + e0;
+        PP.g.cam_pose = cam_pose + (size_t)e0 * 16;
+        PP.g.inst_mesh = inst_mesh ? inst_mesh + (size_t)e0 * K : nullptr;
+        PP.g.inst_xform = inst_xform ? inst_xform + (size_t)e0 * K * 16 : nullptr;
+        PP.g.rgb = rgb_out ? rgb_out + (size_t)e0 * npix * 3 : nullptr;
+        PP.g.depth = depth_out + (size_t)e0 * npix;
+        PP.g.id = id_out ? id_out + (size_t)e0 * npix : nullptr;
+        PP.recs = sc->pool.p;
+        PP.counters = sc->pipe_scratch.p;
+        PP.cnt = sc->pipe_scratch.p + 4;
+        PP.env_flag = sc->pipe_scratch.p + 4 + 2 * (size_t)chunk;
+        PP.cap_n = (int32_t)cap_n;
+        PP.cap_w = (int32_t)cap_w;
+        GX_CUDA(cudaMemsetAsync(sc->pipe_scratch.p, 0, (4 + 3 * (size_t)chunk) * sizeof(uint32_t), stream));
+        if ((rc = launch_pipeline(sc, PP, stream, st)) != GX_OK) return rc;
+        // environments whose records overflowed their pool segment: single-kernel pass over the flagged ones
+        GxParams PL = PP.g;
+        PL.env_counter = sc->pipe_scratch.p + 2;
+        PL.env_filter = PP.env_flag;
+        if ((rc = launch_single(sc, PL, stream, st)) != GX_OK) return rc;
+        launches += 3;
+        sc->last_chunk_n = n;
+    }
+    sc->last_launches = launches;
     return GX_OK;
 }
+
 
 int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
                          const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,

@@ -751,6 +751,114 @@ __device__ __forceinline__ bool cluster_visible(const GxClusterDev &c, const flo
     return true;
 }
 
+
+// ------------------------------------------------------------------------------------------------
+// per-environment setup by the whole CTA (two barriers inside): slot tables, model-view matrices (N1, N2),
+// exclusive scans of triangle and cluster counts over the K+1 slots.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void env_setup(const GxParams &P, int env, const EnvSmem &es, int tid) {
+    const int K = P.K, lane = tid & 31, warp = tid >> 5;
+    for (int sl = tid; sl <= K; sl += (int)blockDim.x) {
+        int mesh = -1;
+        if (sl == 0) mesh = P.env_scene[env];
+        else {
+            const int m = P.inst_mesh[(size_t)env * K + (sl - 1)];
+            if (m >= 0) mesh = P.n_static + m;
+        }
+        uint32_t nt = 0, nc = 0, cl0 = 0;
+        if (mesh >= 0) {
+            const GxMeshDev md = P.meshes[mesh];
+            nt = md.nt; nc = md.ncluster; cl0 = md.cluster_off;
+        }
+        es.slot_mesh[sl] = mesh; es.slot_nt[sl] = nt; es.slot_nc[sl] = nc; es.slot_cl[sl] = cl0;
+        // N1: view matrix from the rigid camera-to-world pose C
+        const float *C = P.cam_pose + (size_t)env * 16;
+        float V[12];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+#pragma unroll
+            for (int j = 0; j < 3; ++j) V[i * 4 + j] = C[j * 4 + i];
+            V[i * 4 + 3] = -fmaf(C[8 + i], C[11], fmaf(C[4 + i], C[7], C[i] * C[3]));
+        }
+        float *MV = es.MV + sl * 12;
+        if (sl == 0) {
+#pragma unroll
+            for (int k = 0; k < 12; ++k) MV[k] = V[k];
+        } else {
+            // N2: MV = V * M (top three rows of the instance transform)
+            const float *M = P.inst_xform + ((size_t)env * K + (sl - 1)) * 16;
+            float Mr[12];
+#pragma unroll
+            for (int k = 0; k < 12; ++k) Mr[k] = M[k];
+#pragma unroll
+            for (int i = 0; i < 3; ++i) {
+#pragma unroll
+                for (int j = 0; j < 3; ++j)
+                    MV[i * 4 + j] = fmaf(V[i * 4 + 2], Mr[8 + j], fmaf(V[i * 4 + 1], Mr[4 + j], V[i * 4] * Mr[j]));
+                MV[i * 4 + 3] = fmaf(V[i * 4 + 2], Mr[11], fmaf(V[i * 4 + 1], Mr[7], fmaf(V[i * 4], Mr[3], V[i * 4 + 3])));
+            }
+        }
+    }
+    __syncthreads();
+    if (warp == 0) {   // exclusive scans of triangle and cluster counts over the K+1 slots
+        uint32_t run_t = 0, run_c = 0;
+        for (int s0 = 0; s0 <= K; s0 += 32) {
+            const int s = s0 + lane;
+            const uint32_t nt = s <= K ? es.slot_nt[s] : 0u, nc = s <= K ? es.slot_nc[s] : 0u;
+            uint32_t it = nt, ic = nc;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, it, d), bq = __shfl_up_sync(0xFFFFFFFFu, ic, d);
+                if (lane >= d) { it += a; ic += bq; }
+            }
+            if (s <= K) { es.id_base[s] = run_t + it - nt; es.cl_base[s] = run_c + ic - nc; }
+            run_t += __shfl_sync(0xFFFFFFFFu, it, 31);
+            run_c += __shfl_sync(0xFFFFFFFFu, ic, 31);
+        }
+        if (lane == 0) { es.id_base[K + 1] = run_t; es.cl_base[K + 1] = run_c; }
+    }
+    __syncthreads();
+}
+
+// ------------------------------------------------------------------------------------------------
+// K1 for the clusters [c0, c1) of the environment's cluster space, by the whole CTA: survivors' batches are
+// appended to es.work by warp-aggregated shared atomics (*s_work_n must be 0 and visible on entry; the
+// caller synchronises afterwards).
+// ------------------------------------------------------------------------------------------------
+template <bool STATS>
+__device__ __forceinline__ void cull_chunk_to_worklist(const GxParams &P, const EnvSmem &es, uint32_t c0, uint32_t c1,
+                                                       int tid, int NT, unsigned *s_work_n, unsigned &st_tested,
+                                                       unsigned &st_drawn) {
+    const int K = P.K, lane = tid & 31, warp = tid >> 5;
+    for (uint32_t g0 = c0 + warp * 32; g0 < c1; g0 += NT) {
+        const uint32_t g = g0 + lane;
+        uint32_t nb = 0, boff = 0, s = 0;
+        if (g < c1) {
+            int lo = 0, hi = K;
+            while (lo < hi) {   // largest slot whose first cluster index is <= g
+                const int mid = (lo + hi + 1) >> 1;
+                if (es.cl_base[mid] <= g) lo = mid; else hi = mid - 1;
+            }
+            s = (uint32_t)lo;
+            const GxClusterDev c = P.clusters[es.slot_cl[s] + (g - es.cl_base[s])];
+            const bool vis = !P.cull || cluster_visible(c, es.MV + s * 12, P.fx, P.fy, P.znear, P.zfar);
+            if (STATS) { ++st_tested; st_drawn += vis ? 1u : 0u; }
+            if (vis) { nb = c.nbatch; boff = c.batch_off; }
+        }
+        uint32_t inc = nb;   // warp-aggregated append: one shared atomic per warp
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+            if (lane >= d) inc += a;
+        }
+        const uint32_t tot = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        uint32_t base = 0;
+        if (lane == 0 && tot) base = atomicAdd(s_work_n, tot);
+        base = __shfl_sync(0xFFFFFFFFu, base, 0) + inc - nb;
+        for (uint32_t k = 0; k < nb; ++k) es.work[base + k] = (s << 24) | (boff + k);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // the kernel
 // ------------------------------------------------------------------------------------------------
@@ -801,74 +909,18 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) render_kernel(const GxParams
         __syncthreads();
         const int env = s_env;
         if (env >= P.N) break;
-
-        // ---- environment setup: slots, model-view matrices (N1, N2), clear the frame -------------
-        if (tid <= K) {
-            int mesh = -1;
-            if (tid == 0) mesh = P.env_scene[env];
-            else {
-                const int m = P.inst_mesh[(size_t)env * K + (tid - 1)];
-                if (m >= 0) mesh = P.n_static + m;
-            }
-            uint32_t nt = 0, nc = 0, cl0 = 0;
-            if (mesh >= 0) {
-                const GxMeshDev md = P.meshes[mesh];
-                nt = md.nt; nc = md.ncluster; cl0 = md.cluster_off;
-            }
-            es.slot_mesh[tid] = mesh; es.slot_nt[tid] = nt; es.slot_nc[tid] = nc; es.slot_cl[tid] = cl0;
-            // N1: view matrix from the rigid camera-to-world pose C
-            const float *C = P.cam_pose + (size_t)env * 16;
-            float V[12];
-#pragma unroll
-            for (int i = 0; i < 3; ++i) {
-#pragma unroll
-                for (int j = 0; j < 3; ++j) V[i * 4 + j] = C[j * 4 + i];
-                V[i * 4 + 3] = -fmaf(C[8 + i], C[11], fmaf(C[4 + i], C[7], C[i] * C[3]));
-            }
-            float *MV = es.MV + tid * 12;
-            if (tid == 0) {
-#pragma unroll
-                for (int k = 0; k < 12; ++k) MV[k] = V[k];
-            } else {
-                // N2: MV = V * M (top three rows of the instance transform)
-                const float *M = P.inst_xform + ((size_t)env * K + (tid - 1)) * 16;
-                float Mr[12];
-#pragma unroll
-                for (int k = 0; k < 12; ++k) Mr[k] = M[k];
-#pragma unroll
-                for (int i = 0; i < 3; ++i) {
-#pragma unroll
-                    for (int j = 0; j < 3; ++j)
-                        MV[i * 4 + j] = fmaf(V[i * 4 + 2], Mr[8 + j], fmaf(V[i * 4 + 1], Mr[4 + j], V[i * 4] * Mr[j]));
-                    MV[i * 4 + 3] = fmaf(V[i * 4 + 2], Mr[11],
-                                         fmaf(V[i * 4 + 1], Mr[7], fmaf(V[i * 4], Mr[3], V[i * 4 + 3])));
-                }
-            }
+        if (P.env_filter && !P.env_filter[env]) {   // overflow pass of the two-kernel path: flagged environments only
+            __syncthreads();
+            continue;
         }
+
+        // ---- environment setup: clear the frame; slots, model-view matrices (N1, N2), id / cluster bases ----
         {
             uint4 *f4 = reinterpret_cast<uint4 *>(fb);
             const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
             for (int k = tid; k < npix / 2; k += NT) f4[k] = ones;
         }
-        __syncthreads();
-        if (warp == 0) {   // exclusive scans of triangle and cluster counts over the K+1 slots
-            uint32_t run_t = 0, run_c = 0;
-            for (int s0 = 0; s0 <= K; s0 += 32) {
-                const int s = s0 + lane;
-                const uint32_t nt = s <= K ? es.slot_nt[s] : 0u, nc = s <= K ? es.slot_nc[s] : 0u;
-                uint32_t it = nt, ic = nc;
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, it, d), bq = __shfl_up_sync(0xFFFFFFFFu, ic, d);
-                    if (lane >= d) { it += a; ic += bq; }
-                }
-                if (s <= K) { es.id_base[s] = run_t + it - nt; es.cl_base[s] = run_c + ic - nc; }
-                run_t += __shfl_sync(0xFFFFFFFFu, it, 31);
-                run_c += __shfl_sync(0xFFFFFFFFu, ic, 31);
-            }
-            if (lane == 0) { es.id_base[K + 1] = run_t; es.cl_base[K + 1] = run_c; }
-        }
-        __syncthreads();
+        env_setup(P, env, es, tid);
 
         // ---- K1 cull + K2..K4 draw, in chunks of the environment's cluster space -------------------
         const uint32_t n_cl = es.cl_base[K + 1];
@@ -876,34 +928,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) render_kernel(const GxParams
         for (uint32_t c0 = 0; c0 < n_cl; c0 += (uint32_t)P.cull_chunk) {
             if (tid == 0) { s_work_n = 0; s_work_next = 0; }
             __syncthreads();
-            const uint32_t c1 = min(c0 + (uint32_t)P.cull_chunk, n_cl);
-            for (uint32_t g0 = c0 + warp * 32; g0 < c1; g0 += NT) {
-                const uint32_t g = g0 + lane;
-                uint32_t nb = 0, boff = 0, s = 0;
-                if (g < c1) {
-                    int lo = 0, hi = K;
-                    while (lo < hi) {   // largest slot whose first cluster index is <= g
-                        const int mid = (lo + hi + 1) >> 1;
-                        if (es.cl_base[mid] <= g) lo = mid; else hi = mid - 1;
-                    }
-                    s = (uint32_t)lo;
-                    const GxClusterDev c = P.clusters[es.slot_cl[s] + (g - es.cl_base[s])];
-                    const bool vis = !P.cull || cluster_visible(c, es.MV + s * 12, P.fx, P.fy, P.znear, P.zfar);
-                    if (STATS) { ++st_tested; st_drawn += vis ? 1u : 0u; }
-                    if (vis) { nb = c.nbatch; boff = c.batch_off; }
-                }
-                uint32_t inc = nb;   // warp-aggregated append: one shared atomic per warp
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, inc, d);
-                    if (lane >= d) inc += a;
-                }
-                const uint32_t tot = __shfl_sync(0xFFFFFFFFu, inc, 31);
-                uint32_t base = 0;
-                if (lane == 0 && tot) base = atomicAdd(&s_work_n, tot);
-                base = __shfl_sync(0xFFFFFFFFu, base, 0) + inc - nb;
-                for (uint32_t k = 0; k < nb; ++k) es.work[base + k] = (s << 24) | (boff + k);
-            }
+            cull_chunk_to_worklist<STATS>(P, es, c0, min(c0 + (uint32_t)P.cull_chunk, n_cl), tid, NT, &s_work_n, st_tested, st_drawn);
             __syncthreads();
             const unsigned n_work = s_work_n;
             for (;;) {

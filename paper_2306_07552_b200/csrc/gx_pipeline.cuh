@@ -1,0 +1,783 @@
+// gx_pipeline.cuh -- the two-kernel render path (sm_100a): geometry kernel -> triangle-record stream -> raster
+// kernel.  DESIGN.md section 5.
+//
+//   geom_kernel   K1 cull + K2 vertex transform / clip / snap / set-up.  No frame in shared memory, so four
+//                 8-warp CTAs fit an SM at 64 registers per thread; every triangle that survives the exact
+//                 pixel-centre bounding-box test leaves as one 64-byte record in the environment's segment
+//                 of the record pool (HBM/L2).
+//   raster_kernel K3 + K4 + K5.  One persistent CTA per SM owns one environment's whole frame of 64-bit
+//                 (depth, record index) keys in shared memory; warps draw groups of 32 records, cut their
+//                 bounding boxes into 4-pixel slots dealt evenly to the lanes, queue the covered pixels and
+//                 shade them densely; the winner's colour is resolved from its record and RGB / depth leave
+//                 as 16-byte stores.
+//
+// An environment whose records do not fit its pool segment is flagged by the geometry kernel, skipped by the
+// raster kernel and rendered by the single-kernel path of gx_kernels.cuh (render_kernel), which needs no
+// pool.  Arithmetic follows DESIGN.md section 3 (N1-N9) operation by operation.
+#pragma once
+#include "gx_kernels.cuh"
+
+namespace gx {
+
+// ------------------------------------------------------------------------------------------------
+// record layout: 16 words = 64 bytes, one uint4 x 4
+// ------------------------------------------------------------------------------------------------
+// narrow record (bounding-box extent < NARROW_EXT sub-pixel units: every edge value fits int32):
+//   w0..2  E_e at the bounding-box origin pixel (i0, j0), e = 0, 1, 2
+//   w3..5  dx_e << 16 | (dy_e & 0xFFFF)
+//   w6     i0 | j0 << 7 | (w-1) << 14 | (h-1) << 21 | bias bits << 28 | float-colour flag << 31
+//   w7     id << 1 | sub
+//   w8..10 q = 1/w of vertices 0, 1, 2 (orientation-normalised)
+//   w11..13 RGBA8 of vertices 0, 1, 2 (unused if the float-colour flag is set)
+// colour slot (follows a narrow record with the flag set, and every wide record):
+//   w0..2 = -1, w3..6 = 0  (as a narrow record it covers nothing)   w7..15 = c[vertex][channel] as float
+// wide record (always followed by a colour slot):
+//   w0..2 X, w3..5 Y (snapped, orientation-normalised), w7 id2, w8..10 q
+enum { P_E0 = 0, P_D0 = 3, P_BB = 6, P_ID = 7, P_Q0 = 8, P_C0 = 11 };
+constexpr uint32_t BB_FLOATCOL = 0x80000000u;
+
+struct PipeParams {
+    GxParams g;              // N = environments of this chunk; per-call arrays already offset to the chunk
+    uint4 *recs;             // [N][cap_n + cap_w][4]
+    uint32_t *cnt;           // [N][2]: narrow slots, wide slots appended
+    uint32_t *env_flag;      // [N]: 1 = pool segment overflowed, render with the single-kernel path
+    unsigned int *counters;  // [0] geometry work-unit counter, [1] raster env counter
+    int32_t cap_n, cap_w;    // slots per environment
+    int32_t split;           // geometry work units per environment (each takes 1/split of the cluster space)
+};
+
+struct GeomWarpSmem {
+    int2 *vXY;            // [GX_VCAP]
+    float *vQ;            // [GX_VCAP]
+    uint32_t *vC;         // [GX_VCAP] RGBA8
+    unsigned char *lst;   // [256]
+};
+constexpr int GEOM_WARP_SMEM = GX_VCAP * 16 + 256;
+
+__host__ __device__ inline size_t geom_smem_bytes(int K, int warps) {
+    size_t b = (size_t)warps * GEOM_WARP_SMEM + env_smem_bytes(K);
+    return (b + 15) & ~(size_t)15;
+}
+
+// N6 set-up of a narrow triangle: orientation normalisation, edge values at the bounding-box origin, packed
+// deltas and the BB word.  Returns false for zero area.  `swapped` tells the caller to swap attributes 1, 2.
+__device__ __forceinline__ bool narrow_setup(int X[3], int Y[3], float q[3], int i0, int i1, int j0, int j1,
+                                             uint32_t E0[3], uint32_t D[3], uint32_t &bb, bool &swapped) {
+    int A = (X[1] - X[0]) * (Y[2] - Y[0]) - (Y[1] - Y[0]) * (X[2] - X[0]);   // < 2^31: narrow
+    swapped = A < 0;
+    if (A == 0) return false;
+    if (swapped) {
+        int ti = X[1]; X[1] = X[2]; X[2] = ti;
+        ti = Y[1]; Y[1] = Y[2]; Y[2] = ti;
+        const float tf = q[1]; q[1] = q[2]; q[2] = tf;
+    }
+    const int px0 = (i0 << 8) + 128, py0 = (j0 << 8) + 128;
+    uint32_t bias_bits = 0;
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+        const int va = (e + 1) % 3, vb = (e + 2) % 3;
+        const int dx = X[vb] - X[va], dy = Y[vb] - Y[va];
+        const bool tl = (dy < 0) || (dy == 0 && dx > 0);
+        E0[e] = (uint32_t)(dx * (py0 - Y[va]) - dy * (px0 - X[va]));
+        D[e] = ((uint32_t)dx << 16) | ((uint32_t)dy & 0xFFFFu);
+        bias_bits |= (tl ? 0u : 1u) << e;
+    }
+    bb = (uint32_t)i0 | ((uint32_t)j0 << 7) | ((uint32_t)(i1 - i0) << 14) | ((uint32_t)(j1 - j0) << 21) | (bias_bits << 28);
+    return true;
+}
+
+__device__ __forceinline__ void store_colour_slot(uint4 *dst, const float c[3][3], uint32_t id2) {
+    dst[0] = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0u);
+    dst[1] = make_uint4(0u, 0u, 0u, __float_as_uint(c[0][0]));
+    dst[2] = make_uint4(__float_as_uint(c[0][1]), __float_as_uint(c[0][2]), __float_as_uint(c[1][0]), __float_as_uint(c[1][1]));
+    dst[3] = make_uint4(__float_as_uint(c[1][2]), __float_as_uint(c[2][0]), __float_as_uint(c[2][1]), __float_as_uint(c[2][2]));
+    (void)id2;
+}
+
+// ------------------------------------------------------------------------------------------------
+// geometry: K2 for one batch, by one warp
+// ------------------------------------------------------------------------------------------------
+template <bool STATS>
+__device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj, uint32_t item, const EnvSmem &es,
+                                           const GeomWarpSmem &ws, int env, int lane, bool &overflow, unsigned &n_in,
+                                           unsigned &n_tri) {
+    const GxParams &P = PP.g;
+    const unsigned FULL = 0xFFFFFFFFu;
+    const uint32_t s = item >> 24;
+    const GxBatchDev b = P.batches[item & 0xFFFFFFu];
+    const int nv = (int)(b.nv_nt & 0xFFFFu), nt = (int)(b.nv_nt >> 16);
+    float M[12];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) M[k] = es.MV[s * 12 + k];
+    const uint32_t idb = es.id_base[s] + b.first_tri;
+    const float4 *__restrict__ verts = P.verts + b.vert_off;
+    const uchar4 *__restrict__ tris = P.tris + b.tri_off;
+    const unsigned lt = (1u << lane) - 1u;
+    uint4 *env_recs = PP.recs + (size_t)env * (size_t)(PP.cap_n + PP.cap_w) * 4;
+    if (STATS) n_in += (lane == 0) ? (unsigned)nt : 0u;
+
+    // K2a: vertex transform, projection, snap -> warp-private staging
+    for (int v = lane; v < nv; v += 32) {
+        const float4 p = __ldg(&verts[v]);
+        const CamVert cv = xform(M, p.x, p.y, p.z);
+        int X = X_OUT, Y = 0;
+        float q = 0.0f;
+        if (cv.w >= P.znear) project(pj, cv.xc, cv.yc, cv.w, X, Y, q);
+        ws.vXY[v] = make_int2(X, Y);
+        ws.vQ[v] = q;
+        ws.vC[v] = __float_as_uint(p.w);
+    }
+    __syncwarp();
+
+    // K2b: near classification and pixel-centre bounding-box reject; compact narrow survivors to the front
+    // of lst and slow-path triangles (wide, or straddling the near plane) to the back
+    int nsurv = 0, nslow = 0;
+    for (int t0 = 0; t0 < nt; t0 += 32) {
+        const int t = t0 + lane;
+        bool ok = false, slow = false;
+        if (t < nt) {
+            const uchar4 ix = __ldg(&tris[t]);
+            const int2 a = ws.vXY[ix.x], bb = ws.vXY[ix.y], c = ws.vXY[ix.z];
+            const int nout = (int)(a.x == X_OUT) + (int)(bb.x == X_OUT) + (int)(c.x == X_OUT);
+            if (nout == 0) {
+                const int Xmin = min(a.x, min(bb.x, c.x)), Xmax = max(a.x, max(bb.x, c.x));
+                const int Ymin = min(a.y, min(bb.y, c.y)), Ymax = max(a.y, max(bb.y, c.y));
+                const int i0 = max((Xmin + 127) >> 8, 0), i1 = min((Xmax - 128) >> 8, P.W - 1);
+                const int j0 = max((Ymin + 127) >> 8, 0), j1 = min((Ymax - 128) >> 8, P.H - 1);
+                if (i0 <= i1 && j0 <= j1) {
+                    ok = max(Xmax - Xmin, Ymax - Ymin) < NARROW_EXT;
+                    slow = !ok;
+                }
+            } else if (nout < 3) {
+                slow = true;
+            }
+        }
+        const unsigned mo = __ballot_sync(FULL, ok), mc = __ballot_sync(FULL, slow);
+        if (ok) ws.lst[nsurv + __popc(mo & lt)] = (unsigned char)t;
+        if (slow) ws.lst[255 - (nslow + __popc(mc & lt))] = (unsigned char)t;
+        nsurv += __popc(mo);
+        nslow += __popc(mc);
+    }
+    __syncwarp();
+
+    // K2c: set-up of the narrow survivors, one record each, written straight to the environment's segment
+    if (nsurv) {
+        uint32_t base = 0;
+        if (lane == 0) base = atomicAdd(&PP.cnt[2 * env], (uint32_t)nsurv);
+        base = __shfl_sync(FULL, base, 0);
+        if (base + (uint32_t)nsurv > (uint32_t)PP.cap_n) {
+            overflow = true;
+        } else {
+            for (int g = lane; g < nsurv; g += 32) {
+                const int t = ws.lst[g];
+                const uchar4 ix = __ldg(&tris[t]);
+                const int2 a = ws.vXY[ix.x], bq = ws.vXY[ix.y], c = ws.vXY[ix.z];
+                int X[3] = {a.x, bq.x, c.x}, Y[3] = {a.y, bq.y, c.y};
+                float q[3] = {ws.vQ[ix.x], ws.vQ[ix.y], ws.vQ[ix.z]};
+                uint32_t col[3] = {ws.vC[ix.x], ws.vC[ix.y], ws.vC[ix.z]};
+                int i0, i1, j0, j1;
+                pixel_bbox(X, Y, P.W, P.H, i0, i1, j0, j1);
+                uint32_t E0[3], D[3], bbw;
+                bool swapped;
+                const bool good = narrow_setup(X, Y, q, i0, i1, j0, j1, E0, D, bbw, swapped);
+                if (swapped) { const uint32_t tc = col[1]; col[1] = col[2]; col[2] = tc; }
+                if (!good) { E0[0] = E0[1] = E0[2] = 0xFFFFFFFFu; D[0] = D[1] = D[2] = 0u; bbw = 0u; }   // covers nothing
+                if (STATS) n_tri += good ? 1u : 0u;
+                uint4 *dst = env_recs + (size_t)(base + (uint32_t)g) * 4;
+                dst[0] = make_uint4(E0[0], E0[1], E0[2], D[0]);
+                dst[1] = make_uint4(D[1], D[2], bbw, (idb + (uint32_t)t) << 1);
+                dst[2] = make_uint4(__float_as_uint(q[0]), __float_as_uint(q[1]), __float_as_uint(q[2]), col[0]);
+                dst[3] = make_uint4(col[1], col[2], 0u, 0u);
+            }
+        }
+    }
+
+    // slow path: wide triangles and near-plane straddlers (N4), piece by piece
+    for (int g = 0; g < nslow; g += 32) {
+        const bool have = g + lane < nslow;
+        CamVert cv[3];
+        float c[3][3];
+        int t = 0;
+        if (have) {
+            t = ws.lst[255 - (g + lane)];
+            const uchar4 ix = __ldg(&tris[t]);
+            const float4 p0 = __ldg(&verts[ix.x]), p1 = __ldg(&verts[ix.y]), p2 = __ldg(&verts[ix.z]);
+            cv[0] = xform(M, p0.x, p0.y, p0.z);
+            cv[1] = xform(M, p1.x, p1.y, p1.z);
+            cv[2] = xform(M, p2.x, p2.y, p2.z);
+            const uint32_t r0 = __float_as_uint(p0.w), r1 = __float_as_uint(p1.w), r2 = __float_as_uint(p2.w);
+#pragma unroll
+            for (int ch = 0; ch < 3; ++ch) {
+                c[0][ch] = (float)((r0 >> (8 * ch)) & 0xFFu);
+                c[1][ch] = (float)((r1 >> (8 * ch)) & 0xFFu);
+                c[2][ch] = (float)((r2 >> (8 * ch)) & 0xFFu);
+            }
+        }
+#pragma unroll 1
+        for (int sub = 0; sub < 2; ++sub) {
+            Tri tri;
+            float oc[3][3];
+            bool narrow = false, wide = false;
+            int i0 = 0, i1 = 0, j0 = 0, j1 = 0;
+            if (have) {
+                CamVert o[3];
+                const int np = clip_near<true>(cv, c, P.znear, sub, o, oc);
+                if (sub < np) {
+#pragma unroll
+                    for (int k = 0; k < 3; ++k) project(pj, o[k].xc, o[k].yc, o[k].w, tri.X[k], tri.Y[k], tri.q[k]);
+                    tri.id2 = ((idb + (uint32_t)t) << 1) | (unsigned)sub;
+                    if (pixel_bbox(tri.X, tri.Y, P.W, P.H, i0, i1, j0, j1)) {
+                        const long long A = area2(tri);
+                        if (A != 0) {
+                            const int ext = max(max(tri.X[0], max(tri.X[1], tri.X[2])) - min(tri.X[0], min(tri.X[1], tri.X[2])),
+                                                max(tri.Y[0], max(tri.Y[1], tri.Y[2])) - min(tri.Y[0], min(tri.Y[1], tri.Y[2])));
+                            narrow = ext < NARROW_EXT;
+                            wide = !narrow;
+                            if (A < 0) {
+                                swap12(tri);
+#pragma unroll
+                                for (int ch = 0; ch < 3; ++ch) { const float f = oc[1][ch]; oc[1][ch] = oc[2][ch]; oc[2][ch] = f; }
+                            }
+                        }
+                    }
+                }
+            }
+            const unsigned mn = __ballot_sync(FULL, narrow), mw = __ballot_sync(FULL, wide);
+            if ((mn | mw) == 0u) continue;
+            uint32_t bn = 0, bw = 0;
+            if (lane == 0) {
+                if (mn) bn = atomicAdd(&PP.cnt[2 * env], 2u * (uint32_t)__popc(mn));
+                if (mw) bw = atomicAdd(&PP.cnt[2 * env + 1], 2u * (uint32_t)__popc(mw));
+            }
+            bn = __shfl_sync(FULL, bn, 0);
+            bw = __shfl_sync(FULL, bw, 0);
+            if (bn + 2u * (uint32_t)__popc(mn) > (uint32_t)PP.cap_n || bw + 2u * (uint32_t)__popc(mw) > (uint32_t)PP.cap_w) {
+                overflow = true;
+                continue;
+            }
+            if (STATS) n_tri += (narrow || wide) ? 1u : 0u;
+            if (narrow) {
+                uint32_t E0[3], D[3], bbw;
+                bool swapped;
+                narrow_setup(tri.X, tri.Y, tri.q, i0, i1, j0, j1, E0, D, bbw, swapped);   // already normalised: no swap
+                uint4 *dst = env_recs + (size_t)(bn + 2u * (uint32_t)__popc(mn & lt)) * 4;
+                dst[0] = make_uint4(E0[0], E0[1], E0[2], D[0]);
+                dst[1] = make_uint4(D[1], D[2], bbw | BB_FLOATCOL, tri.id2);
+                dst[2] = make_uint4(__float_as_uint(tri.q[0]), __float_as_uint(tri.q[1]), __float_as_uint(tri.q[2]), 0u);
+                dst[3] = make_uint4(0u, 0u, 0u, 0u);
+                store_colour_slot(dst + 4, oc, tri.id2);
+            }
+            if (wide) {
+                uint4 *dst = env_recs + ((size_t)PP.cap_n + bw + 2u * (uint32_t)__popc(mw & lt)) * 4;
+                dst[0] = make_uint4((uint32_t)tri.X[0], (uint32_t)tri.X[1], (uint32_t)tri.X[2], (uint32_t)tri.Y[0]);
+                dst[1] = make_uint4((uint32_t)tri.Y[1], (uint32_t)tri.Y[2], 0u, tri.id2);
+                dst[2] = make_uint4(__float_as_uint(tri.q[0]), __float_as_uint(tri.q[1]), __float_as_uint(tri.q[2]), 0u);
+                dst[3] = make_uint4(0u, 0u, 0u, 0u);
+                store_colour_slot(dst + 4, oc, tri.id2);
+            }
+        }
+    }
+    __syncwarp();
+}
+
+}  // namespace gx
+
+namespace gx {
+
+// ------------------------------------------------------------------------------------------------
+// the geometry kernel
+// ------------------------------------------------------------------------------------------------
+template <int WARPS, bool STATS>
+__global__ void __launch_bounds__(WARPS * 32, 1024 / (WARPS * 32)) geom_kernel(const PipeParams PP) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const GxParams &P = PP.g;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int NT = WARPS * 32;
+    const int K = P.K;
+
+    GeomWarpSmem ws;
+    {
+        unsigned char *w = smem + (size_t)warp * GEOM_WARP_SMEM;
+        ws.vXY = reinterpret_cast<int2 *>(w);
+        ws.vQ = reinterpret_cast<float *>(w + GX_VCAP * 8);
+        ws.vC = reinterpret_cast<uint32_t *>(w + GX_VCAP * 12);
+        ws.lst = w + GX_VCAP * 16;
+    }
+    unsigned char *p = smem + (size_t)WARPS * GEOM_WARP_SMEM;
+    EnvSmem es;
+    es.MV = reinterpret_cast<float *>(p);          p += (size_t)(K + 1) * 48;
+    es.id_base = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 2) * 4;
+    es.cl_base = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 2) * 4;
+    es.slot_cl = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
+    es.slot_mesh = reinterpret_cast<int32_t *>(p); p += (size_t)(K + 1) * 4;
+    es.slot_nt = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
+    es.slot_nc = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
+    es.work = reinterpret_cast<uint32_t *>(p);
+
+    __shared__ int s_env;
+    __shared__ unsigned s_work_n, s_work_next;
+    __shared__ unsigned long long s_stat[GX_NSTAT];
+
+    Proj pj;
+    pj.fx = P.fx; pj.fy = P.fy;
+    pj.hw = 128.0f * (float)P.W; pj.hh = 128.0f * (float)P.H;
+
+    unsigned st_tested = 0, st_drawn = 0, st_in = 0, st_tri = 0;
+    if (STATS) {
+        if (tid < GX_NSTAT) s_stat[tid] = 0;
+    }
+
+    for (;;) {
+        if (tid == 0) s_env = (int)atomicAdd(&PP.counters[0], 1u);
+        __syncthreads();
+        const int unit = s_env;
+        if (unit >= P.N * PP.split) break;
+        const int env = unit / PP.split, part = unit - env * PP.split;
+        env_setup(P, env, es, tid);
+
+        const uint32_t n_all = es.cl_base[K + 1];
+        const uint32_t c_lo = (uint32_t)(((unsigned long long)n_all * (unsigned)part) / (unsigned)PP.split);
+        const uint32_t n_cl = (uint32_t)(((unsigned long long)n_all * (unsigned)(part + 1)) / (unsigned)PP.split);
+        bool overflow = false;
+        for (uint32_t c0 = c_lo; c0 < n_cl; c0 += (uint32_t)P.cull_chunk) {
+            if (tid == 0) { s_work_n = 0; s_work_next = 0; }
+            __syncthreads();
+            cull_chunk_to_worklist<STATS>(P, es, c0, min(c0 + (uint32_t)P.cull_chunk, n_cl), tid, NT, &s_work_n, st_tested, st_drawn);
+            __syncthreads();
+            const unsigned n_work = s_work_n;
+            for (;;) {
+                unsigned wi = 0;
+                if (lane == 0) wi = atomicAdd(&s_work_next, 1u);
+                wi = __shfl_sync(0xFFFFFFFFu, wi, 0);
+                if (wi >= n_work) break;
+                geom_batch<STATS>(PP, pj, es.work[wi], es, ws, env, lane, overflow, st_in, st_tri);
+            }
+            __syncthreads();
+        }
+        if (overflow && lane == 0 && atomicExch(&PP.env_flag[env], 1u) == 0u)
+            atomicAdd(&P.stats[GX_STAT_OVERFLOW_ENVS], 1ull);
+        __syncthreads();
+    }
+
+    if (STATS) {
+        atomicAdd(&s_stat[GX_STAT_CLUSTERS_TESTED], (unsigned long long)st_tested);
+        atomicAdd(&s_stat[GX_STAT_CLUSTERS_DRAWN], (unsigned long long)st_drawn);
+        atomicAdd(&s_stat[GX_STAT_TRIS_IN], (unsigned long long)st_in);
+        atomicAdd(&s_stat[GX_STAT_TRIS_RASTER], (unsigned long long)st_tri);
+        __syncthreads();
+        if (tid < GX_NSTAT) atomicAdd(&P.stats[tid], s_stat[tid]);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// raster side
+// ------------------------------------------------------------------------------------------------
+struct RastWarpSmem {
+    uint32_t *rec;   // [REC_WORDS * 32] SoA records of the current group (layout of gx_kernels.cuh R_*)
+    uint32_t *fq;    // [FQ_CAP] covered fragments: r | (x - i0) << 5 | (y - j0) << 12
+};
+constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4;
+
+__host__ __device__ inline size_t raster_smem_bytes(int W, int H, int warps) {
+    return (size_t)W * H * 8 + (size_t)warps * RAST_WARP_SMEM;
+}
+
+// N9 with the frame key (depth bits << 32 | slot index): smaller depth wins; at exactly equal depth the
+// smaller (id << 1 | sub) wins, read from the stored slot's record (rare).  The final frame holds, per pixel,
+// the slot of the lexicographically smallest (depth, id, sub) whatever the order of arrival.
+__device__ __forceinline__ void key_min_rec(unsigned long long *slot, uint32_t dbits, uint32_t idx, uint32_t id2,
+                                            const uint4 *env_recs) {
+    const unsigned long long key = ((unsigned long long)dbits << 32) | idx;
+    unsigned long long cur = *reinterpret_cast<volatile unsigned long long *>(slot);
+    for (;;) {
+        const uint32_t cd = (uint32_t)(cur >> 32);
+        if (dbits > cd) return;
+        if (dbits == cd) {
+            const uint32_t cid2 = __ldg(reinterpret_cast<const uint32_t *>(env_recs + (size_t)(uint32_t)cur * 4) + P_ID);
+            if (id2 >= cid2) return;
+        }
+        const unsigned long long old = atomicCAS(slot, cur, key);
+        if (old == cur) return;
+        cur = old;
+    }
+}
+
+// load the group's records (one per lane) into the warp's SoA staging
+__device__ __forceinline__ void load_group(const RastWarpSmem &ws, const uint4 *env_recs, uint32_t first, int nrec, int lane) {
+    if (lane < nrec) {
+        const uint4 *rp = env_recs + (size_t)(first + (uint32_t)lane) * 4;
+        const uint4 u0 = __ldg(rp), u1 = __ldg(rp + 1), u2 = __ldg(rp + 2);
+        ws.rec[(R_E0 + 0) * 32 + lane] = u0.x;
+        ws.rec[(R_E0 + 1) * 32 + lane] = u0.y;
+        ws.rec[(R_E0 + 2) * 32 + lane] = u0.z;
+        ws.rec[(R_D0 + 0) * 32 + lane] = u0.w;
+        ws.rec[(R_D0 + 1) * 32 + lane] = u1.x;
+        ws.rec[(R_D0 + 2) * 32 + lane] = u1.y;
+        ws.rec[R_BB * 32 + lane] = u1.z;
+        ws.rec[R_ID * 32 + lane] = u1.w;
+        ws.rec[(R_Q0 + 0) * 32 + lane] = u2.x;
+        ws.rec[(R_Q0 + 1) * 32 + lane] = u2.y;
+        ws.rec[(R_Q0 + 2) * 32 + lane] = u2.z;
+        ws.rec[R_FA * 32 + lane] = __float_as_uint((float)(int)(u0.x + u0.y + u0.z));   // E_0 + E_1 + E_2 = A
+    }
+    __syncwarp();
+}
+
+// K4b: depth (N7) and resolve (N9) for the queued fragments, one per lane
+__device__ __forceinline__ void shade_queue_p(const RastWarpSmem &ws, int qn, int W, float zfar, unsigned long long *fb,
+                                              uint32_t first, const uint4 *env_recs, int lane) {
+    for (int f = lane; f < qn; f += 32) {
+        const uint32_t en = ws.fq[f];
+        const int r = (int)(en & 31u), a = (int)((en >> 5) & 127u), b = (int)((en >> 12) & 127u);
+        const uint32_t bb = ws.rec[R_BB * 32 + r];
+        float fe[3], q[3];
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            const uint32_t d = ws.rec[(R_D0 + e) * 32 + r];
+            const int dx = (int)d >> 16, dy = (int)(short)(d & 0xFFFFu);
+            const int Ee = (int)ws.rec[(R_E0 + e) * 32 + r] + ((b * dx - a * dy) << 8);
+            fe[e] = (float)Ee;
+            q[e] = __uint_as_float(ws.rec[(R_Q0 + e) * 32 + r]);
+        }
+        const float num = fmaf(fe[2], q[2], fmaf(fe[1], q[1], fe[0] * q[0]));
+        const float depth = __uint_as_float(ws.rec[R_FA * 32 + r]) / num;
+        if (depth > zfar) continue;
+        const int x = (int)(bb & 127u) + a, y = (int)((bb >> 7) & 127u) + b;
+        key_min_rec(&fb[fb_index(x, y, W)], __float_as_uint(depth), first + (uint32_t)r, ws.rec[R_ID * 32 + r], env_recs);
+    }
+    __syncwarp();
+}
+
+// K3 + K4a: coverage of the nrec records of the warp's group (see raster_group in gx_kernels.cuh for the
+// slot scheme).  The covered pixels of one pass are appended to the fragment queue with four ballots.
+template <bool STATS>
+__device__ __forceinline__ void raster_group_p(const RastWarpSmem &ws, int nrec, int W, float zfar, unsigned long long *fb,
+                                               uint32_t first, const uint4 *env_recs, int lane, unsigned &n_frag) {
+    const unsigned FULL = 0xFFFFFFFFu;
+    const unsigned lt = (1u << lane) - 1u;
+    int ns = 0;
+    if (lane < nrec) {
+        const uint32_t bb = ws.rec[R_BB * 32 + lane];
+        const int w = (int)((bb >> 14) & 127u) + 1, h = (int)((bb >> 21) & 127u) + 1;
+        ns = h * ((w + 3) >> 2);
+    }
+    int inc = ns;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const int v = __shfl_up_sync(FULL, inc, d);
+        if (lane >= d) inc += v;
+    }
+    const int T = __shfl_sync(FULL, inc, 31);
+    const int Pex = inc - ns;
+    const int per = (T + 31) >> 5;
+    const int s0 = lane * per;
+    const int n = min(per, T - s0);
+    int r = 0;   // largest record index with Pex[r] <= s0
+#pragma unroll
+    for (int step = 16; step; step >>= 1) {
+        const int cand = r + step;
+        const int pc = __shfl_sync(FULL, Pex, cand);
+        if (pc <= s0) r = cand;
+    }
+    const int off = s0 - __shfl_sync(FULL, Pex, r);
+
+    int E0[3], dx[3], dy[3], w = 1, h = 1, cw = 1;
+    auto load_rec = [&](int rr) {   // E0 := E_e - bias_e at the origin pixel, so that "covered" is all E0 >= 0
+        const uint32_t bb = ws.rec[R_BB * 32 + rr];
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            E0[e] = (int)ws.rec[(R_E0 + e) * 32 + rr] - (int)((bb >> (28 + e)) & 1u);
+            const uint32_t d = ws.rec[(R_D0 + e) * 32 + rr];
+            dx[e] = (int)d >> 16;
+            dy[e] = (int)(short)(d & 0xFFFFu);
+        }
+        w = (int)((bb >> 14) & 127u) + 1;
+        h = (int)((bb >> 21) & 127u) + 1;
+        cw = (w + 3) >> 2;
+    };
+    load_rec(r & 31);
+    int row = off / cw, chunk = off - row * cw;
+    int qn = 0;
+    const uint32_t fq_addr = (uint32_t)__cvta_generic_to_shared(ws.fq);
+    for (int it = 0; it < per; ++it) {
+        const bool act = it < n;
+        const int a = chunk << 2;
+        unsigned m4 = 0;
+        if (act) {
+            int Ee[3], sx[3];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) {
+                Ee[e] = E0[e] + ((row * dx[e] - a * dy[e]) << 8);
+                sx[e] = -(dy[e] << 8);
+            }
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const bool c = ((Ee[0] | Ee[1] | Ee[2]) >= 0) && (a + k < w);
+                m4 |= (c ? 1u : 0u) << k;
+                Ee[0] += sx[0]; Ee[1] += sx[1]; Ee[2] += sx[2];
+            }
+        }
+        // append the covered pixels: four independent ballots, predicated stores
+        const unsigned b0 = __ballot_sync(FULL, m4 & 1u), b1 = __ballot_sync(FULL, m4 & 2u),
+                       b2 = __ballot_sync(FULL, m4 & 4u), b3 = __ballot_sync(FULL, m4 & 8u);
+        if (b0 | b1 | b2 | b3) {
+            const uint32_t en = (uint32_t)r | ((uint32_t)a << 5) | ((uint32_t)row << 12);
+            const int p0 = qn + __popc(b0 & lt);
+            const int c1 = qn + __popc(b0), p1 = c1 + __popc(b1 & lt);
+            const int c2 = c1 + __popc(b1), p2 = c2 + __popc(b2 & lt);
+            const int c3 = c2 + __popc(b2), p3 = c3 + __popc(b3 & lt);
+            sts_if(fq_addr + (uint32_t)p0 * 4u, en, m4 & 1u);
+            sts_if(fq_addr + (uint32_t)p1 * 4u, en + 32u, m4 & 2u);
+            sts_if(fq_addr + (uint32_t)p2 * 4u, en + 64u, m4 & 4u);
+            sts_if(fq_addr + (uint32_t)p3 * 4u, en + 96u, m4 & 8u);
+            qn = c3 + __popc(b3);
+        }
+        if (act) {
+            if (++chunk == cw) {
+                chunk = 0;
+                if (++row == h) {
+                    row = 0;
+                    ++r;
+                    if (it + 1 < n) load_rec(r);
+                }
+            }
+        }
+        if (qn > FQ_CAP - 128) {
+            __syncwarp();
+            if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
+            shade_queue_p(ws, qn, W, zfar, fb, first, env_recs, lane);
+            qn = 0;
+        }
+    }
+    __syncwarp();
+    if (qn) {
+        if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
+        shade_queue_p(ws, qn, W, zfar, fb, first, env_recs, lane);
+    }
+}
+
+// wide records: one triangle at a time, the whole warp walks its bounding box in 8x4-pixel blocks with the
+// int64 edge functions of N6
+template <bool STATS>
+__device__ __forceinline__ void raster_wide(const uint4 *env_recs, uint32_t slot0, int ntri, int W, int H, float zfar,
+                                            unsigned long long *fb, int lane, unsigned &n_frag) {
+    const unsigned FULL = 0xFFFFFFFFu;
+    Tri tri;
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { tri.X[k] = 0; tri.Y[k] = 0; tri.q[k] = 0.0f; }
+    tri.id2 = 0;
+    if (lane < ntri) {
+        const uint4 *rp = env_recs + (size_t)(slot0 + 2u * (uint32_t)lane) * 4;
+        const uint4 u0 = __ldg(rp), u1 = __ldg(rp + 1), u2 = __ldg(rp + 2);
+        tri.X[0] = (int)u0.x; tri.X[1] = (int)u0.y; tri.X[2] = (int)u0.z;
+        tri.Y[0] = (int)u0.w; tri.Y[1] = (int)u1.x; tri.Y[2] = (int)u1.y;
+        tri.id2 = u1.w;
+        tri.q[0] = __uint_as_float(u2.x); tri.q[1] = __uint_as_float(u2.y); tri.q[2] = __uint_as_float(u2.z);
+    }
+    for (int src = 0; src < ntri; ++src) {
+        Tri bt;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            bt.X[k] = __shfl_sync(FULL, tri.X[k], src);
+            bt.Y[k] = __shfl_sync(FULL, tri.Y[k], src);
+            bt.q[k] = __shfl_sync(FULL, tri.q[k], src);
+        }
+        bt.id2 = __shfl_sync(FULL, tri.id2, src);
+        int bi0, bi1, bj0, bj1;
+        pixel_bbox(bt.X, bt.Y, W, H, bi0, bi1, bj0, bj1);
+        Edges BE;
+        edge_setup(bt, area2(bt), BE);   // orientation-normalised by the geometry kernel: area > 0
+        const int lx = lane & 7, ly = lane >> 3;
+        const uint32_t idx = slot0 + 2u * (uint32_t)src;
+        for (int by = bj0 >> 2; by <= (bj1 >> 2); ++by)
+            for (int bx = bi0 >> 3; bx <= (bi1 >> 3); ++bx) {
+                const int i = bx * 8 + lx, j = by * 4 + ly;
+                float f[3], num, depth;
+                if (!cover_depth(BE, bt.q, i, j, f, num, depth)) continue;
+                if (STATS) ++n_frag;
+                if (depth > zfar) continue;
+                key_min_rec(&fb[fb_index(i, j, W)], __float_as_uint(depth), idx, bt.id2, env_recs);
+            }
+    }
+    __syncwarp();
+}
+
+// K5a: colour (N8) and id of the winning record at pixel (x, y)
+__device__ __forceinline__ uint32_t resolve_rec(const uint4 *env_recs, uint32_t cap_n, uint32_t idx, int x, int y,
+                                                bool want_rgb, uint32_t &id) {
+    const uint4 *rp = env_recs + (size_t)idx * 4;
+    const uint4 u1 = __ldg(rp + 1);
+    id = u1.w >> 1;
+    if (!want_rgb) return 0u;
+    const uint4 u0 = __ldg(rp), u2 = __ldg(rp + 2);
+    const float q[3] = {__uint_as_float(u2.x), __uint_as_float(u2.y), __uint_as_float(u2.z)};
+    float f[3], c[3][3];
+    bool fcol = true;
+    if (idx < cap_n) {
+        const uint32_t bb = u1.z;
+        const int a = x - (int)(bb & 127u), b = y - (int)((bb >> 7) & 127u);
+        const uint32_t D[3] = {u0.w, u1.x, u1.y};
+        const uint32_t E[3] = {u0.x, u0.y, u0.z};
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            const int dx = (int)D[e] >> 16, dy = (int)(short)(D[e] & 0xFFFFu);
+            f[e] = (float)((int)E[e] + ((b * dx - a * dy) << 8));
+        }
+        fcol = (bb & BB_FLOATCOL) != 0u;
+        if (!fcol) {
+            const uint4 u3 = __ldg(rp + 3);
+            const uint32_t col[3] = {u2.w, u3.x, u3.y};
+#pragma unroll
+            for (int v = 0; v < 3; ++v)
+#pragma unroll
+                for (int ch = 0; ch < 3; ++ch) c[v][ch] = (float)((col[v] >> (8 * ch)) & 0xFFu);
+        }
+    } else {
+        Tri t;
+        t.X[0] = (int)u0.x; t.X[1] = (int)u0.y; t.X[2] = (int)u0.z;
+        t.Y[0] = (int)u0.w; t.Y[1] = (int)u1.x; t.Y[2] = (int)u1.y;
+        t.q[0] = q[0]; t.q[1] = q[1]; t.q[2] = q[2];
+        Edges E;
+        edge_setup(t, area2(t), E);
+        float num, depth;
+        cover_depth(E, t.q, x, y, f, num, depth);   // covered by construction: this triangle won the pixel
+    }
+    if (fcol) {
+        const uint4 v1 = __ldg(rp + 5), v2 = __ldg(rp + 6), v3 = __ldg(rp + 7);
+        c[0][0] = __uint_as_float(v1.w); c[0][1] = __uint_as_float(v2.x); c[0][2] = __uint_as_float(v2.y);
+        c[1][0] = __uint_as_float(v2.z); c[1][1] = __uint_as_float(v2.w); c[1][2] = __uint_as_float(v3.x);
+        c[2][0] = __uint_as_float(v3.y); c[2][1] = __uint_as_float(v3.z); c[2][2] = __uint_as_float(v3.w);
+    }
+    const float num = fmaf(f[2], q[2], fmaf(f[1], q[1], f[0] * q[0]));
+    uint32_t out = 0;
+#pragma unroll
+    for (int ch = 0; ch < 3; ++ch) {
+        const float g0 = q[0] * c[0][ch], g1 = q[1] * c[1][ch], g2 = q[2] * c[2][ch];
+        const float cn = fmaf(f[2], g2, fmaf(f[1], g1, f[0] * g0));
+        const float v = cn / num;
+        out |= (uint32_t)fminf(255.0f, fmaxf(0.0f, rintf(v))) << (8 * ch);
+    }
+    return out;
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// the raster kernel
+// ------------------------------------------------------------------------------------------------
+template <int WARPS, int MINB, bool STATS>
+__global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipeParams PP) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const GxParams &P = PP.g;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int NT = WARPS * 32;
+    const int W = P.W, H = P.H, npix = W * H;
+
+    unsigned long long *fb = reinterpret_cast<unsigned long long *>(smem);
+    RastWarpSmem ws;
+    ws.rec = reinterpret_cast<uint32_t *>(smem + (size_t)npix * 8 + (size_t)warp * RAST_WARP_SMEM);
+    ws.fq = ws.rec + REC_WORDS * 32;
+
+    __shared__ int s_env;
+    __shared__ unsigned s_next;
+    __shared__ unsigned long long s_frag;
+
+    unsigned st_frag = 0;
+    if (STATS && tid == 0) s_frag = 0;
+    {
+        uint4 *f4 = reinterpret_cast<uint4 *>(fb);
+        const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+        for (int k = tid; k < npix / 2; k += NT) f4[k] = ones;
+    }
+    const bool want_rgb = P.rgb != nullptr;
+    const uint32_t cap_n = (uint32_t)PP.cap_n;
+
+    for (;;) {
+        if (tid == 0) { s_env = (int)atomicAdd(&PP.counters[1], 1u); s_next = 0; }
+        __syncthreads();
+        const int env = s_env;
+        if (env >= P.N) break;
+        if (PP.env_flag[env]) {   // overflowed its pool segment: left to the single-kernel pass
+            __syncthreads();
+            continue;
+        }
+        const uint4 *env_recs = PP.recs + (size_t)env * (size_t)(PP.cap_n + PP.cap_w) * 4;
+        const uint32_t n_n = PP.cnt[2 * env], n_w = PP.cnt[2 * env + 1] >> 1;
+        const uint32_t g_n = (n_n + 31u) >> 5, g_w = (n_w + 31u) >> 5;
+
+        // ---- K3 + K4: groups of 32 records, drawn dynamically by the warps ------------------------
+        for (;;) {
+            unsigned g = 0;
+            if (lane == 0) g = atomicAdd(&s_next, 1u);
+            g = __shfl_sync(0xFFFFFFFFu, g, 0);
+            if (g >= g_n + g_w) break;
+            if (g < g_n) {
+                const uint32_t first = g * 32u;
+                const int nrec = (int)min(32u, n_n - first);
+                load_group(ws, env_recs, first, nrec, lane);
+                raster_group_p<STATS>(ws, nrec, W, P.zfar, fb, first, env_recs, lane, st_frag);
+            } else {
+                const uint32_t t0 = (g - g_n) * 32u;
+                raster_wide<STATS>(env_recs, cap_n + 2u * t0, (int)min(32u, n_w - t0), W, H, P.zfar, fb, lane, st_frag);
+            }
+        }
+        __syncthreads();
+
+        // ---- K5: resolve the winners, write RGB / depth / id as 16-byte stores, reset the frame ------
+        for (int k = tid; k < npix / 4; k += NT) {
+            const int pix = k * 4;
+            const int j = pix / W, i = pix - j * W;
+            const int a = fb_index(i, j, W);          // 4-aligned columns stay contiguous under the XOR
+            uint4 *slot = reinterpret_cast<uint4 *>(&fb[a]);
+            const uint4 v0 = slot[0], v1 = slot[1];
+            const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+            slot[0] = ones;
+            slot[1] = ones;
+            const uint32_t idx[4] = {v0.x, v0.z, v1.x, v1.z};
+            const uint32_t db[4] = {v0.y, v0.w, v1.y, v1.w};
+            uint32_t col[4], id[4];
+            float4 d;
+            float *dp = &d.x;
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+                col[m] = 0u;
+                id[m] = 0xFFFFFFFFu;
+                dp[m] = 0.0f;
+                if (db[m] != 0xFFFFFFFFu) {
+                    dp[m] = __uint_as_float(db[m]);
+                    if (want_rgb || P.id) col[m] = resolve_rec(env_recs, cap_n, idx[m], i + m, j, want_rgb, id[m]);
+                }
+            }
+            *reinterpret_cast<float4 *>(P.depth + (size_t)env * npix + pix) = d;
+            if (P.id) *reinterpret_cast<uint4 *>(P.id + (size_t)env * npix + pix) = make_uint4(id[0], id[1], id[2], id[3]);
+            if (want_rgb) {
+                // 4 pixels = 12 bytes = 3 words per lane; 4 lanes hold 48 bytes = three 16-byte stores
+                const uint32_t w0 = (col[0] & 0xFFFFFFu) | (col[1] << 24);
+                const uint32_t w1 = ((col[1] >> 8) & 0xFFFFu) | (col[2] << 16);
+                const uint32_t w2 = ((col[2] >> 16) & 0xFFu) | (col[3] << 8);
+                const int g = lane & 3, gb = lane & ~3;
+                uint32_t o[4];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int m = 4 * g + r;          // word of the group's 12-word stream (g < 3)
+                    const int src = gb + (m / 3) % 4, wsel = m % 3;
+                    const uint32_t a0 = __shfl_sync(0xFFFFFFFFu, w0, src), a1 = __shfl_sync(0xFFFFFFFFu, w1, src),
+                                   a2 = __shfl_sync(0xFFFFFFFFu, w2, src);
+                    o[r] = wsel == 0 ? a0 : (wsel == 1 ? a1 : a2);
+                }
+                if (g < 3) {
+                    uint8_t *dst = P.rgb + ((size_t)env * npix + (size_t)(pix - 4 * g)) * 3 + 16 * g;
+                    *reinterpret_cast<uint4 *>(dst) = make_uint4(o[0], o[1], o[2], o[3]);
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    if (STATS) {
+        atomicAdd(&s_frag, (unsigned long long)st_frag);
+        __syncthreads();
+        if (tid == 0) atomicAdd(&P.stats[GX_STAT_FRAGMENTS], s_frag);
+    }
+}
+
+}  // namespace gx

@@ -54,9 +54,10 @@ struct GxParams {
     // scratch
     unsigned int *env_counter;    // zeroed before the launch; persistent CTAs draw environments from it
     unsigned long long *stats;    // [GX_NSTAT], only touched by the STATS instantiation
+    const uint32_t *env_filter;   // NULL = render every environment; else only those with env_filter[env] != 0
     int32_t cull;
     int32_t cull_chunk;           // clusters per cull chunk: WORK_CAP / (largest nbatch of any cluster)
 };
 
 enum { GX_STAT_CLUSTERS_TESTED = 0, GX_STAT_CLUSTERS_DRAWN, GX_STAT_TRIS_IN, GX_STAT_TRIS_RASTER,
-       GX_STAT_FRAGMENTS, GX_NSTAT };
+       GX_STAT_FRAGMENTS, GX_STAT_OVERFLOW_ENVS, GX_NSTAT };

@@ -7,7 +7,7 @@ import numpy as np
 BG = 0xFFFFFFFF
 
 
-def render_gpu(wl, want_id=True, want_rgb=None, cull=1, stats=False, scene=None, host_api=False):
+def render_gpu(wl, want_id=True, want_rgb=None, cull=1, stats=False, scene=None, host_api=False, options=None):
     """Render a workload on cuda:0 through gx_render_batch.  Returns dict(rgb, depth, id[, stats])."""
     import torch
     from paper_2306_07552_b200 import binding as gx
@@ -20,6 +20,8 @@ def render_gpu(wl, want_id=True, want_rgb=None, cull=1, stats=False, scene=None,
     try:
         gx.gx_set_option(scene, "cull", cull)
         gx.gx_set_option(scene, "stats", 1 if stats else 0)
+        for name, value in (options or {}).items():
+            gx.gx_set_option(scene, name, value)
         cam = gx.camera_of(wl)
         N, K, H, W = wl.N, wl.K, wl.height, wl.width
         out = {}
@@ -49,7 +51,7 @@ def render_gpu(wl, want_id=True, want_rgb=None, cull=1, stats=False, scene=None,
         if stats:
             out["stats"] = {k: gx.gx_get_stat(scene, k) for k in
                             ("clusters_tested", "clusters_drawn", "triangles_in", "triangles_raster", "fragments",
-                             "launches")}
+                             "overflow_envs", "launches")}
         return out
     finally:
         if own:
