@@ -377,6 +377,9 @@ struct RastWarpSmem {
     uint32_t *fq;    // [FQ_CAP] covered fragments: r | (x - i0) << 5 | (y - j0) << 12
 };
 constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4;
+constexpr int BIG_SLOTS = 512;     // a group with more slots than this is drawn in pass B, chunk by chunk
+constexpr int CHUNK_SLOTS = 256;   // slots per pass-B task (8 passes of the warp)
+constexpr int BIG_CAP = 768;       // entries of the pass-B list
 
 __host__ __device__ inline size_t raster_smem_bytes(int W, int H, int warps) {
     return (size_t)W * H * 8 + (size_t)warps * RAST_WARP_SMEM;
@@ -448,13 +451,10 @@ __device__ __forceinline__ void shade_queue_p(const RastWarpSmem &ws, int qn, in
     __syncwarp();
 }
 
-// K3 + K4a: coverage of the nrec records of the warp's group (see raster_group in gx_kernels.cuh for the
-// slot scheme).  The covered pixels of one pass are appended to the fragment queue with four ballots.
-template <bool STATS>
-__device__ __forceinline__ void raster_group_p(const RastWarpSmem &ws, int nrec, int W, float zfar, unsigned long long *fb,
-                                               uint32_t first, const uint4 *env_recs, int lane, unsigned &n_frag) {
+// K3: the bounding boxes of the group's records are cut into slots of 4 pixels of one row.  group_slots returns
+// the lane's exclusive prefix of slot counts (Pex, record = lane) and the group's total T.
+__device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int lane, int &Pex) {
     const unsigned FULL = 0xFFFFFFFFu;
-    const unsigned lt = (1u << lane) - 1u;
     int ns = 0;
     if (lane < nrec) {
         const uint32_t bb = ws.rec[R_BB * 32 + lane];
@@ -467,11 +467,23 @@ __device__ __forceinline__ void raster_group_p(const RastWarpSmem &ws, int nrec,
         const int v = __shfl_up_sync(FULL, inc, d);
         if (lane >= d) inc += v;
     }
-    const int T = __shfl_sync(FULL, inc, 31);
-    const int Pex = inc - ns;
-    const int per = (T + 31) >> 5;
-    const int s0 = lane * per;
-    const int n = min(per, T - s0);
+    Pex = inc - ns;
+    return __shfl_sync(FULL, inc, 31);
+}
+
+// K3 + K4a: coverage of the slots [S0, S1) of the warp's group.  The slots are dealt to the lanes in equal
+// contiguous runs (a lane walks through its run, moving to the next record when one is exhausted), so that
+// lanes stay busy whatever the mix of triangle sizes.  The covered pixels of one pass are appended to the
+// fragment queue with four ballots and shaded densely by shade_queue_p.
+template <bool STATS>
+__device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, int S0, int S1, int W, float zfar,
+                                             unsigned long long *fb, uint32_t first, const uint4 *env_recs, int lane,
+                                             unsigned &n_frag) {
+    const unsigned FULL = 0xFFFFFFFFu;
+    const unsigned lt = (1u << lane) - 1u;
+    const int per = (S1 - S0 + 31) >> 5;
+    const int s0 = S0 + lane * per;
+    const int n = max(0, min(per, S1 - s0));
     int r = 0;   // largest record index with Pex[r] <= s0
 #pragma unroll
     for (int step = 16; step; step >>= 1) {
@@ -495,7 +507,7 @@ __device__ __forceinline__ void raster_group_p(const RastWarpSmem &ws, int nrec,
         h = (int)((bb >> 21) & 127u) + 1;
         cw = (w + 3) >> 2;
     };
-    load_rec(r & 31);
+    load_rec(r);
     int row = off / cw, chunk = off - row * cw;
     int qn = 0;
     const uint32_t fq_addr = (uint32_t)__cvta_generic_to_shared(ws.fq);
@@ -678,7 +690,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     ws.fq = ws.rec + REC_WORDS * 32;
 
     __shared__ int s_env;
-    __shared__ unsigned s_next;
+    __shared__ unsigned s_next, s_next_b, s_big;
+    __shared__ uint2 s_big_list[BIG_CAP];   // (group, first chunk) of the groups left to pass B
     __shared__ unsigned long long s_frag;
 
     unsigned st_frag = 0;
@@ -692,7 +705,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     const uint32_t cap_n = (uint32_t)PP.cap_n;
 
     for (;;) {
-        if (tid == 0) { s_env = (int)atomicAdd(&PP.counters[1], 1u); s_next = 0; }
+        if (tid == 0) { s_env = (int)atomicAdd(&PP.counters[1], 1u); s_next = 0; s_next_b = 0; s_big = 0; }
         __syncthreads();
         const int env = s_env;
         if (env >= P.N) break;
@@ -704,7 +717,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
         const uint32_t n_n = PP.cnt[2 * env], n_w = PP.cnt[2 * env + 1] >> 1;
         const uint32_t g_n = (n_n + 31u) >> 5, g_w = (n_w + 31u) >> 5;
 
-        // ---- K3 + K4: groups of 32 records, drawn dynamically by the warps ------------------------
+        // ---- K3 + K4, pass A: groups of 32 records, drawn dynamically by the warps.  A group of more than
+        // BIG_SLOTS slots is only registered: (list index, first chunk) come from one packed atomic, so the
+        // list is ordered by first chunk.
         for (;;) {
             unsigned g = 0;
             if (lane == 0) g = atomicAdd(&s_next, 1u);
@@ -714,10 +729,49 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                 const uint32_t first = g * 32u;
                 const int nrec = (int)min(32u, n_n - first);
                 load_group(ws, env_recs, first, nrec, lane);
-                raster_group_p<STATS>(ws, nrec, W, P.zfar, fb, first, env_recs, lane, st_frag);
+                int Pex;
+                const int T = group_slots(ws, nrec, lane, Pex);
+                if (T <= BIG_SLOTS) {
+                    raster_slots<STATS>(ws, Pex, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
+                } else {
+                    unsigned full = 0;
+                    if (lane == 0) {
+                        const unsigned nch = (unsigned)(T + CHUNK_SLOTS - 1) / CHUNK_SLOTS;
+                        const unsigned old = atomicAdd(&s_big, (1u << 20) | nch);
+                        if ((old >> 20) < (unsigned)BIG_CAP) s_big_list[old >> 20] = make_uint2(g, old & 0xFFFFFu);
+                        else full = 1;
+                    }
+                    if (__shfl_sync(0xFFFFFFFFu, full, 0))   // list full: draw the group here, whole
+                        raster_slots<STATS>(ws, Pex, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
+                }
             } else {
                 const uint32_t t0 = (g - g_n) * 32u;
                 raster_wide<STATS>(env_recs, cap_n + 2u * t0, (int)min(32u, n_w - t0), W, H, P.zfar, fb, lane, st_frag);
+            }
+        }
+        __syncthreads();
+        // ---- pass B: the big groups, in chunks of CHUNK_SLOTS slots drawn dynamically ----------------
+        {
+            const unsigned packed = s_big;
+            const unsigned n_big = min(packed >> 20, (unsigned)BIG_CAP), n_chunks = packed & 0xFFFFFu;
+            for (;;) {
+                unsigned c = 0;
+                if (lane == 0) c = atomicAdd(&s_next_b, 1u);
+                c = __shfl_sync(0xFFFFFFFFu, c, 0);
+                if (c >= n_chunks) break;
+                unsigned lo = 0, hi = n_big - 1;   // last entry whose first chunk is <= c
+                while (lo < hi) {
+                    const unsigned mid = (lo + hi + 1) >> 1;
+                    if (s_big_list[mid].y <= c) lo = mid; else hi = mid - 1;
+                }
+                const uint2 en = s_big_list[lo];
+                const uint32_t first = en.x * 32u;
+                const int nrec = (int)min(32u, n_n - first);
+                load_group(ws, env_recs, first, nrec, lane);
+                int Pex;
+                const int T = group_slots(ws, nrec, lane, Pex);
+                const int S0 = (int)(c - en.y) * CHUNK_SLOTS;   // chunks of entries a full list dropped land beyond T
+                if (S0 < T) raster_slots<STATS>(ws, Pex, S0, min(T, S0 + CHUNK_SLOTS), W, P.zfar, fb, first, env_recs, lane, st_frag);
             }
         }
         __syncthreads();
