@@ -79,6 +79,7 @@ struct GxScene {
     std::vector<uint32_t> mesh_nt;      // host copy, for id-range validation
     uint32_t max_dyn_nt = 0, max_static_nt = 0;
     uint32_t max_nbatch = 1;            // largest number of batches in any cluster
+    uint32_t max_static_batches = 0, max_dyn_batches = 0;   // largest number of batches in any static / dynamic mesh
     int max_smem_optin = 0;
     unsigned int *env_counter = nullptr;
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
@@ -88,7 +89,7 @@ struct GxScene {
     int opt_path = 0;                   // 0 = two-kernel path (geometry -> records -> raster), 1 = single kernel
     int64_t opt_pool_slots = 0;         // narrow record slots per environment; 0 = max(4096, 4*W*H)
     int64_t opt_pool_bytes = 0;         // record pool budget; 0 = 8 GB
-    int opt_geom_split = 0;             // geometry work units per environment; 0 = automatic
+    int opt_big_slots = 512, opt_chunk_slots = 256;   // raster pass B (gx_pipeline.cuh)
     DevBuf<uint4> pool;                 // triangle records of one chunk of environments
     DevBuf<uint32_t> pipe_scratch;      // counters[4] | cnt[2*chunk] | env_flag[chunk]
     int last_launches = 0;
@@ -223,21 +224,22 @@ int launch_raster(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stre
     return GX_OK;
 }
 
-// two-kernel path (gx_pipeline.cuh): geometry kernel, then raster kernel
+// two-kernel path (gx_pipeline.cuh): cull kernel, geometry kernel, raster order, raster kernel
 int launch_pipeline(const GxScene *sc, gx::PipeParams &PP, cudaStream_t stream, bool stats) {
-    constexpr int GW = 8;
+    constexpr int CW = 4, GW = 8;
+    auto ck = stats ? gx::cull_kernel<CW, true> : gx::cull_kernel<CW, false>;
+    const size_t csmem = gx::env_smem_bytes(PP.g.K);
+    ck<<<PP.g.N, CW * 32, csmem, stream>>>(PP);
+    GX_CUDA(cudaGetLastError());
     auto gk = stats ? gx::geom_kernel<GW, true> : gx::geom_kernel<GW, false>;
-    const size_t gsmem = gx::geom_smem_bytes(PP.g.K, GW);
+    const size_t gsmem = (size_t)GW * gx::GEOM_WARP_SMEM;
     GX_CUDA(cudaFuncSetAttribute(gk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem));
     int per_sm = 0;
     GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gk, GW * 32, gsmem));
     if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "geometry kernel does not fit: %zu bytes of shared memory", gsmem);
-    const int slots = sc->num_sms * per_sm;
-    // work units per environment: enough units that the last wave of CTAs is a small part of the whole
-    int split = sc->opt_geom_split;
-    if (split <= 0) split = PP.g.N >= 8 * slots ? 1 : std::min(8, std::max(1, (8 * slots + PP.g.N - 1) / PP.g.N));
-    PP.split = split;
-    gk<<<(int)std::min<long long>((long long)PP.g.N * split, slots), GW * 32, gsmem, stream>>>(PP);
+    gk<<<sc->num_sms * per_sm, GW * 32, gsmem, stream>>>(PP);
+    GX_CUDA(cudaGetLastError());
+    gx::order_kernel<<<1, 1024, 0, stream>>>(PP);
     GX_CUDA(cudaGetLastError());
     if ((size_t)PP.g.W * PP.g.H * 8 <= 32768) return launch_raster<16, 2>(sc, PP, stream, stats);
     return launch_raster<32, 1>(sc, PP, stream, stats);
@@ -270,8 +272,11 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
                 return fail(GX_ERR_INVALID_ARG, "mesh %d has NULL arrays", i);
             }
             GxMeshDev md;
+            const size_t b0 = batches.size();
             const int rc = build_mesh(m, verts, tris, batches, clusters, md);
             if (rc != GX_OK) { delete sc; return rc; }
+            uint32_t &mb = i < n_static ? sc->max_static_batches : sc->max_dyn_batches;
+            mb = std::max<uint32_t>(mb, (uint32_t)(batches.size() - b0));
             meshes.push_back(md);
             sc->mesh_nt.push_back(m.nt);
             if (i < n_static) sc->max_static_nt = std::max(sc->max_static_nt, m.nt);
@@ -359,9 +364,9 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
         sc->opt_pool_bytes = value;
         return GX_OK;
     }
-    if (!strcmp(name, "geom_split")) {
-        if (value < 0 || value > 64) return fail(GX_ERR_INVALID_ARG, "geom_split must be in [0, 64]");
-        sc->opt_geom_split = (int)value;
+    if (!strcmp(name, "big_slots") || !strcmp(name, "chunk_slots")) {
+        if (value < 32 || value > (1 << 20)) return fail(GX_ERR_INVALID_ARG, "%s must be in [32, 2^20]", name);
+        (name[0] == 'b' ? sc->opt_big_slots : sc->opt_chunk_slots) = (int)value;
         return GX_OK;
     }
     return fail(GX_ERR_INVALID_ARG, "unknown option '%s'", name);
@@ -453,7 +458,14 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(N, budget / env_bytes));
     int rc;
     if ((rc = sc->pool.reserve((size_t)chunk * (size_t)(cap_n + cap_w) * 4)) != GX_OK) return rc;
-    if ((rc = sc->pipe_scratch.reserve(4 + 3 * (size_t)chunk)) != GX_OK) return rc;
+    // scratch words: counters[4] | cnt[2*chunk] | env_flag[chunk] | order[chunk] | env_idb[chunk*(K+1)] |
+    //                env_mv[chunk*(K+1)*12] | items[2*chunk*items_per_env]
+    const size_t k1 = (size_t)K + 1;
+    const size_t items_per_env = (size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches;
+    const size_t n_zero = 4 + 3 * (size_t)chunk;
+    const size_t off_order = n_zero, off_idb = off_order + chunk, off_mv = off_idb + chunk * k1;
+    const size_t off_items = (off_mv + chunk * k1 * 12 + 1) & ~(size_t)1;
+    if ((rc = sc->pipe_scratch.reserve(off_items + 2 * (size_t)chunk * std::max<size_t>(items_per_env, 1))) != GX_OK) return rc;
     int launches = 0;
     for (int e0 = 0; e0 < N; e0 += chunk) {
         const int n = std::min(chunk, N - e0);
@@ -473,14 +485,20 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.env_flag = sc->pipe_scratch.p + 4 + 2 * (size_t)chunk;
         PP.cap_n = (int32_t)cap_n;
         PP.cap_w = (int32_t)cap_w;
-        GX_CUDA(cudaMemsetAsync(sc->pipe_scratch.p, 0, (4 + 3 * (size_t)chunk) * sizeof(uint32_t), stream));
+        PP.big_slots = sc->opt_big_slots;
+        PP.chunk_slots = sc->opt_chunk_slots;
+        PP.order = sc->pipe_scratch.p + off_order;
+        PP.env_idb = sc->pipe_scratch.p + off_idb;
+        PP.env_mv = reinterpret_cast<float *>(sc->pipe_scratch.p + off_mv);
+        PP.items = reinterpret_cast<uint2 *>(sc->pipe_scratch.p + off_items);
+        GX_CUDA(cudaMemsetAsync(sc->pipe_scratch.p, 0, n_zero * sizeof(uint32_t), stream));
         if ((rc = launch_pipeline(sc, PP, stream, st)) != GX_OK) return rc;
         // environments whose records overflowed their pool segment: single-kernel pass over the flagged ones
         GxParams PL = PP.g;
-        PL.env_counter = sc->pipe_scratch.p + 2;
+        PL.env_counter = sc->pipe_scratch.p + 3;
         PL.env_filter = PP.env_flag;
         if ((rc = launch_single(sc, PL, stream, st)) != GX_OK) return rc;
-        launches += 3;
+        launches += 5;
         sc->last_chunk_n = n;
     }
     sc->last_launches = launches;

@@ -41,9 +41,13 @@ struct PipeParams {
     uint4 *recs;             // [N][cap_n + cap_w][4]
     uint32_t *cnt;           // [N][2]: narrow slots, wide slots appended
     uint32_t *env_flag;      // [N]: 1 = pool segment overflowed, render with the single-kernel path
-    unsigned int *counters;  // [0] geometry work-unit counter, [1] raster env counter
+    unsigned int *counters;  // [0] geometry item counter, [1] raster env counter, [2] items in the work list
+    uint2 *items;            // work list: (slot << 24 | batch, environment)
+    float *env_mv;           // [N][K+1][12] model-view per slot
+    uint32_t *env_idb;       // [N][K+1] first triangle id per slot
+    uint32_t *order;         // [N] raster order of the environments
     int32_t cap_n, cap_w;    // slots per environment
-    int32_t split;           // geometry work units per environment (each takes 1/split of the cluster space)
+    int32_t big_slots, chunk_slots;   // raster pass B: groups above big_slots are drawn in chunks of chunk_slots
 };
 
 struct GeomWarpSmem {
@@ -98,18 +102,17 @@ __device__ __forceinline__ void store_colour_slot(uint4 *dst, const float c[3][3
 // geometry: K2 for one batch, by one warp
 // ------------------------------------------------------------------------------------------------
 template <bool STATS>
-__device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj, uint32_t item, const EnvSmem &es,
-                                           const GeomWarpSmem &ws, int env, int lane, bool &overflow, unsigned &n_in,
-                                           unsigned &n_tri) {
+__device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj, uint32_t batch, const float *__restrict__ MV,
+                                           uint32_t slot_id_base, const GeomWarpSmem &ws, int env, int lane,
+                                           bool &overflow, unsigned &n_in, unsigned &n_tri) {
     const GxParams &P = PP.g;
     const unsigned FULL = 0xFFFFFFFFu;
-    const uint32_t s = item >> 24;
-    const GxBatchDev b = P.batches[item & 0xFFFFFFu];
+    const GxBatchDev b = P.batches[batch];
     const int nv = (int)(b.nv_nt & 0xFFFFu), nt = (int)(b.nv_nt >> 16);
     float M[12];
 #pragma unroll
-    for (int k = 0; k < 12; ++k) M[k] = es.MV[s * 12 + k];
-    const uint32_t idb = es.id_base[s] + b.first_tri;
+    for (int k = 0; k < 12; ++k) M[k] = MV[k];
+    const uint32_t idb = slot_id_base + b.first_tri;
     const float4 *__restrict__ verts = P.verts + b.vert_off;
     const uchar4 *__restrict__ tris = P.tris + b.tri_off;
     const unsigned lt = (1u << lane) - 1u;
@@ -285,14 +288,87 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
 namespace gx {
 
 // ------------------------------------------------------------------------------------------------
-// the geometry kernel
+// K1: the cull kernel.  One CTA per environment: slot tables, model-view matrices (N1, N2) and id bases go to
+// the environment table in global memory; every cluster AABB of the environment is tested against the
+// frustum and the batches of the survivors are appended to the chunk-wide work list (warp-aggregated atomics).
+// ------------------------------------------------------------------------------------------------
+template <int WARPS, bool STATS>
+__global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
+    extern __shared__ __align__(16) unsigned char smem[];
+    const GxParams &P = PP.g;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int NT = WARPS * 32;
+    const int K = P.K;
+    const int env = blockIdx.x;
+
+    unsigned char *p = smem;
+    EnvSmem es;
+    es.MV = reinterpret_cast<float *>(p);          p += (size_t)(K + 1) * 48;
+    es.id_base = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 2) * 4;
+    es.cl_base = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 2) * 4;
+    es.slot_cl = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
+    es.slot_mesh = reinterpret_cast<int32_t *>(p); p += (size_t)(K + 1) * 4;
+    es.slot_nt = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
+    es.slot_nc = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
+    es.work = nullptr;
+
+    env_setup(P, env, es, tid);
+    float *g_mv = PP.env_mv + (size_t)env * (size_t)(K + 1) * 12;
+    uint32_t *g_idb = PP.env_idb + (size_t)env * (size_t)(K + 1);
+    for (int k = tid; k < (K + 1) * 12; k += NT) g_mv[k] = es.MV[k];
+    for (int k = tid; k <= K; k += NT) g_idb[k] = es.id_base[k];
+
+    unsigned st_tested = 0, st_drawn = 0;
+    const uint32_t n_cl = es.cl_base[K + 1];
+    for (uint32_t g0 = warp * 32; g0 < n_cl; g0 += NT) {
+        const uint32_t g = g0 + lane;
+        uint32_t nb = 0, boff = 0, s = 0;
+        if (g < n_cl) {
+            int lo = 0, hi = K;
+            while (lo < hi) {   // largest slot whose first cluster index is <= g
+                const int mid = (lo + hi + 1) >> 1;
+                if (es.cl_base[mid] <= g) lo = mid; else hi = mid - 1;
+            }
+            s = (uint32_t)lo;
+            const GxClusterDev c = P.clusters[es.slot_cl[s] + (g - es.cl_base[s])];
+            const bool vis = !P.cull || cluster_visible(c, es.MV + s * 12, P.fx, P.fy, P.znear, P.zfar);
+            if (STATS) { ++st_tested; st_drawn += vis ? 1u : 0u; }
+            if (vis) { nb = c.nbatch; boff = c.batch_off; }
+        }
+        uint32_t inc = nb;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+            if (lane >= d) inc += a;
+        }
+        const uint32_t tot = __shfl_sync(0xFFFFFFFFu, inc, 31);
+        uint32_t base = 0;
+        if (lane == 0 && tot) base = atomicAdd(&PP.counters[2], tot);
+        base = __shfl_sync(0xFFFFFFFFu, base, 0) + inc - nb;
+        for (uint32_t k = 0; k < nb; ++k) PP.items[base + k] = make_uint2((s << 24) | (boff + k), (uint32_t)env);
+    }
+    if (STATS) {
+#pragma unroll
+        for (int d = 16; d; d >>= 1) {
+            st_tested += __shfl_xor_sync(0xFFFFFFFFu, st_tested, d);
+            st_drawn += __shfl_xor_sync(0xFFFFFFFFu, st_drawn, d);
+        }
+        if (lane == 0) {
+            atomicAdd(&P.stats[GX_STAT_CLUSTERS_TESTED], (unsigned long long)st_tested);
+            atomicAdd(&P.stats[GX_STAT_CLUSTERS_DRAWN], (unsigned long long)st_drawn);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// K2: the geometry kernel.  Persistent warps draw (environment, slot, batch) items from the work list; there
+// is no CTA-level synchronisation at all.
 // ------------------------------------------------------------------------------------------------
 template <int WARPS, bool STATS>
 __global__ void __launch_bounds__(WARPS * 32, 1024 / (WARPS * 32)) geom_kernel(const PipeParams PP) {
     extern __shared__ __align__(16) unsigned char smem[];
     const GxParams &P = PP.g;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int NT = WARPS * 32;
     const int K = P.K;
 
     GeomWarpSmem ws;
@@ -303,69 +379,69 @@ __global__ void __launch_bounds__(WARPS * 32, 1024 / (WARPS * 32)) geom_kernel(c
         ws.vC = reinterpret_cast<uint32_t *>(w + GX_VCAP * 12);
         ws.lst = w + GX_VCAP * 16;
     }
-    unsigned char *p = smem + (size_t)WARPS * GEOM_WARP_SMEM;
-    EnvSmem es;
-    es.MV = reinterpret_cast<float *>(p);          p += (size_t)(K + 1) * 48;
-    es.id_base = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 2) * 4;
-    es.cl_base = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 2) * 4;
-    es.slot_cl = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
-    es.slot_mesh = reinterpret_cast<int32_t *>(p); p += (size_t)(K + 1) * 4;
-    es.slot_nt = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
-    es.slot_nc = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
-    es.work = reinterpret_cast<uint32_t *>(p);
-
-    __shared__ int s_env;
-    __shared__ unsigned s_work_n, s_work_next;
-    __shared__ unsigned long long s_stat[GX_NSTAT];
-
     Proj pj;
     pj.fx = P.fx; pj.fy = P.fy;
     pj.hw = 128.0f * (float)P.W; pj.hh = 128.0f * (float)P.H;
 
-    unsigned st_tested = 0, st_drawn = 0, st_in = 0, st_tri = 0;
-    if (STATS) {
-        if (tid < GX_NSTAT) s_stat[tid] = 0;
-    }
-
-    for (;;) {
-        if (tid == 0) s_env = (int)atomicAdd(&PP.counters[0], 1u);
-        __syncthreads();
-        const int unit = s_env;
-        if (unit >= P.N * PP.split) break;
-        const int env = unit / PP.split, part = unit - env * PP.split;
-        env_setup(P, env, es, tid);
-
-        const uint32_t n_all = es.cl_base[K + 1];
-        const uint32_t c_lo = (uint32_t)(((unsigned long long)n_all * (unsigned)part) / (unsigned)PP.split);
-        const uint32_t n_cl = (uint32_t)(((unsigned long long)n_all * (unsigned)(part + 1)) / (unsigned)PP.split);
+    unsigned st_in = 0, st_tri = 0;
+    const unsigned n_items = PP.counters[2];
+    unsigned next = 0;
+    if (lane == 0) next = atomicAdd(&PP.counters[0], 1u);
+    next = __shfl_sync(0xFFFFFFFFu, next, 0);
+    while (next < n_items) {
+        const uint2 item = PP.items[next];
+        if (lane == 0) next = atomicAdd(&PP.counters[0], 1u);   // draw the following item while this one is processed
+        const int env = (int)item.y;
+        const uint32_t s = item.x >> 24;
         bool overflow = false;
-        for (uint32_t c0 = c_lo; c0 < n_cl; c0 += (uint32_t)P.cull_chunk) {
-            if (tid == 0) { s_work_n = 0; s_work_next = 0; }
-            __syncthreads();
-            cull_chunk_to_worklist<STATS>(P, es, c0, min(c0 + (uint32_t)P.cull_chunk, n_cl), tid, NT, &s_work_n, st_tested, st_drawn);
-            __syncthreads();
-            const unsigned n_work = s_work_n;
-            for (;;) {
-                unsigned wi = 0;
-                if (lane == 0) wi = atomicAdd(&s_work_next, 1u);
-                wi = __shfl_sync(0xFFFFFFFFu, wi, 0);
-                if (wi >= n_work) break;
-                geom_batch<STATS>(PP, pj, es.work[wi], es, ws, env, lane, overflow, st_in, st_tri);
-            }
-            __syncthreads();
-        }
+        geom_batch<STATS>(PP, pj, item.x & 0xFFFFFFu, PP.env_mv + ((size_t)env * (size_t)(K + 1) + s) * 12,
+                          PP.env_idb[(size_t)env * (size_t)(K + 1) + s], ws, env, lane, overflow, st_in, st_tri);
         if (overflow && lane == 0 && atomicExch(&PP.env_flag[env], 1u) == 0u)
             atomicAdd(&P.stats[GX_STAT_OVERFLOW_ENVS], 1ull);
-        __syncthreads();
+        next = __shfl_sync(0xFFFFFFFFu, next, 0);
     }
-
     if (STATS) {
-        atomicAdd(&s_stat[GX_STAT_CLUSTERS_TESTED], (unsigned long long)st_tested);
-        atomicAdd(&s_stat[GX_STAT_CLUSTERS_DRAWN], (unsigned long long)st_drawn);
-        atomicAdd(&s_stat[GX_STAT_TRIS_IN], (unsigned long long)st_in);
-        atomicAdd(&s_stat[GX_STAT_TRIS_RASTER], (unsigned long long)st_tri);
-        __syncthreads();
-        if (tid < GX_NSTAT) atomicAdd(&P.stats[tid], s_stat[tid]);
+#pragma unroll
+        for (int d = 16; d; d >>= 1) st_tri += __shfl_xor_sync(0xFFFFFFFFu, st_tri, d);
+        if (lane == 0) {
+            atomicAdd(&P.stats[GX_STAT_TRIS_IN], (unsigned long long)st_in);
+            atomicAdd(&P.stats[GX_STAT_TRIS_RASTER], (unsigned long long)st_tri);
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// raster order: environments sorted by record count, heaviest first (one CTA, counting sort in 256 bins), so
+// that the persistent raster CTAs finish together.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024) order_kernel(const PipeParams PP) {
+    __shared__ unsigned hist[256];
+    const int tid = threadIdx.x, N = PP.g.N;
+    if (tid < 256) hist[tid] = 0;
+    __syncthreads();
+    for (int e = tid; e < N; e += 1024) {
+        const unsigned tot = PP.cnt[2 * e] + 4u * PP.cnt[2 * e + 1];
+        atomicAdd(&hist[255u - min(255u, tot >> 7)], 1u);
+    }
+    __syncthreads();
+    if (tid < 32) {   // exclusive scan of the 256 bins by one warp, 8 bins per lane
+        unsigned v[8], sum = 0;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { v[k] = hist[tid * 8 + k]; sum += v[k]; }
+        unsigned inc = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const unsigned a = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+            if (tid >= d) inc += a;
+        }
+        unsigned run = inc - sum;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) { hist[tid * 8 + k] = run; run += v[k]; }
+    }
+    __syncthreads();
+    for (int e = tid; e < N; e += 1024) {
+        const unsigned tot = PP.cnt[2 * e] + 4u * PP.cnt[2 * e + 1];
+        PP.order[atomicAdd(&hist[255u - min(255u, tot >> 7)], 1u)] = (uint32_t)e;
     }
 }
 
@@ -377,8 +453,6 @@ struct RastWarpSmem {
     uint32_t *fq;    // [FQ_CAP] covered fragments: r | (x - i0) << 5 | (y - j0) << 12
 };
 constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4;
-constexpr int BIG_SLOTS = 512;     // a group with more slots than this is drawn in pass B, chunk by chunk
-constexpr int CHUNK_SLOTS = 256;   // slots per pass-B task (8 passes of the warp)
 constexpr int BIG_CAP = 768;       // entries of the pass-B list
 
 __host__ __device__ inline size_t raster_smem_bytes(int W, int H, int warps) {
@@ -705,10 +779,14 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     const uint32_t cap_n = (uint32_t)PP.cap_n;
 
     for (;;) {
-        if (tid == 0) { s_env = (int)atomicAdd(&PP.counters[1], 1u); s_next = 0; s_next_b = 0; s_big = 0; }
+        if (tid == 0) {
+            const unsigned k = atomicAdd(&PP.counters[1], 1u);
+            s_env = k < (unsigned)P.N ? (int)PP.order[k] : -1;
+            s_next = 0; s_next_b = 0; s_big = 0;
+        }
         __syncthreads();
         const int env = s_env;
-        if (env >= P.N) break;
+        if (env < 0) break;
         if (PP.env_flag[env]) {   // overflowed its pool segment: left to the single-kernel pass
             __syncthreads();
             continue;
@@ -731,12 +809,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                 load_group(ws, env_recs, first, nrec, lane);
                 int Pex;
                 const int T = group_slots(ws, nrec, lane, Pex);
-                if (T <= BIG_SLOTS) {
+                if (T <= PP.big_slots) {
                     raster_slots<STATS>(ws, Pex, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
                 } else {
                     unsigned full = 0;
                     if (lane == 0) {
-                        const unsigned nch = (unsigned)(T + CHUNK_SLOTS - 1) / CHUNK_SLOTS;
+                        const unsigned nch = (unsigned)(T + PP.chunk_slots - 1) / (unsigned)PP.chunk_slots;
                         const unsigned old = atomicAdd(&s_big, (1u << 20) | nch);
                         if ((old >> 20) < (unsigned)BIG_CAP) s_big_list[old >> 20] = make_uint2(g, old & 0xFFFFFu);
                         else full = 1;
@@ -770,8 +848,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                 load_group(ws, env_recs, first, nrec, lane);
                 int Pex;
                 const int T = group_slots(ws, nrec, lane, Pex);
-                const int S0 = (int)(c - en.y) * CHUNK_SLOTS;   // chunks of entries a full list dropped land beyond T
-                if (S0 < T) raster_slots<STATS>(ws, Pex, S0, min(T, S0 + CHUNK_SLOTS), W, P.zfar, fb, first, env_recs, lane, st_frag);
+                const int S0 = (int)(c - en.y) * PP.chunk_slots;   // chunks of entries a full list dropped land beyond T
+                if (S0 < T) raster_slots<STATS>(ws, Pex, S0, min(T, S0 + PP.chunk_slots), W, P.zfar, fb, first, env_recs, lane, st_frag);
             }
         }
         __syncthreads();

@@ -85,20 +85,20 @@ def test_cull_is_conservative(oracle_mod):
 def test_paths_pool_overflow_and_chunking(oracle_mod):
     """The two-kernel path (geometry -> record pool -> raster) against the oracle and against the single-kernel
     path; a pool too small for some environments (those fall back to the single kernel) or for all of them;
-    a pool budget that forces several chunks; geometry work units split 1..5 ways: all bit-identical."""
+    a pool budget that forces several chunks; other raster pass-B thresholds: all bit-identical."""
     wl = gen.make_config(2, n_envs=20)
     o = oracle_mod.render(wl)
     ref = render_gpu(wl, stats=True)
     rep = compare(o, ref)
     assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, rep
-    assert ref["stats"]["overflow_envs"] == 0 and ref["stats"]["launches"] == 3
+    assert ref["stats"]["overflow_envs"] == 0 and ref["stats"]["launches"] == 5
     variants = {
         "single kernel": dict(path=1),
         "some overflow": dict(pool_slots=12288),
         "all overflow": dict(pool_slots=64),
         "chunks of 3": dict(pool_bytes=3 * (65536 + 8192) * 64),
-        "split 1": dict(geom_split=1),
-        "split 5": dict(geom_split=5),
+        "small pass-B chunks": dict(big_slots=64, chunk_slots=32),
+        "no pass B": dict(big_slots=1 << 20),
     }
     for name, opts in variants.items():
         g = render_gpu(wl, stats=True, options=opts)
@@ -109,7 +109,7 @@ def test_paths_pool_overflow_and_chunking(oracle_mod):
         if name == "some overflow":
             assert 0 < g["stats"]["overflow_envs"] < wl.N, g["stats"]
         if name == "chunks of 3":
-            assert g["stats"]["launches"] == 3 * 7
+            assert g["stats"]["launches"] == 5 * 7
         if name != "single kernel":
             assert g["stats"]["triangles_raster"] >= ref["stats"]["triangles_raster"]
 
