@@ -91,6 +91,11 @@ struct GxScene {
     int64_t opt_pool_bytes = 0;         // record pool budget; 0 = 8 GB
     int opt_big_slots = 512, opt_chunk_slots = 256;   // raster pass B (gx_pipeline.cuh)
     DevBuf<uint4> pool;                 // triangle records of one chunk of environments
+    DevBuf<unsigned long long> frames;  // frame keys between the two raster phases
+    int opt_occlusion = 1;              // occluder phase + hi-Z culling of clusters and records
+    int opt_occluder_pct = 25;          // share of the visible clusters (nearest first) drawn in the occluder phase
+    DevBuf<uint32_t> zkeys, rec_order;  // depth sort keys of the records; per-raster-CTA order lists
+    int opt_depth_sort = 1;             // raster draws the records near to far and keeps the hi-Z tiles live
     DevBuf<uint32_t> pipe_scratch;      // counters[4] | cnt[2*chunk] | env_flag[chunk]
     int last_launches = 0;
     cudaStream_t last_stream = nullptr;
@@ -211,9 +216,9 @@ int launch_single(const GxScene *sc, const GxParams &P, cudaStream_t stream, boo
     return launch<8, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, st);
 }
 
-template <int WARPS, int MINB>
+template <int WARPS, int MINB, int PHASE>
 int launch_raster(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
-    auto kern = stats ? gx::raster_kernel<WARPS, MINB, true> : gx::raster_kernel<WARPS, MINB, false>;
+    auto kern = stats ? gx::raster_kernel<WARPS, MINB, PHASE, true> : gx::raster_kernel<WARPS, MINB, PHASE, false>;
     const size_t smem = gx::raster_smem_bytes(PP.g.W, PP.g.H, WARPS);
     GX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
@@ -224,10 +229,12 @@ int launch_raster(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stre
     return GX_OK;
 }
 
-// two-kernel path (gx_pipeline.cuh): cull kernel, geometry kernel, raster order, raster kernel
-int launch_pipeline(const GxScene *sc, gx::PipeParams &PP, cudaStream_t stream, bool stats) {
-    constexpr int CW = 4, GW = 8;
-    auto ck = stats ? gx::cull_kernel<CW, true> : gx::cull_kernel<CW, false>;
+// one pass of the pipeline (gx_pipeline.cuh): cull kernel, geometry kernel, raster order, raster kernel.
+// PHASE 0 = everything in one pass; 1 = occluder phase; 2 = the rest, culled against the occluder phase's hi-Z.
+template <int PHASE>
+int launch_pass(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
+    constexpr int CW = 4, GW = 8, CP = PHASE == 2 ? 2 : 1;
+    auto ck = stats ? gx::cull_kernel<CW, CP, true> : gx::cull_kernel<CW, CP, false>;
     const size_t csmem = gx::env_smem_bytes(PP.g.K);
     ck<<<PP.g.N, CW * 32, csmem, stream>>>(PP);
     GX_CUDA(cudaGetLastError());
@@ -239,10 +246,10 @@ int launch_pipeline(const GxScene *sc, gx::PipeParams &PP, cudaStream_t stream, 
     if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "geometry kernel does not fit: %zu bytes of shared memory", gsmem);
     gk<<<sc->num_sms * per_sm, GW * 32, gsmem, stream>>>(PP);
     GX_CUDA(cudaGetLastError());
-    gx::order_kernel<<<1, 1024, 0, stream>>>(PP);
+    gx::order_kernel<<<1, 1024, 0, stream>>>(PP, PHASE == 2 ? 1 : 0);
     GX_CUDA(cudaGetLastError());
-    if ((size_t)PP.g.W * PP.g.H * 8 <= 32768) return launch_raster<16, 2>(sc, PP, stream, stats);
-    return launch_raster<32, 1>(sc, PP, stream, stats);
+    if ((size_t)PP.g.W * PP.g.H * 8 <= 32768) return launch_raster<16, 2, PHASE>(sc, PP, stream, stats);
+    return launch_raster<32, 1, PHASE>(sc, PP, stream, stats);
 }
 
 }  // namespace
@@ -338,7 +345,7 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->meshes);
     cudaFree(sc->env_counter);
     cudaFree(sc->stats);
-    sc->pool.release(); sc->pipe_scratch.release();
+    sc->pool.release(); sc->pipe_scratch.release(); sc->frames.release(); sc->zkeys.release(); sc->rec_order.release();
     sc->h_env_scene.release(); sc->h_inst_mesh.release(); sc->h_cam_pose.release(); sc->h_inst_xform.release();
     sc->h_depth.release(); sc->h_rgb.release(); sc->h_id.release();
     if (sc->host_stream) cudaStreamDestroy(sc->host_stream);
@@ -349,6 +356,13 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
     if (!sc || !name) return fail(GX_ERR_INVALID_ARG, "NULL argument");
     if (!strcmp(name, "cull")) { sc->opt_cull = value != 0; return GX_OK; }
     if (!strcmp(name, "stats")) { sc->opt_stats = value != 0; return GX_OK; }
+    if (!strcmp(name, "depth_sort")) { sc->opt_depth_sort = value != 0; return GX_OK; }
+    if (!strcmp(name, "occlusion")) { sc->opt_occlusion = value != 0; return GX_OK; }
+    if (!strcmp(name, "occluder_pct")) {
+        if (value < 1 || value > 100) return fail(GX_ERR_INVALID_ARG, "occluder_pct must be in [1, 100]");
+        sc->opt_occluder_pct = (int)value;
+        return GX_OK;
+    }
     if (!strcmp(name, "path")) {
         if (value < 0 || value > 1) return fail(GX_ERR_INVALID_ARG, "path must be 0 or 1");
         sc->opt_path = (int)value;
@@ -381,7 +395,7 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
         DeviceGuard guard(sc->device);
         std::vector<uint32_t> cnt(2 * (size_t)sc->last_chunk_n);
         GX_CUDA(cudaStreamSynchronize(sc->last_stream));
-        GX_CUDA(cudaMemcpy(cnt.data(), sc->pipe_scratch.p + 4, cnt.size() * 4, cudaMemcpyDeviceToHost));
+        GX_CUDA(cudaMemcpy(cnt.data(), sc->pipe_scratch.p + 8, cnt.size() * 4, cudaMemcpyDeviceToHost));
         std::vector<uint32_t> tot(sc->last_chunk_n);
         for (int e = 0; e < sc->last_chunk_n; ++e) tot[e] = cnt[2 * e] + cnt[2 * e + 1];
         std::sort(tot.begin(), tot.end());
@@ -389,7 +403,7 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
         return GX_OK;
     }
     static const char *names[GX_NSTAT] = {"clusters_tested", "clusters_drawn", "triangles_in", "triangles_raster",
-                                          "fragments", "overflow_envs"};
+                                          "fragments", "overflow_envs", "clusters_occluded", "records_occluded"};
     for (int k = 0; k < GX_NSTAT; ++k)
         if (!strcmp(name, names[k])) {
             DeviceGuard guard(sc->device);
@@ -458,14 +472,19 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(N, budget / env_bytes));
     int rc;
     if ((rc = sc->pool.reserve((size_t)chunk * (size_t)(cap_n + cap_w) * 4)) != GX_OK) return rc;
-    // scratch words: counters[4] | cnt[2*chunk] | env_flag[chunk] | order[chunk] | env_idb[chunk*(K+1)] |
-    //                env_mv[chunk*(K+1)*12] | items[2*chunk*items_per_env]
+    // scratch words: counters[8] | cnt[2*chunk] | env_flag[chunk] (zeroed per chunk) | order[chunk] | cnt1[2*chunk] |
+    //                thr[chunk] | env_idb[chunk*(K+1)] | env_mv[chunk*(K+1)*12] | hiz[chunk*HZ_STRIDE] | items[2*...]
+    const bool two_phase = sc->opt_cull && sc->opt_occlusion && sc->opt_occluder_pct < 100;
     const size_t k1 = (size_t)K + 1;
     const size_t items_per_env = (size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches;
-    const size_t n_zero = 4 + 3 * (size_t)chunk;
-    const size_t off_order = n_zero, off_idb = off_order + chunk, off_mv = off_idb + chunk * k1;
-    const size_t off_items = (off_mv + chunk * k1 * 12 + 1) & ~(size_t)1;
+    const size_t n_zero = 8 + 3 * (size_t)chunk;
+    const size_t off_order = n_zero, off_cnt1 = off_order + chunk, off_thr = off_cnt1 + 2 * (size_t)chunk;
+    const size_t off_idb = off_thr + chunk, off_mv = off_idb + chunk * k1, off_hiz = off_mv + chunk * k1 * 12;
+    const size_t off_items = (off_hiz + (size_t)chunk * gx::HZ_STRIDE + 1) & ~(size_t)1;
     if ((rc = sc->pipe_scratch.reserve(off_items + 2 * (size_t)chunk * std::max<size_t>(items_per_env, 1))) != GX_OK) return rc;
+    if (two_phase && (rc = sc->frames.reserve((size_t)chunk * (size_t)npix)) != GX_OK) return rc;
+    if ((rc = sc->zkeys.reserve((size_t)chunk * (size_t)cap_n)) != GX_OK) return rc;
+    if ((rc = sc->rec_order.reserve((size_t)sc->num_sms * 2 * (size_t)cap_n)) != GX_OK) return rc;
     int launches = 0;
     for (int e0 = 0; e0 < N; e0 += chunk) {
         const int n = std::min(chunk, N - e0);
@@ -481,8 +500,16 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.g.id = id_out ? id_out + (size_t)e0 * npix : nullptr;
         PP.recs = sc->pool.p;
         PP.counters = sc->pipe_scratch.p;
-        PP.cnt = sc->pipe_scratch.p + 4;
-        PP.env_flag = sc->pipe_scratch.p + 4 + 2 * (size_t)chunk;
+        PP.cnt = sc->pipe_scratch.p + 8;
+        PP.env_flag = sc->pipe_scratch.p + 8 + 2 * (size_t)chunk;
+        PP.cnt1 = sc->pipe_scratch.p + off_cnt1;
+        PP.thr = reinterpret_cast<float *>(sc->pipe_scratch.p + off_thr);
+        PP.hiz = reinterpret_cast<float *>(sc->pipe_scratch.p + off_hiz);
+        PP.frames = sc->frames.p;
+        PP.zkeys = sc->zkeys.p;
+        PP.rec_order = sc->rec_order.p;
+        PP.depth_sort = sc->opt_depth_sort;
+        PP.occl_pct = two_phase ? sc->opt_occluder_pct : 100;
         PP.cap_n = (int32_t)cap_n;
         PP.cap_w = (int32_t)cap_w;
         PP.big_slots = sc->opt_big_slots;
@@ -492,13 +519,21 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.env_mv = reinterpret_cast<float *>(sc->pipe_scratch.p + off_mv);
         PP.items = reinterpret_cast<uint2 *>(sc->pipe_scratch.p + off_items);
         GX_CUDA(cudaMemsetAsync(sc->pipe_scratch.p, 0, n_zero * sizeof(uint32_t), stream));
-        if ((rc = launch_pipeline(sc, PP, stream, st)) != GX_OK) return rc;
+        if (!two_phase) {
+            if ((rc = launch_pass<0>(sc, PP, stream, st)) != GX_OK) return rc;
+            launches += 4;
+        } else {
+            if ((rc = launch_pass<1>(sc, PP, stream, st)) != GX_OK) return rc;
+            PP.counters = sc->pipe_scratch.p + 4;
+            if ((rc = launch_pass<2>(sc, PP, stream, st)) != GX_OK) return rc;
+            launches += 8;
+        }
         // environments whose records overflowed their pool segment: single-kernel pass over the flagged ones
         GxParams PL = PP.g;
         PL.env_counter = sc->pipe_scratch.p + 3;
         PL.env_filter = PP.env_flag;
         if ((rc = launch_single(sc, PL, stream, st)) != GX_OK) return rc;
-        launches += 5;
+        launches += 1;
         sc->last_chunk_n = n;
     }
     sc->last_launches = launches;

@@ -723,8 +723,10 @@ namespace gx {
 // snapped X is <= 0 or >= 256*W (resp. Y), half a pixel away from the nearest pixel centre, which dwarfs
 // the float32 error of the box arithmetic (margin m below).
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ bool cluster_visible(const GxClusterDev &c, const float *M, float fx, float fy, float znear,
-                                                float zfar) {
+// camera-space box of a cluster: centre, inflated half extents, margin m, depth range
+struct CamBox { float cx, cy, ex, ey, m, wmin, wmax; };
+
+__device__ __forceinline__ CamBox cluster_box(const GxClusterDev &c, const float *M) {
     const float hx = 0.5f * (c.bmax[0] - c.bmin[0]), hy = 0.5f * (c.bmax[1] - c.bmin[1]),
                 hz = 0.5f * (c.bmax[2] - c.bmin[2]);
     const float ox = 0.5f * (c.bmax[0] + c.bmin[0]), oy = 0.5f * (c.bmax[1] + c.bmin[1]),
@@ -739,16 +741,30 @@ __device__ __forceinline__ bool cluster_visible(const GxClusterDev &c, const flo
     const float mag = fabsf(M[0] * ox) + fabsf(M[1] * oy) + fabsf(M[2] * oz) + fabsf(M[3]) + fabsf(M[4] * ox) +
                       fabsf(M[5] * oy) + fabsf(M[6] * oz) + fabsf(M[7]) + fabsf(M[8] * ox) + fabsf(M[9] * oy) +
                       fabsf(M[10] * oz) + fabsf(M[11]) + ex + ey + ez;
-    const float m = 1e-4f * mag + 1e-5f;
-    ex += m; ey += m; ez += m;
-    const float wmax = -cz + ez, wmin = -cz - ez;
-    if (wmax < znear) return false;                 // every vertex fails w >= znear
-    if (wmin > zfar * 1.0001f + m) return false;    // every fragment has depth > zfar
-    if (fx * (cx - ex) - wmax > m) return false;    // right of the image
-    if (-fx * (cx + ex) - wmax > m) return false;   // left
-    if (fy * (cy - ey) - wmax > m) return false;    // above
-    if (-fy * (cy + ey) - wmax > m) return false;   // below
+    CamBox b;
+    b.m = 1e-4f * mag + 1e-5f;
+    b.cx = cx; b.cy = cy;
+    b.ex = ex + b.m; b.ey = ey + b.m;
+    ez += b.m;
+    b.wmax = -cz + ez;
+    b.wmin = -cz - ez;
+    return b;
+}
+
+__device__ __forceinline__ bool box_in_frustum(const CamBox &b, float fx, float fy, float znear, float zfar) {
+    const float m = b.m;
+    if (b.wmax < znear) return false;                     // every vertex fails w >= znear
+    if (b.wmin > zfar * 1.0001f + m) return false;        // every fragment has depth > zfar
+    if (fx * (b.cx - b.ex) - b.wmax > m) return false;    // right of the image
+    if (-fx * (b.cx + b.ex) - b.wmax > m) return false;   // left
+    if (fy * (b.cy - b.ey) - b.wmax > m) return false;    // above
+    if (-fy * (b.cy + b.ey) - b.wmax > m) return false;   // below
     return true;
+}
+
+__device__ __forceinline__ bool cluster_visible(const GxClusterDev &c, const float *M, float fx, float fy, float znear,
+                                                float zfar) {
+    return box_in_frustum(cluster_box(c, M), fx, fy, znear, zfar);
 }
 
 

@@ -46,9 +46,45 @@ struct PipeParams {
     float *env_mv;           // [N][K+1][12] model-view per slot
     uint32_t *env_idb;       // [N][K+1] first triangle id per slot
     uint32_t *order;         // [N] raster order of the environments
+    uint32_t *zkeys;         // [N][cap_n] float bits of max(q) of each narrow record (0 for colour slots): depth sort key
+    uint32_t *rec_order;     // [raster CTAs][cap_n] per-CTA scratch: record indices of one environment, near to far
+    int32_t depth_sort;      // raster: draw the records near to far (bucket sort by zkeys) and keep the hi-Z tiles live
+    uint32_t *cnt1;          // [N][2] record counts at the end of the occluder phase
+    float *thr;              // [N] occluder phase: clusters with wmin < thr are drawn first
+    float *hiz;              // [N][HZ_STRIDE] max depth per 8x8-pixel tile (stride 16) and per 32x32 tile (at +256)
+    unsigned long long *frames;   // [N][W*H] frame keys between the two raster phases
+    int32_t occl_pct;        // share of the frustum-visible clusters (nearest first) drawn in the occluder phase
     int32_t cap_n, cap_w;    // slots per environment
     int32_t big_slots, chunk_slots;   // raster pass B: groups above big_slots are drawn in chunks of chunk_slots
 };
+
+constexpr int HZ_STRIDE = 288;   // 16x16 tiles of 8x8 pixels, then 4x4 tiles of 32x32 pixels at +256
+
+// Occlusion test of a cluster's camera-space box against the hi-Z tiles of the occluder phase: true only if
+// every fragment the cluster can produce is strictly behind what is already drawn at every pixel it can
+// touch (so it can never win N9), which leaves the image bit-identical (N10).
+__device__ __forceinline__ bool box_occluded(const CamBox &b, const float *hz, float fx, float fy, int W, int H, float znear) {
+    if (!(b.wmin >= znear)) return false;   // reaches the near plane: no screen bound
+    const float xl = b.cx - b.ex, xh = b.cx + b.ex, yl = b.cy - b.ey, yh = b.cy + b.ey;
+    const float iw0 = 1.0f / b.wmin, iw1 = 1.0f / b.wmax;
+    const float nxl = fx * xl * (xl >= 0.0f ? iw1 : iw0), nxh = fx * xh * (xh >= 0.0f ? iw0 : iw1);
+    const float nyl = fy * yl * (yl >= 0.0f ? iw1 : iw0), nyh = fy * yh * (yh >= 0.0f ? iw0 : iw1);
+    // pixel range, padded by one pixel for the 1/256 snap and the float error of the box arithmetic
+    const float fW = (float)W, fH = (float)H;
+    const int pxl = (int)fminf(fmaxf(floorf((nxl * 0.5f + 0.5f) * fW) - 1.0f, 0.0f), fW - 1.0f);
+    const int pxh = (int)fminf(fmaxf(floorf((nxh * 0.5f + 0.5f) * fW) + 1.0f, 0.0f), fW - 1.0f);
+    const int pyl = (int)fminf(fmaxf(floorf((-nyh * 0.5f + 0.5f) * fH) - 1.0f, 0.0f), fH - 1.0f);
+    const int pyh = (int)fminf(fmaxf(floorf((-nyl * 0.5f + 0.5f) * fH) + 1.0f, 0.0f), fH - 1.0f);
+    float zmax = 0.0f;
+    if (((pxh >> 3) - (pxl >> 3) + 1) * ((pyh >> 3) - (pyl >> 3) + 1) <= 16) {
+        for (int ty = pyl >> 3; ty <= (pyh >> 3); ++ty)
+            for (int tx = pxl >> 3; tx <= (pxh >> 3); ++tx) zmax = fmaxf(zmax, hz[ty * 16 + tx]);
+    } else {
+        for (int ty = pyl >> 5; ty <= (pyh >> 5); ++ty)
+            for (int tx = pxl >> 5; tx <= (pxh >> 5); ++tx) zmax = fmaxf(zmax, hz[256 + ty * 4 + tx]);
+    }
+    return b.wmin * (1.0f - 1e-4f) > zmax;
+}
 
 struct GeomWarpSmem {
     int2 *vXY;            // [GX_VCAP]
@@ -191,6 +227,7 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                 dst[1] = make_uint4(D[1], D[2], bbw, (idb + (uint32_t)t) << 1);
                 dst[2] = make_uint4(__float_as_uint(q[0]), __float_as_uint(q[1]), __float_as_uint(q[2]), col[0]);
                 dst[3] = make_uint4(col[1], col[2], 0u, 0u);
+                PP.zkeys[(size_t)env * PP.cap_n + base + (uint32_t)g] = good ? __float_as_uint(fmaxf(q[0], fmaxf(q[1], q[2]))) : 0u;
             }
         }
     }
@@ -263,7 +300,10 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                 uint32_t E0[3], D[3], bbw;
                 bool swapped;
                 narrow_setup(tri.X, tri.Y, tri.q, i0, i1, j0, j1, E0, D, bbw, swapped);   // already normalised: no swap
-                uint4 *dst = env_recs + (size_t)(bn + 2u * (uint32_t)__popc(mn & lt)) * 4;
+                const uint32_t slot = bn + 2u * (uint32_t)__popc(mn & lt);
+                uint4 *dst = env_recs + (size_t)slot * 4;
+                PP.zkeys[(size_t)env * PP.cap_n + slot] = __float_as_uint(fmaxf(tri.q[0], fmaxf(tri.q[1], tri.q[2])));
+                PP.zkeys[(size_t)env * PP.cap_n + slot + 1] = 0u;
                 dst[0] = make_uint4(E0[0], E0[1], E0[2], D[0]);
                 dst[1] = make_uint4(D[1], D[2], bbw | BB_FLOATCOL, tri.id2);
                 dst[2] = make_uint4(__float_as_uint(tri.q[0]), __float_as_uint(tri.q[1]), __float_as_uint(tri.q[2]), 0u);
@@ -288,11 +328,15 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
 namespace gx {
 
 // ------------------------------------------------------------------------------------------------
-// K1: the cull kernel.  One CTA per environment: slot tables, model-view matrices (N1, N2) and id bases go to
-// the environment table in global memory; every cluster AABB of the environment is tested against the
+// K1: the cull kernel.  One CTA per environment: every cluster AABB of the environment is tested against the
 // frustum and the batches of the survivors are appended to the chunk-wide work list (warp-aggregated atomics).
+//   PHASE 1  writes the environment table (model-view matrices N1/N2, id bases), and, when the occluder
+//            phase is on (occl_pct < 100), keeps only the nearest occl_pct % of the visible clusters: a
+//            256-bin histogram of the boxes' wmin gives the threshold thr[env]; clusters with wmin < thr go.
+//   PHASE 2  takes the other visible clusters and drops those that the hi-Z tiles left by the first raster
+//            phase prove hidden (box_occluded).
 // ------------------------------------------------------------------------------------------------
-template <int WARPS, bool STATS>
+template <int WARPS, int PHASE, bool STATS>
 __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
     extern __shared__ __align__(16) unsigned char smem[];
     const GxParams &P = PP.g;
@@ -311,28 +355,98 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
     es.slot_nt = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
     es.slot_nc = reinterpret_cast<uint32_t *>(p);  p += (size_t)(K + 1) * 4;
     es.work = nullptr;
+    __shared__ unsigned s_hist[256];
+    __shared__ float s_hz[HZ_STRIDE];
+    __shared__ float s_thr;
 
+    if (PHASE == 2 && PP.env_flag[env]) return;   // overflowed in the occluder phase: single-kernel pass
     env_setup(P, env, es, tid);
-    float *g_mv = PP.env_mv + (size_t)env * (size_t)(K + 1) * 12;
-    uint32_t *g_idb = PP.env_idb + (size_t)env * (size_t)(K + 1);
-    for (int k = tid; k < (K + 1) * 12; k += NT) g_mv[k] = es.MV[k];
-    for (int k = tid; k <= K; k += NT) g_idb[k] = es.id_base[k];
+    if (PHASE == 1) {
+        float *g_mv = PP.env_mv + (size_t)env * (size_t)(K + 1) * 12;
+        uint32_t *g_idb = PP.env_idb + (size_t)env * (size_t)(K + 1);
+        for (int k = tid; k < (K + 1) * 12; k += NT) g_mv[k] = es.MV[k];
+        for (int k = tid; k <= K; k += NT) g_idb[k] = es.id_base[k];
+    }
+    const uint32_t n_cl = es.cl_base[K + 1];
+    const bool two_phase = P.cull && PP.occl_pct < 100;
+
+    auto slot_of = [&](uint32_t g) {
+        int lo = 0, hi = K;
+        while (lo < hi) {   // largest slot whose first cluster index is <= g
+            const int mid = (lo + hi + 1) >> 1;
+            if (es.cl_base[mid] <= g) lo = mid; else hi = mid - 1;
+        }
+        return (uint32_t)lo;
+    };
+
+    float thr = 3.0e38f;
+    if (PHASE == 1 && two_phase) {
+        for (int k = tid; k < 256; k += NT) s_hist[k] = 0;
+        __syncthreads();
+        const float inv_bin = 256.0f / P.zfar;
+        for (uint32_t g = tid; g < n_cl; g += NT) {
+            const uint32_t s = slot_of(g);
+            const CamBox b = cluster_box(P.clusters[es.slot_cl[s] + (g - es.cl_base[s])], es.MV + s * 12);
+            if (box_in_frustum(b, P.fx, P.fy, P.znear, P.zfar))
+                atomicAdd(&s_hist[(int)fminf(fmaxf(b.wmin * inv_bin, 0.0f), 255.0f)], 1u);
+        }
+        __syncthreads();
+        if (warp == 0) {   // smallest bin edge below which at least occl_pct % of the visible clusters lie
+            unsigned v[8], sum = 0;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) { v[k] = s_hist[lane * 8 + k]; sum += v[k]; }
+            unsigned inc = sum;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned a = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+                if (lane >= d) inc += a;
+            }
+            const unsigned total = __shfl_sync(0xFFFFFFFFu, inc, 31);
+            const unsigned want = (total * (unsigned)PP.occl_pct + 99u) / 100u;
+            unsigned run = inc - sum;
+            int bin = 256;
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+                run += v[k];
+                if (bin == 256 && run >= want) bin = lane * 8 + k;
+            }
+#pragma unroll
+            for (int d = 16; d; d >>= 1) bin = min(bin, __shfl_xor_sync(0xFFFFFFFFu, bin, d));
+            if (lane == 0) {
+                s_thr = (float)(bin + 1) * (P.zfar / 256.0f);
+                PP.thr[env] = s_thr;
+            }
+        }
+        __syncthreads();
+        thr = s_thr;
+    }
+    if (PHASE == 2) {
+        thr = PP.thr[env];
+        for (int k = tid; k < HZ_STRIDE; k += NT) s_hz[k] = PP.hiz[(size_t)env * HZ_STRIDE + k];
+        __syncthreads();
+    }
 
     unsigned st_tested = 0, st_drawn = 0;
-    const uint32_t n_cl = es.cl_base[K + 1];
     for (uint32_t g0 = warp * 32; g0 < n_cl; g0 += NT) {
         const uint32_t g = g0 + lane;
         uint32_t nb = 0, boff = 0, s = 0;
         if (g < n_cl) {
-            int lo = 0, hi = K;
-            while (lo < hi) {   // largest slot whose first cluster index is <= g
-                const int mid = (lo + hi + 1) >> 1;
-                if (es.cl_base[mid] <= g) lo = mid; else hi = mid - 1;
-            }
-            s = (uint32_t)lo;
+            s = slot_of(g);
             const GxClusterDev c = P.clusters[es.slot_cl[s] + (g - es.cl_base[s])];
-            const bool vis = !P.cull || cluster_visible(c, es.MV + s * 12, P.fx, P.fy, P.znear, P.zfar);
-            if (STATS) { ++st_tested; st_drawn += vis ? 1u : 0u; }
+            bool vis = true;
+            if (P.cull) {
+                const CamBox b = cluster_box(c, es.MV + s * 12);
+                vis = box_in_frustum(b, P.fx, P.fy, P.znear, P.zfar);
+                if (PHASE == 1) {
+                    if (STATS) { ++st_tested; st_drawn += vis ? 1u : 0u; }
+                    vis = vis && b.wmin < thr;
+                } else {
+                    const bool cand = vis && !(b.wmin < thr);
+                    const bool occ = cand && box_occluded(b, s_hz, P.fx, P.fy, P.W, P.H, P.znear);
+                    if (STATS) st_tested += occ ? 1u : 0u;   // (PHASE 2: st_tested counts the clusters proved hidden)
+                    vis = cand && !occ;
+                }
+            } else if (STATS) { ++st_tested; ++st_drawn; }
             if (vis) { nb = c.nbatch; boff = c.batch_off; }
         }
         uint32_t inc = nb;
@@ -354,8 +468,12 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
             st_drawn += __shfl_xor_sync(0xFFFFFFFFu, st_drawn, d);
         }
         if (lane == 0) {
-            atomicAdd(&P.stats[GX_STAT_CLUSTERS_TESTED], (unsigned long long)st_tested);
-            atomicAdd(&P.stats[GX_STAT_CLUSTERS_DRAWN], (unsigned long long)st_drawn);
+            if (PHASE == 1) {
+                atomicAdd(&P.stats[GX_STAT_CLUSTERS_TESTED], (unsigned long long)st_tested);
+                atomicAdd(&P.stats[GX_STAT_CLUSTERS_DRAWN], (unsigned long long)st_drawn);
+            } else {
+                atomicAdd(&P.stats[GX_STAT_CLUSTERS_OCCLUDED], (unsigned long long)st_tested);
+            }
         }
     }
 }
@@ -414,14 +532,18 @@ __global__ void __launch_bounds__(WARPS * 32, 1024 / (WARPS * 32)) geom_kernel(c
 // raster order: environments sorted by record count, heaviest first (one CTA, counting sort in 256 bins), so
 // that the persistent raster CTAs finish together.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(1024) order_kernel(const PipeParams PP) {
+__global__ void __launch_bounds__(1024) order_kernel(const PipeParams PP, const int since_phase1) {
     __shared__ unsigned hist[256];
     const int tid = threadIdx.x, N = PP.g.N;
+    auto cost = [&](int e) {
+        unsigned n = PP.cnt[2 * e], w = PP.cnt[2 * e + 1];
+        if (since_phase1) { n -= PP.cnt1[2 * e]; w -= PP.cnt1[2 * e + 1]; }
+        return n + 4u * w;
+    };
     if (tid < 256) hist[tid] = 0;
     __syncthreads();
     for (int e = tid; e < N; e += 1024) {
-        const unsigned tot = PP.cnt[2 * e] + 4u * PP.cnt[2 * e + 1];
-        atomicAdd(&hist[255u - min(255u, tot >> 7)], 1u);
+        atomicAdd(&hist[255u - min(255u, cost(e) >> 7)], 1u);
     }
     __syncthreads();
     if (tid < 32) {   // exclusive scan of the 256 bins by one warp, 8 bins per lane
@@ -440,8 +562,7 @@ __global__ void __launch_bounds__(1024) order_kernel(const PipeParams PP) {
     }
     __syncthreads();
     for (int e = tid; e < N; e += 1024) {
-        const unsigned tot = PP.cnt[2 * e] + 4u * PP.cnt[2 * e + 1];
-        PP.order[atomicAdd(&hist[255u - min(255u, tot >> 7)], 1u)] = (uint32_t)e;
+        PP.order[atomicAdd(&hist[255u - min(255u, cost(e) >> 7)], 1u)] = (uint32_t)e;
     }
 }
 
@@ -451,9 +572,11 @@ __global__ void __launch_bounds__(1024) order_kernel(const PipeParams PP) {
 struct RastWarpSmem {
     uint32_t *rec;   // [REC_WORDS * 32] SoA records of the current group (layout of gx_kernels.cuh R_*)
     uint32_t *fq;    // [FQ_CAP] covered fragments: r | (x - i0) << 5 | (y - j0) << 12
+    uint32_t *ridx;  // [32] slot index of each record of the group (the low half of the frame key)
 };
-constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4;
-constexpr int BIG_CAP = 768;       // entries of the pass-B list
+constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4 + 32 * 4;
+constexpr int BIG_CAP = 512;       // entries of the pass-B list
+constexpr int ZBINS = 128;         // depth buckets of the raster order (8 per octave of max(q))
 
 __host__ __device__ inline size_t raster_smem_bytes(int W, int H, int warps) {
     return (size_t)W * H * 8 + (size_t)warps * RAST_WARP_SMEM;
@@ -480,9 +603,13 @@ __device__ __forceinline__ void key_min_rec(unsigned long long *slot, uint32_t d
 }
 
 // load the group's records (one per lane) into the warp's SoA staging
-__device__ __forceinline__ void load_group(const RastWarpSmem &ws, const uint4 *env_recs, uint32_t first, int nrec, int lane) {
+// (record `base + order[pos + lane]` when an order list is given, else record `base + pos + lane`)
+__device__ __forceinline__ void load_group(const RastWarpSmem &ws, const uint4 *env_recs, uint32_t base, const uint32_t *order,
+                                           uint32_t pos, int nrec, int lane) {
     if (lane < nrec) {
-        const uint4 *rp = env_recs + (size_t)(first + (uint32_t)lane) * 4;
+        const uint32_t idx = base + (order ? order[pos + (uint32_t)lane] : pos + (uint32_t)lane);
+        ws.ridx[lane] = idx;
+        const uint4 *rp = env_recs + (size_t)idx * 4;
         const uint4 u0 = __ldg(rp), u1 = __ldg(rp + 1), u2 = __ldg(rp + 2);
         ws.rec[(R_E0 + 0) * 32 + lane] = u0.x;
         ws.rec[(R_E0 + 1) * 32 + lane] = u0.y;
@@ -502,39 +629,65 @@ __device__ __forceinline__ void load_group(const RastWarpSmem &ws, const uint4 *
 
 // K4b: depth (N7) and resolve (N9) for the queued fragments, one per lane
 __device__ __forceinline__ void shade_queue_p(const RastWarpSmem &ws, int qn, int W, float zfar, unsigned long long *fb,
-                                              uint32_t first, const uint4 *env_recs, int lane) {
+                                              const uint4 *env_recs, int lane) {
     for (int f = lane; f < qn; f += 32) {
         const uint32_t en = ws.fq[f];
         const int r = (int)(en & 31u), a = (int)((en >> 5) & 127u), b = (int)((en >> 12) & 127u);
         const uint32_t bb = ws.rec[R_BB * 32 + r];
-        float fe[3], q[3];
+        const int x = (int)(bb & 127u) + a, y = (int)((bb >> 7) & 127u) + b;
+        unsigned long long *slot = &fb[fb_index(x, y, W)];
+        float q[3];
+#pragma unroll
+        for (int e = 0; e < 3; ++e) q[e] = __uint_as_float(ws.rec[(R_Q0 + e) * 32 + r]);
+        // early z: every depth of the triangle is >= 1/max(q); behind the stored depth with margin -> cannot win
+        // (the stored depth of a background pixel reads as NaN: the comparison is false)
+        const float stored = __uint_as_float(reinterpret_cast<volatile uint32_t *>(slot)[1]);
+        if (fmaxf(q[0], fmaxf(q[1], q[2])) * stored < 1.0f - 1e-5f) continue;
+        float fe[3];
 #pragma unroll
         for (int e = 0; e < 3; ++e) {
             const uint32_t d = ws.rec[(R_D0 + e) * 32 + r];
             const int dx = (int)d >> 16, dy = (int)(short)(d & 0xFFFFu);
             const int Ee = (int)ws.rec[(R_E0 + e) * 32 + r] + ((b * dx - a * dy) << 8);
             fe[e] = (float)Ee;
-            q[e] = __uint_as_float(ws.rec[(R_Q0 + e) * 32 + r]);
         }
         const float num = fmaf(fe[2], q[2], fmaf(fe[1], q[1], fe[0] * q[0]));
         const float depth = __uint_as_float(ws.rec[R_FA * 32 + r]) / num;
         if (depth > zfar) continue;
-        const int x = (int)(bb & 127u) + a, y = (int)((bb >> 7) & 127u) + b;
-        key_min_rec(&fb[fb_index(x, y, W)], __float_as_uint(depth), first + (uint32_t)r, ws.rec[R_ID * 32 + r], env_recs);
+        key_min_rec(slot, __float_as_uint(depth), ws.ridx[r], ws.rec[R_ID * 32 + r], env_recs);
     }
     __syncwarp();
 }
 
 // K3: the bounding boxes of the group's records are cut into slots of 4 pixels of one row.  group_slots returns
 // the lane's exclusive prefix of slot counts (Pex, record = lane) and the group's total T.
-__device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int lane, int &Pex) {
+// With hz != NULL (second raster phase) a record whose nearest vertex is strictly behind the hi-Z value of
+// every 8x8 tile its bounding box touches gets no slots: none of its fragments could win N9.
+__device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int lane, const float *hz, int &Pex,
+                                           unsigned &skip, unsigned &n_culled) {
     const unsigned FULL = 0xFFFFFFFFu;
     int ns = 0;
+    bool culled = false;
     if (lane < nrec) {
         const uint32_t bb = ws.rec[R_BB * 32 + lane];
         const int w = (int)((bb >> 14) & 127u) + 1, h = (int)((bb >> 21) & 127u) + 1;
         ns = h * ((w + 3) >> 2);
+        if (hz) {
+            const int i0 = (int)(bb & 127u), j0 = (int)((bb >> 7) & 127u);
+            const int tx0 = i0 >> 3, tx1 = (i0 + w - 1) >> 3, ty0 = j0 >> 3, ty1 = (j0 + h - 1) >> 3;
+            if ((tx1 - tx0 + 1) * (ty1 - ty0 + 1) <= 6) {
+                float zmax = 0.0f;
+                for (int ty = ty0; ty <= ty1; ++ty)
+                    for (int tx = tx0; tx <= tx1; ++tx) zmax = fmaxf(zmax, hz[ty * 16 + tx]);
+                const float qmax = fmaxf(__uint_as_float(ws.rec[(R_Q0 + 0) * 32 + lane]),
+                                         fmaxf(__uint_as_float(ws.rec[(R_Q0 + 1) * 32 + lane]),
+                                               __uint_as_float(ws.rec[(R_Q0 + 2) * 32 + lane])));
+                // every depth of the triangle is >= 1/qmax (N7, up to a few ulp): hidden iff 1/qmax > zmax with margin
+                if (qmax * zmax < 1.0f - 1e-5f) { ns = 0; culled = true; ++n_culled; }
+            }
+        }
     }
+    skip = __ballot_sync(FULL, culled);   // records without slots: the slot walk steps over them
     int inc = ns;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -550,8 +703,8 @@ __device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int
 // lanes stay busy whatever the mix of triangle sizes.  The covered pixels of one pass are appended to the
 // fragment queue with four ballots and shaded densely by shade_queue_p.
 template <bool STATS>
-__device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, int S0, int S1, int W, float zfar,
-                                             unsigned long long *fb, uint32_t first, const uint4 *env_recs, int lane,
+__device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, unsigned skip, int S0, int S1, int W, float zfar,
+                                             unsigned long long *fb, const uint4 *env_recs, int lane,
                                              unsigned &n_frag) {
     const unsigned FULL = 0xFFFFFFFFu;
     const unsigned lt = (1u << lane) - 1u;
@@ -623,7 +776,7 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, in
                 chunk = 0;
                 if (++row == h) {
                     row = 0;
-                    ++r;
+                    r = (__ffs((int)(~skip & ~((2u << r) - 1u))) - 1) & 31;   // next record that has slots
                     if (it + 1 < n) load_rec(r);
                 }
             }
@@ -631,14 +784,14 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, in
         if (qn > FQ_CAP - 128) {
             __syncwarp();
             if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
-            shade_queue_p(ws, qn, W, zfar, fb, first, env_recs, lane);
+            shade_queue_p(ws, qn, W, zfar, fb, env_recs, lane);
             qn = 0;
         }
     }
     __syncwarp();
     if (qn) {
         if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
-        shade_queue_p(ws, qn, W, zfar, fb, first, env_recs, lane);
+        shade_queue_p(ws, qn, W, zfar, fb, env_recs, lane);
     }
 }
 
@@ -748,9 +901,12 @@ __device__ __forceinline__ uint32_t resolve_rec(const uint4 *env_recs, uint32_t 
 
 
 // ------------------------------------------------------------------------------------------------
-// the raster kernel
+// the raster kernel.  PHASE 0: draw all records of the environment and write the images.  PHASE 1 (occluder
+// phase): draw the records present so far, then leave the frame keys, the hi-Z tiles and the record counts
+// in global memory.  PHASE 2: start from those keys, draw only the records appended since, skipping records
+// the hi-Z tiles prove hidden, and write the images.
 // ------------------------------------------------------------------------------------------------
-template <int WARPS, int MINB, bool STATS>
+template <int WARPS, int MINB, int PHASE, bool STATS>
 __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipeParams PP) {
     extern __shared__ __align__(16) unsigned char smem[];
     const GxParams &P = PP.g;
@@ -762,21 +918,28 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     RastWarpSmem ws;
     ws.rec = reinterpret_cast<uint32_t *>(smem + (size_t)npix * 8 + (size_t)warp * RAST_WARP_SMEM);
     ws.fq = ws.rec + REC_WORDS * 32;
+    ws.ridx = ws.fq + FQ_CAP;
 
     __shared__ int s_env;
     __shared__ unsigned s_next, s_next_b, s_big;
     __shared__ uint2 s_big_list[BIG_CAP];   // (group, first chunk) of the groups left to pass B
-    __shared__ unsigned long long s_frag;
+    __shared__ float s_hz[HZ_STRIDE];
+    __shared__ unsigned s_bin[ZBINS];
+    __shared__ unsigned long long s_frag, s_culled;
 
-    unsigned st_frag = 0;
-    if (STATS && tid == 0) s_frag = 0;
-    {
+    unsigned st_frag = 0, st_culled = 0;
+    if (STATS && tid == 0) { s_frag = 0; s_culled = 0; }
+    const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+    if (PHASE != 2) {
         uint4 *f4 = reinterpret_cast<uint4 *>(fb);
-        const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
         for (int k = tid; k < npix / 2; k += NT) f4[k] = ones;
     }
     const bool want_rgb = P.rgb != nullptr;
     const uint32_t cap_n = (uint32_t)PP.cap_n;
+    const bool sorted = PP.depth_sort != 0;
+    const float *hz = (PHASE == 2 || sorted) ? s_hz : nullptr;
+    uint32_t *my_order = PP.rec_order + (size_t)blockIdx.x * (size_t)PP.cap_n;
+    const uint32_t qfar = __float_as_uint(1.0f / P.zfar) >> 20;
 
     for (;;) {
         if (tid == 0) {
@@ -793,42 +956,96 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
         }
         const uint4 *env_recs = PP.recs + (size_t)env * (size_t)(PP.cap_n + PP.cap_w) * 4;
         const uint32_t n_n = PP.cnt[2 * env], n_w = PP.cnt[2 * env + 1] >> 1;
-        const uint32_t g_n = (n_n + 31u) >> 5, g_w = (n_w + 31u) >> 5;
+        const uint32_t b_n = PHASE == 2 ? PP.cnt1[2 * env] : 0u, b_w = PHASE == 2 ? PP.cnt1[2 * env + 1] >> 1 : 0u;
+        const uint32_t g_n = (n_n - b_n + 31u) >> 5, g_w = (n_w - b_w + 31u) >> 5;
+        if (PHASE == 2) {   // the occluder phase's frame and hi-Z tiles
+            const uint4 *src = reinterpret_cast<const uint4 *>(PP.frames + (size_t)env * npix);
+            uint4 *f4 = reinterpret_cast<uint4 *>(fb);
+            for (int k = tid; k < npix / 2; k += NT) f4[k] = __ldg(src + k);
+            for (int k = tid; k < HZ_STRIDE; k += NT) s_hz[k] = PP.hiz[(size_t)env * HZ_STRIDE + k];
+        } else if (sorted) {
+            for (int k = tid; k < HZ_STRIDE; k += NT) s_hz[k] = __int_as_float(0x7F800000);
+        }
+        if (sorted) {
+            // bucket sort of the environment's narrow records by nearest depth (8 buckets per octave of max(q)):
+            // my_order[] lists them near to far; the order inside a bucket is arbitrary, the image does not depend on it
+            const uint32_t *zk = PP.zkeys + (size_t)env * PP.cap_n + b_n;
+            const uint32_t n = n_n - b_n;
+            for (int k = tid; k < ZBINS; k += NT) s_bin[k] = 0;
+            __syncthreads();
+            auto bin_of = [&](uint32_t key) {
+                const int d = (int)(key >> 20) - (int)qfar;
+                return (ZBINS - 1) - min(max(d, 0), ZBINS - 1);
+            };
+            for (uint32_t k = tid; k < n; k += NT) atomicAdd(&s_bin[bin_of(__ldg(zk + k))], 1u);
+            __syncthreads();
+            if (warp == 0) {   // exclusive scan of the ZBINS counts, ZBINS / 32 per lane
+                unsigned v[ZBINS / 32], sum = 0;
+#pragma unroll
+                for (int k = 0; k < ZBINS / 32; ++k) { v[k] = s_bin[lane * (ZBINS / 32) + k]; sum += v[k]; }
+                unsigned inc = sum;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const unsigned a = __shfl_up_sync(0xFFFFFFFFu, inc, d);
+                    if (lane >= d) inc += a;
+                }
+                unsigned run = inc - sum;
+#pragma unroll
+                for (int k = 0; k < ZBINS / 32; ++k) { s_bin[lane * (ZBINS / 32) + k] = run; run += v[k]; }
+            }
+            __syncthreads();
+            for (uint32_t k = tid; k < n; k += NT) my_order[atomicAdd(&s_bin[bin_of(__ldg(zk + k))], 1u)] = k;
+        }
+        if (PHASE == 2 || sorted) __syncthreads();
+        const uint32_t *order = sorted ? my_order : nullptr;
 
         // ---- K3 + K4, pass A: groups of 32 records, drawn dynamically by the warps.  A group of more than
-        // BIG_SLOTS slots is only registered: (list index, first chunk) come from one packed atomic, so the
+        // big_slots slots is only registered: (list index, first chunk) come from one packed atomic, so the
         // list is ordered by first chunk.
         for (;;) {
             unsigned g = 0;
             if (lane == 0) g = atomicAdd(&s_next, 1u);
             g = __shfl_sync(0xFFFFFFFFu, g, 0);
             if (g >= g_n + g_w) break;
-            if (g < g_n) {
-                const uint32_t first = g * 32u;
-                const int nrec = (int)min(32u, n_n - first);
-                load_group(ws, env_recs, first, nrec, lane);
+            if (sorted) {   // keep the hi-Z tiles live: every draw recomputes 8 of them from the frame (a stale
+                            // value is a valid bound: depths only decrease)
+                const int tw = W >> 3, nt = tw * (H >> 3);
+                for (int k = 0; k < 8; ++k) {
+                    const int t = (int)((g * 8u + (unsigned)k) % (unsigned)nt);
+                    const int ty = t / tw, tx = t - ty * tw;
+                    const int j = ty * 8 + (lane >> 2), i = tx * 8 + (lane & 3) * 2;
+                    const volatile unsigned long long *kp = &fb[fb_index(i, j, W)];
+                    const unsigned d = __reduce_max_sync(0xFFFFFFFFu, max((unsigned)(kp[0] >> 32), (unsigned)(kp[1] >> 32)));
+                    if (lane == 0) s_hz[ty * 16 + tx] = d == 0xFFFFFFFFu ? __int_as_float(0x7F800000) : __uint_as_float(d);
+                }
+            }
+            if (g >= g_w) {
+                const uint32_t pos = (g - g_w) * 32u;
+                const int nrec = (int)min(32u, n_n - b_n - pos);
+                load_group(ws, env_recs, b_n, order, pos, nrec, lane);
                 int Pex;
-                const int T = group_slots(ws, nrec, lane, Pex);
+                unsigned skip;
+                const int T = group_slots(ws, nrec, lane, hz, Pex, skip, st_culled);
                 if (T <= PP.big_slots) {
-                    raster_slots<STATS>(ws, Pex, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
+                    if (T) raster_slots<STATS>(ws, Pex, skip, 0, T, W, P.zfar, fb, env_recs, lane, st_frag);
                 } else {
                     unsigned full = 0;
                     if (lane == 0) {
                         const unsigned nch = (unsigned)(T + PP.chunk_slots - 1) / (unsigned)PP.chunk_slots;
                         const unsigned old = atomicAdd(&s_big, (1u << 20) | nch);
-                        if ((old >> 20) < (unsigned)BIG_CAP) s_big_list[old >> 20] = make_uint2(g, old & 0xFFFFFu);
+                        if ((old >> 20) < (unsigned)BIG_CAP) s_big_list[old >> 20] = make_uint2(g - g_w, old & 0xFFFFFu);
                         else full = 1;
                     }
                     if (__shfl_sync(0xFFFFFFFFu, full, 0))   // list full: draw the group here, whole
-                        raster_slots<STATS>(ws, Pex, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
+                        raster_slots<STATS>(ws, Pex, skip, 0, T, W, P.zfar, fb, env_recs, lane, st_frag);
                 }
-            } else {
-                const uint32_t t0 = (g - g_n) * 32u;
+            } else {   // wide records first: they reach the near plane and hide the most
+                const uint32_t t0 = b_w + g * 32u;
                 raster_wide<STATS>(env_recs, cap_n + 2u * t0, (int)min(32u, n_w - t0), W, H, P.zfar, fb, lane, st_frag);
             }
         }
         __syncthreads();
-        // ---- pass B: the big groups, in chunks of CHUNK_SLOTS slots drawn dynamically ----------------
+        // ---- pass B: the big groups, in chunks of chunk_slots slots drawn dynamically -----------------
         {
             const unsigned packed = s_big;
             const unsigned n_big = min(packed >> 20, (unsigned)BIG_CAP), n_chunks = packed & 0xFFFFFu;
@@ -843,62 +1060,90 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                     if (s_big_list[mid].y <= c) lo = mid; else hi = mid - 1;
                 }
                 const uint2 en = s_big_list[lo];
-                const uint32_t first = en.x * 32u;
-                const int nrec = (int)min(32u, n_n - first);
-                load_group(ws, env_recs, first, nrec, lane);
+                const uint32_t pos = en.x * 32u;
+                const int nrec = (int)min(32u, n_n - b_n - pos);
+                load_group(ws, env_recs, b_n, order, pos, nrec, lane);
                 int Pex;
-                const int T = group_slots(ws, nrec, lane, Pex);
+                unsigned skip, dummy = 0;
+                const int T = group_slots(ws, nrec, lane, hz, Pex, skip, dummy);
                 const int S0 = (int)(c - en.y) * PP.chunk_slots;   // chunks of entries a full list dropped land beyond T
-                if (S0 < T) raster_slots<STATS>(ws, Pex, S0, min(T, S0 + PP.chunk_slots), W, P.zfar, fb, first, env_recs, lane, st_frag);
+                if (S0 < T) raster_slots<STATS>(ws, Pex, skip, S0, min(T, S0 + PP.chunk_slots), W, P.zfar, fb, env_recs, lane, st_frag);
             }
         }
         __syncthreads();
 
-        // ---- K5: resolve the winners, write RGB / depth / id as 16-byte stores, reset the frame ------
-        for (int k = tid; k < npix / 4; k += NT) {
-            const int pix = k * 4;
-            const int j = pix / W, i = pix - j * W;
-            const int a = fb_index(i, j, W);          // 4-aligned columns stay contiguous under the XOR
-            uint4 *slot = reinterpret_cast<uint4 *>(&fb[a]);
-            const uint4 v0 = slot[0], v1 = slot[1];
-            const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
-            slot[0] = ones;
-            slot[1] = ones;
-            const uint32_t idx[4] = {v0.x, v0.z, v1.x, v1.z};
-            const uint32_t db[4] = {v0.y, v0.w, v1.y, v1.w};
-            uint32_t col[4], id[4];
-            float4 d;
-            float *dp = &d.x;
-#pragma unroll
-            for (int m = 0; m < 4; ++m) {
-                col[m] = 0u;
-                id[m] = 0xFFFFFFFFu;
-                dp[m] = 0.0f;
-                if (db[m] != 0xFFFFFFFFu) {
-                    dp[m] = __uint_as_float(db[m]);
-                    if (want_rgb || P.id) col[m] = resolve_rec(env_recs, cap_n, idx[m], i + m, j, want_rgb, id[m]);
-                }
+        if (PHASE == 1) {
+            // ---- occluder phase: hi-Z tiles (max depth per 8x8 tile, +inf where background shows), the frame
+            // keys and the record counts go to global memory; the frame is reset for the next environment
+            const int tw = W >> 3, th = H >> 3;
+            for (int t = warp; t < tw * th; t += WARPS) {
+                const int ty = t / tw, tx = t - ty * tw;
+                const int j = ty * 8 + (lane >> 2), i = tx * 8 + (lane & 3) * 2;
+                const uint4 v = *reinterpret_cast<const uint4 *>(&fb[fb_index(i, j, W)]);   // two keys: depth bits in .y, .w
+                unsigned d = max(v.y, v.w);
+                d = __reduce_max_sync(0xFFFFFFFFu, d);
+                if (lane == 0) s_hz[ty * 16 + tx] = d == 0xFFFFFFFFu ? __int_as_float(0x7F800000) : __uint_as_float(d);
             }
-            *reinterpret_cast<float4 *>(P.depth + (size_t)env * npix + pix) = d;
-            if (P.id) *reinterpret_cast<uint4 *>(P.id + (size_t)env * npix + pix) = make_uint4(id[0], id[1], id[2], id[3]);
-            if (want_rgb) {
-                // 4 pixels = 12 bytes = 3 words per lane; 4 lanes hold 48 bytes = three 16-byte stores
-                const uint32_t w0 = (col[0] & 0xFFFFFFu) | (col[1] << 24);
-                const uint32_t w1 = ((col[1] >> 8) & 0xFFFFu) | (col[2] << 16);
-                const uint32_t w2 = ((col[2] >> 16) & 0xFFu) | (col[3] << 8);
-                const int g = lane & 3, gb = lane & ~3;
-                uint32_t o[4];
-#pragma unroll
-                for (int r = 0; r < 4; ++r) {
-                    const int m = 4 * g + r;          // word of the group's 12-word stream (g < 3)
-                    const int src = gb + (m / 3) % 4, wsel = m % 3;
-                    const uint32_t a0 = __shfl_sync(0xFFFFFFFFu, w0, src), a1 = __shfl_sync(0xFFFFFFFFu, w1, src),
-                                   a2 = __shfl_sync(0xFFFFFFFFu, w2, src);
-                    o[r] = wsel == 0 ? a0 : (wsel == 1 ? a1 : a2);
+            for (int t = tid; t < 16; t += NT) s_hz[256 + t] = 0.0f;
+            __syncthreads();
+            if (tid < 16) {   // 32x32-pixel tiles: max over 4x4 of the above (tiles outside the frame count as 0)
+                const int by = tid >> 2, bx = tid & 3;
+                float z = 0.0f;
+                for (int ty = by * 4; ty < min(by * 4 + 4, th); ++ty)
+                    for (int tx = bx * 4; tx < min(bx * 4 + 4, tw); ++tx) z = fmaxf(z, s_hz[ty * 16 + tx]);
+                s_hz[256 + tid] = z;
+            }
+            __syncthreads();
+            for (int k = tid; k < HZ_STRIDE; k += NT) PP.hiz[(size_t)env * HZ_STRIDE + k] = s_hz[k];
+            uint4 *dst = reinterpret_cast<uint4 *>(PP.frames + (size_t)env * npix);
+            uint4 *f4 = reinterpret_cast<uint4 *>(fb);
+            for (int k = tid; k < npix / 2; k += NT) { dst[k] = f4[k]; f4[k] = ones; }
+            if (tid < 2) PP.cnt1[2 * env + tid] = PP.cnt[2 * env + tid];
+        } else {
+            // ---- K5: resolve the winners, write RGB / depth / id as 16-byte stores, reset the frame ------
+            for (int k = tid; k < npix / 4; k += NT) {
+                const int pix = k * 4;
+                const int j = pix / W, i = pix - j * W;
+                const int a = fb_index(i, j, W);          // 4-aligned columns stay contiguous under the XOR
+                uint4 *slot = reinterpret_cast<uint4 *>(&fb[a]);
+                const uint4 v0 = slot[0], v1 = slot[1];
+                if (PHASE == 0) { slot[0] = ones; slot[1] = ones; }   // (PHASE 2 reloads the frame per environment)
+                const uint32_t idx[4] = {v0.x, v0.z, v1.x, v1.z};
+                const uint32_t db[4] = {v0.y, v0.w, v1.y, v1.w};
+                uint32_t col[4], id[4];
+                float4 d;
+                float *dp = &d.x;
+    #pragma unroll
+                for (int m = 0; m < 4; ++m) {
+                    col[m] = 0u;
+                    id[m] = 0xFFFFFFFFu;
+                    dp[m] = 0.0f;
+                    if (db[m] != 0xFFFFFFFFu) {
+                        dp[m] = __uint_as_float(db[m]);
+                        if (want_rgb || P.id) col[m] = resolve_rec(env_recs, cap_n, idx[m], i + m, j, want_rgb, id[m]);
+                    }
                 }
-                if (g < 3) {
-                    uint8_t *dst = P.rgb + ((size_t)env * npix + (size_t)(pix - 4 * g)) * 3 + 16 * g;
-                    *reinterpret_cast<uint4 *>(dst) = make_uint4(o[0], o[1], o[2], o[3]);
+                *reinterpret_cast<float4 *>(P.depth + (size_t)env * npix + pix) = d;
+                if (P.id) *reinterpret_cast<uint4 *>(P.id + (size_t)env * npix + pix) = make_uint4(id[0], id[1], id[2], id[3]);
+                if (want_rgb) {
+                    // 4 pixels = 12 bytes = 3 words per lane; 4 lanes hold 48 bytes = three 16-byte stores
+                    const uint32_t w0 = (col[0] & 0xFFFFFFu) | (col[1] << 24);
+                    const uint32_t w1 = ((col[1] >> 8) & 0xFFFFu) | (col[2] << 16);
+                    const uint32_t w2 = ((col[2] >> 16) & 0xFFu) | (col[3] << 8);
+                    const int g = lane & 3, gb = lane & ~3;
+                    uint32_t o[4];
+    #pragma unroll
+                    for (int r = 0; r < 4; ++r) {
+                        const int m = 4 * g + r;          // word of the group's 12-word stream (g < 3)
+                        const int src = gb + (m / 3) % 4, wsel = m % 3;
+                        const uint32_t a0 = __shfl_sync(0xFFFFFFFFu, w0, src), a1 = __shfl_sync(0xFFFFFFFFu, w1, src),
+                                       a2 = __shfl_sync(0xFFFFFFFFu, w2, src);
+                        o[r] = wsel == 0 ? a0 : (wsel == 1 ? a1 : a2);
+                    }
+                    if (g < 3) {
+                        uint8_t *dst = P.rgb + ((size_t)env * npix + (size_t)(pix - 4 * g)) * 3 + 16 * g;
+                        *reinterpret_cast<uint4 *>(dst) = make_uint4(o[0], o[1], o[2], o[3]);
+                    }
                 }
             }
         }
@@ -907,8 +1152,12 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
 
     if (STATS) {
         atomicAdd(&s_frag, (unsigned long long)st_frag);
+        atomicAdd(&s_culled, (unsigned long long)st_culled);
         __syncthreads();
-        if (tid == 0) atomicAdd(&P.stats[GX_STAT_FRAGMENTS], s_frag);
+        if (tid == 0) {
+            atomicAdd(&P.stats[GX_STAT_FRAGMENTS], s_frag);
+            atomicAdd(&P.stats[GX_STAT_RECORDS_OCCLUDED], s_culled);
+        }
     }
 }
 

@@ -60,4 +60,4 @@ struct GxParams {
 };
 
 enum { GX_STAT_CLUSTERS_TESTED = 0, GX_STAT_CLUSTERS_DRAWN, GX_STAT_TRIS_IN, GX_STAT_TRIS_RASTER,
-       GX_STAT_FRAGMENTS, GX_STAT_OVERFLOW_ENVS, GX_NSTAT };
+       GX_STAT_FRAGMENTS, GX_STAT_OVERFLOW_ENVS, GX_STAT_CLUSTERS_OCCLUDED, GX_STAT_RECORDS_OCCLUDED, GX_NSTAT };

@@ -71,15 +71,19 @@ def test_config3_and_4_sampled(oracle_mod):
 
 
 def test_cull_is_conservative(oracle_mod):
-    """N10: the image with frustum culling on equals the image with it off, bit for bit."""
+    """N10: the image with frustum culling on, and with frustum + hi-Z occlusion culling on, equals the image
+    with culling off, bit for bit."""
     wl = gen.make_config(1, n_envs=16)
-    a = render_gpu(wl, cull=1, stats=True)
+    a = render_gpu(wl, cull=1, stats=True, options=dict(occlusion=0))
     b = render_gpu(wl, cull=0, stats=True)
+    c = render_gpu(wl, cull=1, stats=True)            # frustum + occlusion culling (the default)
     for k in ("rgb", "depth", "id"):
         assert np.array_equal(a[k], b[k]), k
+        assert np.array_equal(c[k], b[k]), k
     assert a["stats"]["clusters_drawn"] < b["stats"]["clusters_drawn"]
     assert b["stats"]["clusters_drawn"] == b["stats"]["clusters_tested"]
     assert a["stats"]["triangles_raster"] == b["stats"]["triangles_raster"]
+    assert c["stats"]["triangles_raster"] < a["stats"]["triangles_raster"]
 
 
 def test_paths_pool_overflow_and_chunking(oracle_mod):
@@ -91,12 +95,17 @@ def test_paths_pool_overflow_and_chunking(oracle_mod):
     ref = render_gpu(wl, stats=True)
     rep = compare(o, ref)
     assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, rep
-    assert ref["stats"]["overflow_envs"] == 0 and ref["stats"]["launches"] == 5
+    assert ref["stats"]["overflow_envs"] == 0 and ref["stats"]["launches"] == 9
     variants = {
         "single kernel": dict(path=1),
         "some overflow": dict(pool_slots=12288),
         "all overflow": dict(pool_slots=64),
         "chunks of 3": dict(pool_bytes=3 * (65536 + 8192) * 64),
+        "no occluder phase": dict(occlusion=0),
+        "no depth sort": dict(depth_sort=0),
+        "neither": dict(occlusion=0, depth_sort=0),
+        "occluder phase 5 %": dict(occluder_pct=5),
+        "occluder phase 70 %": dict(occluder_pct=70),
         "small pass-B chunks": dict(big_slots=64, chunk_slots=32),
         "no pass B": dict(big_slots=1 << 20),
     }
@@ -109,9 +118,11 @@ def test_paths_pool_overflow_and_chunking(oracle_mod):
         if name == "some overflow":
             assert 0 < g["stats"]["overflow_envs"] < wl.N, g["stats"]
         if name == "chunks of 3":
-            assert g["stats"]["launches"] == 5 * 7
-        if name != "single kernel":
-            assert g["stats"]["triangles_raster"] >= ref["stats"]["triangles_raster"]
+            assert g["stats"]["launches"] == 9 * 7
+        if name == "no occluder phase":
+            assert g["stats"]["launches"] == 5 and g["stats"]["clusters_occluded"] == 0
+            assert g["stats"]["triangles_raster"] > ref["stats"]["triangles_raster"]
+    assert ref["stats"]["clusters_occluded"] > 0 and ref["stats"]["records_occluded"] > 0
 
 
 def test_sharding_and_determinism():
