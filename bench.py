@@ -51,6 +51,8 @@ def parse_args():
     ap.add_argument("--envs", type=int, default=0, help="render only the first n environments (development)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="gx_set_option before rendering (development: e.g. --opt occlusion=0)")
     return ap.parse_args()
 
 
@@ -205,6 +207,9 @@ def run_gx(args):
     wl = load_workload(args.config, args.envs)
     N, K, H, W = wl.N, wl.K, wl.height, wl.width
     scene = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, local)
+    for o in args.opt:
+        name, value = o.split("=")
+        gx.gx_set_option(scene, name, int(value))
     cam = gx.camera_of(wl)
     h_in = [np.ascontiguousarray(wl.env_scene, np.int32), np.ascontiguousarray(wl.cam_pose, np.float32),
             np.ascontiguousarray(wl.inst_mesh, np.int32), np.ascontiguousarray(wl.inst_xform, np.float32)]

@@ -94,8 +94,6 @@ struct GxScene {
     DevBuf<unsigned long long> frames;  // frame keys between the two raster phases
     int opt_occlusion = 1;              // occluder phase + hi-Z culling of clusters and records
     int opt_occluder_pct = 25;          // share of the visible clusters (nearest first) drawn in the occluder phase
-    DevBuf<uint32_t> zkeys, rec_order;  // depth sort keys of the records; per-raster-CTA order lists
-    int opt_depth_sort = 1;             // raster draws the records near to far and keeps the hi-Z tiles live
     DevBuf<uint32_t> pipe_scratch;      // counters[4] | cnt[2*chunk] | env_flag[chunk]
     int last_launches = 0;
     cudaStream_t last_stream = nullptr;
@@ -345,7 +343,7 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->meshes);
     cudaFree(sc->env_counter);
     cudaFree(sc->stats);
-    sc->pool.release(); sc->pipe_scratch.release(); sc->frames.release(); sc->zkeys.release(); sc->rec_order.release();
+    sc->pool.release(); sc->pipe_scratch.release(); sc->frames.release();
     sc->h_env_scene.release(); sc->h_inst_mesh.release(); sc->h_cam_pose.release(); sc->h_inst_xform.release();
     sc->h_depth.release(); sc->h_rgb.release(); sc->h_id.release();
     if (sc->host_stream) cudaStreamDestroy(sc->host_stream);
@@ -356,7 +354,6 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
     if (!sc || !name) return fail(GX_ERR_INVALID_ARG, "NULL argument");
     if (!strcmp(name, "cull")) { sc->opt_cull = value != 0; return GX_OK; }
     if (!strcmp(name, "stats")) { sc->opt_stats = value != 0; return GX_OK; }
-    if (!strcmp(name, "depth_sort")) { sc->opt_depth_sort = value != 0; return GX_OK; }
     if (!strcmp(name, "occlusion")) { sc->opt_occlusion = value != 0; return GX_OK; }
     if (!strcmp(name, "occluder_pct")) {
         if (value < 1 || value > 100) return fail(GX_ERR_INVALID_ARG, "occluder_pct must be in [1, 100]");
@@ -483,8 +480,6 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     const size_t off_items = (off_hiz + (size_t)chunk * gx::HZ_STRIDE + 1) & ~(size_t)1;
     if ((rc = sc->pipe_scratch.reserve(off_items + 2 * (size_t)chunk * std::max<size_t>(items_per_env, 1))) != GX_OK) return rc;
     if (two_phase && (rc = sc->frames.reserve((size_t)chunk * (size_t)npix)) != GX_OK) return rc;
-    if ((rc = sc->zkeys.reserve((size_t)chunk * (size_t)cap_n)) != GX_OK) return rc;
-    if ((rc = sc->rec_order.reserve((size_t)sc->num_sms * 2 * (size_t)cap_n)) != GX_OK) return rc;
     int launches = 0;
     for (int e0 = 0; e0 < N; e0 += chunk) {
         const int n = std::min(chunk, N - e0);
@@ -506,9 +501,6 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.thr = reinterpret_cast<float *>(sc->pipe_scratch.p + off_thr);
         PP.hiz = reinterpret_cast<float *>(sc->pipe_scratch.p + off_hiz);
         PP.frames = sc->frames.p;
-        PP.zkeys = sc->zkeys.p;
-        PP.rec_order = sc->rec_order.p;
-        PP.depth_sort = sc->opt_depth_sort;
         PP.occl_pct = two_phase ? sc->opt_occluder_pct : 100;
         PP.cap_n = (int32_t)cap_n;
         PP.cap_w = (int32_t)cap_w;

@@ -46,9 +46,6 @@ struct PipeParams {
     float *env_mv;           // [N][K+1][12] model-view per slot
     uint32_t *env_idb;       // [N][K+1] first triangle id per slot
     uint32_t *order;         // [N] raster order of the environments
-    uint32_t *zkeys;         // [N][cap_n] float bits of max(q) of each narrow record (0 for colour slots): depth sort key
-    uint32_t *rec_order;     // [raster CTAs][cap_n] per-CTA scratch: record indices of one environment, near to far
-    int32_t depth_sort;      // raster: draw the records near to far (bucket sort by zkeys) and keep the hi-Z tiles live
     uint32_t *cnt1;          // [N][2] record counts at the end of the occluder phase
     float *thr;              // [N] occluder phase: clusters with wmin < thr are drawn first
     float *hiz;              // [N][HZ_STRIDE] max depth per 8x8-pixel tile (stride 16) and per 32x32 tile (at +256)
@@ -227,7 +224,6 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                 dst[1] = make_uint4(D[1], D[2], bbw, (idb + (uint32_t)t) << 1);
                 dst[2] = make_uint4(__float_as_uint(q[0]), __float_as_uint(q[1]), __float_as_uint(q[2]), col[0]);
                 dst[3] = make_uint4(col[1], col[2], 0u, 0u);
-                PP.zkeys[(size_t)env * PP.cap_n + base + (uint32_t)g] = good ? __float_as_uint(fmaxf(q[0], fmaxf(q[1], q[2]))) : 0u;
             }
         }
     }
@@ -302,8 +298,6 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                 narrow_setup(tri.X, tri.Y, tri.q, i0, i1, j0, j1, E0, D, bbw, swapped);   // already normalised: no swap
                 const uint32_t slot = bn + 2u * (uint32_t)__popc(mn & lt);
                 uint4 *dst = env_recs + (size_t)slot * 4;
-                PP.zkeys[(size_t)env * PP.cap_n + slot] = __float_as_uint(fmaxf(tri.q[0], fmaxf(tri.q[1], tri.q[2])));
-                PP.zkeys[(size_t)env * PP.cap_n + slot + 1] = 0u;
                 dst[0] = make_uint4(E0[0], E0[1], E0[2], D[0]);
                 dst[1] = make_uint4(D[1], D[2], bbw | BB_FLOATCOL, tri.id2);
                 dst[2] = make_uint4(__float_as_uint(tri.q[0]), __float_as_uint(tri.q[1]), __float_as_uint(tri.q[2]), 0u);
@@ -572,11 +566,9 @@ __global__ void __launch_bounds__(1024) order_kernel(const PipeParams PP, const 
 struct RastWarpSmem {
     uint32_t *rec;   // [REC_WORDS * 32] SoA records of the current group (layout of gx_kernels.cuh R_*)
     uint32_t *fq;    // [FQ_CAP] covered fragments: r | (x - i0) << 5 | (y - j0) << 12
-    uint32_t *ridx;  // [32] slot index of each record of the group (the low half of the frame key)
 };
-constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4 + 32 * 4;
+constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4;
 constexpr int BIG_CAP = 512;       // entries of the pass-B list
-constexpr int ZBINS = 128;         // depth buckets of the raster order (8 per octave of max(q))
 
 __host__ __device__ inline size_t raster_smem_bytes(int W, int H, int warps) {
     return (size_t)W * H * 8 + (size_t)warps * RAST_WARP_SMEM;
@@ -603,13 +595,9 @@ __device__ __forceinline__ void key_min_rec(unsigned long long *slot, uint32_t d
 }
 
 // load the group's records (one per lane) into the warp's SoA staging
-// (record `base + order[pos + lane]` when an order list is given, else record `base + pos + lane`)
-__device__ __forceinline__ void load_group(const RastWarpSmem &ws, const uint4 *env_recs, uint32_t base, const uint32_t *order,
-                                           uint32_t pos, int nrec, int lane) {
+__device__ __forceinline__ void load_group(const RastWarpSmem &ws, const uint4 *env_recs, uint32_t first, int nrec, int lane) {
     if (lane < nrec) {
-        const uint32_t idx = base + (order ? order[pos + (uint32_t)lane] : pos + (uint32_t)lane);
-        ws.ridx[lane] = idx;
-        const uint4 *rp = env_recs + (size_t)idx * 4;
+        const uint4 *rp = env_recs + (size_t)(first + (uint32_t)lane) * 4;
         const uint4 u0 = __ldg(rp), u1 = __ldg(rp + 1), u2 = __ldg(rp + 2);
         ws.rec[(R_E0 + 0) * 32 + lane] = u0.x;
         ws.rec[(R_E0 + 1) * 32 + lane] = u0.y;
@@ -629,7 +617,7 @@ __device__ __forceinline__ void load_group(const RastWarpSmem &ws, const uint4 *
 
 // K4b: depth (N7) and resolve (N9) for the queued fragments, one per lane
 __device__ __forceinline__ void shade_queue_p(const RastWarpSmem &ws, int qn, int W, float zfar, unsigned long long *fb,
-                                              const uint4 *env_recs, int lane) {
+                                              uint32_t first, const uint4 *env_recs, int lane) {
     for (int f = lane; f < qn; f += 32) {
         const uint32_t en = ws.fq[f];
         const int r = (int)(en & 31u), a = (int)((en >> 5) & 127u), b = (int)((en >> 12) & 127u);
@@ -654,7 +642,7 @@ __device__ __forceinline__ void shade_queue_p(const RastWarpSmem &ws, int qn, in
         const float num = fmaf(fe[2], q[2], fmaf(fe[1], q[1], fe[0] * q[0]));
         const float depth = __uint_as_float(ws.rec[R_FA * 32 + r]) / num;
         if (depth > zfar) continue;
-        key_min_rec(slot, __float_as_uint(depth), ws.ridx[r], ws.rec[R_ID * 32 + r], env_recs);
+        key_min_rec(slot, __float_as_uint(depth), first + (uint32_t)r, ws.rec[R_ID * 32 + r], env_recs);
     }
     __syncwarp();
 }
@@ -704,7 +692,7 @@ __device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int
 // fragment queue with four ballots and shaded densely by shade_queue_p.
 template <bool STATS>
 __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, unsigned skip, int S0, int S1, int W, float zfar,
-                                             unsigned long long *fb, const uint4 *env_recs, int lane,
+                                             unsigned long long *fb, uint32_t first, const uint4 *env_recs, int lane,
                                              unsigned &n_frag) {
     const unsigned FULL = 0xFFFFFFFFu;
     const unsigned lt = (1u << lane) - 1u;
@@ -784,14 +772,14 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, un
         if (qn > FQ_CAP - 128) {
             __syncwarp();
             if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
-            shade_queue_p(ws, qn, W, zfar, fb, env_recs, lane);
+            shade_queue_p(ws, qn, W, zfar, fb, first, env_recs, lane);
             qn = 0;
         }
     }
     __syncwarp();
     if (qn) {
         if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
-        shade_queue_p(ws, qn, W, zfar, fb, env_recs, lane);
+        shade_queue_p(ws, qn, W, zfar, fb, first, env_recs, lane);
     }
 }
 
@@ -918,13 +906,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     RastWarpSmem ws;
     ws.rec = reinterpret_cast<uint32_t *>(smem + (size_t)npix * 8 + (size_t)warp * RAST_WARP_SMEM);
     ws.fq = ws.rec + REC_WORDS * 32;
-    ws.ridx = ws.fq + FQ_CAP;
 
     __shared__ int s_env;
     __shared__ unsigned s_next, s_next_b, s_big;
     __shared__ uint2 s_big_list[BIG_CAP];   // (group, first chunk) of the groups left to pass B
     __shared__ float s_hz[HZ_STRIDE];
-    __shared__ unsigned s_bin[ZBINS];
     __shared__ unsigned long long s_frag, s_culled;
 
     unsigned st_frag = 0, st_culled = 0;
@@ -936,10 +922,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     }
     const bool want_rgb = P.rgb != nullptr;
     const uint32_t cap_n = (uint32_t)PP.cap_n;
-    const bool sorted = PP.depth_sort != 0;
-    const float *hz = (PHASE == 2 || sorted) ? s_hz : nullptr;
-    uint32_t *my_order = PP.rec_order + (size_t)blockIdx.x * (size_t)PP.cap_n;
-    const uint32_t qfar = __float_as_uint(1.0f / P.zfar) >> 20;
+    const float *hz = PHASE == 2 ? s_hz : nullptr;
 
     for (;;) {
         if (tid == 0) {
@@ -963,41 +946,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
             uint4 *f4 = reinterpret_cast<uint4 *>(fb);
             for (int k = tid; k < npix / 2; k += NT) f4[k] = __ldg(src + k);
             for (int k = tid; k < HZ_STRIDE; k += NT) s_hz[k] = PP.hiz[(size_t)env * HZ_STRIDE + k];
-        } else if (sorted) {
-            for (int k = tid; k < HZ_STRIDE; k += NT) s_hz[k] = __int_as_float(0x7F800000);
+            __syncthreads();
         }
-        if (sorted) {
-            // bucket sort of the environment's narrow records by nearest depth (8 buckets per octave of max(q)):
-            // my_order[] lists them near to far; the order inside a bucket is arbitrary, the image does not depend on it
-            const uint32_t *zk = PP.zkeys + (size_t)env * PP.cap_n + b_n;
-            const uint32_t n = n_n - b_n;
-            for (int k = tid; k < ZBINS; k += NT) s_bin[k] = 0;
-            __syncthreads();
-            auto bin_of = [&](uint32_t key) {
-                const int d = (int)(key >> 20) - (int)qfar;
-                return (ZBINS - 1) - min(max(d, 0), ZBINS - 1);
-            };
-            for (uint32_t k = tid; k < n; k += NT) atomicAdd(&s_bin[bin_of(__ldg(zk + k))], 1u);
-            __syncthreads();
-            if (warp == 0) {   // exclusive scan of the ZBINS counts, ZBINS / 32 per lane
-                unsigned v[ZBINS / 32], sum = 0;
-#pragma unroll
-                for (int k = 0; k < ZBINS / 32; ++k) { v[k] = s_bin[lane * (ZBINS / 32) + k]; sum += v[k]; }
-                unsigned inc = sum;
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) {
-                    const unsigned a = __shfl_up_sync(0xFFFFFFFFu, inc, d);
-                    if (lane >= d) inc += a;
-                }
-                unsigned run = inc - sum;
-#pragma unroll
-                for (int k = 0; k < ZBINS / 32; ++k) { s_bin[lane * (ZBINS / 32) + k] = run; run += v[k]; }
-            }
-            __syncthreads();
-            for (uint32_t k = tid; k < n; k += NT) my_order[atomicAdd(&s_bin[bin_of(__ldg(zk + k))], 1u)] = k;
-        }
-        if (PHASE == 2 || sorted) __syncthreads();
-        const uint32_t *order = sorted ? my_order : nullptr;
 
         // ---- K3 + K4, pass A: groups of 32 records, drawn dynamically by the warps.  A group of more than
         // big_slots slots is only registered: (list index, first chunk) come from one packed atomic, so the
@@ -1007,27 +957,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
             if (lane == 0) g = atomicAdd(&s_next, 1u);
             g = __shfl_sync(0xFFFFFFFFu, g, 0);
             if (g >= g_n + g_w) break;
-            if (sorted) {   // keep the hi-Z tiles live: every draw recomputes 8 of them from the frame (a stale
-                            // value is a valid bound: depths only decrease)
-                const int tw = W >> 3, nt = tw * (H >> 3);
-                for (int k = 0; k < 8; ++k) {
-                    const int t = (int)((g * 8u + (unsigned)k) % (unsigned)nt);
-                    const int ty = t / tw, tx = t - ty * tw;
-                    const int j = ty * 8 + (lane >> 2), i = tx * 8 + (lane & 3) * 2;
-                    const volatile unsigned long long *kp = &fb[fb_index(i, j, W)];
-                    const unsigned d = __reduce_max_sync(0xFFFFFFFFu, max((unsigned)(kp[0] >> 32), (unsigned)(kp[1] >> 32)));
-                    if (lane == 0) s_hz[ty * 16 + tx] = d == 0xFFFFFFFFu ? __int_as_float(0x7F800000) : __uint_as_float(d);
-                }
-            }
             if (g >= g_w) {
                 const uint32_t pos = (g - g_w) * 32u;
                 const int nrec = (int)min(32u, n_n - b_n - pos);
-                load_group(ws, env_recs, b_n, order, pos, nrec, lane);
+                const uint32_t first = b_n + pos;
+                load_group(ws, env_recs, first, nrec, lane);
                 int Pex;
                 unsigned skip;
                 const int T = group_slots(ws, nrec, lane, hz, Pex, skip, st_culled);
                 if (T <= PP.big_slots) {
-                    if (T) raster_slots<STATS>(ws, Pex, skip, 0, T, W, P.zfar, fb, env_recs, lane, st_frag);
+                    if (T) raster_slots<STATS>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
                 } else {
                     unsigned full = 0;
                     if (lane == 0) {
@@ -1037,7 +976,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                         else full = 1;
                     }
                     if (__shfl_sync(0xFFFFFFFFu, full, 0))   // list full: draw the group here, whole
-                        raster_slots<STATS>(ws, Pex, skip, 0, T, W, P.zfar, fb, env_recs, lane, st_frag);
+                        raster_slots<STATS>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
                 }
             } else {   // wide records first: they reach the near plane and hide the most
                 const uint32_t t0 = b_w + g * 32u;
@@ -1062,12 +1001,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                 const uint2 en = s_big_list[lo];
                 const uint32_t pos = en.x * 32u;
                 const int nrec = (int)min(32u, n_n - b_n - pos);
-                load_group(ws, env_recs, b_n, order, pos, nrec, lane);
+                const uint32_t first = b_n + pos;
+                load_group(ws, env_recs, first, nrec, lane);
                 int Pex;
                 unsigned skip, dummy = 0;
                 const int T = group_slots(ws, nrec, lane, hz, Pex, skip, dummy);
                 const int S0 = (int)(c - en.y) * PP.chunk_slots;   // chunks of entries a full list dropped land beyond T
-                if (S0 < T) raster_slots<STATS>(ws, Pex, skip, S0, min(T, S0 + PP.chunk_slots), W, P.zfar, fb, env_recs, lane, st_frag);
+                if (S0 < T) raster_slots<STATS>(ws, Pex, skip, S0, min(T, S0 + PP.chunk_slots), W, P.zfar, fb, first, env_recs, lane, st_frag);
             }
         }
         __syncthreads();

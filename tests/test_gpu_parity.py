@@ -102,8 +102,6 @@ def test_paths_pool_overflow_and_chunking(oracle_mod):
         "all overflow": dict(pool_slots=64),
         "chunks of 3": dict(pool_bytes=3 * (65536 + 8192) * 64),
         "no occluder phase": dict(occlusion=0),
-        "no depth sort": dict(depth_sort=0),
-        "neither": dict(occlusion=0, depth_sort=0),
         "occluder phase 5 %": dict(occluder_pct=5),
         "occluder phase 70 %": dict(occluder_pct=70),
         "small pass-B chunks": dict(big_slots=64, chunk_slots=32),
