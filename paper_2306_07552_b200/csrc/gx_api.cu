@@ -74,6 +74,7 @@ struct GxScene {
     float4 *verts = nullptr;
     uchar4 *tris = nullptr;
     GxBatchDev *batches = nullptr;
+    GxClusterDev *subs = nullptr;
     GxClusterDev *clusters = nullptr;
     GxMeshDev *meshes = nullptr;
     std::vector<uint32_t> mesh_nt;      // host copy, for id-range validation
@@ -92,7 +93,9 @@ struct GxScene {
     int opt_big_slots = 512, opt_chunk_slots = 256;   // raster pass B (gx_pipeline.cuh)
     DevBuf<uint4> pool;                 // triangle records of one chunk of environments
     DevBuf<unsigned long long> frames;  // frame keys between the two raster phases
-    int opt_occlusion = 1;              // occluder phase + hi-Z culling of clusters and records
+    int opt_subcull = 1;                // geometry kernel: frustum (and hi-Z) test per 32-triangle sub-cluster
+    int opt_bands = 0;                  // raster bands per frame; 0 = automatic
+    int opt_occlusion = 0;              // occluder phase + hi-Z culling of clusters and records
     int opt_occluder_pct = 25;          // share of the visible clusters (nearest first) drawn in the occluder phase
     DevBuf<uint32_t> pipe_scratch;      // counters[4] | cnt[2*chunk] | env_flag[chunk]
     int last_launches = 0;
@@ -110,7 +113,7 @@ namespace {
 // Cut one mesh into clusters of GX_CLUSTER_TRIS consecutive triangles and batches of <= GX_VCAP unique
 // vertices (gx_types.h).  Vertices are copied per batch in first-use order with the colour packed into .w.
 int build_mesh(const GxMesh &m, std::vector<float4> &verts, std::vector<uchar4> &tris, std::vector<GxBatchDev> &batches,
-               std::vector<GxClusterDev> &clusters, GxMeshDev &out) {
+               std::vector<GxClusterDev> &subs, std::vector<GxClusterDev> &clusters, GxMeshDev &out) {
     out.cluster_off = (uint32_t)clusters.size();
     out.nt = m.nt;
     out.pad = 0;
@@ -165,6 +168,21 @@ int build_mesh(const GxMesh &m, std::vector<float4> &verts, std::vector<uchar4> 
             }
             for (uint32_t v : touched) local[v] = -1;
             b.nv_nt = nv | (nt << 16);
+            // sub-clusters: AABB of every run of 32 consecutive triangles of the batch
+            for (uint32_t k = 0; k < (uint32_t)GX_SUBS_PER_BATCH; ++k) {
+                GxClusterDev sb;
+                sb.batch_off = 0; sb.nbatch = 0;
+                for (int a = 0; a < 3; ++a) { sb.bmin[a] = 3.0e38f; sb.bmax[a] = -3.0e38f; }
+                for (uint32_t tt = b.first_tri + 32 * k; tt < std::min(b.first_tri + 32 * (k + 1), b.first_tri + nt); ++tt)
+                    for (int kk = 0; kk < 3; ++kk) {
+                        const float *pp = m.positions + 3 * (size_t)m.indices[3 * (size_t)tt + kk];
+                        for (int a = 0; a < 3; ++a) {
+                            sb.bmin[a] = std::min(sb.bmin[a], pp[a]);
+                            sb.bmax[a] = std::max(sb.bmax[a], pp[a]);
+                        }
+                    }
+                subs.push_back(sb);
+            }
             batches.push_back(b);
             ++c.nbatch;
         }
@@ -217,12 +235,12 @@ int launch_single(const GxScene *sc, const GxParams &P, cudaStream_t stream, boo
 template <int WARPS, int MINB, int PHASE>
 int launch_raster(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
     auto kern = stats ? gx::raster_kernel<WARPS, MINB, PHASE, true> : gx::raster_kernel<WARPS, MINB, PHASE, false>;
-    const size_t smem = gx::raster_smem_bytes(PP.g.W, PP.g.H, WARPS);
+    const size_t smem = gx::raster_smem_bytes(PP.g.W, PP.bh, WARPS);
     GX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
     GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem));
     if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "raster kernel does not fit: %zu bytes of shared memory", smem);
-    kern<<<std::min(PP.g.N, sc->num_sms * per_sm), WARPS * 32, smem, stream>>>(PP);
+    kern<<<std::min(PP.g.N * PP.bands, sc->num_sms * per_sm), WARPS * 32, smem, stream>>>(PP);
     GX_CUDA(cudaGetLastError());
     return GX_OK;
 }
@@ -246,7 +264,10 @@ int launch_pass(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream
     GX_CUDA(cudaGetLastError());
     gx::order_kernel<<<1, 1024, 0, stream>>>(PP, PHASE == 2 ? 1 : 0);
     GX_CUDA(cudaGetLastError());
-    if ((size_t)PP.g.W * PP.g.H * 8 <= 32768) return launch_raster<16, 2, PHASE>(sc, PP, stream, stats);
+    // one band of 64-bit keys per CTA: the smaller the band, the more CTAs share an SM (32 warps per SM in all cases)
+    const size_t band_bytes = (size_t)PP.g.W * PP.bh * 8;
+    if (band_bytes <= 32768) return launch_raster<8, 4, PHASE>(sc, PP, stream, stats);
+    if (band_bytes <= 65536) return launch_raster<16, 2, PHASE>(sc, PP, stream, stats);
     return launch_raster<32, 1, PHASE>(sc, PP, stream, stats);
 }
 
@@ -265,7 +286,7 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
     std::vector<float4> verts;
     std::vector<uchar4> tris;
     std::vector<GxBatchDev> batches;
-    std::vector<GxClusterDev> clusters;
+    std::vector<GxClusterDev> clusters, subs;
     std::vector<GxMeshDev> meshes;
     GxScene *sc = new (std::nothrow) GxScene();
     if (!sc) return fail(GX_ERR_OOM, "host allocation failed");
@@ -278,7 +299,7 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
             }
             GxMeshDev md;
             const size_t b0 = batches.size();
-            const int rc = build_mesh(m, verts, tris, batches, clusters, md);
+            const int rc = build_mesh(m, verts, tris, batches, subs, clusters, md);
             if (rc != GX_OK) { delete sc; return rc; }
             uint32_t &mb = i < n_static ? sc->max_static_batches : sc->max_dyn_batches;
             mb = std::max<uint32_t>(mb, (uint32_t)(batches.size() - b0));
@@ -312,6 +333,7 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
     if (rc == GX_OK) rc = upload(sc->verts, verts);
     if (rc == GX_OK) rc = upload(sc->tris, tris);
     if (rc == GX_OK) rc = upload(sc->batches, batches);
+    if (rc == GX_OK) rc = upload(sc->subs, subs);
     if (rc == GX_OK) rc = upload(sc->clusters, clusters);
     if (rc == GX_OK) rc = upload(sc->meshes, meshes);
     if (rc == GX_OK) {
@@ -339,6 +361,7 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->verts);
     cudaFree(sc->tris);
     cudaFree(sc->batches);
+    cudaFree(sc->subs);
     cudaFree(sc->clusters);
     cudaFree(sc->meshes);
     cudaFree(sc->env_counter);
@@ -354,6 +377,12 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
     if (!sc || !name) return fail(GX_ERR_INVALID_ARG, "NULL argument");
     if (!strcmp(name, "cull")) { sc->opt_cull = value != 0; return GX_OK; }
     if (!strcmp(name, "stats")) { sc->opt_stats = value != 0; return GX_OK; }
+    if (!strcmp(name, "subcull")) { sc->opt_subcull = value != 0; return GX_OK; }
+    if (!strcmp(name, "bands")) {
+        if (value != 0 && value != 1 && value != 2 && value != 4) return fail(GX_ERR_INVALID_ARG, "bands must be 0, 1, 2 or 4");
+        sc->opt_bands = (int)value;
+        return GX_OK;
+    }
     if (!strcmp(name, "occlusion")) { sc->opt_occlusion = value != 0; return GX_OK; }
     if (!strcmp(name, "occluder_pct")) {
         if (value < 1 || value > 100) return fail(GX_ERR_INVALID_ARG, "occluder_pct must be in [1, 100]");
@@ -437,7 +466,7 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     if (cam->width > 128 || cam->height > 128)
         return fail(GX_ERR_UNSUPPORTED, "width and height must be <= 128 in this build, got %dx%d", cam->width, cam->height);
     GxParams P;
-    P.verts = sc->verts; P.tris = sc->tris; P.batches = sc->batches; P.clusters = sc->clusters; P.meshes = sc->meshes;
+    P.verts = sc->verts; P.tris = sc->tris; P.batches = sc->batches; P.subs = sc->subs; P.clusters = sc->clusters; P.meshes = sc->meshes;
     P.n_static = sc->n_static; P.n_dyn = sc->n_dyn;
     P.N = N; P.K = K; P.W = cam->width; P.H = cam->height;
     P.fx = cam->fx; P.fy = cam->fy; P.znear = cam->znear; P.zfar = cam->zfar;
@@ -462,20 +491,24 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
 
     // ---- two-kernel path, in chunks of environments that share the record pool ----------------------
     const int64_t npix = (int64_t)P.W * P.H;
-    const int64_t cap_n = sc->opt_pool_slots > 0 ? sc->opt_pool_slots : std::max<int64_t>(4096, 4 * npix);
+    // bands: (environment, band) is the raster task; several bands only if each is a multiple of 32 rows
+    int bands = sc->opt_bands > 0 ? sc->opt_bands : (npix * 8 > 65536 ? 2 : 1);
+    while (bands > 1 && (P.H % bands || (P.H / bands) % 32)) bands >>= 1;
+    const int bh = P.H / bands;
+    const int64_t cap_n = sc->opt_pool_slots > 0 ? sc->opt_pool_slots : std::max<int64_t>(2048, 4 * npix / bands);
     const int64_t cap_w = std::max<int64_t>(64, cap_n / 8) & ~(int64_t)1;
-    const int64_t env_bytes = (cap_n + cap_w) * 64;
+    const int64_t env_bytes = (cap_n + cap_w) * 64 * bands;
     const int64_t budget = sc->opt_pool_bytes > 0 ? sc->opt_pool_bytes : (int64_t)8 << 30;
     const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(N, budget / env_bytes));
     int rc;
-    if ((rc = sc->pool.reserve((size_t)chunk * (size_t)(cap_n + cap_w) * 4)) != GX_OK) return rc;
-    // scratch words: counters[8] | cnt[2*chunk] | env_flag[chunk] (zeroed per chunk) | order[chunk] | cnt1[2*chunk] |
+    if ((rc = sc->pool.reserve((size_t)chunk * bands * (size_t)(cap_n + cap_w) * 4)) != GX_OK) return rc;
+    // scratch words: counters[8] | cnt[2*tasks] | env_flag[chunk] (zeroed per chunk) | order[tasks] | cnt1[2*tasks] |
     //                thr[chunk] | env_idb[chunk*(K+1)] | env_mv[chunk*(K+1)*12] | hiz[chunk*HZ_STRIDE] | items[2*...]
     const bool two_phase = sc->opt_cull && sc->opt_occlusion && sc->opt_occluder_pct < 100;
-    const size_t k1 = (size_t)K + 1;
+    const size_t k1 = (size_t)K + 1, tasks = (size_t)chunk * bands;
     const size_t items_per_env = (size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches;
-    const size_t n_zero = 8 + 3 * (size_t)chunk;
-    const size_t off_order = n_zero, off_cnt1 = off_order + chunk, off_thr = off_cnt1 + 2 * (size_t)chunk;
+    const size_t n_zero = 8 + 2 * tasks + (size_t)chunk;
+    const size_t off_order = n_zero, off_cnt1 = off_order + tasks, off_thr = off_cnt1 + 2 * tasks;
     const size_t off_idb = off_thr + chunk, off_mv = off_idb + chunk * k1, off_hiz = off_mv + chunk * k1 * 12;
     const size_t off_items = (off_hiz + (size_t)chunk * gx::HZ_STRIDE + 1) & ~(size_t)1;
     if ((rc = sc->pipe_scratch.reserve(off_items + 2 * (size_t)chunk * std::max<size_t>(items_per_env, 1))) != GX_OK) return rc;
@@ -496,7 +529,7 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.recs = sc->pool.p;
         PP.counters = sc->pipe_scratch.p;
         PP.cnt = sc->pipe_scratch.p + 8;
-        PP.env_flag = sc->pipe_scratch.p + 8 + 2 * (size_t)chunk;
+        PP.env_flag = sc->pipe_scratch.p + 8 + 2 * tasks;
         PP.cnt1 = sc->pipe_scratch.p + off_cnt1;
         PP.thr = reinterpret_cast<float *>(sc->pipe_scratch.p + off_thr);
         PP.hiz = reinterpret_cast<float *>(sc->pipe_scratch.p + off_hiz);
@@ -504,6 +537,10 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.occl_pct = two_phase ? sc->opt_occluder_pct : 100;
         PP.cap_n = (int32_t)cap_n;
         PP.cap_w = (int32_t)cap_w;
+        PP.bands = bands;
+        PP.subcull = sc->opt_cull && sc->opt_subcull;
+        PP.phase = 0;
+        PP.bh = bh;
         PP.big_slots = sc->opt_big_slots;
         PP.chunk_slots = sc->opt_chunk_slots;
         PP.order = sc->pipe_scratch.p + off_order;
@@ -517,6 +554,7 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         } else {
             if ((rc = launch_pass<1>(sc, PP, stream, st)) != GX_OK) return rc;
             PP.counters = sc->pipe_scratch.p + 4;
+            PP.phase = 2;
             if ((rc = launch_pass<2>(sc, PP, stream, st)) != GX_OK) return rc;
             launches += 8;
         }
@@ -526,7 +564,7 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PL.env_filter = PP.env_flag;
         if ((rc = launch_single(sc, PL, stream, st)) != GX_OK) return rc;
         launches += 1;
-        sc->last_chunk_n = n;
+        sc->last_chunk_n = n * bands;
     }
     sc->last_launches = launches;
     return GX_OK;

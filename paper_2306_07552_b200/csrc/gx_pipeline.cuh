@@ -51,7 +51,10 @@ struct PipeParams {
     float *hiz;              // [N][HZ_STRIDE] max depth per 8x8-pixel tile (stride 16) and per 32x32 tile (at +256)
     unsigned long long *frames;   // [N][W*H] frame keys between the two raster phases
     int32_t occl_pct;        // share of the frustum-visible clusters (nearest first) drawn in the occluder phase
-    int32_t cap_n, cap_w;    // slots per environment
+    int32_t cap_n, cap_w;    // slots per (environment, band)
+    int32_t subcull;         // geometry: test every 32-triangle sub-cluster of a batch (frustum; hi-Z in phase 2)
+    int32_t phase;           // 2 while the second pass of the occluder scheme runs, else 0
+    int32_t bands, bh;       // horizontal bands per frame, rows per band (H = bands * bh)
     int32_t big_slots, chunk_slots;   // raster pass B: groups above big_slots are drawn in chunks of chunk_slots
 };
 
@@ -131,6 +134,71 @@ __device__ __forceinline__ void store_colour_slot(uint4 *dst, const float c[3][3
     (void)id2;
 }
 
+// The frame is cut into PP.bands horizontal bands of PP.bh rows; every (environment, band) pair is one raster
+// task with its own record lists ("virtual environment" v = env * bands + band).  emit_narrow appends a set-up
+// narrow record to the list of every band its bounding box touches, with the box clipped to the band's rows
+// (edge values moved to the new origin, j0 relative to the band), so that the raster kernel needs no clipping.
+// Called converged by the whole warp; PAIR: a colour slot (oc) follows the record.
+template <bool PAIR>
+__device__ __forceinline__ void emit_narrow(const PipeParams &PP, int env, int lane, bool valid, const uint32_t E0[3],
+                                            const uint32_t D[3], uint32_t bbw, int j0, int j1, uint32_t id2,
+                                            const float q[3], const uint32_t col[3], const float (*oc)[3], bool &overflow) {
+    const unsigned FULL = 0xFFFFFFFFu;
+    const unsigned lt = (1u << lane) - 1u;
+    for (int b = 0; b < PP.bands; ++b) {
+        const int lo = b * PP.bh, hi = lo + PP.bh - 1;
+        const bool touch = valid && j0 <= hi && j1 >= lo;
+        const unsigned m = __ballot_sync(FULL, touch);
+        if (m == 0u) continue;
+        const int v = env * PP.bands + b;
+        const uint32_t n = (PAIR ? 2u : 1u) * (uint32_t)__popc(m);
+        uint32_t base = 0;
+        if (lane == 0) base = atomicAdd(&PP.cnt[2 * v], n);
+        base = __shfl_sync(FULL, base, 0);
+        if (base + n > (uint32_t)PP.cap_n) { overflow = true; continue; }
+        if (touch) {
+            const int jj0 = max(j0, lo), jj1 = min(j1, hi), dj = jj0 - j0;
+            uint32_t E[3];
+#pragma unroll
+            for (int e = 0; e < 3; ++e) E[e] = E0[e] + (uint32_t)((dj * ((int)D[e] >> 16)) << 8);
+            const uint32_t bb = (bbw & ~((127u << 7) | (127u << 21))) | ((uint32_t)(jj0 - lo) << 7) | ((uint32_t)(jj1 - jj0) << 21);
+            uint4 *dst = PP.recs + ((size_t)v * (size_t)(PP.cap_n + PP.cap_w) + base + (PAIR ? 2u : 1u) * (uint32_t)__popc(m & lt)) * 4;
+            dst[0] = make_uint4(E[0], E[1], E[2], D[0]);
+            dst[1] = make_uint4(D[1], D[2], bb | (PAIR ? BB_FLOATCOL : 0u), id2);
+            dst[2] = make_uint4(__float_as_uint(q[0]), __float_as_uint(q[1]), __float_as_uint(q[2]), PAIR ? 0u : col[0]);
+            dst[3] = PAIR ? make_uint4(0u, 0u, 0u, 0u) : make_uint4(col[1], col[2], 0u, 0u);
+            if (PAIR) store_colour_slot(dst + 4, oc, id2);
+        }
+    }
+}
+
+// wide record + colour slot, appended to the wide list of every band the (frame-clamped) rows j0..j1 touch
+__device__ __forceinline__ void emit_wide(const PipeParams &PP, int env, int lane, bool valid, const Tri &tri, int j0, int j1,
+                                          const float (*oc)[3], bool &overflow) {
+    const unsigned FULL = 0xFFFFFFFFu;
+    const unsigned lt = (1u << lane) - 1u;
+    for (int b = 0; b < PP.bands; ++b) {
+        const int lo = b * PP.bh, hi = lo + PP.bh - 1;
+        const bool touch = valid && j0 <= hi && j1 >= lo;
+        const unsigned m = __ballot_sync(FULL, touch);
+        if (m == 0u) continue;
+        const int v = env * PP.bands + b;
+        const uint32_t n = 2u * (uint32_t)__popc(m);
+        uint32_t base = 0;
+        if (lane == 0) base = atomicAdd(&PP.cnt[2 * v + 1], n);
+        base = __shfl_sync(FULL, base, 0);
+        if (base + n > (uint32_t)PP.cap_w) { overflow = true; continue; }
+        if (touch) {
+            uint4 *dst = PP.recs + ((size_t)v * (size_t)(PP.cap_n + PP.cap_w) + (size_t)PP.cap_n + base + 2u * (uint32_t)__popc(m & lt)) * 4;
+            dst[0] = make_uint4((uint32_t)tri.X[0], (uint32_t)tri.X[1], (uint32_t)tri.X[2], (uint32_t)tri.Y[0]);
+            dst[1] = make_uint4((uint32_t)tri.Y[1], (uint32_t)tri.Y[2], 0u, tri.id2);
+            dst[2] = make_uint4(__float_as_uint(tri.q[0]), __float_as_uint(tri.q[1]), __float_as_uint(tri.q[2]), 0u);
+            dst[3] = make_uint4(0u, 0u, 0u, 0u);
+            store_colour_slot(dst + 4, oc, tri.id2);
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // geometry: K2 for one batch, by one warp
 // ------------------------------------------------------------------------------------------------
@@ -149,8 +217,21 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
     const float4 *__restrict__ verts = P.verts + b.vert_off;
     const uchar4 *__restrict__ tris = P.tris + b.tri_off;
     const unsigned lt = (1u << lane) - 1u;
-    uint4 *env_recs = PP.recs + (size_t)env * (size_t)(PP.cap_n + PP.cap_w) * 4;
-    if (STATS) n_in += (lane == 0) ? (unsigned)nt : 0u;
+    // K1b: sub-cluster culling.  Every pass of the triangle loop below takes 32 consecutive triangles; lane k
+    // tests the AABB of pass k against the frustum (and, in the second pass of the occluder scheme, against
+    // the hi-Z tiles).  A pass whose bit is clear is skipped; a batch with no bit set costs nothing more.
+    unsigned sub_mask = 0xFFFFFFFFu;
+    if (PP.subcull) {
+        bool vis = false;
+        if (lane * 32 < nt) {
+            const CamBox bx = cluster_box(P.subs[(size_t)batch * GX_SUBS_PER_BATCH + lane], M);
+            vis = box_in_frustum(bx, P.fx, P.fy, P.znear, P.zfar);
+            if (vis && PP.phase == 2) vis = !box_occluded(bx, PP.hiz + (size_t)env * HZ_STRIDE, P.fx, P.fy, P.W, P.H, P.znear);
+        }
+        sub_mask = __ballot_sync(FULL, vis);
+        if (sub_mask == 0u) return;
+    }
+    if (STATS) n_in += (lane == 0) ? 32u * (unsigned)__popc(sub_mask & ((nt + 31) / 32 < 32 ? (1u << ((nt + 31) / 32)) - 1u : 0xFFFFFFFFu)) : 0u;
 
     // K2a: vertex transform, projection, snap -> warp-private staging
     for (int v = lane; v < nv; v += 32) {
@@ -169,6 +250,7 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
     // of lst and slow-path triangles (wide, or straddling the near plane) to the back
     int nsurv = 0, nslow = 0;
     for (int t0 = 0; t0 < nt; t0 += 32) {
+        if (!((sub_mask >> (t0 >> 5)) & 1u)) continue;
         const int t = t0 + lane;
         bool ok = false, slow = false;
         if (t < nt) {
@@ -196,36 +278,29 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
     }
     __syncwarp();
 
-    // K2c: set-up of the narrow survivors, one record each, written straight to the environment's segment
-    if (nsurv) {
-        uint32_t base = 0;
-        if (lane == 0) base = atomicAdd(&PP.cnt[2 * env], (uint32_t)nsurv);
-        base = __shfl_sync(FULL, base, 0);
-        if (base + (uint32_t)nsurv > (uint32_t)PP.cap_n) {
-            overflow = true;
-        } else {
-            for (int g = lane; g < nsurv; g += 32) {
-                const int t = ws.lst[g];
-                const uchar4 ix = __ldg(&tris[t]);
-                const int2 a = ws.vXY[ix.x], bq = ws.vXY[ix.y], c = ws.vXY[ix.z];
-                int X[3] = {a.x, bq.x, c.x}, Y[3] = {a.y, bq.y, c.y};
-                float q[3] = {ws.vQ[ix.x], ws.vQ[ix.y], ws.vQ[ix.z]};
-                uint32_t col[3] = {ws.vC[ix.x], ws.vC[ix.y], ws.vC[ix.z]};
-                int i0, i1, j0, j1;
-                pixel_bbox(X, Y, P.W, P.H, i0, i1, j0, j1);
-                uint32_t E0[3], D[3], bbw;
-                bool swapped;
-                const bool good = narrow_setup(X, Y, q, i0, i1, j0, j1, E0, D, bbw, swapped);
-                if (swapped) { const uint32_t tc = col[1]; col[1] = col[2]; col[2] = tc; }
-                if (!good) { E0[0] = E0[1] = E0[2] = 0xFFFFFFFFu; D[0] = D[1] = D[2] = 0u; bbw = 0u; }   // covers nothing
-                if (STATS) n_tri += good ? 1u : 0u;
-                uint4 *dst = env_recs + (size_t)(base + (uint32_t)g) * 4;
-                dst[0] = make_uint4(E0[0], E0[1], E0[2], D[0]);
-                dst[1] = make_uint4(D[1], D[2], bbw, (idb + (uint32_t)t) << 1);
-                dst[2] = make_uint4(__float_as_uint(q[0]), __float_as_uint(q[1]), __float_as_uint(q[2]), col[0]);
-                dst[3] = make_uint4(col[1], col[2], 0u, 0u);
-            }
+    // K2c: set-up of the narrow survivors, 32 at a time; each leaves as one record per band it touches
+    for (int g0 = 0; g0 < nsurv; g0 += 32) {
+        const bool have = g0 + lane < nsurv;
+        uint32_t E0[3] = {0u, 0u, 0u}, D[3] = {0u, 0u, 0u}, bbw = 0u, col[3] = {0u, 0u, 0u}, id2 = 0u;
+        float q[3] = {0.0f, 0.0f, 0.0f};
+        int j0 = 0, j1 = 0;
+        bool good = false;
+        if (have) {
+            const int t = ws.lst[g0 + lane];
+            const uchar4 ix = __ldg(&tris[t]);
+            const int2 a = ws.vXY[ix.x], bq = ws.vXY[ix.y], c = ws.vXY[ix.z];
+            int X[3] = {a.x, bq.x, c.x}, Y[3] = {a.y, bq.y, c.y};
+            q[0] = ws.vQ[ix.x]; q[1] = ws.vQ[ix.y]; q[2] = ws.vQ[ix.z];
+            col[0] = ws.vC[ix.x]; col[1] = ws.vC[ix.y]; col[2] = ws.vC[ix.z];
+            int i0, i1;
+            pixel_bbox(X, Y, P.W, P.H, i0, i1, j0, j1);
+            bool swapped;
+            good = narrow_setup(X, Y, q, i0, i1, j0, j1, E0, D, bbw, swapped);   // zero area: dropped
+            if (swapped) { const uint32_t tc = col[1]; col[1] = col[2]; col[2] = tc; }
+            id2 = (idb + (uint32_t)t) << 1;
+            if (STATS) n_tri += good ? 1u : 0u;
         }
+        emit_narrow<false>(PP, env, lane, good, E0, D, bbw, j0, j1, id2, q, col, nullptr, overflow);
     }
 
     // slow path: wide triangles and near-plane straddlers (N4), piece by piece
@@ -278,40 +353,15 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                     }
                 }
             }
-            const unsigned mn = __ballot_sync(FULL, narrow), mw = __ballot_sync(FULL, wide);
-            if ((mn | mw) == 0u) continue;
-            uint32_t bn = 0, bw = 0;
-            if (lane == 0) {
-                if (mn) bn = atomicAdd(&PP.cnt[2 * env], 2u * (uint32_t)__popc(mn));
-                if (mw) bw = atomicAdd(&PP.cnt[2 * env + 1], 2u * (uint32_t)__popc(mw));
-            }
-            bn = __shfl_sync(FULL, bn, 0);
-            bw = __shfl_sync(FULL, bw, 0);
-            if (bn + 2u * (uint32_t)__popc(mn) > (uint32_t)PP.cap_n || bw + 2u * (uint32_t)__popc(mw) > (uint32_t)PP.cap_w) {
-                overflow = true;
-                continue;
-            }
+            if (__ballot_sync(FULL, narrow || wide) == 0u) continue;
             if (STATS) n_tri += (narrow || wide) ? 1u : 0u;
-            if (narrow) {
-                uint32_t E0[3], D[3], bbw;
+            {
+                uint32_t E0[3] = {0u, 0u, 0u}, D[3] = {0u, 0u, 0u}, bbw = 0u;
                 bool swapped;
-                narrow_setup(tri.X, tri.Y, tri.q, i0, i1, j0, j1, E0, D, bbw, swapped);   // already normalised: no swap
-                const uint32_t slot = bn + 2u * (uint32_t)__popc(mn & lt);
-                uint4 *dst = env_recs + (size_t)slot * 4;
-                dst[0] = make_uint4(E0[0], E0[1], E0[2], D[0]);
-                dst[1] = make_uint4(D[1], D[2], bbw | BB_FLOATCOL, tri.id2);
-                dst[2] = make_uint4(__float_as_uint(tri.q[0]), __float_as_uint(tri.q[1]), __float_as_uint(tri.q[2]), 0u);
-                dst[3] = make_uint4(0u, 0u, 0u, 0u);
-                store_colour_slot(dst + 4, oc, tri.id2);
+                if (narrow) narrow_setup(tri.X, tri.Y, tri.q, i0, i1, j0, j1, E0, D, bbw, swapped);   // already normalised: no swap
+                emit_narrow<true>(PP, env, lane, narrow, E0, D, bbw, j0, j1, tri.id2, tri.q, nullptr, oc, overflow);
             }
-            if (wide) {
-                uint4 *dst = env_recs + ((size_t)PP.cap_n + bw + 2u * (uint32_t)__popc(mw & lt)) * 4;
-                dst[0] = make_uint4((uint32_t)tri.X[0], (uint32_t)tri.X[1], (uint32_t)tri.X[2], (uint32_t)tri.Y[0]);
-                dst[1] = make_uint4((uint32_t)tri.Y[1], (uint32_t)tri.Y[2], 0u, tri.id2);
-                dst[2] = make_uint4(__float_as_uint(tri.q[0]), __float_as_uint(tri.q[1]), __float_as_uint(tri.q[2]), 0u);
-                dst[3] = make_uint4(0u, 0u, 0u, 0u);
-                store_colour_slot(dst + 4, oc, tri.id2);
-            }
+            emit_wide(PP, env, lane, wide, tri, j0, j1, oc, overflow);
         }
     }
     __syncwarp();
@@ -528,7 +578,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1024 / (WARPS * 32)) geom_kernel(c
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(1024) order_kernel(const PipeParams PP, const int since_phase1) {
     __shared__ unsigned hist[256];
-    const int tid = threadIdx.x, N = PP.g.N;
+    const int tid = threadIdx.x, N = PP.g.N * PP.bands;   // tasks: (environment, band)
     auto cost = [&](int e) {
         unsigned n = PP.cnt[2 * e], w = PP.cnt[2 * e + 1];
         if (since_phase1) { n -= PP.cnt1[2 * e]; w -= PP.cnt1[2 * e + 1]; }
@@ -568,7 +618,6 @@ struct RastWarpSmem {
     uint32_t *fq;    // [FQ_CAP] covered fragments: r | (x - i0) << 5 | (y - j0) << 12
 };
 constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4;
-constexpr int BIG_CAP = 512;       // entries of the pass-B list
 
 __host__ __device__ inline size_t raster_smem_bytes(int W, int H, int warps) {
     return (size_t)W * H * 8 + (size_t)warps * RAST_WARP_SMEM;
@@ -786,8 +835,8 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, un
 // wide records: one triangle at a time, the whole warp walks its bounding box in 8x4-pixel blocks with the
 // int64 edge functions of N6
 template <bool STATS>
-__device__ __forceinline__ void raster_wide(const uint4 *env_recs, uint32_t slot0, int ntri, int W, int H, float zfar,
-                                            unsigned long long *fb, int lane, unsigned &n_frag) {
+__device__ __forceinline__ void raster_wide(const uint4 *env_recs, uint32_t slot0, int ntri, int W, int H, int y_lo, int bh,
+                                            float zfar, unsigned long long *fb, int lane, unsigned &n_frag) {
     const unsigned FULL = 0xFFFFFFFFu;
     Tri tri;
 #pragma unroll
@@ -812,6 +861,8 @@ __device__ __forceinline__ void raster_wide(const uint4 *env_recs, uint32_t slot
         bt.id2 = __shfl_sync(FULL, tri.id2, src);
         int bi0, bi1, bj0, bj1;
         pixel_bbox(bt.X, bt.Y, W, H, bi0, bi1, bj0, bj1);
+        bj0 = max(bj0, y_lo);                 // the band's rows only (frame rows y_lo .. y_lo + bh - 1)
+        bj1 = min(bj1, y_lo + bh - 1);
         Edges BE;
         edge_setup(bt, area2(bt), BE);   // orientation-normalised by the geometry kernel: area > 0
         const int lx = lane & 7, ly = lane >> 3;
@@ -823,14 +874,14 @@ __device__ __forceinline__ void raster_wide(const uint4 *env_recs, uint32_t slot
                 if (!cover_depth(BE, bt.q, i, j, f, num, depth)) continue;
                 if (STATS) ++n_frag;
                 if (depth > zfar) continue;
-                key_min_rec(&fb[fb_index(i, j, W)], __float_as_uint(depth), idx, bt.id2, env_recs);
+                key_min_rec(&fb[fb_index(i, j - y_lo, W)], __float_as_uint(depth), idx, bt.id2, env_recs);
             }
     }
     __syncwarp();
 }
 
-// K5a: colour (N8) and id of the winning record at pixel (x, y)
-__device__ __forceinline__ uint32_t resolve_rec(const uint4 *env_recs, uint32_t cap_n, uint32_t idx, int x, int y,
+// K5a: colour (N8) and id of the winning record at pixel (x, y) of the band whose first frame row is y_lo
+__device__ __forceinline__ uint32_t resolve_rec(const uint4 *env_recs, uint32_t cap_n, uint32_t idx, int x, int y, int y_lo,
                                                 bool want_rgb, uint32_t &id) {
     const uint4 *rp = env_recs + (size_t)idx * 4;
     const uint4 u1 = __ldg(rp + 1);
@@ -867,7 +918,7 @@ __device__ __forceinline__ uint32_t resolve_rec(const uint4 *env_recs, uint32_t 
         Edges E;
         edge_setup(t, area2(t), E);
         float num, depth;
-        cover_depth(E, t.q, x, y, f, num, depth);   // covered by construction: this triangle won the pixel
+        cover_depth(E, t.q, x, y + y_lo, f, num, depth);   // covered by construction: this triangle won the pixel
     }
     if (fcol) {
         const uint4 v1 = __ldg(rp + 5), v2 = __ldg(rp + 6), v3 = __ldg(rp + 7);
@@ -901,14 +952,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int NT = WARPS * 32;
     const int W = P.W, H = P.H, npix = W * H;
+    const int bh = PP.bh, npb = W * bh;   // rows and pixels of one band: the CTA's frame
 
     unsigned long long *fb = reinterpret_cast<unsigned long long *>(smem);
     RastWarpSmem ws;
-    ws.rec = reinterpret_cast<uint32_t *>(smem + (size_t)npix * 8 + (size_t)warp * RAST_WARP_SMEM);
+    ws.rec = reinterpret_cast<uint32_t *>(smem + (size_t)npb * 8 + (size_t)warp * RAST_WARP_SMEM);
     ws.fq = ws.rec + REC_WORDS * 32;
 
     __shared__ int s_env;
     __shared__ unsigned s_next, s_next_b, s_big;
+    constexpr int BIG_CAP = 16 * WARPS;     // entries of the pass-B list
     __shared__ uint2 s_big_list[BIG_CAP];   // (group, first chunk) of the groups left to pass B
     __shared__ float s_hz[HZ_STRIDE];
     __shared__ unsigned long long s_frag, s_culled;
@@ -918,33 +971,34 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
     if (PHASE != 2) {
         uint4 *f4 = reinterpret_cast<uint4 *>(fb);
-        for (int k = tid; k < npix / 2; k += NT) f4[k] = ones;
+        for (int k = tid; k < npb / 2; k += NT) f4[k] = ones;
     }
     const bool want_rgb = P.rgb != nullptr;
     const uint32_t cap_n = (uint32_t)PP.cap_n;
-    const float *hz = PHASE == 2 ? s_hz : nullptr;
 
     for (;;) {
-        if (tid == 0) {
+        if (tid == 0) {   // next task: (environment, band), heaviest first
             const unsigned k = atomicAdd(&PP.counters[1], 1u);
-            s_env = k < (unsigned)P.N ? (int)PP.order[k] : -1;
+            s_env = k < (unsigned)(P.N * PP.bands) ? (int)PP.order[k] : -1;
             s_next = 0; s_next_b = 0; s_big = 0;
         }
         __syncthreads();
-        const int env = s_env;
-        if (env < 0) break;
+        const int v = s_env;
+        if (v < 0) break;
+        const int env = v / PP.bands, y_lo = (v - env * PP.bands) * bh;
+        const float *hz = PHASE == 2 ? s_hz + (y_lo >> 3) * 16 : nullptr;
         if (PP.env_flag[env]) {   // overflowed its pool segment: left to the single-kernel pass
             __syncthreads();
             continue;
         }
-        const uint4 *env_recs = PP.recs + (size_t)env * (size_t)(PP.cap_n + PP.cap_w) * 4;
-        const uint32_t n_n = PP.cnt[2 * env], n_w = PP.cnt[2 * env + 1] >> 1;
-        const uint32_t b_n = PHASE == 2 ? PP.cnt1[2 * env] : 0u, b_w = PHASE == 2 ? PP.cnt1[2 * env + 1] >> 1 : 0u;
+        const uint4 *env_recs = PP.recs + (size_t)v * (size_t)(PP.cap_n + PP.cap_w) * 4;
+        const uint32_t n_n = PP.cnt[2 * v], n_w = PP.cnt[2 * v + 1] >> 1;
+        const uint32_t b_n = PHASE == 2 ? PP.cnt1[2 * v] : 0u, b_w = PHASE == 2 ? PP.cnt1[2 * v + 1] >> 1 : 0u;
         const uint32_t g_n = (n_n - b_n + 31u) >> 5, g_w = (n_w - b_w + 31u) >> 5;
         if (PHASE == 2) {   // the occluder phase's frame and hi-Z tiles
-            const uint4 *src = reinterpret_cast<const uint4 *>(PP.frames + (size_t)env * npix);
+            const uint4 *src = reinterpret_cast<const uint4 *>(PP.frames + (size_t)v * npb);
             uint4 *f4 = reinterpret_cast<uint4 *>(fb);
-            for (int k = tid; k < npix / 2; k += NT) f4[k] = __ldg(src + k);
+            for (int k = tid; k < npb / 2; k += NT) f4[k] = __ldg(src + k);
             for (int k = tid; k < HZ_STRIDE; k += NT) s_hz[k] = PP.hiz[(size_t)env * HZ_STRIDE + k];
             __syncthreads();
         }
@@ -980,7 +1034,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                 }
             } else {   // wide records first: they reach the near plane and hide the most
                 const uint32_t t0 = b_w + g * 32u;
-                raster_wide<STATS>(env_recs, cap_n + 2u * t0, (int)min(32u, n_w - t0), W, H, P.zfar, fb, lane, st_frag);
+                raster_wide<STATS>(env_recs, cap_n + 2u * t0, (int)min(32u, n_w - t0), W, H, y_lo, bh, P.zfar, fb, lane, st_frag);
             }
         }
         __syncthreads();
@@ -1015,7 +1069,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
         if (PHASE == 1) {
             // ---- occluder phase: hi-Z tiles (max depth per 8x8 tile, +inf where background shows), the frame
             // keys and the record counts go to global memory; the frame is reset for the next environment
-            const int tw = W >> 3, th = H >> 3;
+            const int tw = W >> 3, th = bh >> 3, ty0 = y_lo >> 3;   // the band's tile rows are ty0 .. ty0 + th - 1
             for (int t = warp; t < tw * th; t += WARPS) {
                 const int ty = t / tw, tx = t - ty * tw;
                 const int j = ty * 8 + (lane >> 2), i = tx * 8 + (lane & 3) * 2;
@@ -1024,24 +1078,25 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                 d = __reduce_max_sync(0xFFFFFFFFu, d);
                 if (lane == 0) s_hz[ty * 16 + tx] = d == 0xFFFFFFFFu ? __int_as_float(0x7F800000) : __uint_as_float(d);
             }
-            for (int t = tid; t < 16; t += NT) s_hz[256 + t] = 0.0f;
             __syncthreads();
-            if (tid < 16) {   // 32x32-pixel tiles: max over 4x4 of the above (tiles outside the frame count as 0)
-                const int by = tid >> 2, bx = tid & 3;
+            float *g_hz = PP.hiz + (size_t)env * HZ_STRIDE;
+            for (int t = tid; t < th * 16; t += NT) g_hz[ty0 * 16 + t] = s_hz[t];
+            // 32x32-pixel tiles: max over 4x4 of the above (a band of several bands is a multiple of 32 rows high)
+            for (int t = tid; t < ((th + 3) >> 2) * 4; t += NT) {
+                const int by = t >> 2, bx = t & 3;
                 float z = 0.0f;
                 for (int ty = by * 4; ty < min(by * 4 + 4, th); ++ty)
                     for (int tx = bx * 4; tx < min(bx * 4 + 4, tw); ++tx) z = fmaxf(z, s_hz[ty * 16 + tx]);
-                s_hz[256 + tid] = z;
+                g_hz[256 + ((ty0 >> 2) + by) * 4 + bx] = z;
             }
-            __syncthreads();
-            for (int k = tid; k < HZ_STRIDE; k += NT) PP.hiz[(size_t)env * HZ_STRIDE + k] = s_hz[k];
-            uint4 *dst = reinterpret_cast<uint4 *>(PP.frames + (size_t)env * npix);
+            uint4 *dst = reinterpret_cast<uint4 *>(PP.frames + (size_t)v * npb);
             uint4 *f4 = reinterpret_cast<uint4 *>(fb);
-            for (int k = tid; k < npix / 2; k += NT) { dst[k] = f4[k]; f4[k] = ones; }
-            if (tid < 2) PP.cnt1[2 * env + tid] = PP.cnt[2 * env + tid];
+            for (int k = tid; k < npb / 2; k += NT) { dst[k] = f4[k]; f4[k] = ones; }
+            if (tid < 2) PP.cnt1[2 * v + tid] = PP.cnt[2 * v + tid];
         } else {
             // ---- K5: resolve the winners, write RGB / depth / id as 16-byte stores, reset the frame ------
-            for (int k = tid; k < npix / 4; k += NT) {
+            const size_t out0 = (size_t)env * npix + (size_t)y_lo * W;   // first pixel of the band in the outputs
+            for (int k = tid; k < npb / 4; k += NT) {
                 const int pix = k * 4;
                 const int j = pix / W, i = pix - j * W;
                 const int a = fb_index(i, j, W);          // 4-aligned columns stay contiguous under the XOR
@@ -1060,11 +1115,11 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                     dp[m] = 0.0f;
                     if (db[m] != 0xFFFFFFFFu) {
                         dp[m] = __uint_as_float(db[m]);
-                        if (want_rgb || P.id) col[m] = resolve_rec(env_recs, cap_n, idx[m], i + m, j, want_rgb, id[m]);
+                        if (want_rgb || P.id) col[m] = resolve_rec(env_recs, cap_n, idx[m], i + m, j, y_lo, want_rgb, id[m]);
                     }
                 }
-                *reinterpret_cast<float4 *>(P.depth + (size_t)env * npix + pix) = d;
-                if (P.id) *reinterpret_cast<uint4 *>(P.id + (size_t)env * npix + pix) = make_uint4(id[0], id[1], id[2], id[3]);
+                *reinterpret_cast<float4 *>(P.depth + out0 + pix) = d;
+                if (P.id) *reinterpret_cast<uint4 *>(P.id + out0 + pix) = make_uint4(id[0], id[1], id[2], id[3]);
                 if (want_rgb) {
                     // 4 pixels = 12 bytes = 3 words per lane; 4 lanes hold 48 bytes = three 16-byte stores
                     const uint32_t w0 = (col[0] & 0xFFFFFFu) | (col[1] << 24);
@@ -1081,7 +1136,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                         o[r] = wsel == 0 ? a0 : (wsel == 1 ? a1 : a2);
                     }
                     if (g < 3) {
-                        uint8_t *dst = P.rgb + ((size_t)env * npix + (size_t)(pix - 4 * g)) * 3 + 16 * g;
+                        uint8_t *dst = P.rgb + (out0 + (size_t)(pix - 4 * g)) * 3 + 16 * g;
                         *reinterpret_cast<uint4 *>(dst) = make_uint4(o[0], o[1], o[2], o[3]);
                     }
                 }

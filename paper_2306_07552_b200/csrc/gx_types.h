@@ -12,6 +12,7 @@
 // batches.  Triangle order is never changed, so triangle id = position in the caller's index array.
 constexpr int GX_CLUSTER_TRIS = 256;
 constexpr int GX_VCAP = 256;            // unique vertices per batch (8-bit local indices)
+constexpr int GX_SUBS_PER_BATCH = GX_CLUSTER_TRIS / 32;   // sub-cluster = 32 consecutive triangles = one warp pass
 constexpr int GX_MAX_BATCH_PER_CLUSTER = 4;  // 85 soup triangles need 255 vertices -> ceil(256/85) = 4
 
 struct __align__(16) GxBatchDev {
@@ -38,6 +39,7 @@ struct GxParams {
     const float4 *verts;          // x, y, z, rgba8 bits; per batch contiguous
     const uchar4 *tris;           // three batch-local vertex indices; per batch contiguous
     const GxBatchDev *batches;
+    const GxClusterDev *subs;     // [batch][GX_SUBS_PER_BATCH] AABB of each run of 32 consecutive triangles of a batch
     const GxClusterDev *clusters;
     const GxMeshDev *meshes;      // static meshes first, then dynamic
     int32_t n_static, n_dyn;

@@ -76,7 +76,7 @@ def test_cull_is_conservative(oracle_mod):
     wl = gen.make_config(1, n_envs=16)
     a = render_gpu(wl, cull=1, stats=True, options=dict(occlusion=0))
     b = render_gpu(wl, cull=0, stats=True)
-    c = render_gpu(wl, cull=1, stats=True)            # frustum + occlusion culling (the default)
+    c = render_gpu(wl, cull=1, stats=True, options=dict(occlusion=1))   # frustum + hi-Z occlusion culling
     for k in ("rgb", "depth", "id"):
         assert np.array_equal(a[k], b[k]), k
         assert np.array_equal(c[k], b[k]), k
@@ -92,7 +92,7 @@ def test_paths_pool_overflow_and_chunking(oracle_mod):
     a pool budget that forces several chunks; other raster pass-B thresholds: all bit-identical."""
     wl = gen.make_config(2, n_envs=20)
     o = oracle_mod.render(wl)
-    ref = render_gpu(wl, stats=True)
+    ref = render_gpu(wl, stats=True, options=dict(occlusion=1))
     rep = compare(o, ref)
     assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, rep
     assert ref["stats"]["overflow_envs"] == 0 and ref["stats"]["launches"] == 9
@@ -100,10 +100,15 @@ def test_paths_pool_overflow_and_chunking(oracle_mod):
         "single kernel": dict(path=1),
         "some overflow": dict(pool_slots=12288),
         "all overflow": dict(pool_slots=64),
-        "chunks of 3": dict(pool_bytes=3 * (65536 + 8192) * 64),
+        "chunks of 3": dict(pool_bytes=3 * (65536 + 8192) * 64, occlusion=1),
         "no occluder phase": dict(occlusion=0),
-        "occluder phase 5 %": dict(occluder_pct=5),
-        "occluder phase 70 %": dict(occluder_pct=70),
+        "1 band": dict(bands=1),
+        "no sub-cluster culling": dict(subcull=0),
+        "4 bands": dict(bands=4),
+        "4 bands, no occluder phase": dict(bands=4, occlusion=0),
+        "occluder phase 5 %": dict(occlusion=1, occluder_pct=5),
+        "occluder phase 70 %": dict(occlusion=1, occluder_pct=70),
+        "4 bands, occluder phase": dict(bands=4, occlusion=1),
         "small pass-B chunks": dict(big_slots=64, chunk_slots=32),
         "no pass B": dict(big_slots=1 << 20),
     }
