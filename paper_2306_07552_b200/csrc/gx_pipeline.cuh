@@ -787,26 +787,26 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, un
                 sx[e] = -(dy[e] << 8);
             }
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const bool c = ((Ee[0] | Ee[1] | Ee[2]) >= 0) && (a + k < w);
-                m4 |= (c ? 1u : 0u) << k;
+            for (int k = 0; k < 4; ++k) {   // covered iff no edge value (bias already subtracted) is negative
+                m4 |= ((unsigned)~(Ee[0] | Ee[1] | Ee[2]) >> 31) << k;
                 Ee[0] += sx[0]; Ee[1] += sx[1]; Ee[2] += sx[2];
             }
+            m4 &= (1u << min(4, w - a)) - 1u;   // pixels beyond the bounding box
         }
-        // append the covered pixels: four independent ballots, predicated stores
-        const unsigned b0 = __ballot_sync(FULL, m4 & 1u), b1 = __ballot_sync(FULL, m4 & 2u),
-                       b2 = __ballot_sync(FULL, m4 & 4u), b3 = __ballot_sync(FULL, m4 & 8u);
-        if (b0 | b1 | b2 | b3) {
-            const uint32_t en = (uint32_t)r | ((uint32_t)a << 5) | ((uint32_t)row << 12);
-            const int p0 = qn + __popc(b0 & lt);
-            const int c1 = qn + __popc(b0), p1 = c1 + __popc(b1 & lt);
-            const int c2 = c1 + __popc(b1), p2 = c2 + __popc(b2 & lt);
-            const int c3 = c2 + __popc(b2), p3 = c3 + __popc(b3 & lt);
-            sts_if(fq_addr + (uint32_t)p0 * 4u, en, m4 & 1u);
-            sts_if(fq_addr + (uint32_t)p1 * 4u, en + 32u, m4 & 2u);
-            sts_if(fq_addr + (uint32_t)p2 * 4u, en + 64u, m4 & 4u);
-            sts_if(fq_addr + (uint32_t)p3 * 4u, en + 96u, m4 & 8u);
-            qn = c3 + __popc(b3);
+        // append the covered pixels: the lanes' counts (0..4) are prefix-summed with three ballots, one per bit
+        const int cnt = __popc(m4);
+        const unsigned c0 = __ballot_sync(FULL, cnt & 1), c1 = __ballot_sync(FULL, cnt & 2), c2 = __ballot_sync(FULL, cnt & 4);
+        if (c0 | c1 | c2) {
+            uint32_t en = (uint32_t)r | ((uint32_t)a << 5) | ((uint32_t)row << 12);
+            uint32_t addr = fq_addr + (uint32_t)(qn + __popc(c0 & lt) + 2 * __popc(c1 & lt) + 4 * __popc(c2 & lt)) * 4u;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t bit = (m4 >> k) & 1u;
+                sts_if(addr, en, bit);
+                addr += bit << 2;
+                en += 32u;
+            }
+            qn += __popc(c0) + 2 * __popc(c1) + 4 * __popc(c2);
         }
         if (act) {
             if (++chunk == cw) {
