@@ -182,7 +182,7 @@ def run_reference(args):
 def run_gx(args):
     import torch
     import torch.distributed as dist
-    from paper_2306_07552_b200 import accounting, binding as gx, build as gx_build
+    from paper_2306_07552_b200 import accounting, binding as gx, build as gx_build, sharding
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -227,6 +227,7 @@ def run_gx(args):
         for _ in range(max(args.warmup, 0)):
             step()
         barrier()
+        gx.gx_set_option(scene, "timing", 1)     # CUDA events around every kernel, on the stream the kernels run on
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
         for a, b in ev:
             flush.zero_()            # L2 flush between timed iterations (untimed)
@@ -235,6 +236,9 @@ def run_gx(args):
             b.record()
         barrier()
         ms = [a.elapsed_time(b) for a, b in ev]
+        kernel_ns = {k: gx.gx_get_stat(scene, "ns_" + k) for k in ("cull", "geom", "order", "raster", "fallback")}
+        timed_calls = gx.gx_get_stat(scene, "timed_calls")
+        gx.gx_set_option(scene, "timing", 0)
         # keep the GPU under load a little longer so that nvidia-smi (200 ms period) sees the render clocks
         t_end = time.perf_counter() + max(0.0, 1.0 - 1e-3 * sum(ms))
         while time.perf_counter() < t_end:
@@ -242,10 +246,7 @@ def run_gx(args):
             torch.cuda.synchronize()
     total_ms = float(sum(ms))
     launches = gx.gx_get_stat(scene, "launches")
-    t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms_max = float(t.item())
+    total_ms_max = sharding.max_over_ranks(total_ms, dev)        # time of the job = the slowest rank's
     ms_per_step = total_ms_max / args.steps
     value = world * N * args.steps / (total_ms_max * 1e-3)
 
@@ -284,18 +285,37 @@ def run_gx(args):
             dist.destroy_process_group()
         return
 
-    # ---- roofline: algorithmic bytes / render-kernel time --------------------------------------------
+    # ---- roofline: algorithmic bytes of the whole path / time of the path's kernels -----------------------
+    # The algorithmic bytes (accounting.py) belong to the whole hot path K1..K5, which is four kernels per step
+    # (cull, geometry, raster order, raster) plus the overflow pass; `achieved` divides by the sum of their
+    # event-timed durations.  The dominant kernel (raster) and every kernel's share are reported beside it.
     peak, peak_src = measured_peak()
     b = accounting.env_bytes(wl)
     bytes_per_launch = float(b["total"].sum())
-    kernel_ms = total_ms / args.steps                  # one kernel per step: its duration is the step's
+    kernels_ms = {k: v * 1e-6 / max(timed_calls, 1) for k, v in kernel_ns.items()}
+    kernel_ms = sum(kernels_ms.values()) if timed_calls else total_ms / args.steps
     achieved = bytes_per_launch / (kernel_ms * 1e-3) / 1e9
+    traffic = None      # DRAM bytes per launch of all our kernels, from the committed ncu capture of this workload
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "r1e_traffic.csv")) as f:
+            rows = [r for r in csv.DictReader(f) if int(r["workload_config"]) == args.config]
+        if rows and not args.opt and not args.envs:
+            traffic = float(sum(int(r["dram_bytes_per_launch"]) for r in rows))
+    except Exception:
+        pass
+    dom = max(kernels_ms, key=kernels_ms.get) if timed_calls else "raster"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "kernel": "gx::render_kernel",
-                "kernel_ms": kernel_ms, "algorithmic_bytes_per_launch": bytes_per_launch,
+                "traffic": traffic, "peak_source": peak_src,
+                "kernel": "gx pipeline: cull_kernel + geom_kernel + order_kernel + raster_kernel (+ overflow pass)",
+                "kernel_ms": kernel_ms, "kernels_ms": kernels_ms,
+                "dominant_kernel": {"name": "gx::" + dom + "_kernel", "ms": kernels_ms.get(dom),
+                                    "share_of_kernel_time": (kernels_ms.get(dom, 0.0) / kernel_ms) if kernel_ms else None},
+                "algorithmic_bytes_per_launch": bytes_per_launch,
                 "bytes_per_env": {k: float(b[k].mean()) for k in ("cull", "geom", "out", "total")},
                 "post_cull_tris_per_env": float(b["tris"].mean()),
-                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS}
+                "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
+                "note": "issue-bound, not DRAM-bound: see DESIGN.md section 7"}
     cpu = None if args.no_cpu_baseline else time_oracle(wl)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

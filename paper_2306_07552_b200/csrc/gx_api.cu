@@ -93,6 +93,12 @@ struct GxScene {
     int opt_big_slots = 512, opt_chunk_slots = 256;   // raster pass B (gx_pipeline.cuh)
     DevBuf<uint4> pool;                 // triangle records of one chunk of environments
     DevBuf<unsigned long long> frames;  // frame keys between the two raster phases
+    // kernel timing (option "timing"): CUDA events recorded on the caller's stream around every kernel class
+    int opt_timing = 0;
+    std::vector<cudaEvent_t> t_ev;      // recorded marks, in order
+    std::vector<int> t_kind;            // what ran before the mark: 0 = start of a pass, 1 cull, 2 geom, 3 order, 4 raster, 5 fallback
+    size_t t_used = 0;
+    int t_calls = 0;
     int opt_subcull = 1;                // geometry kernel: frustum (and hi-Z) test per 32-triangle sub-cluster
     int opt_bands = 0;                  // raster bands per frame; 0 = automatic
     int opt_occlusion = 0;              // occluder phase + hi-Z culling of clusters and records
@@ -245,15 +251,33 @@ int launch_raster(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stre
     return GX_OK;
 }
 
+// timing mark: an event on the stream; the time since the previous mark belongs to kernel class `kind`
+int mark(GxScene *sc, cudaStream_t stream, int kind) {
+    if (!sc->opt_timing || sc->t_used >= 8192) return GX_OK;
+    if (sc->t_used == sc->t_ev.size()) {
+        cudaEvent_t e;
+        GX_CUDA(cudaEventCreate(&e));
+        sc->t_ev.push_back(e);
+        sc->t_kind.push_back(0);
+    }
+    sc->t_kind[sc->t_used] = kind;
+    GX_CUDA(cudaEventRecord(sc->t_ev[sc->t_used], stream));
+    ++sc->t_used;
+    return GX_OK;
+}
+
 // one pass of the pipeline (gx_pipeline.cuh): cull kernel, geometry kernel, raster order, raster kernel.
 // PHASE 0 = everything in one pass; 1 = occluder phase; 2 = the rest, culled against the occluder phase's hi-Z.
 template <int PHASE>
-int launch_pass(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
+int launch_pass(GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
+    int rc;
+    if ((rc = mark(sc, stream, 0)) != GX_OK) return rc;
     constexpr int CW = 4, GW = 8, CP = PHASE == 2 ? 2 : 1;
     auto ck = stats ? gx::cull_kernel<CW, CP, true> : gx::cull_kernel<CW, CP, false>;
     const size_t csmem = gx::env_smem_bytes(PP.g.K);
     ck<<<PP.g.N, CW * 32, csmem, stream>>>(PP);
     GX_CUDA(cudaGetLastError());
+    if ((rc = mark(sc, stream, 1)) != GX_OK) return rc;
     auto gk = stats ? gx::geom_kernel<GW, true> : gx::geom_kernel<GW, false>;
     const size_t gsmem = (size_t)GW * gx::GEOM_WARP_SMEM;
     GX_CUDA(cudaFuncSetAttribute(gk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem));
@@ -262,13 +286,17 @@ int launch_pass(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream
     if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "geometry kernel does not fit: %zu bytes of shared memory", gsmem);
     gk<<<sc->num_sms * per_sm, GW * 32, gsmem, stream>>>(PP);
     GX_CUDA(cudaGetLastError());
+    if ((rc = mark(sc, stream, 2)) != GX_OK) return rc;
     gx::order_kernel<<<1, 1024, 0, stream>>>(PP, PHASE == 2 ? 1 : 0);
     GX_CUDA(cudaGetLastError());
+    if ((rc = mark(sc, stream, 3)) != GX_OK) return rc;
     // one band of 64-bit keys per CTA: the smaller the band, the more CTAs share an SM (32 warps per SM in all cases)
     const size_t band_bytes = (size_t)PP.g.W * PP.bh * 8;
-    if (band_bytes <= 32768) return launch_raster<8, 4, PHASE>(sc, PP, stream, stats);
-    if (band_bytes <= 65536) return launch_raster<16, 2, PHASE>(sc, PP, stream, stats);
-    return launch_raster<32, 1, PHASE>(sc, PP, stream, stats);
+    if (band_bytes <= 32768) rc = launch_raster<8, 4, PHASE>(sc, PP, stream, stats);
+    else if (band_bytes <= 65536) rc = launch_raster<16, 2, PHASE>(sc, PP, stream, stats);
+    else rc = launch_raster<32, 1, PHASE>(sc, PP, stream, stats);
+    if (rc != GX_OK) return rc;
+    return mark(sc, stream, 4);
 }
 
 }  // namespace
@@ -367,6 +395,7 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->env_counter);
     cudaFree(sc->stats);
     sc->pool.release(); sc->pipe_scratch.release(); sc->frames.release();
+    for (cudaEvent_t e : sc->t_ev) cudaEventDestroy(e);
     sc->h_env_scene.release(); sc->h_inst_mesh.release(); sc->h_cam_pose.release(); sc->h_inst_xform.release();
     sc->h_depth.release(); sc->h_rgb.release(); sc->h_id.release();
     if (sc->host_stream) cudaStreamDestroy(sc->host_stream);
@@ -377,6 +406,11 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
     if (!sc || !name) return fail(GX_ERR_INVALID_ARG, "NULL argument");
     if (!strcmp(name, "cull")) { sc->opt_cull = value != 0; return GX_OK; }
     if (!strcmp(name, "stats")) { sc->opt_stats = value != 0; return GX_OK; }
+    if (!strcmp(name, "timing")) {   // 1 = start (and reset) the per-kernel event timing, 0 = stop recording
+        sc->opt_timing = value != 0;
+        if (value) { sc->t_used = 0; sc->t_calls = 0; }
+        return GX_OK;
+    }
     if (!strcmp(name, "subcull")) { sc->opt_subcull = value != 0; return GX_OK; }
     if (!strcmp(name, "bands")) {
         if (value != 0 && value != 1 && value != 2 && value != 4) return fail(GX_ERR_INVALID_ARG, "bands must be 0, 1, 2 or 4");
@@ -415,6 +449,24 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
 int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
     if (!sc || !name || !out) return fail(GX_ERR_INVALID_ARG, "NULL argument");
     if (!strcmp(name, "launches")) { *out = sc->last_launches; return GX_OK; }
+    if (!strcmp(name, "timed_calls")) { *out = sc->t_calls; return GX_OK; }
+    if (!strncmp(name, "ns_", 3)) {   // nanoseconds per kernel class, summed over the calls since "timing" was set
+        static const char *kinds[6] = {"", "cull", "geom", "order", "raster", "fallback"};
+        int kind = 0;
+        for (int k = 1; k < 6; ++k) if (!strcmp(name + 3, kinds[k])) kind = k;
+        if (!kind) return fail(GX_ERR_INVALID_ARG, "unknown stat '%s'", name);
+        DeviceGuard guard(sc->device);
+        if (sc->t_used) GX_CUDA(cudaEventSynchronize(sc->t_ev[sc->t_used - 1]));
+        double ns = 0.0;
+        for (size_t k = 1; k < sc->t_used; ++k)
+            if (sc->t_kind[k] == kind) {
+                float ms = 0.0f;
+                GX_CUDA(cudaEventElapsedTime(&ms, sc->t_ev[k - 1], sc->t_ev[k]));
+                ns += 1e6 * (double)ms;
+            }
+        *out = (int64_t)ns;
+        return GX_OK;
+    }
     if (!strcmp(name, "max_env_records") || !strcmp(name, "p50_env_records")) {   // last chunk of the two-kernel path
         *out = 0;
         if (sc->last_chunk_n <= 0) return GX_OK;
@@ -563,10 +615,12 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PL.env_counter = sc->pipe_scratch.p + 3;
         PL.env_filter = PP.env_flag;
         if ((rc = launch_single(sc, PL, stream, st)) != GX_OK) return rc;
+        if ((rc = mark(sc, stream, 5)) != GX_OK) return rc;
         launches += 1;
         sc->last_chunk_n = n * bands;
     }
     sc->last_launches = launches;
+    if (sc->opt_timing) ++sc->t_calls;
     return GX_OK;
 }
 
