@@ -47,7 +47,7 @@ typedef struct {
 
 /* Pinhole camera shared by all environments of a call. */
 typedef struct {
-    int32_t width, height; /* pixels; multiples of 16; width*height <= 16384 in this build */
+    int32_t width, height; /* pixels; multiples of 16; each <= 128 in this build */
     float fx, fy;          /* NDC focal lengths: fy = 1/tan(fovy/2), fx = fy*height/width; 90 deg square: 1 */
     float znear, zfar;     /* metres, 0 < znear < zfar; fragments with view depth > zfar are dropped */
 } GxCamera;
@@ -89,7 +89,7 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
  * NaN/Inf inputs and out-of-range env_scene/inst_mesh values are precondition violations: the image is
  * undefined, but no out-of-bounds write occurs for in-range ids.
  * Errors: INVALID_ARG (null handle/camera/required pointer, N <= 0, K < 0, K > GX_MAX_INSTANCES, width or
- * height not a positive multiple of 16, znear <= 0, zfar <= znear), UNSUPPORTED (width*height > 16384),
+ * height not a positive multiple of 16, znear <= 0, zfar <= znear), UNSUPPORTED (width or height > 128),
  * OOM, CUDA.
  */
 int gx_render_batch(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K, const int32_t *env_scene,
@@ -106,17 +106,35 @@ int gx_render_batch_host(GxScene *scene, const GxCamera *camera, int32_t N, int3
                          uint8_t *rgb_out, float *depth_out, uint32_t *id_out);
 
 /*
- * gx_set_option -- tuning / verification switches of a handle.  Unknown names return INVALID_ARG.
- *   "cull"  0|1  (default 1): per-environment frustum culling of clusters (K1).  Culling is
- *                conservative: the images with 0 and 1 are bit-identical (tested).
+ * gx_set_option -- tuning / verification switches of a handle.  Unknown names and out-of-range values return
+ * INVALID_ARG.  Every switch leaves the images bit-identical (tested); they only move time around.
+ *   "cull"         0|1 (1)   per-environment frustum culling of clusters and 32-triangle sub-clusters (K1).
+ *   "subcull"      0|1 (1)   the sub-cluster test in the geometry kernel.
+ *   "path"         0|1 (0)   0 = cull / geometry / raster kernels over a triangle-record pool;
+ *                            1 = the single-kernel renderer (also the pass that renders environments whose
+ *                            records overflow their pool segment).
+ *   "bands"        0|1|2|4 (0 = automatic: 2 for frames above 64 KB of keys) raster tasks per frame.
+ *   "occlusion"    0|1 (0)   occluder pass + hi-Z culling of clusters, sub-clusters and records in a second pass.
+ *   "occluder_pct" 1..100 (25) share of the visible clusters, nearest first, drawn in the occluder pass.
+ *   "pool_slots"   narrow record slots per (environment, band); 0 = max(2048, 4*W*H/bands).
+ *   "pool_bytes"   record pool budget, which bounds the environments per pass; 0 = 8 GB.
+ *   "big_slots", "chunk_slots"  raster pass B: a group of more than big_slots 4-pixel slots is drawn in chunks
+ *                            of chunk_slots (512, 256).
+ *   "stats"        0|1 (0)   count what gx_get_stat reports (slower kernels).
+ *   "timing"       0|1 (0)   1 starts (and resets), 0 stops recording CUDA events around every kernel of
+ *                            subsequent gx_render_batch calls on their stream.
  */
 int gx_set_option(GxScene *scene, const char *name, int64_t value);
 
 /*
- * gx_get_stat -- counters of the most recent gx_render_batch on this handle; synchronises the stream the
- * call ran on.  Names: "clusters_tested", "clusters_drawn", "triangles_in" (triangles of drawn clusters),
- * "triangles_raster" (survived clip, zero-area and pixel-centre bounding-box rejection), "fragments"
- * (pixel-centre hits before the depth test), "launches" (kernels launched by the call).
+ * gx_get_stat -- counters of the most recent gx_render_batch on this handle ("stats" = 1); synchronises the
+ * stream the call ran on.  Names: "clusters_tested", "clusters_drawn", "triangles_in" (triangles of drawn
+ * sub-clusters), "triangles_raster" (survived clip, zero-area and pixel-centre bounding-box rejection),
+ * "fragments" (pixel-centre hits before the depth test), "overflow_envs" (environments rendered by the overflow
+ * pass), "clusters_occluded", "records_occluded" (occluder scheme), "max_env_records", "p50_env_records"
+ * (records per raster task, last chunk), "launches" (kernels launched by the call).
+ * With "timing": "timed_calls" and "ns_cull", "ns_geom", "ns_order", "ns_raster", "ns_fallback" = nanoseconds
+ * spent in each kernel class, summed over the calls since timing was started.
  * Unknown names return INVALID_ARG; *out receives the value.
  */
 int gx_get_stat(GxScene *scene, const char *name, int64_t *out);
