@@ -226,6 +226,7 @@ def run_gx(args):
     with ClockSampler(local) as clk:
         for _ in range(max(args.warmup, 0)):
             step()
+            torch.cuda.synchronize()   # lets the handle read back its record counts and size its pool (one-off)
         barrier()
         gx.gx_set_option(scene, "timing", 1)     # CUDA events around every kernel, on the stream the kernels run on
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]

@@ -103,6 +103,11 @@ struct GxScene {
     int opt_bands = 0;                  // raster bands per frame; 0 = automatic
     int opt_occlusion = 0;              // occluder phase + hi-Z culling of clusters and records
     int opt_occluder_pct = 25;          // share of the visible clusters (nearest first) drawn in the occluder phase
+    // pool sizing from history: the largest record counts any raster task of earlier calls produced
+    uint32_t *d_maxrec = nullptr, *h_maxrec = nullptr;   // device [2]; pinned host [2]
+    cudaEvent_t ev_maxrec = nullptr;
+    bool maxrec_pending = false;
+    uint32_t hist_n = 0, hist_w = 0;
     DevBuf<uint32_t> pipe_scratch;      // counters[4] | cnt[2*chunk] | env_flag[chunk]
     int last_launches = 0;
     cudaStream_t last_stream = nullptr;
@@ -396,6 +401,9 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->stats);
     sc->pool.release(); sc->pipe_scratch.release(); sc->frames.release();
     for (cudaEvent_t e : sc->t_ev) cudaEventDestroy(e);
+    if (sc->d_maxrec) cudaFree(sc->d_maxrec);
+    if (sc->h_maxrec) cudaFreeHost(sc->h_maxrec);
+    if (sc->ev_maxrec) cudaEventDestroy(sc->ev_maxrec);
     sc->h_env_scene.release(); sc->h_inst_mesh.release(); sc->h_cam_pose.release(); sc->h_inst_xform.release();
     sc->h_depth.release(); sc->h_rgb.release(); sc->h_id.release();
     if (sc->host_stream) cudaStreamDestroy(sc->host_stream);
@@ -547,8 +555,25 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     int bands = sc->opt_bands > 0 ? sc->opt_bands : (npix * 8 > 65536 ? 2 : 1);
     while (bands > 1 && (P.H % bands || (P.H / bands) % 32)) bands >>= 1;
     const int bh = P.H / bands;
-    const int64_t cap_n = sc->opt_pool_slots > 0 ? sc->opt_pool_slots : std::max<int64_t>(2048, 4 * npix / bands);
-    const int64_t cap_w = std::max<int64_t>(64, cap_n / 8) & ~(int64_t)1;
+    // pool segment per raster task: a default from the frame size, raised to 1.25 x the largest record count any
+    // task of an earlier call on this handle produced (read back asynchronously; a call whose segments are too
+    // small is still rendered correctly, by the overflow pass, and the next call is sized for it)
+    if (!sc->d_maxrec) {
+        GX_CUDA(cudaMalloc(&sc->d_maxrec, 2 * sizeof(uint32_t)));
+        GX_CUDA(cudaMallocHost(&sc->h_maxrec, 2 * sizeof(uint32_t)));
+        GX_CUDA(cudaEventCreateWithFlags(&sc->ev_maxrec, cudaEventDisableTiming));
+    }
+    if (sc->maxrec_pending && cudaEventQuery(sc->ev_maxrec) == cudaSuccess) {
+        sc->hist_n = std::max(sc->hist_n, sc->h_maxrec[0]);
+        sc->hist_w = std::max(sc->hist_w, sc->h_maxrec[1]);
+        sc->maxrec_pending = false;
+    }
+    cudaGetLastError();   // (cudaErrorNotReady of the query is not an error)
+    auto grow = [](uint32_t seen) { return ((int64_t)seen + seen / 4 + 1023) & ~(int64_t)1023; };
+    const int64_t cap_n = sc->opt_pool_slots > 0 ? sc->opt_pool_slots
+                                                 : std::max<int64_t>(std::max<int64_t>(2048, 4 * npix / bands), grow(sc->hist_n));
+    const int64_t cap_w = sc->opt_pool_slots > 0 ? (std::max<int64_t>(64, cap_n / 8) & ~(int64_t)1)
+                                                 : std::max<int64_t>(std::max<int64_t>(64, cap_n / 8) & ~(int64_t)1, grow(sc->hist_w));
     const int64_t env_bytes = (cap_n + cap_w) * 64 * bands;
     const int64_t budget = sc->opt_pool_bytes > 0 ? sc->opt_pool_bytes : (int64_t)8 << 30;
     const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(N, budget / env_bytes));
@@ -566,6 +591,7 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     if ((rc = sc->pipe_scratch.reserve(off_items + 2 * (size_t)chunk * std::max<size_t>(items_per_env, 1))) != GX_OK) return rc;
     if (two_phase && (rc = sc->frames.reserve((size_t)chunk * (size_t)npix)) != GX_OK) return rc;
     int launches = 0;
+    GX_CUDA(cudaMemsetAsync(sc->d_maxrec, 0, 2 * sizeof(uint32_t), stream));
     for (int e0 = 0; e0 < N; e0 += chunk) {
         const int n = std::min(chunk, N - e0);
         gx::PipeParams PP;
@@ -596,6 +622,7 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.big_slots = sc->opt_big_slots;
         PP.chunk_slots = sc->opt_chunk_slots;
         PP.order = sc->pipe_scratch.p + off_order;
+        PP.maxrec = sc->d_maxrec;
         PP.env_idb = sc->pipe_scratch.p + off_idb;
         PP.env_mv = reinterpret_cast<float *>(sc->pipe_scratch.p + off_mv);
         PP.items = reinterpret_cast<uint2 *>(sc->pipe_scratch.p + off_items);
@@ -618,6 +645,11 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         if ((rc = mark(sc, stream, 5)) != GX_OK) return rc;
         launches += 1;
         sc->last_chunk_n = n * bands;
+    }
+    if (!sc->maxrec_pending) {   // (a read-back still in flight keeps its buffer)
+        GX_CUDA(cudaMemcpyAsync(sc->h_maxrec, sc->d_maxrec, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
+        GX_CUDA(cudaEventRecord(sc->ev_maxrec, stream));
+        sc->maxrec_pending = true;
     }
     sc->last_launches = launches;
     if (sc->opt_timing) ++sc->t_calls;

@@ -46,6 +46,7 @@ struct PipeParams {
     float *env_mv;           // [N][K+1][12] model-view per slot
     uint32_t *env_idb;       // [N][K+1] first triangle id per slot
     uint32_t *order;         // [N] raster order of the environments
+    uint32_t *maxrec;        // [2] largest narrow / wide record count of any task of the call (sizes the next call's pool)
     uint32_t *cnt1;          // [N][2] record counts at the end of the occluder phase
     float *thr;              // [N] occluder phase: clusters with wmin < thr are drawn first
     float *hiz;              // [N][HZ_STRIDE] max depth per 8x8-pixel tile (stride 16) and per 32x32 tile (at +256)
@@ -586,9 +587,15 @@ __global__ void __launch_bounds__(1024) order_kernel(const PipeParams PP, const 
     };
     if (tid < 256) hist[tid] = 0;
     __syncthreads();
+    unsigned mx_n = 0, mx_w = 0;
     for (int e = tid; e < N; e += 1024) {
         atomicAdd(&hist[255u - min(255u, cost(e) >> 7)], 1u);
+        mx_n = max(mx_n, PP.cnt[2 * e]);
+        mx_w = max(mx_w, PP.cnt[2 * e + 1]);
     }
+    mx_n = __reduce_max_sync(0xFFFFFFFFu, mx_n);
+    mx_w = __reduce_max_sync(0xFFFFFFFFu, mx_w);
+    if ((tid & 31) == 0) { atomicMax(&PP.maxrec[0], mx_n); atomicMax(&PP.maxrec[1], mx_w); }
     __syncthreads();
     if (tid < 32) {   // exclusive scan of the 256 bins by one warp, 8 bins per lane
         unsigned v[8], sum = 0;
