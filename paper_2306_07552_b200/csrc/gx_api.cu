@@ -101,8 +101,9 @@ struct GxScene {
     int t_calls = 0;
     int opt_subcull = 1;                // geometry kernel: frustum (and hi-Z) test per 32-triangle sub-cluster
     int opt_bands = 0;                  // raster bands per frame; 0 = automatic
-    int opt_occlusion = 0;              // occluder phase + hi-Z culling of clusters and records
-    int opt_occluder_pct = 25;          // share of the visible clusters (nearest first) drawn in the occluder phase
+    int opt_occlusion = 2;              // occluder phase + hi-Z culling of clusters and records
+    int opt_occl_area = 64;              // occluder scheme: sub-clusters with >= this many screen-box pixels per triangle go first
+    int opt_occluder_pct = 50;          // share of the visible clusters (nearest first) drawn in the occluder phase
     // pool sizing from history: the largest record counts any raster task of earlier calls produced
     uint32_t *d_maxrec = nullptr, *h_maxrec = nullptr;   // device [2]; pinned host [2]
     cudaEvent_t ev_maxrec = nullptr;
@@ -277,7 +278,7 @@ template <int PHASE>
 int launch_pass(GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
     int rc;
     if ((rc = mark(sc, stream, 0)) != GX_OK) return rc;
-    constexpr int CW = 4, GW = 8, CP = PHASE == 2 ? 2 : 1;
+    constexpr int CW = 4, GW = 8, CP = PHASE >= 2 ? 2 : 1;
     auto ck = stats ? gx::cull_kernel<CW, CP, true> : gx::cull_kernel<CW, CP, false>;
     const size_t csmem = gx::env_smem_bytes(PP.g.K);
     ck<<<PP.g.N, CW * 32, csmem, stream>>>(PP);
@@ -292,7 +293,7 @@ int launch_pass(GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool
     gk<<<sc->num_sms * per_sm, GW * 32, gsmem, stream>>>(PP);
     GX_CUDA(cudaGetLastError());
     if ((rc = mark(sc, stream, 2)) != GX_OK) return rc;
-    gx::order_kernel<<<1, 1024, 0, stream>>>(PP, PHASE == 2 ? 1 : 0);
+    gx::order_kernel<<<1, 1024, 0, stream>>>(PP, PHASE >= 2 ? 1 : 0);
     GX_CUDA(cudaGetLastError());
     if ((rc = mark(sc, stream, 3)) != GX_OK) return rc;
     // one band of 64-bit keys per CTA: the smaller the band, the more CTAs share an SM (32 warps per SM in all cases)
@@ -425,7 +426,16 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
         sc->opt_bands = (int)value;
         return GX_OK;
     }
-    if (!strcmp(name, "occlusion")) { sc->opt_occlusion = value != 0; return GX_OK; }
+    if (!strcmp(name, "occlusion")) {
+        if (value != 0 && value != 2 && value != 3) return fail(GX_ERR_INVALID_ARG, "occlusion must be 0, 2 or 3 (passes)");
+        sc->opt_occlusion = (int)value;
+        return GX_OK;
+    }
+    if (!strcmp(name, "occl_area")) {
+        if (value < 0 || value > 16384) return fail(GX_ERR_INVALID_ARG, "occl_area out of range");
+        sc->opt_occl_area = (int)value;
+        return GX_OK;
+    }
     if (!strcmp(name, "occluder_pct")) {
         if (value < 1 || value > 100) return fail(GX_ERR_INVALID_ARG, "occluder_pct must be in [1, 100]");
         sc->opt_occluder_pct = (int)value;
@@ -481,7 +491,7 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
         DeviceGuard guard(sc->device);
         std::vector<uint32_t> cnt(2 * (size_t)sc->last_chunk_n);
         GX_CUDA(cudaStreamSynchronize(sc->last_stream));
-        GX_CUDA(cudaMemcpy(cnt.data(), sc->pipe_scratch.p + 8, cnt.size() * 4, cudaMemcpyDeviceToHost));
+        GX_CUDA(cudaMemcpy(cnt.data(), sc->pipe_scratch.p + 12, cnt.size() * 4, cudaMemcpyDeviceToHost));
         std::vector<uint32_t> tot(sc->last_chunk_n);
         for (int e = 0; e < sc->last_chunk_n; ++e) tot[e] = cnt[2 * e] + cnt[2 * e + 1];
         std::sort(tot.begin(), tot.end());
@@ -579,12 +589,12 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(N, budget / env_bytes));
     int rc;
     if ((rc = sc->pool.reserve((size_t)chunk * bands * (size_t)(cap_n + cap_w) * 4)) != GX_OK) return rc;
-    // scratch words: counters[8] | cnt[2*tasks] | env_flag[chunk] (zeroed per chunk) | order[tasks] | cnt1[2*tasks] |
+    // scratch words: counters[12] | cnt[2*tasks] | env_flag[chunk] (zeroed per chunk) | order[tasks] | cnt1[2*tasks] |
     //                thr[chunk] | env_idb[chunk*(K+1)] | env_mv[chunk*(K+1)*12] | hiz[chunk*HZ_STRIDE] | items[2*...]
-    const bool two_phase = sc->opt_cull && sc->opt_occlusion && sc->opt_occluder_pct < 100;
+    const bool two_phase = sc->opt_cull && sc->opt_occlusion >= 2;   // occluder scheme: 2 or 3 passes
     const size_t k1 = (size_t)K + 1, tasks = (size_t)chunk * bands;
     const size_t items_per_env = (size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches;
-    const size_t n_zero = 8 + 2 * tasks + (size_t)chunk;
+    const size_t n_zero = 12 + 2 * tasks + (size_t)chunk;
     const size_t off_order = n_zero, off_cnt1 = off_order + tasks, off_thr = off_cnt1 + 2 * tasks;
     const size_t off_idb = off_thr + chunk, off_mv = off_idb + chunk * k1, off_hiz = off_mv + chunk * k1 * 12;
     const size_t off_items = (off_hiz + (size_t)chunk * gx::HZ_STRIDE + 1) & ~(size_t)1;
@@ -606,8 +616,8 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.g.id = id_out ? id_out + (size_t)e0 * npix : nullptr;
         PP.recs = sc->pool.p;
         PP.counters = sc->pipe_scratch.p;
-        PP.cnt = sc->pipe_scratch.p + 8;
-        PP.env_flag = sc->pipe_scratch.p + 8 + 2 * tasks;
+        PP.cnt = sc->pipe_scratch.p + 12;
+        PP.env_flag = sc->pipe_scratch.p + 12 + 2 * tasks;
         PP.cnt1 = sc->pipe_scratch.p + off_cnt1;
         PP.thr = reinterpret_cast<float *>(sc->pipe_scratch.p + off_thr);
         PP.hiz = reinterpret_cast<float *>(sc->pipe_scratch.p + off_hiz);
@@ -627,13 +637,22 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.env_mv = reinterpret_cast<float *>(sc->pipe_scratch.p + off_mv);
         PP.items = reinterpret_cast<uint2 *>(sc->pipe_scratch.p + off_items);
         GX_CUDA(cudaMemsetAsync(sc->pipe_scratch.p, 0, n_zero * sizeof(uint32_t), stream));
+        PP.nphase = two_phase ? sc->opt_occlusion : 0;
+        PP.occl_area = (float)sc->opt_occl_area;
         if (!two_phase) {
             if ((rc = launch_pass<0>(sc, PP, stream, st)) != GX_OK) return rc;
             launches += 4;
         } else {
+            PP.phase = 1;
             if ((rc = launch_pass<1>(sc, PP, stream, st)) != GX_OK) return rc;
+            if (PP.nphase == 3) {
+                PP.counters = sc->pipe_scratch.p + 8;
+                PP.phase = 2;
+                if ((rc = launch_pass<3>(sc, PP, stream, st)) != GX_OK) return rc;
+                launches += 4;
+            }
             PP.counters = sc->pipe_scratch.p + 4;
-            PP.phase = 2;
+            PP.phase = PP.nphase;
             if ((rc = launch_pass<2>(sc, PP, stream, st)) != GX_OK) return rc;
             launches += 8;
         }

@@ -54,7 +54,8 @@ struct PipeParams {
     int32_t occl_pct;        // share of the frustum-visible clusters (nearest first) drawn in the occluder phase
     int32_t cap_n, cap_w;    // slots per (environment, band)
     int32_t subcull;         // geometry: test every 32-triangle sub-cluster of a batch (frustum; hi-Z in phase 2)
-    int32_t phase;           // 2 while the second pass of the occluder scheme runs, else 0
+    int32_t phase, nphase;   // occluder scheme: pass 1 .. nphase of nphase (2 or 3); 0 = single pass
+    float occl_area;         // a sub-cluster is a 'big-triangle' occluder if its screen box has this many pixels per triangle
     int32_t bands, bh;       // horizontal bands per frame, rows per band (H = bands * bh)
     int32_t big_slots, chunk_slots;   // raster pass B: groups above big_slots are drawn in chunks of chunk_slots
 };
@@ -85,6 +86,21 @@ __device__ __forceinline__ bool box_occluded(const CamBox &b, const float *hz, f
             for (int tx = pxl >> 5; tx <= (pxh >> 5); ++tx) zmax = fmaxf(zmax, hz[256 + ty * 4 + tx]);
     }
     return b.wmin * (1.0f - 1e-4f) > zmax;
+}
+
+// class of a sub-cluster (32 triangles) in the occluder scheme: 0 = drawn in the first pass, ..., n - 1 = in the last.
+// Big-triangle sub-clusters (screen box area / 32 >= occl_area, or reaching the near plane) are the occluders:
+// they cover many pixels for little geometry.  With three passes the far ones of them (wmin >= thr) wait for
+// the second pass.  Any classification gives the same image; this one only decides what can be culled.
+__device__ __forceinline__ int sub_class(const CamBox &b, float fx, float fy, int W, int H, float znear, float occl_area,
+                                         float thr, int nphase) {
+    if (!(b.wmin >= znear)) return 0;
+    const float iw = 1.0f / b.wmin;   // the nearest depth gives the largest possible screen box
+    const float wpx = fminf(2.0f * b.ex * fx * iw * 0.5f * (float)W, (float)W);
+    const float hpx = fminf(2.0f * b.ey * fy * iw * 0.5f * (float)H, (float)H);
+    const bool big = wpx * hpx >= occl_area * 32.0f;
+    if (nphase == 2) return big ? 0 : 1;
+    return big ? (b.wmin < thr ? 0 : 1) : 2;
 }
 
 struct GeomWarpSmem {
@@ -222,12 +238,19 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
     // tests the AABB of pass k against the frustum (and, in the second pass of the occluder scheme, against
     // the hi-Z tiles).  A pass whose bit is clear is skipped; a batch with no bit set costs nothing more.
     unsigned sub_mask = 0xFFFFFFFFu;
-    if (PP.subcull) {
+    if (PP.subcull || PP.phase) {
         bool vis = false;
         if (lane * 32 < nt) {
             const CamBox bx = cluster_box(P.subs[(size_t)batch * GX_SUBS_PER_BATCH + lane], M);
-            vis = box_in_frustum(bx, P.fx, P.fy, P.znear, P.zfar);
-            if (vis && PP.phase == 2) vis = !box_occluded(bx, PP.hiz + (size_t)env * HZ_STRIDE, P.fx, P.fy, P.W, P.H, P.znear);
+            vis = !PP.subcull || box_in_frustum(bx, P.fx, P.fy, P.znear, P.zfar);
+            if (vis && PP.phase) {
+                // occluder scheme: pass 1 draws the sub-clusters whose triangles are big on screen (cheap
+                // occluders) -- only the near ones of them when there are three passes --, the later passes
+                // draw the rest, minus what the hi-Z tiles of the passes before prove hidden
+                const int cls = sub_class(bx, P.fx, P.fy, P.W, P.H, P.znear, PP.occl_area, PP.thr[env], PP.nphase);
+                vis = cls == PP.phase - 1 &&
+                      (PP.phase == 1 || !box_occluded(bx, PP.hiz + (size_t)env * HZ_STRIDE, P.fx, P.fy, P.W, P.H, P.znear));
+            }
         }
         sub_mask = __ballot_sync(FULL, vis);
         if (sub_mask == 0u) return;
@@ -413,7 +436,7 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
         for (int k = tid; k <= K; k += NT) g_idb[k] = es.id_base[k];
     }
     const uint32_t n_cl = es.cl_base[K + 1];
-    const bool two_phase = P.cull && PP.occl_pct < 100;
+    const bool two_phase = P.cull && PP.nphase >= 2;
 
     auto slot_of = [&](uint32_t g) {
         int lo = 0, hi = K;
@@ -484,12 +507,10 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
                 vis = box_in_frustum(b, P.fx, P.fy, P.znear, P.zfar);
                 if (PHASE == 1) {
                     if (STATS) { ++st_tested; st_drawn += vis ? 1u : 0u; }
-                    vis = vis && b.wmin < thr;
                 } else {
-                    const bool cand = vis && !(b.wmin < thr);
-                    const bool occ = cand && box_occluded(b, s_hz, P.fx, P.fy, P.W, P.H, P.znear);
+                    const bool occ = vis && box_occluded(b, s_hz, P.fx, P.fy, P.W, P.H, P.znear);
                     if (STATS) st_tested += occ ? 1u : 0u;   // (PHASE 2: st_tested counts the clusters proved hidden)
-                    vis = cand && !occ;
+                    vis = vis && !occ;
                 }
             } else if (STATS) { ++st_tested; ++st_drawn; }
             if (vis) { nb = c.nbatch; boff = c.batch_off; }
@@ -947,15 +968,17 @@ __device__ __forceinline__ uint32_t resolve_rec(const uint4 *env_recs, uint32_t 
 
 
 // ------------------------------------------------------------------------------------------------
-// the raster kernel.  PHASE 0: draw all records of the environment and write the images.  PHASE 1 (occluder
-// phase): draw the records present so far, then leave the frame keys, the hi-Z tiles and the record counts
-// in global memory.  PHASE 2: start from those keys, draw only the records appended since, skipping records
-// the hi-Z tiles prove hidden, and write the images.
+// the raster kernel.  PHASE 0: draw all records of the task and write the images.  PHASE 1 (first occluder
+// pass): draw the records present so far, then leave the frame keys, the hi-Z tiles and the record counts in
+// global memory.  PHASE 2 (last pass): start from those keys, draw only the records appended since, skipping
+// records the hi-Z tiles prove hidden, and write the images.  PHASE 3 (middle pass): start like 2, end like 1.
 // ------------------------------------------------------------------------------------------------
 template <int WARPS, int MINB, int PHASE, bool STATS>
 __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipeParams PP) {
     extern __shared__ __align__(16) unsigned char smem[];
     const GxParams &P = PP.g;
+    constexpr bool LOAD = PHASE == 2 || PHASE == 3;   // start from the previous pass's frame keys and hi-Z tiles
+    constexpr bool DUMP = PHASE == 1 || PHASE == 3;   // leave frame keys, hi-Z tiles and record counts for the next pass
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int NT = WARPS * 32;
     const int W = P.W, H = P.H, npix = W * H;
@@ -976,7 +999,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     unsigned st_frag = 0, st_culled = 0;
     if (STATS && tid == 0) { s_frag = 0; s_culled = 0; }
     const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
-    if (PHASE != 2) {
+    if (!LOAD) {
         uint4 *f4 = reinterpret_cast<uint4 *>(fb);
         for (int k = tid; k < npb / 2; k += NT) f4[k] = ones;
     }
@@ -993,16 +1016,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
         const int v = s_env;
         if (v < 0) break;
         const int env = v / PP.bands, y_lo = (v - env * PP.bands) * bh;
-        const float *hz = PHASE == 2 ? s_hz + (y_lo >> 3) * 16 : nullptr;
+        const float *hz = LOAD ? s_hz + (y_lo >> 3) * 16 : nullptr;
         if (PP.env_flag[env]) {   // overflowed its pool segment: left to the single-kernel pass
             __syncthreads();
             continue;
         }
         const uint4 *env_recs = PP.recs + (size_t)v * (size_t)(PP.cap_n + PP.cap_w) * 4;
         const uint32_t n_n = PP.cnt[2 * v], n_w = PP.cnt[2 * v + 1] >> 1;
-        const uint32_t b_n = PHASE == 2 ? PP.cnt1[2 * v] : 0u, b_w = PHASE == 2 ? PP.cnt1[2 * v + 1] >> 1 : 0u;
+        const uint32_t b_n = LOAD ? PP.cnt1[2 * v] : 0u, b_w = LOAD ? PP.cnt1[2 * v + 1] >> 1 : 0u;
         const uint32_t g_n = (n_n - b_n + 31u) >> 5, g_w = (n_w - b_w + 31u) >> 5;
-        if (PHASE == 2) {   // the occluder phase's frame and hi-Z tiles
+        if (LOAD) {   // the previous pass's frame and hi-Z tiles
             const uint4 *src = reinterpret_cast<const uint4 *>(PP.frames + (size_t)v * npb);
             uint4 *f4 = reinterpret_cast<uint4 *>(fb);
             for (int k = tid; k < npb / 2; k += NT) f4[k] = __ldg(src + k);
@@ -1073,8 +1096,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
         }
         __syncthreads();
 
-        if (PHASE == 1) {
-            // ---- occluder phase: hi-Z tiles (max depth per 8x8 tile, +inf where background shows), the frame
+        if (DUMP) {
+            // ---- occluder pass: hi-Z tiles (max depth per 8x8 tile, +inf where background shows), the frame
             // keys and the record counts go to global memory; the frame is reset for the next environment
             const int tw = W >> 3, th = bh >> 3, ty0 = y_lo >> 3;   // the band's tile rows are ty0 .. ty0 + th - 1
             for (int t = warp; t < tw * th; t += WARPS) {
@@ -1098,7 +1121,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
             }
             uint4 *dst = reinterpret_cast<uint4 *>(PP.frames + (size_t)v * npb);
             uint4 *f4 = reinterpret_cast<uint4 *>(fb);
-            for (int k = tid; k < npb / 2; k += NT) { dst[k] = f4[k]; f4[k] = ones; }
+            for (int k = tid; k < npb / 2; k += NT) { dst[k] = f4[k]; if (!LOAD) f4[k] = ones; }
             if (tid < 2) PP.cnt1[2 * v + tid] = PP.cnt[2 * v + tid];
         } else {
             // ---- K5: resolve the winners, write RGB / depth / id as 16-byte stores, reset the frame ------
