@@ -98,8 +98,9 @@ int gx_render_batch(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K
 
 /*
  * gx_render_batch_host -- the same operation with every array argument in HOST memory (pageable or
- * pinned): copies the inputs to the device, renders, copies the outputs back and synchronises the stream
- * before returning.  This is the end-to-end entry point bench.py times for its "e2e" figure.
+ * pinned): copies the inputs to the device, renders in sub-batches of 512 environments while the images of
+ * the previous sub-batch are copied back on a second stream, and synchronises before returning.  This is the
+ * end-to-end entry point bench.py times for its "e2e" figure.
  */
 int gx_render_batch_host(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K, const int32_t *env_scene,
                          const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform,
@@ -114,8 +115,12 @@ int gx_render_batch_host(GxScene *scene, const GxCamera *camera, int32_t N, int3
  *                            1 = the single-kernel renderer (also the pass that renders environments whose
  *                            records overflow their pool segment).
  *   "bands"        0|1|2|4 (0 = automatic: 2 for frames above 64 KB of keys) raster tasks per frame.
- *   "occlusion"    0|1 (0)   occluder pass + hi-Z culling of clusters, sub-clusters and records in a second pass.
- *   "occluder_pct" 1..100 (25) share of the visible clusters, nearest first, drawn in the occluder pass.
+ *   "occlusion"    0..3 (1)  occluder scheme: 0 = one pass; 2 = the sub-clusters whose triangles are
+ *                            big on screen are drawn first, the others are culled against their hi-Z tiles and
+ *                            drawn in a second pass; 3 = the far big ones wait for a middle pass; 1 = automatic
+ *                            (2 passes for frames of >= 8192 pixels and batches of >= 512 environments).
+ *   "occl_area"    (64)      screen-box pixels per triangle from which a sub-cluster counts as big.
+ *   "occluder_pct" 1..100 (50) three passes only: share of the visible clusters, nearest first, that are "near".
  *   "pool_slots"   narrow record slots per (environment, band); 0 = max(2048, 4*W*H/bands).
  *   "pool_bytes"   record pool budget, which bounds the environments per pass; 0 = 8 GB.
  *   "big_slots", "chunk_slots"  raster pass B: a group of more than big_slots 4-pixel slots is drawn in chunks

@@ -101,7 +101,7 @@ struct GxScene {
     int t_calls = 0;
     int opt_subcull = 1;                // geometry kernel: frustum (and hi-Z) test per 32-triangle sub-cluster
     int opt_bands = 0;                  // raster bands per frame; 0 = automatic
-    int opt_occlusion = 2;              // occluder phase + hi-Z culling of clusters and records
+    int opt_occlusion = 1;              // occluder scheme: 0 off, 2 or 3 passes, 1 = automatic
     int opt_occl_area = 64;              // occluder scheme: sub-clusters with >= this many screen-box pixels per triangle go first
     int opt_occluder_pct = 50;          // share of the visible clusters (nearest first) drawn in the occluder phase
     // pool sizing from history: the largest record counts any raster task of earlier calls produced
@@ -117,7 +117,8 @@ struct GxScene {
     DevBuf<float> h_cam_pose, h_inst_xform, h_depth;
     DevBuf<uint8_t> h_rgb;
     DevBuf<uint32_t> h_id;
-    cudaStream_t host_stream = nullptr;
+    cudaStream_t host_stream = nullptr, copy_stream = nullptr;
+    cudaEvent_t ev_sub = nullptr;
 };
 
 namespace {
@@ -408,6 +409,8 @@ void gx_destroy(GxScene *sc) {
     sc->h_env_scene.release(); sc->h_inst_mesh.release(); sc->h_cam_pose.release(); sc->h_inst_xform.release();
     sc->h_depth.release(); sc->h_rgb.release(); sc->h_id.release();
     if (sc->host_stream) cudaStreamDestroy(sc->host_stream);
+    if (sc->copy_stream) cudaStreamDestroy(sc->copy_stream);
+    if (sc->ev_sub) cudaEventDestroy(sc->ev_sub);
     delete sc;
 }
 
@@ -427,7 +430,7 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
         return GX_OK;
     }
     if (!strcmp(name, "occlusion")) {
-        if (value != 0 && value != 2 && value != 3) return fail(GX_ERR_INVALID_ARG, "occlusion must be 0, 2 or 3 (passes)");
+        if (value < 0 || value > 3) return fail(GX_ERR_INVALID_ARG, "occlusion must be 0 (off), 1 (automatic), 2 or 3 (passes)");
         sc->opt_occlusion = (int)value;
         return GX_OK;
     }
@@ -591,7 +594,10 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     if ((rc = sc->pool.reserve((size_t)chunk * bands * (size_t)(cap_n + cap_w) * 4)) != GX_OK) return rc;
     // scratch words: counters[12] | cnt[2*tasks] | env_flag[chunk] (zeroed per chunk) | order[tasks] | cnt1[2*tasks] |
     //                thr[chunk] | env_idb[chunk*(K+1)] | env_mv[chunk*(K+1)*12] | hiz[chunk*HZ_STRIDE] | items[2*...]
-    const bool two_phase = sc->opt_cull && sc->opt_occlusion >= 2;   // occluder scheme: 2 or 3 passes
+    // occluder scheme: 2 or 3 passes; automatic = 2 passes where they pay: frames of 8192 pixels or more (the hi-Z
+    // tiles are 8x8 pixels) and enough environments that two rounds of kernels still fill the GPU
+    const int n_pass = sc->opt_occlusion == 1 ? ((npix >= 8192 && N >= 512) ? 2 : 0) : sc->opt_occlusion;
+    const bool two_phase = sc->opt_cull && n_pass >= 2;
     const size_t k1 = (size_t)K + 1, tasks = (size_t)chunk * bands;
     const size_t items_per_env = (size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches;
     const size_t n_zero = 12 + 2 * tasks + (size_t)chunk;
@@ -637,7 +643,7 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.env_mv = reinterpret_cast<float *>(sc->pipe_scratch.p + off_mv);
         PP.items = reinterpret_cast<uint2 *>(sc->pipe_scratch.p + off_items);
         GX_CUDA(cudaMemsetAsync(sc->pipe_scratch.p, 0, n_zero * sizeof(uint32_t), stream));
-        PP.nphase = two_phase ? sc->opt_occlusion : 0;
+        PP.nphase = two_phase ? n_pass : 0;
         PP.occl_area = (float)sc->opt_occl_area;
         if (!two_phase) {
             if ((rc = launch_pass<0>(sc, PP, stream, st)) != GX_OK) return rc;
@@ -701,13 +707,28 @@ int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K,
         GX_CUDA(cudaMemcpyAsync(sc->h_inst_mesh.p, inst_mesh, nk * 4, cudaMemcpyHostToDevice, st));
         GX_CUDA(cudaMemcpyAsync(sc->h_inst_xform.p, inst_xform, nk * 64, cudaMemcpyHostToDevice, st));
     }
-    rc = gx_render_batch(sc, cam, N, K, sc->h_env_scene.p, sc->h_cam_pose.p, K > 0 ? sc->h_inst_mesh.p : nullptr,
-                         K > 0 ? sc->h_inst_xform.p : nullptr, rgb_out ? sc->h_rgb.p : nullptr, sc->h_depth.p,
-                         id_out ? sc->h_id.p : nullptr, st);
-    if (rc != GX_OK) return rc;
-    GX_CUDA(cudaMemcpyAsync(depth_out, sc->h_depth.p, N * npix * 4, cudaMemcpyDeviceToHost, st));
-    if (rgb_out) GX_CUDA(cudaMemcpyAsync(rgb_out, sc->h_rgb.p, N * npix * 3, cudaMemcpyDeviceToHost, st));
-    if (id_out) GX_CUDA(cudaMemcpyAsync(id_out, sc->h_id.p, N * npix * 4, cudaMemcpyDeviceToHost, st));
+    // render in sub-batches of 512 environments and copy each one's images back on a second stream while the next
+    // one renders (the device-to-host copy of RGBD is as long as the rendering itself)
+    if (!sc->copy_stream) {
+        GX_CUDA(cudaStreamCreateWithFlags(&sc->copy_stream, cudaStreamNonBlocking));
+        GX_CUDA(cudaEventCreateWithFlags(&sc->ev_sub, cudaEventDisableTiming));
+    }
+    const int sub = 512;
+    for (int e0 = 0; e0 < N; e0 += sub) {
+        const int n = std::min(sub, N - e0);
+        const size_t o = (size_t)e0 * npix, cnt = (size_t)n * npix;
+        rc = gx_render_batch(sc, cam, n, K, sc->h_env_scene.p + e0, sc->h_cam_pose.p + (size_t)e0 * 16,
+                             K > 0 ? sc->h_inst_mesh.p + (size_t)e0 * K : nullptr,
+                             K > 0 ? sc->h_inst_xform.p + (size_t)e0 * K * 16 : nullptr,
+                             rgb_out ? sc->h_rgb.p + o * 3 : nullptr, sc->h_depth.p + o, id_out ? sc->h_id.p + o : nullptr, st);
+        if (rc != GX_OK) return rc;
+        GX_CUDA(cudaEventRecord(sc->ev_sub, st));
+        GX_CUDA(cudaStreamWaitEvent(sc->copy_stream, sc->ev_sub, 0));
+        GX_CUDA(cudaMemcpyAsync(depth_out + o, sc->h_depth.p + o, cnt * 4, cudaMemcpyDeviceToHost, sc->copy_stream));
+        if (rgb_out) GX_CUDA(cudaMemcpyAsync(rgb_out + o * 3, sc->h_rgb.p + o * 3, cnt * 3, cudaMemcpyDeviceToHost, sc->copy_stream));
+        if (id_out) GX_CUDA(cudaMemcpyAsync(id_out + o, sc->h_id.p + o, cnt * 4, cudaMemcpyDeviceToHost, sc->copy_stream));
+    }
+    GX_CUDA(cudaStreamSynchronize(sc->copy_stream));
     GX_CUDA(cudaStreamSynchronize(st));
     return GX_OK;
 }
