@@ -179,23 +179,28 @@ int build_mesh(const GxMesh &m, std::vector<float4> &verts, std::vector<uchar4> 
                 li.w = 0;
                 tris.push_back(li);
             }
-            for (uint32_t v : touched) local[v] = -1;
             b.nv_nt = nv | (nt << 16);
             // sub-clusters: AABB of every run of 32 consecutive triangles of the batch
             for (uint32_t k = 0; k < (uint32_t)GX_SUBS_PER_BATCH; ++k) {
                 GxClusterDev sb;
-                sb.batch_off = 0; sb.nbatch = 0;
+                uint32_t vlo = 0xFFFFu, vhi = 0;   // batch-local vertex index range of the sub-cluster's triangles
                 for (int a = 0; a < 3; ++a) { sb.bmin[a] = 3.0e38f; sb.bmax[a] = -3.0e38f; }
                 for (uint32_t tt = b.first_tri + 32 * k; tt < std::min(b.first_tri + 32 * (k + 1), b.first_tri + nt); ++tt)
                     for (int kk = 0; kk < 3; ++kk) {
+                        const uint32_t lv = (uint32_t)local[m.indices[3 * (size_t)tt + kk]];
+                        vlo = std::min(vlo, lv);
+                        vhi = std::max(vhi, lv);
                         const float *pp = m.positions + 3 * (size_t)m.indices[3 * (size_t)tt + kk];
                         for (int a = 0; a < 3; ++a) {
                             sb.bmin[a] = std::min(sb.bmin[a], pp[a]);
                             sb.bmax[a] = std::max(sb.bmax[a], pp[a]);
                         }
                     }
+                sb.batch_off = vlo;   // (fields reused: first and last vertex the sub-cluster references)
+                sb.nbatch = vhi;
                 subs.push_back(sb);
             }
+            for (uint32_t v : touched) local[v] = -1;
             batches.push_back(b);
             ++c.nbatch;
         }

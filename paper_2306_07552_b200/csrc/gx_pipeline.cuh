@@ -238,10 +238,13 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
     // tests the AABB of pass k against the frustum (and, in the second pass of the occluder scheme, against
     // the hi-Z tiles).  A pass whose bit is clear is skipped; a batch with no bit set costs nothing more.
     unsigned sub_mask = 0xFFFFFFFFu;
+    int v_lo = 0, v_hi = nv - 1;   // vertices the visible sub-clusters reference
     if (PP.subcull || PP.phase) {
         bool vis = false;
+        int lo = 0xFFFF, hi = -1;
         if (lane * 32 < nt) {
-            const CamBox bx = cluster_box(P.subs[(size_t)batch * GX_SUBS_PER_BATCH + lane], M);
+            const GxClusterDev sb = P.subs[(size_t)batch * GX_SUBS_PER_BATCH + lane];
+            const CamBox bx = cluster_box(sb, M);
             vis = !PP.subcull || box_in_frustum(bx, P.fx, P.fy, P.znear, P.zfar);
             if (vis && PP.phase) {
                 // occluder scheme: pass 1 draws the sub-clusters whose triangles are big on screen (cheap
@@ -251,14 +254,17 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                 vis = cls == PP.phase - 1 &&
                       (PP.phase == 1 || !box_occluded(bx, PP.hiz + (size_t)env * HZ_STRIDE, P.fx, P.fy, P.W, P.H, P.znear));
             }
+            if (vis) { lo = (int)sb.batch_off; hi = (int)sb.nbatch; }
         }
         sub_mask = __ballot_sync(FULL, vis);
         if (sub_mask == 0u) return;
+        v_lo = __reduce_min_sync(FULL, lo);
+        v_hi = __reduce_max_sync(FULL, hi);
     }
     if (STATS) n_in += (lane == 0) ? 32u * (unsigned)__popc(sub_mask & ((nt + 31) / 32 < 32 ? (1u << ((nt + 31) / 32)) - 1u : 0xFFFFFFFFu)) : 0u;
 
     // K2a: vertex transform, projection, snap -> warp-private staging
-    for (int v = lane; v < nv; v += 32) {
+    for (int v = v_lo + lane; v <= v_hi; v += 32) {
         const float4 p = __ldg(&verts[v]);
         const CamVert cv = xform(M, p.x, p.y, p.z);
         int X = X_OUT, Y = 0;
