@@ -70,6 +70,36 @@ def test_config3_and_4_sampled(oracle_mod):
         _check(oracle_mod, wl)
 
 
+@pytest.mark.parametrize("cfg,n", [(3, 12), (4, 32)])
+def test_config3_and_4_full_batch(oracle_mod, cfg, n):
+    """configs[3] (4096 envs, 500k-triangle scenes) and configs[4] (16384 envs, 64x64 depth-only) at full size,
+    in the launch configuration bench.py --config times: several chunks of environments per call, two passes
+    (occluder scheme) on cfg 3, four 8-warp raster CTAs per SM on cfg 4.  The oracle renders n sampled
+    environments one by one.  The first call sizes the record pool from defaults (many environments overflow
+    and take the single-kernel pass), the second from the first call's record counts: both must match."""
+    import torch
+    from paper_2306_07552_b200 import binding as gx
+    wl = gen.make_config(cfg)
+    rng = np.random.Generator(np.random.Philox(key=[78, cfg]))
+    sel = np.sort(rng.choice(wl.N, n, replace=False))
+    o = oracle_mod.render(wl.subset(sel))
+    scene = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, 0)
+    try:
+        g1 = render_gpu(wl, scene=scene, stats=True)
+        torch.cuda.synchronize()
+        g2 = render_gpu(wl, scene=scene, stats=True)
+    finally:
+        gx.gx_destroy(scene)
+    assert g1["stats"]["overflow_envs"] > g2["stats"]["overflow_envs"]
+    assert g2["stats"]["overflow_envs"] <= wl.N // 100
+    for g in (g1, g2):
+        gs = {k: (v[sel] if isinstance(v, np.ndarray) else None) for k, v in g.items()}
+        rep = compare(o, gs, check_rgb=not wl.depth_only)
+        assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, rep
+    for k in ("depth", "id") + (() if wl.depth_only else ("rgb",)):
+        assert np.array_equal(g1[k], g2[k]), k
+
+
 def test_cull_is_conservative(oracle_mod):
     """N10: the image with frustum culling on, and with frustum + hi-Z occlusion culling on, equals the image
     with culling off, bit for bit."""
