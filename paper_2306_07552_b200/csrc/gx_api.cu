@@ -90,7 +90,7 @@ struct GxScene {
     int opt_path = 0;                   // 0 = two-kernel path (geometry -> records -> raster), 1 = single kernel
     int64_t opt_pool_slots = 0;         // narrow record slots per environment; 0 = max(4096, 4*W*H)
     int64_t opt_pool_bytes = 0;         // record pool budget; 0 = 8 GB
-    int opt_big_slots = 512, opt_chunk_slots = 256;   // raster pass B (gx_pipeline.cuh)
+    int opt_big_slots = 512, opt_chunk_slots = 128;   // raster pass B (gx_pipeline.cuh)
     DevBuf<uint4> pool;                 // triangle records of one chunk of environments
     DevBuf<unsigned long long> frames;  // frame keys between the two raster phases
     // kernel timing (option "timing"): CUDA events recorded on the caller's stream around every kernel class

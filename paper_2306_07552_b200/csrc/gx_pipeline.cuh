@@ -734,6 +734,7 @@ __device__ __forceinline__ void shade_queue_p(const RastWarpSmem &ws, int qn, in
 // the lane's exclusive prefix of slot counts (Pex, record = lane) and the group's total T.
 // With hz != NULL (second raster phase) a record whose nearest vertex is strictly behind the hi-Z value of
 // every 8x8 tile its bounding box touches gets no slots: none of its fragments could win N9.
+template <int SW>
 __device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int lane, const float *hz, int &Pex,
                                            unsigned &skip, unsigned &n_culled) {
     const unsigned FULL = 0xFFFFFFFFu;
@@ -742,7 +743,7 @@ __device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int
     if (lane < nrec) {
         const uint32_t bb = ws.rec[R_BB * 32 + lane];
         const int w = (int)((bb >> 14) & 127u) + 1, h = (int)((bb >> 21) & 127u) + 1;
-        ns = h * ((w + 3) >> 2);
+        ns = h * ((w + SW - 1) / SW);
         if (hz) {
             const int i0 = (int)(bb & 127u), j0 = (int)((bb >> 7) & 127u);
             const int tx0 = i0 >> 3, tx1 = (i0 + w - 1) >> 3, ty0 = j0 >> 3, ty1 = (j0 + h - 1) >> 3;
@@ -773,7 +774,7 @@ __device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int
 // contiguous runs (a lane walks through its run, moving to the next record when one is exhausted), so that
 // lanes stay busy whatever the mix of triangle sizes.  The covered pixels of one pass are appended to the
 // fragment queue with four ballots and shaded densely by shade_queue_p.
-template <bool STATS>
+template <bool STATS, int SW>
 __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, unsigned skip, int S0, int S1, int W, float zfar,
                                              unsigned long long *fb, uint32_t first, const uint4 *env_recs, int lane,
                                              unsigned &n_frag) {
@@ -803,7 +804,7 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, un
         }
         w = (int)((bb >> 14) & 127u) + 1;
         h = (int)((bb >> 21) & 127u) + 1;
-        cw = (w + 3) >> 2;
+        cw = (w + SW - 1) / SW;
     };
     load_rec(r);
     int row = off / cw, chunk = off - row * cw;
@@ -811,8 +812,8 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, un
     const uint32_t fq_addr = (uint32_t)__cvta_generic_to_shared(ws.fq);
     for (int it = 0; it < per; ++it) {
         const bool act = it < n;
-        const int a = chunk << 2;
-        unsigned m4 = 0;
+        const int a = chunk * SW;
+        unsigned m4 = 0;   // coverage mask of the slot's SW pixels
         if (act) {
             int Ee[3], sx[3];
 #pragma unroll
@@ -821,26 +822,35 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, un
                 sx[e] = -(dy[e] << 8);
             }
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {   // covered iff no edge value (bias already subtracted) is negative
+            for (int k = 0; k < SW; ++k) {   // covered iff no edge value (bias already subtracted) is negative
                 m4 |= ((unsigned)~(Ee[0] | Ee[1] | Ee[2]) >> 31) << k;
                 Ee[0] += sx[0]; Ee[1] += sx[1]; Ee[2] += sx[2];
             }
-            m4 &= (1u << min(4, w - a)) - 1u;   // pixels beyond the bounding box
+            m4 &= (1u << min(SW, w - a)) - 1u;   // pixels beyond the bounding box
         }
-        // append the covered pixels: the lanes' counts (0..4) are prefix-summed with three ballots, one per bit
+        // append the covered pixels: the lanes' counts (0..SW) are prefix-summed with one ballot per bit; the queue
+        // is shaded first if this pass would not fit
         const int cnt = __popc(m4);
         const unsigned c0 = __ballot_sync(FULL, cnt & 1), c1 = __ballot_sync(FULL, cnt & 2), c2 = __ballot_sync(FULL, cnt & 4);
-        if (c0 | c1 | c2) {
+        const unsigned c3 = SW > 4 ? __ballot_sync(FULL, cnt & 8) : 0u;
+        if (c0 | c1 | c2 | c3) {
+            const int tot = __popc(c0) + 2 * __popc(c1) + 4 * __popc(c2) + 8 * __popc(c3);
+            if (qn + tot > FQ_CAP) {
+                __syncwarp();
+                if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
+                shade_queue_p(ws, qn, W, zfar, fb, first, env_recs, lane);
+                qn = 0;
+            }
             uint32_t en = (uint32_t)r | ((uint32_t)a << 5) | ((uint32_t)row << 12);
-            uint32_t addr = fq_addr + (uint32_t)(qn + __popc(c0 & lt) + 2 * __popc(c1 & lt) + 4 * __popc(c2 & lt)) * 4u;
+            uint32_t addr = fq_addr + (uint32_t)(qn + __popc(c0 & lt) + 2 * __popc(c1 & lt) + 4 * __popc(c2 & lt) + 8 * __popc(c3 & lt)) * 4u;
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
+            for (int k = 0; k < SW; ++k) {
                 const uint32_t bit = (m4 >> k) & 1u;
                 sts_if(addr, en, bit);
                 addr += bit << 2;
                 en += 32u;
             }
-            qn += __popc(c0) + 2 * __popc(c1) + 4 * __popc(c2);
+            qn += tot;
         }
         if (act) {
             if (++chunk == cw) {
@@ -851,12 +861,6 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, un
                     if (it + 1 < n) load_rec(r);
                 }
             }
-        }
-        if (qn > FQ_CAP - 128) {
-            __syncwarp();
-            if (STATS) n_frag += (lane == 0) ? (unsigned)qn : 0u;
-            shade_queue_p(ws, qn, W, zfar, fb, first, env_recs, lane);
-            qn = 0;
         }
     }
     __syncwarp();
@@ -983,6 +987,7 @@ template <int WARPS, int MINB, int PHASE, bool STATS>
 __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipeParams PP) {
     extern __shared__ __align__(16) unsigned char smem[];
     const GxParams &P = PP.g;
+    constexpr int SW = (PHASE == 2 || PHASE == 3) ? 4 : 8;            // pixels per slot: the occluder pass draws big triangles
     constexpr bool LOAD = PHASE == 2 || PHASE == 3;   // start from the previous pass's frame keys and hi-Z tiles
     constexpr bool DUMP = PHASE == 1 || PHASE == 3;   // leave frame keys, hi-Z tiles and record counts for the next pass
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -1054,9 +1059,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                 load_group(ws, env_recs, first, nrec, lane);
                 int Pex;
                 unsigned skip;
-                const int T = group_slots(ws, nrec, lane, hz, Pex, skip, st_culled);
+                const int T = group_slots<SW>(ws, nrec, lane, hz, Pex, skip, st_culled);
                 if (T <= PP.big_slots) {
-                    if (T) raster_slots<STATS>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
+                    if (T) raster_slots<STATS, SW>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
                 } else {
                     unsigned full = 0;
                     if (lane == 0) {
@@ -1066,7 +1071,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                         else full = 1;
                     }
                     if (__shfl_sync(0xFFFFFFFFu, full, 0))   // list full: draw the group here, whole
-                        raster_slots<STATS>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
+                        raster_slots<STATS, SW>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
                 }
             } else {   // wide records first: they reach the near plane and hide the most
                 const uint32_t t0 = b_w + g * 32u;
@@ -1095,9 +1100,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                 load_group(ws, env_recs, first, nrec, lane);
                 int Pex;
                 unsigned skip, dummy = 0;
-                const int T = group_slots(ws, nrec, lane, hz, Pex, skip, dummy);
+                const int T = group_slots<SW>(ws, nrec, lane, hz, Pex, skip, dummy);
                 const int S0 = (int)(c - en.y) * PP.chunk_slots;   // chunks of entries a full list dropped land beyond T
-                if (S0 < T) raster_slots<STATS>(ws, Pex, skip, S0, min(T, S0 + PP.chunk_slots), W, P.zfar, fb, first, env_recs, lane, st_frag);
+                if (S0 < T) raster_slots<STATS, SW>(ws, Pex, skip, S0, min(T, S0 + PP.chunk_slots), W, P.zfar, fb, first, env_recs, lane, st_frag);
             }
         }
         __syncthreads();
