@@ -110,6 +110,9 @@ struct GeomWarpSmem {
     unsigned char *lst;   // [256]
 };
 constexpr int GEOM_WARP_SMEM = GX_VCAP * 16 + 256;
+#ifndef GEOM_MINB
+#define GEOM_MINB 4
+#endif
 
 __host__ __device__ inline size_t geom_smem_bytes(int K, int warps) {
     size_t b = (size_t)warps * GEOM_WARP_SMEM + env_smem_bytes(K);
@@ -555,7 +558,7 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
 // is no CTA-level synchronisation at all.
 // ------------------------------------------------------------------------------------------------
 template <int WARPS, bool STATS>
-__global__ void __launch_bounds__(WARPS * 32, 1024 / (WARPS * 32)) geom_kernel(const PipeParams PP) {
+__global__ void __launch_bounds__(WARPS * 32, GEOM_MINB) geom_kernel(const PipeParams PP) {
     extern __shared__ __align__(16) unsigned char smem[];
     const GxParams &P = PP.g;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
