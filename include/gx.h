@@ -124,7 +124,7 @@ int gx_render_batch_host(GxScene *scene, const GxCamera *camera, int32_t N, int3
  *   "pool_slots"   narrow record slots per (environment, band); 0 = max(2048, 4*W*H/bands).
  *   "pool_bytes"   record pool budget, which bounds the environments per pass; 0 = 8 GB.
  *   "big_slots", "chunk_slots"  raster pass B: a group of more than big_slots 4-pixel slots is drawn in chunks
- *                            of chunk_slots (512, 256).
+ *                            of chunk_slots (512, 128).
  *   "stats"        0|1 (0)   count what gx_get_stat reports (slower kernels).
  *   "timing"       0|1 (0)   1 starts (and resets), 0 stops recording CUDA events around every kernel of
  *                            subsequent gx_render_batch calls on their stream.
