@@ -51,6 +51,9 @@ def parse_args():
     ap.add_argument("--envs", type=int, default=0, help="render only the first n environments (development)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--obs", action="store_true",
+                    help="time gx_render_batch_obs (packed [N,4,H,W] float16 observation, DESIGN.md N11) instead of "
+                         "gx_render_batch; device timing only")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="gx_set_option before rendering (development: e.g. --opt occlusion=0)")
     return ap.parse_args()
@@ -219,9 +222,15 @@ def run_gx(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
     stream = torch.cuda.current_stream().cuda_stream
 
+    obs = torch.empty((N, 4, H, W), dtype=torch.float16, device=dev) if args.obs else None
+
     def step():
-        gx.gx_render_batch(scene, cam, N, K, d_in[0], d_in[1], d_in[2] if K else None, d_in[3] if K else None,
-                           rgb, depth, None, stream)
+        if args.obs:
+            gx.gx_render_batch_obs(scene, cam, N, K, d_in[0], d_in[1], d_in[2] if K else None, d_in[3] if K else None,
+                                   obs, 0.0, 10.0, stream)
+        else:
+            gx.gx_render_batch(scene, cam, N, K, d_in[0], d_in[1], d_in[2] if K else None, d_in[3] if K else None,
+                               rgb, depth, None, stream)
 
     with ClockSampler(local) as clk:
         for _ in range(max(args.warmup, 0)):
@@ -253,7 +262,7 @@ def run_gx(args):
 
     # ---- e2e: host buffers in, host buffers out, through gx_render_batch_host -------------------------
     e2e = None
-    if not args.no_e2e:
+    if not args.no_e2e and not args.obs:
         p_in = [torch.from_numpy(a).pin_memory() for a in h_in]
         p_rgb = None if wl.depth_only else torch.empty((N, H, W, 3), dtype=torch.uint8).pin_memory()
         p_depth = torch.empty((N, H, W), dtype=torch.float32).pin_memory()
@@ -324,7 +333,8 @@ def run_gx(args):
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_name(args.config, wl), "envs_per_gpu": N, "width": W, "height": H,
                    "instances_per_env": K, "tris_per_env": float(wl.tris_per_env().mean()),
-                   "outputs": "depth f32" if wl.depth_only else "rgb u8 + depth f32",
+                   "outputs": "obs f16 [N,4,H,W] (gx_render_batch_obs)" if args.obs else
+                              ("depth f32" if wl.depth_only else "rgb u8 + depth f32"),
                    "l2": "256 MB buffer written between timed iterations (untimed)",
                    "arithmetic": "f32 vertex stage, i32/i64 fixed-point coverage, f32 depth/colour"},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches) * args.steps,

@@ -97,6 +97,22 @@ int gx_render_batch(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K
                     float *depth_out, uint32_t *id_out, void *cuda_stream);
 
 /*
+ * gx_render_batch_obs -- the same rasterisation, written as the packed observation tensor the policy reads
+ * ("directly consumed by PyTorch GPU-based batch DNN inference"; the visual encoder takes RGBD,
+ * PAPER.md:141, Table 3).  The paper is silent on the layout and normalisation; N11 fixes them:
+ *   obs_out [N,4,H,W] IEEE binary16, DEVICE pointer, 8-byte aligned: planes R, G, B = binary16(c / 255.0f) with c
+ *   the uint8 channel of gx_render_batch, plane D = binary16((clamp(depth, depth_min, depth_max) - depth_min) /
+ *   (depth_max - depth_min)) with depth the float32 depth of gx_render_batch (background 0.0f, so its D is 0);
+ *   all operations float32, conversions round-to-nearest-even.  The packing is fused into the last step of the
+ *   raster kernel: no RGB or depth image is written.
+ * Other arguments, stream semantics and errors as gx_render_batch; additionally INVALID_ARG if obs_out is NULL
+ * or depth_max <= depth_min.
+ */
+int gx_render_batch_obs(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K, const int32_t *env_scene,
+                        const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint16_t *obs_out,
+                        float depth_min, float depth_max, void *cuda_stream);
+
+/*
  * gx_render_batch_host -- the same operation with every array argument in HOST memory (pageable or
  * pinned): copies the inputs to the device, renders in sub-batches of 512 environments while the images of
  * the previous sub-batch are copied back on a second stream, and synchronises before returning.  This is the

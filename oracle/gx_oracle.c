@@ -382,3 +382,60 @@ int gx_oracle_vertex_stage(const OrCamera *cam, const float *cam_pose, const flo
     }
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------------
+ * N11 (NEXT-1 of SURVEY.md 8(f)): the packed observation the policy reads (PAPER.md:91,
+ * PAPER.md:141 "RGBD").  The paper is silent on layout and normalisation; the reading is
+ *   out[n][0..2][y][x] = binary16( (float)c / 255.0f ),  c = uint8 channel of the rendered image
+ *   out[n][3][y][x]    = binary16( (clamp(depth, dmin, dmax) - dmin) / (dmax - dmin) )
+ * all operations IEEE binary32, conversions round-to-nearest-even.
+ * or_half_rn: binary32 -> binary16 bits, written out by hand (non-negative finite inputs): normal, subnormal,
+ * ties to even, overflow to infinity.
+ * ------------------------------------------------------------------------------------------------ */
+static uint16_t or_half_rn(float f) {
+    uint32_t x;
+    memcpy(&x, &f, 4);
+    const uint32_t sign = (x >> 16) & 0x8000u;
+    const int exp = (int)((x >> 23) & 0xFFu);
+    uint32_t man = x & 0x7FFFFFu;
+    if (exp == 0xFF) return (uint16_t)(sign | 0x7C00u | (man ? 0x200u : 0u));
+    if (exp == 0) return (uint16_t)sign;                 /* binary32 subnormal: far below half of the smallest binary16 */
+    const int e = exp - 127 + 15;
+    if (e >= 31) return (uint16_t)(sign | 0x7C00u);
+    if (e <= 0) {                                        /* binary16 subnormal: value = man16 * 2^-24 */
+        if (e < -10) return (uint16_t)sign;
+        man |= 0x800000u;
+        const int shift = 14 - e;                        /* 14 .. 24 */
+        uint32_t h = man >> shift;
+        const uint32_t rem = man & ((1u << shift) - 1u), half = 1u << (shift - 1);
+        if (rem > half || (rem == half && (h & 1u))) ++h;
+        return (uint16_t)(sign | h);
+    }
+    uint32_t h = ((uint32_t)e << 10) | (man >> 13);
+    const uint32_t rem = man & 0x1FFFu;
+    if (rem > 0x1000u || (rem == 0x1000u && (h & 1u))) ++h;   /* a carry into the exponent is the right answer */
+    return (uint16_t)(sign | h);
+}
+
+int gx_oracle_pack_obs(const uint8_t *rgb /* [N,H,W,3] */, const float *depth /* [N,H,W] */, int32_t N, int32_t H,
+                       int32_t W, float dmin, float dmax, uint16_t *out /* [N,4,H,W] */) {
+    if (!rgb || !depth || !out || N <= 0 || H <= 0 || W <= 0 || !(dmax > dmin)) return -1;
+    const size_t npix = (size_t)H * (size_t)W;
+    const float range = dmax - dmin;
+    for (int32_t n = 0; n < N; ++n)
+        for (size_t p = 0; p < npix; ++p) {
+            for (int ch = 0; ch < 3; ++ch) {
+                const float v = (float)rgb[((size_t)n * npix + p) * 3 + ch] / 255.0f;
+                out[((size_t)n * 4 + ch) * npix + p] = or_half_rn(v);
+            }
+            float d = depth[(size_t)n * npix + p];
+            d = fminf(fmaxf(d, dmin), dmax);
+            out[((size_t)n * 4 + 3) * npix + p] = or_half_rn((d - dmin) / range);
+        }
+    return 0;
+}
+
+/* binary32 -> binary16 of an array: exposes or_half_rn to its pins */
+void gx_oracle_half_rn(const float *in, uint16_t *out, size_t n) {
+    for (size_t k = 0; k < n; ++k) out[k] = or_half_rn(in[k]);
+}

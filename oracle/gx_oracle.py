@@ -146,3 +146,27 @@ def vertex_stage(W, H, fx, fy, znear, zfar, cam_pose, xform, positions):
     if rc != 0:
         raise RuntimeError(f"gx_oracle_vertex_stage failed: {rc}")
     return o
+
+
+def pack_obs(rgb: np.ndarray, depth: np.ndarray, dmin: float, dmax: float) -> np.ndarray:
+    """N11: packed observation [N,4,H,W] as uint16 bit patterns of binary16 (view as np.float16 to read)."""
+    L = _load()
+    rgb = np.ascontiguousarray(rgb, np.uint8)
+    depth = np.ascontiguousarray(depth, np.float32)
+    N, H, W = depth.shape
+    out = np.empty((N, 4, H, W), np.uint16)
+    L.gx_oracle_pack_obs.restype = C.c_int
+    rc = L.gx_oracle_pack_obs(_p(rgb), _p(depth), C.c_int32(N), C.c_int32(H), C.c_int32(W), C.c_float(dmin), C.c_float(dmax), _p(out))
+    if rc != 0:
+        raise ValueError("gx_oracle_pack_obs: bad arguments")
+    return out
+
+
+def half_rn(x: np.ndarray) -> np.ndarray:
+    """binary32 -> binary16 bit patterns with the oracle's hand-written conversion."""
+    L = _load()
+    x = np.ascontiguousarray(x, np.float32)
+    out = np.empty(x.shape, np.uint16)
+    L.gx_oracle_half_rn.restype = None
+    L.gx_oracle_half_rn(_p(x), _p(out), C.c_size_t(x.size))
+    return out

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgx.so")
 GX_OK, GX_ERR_INVALID_ARG, GX_ERR_CUDA, GX_ERR_OOM, GX_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 GX_BACKGROUND_ID = 0xFFFFFFFF
 EXPORTS = ("gx_create_scene", "gx_render_batch", "gx_render_batch_host", "gx_set_option", "gx_get_stat",
-           "gx_destroy", "gx_last_error")
+           "gx_render_batch_obs", "gx_destroy", "gx_last_error")
 
 
 class GxMesh(C.Structure):
@@ -51,7 +51,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.gx_last_error.restype = C.c_char_p
         L.gx_destroy.restype = None
-        for n in EXPORTS[:5]:
+        for n in EXPORTS[:6]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -111,6 +111,14 @@ def gx_render_batch(scene, camera: GxCamera, N: int, K: int, env_scene, cam_pose
     _check(lib().gx_render_batch(scene, C.byref(camera), C.c_int32(N), C.c_int32(K), _dev(env_scene), _dev(cam_pose),
                                  _dev(inst_mesh), _dev(inst_xform), _dev(rgb_out), _dev(depth_out), _dev(id_out),
                                  C.c_void_p(cuda_stream)))
+
+
+def gx_render_batch_obs(scene, camera: GxCamera, N: int, K: int, env_scene, cam_pose, inst_mesh, inst_xform, obs_out,
+                        depth_min: float, depth_max: float, cuda_stream: int = 0) -> None:
+    """Packed observation [N,4,H,W] float16 (device tensor / address); enqueues on cuda_stream and returns."""
+    _check(lib().gx_render_batch_obs(scene, C.byref(camera), C.c_int32(N), C.c_int32(K), _dev(env_scene), _dev(cam_pose),
+                                     _dev(inst_mesh), _dev(inst_xform), _dev(obs_out), C.c_float(depth_min),
+                                     C.c_float(depth_max), C.c_void_p(cuda_stream)))
 
 
 def gx_render_batch_host(scene, camera: GxCamera, N: int, K: int, env_scene, cam_pose, inst_mesh, inst_xform,

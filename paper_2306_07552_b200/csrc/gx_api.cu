@@ -520,13 +520,16 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
     return fail(GX_ERR_INVALID_ARG, "unknown stat '%s'", name);
 }
 
-int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
-                    const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,
-                    float *depth_out, uint32_t *id_out, void *cuda_stream) {
+static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
+                       const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,
+                       float *depth_out, uint32_t *id_out, uint16_t *obs_out, float obs_dmin, float obs_dmax,
+                       void *cuda_stream) {
     if (!sc || !cam) return fail(GX_ERR_INVALID_ARG, "NULL scene or camera");
     if (N <= 0) return fail(GX_ERR_INVALID_ARG, "N must be positive, got %d", N);
     if (K < 0 || K > GX_MAX_INSTANCES) return fail(GX_ERR_INVALID_ARG, "K must be in [0, %d], got %d", GX_MAX_INSTANCES, K);
-    if (!env_scene || !cam_pose || !depth_out) return fail(GX_ERR_INVALID_ARG, "env_scene, cam_pose and depth_out are required");
+    if (!env_scene || !cam_pose || (!depth_out && !obs_out))
+        return fail(GX_ERR_INVALID_ARG, "env_scene, cam_pose and depth_out (or obs_out) are required");
+    if (obs_out && !(obs_dmax > obs_dmin)) return fail(GX_ERR_INVALID_ARG, "need depth_min < depth_max");
     if (K > 0 && (!inst_mesh || !inst_xform)) return fail(GX_ERR_INVALID_ARG, "inst_mesh and inst_xform are required when K > 0");
     if (cam->width <= 0 || cam->height <= 0 || cam->width % 16 || cam->height % 16)
         return fail(GX_ERR_INVALID_ARG, "width and height must be positive multiples of 16, got %dx%d", cam->width, cam->height);
@@ -550,6 +553,7 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     P.fx = cam->fx; P.fy = cam->fy; P.znear = cam->znear; P.zfar = cam->zfar;
     P.env_scene = env_scene; P.cam_pose = cam_pose; P.inst_mesh = inst_mesh; P.inst_xform = inst_xform;
     P.rgb = rgb_out; P.depth = depth_out; P.id = id_out;
+    P.obs = obs_out; P.obs_dmin = obs_dmin; P.obs_range = obs_dmax - obs_dmin;
     P.env_counter = sc->env_counter; P.stats = sc->stats;
     P.env_filter = nullptr;
     P.cull = sc->opt_cull;
@@ -623,7 +627,8 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
         PP.g.inst_mesh = inst_mesh ? inst_mesh + (size_t)e0 * K : nullptr;
         PP.g.inst_xform = inst_xform ? inst_xform + (size_t)e0 * K * 16 : nullptr;
         PP.g.rgb = rgb_out ? rgb_out + (size_t)e0 * npix * 3 : nullptr;
-        PP.g.depth = depth_out + (size_t)e0 * npix;
+        PP.g.depth = depth_out ? depth_out + (size_t)e0 * npix : nullptr;
+        PP.g.obs = obs_out ? obs_out + (size_t)e0 * npix * 4 : nullptr;
         PP.g.id = id_out ? id_out + (size_t)e0 * npix : nullptr;
         PP.recs = sc->pool.p;
         PP.counters = sc->pipe_scratch.p;
@@ -686,6 +691,22 @@ int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, cons
     return GX_OK;
 }
 
+
+int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
+                    const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,
+                    float *depth_out, uint32_t *id_out, void *cuda_stream) {
+    if (!depth_out) return fail(GX_ERR_INVALID_ARG, "depth_out is required");
+    return render_impl(sc, cam, N, K, env_scene, cam_pose, inst_mesh, inst_xform, rgb_out, depth_out, id_out, nullptr, 0.0f,
+                       1.0f, cuda_stream);
+}
+
+int gx_render_batch_obs(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
+                        const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint16_t *obs_out,
+                        float depth_min, float depth_max, void *cuda_stream) {
+    if (!obs_out) return fail(GX_ERR_INVALID_ARG, "obs_out is required");
+    return render_impl(sc, cam, N, K, env_scene, cam_pose, inst_mesh, inst_xform, nullptr, nullptr, nullptr, obs_out, depth_min,
+                       depth_max, cuda_stream);
+}
 
 int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
                          const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,

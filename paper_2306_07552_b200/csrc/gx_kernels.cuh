@@ -14,6 +14,7 @@
 // Arithmetic follows DESIGN.md section 3 (N1-N9) operation by operation; compiled with -fmad=false so that
 // only the fmaf() calls written here fuse.
 #pragma once
+#include <cuda_fp16.h>
 #include "gx_types.h"
 
 namespace gx {
@@ -58,6 +59,26 @@ __device__ __forceinline__ float clip_lerp(float t, float a_in, float a_out) { r
 // of 64-bit keys touches every bank exactly twice (two wavefronts, the minimum) and a row segment stays a
 // contiguous run.
 __device__ __forceinline__ int fb_index(int i, int j, int W) { return j * W + (i ^ ((j & 1) << 3)); }
+
+// N11: packed policy observation of 4 consecutive pixels of one row: planes R, G, B =
+// binary16(c / 255.0f), plane D = binary16((clamp(depth, dmin, dmin + range) - dmin) / range); all float32
+// operations, round-to-nearest-even conversions.  obs points at plane 0 of the environment, pix = y * W + x.
+__device__ __forceinline__ void store_obs4(uint16_t *obs, size_t npix, size_t pix, const uint32_t col[4], const float d[4],
+                                           float dmin, float range) {
+#pragma unroll
+    for (int ch = 0; ch < 4; ++ch) {
+        unsigned short h[4];
+#pragma unroll
+        for (int m = 0; m < 4; ++m) {
+            float v;
+            if (ch < 3) v = (float)((col[m] >> (8 * ch)) & 0xFFu) / 255.0f;
+            else v = (fminf(fmaxf(d[m], dmin), dmin + range) - dmin) / range;
+            h[m] = __half_as_ushort(__float2half_rn(v));
+        }
+        *reinterpret_cast<uint2 *>(obs + (size_t)ch * npix + pix) =
+            make_uint2((uint32_t)h[0] | ((uint32_t)h[1] << 16), (uint32_t)h[2] | ((uint32_t)h[3] << 16));
+    }
+}
 
 // st.shared.u32 [addr], v if pred != 0 (a predicated store, no branch)
 __device__ __forceinline__ void sts_if(uint32_t addr, uint32_t v, uint32_t pred) {
@@ -963,7 +984,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) render_kernel(const GxParams
         __syncthreads();
 
         // ---- K5a: resolve in place: key -> (depth bits, rgba) ------------------------------------
-        const bool want_rgb = P.rgb != nullptr;
+        const bool want_rgb = P.rgb != nullptr || P.obs != nullptr;
         for (int k = tid; k < npix; k += NT) {
             const int j = k / W, i = k - j * W;       // row-linear order: coalesced id stores
             const int a = fb_index(i, j, W);
@@ -989,8 +1010,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) render_kernel(const GxParams
             float4 d;
             d.x = __uint_as_float(v0.x); d.y = __uint_as_float(v0.z);
             d.z = __uint_as_float(v1.x); d.w = __uint_as_float(v1.z);
-            *reinterpret_cast<float4 *>(P.depth + (size_t)env * npix + pix) = d;
-            if (want_rgb) {
+            if (P.depth) *reinterpret_cast<float4 *>(P.depth + (size_t)env * npix + pix) = d;
+            if (P.obs) {
+                const uint32_t oc[4] = {v0.y, v0.w, v1.y, v1.w};
+                const float od[4] = {d.x, d.y, d.z, d.w};
+                store_obs4(P.obs + (size_t)env * 4 * npix, (size_t)npix, (size_t)pix, oc, od, P.obs_dmin, P.obs_range);
+            }
+            if (P.rgb) {
                 // 4 pixels = 12 bytes = 3 words per lane; 4 lanes hold 48 bytes = three 16-byte stores
                 const uint32_t c0 = v0.y, c1 = v0.w, c2 = v1.y, c3 = v1.w;
                 const uint32_t w0 = (c0 & 0xFFFFFFu) | (c1 << 24);

@@ -1017,7 +1017,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
         uint4 *f4 = reinterpret_cast<uint4 *>(fb);
         for (int k = tid; k < npb / 2; k += NT) f4[k] = ones;
     }
-    const bool want_rgb = P.rgb != nullptr;
+    const bool want_rgb = P.rgb != nullptr || P.obs != nullptr;
     const uint32_t cap_n = (uint32_t)PP.cap_n;
 
     for (;;) {
@@ -1162,9 +1162,10 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                         if (want_rgb || P.id) col[m] = resolve_rec(env_recs, cap_n, idx[m], i + m, j, y_lo, want_rgb, id[m]);
                     }
                 }
-                *reinterpret_cast<float4 *>(P.depth + out0 + pix) = d;
+                if (P.depth) *reinterpret_cast<float4 *>(P.depth + out0 + pix) = d;
+                if (P.obs) store_obs4(P.obs + (size_t)env * 4 * npix, (size_t)npix, (size_t)y_lo * W + pix, col, dp, P.obs_dmin, P.obs_range);
                 if (P.id) *reinterpret_cast<uint4 *>(P.id + out0 + pix) = make_uint4(id[0], id[1], id[2], id[3]);
-                if (want_rgb) {
+                if (P.rgb) {
                     // 4 pixels = 12 bytes = 3 words per lane; 4 lanes hold 48 bytes = three 16-byte stores
                     const uint32_t w0 = (col[0] & 0xFFFFFFu) | (col[1] << 24);
                     const uint32_t w1 = ((col[1] >> 8) & 0xFFFFu) | (col[2] << 16);

@@ -53,6 +53,8 @@ struct GxParams {
     uint8_t *rgb;
     float *depth;
     uint32_t *id;
+    uint16_t *obs;                // [N,4,H,W] binary16 packed observation (N11), or NULL
+    float obs_dmin, obs_range;    // depth channel = (clamp(depth, dmin, dmin + range) - dmin) / range
     // scratch
     unsigned int *env_counter;    // zeroed before the launch; persistent CTAs draw environments from it
     unsigned long long *stats;    // [GX_NSTAT], only touched by the STATS instantiation

@@ -555,3 +555,56 @@ def test_generators_are_subset_reproducible():
     assert np.array_equal(b.cam_pose, a.cam_pose[[4, 1]]) and np.array_equal(b.inst_xform, a.inst_xform[[4, 1]])
     assert a.static_meshes[0].nt == 50_000 and [m.nt for m in a.dyn_meshes] == [980, 400, 400, 400, 400, 400]
     assert a.K == 25 and np.all(a.tris_per_env() == 71_600)
+
+
+# ---------------------------------------------------------------------------------------------------
+# N11: packed observation (NEXT-1).  Pins: closed forms (dyadic values that binary16 holds exactly), the
+# hand-written binary32 -> binary16 conversion against numpy's (a library routine, round-to-nearest-even) on
+# every binary16 value, every midpoint between neighbours and random floats, and the layout.
+# ---------------------------------------------------------------------------------------------------
+def test_n11_half_conversion_matches_numpy_and_closed_forms(oracle_mod):
+    # exact cases
+    x = np.array([0.0, 1.0, 0.5, 0.25, 2.0 ** -14, 2.0 ** -24, 65504.0, 1.0 / 3.0, 2.0 ** -25, 1e-10, 70000.0], np.float32)
+    got = oracle_mod.half_rn(x)
+    assert got[0] == 0 and got[1] == 0x3C00 and got[2] == 0x3800 and got[3] == 0x3400
+    assert got[4] == 0x0400 and got[5] == 0x0001 and got[6] == 0x7BFF
+    assert got[7] == 0x3555                         # 1/3 -> 0.33325195 (nearest)
+    assert got[8] == 0x0000                         # exactly half of the smallest subnormal: tie -> even (0)
+    assert got[9] == 0 and got[10] == 0x7C00
+    # every finite non-negative binary16 value converts to itself; every midpoint goes to the even neighbour
+    h = np.arange(0, 0x7C00, dtype=np.uint16)
+    v = h.view(np.float16).astype(np.float32)
+    assert np.array_equal(oracle_mod.half_rn(v), h)
+    mid = ((v[:-1].astype(np.float64) + v[1:].astype(np.float64)) / 2).astype(np.float32)   # exact in binary32
+    exp = np.where(h[:-1] % 2 == 0, h[:-1], h[1:])
+    assert np.array_equal(oracle_mod.half_rn(mid), exp)
+    # random floats against numpy's conversion
+    rng = np.random.Generator(np.random.Philox(key=[5, 11]))
+    r = np.concatenate([rng.uniform(0, 1, 200000), rng.uniform(0, 2 ** -13, 50000), rng.uniform(0, 70000, 50000)]).astype(np.float32)
+    with np.errstate(over="ignore"):
+        assert np.array_equal(oracle_mod.half_rn(r), r.astype(np.float16).view(np.uint16))
+
+
+def test_n11_pack_obs_layout_and_values(oracle_mod):
+    rng = np.random.Generator(np.random.Philox(key=[5, 12]))
+    N, H, W = 2, 4, 6
+    rgb = rng.integers(0, 256, (N, H, W, 3)).astype(np.uint8)
+    depth = rng.uniform(0, 12, (N, H, W)).astype(np.float32)
+    depth[0, 0, 0] = 0.0            # background
+    depth[0, 0, 1] = 0.5            # = dmin
+    depth[0, 0, 2] = 10.5           # = dmax
+    depth[0, 0, 3] = 5.5            # midpoint
+    depth[0, 0, 4] = 11.0           # beyond dmax
+    rgb[0, 0, 0] = (0, 255, 51)     # 51/255 = 0.2
+    o = oracle_mod.pack_obs(rgb, depth, 0.5, 10.5)
+    assert o.shape == (N, 4, H, W)
+    f = o.view(np.float16).astype(np.float64)
+    assert f[0, 0, 0, 0] == 0.0 and f[0, 1, 0, 0] == 1.0 and abs(f[0, 2, 0, 0] - 0.2) < 2 ** -12
+    assert f[0, 3, 0, 0] == 0.0 and f[0, 3, 0, 1] == 0.0 and f[0, 3, 0, 2] == 1.0 and f[0, 3, 0, 3] == 0.5 and f[0, 3, 0, 4] == 1.0
+    # the whole tensor against numpy float32 arithmetic + numpy's binary16 conversion
+    ref = np.empty((N, 4, H, W), np.float16)
+    ref[:, :3] = (rgb.astype(np.float32) / np.float32(255.0)).transpose(0, 3, 1, 2).astype(np.float16)
+    ref[:, 3] = ((np.clip(depth, np.float32(0.5), np.float32(10.5)) - np.float32(0.5)) / np.float32(10.0)).astype(np.float16)
+    assert np.array_equal(o, ref.view(np.uint16))
+    with pytest.raises(ValueError):
+        oracle_mod.pack_obs(rgb, depth, 1.0, 1.0)
