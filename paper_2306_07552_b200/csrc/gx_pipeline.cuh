@@ -1004,7 +1004,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
     ws.fq = ws.rec + REC_WORDS * 32;
 
     __shared__ int s_env;
-    __shared__ unsigned s_next, s_next_b, s_big;
+    __shared__ unsigned s_next, s_next_b, s_big, s_classified;
     constexpr int BIG_CAP = 16 * WARPS;     // entries of the pass-B list
     __shared__ uint2 s_big_list[BIG_CAP];   // (group, first chunk) of the groups left to pass B
     __shared__ float s_hz[HZ_STRIDE];
@@ -1024,7 +1024,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
         if (tid == 0) {   // next task: (environment, band), heaviest first
             const unsigned k = atomicAdd(&PP.counters[1], 1u);
             s_env = k < (unsigned)(P.N * PP.bands) ? (int)PP.order[k] : -1;
-            s_next = 0; s_next_b = 0; s_big = 0;
+            s_next = 0; s_next_b = 0; s_big = 0; s_classified = 0;
         }
         __syncthreads();
         const int v = s_env;
@@ -1049,7 +1049,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
 
         // ---- K3 + K4, pass A: groups of 32 records, drawn dynamically by the warps.  A group of more than
         // big_slots slots is only registered: (list index, first chunk) come from one packed atomic, so the
-        // list is ordered by first chunk.
+        // list is ordered by first chunk.  Every group counts itself as classified as soon as that is decided.
         for (;;) {
             unsigned g = 0;
             if (lane == 0) g = atomicAdd(&s_next, 1u);
@@ -1063,28 +1063,36 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                 int Pex;
                 unsigned skip;
                 const int T = group_slots<SW>(ws, nrec, lane, hz, Pex, skip, st_culled);
-                if (T <= PP.big_slots) {
-                    if (T) raster_slots<STATS, SW>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
-                } else {
-                    unsigned full = 0;
-                    if (lane == 0) {
+                const bool big = T > PP.big_slots;
+                unsigned full = 0;
+                if (lane == 0) {
+                    if (big) {
                         const unsigned nch = (unsigned)(T + PP.chunk_slots - 1) / (unsigned)PP.chunk_slots;
                         const unsigned old = atomicAdd(&s_big, (1u << 20) | nch);
                         if ((old >> 20) < (unsigned)BIG_CAP) s_big_list[old >> 20] = make_uint2(g - g_w, old & 0xFFFFFu);
                         else full = 1;
                     }
-                    if (__shfl_sync(0xFFFFFFFFu, full, 0))   // list full: draw the group here, whole
-                        raster_slots<STATS, SW>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
+                    __threadfence_block();
+                    atomicAdd(&s_classified, 1u);   // this group's entry (if any) is in the list
                 }
+                // small group, or list full: drawn here, whole
+                if ((!big || __shfl_sync(0xFFFFFFFFu, full, 0)) && T)
+                    raster_slots<STATS, SW>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
             } else {   // wide records first: they reach the near plane and hide the most
+                if (lane == 0) atomicAdd(&s_classified, 1u);
                 const uint32_t t0 = b_w + g * 32u;
                 raster_wide<STATS>(env_recs, cap_n + 2u * t0, (int)min(32u, n_w - t0), W, H, y_lo, bh, P.zfar, fb, lane, st_frag);
             }
         }
-        __syncthreads();
+        // No barrier between the passes: a warp that finds no group left waits only until every group has been
+        // classified (each is, right after it is loaded), not until the small ones have been drawn.
+        if (lane == 0)
+            while (*reinterpret_cast<volatile unsigned *>(&s_classified) < g_n + g_w) __nanosleep(32);
+        __syncwarp();
+        __threadfence_block();
         // ---- pass B: the big groups, in chunks of chunk_slots slots drawn dynamically -----------------
         {
-            const unsigned packed = s_big;
+            const unsigned packed = *reinterpret_cast<volatile unsigned *>(&s_big);
             const unsigned n_big = min(packed >> 20, (unsigned)BIG_CAP), n_chunks = packed & 0xFFFFFu;
             for (;;) {
                 unsigned c = 0;
