@@ -284,10 +284,16 @@ template <int PHASE>
 int launch_pass(GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
     int rc;
     if ((rc = mark(sc, stream, 0)) != GX_OK) return rc;
-    constexpr int CW = 4, GW = 8, CP = PHASE >= 2 ? 2 : 1;
-    auto ck = stats ? gx::cull_kernel<CW, CP, true> : gx::cull_kernel<CW, CP, false>;
+    constexpr int GW = 8, CP = PHASE >= 2 ? 2 : 1;
     const size_t csmem = gx::env_smem_bytes(PP.g.K);
-    ck<<<PP.g.N, CW * 32, csmem, stream>>>(PP);
+    // one CTA per environment: 4 warps for small scenes, 16 where an environment has thousands of sub-clusters to test
+    if ((size_t)sc->max_static_batches + (size_t)PP.g.K * sc->max_dyn_batches > 512) {
+        auto ck = stats ? gx::cull_kernel<16, CP, true> : gx::cull_kernel<16, CP, false>;
+        ck<<<PP.g.N, 16 * 32, csmem, stream>>>(PP);
+    } else {
+        auto ck = stats ? gx::cull_kernel<4, CP, true> : gx::cull_kernel<4, CP, false>;
+        ck<<<PP.g.N, 4 * 32, csmem, stream>>>(PP);
+    }
     GX_CUDA(cudaGetLastError());
     if ((rc = mark(sc, stream, 1)) != GX_OK) return rc;
     auto gk = stats ? gx::geom_kernel<GW, true> : gx::geom_kernel<GW, false>;
@@ -602,7 +608,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     int rc;
     if ((rc = sc->pool.reserve((size_t)chunk * bands * (size_t)(cap_n + cap_w) * 4)) != GX_OK) return rc;
     // scratch words: counters[12] | cnt[2*tasks] | env_flag[chunk] (zeroed per chunk) | order[tasks] | cnt1[2*tasks] |
-    //                thr[chunk] | env_idb[chunk*(K+1)] | env_mv[chunk*(K+1)*12] | hiz[chunk*HZ_STRIDE] | items[2*...]
+    //                thr[chunk] | env_idb[chunk*(K+1)] | env_mv[chunk*(K+1)*12] | hiz[chunk*HZ_STRIDE] | items[4*...]
     // occluder scheme: 2 or 3 passes; automatic = 2 passes where they pay: frames of 8192 pixels or more (the hi-Z
     // tiles are 8x8 pixels) and enough environments that two rounds of kernels still fill the GPU
     const int n_pass = sc->opt_occlusion == 1 ? ((npix >= 8192 && N >= 512) ? 2 : 0) : sc->opt_occlusion;
@@ -612,8 +618,8 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     const size_t n_zero = 12 + 2 * tasks + (size_t)chunk;
     const size_t off_order = n_zero, off_cnt1 = off_order + tasks, off_thr = off_cnt1 + 2 * tasks;
     const size_t off_idb = off_thr + chunk, off_mv = off_idb + chunk * k1, off_hiz = off_mv + chunk * k1 * 12;
-    const size_t off_items = (off_hiz + (size_t)chunk * gx::HZ_STRIDE + 1) & ~(size_t)1;
-    if ((rc = sc->pipe_scratch.reserve(off_items + 2 * (size_t)chunk * std::max<size_t>(items_per_env, 1))) != GX_OK) return rc;
+    const size_t off_items = (off_hiz + (size_t)chunk * gx::HZ_STRIDE + 3) & ~(size_t)3;
+    if ((rc = sc->pipe_scratch.reserve(off_items + 4 * (size_t)chunk * std::max<size_t>(items_per_env, 1))) != GX_OK) return rc;
     if (two_phase && (rc = sc->frames.reserve((size_t)chunk * (size_t)npix)) != GX_OK) return rc;
     int launches = 0;
     GX_CUDA(cudaMemsetAsync(sc->d_maxrec, 0, 2 * sizeof(uint32_t), stream));
@@ -651,7 +657,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
         PP.maxrec = sc->d_maxrec;
         PP.env_idb = sc->pipe_scratch.p + off_idb;
         PP.env_mv = reinterpret_cast<float *>(sc->pipe_scratch.p + off_mv);
-        PP.items = reinterpret_cast<uint2 *>(sc->pipe_scratch.p + off_items);
+        PP.items = reinterpret_cast<uint4 *>(sc->pipe_scratch.p + off_items);
         GX_CUDA(cudaMemsetAsync(sc->pipe_scratch.p, 0, n_zero * sizeof(uint32_t), stream));
         PP.nphase = two_phase ? n_pass : 0;
         PP.occl_area = (float)sc->opt_occl_area;

@@ -42,7 +42,8 @@ struct PipeParams {
     uint32_t *cnt;           // [N][2]: narrow slots, wide slots appended
     uint32_t *env_flag;      // [N]: 1 = pool segment overflowed, render with the single-kernel path
     unsigned int *counters;  // [0] geometry item counter, [1] raster env counter, [2] items in the work list
-    uint2 *items;            // work list: (slot << 24 | batch, environment)
+    uint4 *items;            // work list: (slot << 24 | batch, environment, mask of the 32-triangle runs to draw,
+                             //            first | last << 16 vertex those runs reference)
     float *env_mv;           // [N][K+1][12] model-view per slot
     uint32_t *env_idb;       // [N][K+1] first triangle id per slot
     uint32_t *order;         // [N] raster order of the environments
@@ -220,12 +221,14 @@ __device__ __forceinline__ void emit_wide(const PipeParams &PP, int env, int lan
 }
 
 // ------------------------------------------------------------------------------------------------
-// geometry: K2 for one batch, by one warp
+// geometry: K2 for one batch, by one warp.  sub_mask: bit r set = pass r of the triangle loop (32 consecutive
+// triangles, one sub-cluster) is drawn; [v_lo, v_hi]: the vertices those passes reference (K1b, cull_kernel)
 // ------------------------------------------------------------------------------------------------
 template <bool STATS>
 __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj, uint32_t batch, const float *__restrict__ MV,
                                            uint32_t slot_id_base, const GeomWarpSmem &ws, int env, int lane,
-                                           bool &overflow, unsigned &n_in, unsigned &n_tri) {
+                                           unsigned sub_mask, int v_lo, int v_hi, bool &overflow, unsigned &n_in,
+                                           unsigned &n_tri) {
     const GxParams &P = PP.g;
     const unsigned FULL = 0xFFFFFFFFu;
     const GxBatchDev b = P.batches[batch];
@@ -237,33 +240,6 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
     const float4 *__restrict__ verts = P.verts + b.vert_off;
     const uchar4 *__restrict__ tris = P.tris + b.tri_off;
     const unsigned lt = (1u << lane) - 1u;
-    // K1b: sub-cluster culling.  Every pass of the triangle loop below takes 32 consecutive triangles; lane k
-    // tests the AABB of pass k against the frustum (and, in the second pass of the occluder scheme, against
-    // the hi-Z tiles).  A pass whose bit is clear is skipped; a batch with no bit set costs nothing more.
-    unsigned sub_mask = 0xFFFFFFFFu;
-    int v_lo = 0, v_hi = nv - 1;   // vertices the visible sub-clusters reference
-    if (PP.subcull || PP.phase) {
-        bool vis = false;
-        int lo = 0xFFFF, hi = -1;
-        if (lane * 32 < nt) {
-            const GxClusterDev sb = P.subs[(size_t)batch * GX_SUBS_PER_BATCH + lane];
-            const CamBox bx = cluster_box(sb, M);
-            vis = !PP.subcull || box_in_frustum(bx, P.fx, P.fy, P.znear, P.zfar);
-            if (vis && PP.phase) {
-                // occluder scheme: pass 1 draws the sub-clusters whose triangles are big on screen (cheap
-                // occluders) -- only the near ones of them when there are three passes --, the later passes
-                // draw the rest, minus what the hi-Z tiles of the passes before prove hidden
-                const int cls = sub_class(bx, P.fx, P.fy, P.W, P.H, P.znear, PP.occl_area, PP.thr[env], PP.nphase);
-                vis = cls == PP.phase - 1 &&
-                      (PP.phase == 1 || !box_occluded(bx, PP.hiz + (size_t)env * HZ_STRIDE, P.fx, P.fy, P.W, P.H, P.znear));
-            }
-            if (vis) { lo = (int)sb.batch_off; hi = (int)sb.nbatch; }
-        }
-        sub_mask = __ballot_sync(FULL, vis);
-        if (sub_mask == 0u) return;
-        v_lo = __reduce_min_sync(FULL, lo);
-        v_hi = __reduce_max_sync(FULL, hi);
-    }
     if (STATS) n_in += (lane == 0) ? 32u * (unsigned)__popc(sub_mask & ((nt + 31) / 32 < 32 ? (1u << ((nt + 31) / 32)) - 1u : 0xFFFFFFFFu)) : 0u;
 
     // K2a: vertex transform, projection, snap -> warp-private staging
@@ -504,11 +480,17 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
     }
 
     unsigned st_tested = 0, st_drawn = 0;
-    for (uint32_t g0 = warp * 32; g0 < n_cl; g0 += NT) {
-        const uint32_t g = g0 + lane;
-        uint32_t nb = 0, boff = 0, s = 0;
-        if (g < n_cl) {
-            s = slot_of(g);
+    constexpr int CCH = 256;                                   // clusters per round
+    constexpr int VB_CAP = CCH * GX_MAX_BATCH_PER_CLUSTER;     // batches of the visible clusters of a round
+    __shared__ uint32_t s_vb[VB_CAP], s_vm[VB_CAP], s_vlo[VB_CAP], s_vhi[VB_CAP];
+    __shared__ unsigned s_nvb;
+    for (uint32_t c0 = 0; c0 < n_cl; c0 += CCH) {
+        if (tid == 0) s_nvb = 0;
+        __syncthreads();
+        // step 1, one thread per cluster: frustum (and, in a later pass of the occluder scheme, hi-Z) test of the
+        // cluster AABB; the batches of the survivors are listed in shared memory
+        for (uint32_t g = c0 + tid; g < min(c0 + (uint32_t)CCH, n_cl); g += NT) {
+            const uint32_t s = slot_of(g);
             const GxClusterDev c = P.clusters[es.slot_cl[s] + (g - es.cl_base[s])];
             bool vis = true;
             if (P.cull) {
@@ -522,19 +504,52 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
                     vis = vis && !occ;
                 }
             } else if (STATS) { ++st_tested; ++st_drawn; }
-            if (vis) { nb = c.nbatch; boff = c.batch_off; }
+            if (vis) {
+                const uint32_t nb = min(c.nbatch, (uint32_t)GX_MAX_BATCH_PER_CLUSTER);
+                const uint32_t at = atomicAdd(&s_nvb, nb);
+                for (uint32_t k = 0; k < nb; ++k) {
+                    s_vb[at + k] = (s << 24) | (c.batch_off + k);
+                    s_vm[at + k] = 0u; s_vlo[at + k] = 0xFFFFu; s_vhi[at + k] = 0u;
+                }
+            }
         }
-        uint32_t inc = nb;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, inc, d);
-            if (lane >= d) inc += a;
+        __syncthreads();
+        const unsigned nvb = s_nvb;
+        // step 2 (K1b, sub-cluster culling), one thread per run of 32 triangles of a listed batch: its AABB is
+        // tested against the frustum and, in the occluder scheme, classified (pass 1: big-triangle sub-clusters,
+        // the cheap occluders; later passes: the rest) and tested against the hi-Z tiles
+        for (unsigned idx = tid; idx < nvb * GX_SUBS_PER_BATCH; idx += NT) {
+            const unsigned v = idx / GX_SUBS_PER_BATCH, r = idx % GX_SUBS_PER_BATCH;
+            const uint32_t batch = s_vb[v] & 0xFFFFFFu, s = s_vb[v] >> 24;
+            if ((int)r * 32 >= (int)(P.batches[batch].nv_nt >> 16)) continue;
+            const GxClusterDev sb = P.subs[(size_t)batch * GX_SUBS_PER_BATCH + r];
+            bool sv = true;
+            if (PP.subcull || PP.phase) {
+                const CamBox bx = cluster_box(sb, es.MV + s * 12);
+                sv = !PP.subcull || box_in_frustum(bx, P.fx, P.fy, P.znear, P.zfar);
+                if (sv && PP.phase) {
+                    const int cls = sub_class(bx, P.fx, P.fy, P.W, P.H, P.znear, PP.occl_area, thr, PP.nphase);
+                    sv = cls == PP.phase - 1 && (PHASE == 1 || !box_occluded(bx, s_hz, P.fx, P.fy, P.W, P.H, P.znear));
+                }
+            }
+            if (sv) {
+                atomicOr(&s_vm[v], 1u << r);
+                atomicMin(&s_vlo[v], sb.batch_off);   // (fields reused: first and last vertex the run references)
+                atomicMax(&s_vhi[v], sb.nbatch);
+            }
         }
-        const uint32_t tot = __shfl_sync(0xFFFFFFFFu, inc, 31);
-        uint32_t base = 0;
-        if (lane == 0 && tot) base = atomicAdd(&PP.counters[2], tot);
-        base = __shfl_sync(0xFFFFFFFFu, base, 0) + inc - nb;
-        for (uint32_t k = 0; k < nb; ++k) PP.items[base + k] = make_uint2((s << 24) | (boff + k), (uint32_t)env);
+        __syncthreads();
+        // step 3: one work item per batch that has a run left: (slot | batch, environment, mask of runs, vertex range)
+        for (unsigned v0 = warp * 32; v0 < nvb; v0 += NT) {
+            const unsigned v = v0 + lane;
+            const bool has = v < nvb && s_vm[v] != 0u;
+            const unsigned m = __ballot_sync(0xFFFFFFFFu, has);
+            uint32_t base = 0;
+            if (lane == 0 && m) base = atomicAdd(&PP.counters[2], (unsigned)__popc(m));
+            base = __shfl_sync(0xFFFFFFFFu, base, 0);
+            if (has) PP.items[base + __popc(m & ((1u << lane) - 1u))] = make_uint4(s_vb[v], (uint32_t)env, s_vm[v], s_vlo[v] | (s_vhi[v] << 16));
+        }
+        __syncthreads();
     }
     if (STATS) {
 #pragma unroll
@@ -582,13 +597,14 @@ __global__ void __launch_bounds__(WARPS * 32, GEOM_MINB) geom_kernel(const PipeP
     if (lane == 0) next = atomicAdd(&PP.counters[0], 1u);
     next = __shfl_sync(0xFFFFFFFFu, next, 0);
     while (next < n_items) {
-        const uint2 item = PP.items[next];
+        const uint4 item = PP.items[next];
         if (lane == 0) next = atomicAdd(&PP.counters[0], 1u);   // draw the following item while this one is processed
         const int env = (int)item.y;
         const uint32_t s = item.x >> 24;
         bool overflow = false;
         geom_batch<STATS>(PP, pj, item.x & 0xFFFFFFu, PP.env_mv + ((size_t)env * (size_t)(K + 1) + s) * 12,
-                          PP.env_idb[(size_t)env * (size_t)(K + 1) + s], ws, env, lane, overflow, st_in, st_tri);
+                          PP.env_idb[(size_t)env * (size_t)(K + 1) + s], ws, env, lane, item.z, (int)(item.w & 0xFFFFu),
+                          (int)(item.w >> 16), overflow, st_in, st_tri);
         if (overflow && lane == 0 && atomicExch(&PP.env_flag[env], 1u) == 0u)
             atomicAdd(&P.stats[GX_STAT_OVERFLOW_ENVS], 1ull);
         next = __shfl_sync(0xFFFFFFFFu, next, 0);
