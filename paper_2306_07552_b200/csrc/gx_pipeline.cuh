@@ -421,7 +421,7 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
         for (int k = tid; k <= K; k += NT) g_idb[k] = es.id_base[k];
     }
     const uint32_t n_cl = es.cl_base[K + 1];
-    const bool two_phase = P.cull && PP.nphase >= 2;
+    const bool need_thr = P.cull && PP.nphase >= 3;   // the depth threshold only splits the big sub-clusters of a 3-pass scheme
 
     auto slot_of = [&](uint32_t g) {
         int lo = 0, hi = K;
@@ -433,7 +433,7 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
     };
 
     float thr = 3.0e38f;
-    if (PHASE == 1 && two_phase) {
+    if (PHASE == 1 && need_thr) {
         for (int k = tid; k < 256; k += NT) s_hist[k] = 0;
         __syncthreads();
         const float inv_bin = 256.0f / P.zfar;
