@@ -308,7 +308,7 @@ def run_gx(args):
     traffic = None      # DRAM bytes per launch of all our kernels, from the committed ncu capture of this workload
     try:
         import csv
-        with open(os.path.join(ROOT, "profiles", "r1f_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", "r1g_traffic.csv")) as f:
             rows = [r for r in csv.DictReader(f) if int(r["workload_config"]) == args.config]
         if rows and not args.opt and not args.envs:
             traffic = float(sum(int(r["dram_bytes_per_launch"]) for r in rows))

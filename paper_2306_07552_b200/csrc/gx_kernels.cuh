@@ -443,7 +443,6 @@ template <bool STATS>
 __device__ __forceinline__ void raster_group(const WarpSmem &ws, int nrec, int W, float zfar, unsigned long long *fb,
                                              int lane, unsigned &n_frag) {
     const unsigned FULL = 0xFFFFFFFFu;
-    const unsigned lt = (1u << lane) - 1u;
     int ns = 0;
     if (lane < nrec) {
         const uint32_t bb = ws.rec[R_BB * 32 + lane];

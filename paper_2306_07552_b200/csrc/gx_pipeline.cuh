@@ -232,7 +232,7 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
     const GxParams &P = PP.g;
     const unsigned FULL = 0xFFFFFFFFu;
     const GxBatchDev b = P.batches[batch];
-    const int nv = (int)(b.nv_nt & 0xFFFFu), nt = (int)(b.nv_nt >> 16);
+    const int nt = (int)(b.nv_nt >> 16);
     float M[12];
 #pragma unroll
     for (int k = 0; k < 12; ++k) M[k] = MV[k];
