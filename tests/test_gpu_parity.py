@@ -229,7 +229,7 @@ def test_edge_cases(oracle_mod):
     g = render_gpu(wl)
     assert np.all(g["id"] == BG) and np.all(g["depth"] == 0) and np.all(g["rgb"] == 0)
     # huge quad over the whole frame, partially behind the camera after a pitch: near clip + all borders
-    for (W, H) in ((128, 128), (16, 16), (128, 64), (48, 112)):
+    for (W, H) in ((128, 128), (16, 16), (128, 64), (48, 112), (128, 96), (96, 128), (64, 128), (112, 80)):
         wl = _quad_workload(W, H, 1.0, 50.0)
         c, s = np.cos(1.2), np.sin(1.2)
         wl.cam_pose = np.array([[1, 0, 0, 0, 0, c, -s, 0.3, 0, s, c, 0, 0, 0, 0, 1]], np.float32)
@@ -331,3 +331,19 @@ def test_packed_observation(oracle_mod):
                                            obs, 1.0, 1.0, 0)
             finally:
                 gx.gx_destroy(sc)
+
+
+@pytest.mark.parametrize("W,H", [(128, 96), (96, 128), (64, 128), (80, 48)])
+def test_other_frame_shapes_room_scene(oracle_mod, W, H):
+    """Frame shapes other than the configs': the room scene of configs[1] rendered at W x H (fx = fy * H / W), which
+    exercises one, two and four raster CTAs per SM, bands that are and are not possible (H / 2 a multiple of 32 or
+    not), with and without the occluder scheme."""
+    wl = gen.make_config(1, n_envs=6)
+    wl.width, wl.height = W, H
+    wl.fy = 1.0
+    wl.fx = H / W
+    o = oracle_mod.render(wl)
+    for opts in ({}, {"occlusion": 2}, {"occlusion": 2, "bands": 1}, {"path": 1}):
+        g = render_gpu(wl, options=opts)
+        rep = compare(o, g)
+        assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, (opts, rep)
