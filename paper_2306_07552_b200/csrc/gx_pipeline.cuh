@@ -623,13 +623,15 @@ __global__ void __launch_bounds__(WARPS * 32, GEOM_MINB) geom_kernel(const PipeP
 // raster order: environments sorted by record count, heaviest first (one CTA, counting sort in 256 bins), so
 // that the persistent raster CTAs finish together.
 // ------------------------------------------------------------------------------------------------
+constexpr unsigned WIDE_COST = 1024;   // raster cost of a wide record in units of a narrow record: a whole warp walks
+                                       // its (often frame-sized) bounding box block by block
 __global__ void __launch_bounds__(1024) order_kernel(const PipeParams PP, const int since_phase1) {
     __shared__ unsigned hist[256];
     const int tid = threadIdx.x, N = PP.g.N * PP.bands;   // tasks: (environment, band)
     auto cost = [&](int e) {
         unsigned n = PP.cnt[2 * e], w = PP.cnt[2 * e + 1];
         if (since_phase1) { n -= PP.cnt1[2 * e]; w -= PP.cnt1[2 * e + 1]; }
-        return n + 4u * w;
+        return n + WIDE_COST / 2u * w;   // (w counts two slots per wide record)
     };
     if (tid < 256) hist[tid] = 0;
     __syncthreads();
@@ -671,6 +673,7 @@ struct RastWarpSmem {
     uint32_t *fq;    // [FQ_CAP] covered fragments: r | (x - i0) << 5 | (y - j0) << 12
 };
 constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4;
+constexpr uint32_t WIDE_GROUP = 2;   // wide records per draw: each is walked by a whole warp, one after the other
 
 __host__ __device__ inline size_t raster_smem_bytes(int W, int H, int warps) {
     return (size_t)W * H * 8 + (size_t)warps * RAST_WARP_SMEM;
@@ -1054,7 +1057,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
         const uint4 *env_recs = PP.recs + (size_t)v * (size_t)(PP.cap_n + PP.cap_w) * 4;
         const uint32_t n_n = PP.cnt[2 * v], n_w = PP.cnt[2 * v + 1] >> 1;
         const uint32_t b_n = LOAD ? PP.cnt1[2 * v] : 0u, b_w = LOAD ? PP.cnt1[2 * v + 1] >> 1 : 0u;
-        const uint32_t g_n = (n_n - b_n + 31u) >> 5, g_w = (n_w - b_w + 31u) >> 5;
+        const uint32_t g_n = (n_n - b_n + 31u) >> 5, g_w = (n_w - b_w + WIDE_GROUP - 1u) / WIDE_GROUP;
         if (LOAD) {   // the previous pass's frame and hi-Z tiles
             const uint4 *src = reinterpret_cast<const uint4 *>(PP.frames + (size_t)v * npb);
             uint4 *f4 = reinterpret_cast<uint4 *>(fb);
@@ -1096,8 +1099,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                     raster_slots<STATS, SW>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
             } else {   // wide records first: they reach the near plane and hide the most
                 if (lane == 0) atomicAdd(&s_classified, 1u);
-                const uint32_t t0 = b_w + g * 32u;
-                raster_wide<STATS>(env_recs, cap_n + 2u * t0, (int)min(32u, n_w - t0), W, H, y_lo, bh, P.zfar, fb, lane, st_frag);
+                const uint32_t t0 = b_w + g * WIDE_GROUP;
+                raster_wide<STATS>(env_recs, cap_n + 2u * t0, (int)min(WIDE_GROUP, n_w - t0), W, H, y_lo, bh, P.zfar, fb, lane, st_frag);
             }
         }
         // No barrier between the passes: a warp that finds no group left waits only until every group has been
