@@ -673,7 +673,7 @@ struct RastWarpSmem {
     uint32_t *fq;    // [FQ_CAP] covered fragments: r | (x - i0) << 5 | (y - j0) << 12
 };
 constexpr int RAST_WARP_SMEM = REC_WORDS * 32 * 4 + FQ_CAP * 4;
-constexpr uint32_t WIDE_GROUP = 2;   // wide records per draw: each is walked by a whole warp, one after the other
+constexpr int WIDE_ROWS = 16;   // a wide record is drawn strip by strip: one draw = one strip of this many rows, by one warp
 
 __host__ __device__ inline size_t raster_smem_bytes(int W, int H, int warps) {
     return (size_t)W * H * 8 + (size_t)warps * RAST_WARP_SMEM;
@@ -896,7 +896,7 @@ __device__ __forceinline__ void raster_slots(const RastWarpSmem &ws, int Pex, un
 // int64 edge functions of N6
 template <bool STATS>
 __device__ __forceinline__ void raster_wide(const uint4 *env_recs, uint32_t slot0, int ntri, int W, int H, int y_lo, int bh,
-                                            float zfar, unsigned long long *fb, int lane, unsigned &n_frag) {
+                                            int y_fb, float zfar, unsigned long long *fb, int lane, unsigned &n_frag) {
     const unsigned FULL = 0xFFFFFFFFu;
     Tri tri;
 #pragma unroll
@@ -921,7 +921,7 @@ __device__ __forceinline__ void raster_wide(const uint4 *env_recs, uint32_t slot
         bt.id2 = __shfl_sync(FULL, tri.id2, src);
         int bi0, bi1, bj0, bj1;
         pixel_bbox(bt.X, bt.Y, W, H, bi0, bi1, bj0, bj1);
-        bj0 = max(bj0, y_lo);                 // the band's rows only (frame rows y_lo .. y_lo + bh - 1)
+        bj0 = max(bj0, y_lo);                 // the strip's rows only (frame rows y_lo .. y_lo + bh - 1; the band starts at y_fb)
         bj1 = min(bj1, y_lo + bh - 1);
         Edges BE;
         edge_setup(bt, area2(bt), BE);   // orientation-normalised by the geometry kernel: area > 0
@@ -934,7 +934,7 @@ __device__ __forceinline__ void raster_wide(const uint4 *env_recs, uint32_t slot
                 if (!cover_depth(BE, bt.q, i, j, f, num, depth)) continue;
                 if (STATS) ++n_frag;
                 if (depth > zfar) continue;
-                key_min_rec(&fb[fb_index(i, j - y_lo, W)], __float_as_uint(depth), idx, bt.id2, env_recs);
+                key_min_rec(&fb[fb_index(i, j - y_fb, W)], __float_as_uint(depth), idx, bt.id2, env_recs);
             }
     }
     __syncwarp();
@@ -1057,7 +1057,8 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
         const uint4 *env_recs = PP.recs + (size_t)v * (size_t)(PP.cap_n + PP.cap_w) * 4;
         const uint32_t n_n = PP.cnt[2 * v], n_w = PP.cnt[2 * v + 1] >> 1;
         const uint32_t b_n = LOAD ? PP.cnt1[2 * v] : 0u, b_w = LOAD ? PP.cnt1[2 * v + 1] >> 1 : 0u;
-        const uint32_t g_n = (n_n - b_n + 31u) >> 5, g_w = (n_w - b_w + WIDE_GROUP - 1u) / WIDE_GROUP;
+        const uint32_t wu = (uint32_t)(bh + WIDE_ROWS - 1) / WIDE_ROWS;   // strips of WIDE_ROWS rows per band
+        const uint32_t g_n = (n_n - b_n + 31u) >> 5, g_w = (n_w - b_w) * wu;   // one draw = one strip of one wide record
         if (LOAD) {   // the previous pass's frame and hi-Z tiles
             const uint4 *src = reinterpret_cast<const uint4 *>(PP.frames + (size_t)v * npb);
             uint4 *f4 = reinterpret_cast<uint4 *>(fb);
@@ -1099,8 +1100,9 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
                     raster_slots<STATS, SW>(ws, Pex, skip, 0, T, W, P.zfar, fb, first, env_recs, lane, st_frag);
             } else {   // wide records first: they reach the near plane and hide the most
                 if (lane == 0) atomicAdd(&s_classified, 1u);
-                const uint32_t t0 = b_w + g * WIDE_GROUP;
-                raster_wide<STATS>(env_recs, cap_n + 2u * t0, (int)min(WIDE_GROUP, n_w - t0), W, H, y_lo, bh, P.zfar, fb, lane, st_frag);
+                const uint32_t t0 = b_w + g / wu, strip = g % wu;
+                const int ys = y_lo + (int)strip * WIDE_ROWS;
+                raster_wide<STATS>(env_recs, cap_n + 2u * t0, 1, W, H, ys, min(WIDE_ROWS, y_lo + bh - ys), y_lo, P.zfar, fb, lane, st_frag);
             }
         }
         // No barrier between the passes: a warp that finds no group left waits only until every group has been
