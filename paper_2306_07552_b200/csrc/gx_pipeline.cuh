@@ -1,19 +1,25 @@
-// gx_pipeline.cuh -- the two-kernel render path (sm_100a): geometry kernel -> triangle-record stream -> raster
-// kernel.  DESIGN.md section 5.
+// gx_pipeline.cuh -- the render path of gx_render_batch (sm_100a): cull kernel -> work list -> geometry kernel ->
+// triangle-record pool -> raster order -> raster kernel.  DESIGN.md section 5.
 //
-//   geom_kernel   K1 cull + K2 vertex transform / clip / snap / set-up.  No frame in shared memory, so four
-//                 8-warp CTAs fit an SM at 64 registers per thread; every triangle that survives the exact
-//                 pixel-centre bounding-box test leaves as one 64-byte record in the environment's segment
-//                 of the record pool (HBM/L2).
-//   raster_kernel K3 + K4 + K5.  One persistent CTA per SM owns one environment's whole frame of 64-bit
-//                 (depth, record index) keys in shared memory; warps draw groups of 32 records, cut their
-//                 bounding boxes into 4-pixel slots dealt evenly to the lanes, queue the covered pixels and
-//                 shade them densely; the winner's colour is resolved from its record and RGB / depth leave
-//                 as 16-byte stores.
+//   cull_kernel   K1: per environment, cluster AABBs against the frustum, then the 32-triangle sub-clusters of
+//                 the survivors (frustum; class and hi-Z tiles in the occluder scheme); one 16-byte work item
+//                 per batch that has a run of triangles left.
+//   geom_kernel   K2: vertex transform / clip / snap / set-up.  No frame in shared memory and no CTA-level
+//                 synchronisation, so four 8-warp CTAs fit an SM at 64 registers per thread; every triangle
+//                 that survives the exact pixel-centre bounding-box test leaves as one 64-byte record per band
+//                 it touches, in that (environment, band)'s segment of the record pool.
+//   order_kernel  the (environment, band) raster tasks sorted by estimated cost, heaviest first.
+//   raster_kernel K3 + K4 + K5.  Persistent CTAs, two per SM; a task's band of 64-bit (depth, record slot) keys
+//                 lives in shared memory; warps draw groups of 32 records, cut their bounding boxes into
+//                 8-pixel slots dealt evenly to the lanes, queue the covered pixels and shade them densely; the
+//                 winner's colour is resolved from its record and RGB / depth (or the packed observation)
+//                 leave as 16-byte stores.
+// With the occluder scheme the four kernels run twice: big-triangle sub-clusters first, the rest culled against
+// the hi-Z tiles the first raster pass leaves behind.
 //
-// An environment whose records do not fit its pool segment is flagged by the geometry kernel, skipped by the
+// An environment whose records do not fit a pool segment is flagged by the geometry kernel, skipped by the
 // raster kernel and rendered by the single-kernel path of gx_kernels.cuh (render_kernel), which needs no
-// pool.  Arithmetic follows DESIGN.md section 3 (N1-N9) operation by operation.
+// pool.  Arithmetic follows DESIGN.md section 3 (N1-N9, N11) operation by operation.
 #pragma once
 #include "gx_kernels.cuh"
 
