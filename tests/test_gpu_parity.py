@@ -347,3 +347,31 @@ def test_other_frame_shapes_room_scene(oracle_mod, W, H):
         g = render_gpu(wl, options=opts)
         rep = compare(o, g)
         assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, (opts, rep)
+
+
+def test_handle_reuse_varying_batches_and_host_subbatches(oracle_mod):
+    """One handle, calls of different sizes and options in a row (the record pool and its history-based sizing,
+    the scratch buffers and the frame keys are reused and regrown), and the host entry point with a batch that is
+    not a multiple of its 512-environment sub-batches: every call must match the oracle."""
+    import torch
+    from paper_2306_07552_b200 import binding as gx
+    wl = gen.make_config(2, n_envs=40)
+    o = oracle_mod.render(wl)
+    sc = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, 0)
+    try:
+        for sel, opts in ((np.arange(40), {}), (np.arange(7), {"occlusion": 2}), (np.arange(5, 38), {"occlusion": 3}),
+                          (np.arange(40), {"occlusion": 2, "pool_slots": 4096}), (np.arange(1), {"occlusion": 0, "pool_slots": 0}),
+                          (np.arange(40), {"occlusion": 1})):
+            sub = wl.subset(sel)
+            g = render_gpu(sub, scene=sc, options=opts)
+            rep = compare({k: v[sel] for k, v in o.items()}, g)
+            assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, (opts, rep)
+            torch.cuda.synchronize()
+    finally:
+        gx.gx_destroy(sc)
+    # host entry point: 1100 environments = sub-batches of 512, 512 and 76 (the 40 environments repeated)
+    rep_idx = np.arange(1100) % 40
+    big = wl.subset(rep_idx)
+    g = render_gpu(big, host_api=True)
+    rep = compare({k: v[rep_idx] for k, v in o.items()}, g)
+    assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, rep
