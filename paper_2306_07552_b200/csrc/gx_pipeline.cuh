@@ -1149,13 +1149,16 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) raster_kernel(const PipePara
             // ---- occluder pass: hi-Z tiles (max depth per 8x8 tile, +inf where background shows), the frame
             // keys and the record counts go to global memory; the frame is reset for the next environment
             const int tw = W >> 3, th = bh >> 3, ty0 = y_lo >> 3;   // the band's tile rows are ty0 .. ty0 + th - 1
-            for (int t = warp; t < tw * th; t += WARPS) {
-                const int ty = t / tw, tx = t - ty * tw;
-                const int j = ty * 8 + (lane >> 2), i = tx * 8 + (lane & 3) * 2;
-                const uint4 v = *reinterpret_cast<const uint4 *>(&fb[fb_index(i, j, W)]);   // two keys: depth bits in .y, .w
-                unsigned d = max(v.y, v.w);
-                d = __reduce_max_sync(0xFFFFFFFFu, d);
-                if (lane == 0) s_hz[ty * 16 + tx] = d == 0xFFFFFFFFu ? __int_as_float(0x7F800000) : __uint_as_float(d);
+            for (int u = warp; u < th * 2; u += WARPS) {   // a warp takes half a row of tiles; a lane, 2 of a tile's 64 keys
+                const int ty = u >> 1, j = ty * 8 + (lane >> 2);
+                const unsigned long long *row = fb + j * W;
+                const int sw = (j & 1) << 3, i0 = (lane & 3) * 2;
+                const int tx_lo = (u & 1) ? (tw >> 1) : 0, tx_hi = (u & 1) ? tw : (tw >> 1);
+                for (int tx = tx_lo; tx < tx_hi; ++tx) {
+                    const uint4 v = *reinterpret_cast<const uint4 *>(row + ((tx * 8 + i0) ^ sw));   // depth bits in .y, .w
+                    const unsigned d = __reduce_max_sync(0xFFFFFFFFu, max(v.y, v.w));
+                    if (lane == 0) s_hz[ty * 16 + tx] = d == 0xFFFFFFFFu ? __int_as_float(0x7F800000) : __uint_as_float(d);
+                }
             }
             __syncthreads();
             float *g_hz = PP.hiz + (size_t)env * HZ_STRIDE;
