@@ -59,18 +59,25 @@ def render_gpu(wl, want_id=True, want_rgb=None, cull=1, stats=False, scene=None,
 
 
 def compare(o, g, check_rgb=True):
-    """north_star tolerances: coverage and id bit-exact (ids may differ only where the two nearest surfaces
-    are within 1e-5 relative depth, <= 1e-4 of pixels); depth within 1e-5 relative; RGB within +-1 LSB.
-    Returns a dict of counts for reporting."""
+    """north_star tolerances, complete: coverage bit-exact; depth within 1e-5 relative at EVERY pixel; the id
+    equal, except that where the GPU picked another triangle its depth must still be within 1e-5 relative of the
+    oracle's winner (two surfaces inside the depth tolerance) and such pixels must stay <= 1e-4 of all pixels; RGB
+    within +-1 LSB everywhere except exactly those id-mismatch pixels (their colour belongs to the other
+    triangle).  Nothing else is exempt.  Returns a dict of counts for reporting."""
     oid, gid = o["id"], g["id"]
     cov_o, cov_g = oid != BG, gid != BG
     assert np.array_equal(cov_o, cov_g), f"coverage differs at {int((cov_o != cov_g).sum())} pixels"
+    od, gd = o["depth"], g["depth"]
+    od64, gd64 = od.astype(np.float64), gd.astype(np.float64)
+    assert np.all(np.isfinite(gd64)), "non-finite depth"
+    assert np.all(gd[~cov_o] == 0.0) and np.all(od[~cov_o] == 0.0), "background depth must be exactly 0"
+    rel = np.zeros_like(od64)
+    rel[cov_o] = np.abs(od64[cov_o] - gd64[cov_o]) / np.abs(od64[cov_o])
+    assert rel.max(initial=0.0) <= 1e-5, f"max relative depth error {rel.max():.3e}"
     id_diff = oid != gid
     n_id = int(id_diff.sum())
-    od, gd = o["depth"], g["depth"]
-    rel = np.abs(od.astype(np.float64) - gd.astype(np.float64)) / np.maximum(np.abs(od.astype(np.float64)), 1e-30)
-    rel[~cov_o] = np.abs(od[~cov_o] - gd[~cov_o])   # background: both must be exactly 0
-    assert rel.max() <= 1e-5, f"max relative depth error {rel.max():.3e}"
+    # an id mismatch is only legitimate between two surfaces within the depth tolerance of each other
+    assert np.all(rel[id_diff] <= 1e-5), "id mismatch at a pixel whose depths differ by more than the tolerance"
     assert n_id <= 1e-4 * oid.size, f"{n_id} id mismatches of {oid.size} pixels"
     n_rgb = 0
     max_rgb = 0
@@ -80,5 +87,6 @@ def compare(o, g, check_rgb=True):
         n_rgb = int((d > 0).sum())
         max_rgb = int(d[~id_diff].max()) if (~id_diff).any() else 0
         assert not bad.any(), f"{int(bad.sum())} pixels with RGB error > 1 LSB (max {int(d.max())})"
+        assert np.all(g["rgb"][~cov_o] == 0), "background RGB must be 0"
     return dict(id_mismatch=n_id, depth_bits_differ=int((od.view(np.uint32) != gd.view(np.uint32)).sum()),
-                max_rel_depth=float(rel.max()), rgb_differ=n_rgb, max_rgb=max_rgb)
+                max_rel_depth=float(rel.max(initial=0.0)), rgb_differ=n_rgb, max_rgb=max_rgb)

@@ -608,3 +608,115 @@ def test_n11_pack_obs_layout_and_values(oracle_mod):
     assert np.array_equal(o, ref.view(np.uint16))
     with pytest.raises(ValueError):
         oracle_mod.pack_obs(rgb, depth, 1.0, 1.0)
+
+
+# --------------------------------------------------------------------------------------------
+# equality boundaries of N3 / N5 / N7 / N9 (each is a separate clause of the definition)
+# --------------------------------------------------------------------------------------------
+
+def test_snap_is_round_half_even(oracle_mod):
+    """N5: X lands on exactly k + 0.5 sub-pixel units; ties go to the even integer (rintf), which
+    floor(x + 0.5) gets wrong for every even k.  Values derived by hand in tests/golden/vertex_closed_form.txt;
+    here the same construction over many k, expected values from exact rationals."""
+    from fractions import Fraction as F
+    W = H = 64
+    ks = list(range(4090, 4110)) + list(range(12280, 12300))
+    pos = np.array([[float(F(2 * k + 1 - 2 * 8192, 8192)), float(-F(2 * k + 1 - 2 * 8192, 8192)), -2.0] for k in ks], np.float32)
+    for k, p in zip(ks, pos):   # the inputs are exact in binary32
+        assert F(float(p[0])) == F(2 * k + 1 - 2 * 8192, 8192)
+    o = oracle_mod.vertex_stage(W, H, 1.0, 1.0, 0.1, 20.0, _pose("I"), None, pos)
+    want = np.array([k if k % 2 == 0 else k + 1 for k in ks])   # nearest even of k + 1/2
+    assert np.array_equal(o["Xi"], want)
+    assert np.array_equal(o["Yi"], want)
+    # the same rule on the raster path (N5 inside the triangle pipeline): a quad whose corners land on exactly
+    # 256 i + 128.5 snaps to 256 i + 128 (even), i.e. onto the pixel centres: by the closed form of
+    # test_quad_closed_form it then covers columns 5..19 and rows 7..12 (left/top inclusive, right/bottom
+    # exclusive).  Rounding half up would give 256 i + 129 and shift the cover to columns 6..20, rows 8..13.
+    W = H = 64
+    x0, x1, y0, y1 = 256 * 5 + 128.5, 256 * 20 + 128.5, 256 * 7 + 128.5, 256 * 13 + 128.5
+    XY = [[(x0, y0), (x1, y0), (x1, y1)], [(x0, y0), (x1, y1), (x0, y1)]]
+    soup = _soup_from_snapped(XY, W, H, w=2.0)
+    assert np.all(soup[:, :, :2].astype(np.float64) * 4096 % 0.5 == 0)   # inputs exact in binary32
+    r = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, soup, [0, 1], want_count=True)
+    want_cov = np.zeros((H, W), bool)
+    want_cov[7:13, 5:20] = True
+    assert np.array_equal(r["id"] != BG, want_cov) and r["count"].max() == 1
+
+
+def test_vertex_on_the_near_plane_is_inside(oracle_mod):
+    """N3: inside iff w >= znear, so a triangle with a vertex at exactly w == znear is not clipped.  Not being
+    clipped is observable without knowing any formula: with znear lowered by one ulp all three vertices are
+    strictly inside, and the two images must be bit-identical.  If the vertex counted as outside, N4 would
+    rebuild it as fma(1, x_out - x_in, x_in), which rounds (x_in is large and not dyadic), and the snapped
+    corner, and with it the depth bits, would move."""
+    W = H = 256
+    zn = np.float32(0.5)
+    v = np.zeros((1, 3, 6), np.float32)
+    v[0, 0] = (-1003.7, 0.3, 3.0, 250, 10, 30)     # far off-screen to the left: large, non-dyadic x
+    v[0, 1] = (0.9, -777.77, 2.0, 20, 240, 60)
+    v[0, 2] = (0.1, 0.2, zn, 90, 80, 255)          # exactly on the near plane
+    below = float(np.nextafter(zn, np.float32(0)))
+    for perm in ((0, 1, 2), (1, 2, 0), (2, 0, 1), (0, 2, 1)):
+        vv = np.ascontiguousarray(v[:, list(perm)])
+        a = oracle_mod.raster_soup(W, H, 1.0, 1.0, float(zn), 20.0, vv, [3], want_count=True)
+        b = oracle_mod.raster_soup(W, H, 1.0, 1.0, below, 20.0, vv, [3], want_count=True)
+        assert (a["id"] == 3).sum() > 1000
+        assert a["count"].max() == 1 and a["sub"].max() == 0
+        for k in ("id", "rgb", "count"):
+            assert np.array_equal(a[k], b[k]), k
+        assert np.array_equal(a["depth"].view(np.uint32), b["depth"].view(np.uint32))
+    # and the vertex stage says so directly
+    o = oracle_mod.vertex_stage(64, 64, 1.0, 1.0, 0.5, 20.0, _pose("I"), None,
+                                np.array([[0.0, 0.0, -0.5], [0.0, 0.0, np.nextafter(np.float32(-0.5), np.float32(0))]], np.float32))
+    assert list(o["inside"]) == [1, 0]
+
+
+def test_far_plane_is_inclusive(oracle_mod):
+    """N7: a fragment is dropped iff depth > zfar.  A fronto-parallel quad of <= 16x16 px at a power-of-two depth d
+    has depth exactly d at every covered pixel (test_depth_exact_for_power_of_two), so with zfar == d it is kept
+    and with zfar one ulp below d it is dropped, entirely."""
+    W = H = 32
+    d = 16.0
+    x0, y0, x1, y1 = 256 * 5 + 7, 256 * 9 + 200, 256 * 18 + 130, 256 * 21 + 1
+    XY = [[(x0, y0), (x1, y0), (x1, y1)], [(x0, y0), (x1, y1), (x0, y1)]]
+    soup = _soup_from_snapped(XY, W, H, w=d)
+    keep = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, d, soup, [0, 1])
+    cov = keep["id"] != BG
+    # pixel centres with x0 <= 256i+128 < x1 (i = 5..18) and y0 <= 256j+128 < y1 (j = 10..20)
+    assert cov.sum() == 14 * 11 and cov[10:21, 5:19].all()
+    assert np.all(keep["depth"][cov] == np.float32(d))
+    drop = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, float(np.nextafter(np.float32(d), np.float32(0))), soup, [0, 1])
+    assert np.all(drop["id"] == BG) and np.all(drop["depth"] == 0.0) and np.all(drop["rgb"] == 0)
+
+
+def test_clip_pieces_tie_goes_to_sub_zero(oracle_mod):
+    """N9, third key: the two pieces of a near-clipped triangle keep the parent id; where both cover a pixel at
+    exactly equal depth, sub 0 wins.  Construction: vertex a sits exactly on a pixel centre at w = 1 (q = 1) and
+    just inside a near plane at 1 - 2^-k, so the second piece (a, P(b,c), P(a,c)) is a sliver whose apex a can
+    land on either side of its base after snapping; when it folds over the first piece, the pixel at a is covered
+    by both (count == 2).  At that pixel the edge functions of both pieces are (A, 0, 0), so depth = A / (A * 1)
+    = 1 exactly in both: an exact tie.  The search is seeded and bounded; it uses only the coverage count."""
+    W = H = 16
+    hw = 128.0 * W
+    rng = np.random.default_rng(11)
+    found = 0
+    for _ in range(40000):
+        i, j = rng.integers(2, 14, 2)
+        zn = np.float32(1.0 - 2.0 ** -int(rng.integers(8, 22)))
+        a = [(256 * i + 128 - hw) / hw, -(256 * j + 128 - hw) / hw, 1.0]
+        wb, wc = np.float32(rng.uniform(1.0, 3.0)), np.float32(rng.uniform(0.2, 0.999))
+        b = [rng.uniform(-1, 1) * wb, rng.uniform(-1, 1) * wb, wb]
+        c = [rng.uniform(-1, 1) * wc, rng.uniform(-1, 1) * wc, wc]
+        v = np.zeros((1, 3, 6), np.float32)
+        for s, p in zip(rng.permutation(3), (a, b, c)):
+            v[0, s, :3] = p
+        v[0, :, 3:] = rng.integers(0, 256, (3, 3))
+        o = oracle_mod.raster_soup(W, H, 1.0, 1.0, float(zn), 20.0, v, [5], want_count=True)
+        if o["count"][j, i] == 2:
+            found += 1
+            assert o["id"][j, i] == 5
+            assert o["depth"][j, i] == np.float32(1.0)     # the exact tie
+            assert o["sub"][j, i] == 0
+            if found >= 6:
+                break
+    assert found >= 6, found
