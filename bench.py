@@ -246,7 +246,7 @@ def run_gx(args):
             b.record()
         barrier()
         ms = [a.elapsed_time(b) for a, b in ev]
-        kernel_ns = {k: gx.gx_get_stat(scene, "ns_" + k) for k in ("cull", "geom", "order", "raster", "fallback")}
+        kernel_ns = {k: gx.gx_get_stat(scene, "ns_" + k) for k in ("cull", "geom", "bin", "raster", "tail")}
         timed_calls = gx.gx_get_stat(scene, "timed_calls")
         gx.gx_set_option(scene, "timing", 0)
         # keep the GPU under load a little longer so that nvidia-smi (200 ms period) sees the render clocks
@@ -317,7 +317,7 @@ def run_gx(args):
     dom = max(kernels_ms, key=kernels_ms.get) if timed_calls else "raster"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "peak_source": peak_src,
-                "kernel": "gx pipeline: cull_kernel + geom_kernel + order_kernel + raster_kernel (+ overflow pass)",
+                "kernel": "gx pipeline: cull_kernel + geom_kernel + bin_kernel + raster_kernel + tail_kernel",
                 "kernel_ms": kernel_ms, "kernels_ms": kernels_ms,
                 "dominant_kernel": {"name": "gx::" + dom + "_kernel", "ms": kernels_ms.get(dom),
                                     "share_of_kernel_time": (kernels_ms.get(dom, 0.0) / kernel_ms) if kernel_ms else None},

@@ -34,6 +34,7 @@ extern "C" {
 
 #define GX_BACKGROUND_ID 0xFFFFFFFFu
 #define GX_MAX_INSTANCES 254 /* K, instance slots per environment */
+#define GX_MAX_FRAME 256     /* width and height limit: the box fields of a triangle record are 8 bits */
 
 typedef struct GxScene GxScene; /* opaque; owns the device copies of all meshes and all scratch memory */
 

@@ -77,48 +77,45 @@ struct GxScene {
     GxClusterDev *subs = nullptr;
     GxClusterDev *clusters = nullptr;
     GxMeshDev *meshes = nullptr;
-    std::vector<uint32_t> mesh_nt;      // host copy, for id-range validation
     uint32_t max_dyn_nt = 0, max_static_nt = 0;
-    uint32_t max_nbatch = 1;            // largest number of batches in any cluster
     uint32_t max_static_batches = 0, max_dyn_batches = 0;   // largest number of batches in any static / dynamic mesh
     int max_smem_optin = 0;
-    unsigned int *env_counter = nullptr;
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
-    int opt_cull = 1;
-    int opt_stats = 0;
-    int last_chunk_n = 0;               // environments in the last chunk of the last two-kernel call
-    int opt_path = 0;                   // 0 = two-kernel path (geometry -> records -> raster), 1 = single kernel
-    int64_t opt_pool_slots = 0;         // narrow record slots per environment; 0 = max(4096, 4*W*H)
-    int64_t opt_pool_bytes = 0;         // record pool budget; 0 = 8 GB
-    int opt_big_slots = 512, opt_chunk_slots = 128;   // raster pass B (gx_pipeline.cuh)
-    DevBuf<uint4> pool;                 // triangle records of one chunk of environments
-    DevBuf<unsigned long long> frames;  // frame keys between the two raster phases
-    // kernel timing (option "timing"): CUDA events recorded on the caller's stream around every kernel class
+    // options (gx_set_option)
+    int opt_cull = 1, opt_subcull = 1, opt_stats = 0, opt_hiz = 1, opt_big_px = gx::TILE;
+    int64_t opt_pool_bytes = 0;         // arena budget; 0 = 4 GB
+    int64_t opt_arena_slots = 0;        // force the arena size in record slots (tests: several waves); 0 = automatic
+    // scratch owned by the handle: grows on demand, never inside a steady-state call
+    DevBuf<uint4> arena_recs;
+    DevBuf<uint2> arena_bbs;
+    DevBuf<uint32_t> arena_refs;
+    size_t arena_slots = 0;
+    DevBuf<uint32_t> scratch;           // ctl | per-environment tables | tile offsets | task lists | items
+    // arena sizing from history: the per-environment mean and the maximum of U of earlier calls
+    uint32_t *h_ctl = nullptr;          // pinned host copy of the control words of the last call
+    cudaEvent_t ev_ctl = nullptr;
+    bool ctl_pending = false;
+    int ctl_N = 0;
+    double hist_u_per_env = 0.0;
+    // kernel timing (option "timing"): CUDA events recorded on the caller's stream around every kernel
     int opt_timing = 0;
     std::vector<cudaEvent_t> t_ev;      // recorded marks, in order
-    std::vector<int> t_kind;            // what ran before the mark: 0 = start of a pass, 1 cull, 2 geom, 3 order, 4 raster, 5 fallback
+    std::vector<int> t_kind;            // what ran before the mark: 0 = start of a call, 1 cull, 2 geom, 3 bin, 4 raster, 5 tail
     size_t t_used = 0;
     int t_calls = 0;
-    int opt_subcull = 1;                // geometry kernel: frustum (and hi-Z) test per 32-triangle sub-cluster
-    int opt_bands = 0;                  // raster bands per frame; 0 = automatic
-    int opt_occlusion = 1;              // occluder scheme: 0 off, 2 or 3 passes, 1 = automatic
-    int opt_occl_area = 64;              // occluder scheme: sub-clusters with >= this many screen-box pixels per triangle go first
-    int opt_occluder_pct = 50;          // share of the visible clusters (nearest first) drawn in the occluder phase
-    // pool sizing from history: the largest record counts any raster task of earlier calls produced
-    uint32_t *d_maxrec = nullptr, *h_maxrec = nullptr;   // device [2]; pinned host [2]
-    cudaEvent_t ev_maxrec = nullptr;
-    bool maxrec_pending = false;
-    uint32_t hist_n = 0, hist_w = 0;
-    DevBuf<uint32_t> pipe_scratch;      // counters[4] | cnt[2*chunk] | env_flag[chunk]
+    bool t_full = false;
     int last_launches = 0;
     cudaStream_t last_stream = nullptr;
+    // launch configurations, resolved once per kernel instantiation (occupancy queries are not free)
+    struct Plan { const void *fn; size_t smem; int per_sm; };
+    std::vector<Plan> plans;
     // staging for gx_render_batch_host
     DevBuf<int32_t> h_env_scene, h_inst_mesh;
     DevBuf<float> h_cam_pose, h_inst_xform, h_depth;
     DevBuf<uint8_t> h_rgb;
     DevBuf<uint32_t> h_id;
     cudaStream_t host_stream = nullptr, copy_stream = nullptr;
-    cudaEvent_t ev_sub = nullptr;
+    std::vector<cudaEvent_t> ev_sub;
 };
 
 namespace {
@@ -218,54 +215,23 @@ int upload(T *&dst, const std::vector<T> &src) {
     return GX_OK;
 }
 
-struct LaunchPlan {
-    int warps, minb;
-    size_t smem;
-    int grid;
-};
-
-template <int WARPS, int MINB>
-int launch(const GxScene *sc, const GxParams &P, size_t smem, cudaStream_t stream, bool stats) {
-    auto kern = stats ? gx::render_kernel<WARPS, MINB, true> : gx::render_kernel<WARPS, MINB, false>;
-    GX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int per_sm = 0;
-    GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem));
-    if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "kernel does not fit: %zu bytes of shared memory", smem);
-    const int grid = std::min(P.N, sc->num_sms * per_sm);
-    kern<<<grid, WARPS * 32, smem, stream>>>(P);
-    GX_CUDA(cudaGetLastError());
-    return GX_OK;
-}
-
-
-// single-kernel path (gx_kernels.cuh): small frames (<= 32 KB of keys) use 8-warp CTAs, several per SM; big
-// frames one CTA per SM with as many warps as the rest of the 227 KB of shared memory holds staging for.
-int launch_single(const GxScene *sc, const GxParams &P, cudaStream_t stream, bool st) {
-    const int K = P.K;
-    const bool small_frame = (size_t)P.W * P.H * 8 <= 32768;
-    const size_t cap = (size_t)sc->max_smem_optin - 256;   // static shared memory of the kernel
-    if (small_frame) return launch<8, 2>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, st);
-    if (gx::kernel_smem_bytes(P.W, P.H, K, 16) <= cap) return launch<16, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 16), stream, st);
-    if (gx::kernel_smem_bytes(P.W, P.H, K, 12) <= cap) return launch<12, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 12), stream, st);
-    return launch<8, 1>(sc, P, gx::kernel_smem_bytes(P.W, P.H, K, 8), stream, st);
-}
-
-template <int WARPS, int MINB, int PHASE>
-int launch_raster(const GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
-    auto kern = stats ? gx::raster_kernel<WARPS, MINB, PHASE, true> : gx::raster_kernel<WARPS, MINB, PHASE, false>;
-    const size_t smem = gx::raster_smem_bytes(PP.g.W, PP.bh, WARPS);
-    GX_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    int per_sm = 0;
-    GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, WARPS * 32, smem));
-    if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "raster kernel does not fit: %zu bytes of shared memory", smem);
-    kern<<<std::min(PP.g.N * PP.bands, sc->num_sms * per_sm), WARPS * 32, smem, stream>>>(PP);
-    GX_CUDA(cudaGetLastError());
+// blocks per SM of a kernel at a block size and dynamic shared memory size; sets the opt-in attribute once
+int plan_of(GxScene *sc, const void *fn, int threads, size_t smem, int *per_sm) {
+    for (const GxScene::Plan &p : sc->plans)
+        if (p.fn == fn && p.smem == smem) { *per_sm = p.per_sm; return GX_OK; }
+    GX_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int n = 0;
+    GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, threads, smem));
+    if (n < 1) return fail(GX_ERR_UNSUPPORTED, "kernel does not fit: %zu bytes of shared memory", smem);
+    sc->plans.push_back({fn, smem, n});
+    *per_sm = n;
     return GX_OK;
 }
 
 // timing mark: an event on the stream; the time since the previous mark belongs to kernel class `kind`
 int mark(GxScene *sc, cudaStream_t stream, int kind) {
-    if (!sc->opt_timing || sc->t_used >= 8192) return GX_OK;
+    if (!sc->opt_timing || sc->t_full) return GX_OK;
+    if (sc->t_used >= 8192) { sc->t_full = true; return GX_OK; }
     if (sc->t_used == sc->t_ev.size()) {
         cudaEvent_t e;
         GX_CUDA(cudaEventCreate(&e));
@@ -276,45 +242,6 @@ int mark(GxScene *sc, cudaStream_t stream, int kind) {
     GX_CUDA(cudaEventRecord(sc->t_ev[sc->t_used], stream));
     ++sc->t_used;
     return GX_OK;
-}
-
-// one pass of the pipeline (gx_pipeline.cuh): cull kernel, geometry kernel, raster order, raster kernel.
-// PHASE 0 = everything in one pass; 1 = occluder phase; 2 = the rest, culled against the occluder phase's hi-Z.
-template <int PHASE>
-int launch_pass(GxScene *sc, const gx::PipeParams &PP, cudaStream_t stream, bool stats) {
-    int rc;
-    if ((rc = mark(sc, stream, 0)) != GX_OK) return rc;
-    constexpr int GW = 8, CP = PHASE >= 2 ? 2 : 1;
-    const size_t csmem = gx::env_smem_bytes(PP.g.K);
-    // one CTA per environment: 4 warps for small scenes, 16 where an environment has thousands of sub-clusters to test
-    if ((size_t)sc->max_static_batches + (size_t)PP.g.K * sc->max_dyn_batches > 512) {
-        auto ck = stats ? gx::cull_kernel<16, CP, true> : gx::cull_kernel<16, CP, false>;
-        ck<<<PP.g.N, 16 * 32, csmem, stream>>>(PP);
-    } else {
-        auto ck = stats ? gx::cull_kernel<4, CP, true> : gx::cull_kernel<4, CP, false>;
-        ck<<<PP.g.N, 4 * 32, csmem, stream>>>(PP);
-    }
-    GX_CUDA(cudaGetLastError());
-    if ((rc = mark(sc, stream, 1)) != GX_OK) return rc;
-    auto gk = stats ? gx::geom_kernel<GW, true> : gx::geom_kernel<GW, false>;
-    const size_t gsmem = (size_t)GW * gx::GEOM_WARP_SMEM;
-    GX_CUDA(cudaFuncSetAttribute(gk, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gsmem));
-    int per_sm = 0;
-    GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, gk, GW * 32, gsmem));
-    if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "geometry kernel does not fit: %zu bytes of shared memory", gsmem);
-    gk<<<sc->num_sms * per_sm, GW * 32, gsmem, stream>>>(PP);
-    GX_CUDA(cudaGetLastError());
-    if ((rc = mark(sc, stream, 2)) != GX_OK) return rc;
-    gx::order_kernel<<<1, 1024, 0, stream>>>(PP, PHASE >= 2 ? 1 : 0);
-    GX_CUDA(cudaGetLastError());
-    if ((rc = mark(sc, stream, 3)) != GX_OK) return rc;
-    // one band of 64-bit keys per CTA: the smaller the band, the more CTAs share an SM (32 warps per SM in all cases)
-    const size_t band_bytes = (size_t)PP.g.W * PP.bh * 8;
-    if (band_bytes <= 32768) rc = launch_raster<8, 4, PHASE>(sc, PP, stream, stats);
-    else if (band_bytes <= 65536) rc = launch_raster<16, 2, PHASE>(sc, PP, stream, stats);
-    else rc = launch_raster<32, 1, PHASE>(sc, PP, stream, stats);
-    if (rc != GX_OK) return rc;
-    return mark(sc, stream, 4);
 }
 
 }  // namespace
@@ -350,7 +277,6 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
             uint32_t &mb = i < n_static ? sc->max_static_batches : sc->max_dyn_batches;
             mb = std::max<uint32_t>(mb, (uint32_t)(batches.size() - b0));
             meshes.push_back(md);
-            sc->mesh_nt.push_back(m.nt);
             if (i < n_static) sc->max_static_nt = std::max(sc->max_static_nt, m.nt);
             else sc->max_dyn_nt = std::max(sc->max_dyn_nt, m.nt);
         }
@@ -374,7 +300,6 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
     if (rc == GX_OK) {
         sc->num_sms = prop.multiProcessorCount;
         sc->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
-        for (const GxClusterDev &c : clusters) sc->max_nbatch = std::max(sc->max_nbatch, c.nbatch);
     }
     if (rc == GX_OK) rc = upload(sc->verts, verts);
     if (rc == GX_OK) rc = upload(sc->tris, tris);
@@ -384,9 +309,11 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
     if (rc == GX_OK) rc = upload(sc->meshes, meshes);
     if (rc == GX_OK) {
         auto alloc = [&]() -> int {
-            GX_CUDA(cudaMalloc(&sc->env_counter, sizeof(unsigned int)));
             GX_CUDA(cudaMalloc(&sc->stats, GX_NSTAT * sizeof(unsigned long long)));
             GX_CUDA(cudaMemset(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long)));
+            GX_CUDA(cudaMallocHost(&sc->h_ctl, gx::C_NCTL * sizeof(uint32_t)));
+            memset(sc->h_ctl, 0, gx::C_NCTL * sizeof(uint32_t));
+            GX_CUDA(cudaEventCreateWithFlags(&sc->ev_ctl, cudaEventDisableTiming));
             return GX_OK;
         };
         rc = alloc();
@@ -410,59 +337,33 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->subs);
     cudaFree(sc->clusters);
     cudaFree(sc->meshes);
-    cudaFree(sc->env_counter);
     cudaFree(sc->stats);
-    sc->pool.release(); sc->pipe_scratch.release(); sc->frames.release();
+    sc->arena_recs.release(); sc->arena_bbs.release(); sc->arena_refs.release(); sc->scratch.release();
     for (cudaEvent_t e : sc->t_ev) cudaEventDestroy(e);
-    if (sc->d_maxrec) cudaFree(sc->d_maxrec);
-    if (sc->h_maxrec) cudaFreeHost(sc->h_maxrec);
-    if (sc->ev_maxrec) cudaEventDestroy(sc->ev_maxrec);
+    if (sc->h_ctl) cudaFreeHost(sc->h_ctl);
+    if (sc->ev_ctl) cudaEventDestroy(sc->ev_ctl);
     sc->h_env_scene.release(); sc->h_inst_mesh.release(); sc->h_cam_pose.release(); sc->h_inst_xform.release();
     sc->h_depth.release(); sc->h_rgb.release(); sc->h_id.release();
     if (sc->host_stream) cudaStreamDestroy(sc->host_stream);
     if (sc->copy_stream) cudaStreamDestroy(sc->copy_stream);
-    if (sc->ev_sub) cudaEventDestroy(sc->ev_sub);
+    for (cudaEvent_t e : sc->ev_sub) cudaEventDestroy(e);
     delete sc;
 }
 
 int gx_set_option(GxScene *sc, const char *name, int64_t value) {
     if (!sc || !name) return fail(GX_ERR_INVALID_ARG, "NULL argument");
     if (!strcmp(name, "cull")) { sc->opt_cull = value != 0; return GX_OK; }
+    if (!strcmp(name, "subcull")) { sc->opt_subcull = value != 0; return GX_OK; }
+    if (!strcmp(name, "hiz")) { sc->opt_hiz = value != 0; return GX_OK; }
     if (!strcmp(name, "stats")) { sc->opt_stats = value != 0; return GX_OK; }
     if (!strcmp(name, "timing")) {   // 1 = start (and reset) the per-kernel event timing, 0 = stop recording
         sc->opt_timing = value != 0;
-        if (value) { sc->t_used = 0; sc->t_calls = 0; }
+        if (value) { sc->t_used = 0; sc->t_calls = 0; sc->t_full = false; }
         return GX_OK;
     }
-    if (!strcmp(name, "subcull")) { sc->opt_subcull = value != 0; return GX_OK; }
-    if (!strcmp(name, "bands")) {
-        if (value != 0 && value != 1 && value != 2 && value != 4) return fail(GX_ERR_INVALID_ARG, "bands must be 0, 1, 2 or 4");
-        sc->opt_bands = (int)value;
-        return GX_OK;
-    }
-    if (!strcmp(name, "occlusion")) {
-        if (value < 0 || value > 3) return fail(GX_ERR_INVALID_ARG, "occlusion must be 0 (off), 1 (automatic), 2 or 3 (passes)");
-        sc->opt_occlusion = (int)value;
-        return GX_OK;
-    }
-    if (!strcmp(name, "occl_area")) {
-        if (value < 0 || value > 16384) return fail(GX_ERR_INVALID_ARG, "occl_area out of range");
-        sc->opt_occl_area = (int)value;
-        return GX_OK;
-    }
-    if (!strcmp(name, "occluder_pct")) {
-        if (value < 1 || value > 100) return fail(GX_ERR_INVALID_ARG, "occluder_pct must be in [1, 100]");
-        sc->opt_occluder_pct = (int)value;
-        return GX_OK;
-    }
-    if (!strcmp(name, "path")) {
-        if (value < 0 || value > 1) return fail(GX_ERR_INVALID_ARG, "path must be 0 or 1");
-        sc->opt_path = (int)value;
-        return GX_OK;
-    }
-    if (!strcmp(name, "pool_slots")) {
-        if (value < 0 || value > (1 << 24)) return fail(GX_ERR_INVALID_ARG, "pool_slots out of range");
-        sc->opt_pool_slots = value;
+    if (!strcmp(name, "big_px")) {
+        if (value < 1 || value > gx::TILE) return fail(GX_ERR_INVALID_ARG, "big_px must be in [1, %d]", gx::TILE);
+        sc->opt_big_px = (int)value;
         return GX_OK;
     }
     if (!strcmp(name, "pool_bytes")) {
@@ -470,9 +371,9 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
         sc->opt_pool_bytes = value;
         return GX_OK;
     }
-    if (!strcmp(name, "big_slots") || !strcmp(name, "chunk_slots")) {
-        if (value < 32 || value > (1 << 20)) return fail(GX_ERR_INVALID_ARG, "%s must be in [32, 2^20]", name);
-        (name[0] == 'b' ? sc->opt_big_slots : sc->opt_chunk_slots) = (int)value;
+    if (!strcmp(name, "arena_slots")) {
+        if (value < 0 || value > 0xFFFFFFFFll) return fail(GX_ERR_INVALID_ARG, "arena_slots out of range");
+        sc->opt_arena_slots = value;
         return GX_OK;
     }
     return fail(GX_ERR_INVALID_ARG, "unknown option '%s'", name);
@@ -482,8 +383,9 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
     if (!sc || !name || !out) return fail(GX_ERR_INVALID_ARG, "NULL argument");
     if (!strcmp(name, "launches")) { *out = sc->last_launches; return GX_OK; }
     if (!strcmp(name, "timed_calls")) { *out = sc->t_calls; return GX_OK; }
+    if (!strcmp(name, "arena_bytes")) { *out = (int64_t)(sc->arena_slots * 88); return GX_OK; }
     if (!strncmp(name, "ns_", 3)) {   // nanoseconds per kernel class, summed over the calls since "timing" was set
-        static const char *kinds[6] = {"", "cull", "geom", "order", "raster", "fallback"};
+        static const char *kinds[6] = {"", "cull", "geom", "bin", "raster", "tail"};
         int kind = 0;
         for (int k = 1; k < 6; ++k) if (!strcmp(name + 3, kinds[k])) kind = k;
         if (!kind) return fail(GX_ERR_INVALID_ARG, "unknown stat '%s'", name);
@@ -499,21 +401,24 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
         *out = (int64_t)ns;
         return GX_OK;
     }
-    if (!strcmp(name, "max_env_records") || !strcmp(name, "p50_env_records")) {   // last chunk of the two-kernel path
-        *out = 0;
-        if (sc->last_chunk_n <= 0) return GX_OK;
-        DeviceGuard guard(sc->device);
-        std::vector<uint32_t> cnt(2 * (size_t)sc->last_chunk_n);
-        GX_CUDA(cudaStreamSynchronize(sc->last_stream));
-        GX_CUDA(cudaMemcpy(cnt.data(), sc->pipe_scratch.p + 12, cnt.size() * 4, cudaMemcpyDeviceToHost));
-        std::vector<uint32_t> tot(sc->last_chunk_n);
-        for (int e = 0; e < sc->last_chunk_n; ++e) tot[e] = cnt[2 * e] + cnt[2 * e + 1];
-        std::sort(tot.begin(), tot.end());
-        *out = name[0] == 'm' ? tot.back() : tot[tot.size() / 2];
-        return GX_OK;
+    {   // control words of the most recent call: waves, the sum and maximum of the per-environment slot bounds
+        static const char *cnames[4] = {"waves", "sum_slots", "max_env_slots", "bad_ids"};
+        for (int k = 0; k < 4; ++k)
+            if (!strcmp(name, cnames[k])) {
+                DeviceGuard guard(sc->device);
+                if (!sc->scratch.p) { *out = 0; return GX_OK; }
+                uint32_t c[gx::C_NCTL];
+                GX_CUDA(cudaStreamSynchronize(sc->last_stream));
+                GX_CUDA(cudaMemcpy(c, sc->scratch.p, sizeof(c), cudaMemcpyDeviceToHost));
+                if (k == 0) *out = c[gx::C_WAVES];
+                else if (k == 1) *out = (int64_t)((uint64_t)c[gx::C_SUM_U] | ((uint64_t)c[gx::C_SUM_U + 1] << 32));
+                else if (k == 2) *out = c[gx::C_MAX_U];
+                else *out = c[gx::C_BAD_ENVS];
+                return GX_OK;
+            }
     }
     static const char *names[GX_NSTAT] = {"clusters_tested", "clusters_drawn", "triangles_in", "triangles_raster",
-                                          "fragments", "overflow_envs", "clusters_occluded", "records_occluded"};
+                                          "fragments", "records_occluded", "blocks_drawn", "tile_refs"};
     for (int k = 0; k < GX_NSTAT; ++k)
         if (!strcmp(name, names[k])) {
             DeviceGuard guard(sc->device);
@@ -541,162 +446,159 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
         return fail(GX_ERR_INVALID_ARG, "width and height must be positive multiples of 16, got %dx%d", cam->width, cam->height);
     if (!(cam->znear > 0.0f) || !(cam->zfar > cam->znear)) return fail(GX_ERR_INVALID_ARG, "need 0 < znear < zfar");
     if (!(cam->fx > 0.0f) || !(cam->fy > 0.0f)) return fail(GX_ERR_INVALID_ARG, "fx and fy must be positive");
-    if ((long long)cam->width * cam->height > 16384)
-        return fail(GX_ERR_UNSUPPORTED, "width*height = %lld exceeds 16384 (the frame must fit shared memory)",
-                    (long long)cam->width * cam->height);
-    if ((unsigned long long)sc->max_static_nt + (unsigned long long)K * sc->max_dyn_nt >= (1ull << 31))
-        return fail(GX_ERR_UNSUPPORTED, "more than 2^31 triangles per environment");
+    if (cam->width > GX_MAX_FRAME || cam->height > GX_MAX_FRAME)
+        return fail(GX_ERR_UNSUPPORTED, "width and height must be <= %d (8-bit box fields of a record), got %dx%d",
+                    GX_MAX_FRAME, cam->width, cam->height);
+    const unsigned long long worst_tris = (unsigned long long)sc->max_static_nt + (unsigned long long)K * sc->max_dyn_nt;
+    if (worst_tris >= (1ull << 29)) return fail(GX_ERR_UNSUPPORTED, "more than 2^29 triangles per environment");
+    if ((unsigned long long)N * (unsigned long long)((cam->width / 16) * (cam->height / 16)) >= (1ull << 31))
+        return fail(GX_ERR_UNSUPPORTED, "more than 2^31 tiles per call");
     DeviceGuard guard(sc->device);
     if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
+    const bool st = sc->opt_stats != 0;
 
-    if (cam->width > 128 || cam->height > 128)
-        return fail(GX_ERR_UNSUPPORTED, "width and height must be <= 128 in this build, got %dx%d", cam->width, cam->height);
-    GxParams P;
+    gx::PipeParams PP;
+    GxParams &P = PP.g;
     P.verts = sc->verts; P.tris = sc->tris; P.batches = sc->batches; P.subs = sc->subs; P.clusters = sc->clusters; P.meshes = sc->meshes;
     P.n_static = sc->n_static; P.n_dyn = sc->n_dyn;
     P.N = N; P.K = K; P.W = cam->width; P.H = cam->height;
     P.fx = cam->fx; P.fy = cam->fy; P.znear = cam->znear; P.zfar = cam->zfar;
     P.env_scene = env_scene; P.cam_pose = cam_pose; P.inst_mesh = inst_mesh; P.inst_xform = inst_xform;
     P.rgb = rgb_out; P.depth = depth_out; P.id = id_out;
-    P.obs = obs_out; P.obs_dmin = obs_dmin; P.obs_range = obs_dmax - obs_dmin;
-    P.env_counter = sc->env_counter; P.stats = sc->stats;
-    P.env_filter = nullptr;
+    P.obs = obs_out; P.obs_dmin = obs_dmin; P.obs_dmax = obs_dmax; P.obs_range = obs_dmax - obs_dmin;
+    P.stats = sc->stats;
     P.cull = sc->opt_cull;
-    P.cull_chunk = gx::WORK_CAP / (int)sc->max_nbatch;
+    PP.tiles_x = P.W / gx::TILE; PP.tiles_y = P.H / gx::TILE; PP.T = PP.tiles_x * PP.tiles_y;
+    PP.bucket_off = -log2f(P.znear);
+    PP.bucket_scale = (float)gx::NBUCKET / log2f(P.zfar / P.znear);
+    PP.subcull = sc->opt_subcull;
+    PP.big_px = sc->opt_big_px;
+    PP.hiz = sc->opt_hiz;
 
-    GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
-    const bool st = sc->opt_stats != 0;
-    sc->last_stream = stream;
-    sc->last_chunk_n = 0;
-    if (sc->opt_path == 1) {
-        GX_CUDA(cudaMemsetAsync(sc->env_counter, 0, sizeof(unsigned int), stream));
-        const int rc = launch_single(sc, P, stream, st);
-        if (rc != GX_OK) return rc;
-        sc->last_launches = 1;
-        return GX_OK;
-    }
-
-    // ---- two-kernel path, in chunks of environments that share the record pool ----------------------
-    const int64_t npix = (int64_t)P.W * P.H;
-    // bands: (environment, band) is the raster task; several bands only if each is a multiple of 32 rows
-    int bands = sc->opt_bands > 0 ? sc->opt_bands : (npix * 8 > 65536 ? 2 : 1);
-    while (bands > 1 && (P.H % bands || (P.H / bands) % 32)) bands >>= 1;
-    const int bh = P.H / bands;
-    // pool segment per raster task: a default from the frame size, raised to 1.25 x the largest record count any
-    // task of an earlier call on this handle produced (read back asynchronously; a call whose segments are too
-    // small is still rendered correctly, by the overflow pass, and the next call is sized for it)
-    if (!sc->d_maxrec) {
-        GX_CUDA(cudaMalloc(&sc->d_maxrec, 2 * sizeof(uint32_t)));
-        GX_CUDA(cudaMallocHost(&sc->h_maxrec, 2 * sizeof(uint32_t)));
-        GX_CUDA(cudaEventCreateWithFlags(&sc->ev_maxrec, cudaEventDisableTiming));
-    }
-    if (sc->maxrec_pending && cudaEventQuery(sc->ev_maxrec) == cudaSuccess) {
-        sc->hist_n = std::max(sc->hist_n, sc->h_maxrec[0]);
-        sc->hist_w = std::max(sc->hist_w, sc->h_maxrec[1]);
-        sc->maxrec_pending = false;
+    // ---- arena: record slots shared by the environments of a wave ------------------------------------
+    // An environment's segment is sized by U, the bound cull_kernel computes; the arena must hold the largest
+    // possible U (four slots per triangle: everything clipped by the near plane into two pieces with float
+    // colours), so that a wave always has room for at least one environment.  Beyond that it is sized from the
+    // history of earlier calls (mean U per environment, read back asynchronously) or, on the first call, from a
+    // default of 32 Ki slots per environment, and capped by the budget; what does not fit goes to later waves.
+    if (sc->ctl_pending && cudaEventQuery(sc->ev_ctl) == cudaSuccess) {
+        const uint64_t sum = (uint64_t)sc->h_ctl[gx::C_SUM_U] | ((uint64_t)sc->h_ctl[gx::C_SUM_U + 1] << 32);
+        sc->hist_u_per_env = std::max(sc->hist_u_per_env, (double)sum / (double)std::max(sc->ctl_N, 1));
+        sc->ctl_pending = false;
     }
     cudaGetLastError();   // (cudaErrorNotReady of the query is not an error)
-    auto grow = [](uint32_t seen) { return ((int64_t)seen + seen / 4 + 1023) & ~(int64_t)1023; };
-    const int64_t cap_n = sc->opt_pool_slots > 0 ? sc->opt_pool_slots
-                                                 : std::max<int64_t>(std::max<int64_t>(2048, 4 * npix / bands), grow(sc->hist_n));
-    const int64_t cap_w = sc->opt_pool_slots > 0 ? (std::max<int64_t>(64, cap_n / 8) & ~(int64_t)1)
-                                                 : std::max<int64_t>(std::max<int64_t>(64, cap_n / 8) & ~(int64_t)1, grow(sc->hist_w));
-    const int64_t env_bytes = (cap_n + cap_w) * 64 * bands;
-    const int64_t budget = sc->opt_pool_bytes > 0 ? sc->opt_pool_bytes : (int64_t)8 << 30;
-    const int chunk = (int)std::max<int64_t>(1, std::min<int64_t>(N, budget / env_bytes));
+    const uint64_t worst_env = 4ull * worst_tris + 64;
+    const int64_t budget = sc->opt_pool_bytes > 0 ? sc->opt_pool_bytes : (int64_t)4 << 30;
+    uint64_t want;
+    if (sc->opt_arena_slots > 0) want = (uint64_t)sc->opt_arena_slots;
+    else {
+        const double per_env = sc->hist_u_per_env > 0.0 ? 1.25 * sc->hist_u_per_env + 1024.0 : (double)std::min<uint64_t>(worst_env, 32768);
+        want = std::min<uint64_t>((uint64_t)(per_env * N), (uint64_t)N * worst_env);
+        want = std::min<uint64_t>(want, (uint64_t)budget / 88);
+    }
+    want = std::min<uint64_t>(std::max<uint64_t>(want, worst_env), 0xFFFFFF00ull);
     int rc;
-    if ((rc = sc->pool.reserve((size_t)chunk * bands * (size_t)(cap_n + cap_w) * 4)) != GX_OK) return rc;
-    // scratch words: counters[12] | cnt[2*tasks] | env_flag[chunk] (zeroed per chunk) | order[tasks] | cnt1[2*tasks] |
-    //                thr[chunk] | env_idb[chunk*(K+1)] | env_mv[chunk*(K+1)*12] | hiz[chunk*HZ_STRIDE] | items[4*...]
-    // occluder scheme: 2 or 3 passes; automatic = 2 passes where they pay: frames of 8192 pixels or more (the hi-Z
-    // tiles are 8x8 pixels) and enough environments that two rounds of kernels still fill the GPU
-    const int n_pass = sc->opt_occlusion == 1 ? ((npix >= 8192 && N >= 512) ? 2 : 0) : sc->opt_occlusion;
-    const bool two_phase = sc->opt_cull && n_pass >= 2;
-    const size_t k1 = (size_t)K + 1, tasks = (size_t)chunk * bands;
-    const size_t items_per_env = (size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches;
-    const size_t n_zero = 12 + 2 * tasks + (size_t)chunk;
-    const size_t off_order = n_zero, off_cnt1 = off_order + tasks, off_thr = off_cnt1 + 2 * tasks;
-    const size_t off_idb = off_thr + chunk, off_mv = off_idb + chunk * k1, off_hiz = off_mv + chunk * k1 * 12;
-    const size_t off_items = (off_hiz + (size_t)chunk * gx::HZ_STRIDE + 3) & ~(size_t)3;
-    if ((rc = sc->pipe_scratch.reserve(off_items + 4 * (size_t)chunk * std::max<size_t>(items_per_env, 1))) != GX_OK) return rc;
-    if (two_phase && (rc = sc->frames.reserve((size_t)chunk * (size_t)npix)) != GX_OK) return rc;
-    int launches = 0;
-    GX_CUDA(cudaMemsetAsync(sc->d_maxrec, 0, 2 * sizeof(uint32_t), stream));
-    for (int e0 = 0; e0 < N; e0 += chunk) {
-        const int n = std::min(chunk, N - e0);
-        gx::PipeParams PP;
-        PP.g = P;
-        PP.g.N = n;
-        PP.g.env_scene = env_scene + e0;
-        PP.g.cam_pose = cam_pose + (size_t)e0 * 16;
-        PP.g.inst_mesh = inst_mesh ? inst_mesh + (size_t)e0 * K : nullptr;
-        PP.g.inst_xform = inst_xform ? inst_xform + (size_t)e0 * K * 16 : nullptr;
-        PP.g.rgb = rgb_out ? rgb_out + (size_t)e0 * npix * 3 : nullptr;
-        PP.g.depth = depth_out ? depth_out + (size_t)e0 * npix : nullptr;
-        PP.g.obs = obs_out ? obs_out + (size_t)e0 * npix * 4 : nullptr;
-        PP.g.id = id_out ? id_out + (size_t)e0 * npix : nullptr;
-        PP.recs = sc->pool.p;
-        PP.counters = sc->pipe_scratch.p;
-        PP.cnt = sc->pipe_scratch.p + 12;
-        PP.env_flag = sc->pipe_scratch.p + 12 + 2 * tasks;
-        PP.cnt1 = sc->pipe_scratch.p + off_cnt1;
-        PP.thr = reinterpret_cast<float *>(sc->pipe_scratch.p + off_thr);
-        PP.hiz = reinterpret_cast<float *>(sc->pipe_scratch.p + off_hiz);
-        PP.frames = sc->frames.p;
-        PP.occl_pct = two_phase ? sc->opt_occluder_pct : 100;
-        PP.cap_n = (int32_t)cap_n;
-        PP.cap_w = (int32_t)cap_w;
-        PP.bands = bands;
-        PP.subcull = sc->opt_cull && sc->opt_subcull;
-        PP.phase = 0;
-        PP.bh = bh;
-        PP.big_slots = sc->opt_big_slots;
-        PP.chunk_slots = sc->opt_chunk_slots;
-        PP.order = sc->pipe_scratch.p + off_order;
-        PP.maxrec = sc->d_maxrec;
-        PP.env_idb = sc->pipe_scratch.p + off_idb;
-        PP.env_mv = reinterpret_cast<float *>(sc->pipe_scratch.p + off_mv);
-        PP.items = reinterpret_cast<uint4 *>(sc->pipe_scratch.p + off_items);
-        GX_CUDA(cudaMemsetAsync(sc->pipe_scratch.p, 0, n_zero * sizeof(uint32_t), stream));
-        PP.nphase = two_phase ? n_pass : 0;
-        PP.occl_area = (float)sc->opt_occl_area;
-        if (!two_phase) {
-            if ((rc = launch_pass<0>(sc, PP, stream, st)) != GX_OK) return rc;
-            launches += 4;
+    if (want > sc->arena_slots) {
+        if ((rc = sc->arena_recs.reserve((size_t)want * 4)) != GX_OK) return rc;
+        if ((rc = sc->arena_bbs.reserve((size_t)want)) != GX_OK) return rc;
+        if ((rc = sc->arena_refs.reserve((size_t)want * 4)) != GX_OK) return rc;
+        sc->arena_slots = (size_t)want;
+    }
+    PP.recs = sc->arena_recs.p; PP.bbs = sc->arena_bbs.p; PP.refs = sc->arena_refs.p;
+    PP.arena_slots = (uint32_t)(sc->opt_arena_slots > 0 ? std::max<uint64_t>((uint64_t)sc->opt_arena_slots, worst_env) : sc->arena_slots);
+
+    // ---- scratch words: ctl | n_items | U | rec_base | item_pre | cnt | env_idb | env_mv | tile_off | tasks | items
+    const size_t n = (size_t)N, k1 = (size_t)K + 1, NK1 = (size_t)PP.T * gx::NBUCKET + 1;
+    PP.item_stride = (int32_t)std::max<size_t>((size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches, 1);
+    size_t off = 32;
+    const size_t o_nitems = off; off += n;
+    const size_t o_U = off; off += n;
+    const size_t o_base = off; off += n;
+    const size_t o_ipre = off; off += n + 1;
+    const size_t o_cnt = off; off += 2 * n;
+    const size_t o_idb = off; off += n * k1;
+    const size_t o_mv = off; off += n * k1 * 12;
+    const size_t o_toff = off; off += n * NK1;
+    const size_t o_tasks = off; off += (size_t)gx::NCLASS * n * (size_t)PP.T;
+    off = (off + 3) & ~(size_t)3;
+    const size_t o_items = off; off += 4 * n * (size_t)PP.item_stride;
+    if ((rc = sc->scratch.reserve(off)) != GX_OK) return rc;
+    uint32_t *sp = sc->scratch.p;
+    PP.ctl = sp; PP.n_items = sp + o_nitems; PP.U = sp + o_U; PP.rec_base = sp + o_base; PP.item_pre = sp + o_ipre;
+    PP.cnt = sp + o_cnt; PP.env_idb = sp + o_idb; PP.env_mv = reinterpret_cast<float *>(sp + o_mv);
+    PP.tile_off = sp + o_toff; PP.tasks = sp + o_tasks; PP.items = reinterpret_cast<uint4 *>(sp + o_items);
+
+    sc->last_stream = stream;
+    if (st) GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
+    GX_CUDA(cudaMemsetAsync(PP.ctl, 0, 32 * sizeof(uint32_t), stream));
+    if ((rc = mark(sc, stream, 0)) != GX_OK) return rc;
+
+    // K1: one CTA per environment: 4 warps for small scenes, 16 where an environment has thousands of sub-clusters
+    {
+        const size_t csmem = gx::env_smem_bytes(K);
+        if ((size_t)PP.item_stride > 512) {
+            auto ck = st ? gx::cull_kernel<16, true> : gx::cull_kernel<16, false>;
+            ck<<<N, 16 * 32, csmem, stream>>>(PP);
         } else {
-            PP.phase = 1;
-            if ((rc = launch_pass<1>(sc, PP, stream, st)) != GX_OK) return rc;
-            if (PP.nphase == 3) {
-                PP.counters = sc->pipe_scratch.p + 8;
-                PP.phase = 2;
-                if ((rc = launch_pass<3>(sc, PP, stream, st)) != GX_OK) return rc;
-                launches += 4;
-            }
-            PP.counters = sc->pipe_scratch.p + 4;
-            PP.phase = PP.nphase;
-            if ((rc = launch_pass<2>(sc, PP, stream, st)) != GX_OK) return rc;
-            launches += 8;
+            auto ck = st ? gx::cull_kernel<4, true> : gx::cull_kernel<4, false>;
+            ck<<<N, 4 * 32, csmem, stream>>>(PP);
         }
-        // environments whose records overflowed their pool segment: single-kernel pass over the flagged ones
-        GxParams PL = PP.g;
-        PL.env_counter = sc->pipe_scratch.p + 3;
-        PL.env_filter = PP.env_flag;
-        if ((rc = launch_single(sc, PL, stream, st)) != GX_OK) return rc;
+        GX_CUDA(cudaGetLastError());
+        if ((rc = mark(sc, stream, 1)) != GX_OK) return rc;
+    }
+    // K2: persistent independent warps
+    {
+        constexpr int GW = 8;
+        auto gk = st ? gx::geom_kernel<GW, true> : gx::geom_kernel<GW, false>;
+        const size_t gsmem = (size_t)GW * gx::GEOM_WARP_SMEM;
+        int per_sm = 0;
+        if ((rc = plan_of(sc, (const void *)gk, GW * 32, gsmem, &per_sm)) != GX_OK) return rc;
+        gk<<<sc->num_sms * per_sm, GW * 32, gsmem, stream>>>(PP);
+        GX_CUDA(cudaGetLastError());
+        if ((rc = mark(sc, stream, 2)) != GX_OK) return rc;
+    }
+    // K3: one CTA per environment at a time
+    {
+        auto bk = st ? gx::bin_kernel<true> : gx::bin_kernel<false>;
+        const size_t bsmem = (size_t)2 * PP.T * gx::NBUCKET * 4;
+        int per_sm = 0;
+        if ((rc = plan_of(sc, (const void *)bk, 256, bsmem, &per_sm)) != GX_OK) return rc;
+        bk<<<std::min(N, sc->num_sms * per_sm), 256, bsmem, stream>>>(PP);
+        GX_CUDA(cudaGetLastError());
+        if ((rc = mark(sc, stream, 3)) != GX_OK) return rc;
+    }
+    // K4 + K5: persistent independent warps, one tile each at a time
+    {
+        constexpr int RW = 8;
+        auto rk = st ? gx::raster_kernel<RW, true> : gx::raster_kernel<RW, false>;
+        const size_t rsmem = (size_t)RW * gx::RAST_WARP_SMEM;
+        int per_sm = 0;
+        if ((rc = plan_of(sc, (const void *)rk, RW * 32, rsmem, &per_sm)) != GX_OK) return rc;
+        rk<<<sc->num_sms * per_sm, RW * 32, rsmem, stream>>>(PP);
+        GX_CUDA(cudaGetLastError());
+        if ((rc = mark(sc, stream, 4)) != GX_OK) return rc;
+    }
+    // the tail: later waves, on the device (exits at once when the first wave took every environment)
+    {
+        auto tk = st ? gx::tail_kernel<true> : gx::tail_kernel<false>;
+        const size_t tsmem = gx::tail_smem_bytes(PP.T);
+        int per_sm = 0;
+        if ((rc = plan_of(sc, (const void *)tk, gx::TAIL_WARPS * 32, tsmem, &per_sm)) != GX_OK) return rc;
+        void *args[1] = {(void *)&PP};
+        GX_CUDA(cudaLaunchCooperativeKernel((const void *)tk, dim3((unsigned)(sc->num_sms * per_sm)), dim3(gx::TAIL_WARPS * 32), args, tsmem, stream));
         if ((rc = mark(sc, stream, 5)) != GX_OK) return rc;
-        launches += 1;
-        sc->last_chunk_n = n * bands;
     }
-    if (!sc->maxrec_pending) {   // (a read-back still in flight keeps its buffer)
-        GX_CUDA(cudaMemcpyAsync(sc->h_maxrec, sc->d_maxrec, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
-        GX_CUDA(cudaEventRecord(sc->ev_maxrec, stream));
-        sc->maxrec_pending = true;
+    if (!sc->ctl_pending) {   // (a read-back still in flight keeps its buffer)
+        GX_CUDA(cudaMemcpyAsync(sc->h_ctl, PP.ctl, gx::C_NCTL * sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
+        GX_CUDA(cudaEventRecord(sc->ev_ctl, stream));
+        sc->ctl_pending = true;
+        sc->ctl_N = N;
     }
-    sc->last_launches = launches;
-    if (sc->opt_timing) ++sc->t_calls;
+    sc->last_launches = 5;
+    if (sc->opt_timing && !sc->t_full) ++sc->t_calls;
     return GX_OK;
 }
-
 
 int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
                     const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,
@@ -725,6 +627,7 @@ int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K,
     DeviceGuard guard(sc->device);
     if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
     if (!sc->host_stream) GX_CUDA(cudaStreamCreateWithFlags(&sc->host_stream, cudaStreamNonBlocking));
+    if (!sc->copy_stream) GX_CUDA(cudaStreamCreateWithFlags(&sc->copy_stream, cudaStreamNonBlocking));
     cudaStream_t st = sc->host_stream;
     const size_t npix = (size_t)cam->width * cam->height, nk = (size_t)N * K;
     int rc;
@@ -739,14 +642,12 @@ int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K,
         GX_CUDA(cudaMemcpyAsync(sc->h_inst_mesh.p, inst_mesh, nk * 4, cudaMemcpyHostToDevice, st));
         GX_CUDA(cudaMemcpyAsync(sc->h_inst_xform.p, inst_xform, nk * 64, cudaMemcpyHostToDevice, st));
     }
-    // render in sub-batches of 512 environments and copy each one's images back on a second stream while the next
-    // one renders (the device-to-host copy of RGBD is as long as the rendering itself)
-    if (!sc->copy_stream) {
-        GX_CUDA(cudaStreamCreateWithFlags(&sc->copy_stream, cudaStreamNonBlocking));
-        GX_CUDA(cudaEventCreateWithFlags(&sc->ev_sub, cudaEventDisableTiming));
-    }
-    const int sub = 512;
-    for (int e0 = 0; e0 < N; e0 += sub) {
+    // render in sub-batches and copy each one's images back on a second stream while the next one renders: the
+    // device-to-host copy of RGBD over PCIe takes several times longer than the rendering, so the sub-batches are
+    // small (the first render and the last copy are the only parts not overlapped)
+    const int sub = std::max(64, std::min(256, (N + 7) / 8));
+    size_t n_sub = 0;
+    for (int e0 = 0; e0 < N; e0 += sub, ++n_sub) {
         const int n = std::min(sub, N - e0);
         const size_t o = (size_t)e0 * npix, cnt = (size_t)n * npix;
         rc = gx_render_batch(sc, cam, n, K, sc->h_env_scene.p + e0, sc->h_cam_pose.p + (size_t)e0 * 16,
@@ -754,8 +655,13 @@ int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K,
                              K > 0 ? sc->h_inst_xform.p + (size_t)e0 * K * 16 : nullptr,
                              rgb_out ? sc->h_rgb.p + o * 3 : nullptr, sc->h_depth.p + o, id_out ? sc->h_id.p + o : nullptr, st);
         if (rc != GX_OK) return rc;
-        GX_CUDA(cudaEventRecord(sc->ev_sub, st));
-        GX_CUDA(cudaStreamWaitEvent(sc->copy_stream, sc->ev_sub, 0));
+        if (n_sub == sc->ev_sub.size()) {
+            cudaEvent_t e;
+            GX_CUDA(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+            sc->ev_sub.push_back(e);
+        }
+        GX_CUDA(cudaEventRecord(sc->ev_sub[n_sub], st));
+        GX_CUDA(cudaStreamWaitEvent(sc->copy_stream, sc->ev_sub[n_sub], 0));
         GX_CUDA(cudaMemcpyAsync(depth_out + o, sc->h_depth.p + o, cnt * 4, cudaMemcpyDeviceToHost, sc->copy_stream));
         if (rgb_out) GX_CUDA(cudaMemcpyAsync(rgb_out + o * 3, sc->h_rgb.p + o * 3, cnt * 3, cudaMemcpyDeviceToHost, sc->copy_stream));
         if (id_out) GX_CUDA(cudaMemcpyAsync(id_out + o, sc->h_id.p + o, cnt * 4, cudaMemcpyDeviceToHost, sc->copy_stream));

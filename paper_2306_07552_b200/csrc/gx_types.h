@@ -33,7 +33,7 @@ struct __align__(16) GxMeshDev {
     uint32_t cluster_off, ncluster, nt, pad;
 };
 
-// Everything one launch needs; passed by value.
+// What every stage of one gx_render_batch call needs; passed by value inside PipeParams (gx_pipeline.cuh).
 struct GxParams {
     // scene (device)
     const float4 *verts;          // x, y, z, rgba8 bits; per batch contiguous
@@ -54,14 +54,10 @@ struct GxParams {
     float *depth;
     uint32_t *id;
     uint16_t *obs;                // [N,4,H,W] binary16 packed observation (N11), or NULL
-    float obs_dmin, obs_range;    // depth channel = (clamp(depth, dmin, dmin + range) - dmin) / range
-    // scratch
-    unsigned int *env_counter;    // zeroed before the launch; persistent CTAs draw environments from it
-    unsigned long long *stats;    // [GX_NSTAT], only touched by the STATS instantiation
-    const uint32_t *env_filter;   // NULL = render every environment; else only those with env_filter[env] != 0
-    int32_t cull;
-    int32_t cull_chunk;           // clusters per cull chunk: WORK_CAP / (largest nbatch of any cluster)
+    float obs_dmin, obs_dmax, obs_range;   // depth channel = (clamp(depth, dmin, dmax) - dmin) / range, range = dmax - dmin
+    unsigned long long *stats;    // [GX_NSTAT], only touched by the STATS instantiations
+    int32_t cull;                 // 0 = draw every cluster (verification)
 };
 
 enum { GX_STAT_CLUSTERS_TESTED = 0, GX_STAT_CLUSTERS_DRAWN, GX_STAT_TRIS_IN, GX_STAT_TRIS_RASTER,
-       GX_STAT_FRAGMENTS, GX_STAT_OVERFLOW_ENVS, GX_STAT_CLUSTERS_OCCLUDED, GX_STAT_RECORDS_OCCLUDED, GX_NSTAT };
+       GX_STAT_FRAGMENTS, GX_STAT_RECORDS_OCCLUDED, GX_STAT_BLOCKS_DRAWN, GX_STAT_REFS, GX_NSTAT };

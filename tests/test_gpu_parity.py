@@ -73,10 +73,10 @@ def test_config3_and_4_sampled(oracle_mod):
 @pytest.mark.parametrize("cfg,n", [(3, 12), (4, 32)])
 def test_config3_and_4_full_batch(oracle_mod, cfg, n):
     """configs[3] (4096 envs, 500k-triangle scenes) and configs[4] (16384 envs, 64x64 depth-only) at full size,
-    in the launch configuration bench.py --config times: several chunks of environments per call, two passes
-    (occluder scheme) on cfg 3, four 8-warp raster CTAs per SM on cfg 4.  The oracle renders n sampled
-    environments one by one.  The first call sizes the record pool from defaults (many environments overflow
-    and take the single-kernel pass), the second from the first call's record counts: both must match."""
+    in the launch configuration bench.py --config times.  The oracle renders n sampled environments one by one.
+    The first call sizes the record arena from defaults, the second from the first call's slot bounds; on cfg 3
+    the arena budget cannot hold the whole batch, so the later waves run inside the cooperative tail kernel: all
+    must match."""
     import torch
     from paper_2306_07552_b200 import binding as gx
     wl = gen.make_config(cfg)
@@ -90,8 +90,9 @@ def test_config3_and_4_full_batch(oracle_mod, cfg, n):
         g2 = render_gpu(wl, scene=scene, stats=True)
     finally:
         gx.gx_destroy(scene)
-    assert g1["stats"]["overflow_envs"] > g2["stats"]["overflow_envs"]
-    assert g2["stats"]["overflow_envs"] <= wl.N // 100
+    assert g1["stats"]["bad_ids"] == 0 and g1["stats"]["waves"] >= 1 and g2["stats"]["waves"] >= 1
+    if cfg == 3:
+        assert g1["stats"]["waves"] > 1      # 4096 environments of ~10^5 slots each do not fit 4 GB at once
     for g in (g1, g2):
         gs = {k: (v[sel] if isinstance(v, np.ndarray) else None) for k, v in g.items()}
         rep = compare(o, gs, check_rgb=not wl.depth_only)
@@ -101,73 +102,75 @@ def test_config3_and_4_full_batch(oracle_mod, cfg, n):
 
 
 def test_cull_is_conservative(oracle_mod):
-    """N10: the image with frustum culling on, and with frustum + hi-Z occlusion culling on, equals the image
-    with culling off, bit for bit."""
+    """N10: the image with frustum culling of clusters and sub-clusters and with hi-Z rejection in the tiles equals
+    the image with all of them off, bit for bit."""
     wl = gen.make_config(1, n_envs=16)
-    a = render_gpu(wl, cull=1, stats=True, options=dict(occlusion=0))
-    b = render_gpu(wl, cull=0, stats=True, options=dict(occlusion=0))
-    c = render_gpu(wl, cull=1, stats=True, options=dict(occlusion=2))   # frustum + hi-Z occlusion culling
+    a = render_gpu(wl, cull=1, stats=True)
+    b = render_gpu(wl, cull=0, stats=True, options=dict(hiz=0))
+    c = render_gpu(wl, cull=1, stats=True, options=dict(subcull=0))
+    d = render_gpu(wl, cull=1, stats=True, options=dict(hiz=0))
     for k in ("rgb", "depth", "id"):
         assert np.array_equal(a[k], b[k]), k
         assert np.array_equal(c[k], b[k]), k
+        assert np.array_equal(d[k], b[k]), k
     assert a["stats"]["clusters_drawn"] < b["stats"]["clusters_drawn"]
     assert b["stats"]["clusters_drawn"] == b["stats"]["clusters_tested"]
-    assert a["stats"]["triangles_raster"] == b["stats"]["triangles_raster"]
-    assert c["stats"]["triangles_raster"] < a["stats"]["triangles_raster"]
+    assert a["stats"]["triangles_raster"] == b["stats"]["triangles_raster"]     # culling only drops what covers nothing
+    assert a["stats"]["triangles_in"] < c["stats"]["triangles_in"] < b["stats"]["triangles_in"]
+    assert a["stats"]["records_occluded"] > 0 and d["stats"]["records_occluded"] == 0
+    assert a["stats"]["fragments"] < d["stats"]["fragments"]
 
 
-def test_paths_pool_overflow_and_chunking(oracle_mod):
-    """The two-kernel path (geometry -> record pool -> raster) against the oracle and against the single-kernel
-    path; a pool too small for some environments (those fall back to the single kernel) or for all of them;
-    a pool budget that forces several chunks; other raster pass-B thresholds: all bit-identical."""
+def test_waves_and_option_variants(oracle_mod):
+    """The pipeline against the oracle, then against itself under every switch that moves work around: an arena
+    too small for the batch (several waves of environments, the later ones inside the cooperative tail kernel, down
+    to one environment per wave), the block path for every record size (big_px), no hi-Z, no sub-cluster culling:
+    all bit-identical."""
     wl = gen.make_config(2, n_envs=20)
     o = oracle_mod.render(wl)
-    ref = render_gpu(wl, stats=True, options=dict(occlusion=2))
+    ref = render_gpu(wl, stats=True)
     rep = compare(o, ref)
     assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, rep
-    assert ref["stats"]["overflow_envs"] == 0 and ref["stats"]["launches"] == 9
+    assert ref["stats"]["waves"] == 1 and ref["stats"]["launches"] == 5 and ref["stats"]["bad_ids"] == 0
+    assert ref["stats"]["max_env_slots"] * wl.N >= ref["stats"]["sum_slots"] > ref["stats"]["triangles_raster"]
+    per_env = ref["stats"]["max_env_slots"]
     variants = {
-        "single kernel": dict(path=1),
-        "some overflow": dict(pool_slots=12288),
-        "all overflow": dict(pool_slots=64),
-        "chunks of 3": dict(pool_bytes=3 * (65536 + 8192) * 64, occlusion=2),
-        "no occluder phase": dict(occlusion=0),
-        "2 passes, area 8": dict(occlusion=2, occl_area=8),
-        "1 band": dict(bands=1),
+        "arena for ~3 environments": dict(arena_slots=3 * per_env),
+        "arena for 1 environment": dict(arena_slots=1),
+        "arena by budget": dict(pool_bytes=88 * 7 * per_env),
+        "block path for every record": dict(big_px=1),
+        "block path from 4 px": dict(big_px=4),
+        "block path from 8 px": dict(big_px=8),
+        "no hi-Z": dict(hiz=0),
         "no sub-cluster culling": dict(subcull=0),
-        "4 bands": dict(bands=4),
-        "4 bands, no occluder phase": dict(bands=4, occlusion=0),
-        "3 passes": dict(occlusion=3),
-        "3 passes, area 1, 20 %": dict(occlusion=3, occl_area=1, occluder_pct=20),
-        "2 passes, area 64": dict(occlusion=2, occl_area=64),
-        "occluder phase 5 %": dict(occlusion=2, occluder_pct=5),
-        "occluder phase 70 %": dict(occlusion=2, occluder_pct=70),
-        "4 bands, occluder phase": dict(bands=4, occlusion=2),
-        "small pass-B chunks": dict(big_slots=64, chunk_slots=32),
-        "no pass B": dict(big_slots=1 << 20),
+        "no hi-Z, blocks from 2 px, 2 environments per wave": dict(hiz=0, big_px=2, arena_slots=2 * per_env),
     }
     for name, opts in variants.items():
         g = render_gpu(wl, stats=True, options=opts)
         for k in ("rgb", "depth", "id"):
             assert np.array_equal(ref[k], g[k]), (name, k)
-        if name == "all overflow":
-            assert g["stats"]["overflow_envs"] == wl.N
-        if name == "some overflow":
-            assert 0 < g["stats"]["overflow_envs"] < wl.N, g["stats"]
-        if name == "chunks of 3":
-            assert g["stats"]["launches"] == 9 * 7
-        if name == "no occluder phase":
-            assert g["stats"]["launches"] == 5 and g["stats"]["clusters_occluded"] == 0
-            assert g["stats"]["triangles_raster"] > ref["stats"]["triangles_raster"]
-    assert ref["stats"]["clusters_occluded"] >= 0 and ref["stats"]["records_occluded"] > 0
+        if name == "arena for 1 environment":
+            assert g["stats"]["waves"] == wl.N, g["stats"]
+        if name.startswith("arena for ~3") or name == "arena by budget":
+            assert 1 < g["stats"]["waves"] < wl.N, g["stats"]
+        if name == "block path for every record":
+            assert g["stats"]["tile_refs"] == 0 and g["stats"]["blocks_drawn"] > ref["stats"]["blocks_drawn"]
+    assert ref["stats"]["records_occluded"] > 0 and ref["stats"]["tile_refs"] > 0
 
 
 def test_sharding_and_determinism():
     """concatenating per-shard outputs equals the single call, bit-identical; and the same
-    call twice gives the same bits."""
+    call ten times gives the same bits (the order in which warps append records and fill tile lists differs from
+    run to run; the image must not)."""
     wl = gen.make_config(1, n_envs=20)
     full = render_gpu(wl)
     again = render_gpu(wl)
+    big = gen.make_config(2, n_envs=64)
+    first = render_gpu(big)
+    for _ in range(9):
+        nxt = render_gpu(big)
+        for k in ("rgb", "depth", "id"):
+            assert np.array_equal(first[k], nxt[k]), k
     parts = [render_gpu(wl.subset(np.arange(a, b))) for a, b in ((0, 7), (7, 8), (8, 20))]
     for k in ("rgb", "depth", "id"):
         assert np.array_equal(full[k], again[k]), k
@@ -209,7 +212,7 @@ def _quad_workload(W, H, z, half, K=0):
 
 def test_edge_cases(oracle_mod):
     """Degenerate inputs: K = 0; all slots empty; a frame with nothing in view (all background); a quad that
-    fills the whole frame and crosses all four image borders; the far plane; maximum frame size 128x128 and
+    fills the whole frame and crosses all four image borders; the far plane; the maximum frame size 256x256 and
     the smallest 16x16; non-square frames."""
     # K = 0, small quad: closed form -- pixel rectangle at exactly depth 2
     wl = _quad_workload(64, 64, 2.0, 0.5)
@@ -229,7 +232,8 @@ def test_edge_cases(oracle_mod):
     g = render_gpu(wl)
     assert np.all(g["id"] == BG) and np.all(g["depth"] == 0) and np.all(g["rgb"] == 0)
     # huge quad over the whole frame, partially behind the camera after a pitch: near clip + all borders
-    for (W, H) in ((128, 128), (16, 16), (128, 64), (48, 112), (128, 96), (96, 128), (64, 128), (112, 80)):
+    for (W, H) in ((128, 128), (16, 16), (128, 64), (48, 112), (128, 96), (96, 128), (64, 128), (112, 80), (256, 256), (224, 224),
+                   (256, 16), (16, 256)):
         wl = _quad_workload(W, H, 1.0, 50.0)
         c, s = np.cos(1.2), np.sin(1.2)
         wl.cam_pose = np.array([[1, 0, 0, 0, 0, c, -s, 0.3, 0, s, c, 0, 0, 0, 0, 1]], np.float32)
@@ -287,7 +291,7 @@ def test_argument_errors():
                 gx.gx_render_batch(sc, cam, N, 0, es, cp, None, None, None, d)
             assert e.value.code == gx.GX_ERR_INVALID_ARG
         with pytest.raises(gx.GxError) as e:
-            gx.gx_render_batch(sc, gx.GxCamera(256, 128, 1, 1, 0.1, 20), 4, 0, es, cp, None, None, None, d)
+            gx.gx_render_batch(sc, gx.GxCamera(272, 128, 1, 1, 0.1, 20), 4, 0, es, cp, None, None, None, d)
         assert e.value.code == gx.GX_ERR_UNSUPPORTED
         with pytest.raises(gx.GxError):
             gx.gx_set_option(sc, "nope", 1)
@@ -297,13 +301,14 @@ def test_argument_errors():
 
 def test_packed_observation(oracle_mod):
     """N11 / NEXT-1: gx_render_batch_obs writes the [N,4,H,W] binary16 observation bit-identical to the oracle's
-    packing of the oracle's images -- through the two-kernel path, the single-kernel path and the overflow pass."""
+    packing of the oracle's images -- with the default switches, with every record on the block path, without hi-Z
+    and through the waves of the tail kernel."""
     import torch
     from paper_2306_07552_b200 import binding as gx
     for wl in (gen.make_config(0), gen.make_config(2, n_envs=12)):
         o = oracle_mod.render(wl)
         ref = oracle_mod.pack_obs(o["rgb"], o["depth"], 0.1, 10.0)
-        for opts in ({}, {"path": 1}, {"pool_slots": 64}, {"occlusion": 2}):
+        for opts in ({}, {"big_px": 1}, {"arena_slots": 1}, {"hiz": 0}):
             sc = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, 0)
             try:
                 for k, v in opts.items():
@@ -333,35 +338,69 @@ def test_packed_observation(oracle_mod):
                 gx.gx_destroy(sc)
 
 
-@pytest.mark.parametrize("W,H", [(128, 96), (96, 128), (64, 128), (80, 48)])
+@pytest.mark.parametrize("W,H", [(128, 96), (96, 128), (64, 128), (80, 48), (224, 224), (256, 144), (256, 256)])
 def test_other_frame_shapes_room_scene(oracle_mod, W, H):
-    """Frame shapes other than the configs': the room scene of configs[1] rendered at W x H (fx = fy * H / W), which
-    exercises one, two and four raster CTAs per SM, bands that are and are not possible (H / 2 a multiple of 32 or
-    not), with and without the occluder scheme."""
-    wl = gen.make_config(1, n_envs=6)
+    """NEXT-3: frame shapes other than the configs' -- the room scene of configs[1] rendered at W x H (fx = fy * H / W),
+    up to the 256x256 limit (Table 1 of the paper compares simulators at 128 to 256 pixels): more tiles
+    per frame, more triangles on the block path and on the int64 path."""
+    wl = gen.make_config(1, n_envs=6 if W * H <= 128 * 128 else 3)
     wl.width, wl.height = W, H
     wl.fy = 1.0
     wl.fx = H / W
     o = oracle_mod.render(wl)
-    for opts in ({}, {"occlusion": 2}, {"occlusion": 2, "bands": 1}, {"path": 1}):
+    for opts in ({}, {"big_px": 6}, {"hiz": 0, "arena_slots": 1}):
         g = render_gpu(wl, options=opts)
         rep = compare(o, g)
         assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, (opts, rep)
 
 
+def test_second_camera_is_a_second_slot(oracle_mod):
+    """NEXT-3, several cameras per environment (the third-person debug view of PAPER.md:465-467): a second camera
+    is a second environment slot with the same scene id and instance transforms and its own camera pose; the call
+    renders both.  Checked against the oracle rendering the same doubled batch."""
+    wl = gen.make_config(1, n_envs=4)
+    other = gen.make_config(1, env_ids=[100, 101, 102, 103])     # poses of other environments of the same scene
+    two = wl.subset(np.repeat(np.arange(4), 2))
+    two.cam_pose = two.cam_pose.copy()
+    two.cam_pose[1::2] = other.cam_pose                       # odd slots: the second camera, same instances
+    o = oracle_mod.render(two)
+    g = render_gpu(two)
+    rep = compare(o, g)
+    assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, rep
+    assert not np.array_equal(g["depth"][0], g["depth"][1])
+
+
+def test_out_of_range_mesh_ids_are_empty_slots():
+    """include/gx.h: an out-of-range env_scene / inst_mesh value is a precondition violation; the library treats
+    the slot as empty and counts it instead of reading out of bounds."""
+    wl = gen.make_config(0)
+    ok = render_gpu(wl, stats=True)
+    assert ok["stats"]["bad_ids"] == 0
+    bad = wl.subset(np.arange(wl.N))
+    bad.inst_mesh = bad.inst_mesh.copy()
+    bad.inst_mesh[0, 0] = 7          # only mesh 0 exists
+    bad.env_scene = bad.env_scene.copy()
+    bad.env_scene[3] = 5
+    g = render_gpu(bad, stats=True)
+    assert g["stats"]["bad_ids"] == 2
+    assert np.all(g["id"][3] == BG)                       # no scene: background
+    for k in ("rgb", "depth", "id"):
+        assert np.array_equal(g[k][1:3], ok[k][1:3])
+
+
 def test_handle_reuse_varying_batches_and_host_subbatches(oracle_mod):
-    """One handle, calls of different sizes and options in a row (the record pool and its history-based sizing,
-    the scratch buffers and the frame keys are reused and regrown), and the host entry point with a batch that is
-    not a multiple of its 512-environment sub-batches: every call must match the oracle."""
+    """One handle, calls of different sizes and options in a row (the arena and its history-based sizing and the
+    scratch buffers are reused and regrown), and the host entry point with a batch that is not a multiple of its
+    sub-batches: every call must match the oracle."""
     import torch
     from paper_2306_07552_b200 import binding as gx
     wl = gen.make_config(2, n_envs=40)
     o = oracle_mod.render(wl)
     sc = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, 0)
     try:
-        for sel, opts in ((np.arange(40), {}), (np.arange(7), {"occlusion": 2}), (np.arange(5, 38), {"occlusion": 3}),
-                          (np.arange(40), {"occlusion": 2, "pool_slots": 4096}), (np.arange(1), {"occlusion": 0, "pool_slots": 0}),
-                          (np.arange(40), {"occlusion": 1})):
+        for sel, opts in ((np.arange(40), {}), (np.arange(7), {"big_px": 3}), (np.arange(5, 38), {"hiz": 0}),
+                          (np.arange(40), {"arena_slots": 100000, "hiz": 1, "big_px": 16}), (np.arange(1), {"arena_slots": 0}),
+                          (np.arange(40), {"subcull": 0})):
             sub = wl.subset(sel)
             g = render_gpu(sub, scene=sc, options=opts)
             rep = compare({k: v[sel] for k, v in o.items()}, g)
@@ -369,7 +408,7 @@ def test_handle_reuse_varying_batches_and_host_subbatches(oracle_mod):
             torch.cuda.synchronize()
     finally:
         gx.gx_destroy(sc)
-    # host entry point: 1100 environments = sub-batches of 512, 512 and 76 (the 40 environments repeated)
+    # host entry point: 1100 environments (the 40 environments repeated), uneven last sub-batch
     rep_idx = np.arange(1100) % 40
     big = wl.subset(rep_idx)
     g = render_gpu(big, host_api=True)
