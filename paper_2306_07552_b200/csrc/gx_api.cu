@@ -83,6 +83,8 @@ struct GxScene {
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
     // options (gx_set_option)
     int opt_cull = 1, opt_subcull = 1, opt_stats = 0, opt_hiz = 1, opt_big_px = gx::TILE;
+    int opt_occlusion = -1;             // occluder scheme: 1 on, 0 off, -1 automatic (on for frames of at least 8192 pixels)
+    int opt_occl_area = 64;             // pixels per triangle of a sub-cluster's screen box that make it an occluder
     int64_t opt_pool_bytes = 0;         // arena budget; 0 = 4 GB
     int64_t opt_arena_slots = 0;        // force the arena size in record slots (tests: several waves); 0 = automatic
     // scratch owned by the handle: grows on demand, never inside a steady-state call
@@ -361,6 +363,16 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
         if (value) { sc->t_used = 0; sc->t_calls = 0; sc->t_full = false; }
         return GX_OK;
     }
+    if (!strcmp(name, "occlusion")) {
+        if (value < -1 || value > 1) return fail(GX_ERR_INVALID_ARG, "occlusion must be -1 (automatic), 0 or 1");
+        sc->opt_occlusion = (int)value;
+        return GX_OK;
+    }
+    if (!strcmp(name, "occl_area")) {
+        if (value < 0 || value > (1 << 20)) return fail(GX_ERR_INVALID_ARG, "occl_area out of range");
+        sc->opt_occl_area = (int)value;
+        return GX_OK;
+    }
     if (!strcmp(name, "big_px")) {
         if (value < 1 || value > gx::TILE) return fail(GX_ERR_INVALID_ARG, "big_px must be in [1, %d]", gx::TILE);
         sc->opt_big_px = (int)value;
@@ -418,7 +430,8 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
             }
     }
     static const char *names[GX_NSTAT] = {"clusters_tested", "clusters_drawn", "triangles_in", "triangles_raster",
-                                          "fragments", "records_occluded", "blocks_drawn", "tile_refs"};
+                                          "fragments", "records_occluded", "blocks_drawn", "tile_refs", "triangles_hidden",
+                                          "subclusters_hidden", "large_records", "large_draws"};
     for (int k = 0; k < GX_NSTAT; ++k)
         if (!strcmp(name, names[k])) {
             DeviceGuard guard(sc->device);
@@ -475,13 +488,15 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     PP.subcull = sc->opt_subcull;
     PP.big_px = sc->opt_big_px;
     PP.hiz = sc->opt_hiz;
+    PP.occl = sc->opt_hiz && (sc->opt_occlusion == 1 || (sc->opt_occlusion < 0 && P.W * P.H >= 8192)) ? 1 : 0;
+    PP.occl_area = (float)sc->opt_occl_area;
 
     // ---- arena: record slots shared by the environments of a wave ------------------------------------
     // An environment's segment is sized by U, the bound cull_kernel computes; the arena must hold the largest
     // possible U (four slots per triangle: everything clipped by the near plane into two pieces with float
     // colours), so that a wave always has room for at least one environment.  Beyond that it is sized from the
     // history of earlier calls (mean U per environment, read back asynchronously) or, on the first call, from a
-    // default of 32 Ki slots per environment, and capped by the budget; what does not fit goes to later waves.
+    // default of 48 Ki slots per environment, and capped by the budget; what does not fit goes to later waves.
     if (sc->ctl_pending && cudaEventQuery(sc->ev_ctl) == cudaSuccess) {
         const uint64_t sum = (uint64_t)sc->h_ctl[gx::C_SUM_U] | ((uint64_t)sc->h_ctl[gx::C_SUM_U + 1] << 32);
         sc->hist_u_per_env = std::max(sc->hist_u_per_env, (double)sum / (double)std::max(sc->ctl_N, 1));
@@ -493,7 +508,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     uint64_t want;
     if (sc->opt_arena_slots > 0) want = (uint64_t)sc->opt_arena_slots;
     else {
-        const double per_env = sc->hist_u_per_env > 0.0 ? 1.25 * sc->hist_u_per_env + 1024.0 : (double)std::min<uint64_t>(worst_env, 32768);
+        const double per_env = sc->hist_u_per_env > 0.0 ? 1.25 * sc->hist_u_per_env + 1024.0 : (double)std::min<uint64_t>(worst_env, 49152);
         want = std::min<uint64_t>((uint64_t)(per_env * N), (uint64_t)N * worst_env);
         want = std::min<uint64_t>(want, (uint64_t)budget / 88);
     }
@@ -508,30 +523,36 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     PP.recs = sc->arena_recs.p; PP.bbs = sc->arena_bbs.p; PP.refs = sc->arena_refs.p;
     PP.arena_slots = (uint32_t)(sc->opt_arena_slots > 0 ? std::max<uint64_t>((uint64_t)sc->opt_arena_slots, worst_env) : sc->arena_slots);
 
-    // ---- scratch words: ctl | n_items | U | rec_base | item_pre | cnt | env_idb | env_mv | tile_off | tasks | items
+    // ---- scratch words: ctl | U | rec_base | cnt | cntA | n_large | env_idb | env_mv | tile_off | tasks | hizt | hizb | items | keys
     const size_t n = (size_t)N, k1 = (size_t)K + 1, NK1 = (size_t)PP.T * gx::NBUCKET + 1;
     PP.item_stride = (int32_t)std::max<size_t>((size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches, 1);
-    size_t off = 32;
-    const size_t o_nitems = off; off += n;
+    size_t off = 64;
     const size_t o_U = off; off += n;
     const size_t o_base = off; off += n;
-    const size_t o_ipre = off; off += n + 1;
     const size_t o_cnt = off; off += 2 * n;
+    const size_t o_cntA = off; off += 2 * n;
+    const size_t o_nl = off; off += n;
     const size_t o_idb = off; off += n * k1;
     const size_t o_mv = off; off += n * k1 * 12;
     const size_t o_toff = off; off += n * NK1;
     const size_t o_tasks = off; off += (size_t)gx::NCLASS * n * (size_t)PP.T;
+    const size_t o_hizt = off; off += PP.occl ? n * (size_t)PP.T : 0;
+    const size_t o_hizb = off; off += PP.occl ? n * (size_t)PP.T * 8 : 0;
     off = (off + 3) & ~(size_t)3;
     const size_t o_items = off; off += 4 * n * (size_t)PP.item_stride;
+    const size_t o_keys = off; off += PP.occl ? n * (size_t)P.W * (size_t)P.H * 2 : 0;
     if ((rc = sc->scratch.reserve(off)) != GX_OK) return rc;
     uint32_t *sp = sc->scratch.p;
-    PP.ctl = sp; PP.n_items = sp + o_nitems; PP.U = sp + o_U; PP.rec_base = sp + o_base; PP.item_pre = sp + o_ipre;
-    PP.cnt = sp + o_cnt; PP.env_idb = sp + o_idb; PP.env_mv = reinterpret_cast<float *>(sp + o_mv);
-    PP.tile_off = sp + o_toff; PP.tasks = sp + o_tasks; PP.items = reinterpret_cast<uint4 *>(sp + o_items);
+    PP.ctl = sp; PP.U = sp + o_U; PP.rec_base = sp + o_base;
+    PP.cnt = sp + o_cnt; PP.cntA = sp + o_cntA; PP.n_large = sp + o_nl; PP.env_idb = sp + o_idb;
+    PP.env_mv = reinterpret_cast<float *>(sp + o_mv);
+    PP.tile_off = sp + o_toff; PP.tasks = sp + o_tasks; PP.hizt = sp + o_hizt; PP.hizb = sp + o_hizb;
+    PP.items = reinterpret_cast<uint4 *>(sp + o_items);
+    PP.keys = reinterpret_cast<unsigned long long *>(sp + o_keys);
 
     sc->last_stream = stream;
     if (st) GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
-    GX_CUDA(cudaMemsetAsync(PP.ctl, 0, 32 * sizeof(uint32_t), stream));
+    GX_CUDA(cudaMemsetAsync(PP.ctl, 0, 64 * sizeof(uint32_t), stream));
     if ((rc = mark(sc, stream, 0)) != GX_OK) return rc;
 
     // K1: one CTA per environment: 4 warps for small scenes, 16 where an environment has thousands of sub-clusters
@@ -547,37 +568,45 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
         GX_CUDA(cudaGetLastError());
         if ((rc = mark(sc, stream, 1)) != GX_OK) return rc;
     }
-    // K2: persistent independent warps
-    {
-        constexpr int GW = 8;
-        auto gk = st ? gx::geom_kernel<GW, true> : gx::geom_kernel<GW, false>;
-        const size_t gsmem = (size_t)GW * gx::GEOM_WARP_SMEM;
-        int per_sm = 0;
-        if ((rc = plan_of(sc, (const void *)gk, GW * 32, gsmem, &per_sm)) != GX_OK) return rc;
-        gk<<<sc->num_sms * per_sm, GW * 32, gsmem, stream>>>(PP);
-        GX_CUDA(cudaGetLastError());
-        if ((rc = mark(sc, stream, 2)) != GX_OK) return rc;
-    }
-    // K3: one CTA per environment at a time
-    {
-        auto bk = st ? gx::bin_kernel<true> : gx::bin_kernel<false>;
-        const size_t bsmem = (size_t)2 * PP.T * gx::NBUCKET * 4;
-        int per_sm = 0;
-        if ((rc = plan_of(sc, (const void *)bk, 256, bsmem, &per_sm)) != GX_OK) return rc;
-        bk<<<std::min(N, sc->num_sms * per_sm), 256, bsmem, stream>>>(PP);
-        GX_CUDA(cudaGetLastError());
-        if ((rc = mark(sc, stream, 3)) != GX_OK) return rc;
-    }
-    // K4 + K5: persistent independent warps, one tile each at a time
-    {
-        constexpr int RW = 8;
-        auto rk = st ? gx::raster_kernel<RW, true> : gx::raster_kernel<RW, false>;
-        const size_t rsmem = (size_t)RW * gx::RAST_WARP_SMEM;
-        int per_sm = 0;
-        if ((rc = plan_of(sc, (const void *)rk, RW * 32, rsmem, &per_sm)) != GX_OK) return rc;
-        rk<<<sc->num_sms * per_sm, RW * 32, rsmem, stream>>>(PP);
-        GX_CUDA(cudaGetLastError());
-        if ((rc = mark(sc, stream, 4)) != GX_OK) return rc;
+    int launches = 1;
+    for (int phase = PP.occl ? 1 : 0; phase <= (PP.occl ? 2 : 0); ++phase) {
+        // K2: persistent independent warps
+        {
+            constexpr int GW = 8;
+            const bool hz = phase == 2 && PP.hiz;
+            auto gk = hz ? (st ? gx::geom_kernel<GW, true, true> : gx::geom_kernel<GW, false, true>)
+                         : (st ? gx::geom_kernel<GW, true, false> : gx::geom_kernel<GW, false, false>);
+            const size_t gsmem = (size_t)GW * gx::GEOM_WARP_SMEM;
+            int per_sm = 0;
+            if ((rc = plan_of(sc, (const void *)gk, GW * 32, gsmem, &per_sm)) != GX_OK) return rc;
+            gk<<<sc->num_sms * per_sm, GW * 32, gsmem, stream>>>(PP, phase);
+            GX_CUDA(cudaGetLastError());
+            if ((rc = mark(sc, stream, 2)) != GX_OK) return rc;
+        }
+        // K3: one CTA per environment at a time
+        {
+            auto bk = st ? gx::bin_kernel<true> : gx::bin_kernel<false>;
+            const size_t bsmem = (size_t)2 * PP.T * gx::NBUCKET * 4;
+            int per_sm = 0;
+            if ((rc = plan_of(sc, (const void *)bk, 256, bsmem, &per_sm)) != GX_OK) return rc;
+            bk<<<std::min(N, sc->num_sms * per_sm), 256, bsmem, stream>>>(PP, phase);
+            GX_CUDA(cudaGetLastError());
+            if ((rc = mark(sc, stream, 3)) != GX_OK) return rc;
+        }
+        // K4 + K5: persistent independent warps, one tile each at a time
+        {
+            constexpr int RW = 8;
+            auto rk = phase == 0 ? (st ? gx::raster_kernel<RW, true, 0> : gx::raster_kernel<RW, false, 0>)
+                    : phase == 1 ? (st ? gx::raster_kernel<RW, true, 1> : gx::raster_kernel<RW, false, 1>)
+                                 : (st ? gx::raster_kernel<RW, true, 2> : gx::raster_kernel<RW, false, 2>);
+            const size_t rsmem = (size_t)RW * gx::RAST_WARP_SMEM;
+            int per_sm = 0;
+            if ((rc = plan_of(sc, (const void *)rk, RW * 32, rsmem, &per_sm)) != GX_OK) return rc;
+            rk<<<sc->num_sms * per_sm, RW * 32, rsmem, stream>>>(PP);
+            GX_CUDA(cudaGetLastError());
+            if ((rc = mark(sc, stream, 4)) != GX_OK) return rc;
+        }
+        launches += 3;
     }
     // the tail: later waves, on the device (exits at once when the first wave took every environment)
     {
@@ -595,7 +624,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
         sc->ctl_pending = true;
         sc->ctl_N = N;
     }
-    sc->last_launches = 5;
+    sc->last_launches = launches + 1;
     if (sc->opt_timing && !sc->t_full) ++sc->t_calls;
     return GX_OK;
 }

@@ -260,6 +260,41 @@ __device__ __forceinline__ bool box_in_frustum(const CamBox &b, float fx, float 
     return true;
 }
 
+// Occluder class of a sub-cluster (32 triangles) in the occluder scheme: big on screen (screen box of at least
+// occl_area pixels per triangle) or reaching the near plane -- many pixels for little geometry.  Any
+// classification gives the same image; this one only decides what can be culled.
+__device__ __forceinline__ bool sub_is_occluder(const CamBox &b, float fx, float fy, int W, int H, float znear, float occl_area) {
+    if (!(b.wmin >= znear)) return true;
+    const float iw = 1.0f / b.wmin;   // the nearest depth gives the largest possible screen box
+    const float wpx = fminf(2.0f * b.ex * fx * iw * 0.5f * (float)W, (float)W);
+    const float hpx = fminf(2.0f * b.ey * fy * iw * 0.5f * (float)H, (float)H);
+    return wpx * hpx >= occl_area * 32.0f;
+}
+
+// Occlusion test of a sub-cluster's camera-space box against the per-tile hi-Z values of the occluder phase
+// (hizt: bits of the largest stored depth per 16x16-pixel tile, 0xFFFFFFFF where background shows): true only if
+// every fragment the box can produce is strictly behind what is already drawn at every pixel it can touch, so
+// that it can never win N9 and the image stays bit-identical (N10).
+template <bool COOP>
+__device__ __forceinline__ bool box_occluded(const CamBox &b, const uint32_t *hizt, int tiles_x, float fx, float fy, int W, int H,
+                                             float znear) {
+    if (!(b.wmin >= znear)) return false;   // reaches the near plane: no screen bound
+    const float xl = b.cx - b.ex, xh = b.cx + b.ex, yl = b.cy - b.ey, yh = b.cy + b.ey;
+    const float iw0 = 1.0f / b.wmin, iw1 = 1.0f / b.wmax;
+    const float nxl = fx * xl * (xl >= 0.0f ? iw1 : iw0), nxh = fx * xh * (xh >= 0.0f ? iw0 : iw1);
+    const float nyl = fy * yl * (yl >= 0.0f ? iw1 : iw0), nyh = fy * yh * (yh >= 0.0f ? iw0 : iw1);
+    // pixel range, padded by one pixel for the 1/256 snap and the float error of the box arithmetic
+    const float fW = (float)W, fH = (float)H;
+    const int pxl = (int)fminf(fmaxf(floorf((nxl * 0.5f + 0.5f) * fW) - 1.0f, 0.0f), fW - 1.0f);
+    const int pxh = (int)fminf(fmaxf(floorf((nxh * 0.5f + 0.5f) * fW) + 1.0f, 0.0f), fW - 1.0f);
+    const int pyl = (int)fminf(fmaxf(floorf((-nyh * 0.5f + 0.5f) * fH) - 1.0f, 0.0f), fH - 1.0f);
+    const int pyh = (int)fminf(fmaxf(floorf((-nyl * 0.5f + 0.5f) * fH) + 1.0f, 0.0f), fH - 1.0f);
+    uint32_t zb = 0;
+    for (int ty = pyl >> 4; ty <= (pyh >> 4); ++ty)
+        for (int tx = pxl >> 4; tx <= (pxh >> 4); ++tx) zb = max(zb, COOP ? __ldcg(&hizt[ty * tiles_x + tx]) : __ldg(&hizt[ty * tiles_x + tx]));
+    return b.wmin * (1.0f - 1e-4f) > __uint_as_float(zb);   // (background: NaN, the comparison is false)
+}
+
 __device__ __forceinline__ bool cluster_visible(const GxClusterDev &c, const float *M, float fx, float fy, float znear,
                                                 float zfar) {
     return box_in_frustum(cluster_box(c, M), fx, fy, znear, zfar);

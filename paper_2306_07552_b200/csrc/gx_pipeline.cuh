@@ -36,6 +36,7 @@ namespace cg = cooperative_groups;
 
 constexpr int TILE = 16;            // tile edge, pixels (BASELINE.json north_star (3))
 constexpr int NBUCKET = 8;          // depth buckets per tile (front-to-back order of a tile's list)
+constexpr int NLB = 32;             // depth buckets of an environment's list of large records
 constexpr int NCLASS = 8;           // cost classes of the raster tasks
 constexpr int NARROW_EXT = 30000;   // sub-pixel extent below which every edge value near the box fits int32:
                                     // 2 * 30000 * (30000 + 16 * 256 + 256) < 2^31
@@ -57,23 +58,25 @@ constexpr uint32_t BB_SKIP = 0xFFFFFFFFu;   // box word of a colour slot: not a 
 enum { F_BIAS = 7, F_FLOATCOL = 8, F_WIDE = 16 };
 
 // control words (device): cursors and the current wave
-enum { C_WAVE_E0 = 0, C_WAVE_E1, C_GEOM_CUR, C_BIN_CUR, C_RAST_CUR, C_CULL_DONE, C_WAVE_ITEMS, C_WAVES, C_SUM_U /* 64-bit: two words */,
-       C_MAX_U = C_SUM_U + 2, C_BAD_ENVS, C_TASK_CNT = 16, C_NCTL = C_TASK_CNT + NCLASS };
+// (cursors and task counts exist once per phase of the occluder scheme: index 0 = single pass or occluder phase, 1 = second phase)
+enum { C_WAVE_E0 = 0, C_WAVE_E1, C_GEOM_CUR, C_BIN_CUR = C_GEOM_CUR + 2, C_RAST_CUR = C_BIN_CUR + 2, C_CULL_DONE = C_RAST_CUR + 2,
+       C_N_ITEMS, C_SUM_U /* 64-bit: two words, even index */, C_WAVES = C_SUM_U + 2, C_MAX_U, C_BAD_ENVS, C_TASK_CNT = 16,
+       C_NCTL = C_TASK_CNT + 2 * NCLASS };
+static_assert(C_SUM_U % 2 == 0 && C_BAD_ENVS < C_TASK_CNT, "control word layout");
 
 struct PipeParams {
     GxParams g;
     // environment table and K1 output
     float *env_mv;           // [N][K+1][12] model-view per slot
     uint32_t *env_idb;       // [N][K+1] first triangle id per slot
-    uint4 *items;            // [N][item_stride]: (slot << 24 | batch, mask of the 32-triangle runs to draw,
-                             //                    first | last << 16 vertex those runs reference, unused)
-    uint32_t *n_items;       // [N]
+    uint4 *items;            // [ctl[C_N_ITEMS]] one flat list for the call: (slot << 24 | batch, runs of 32 triangles
+                             //   to draw: occluder class | the rest << 8, environment, unused)
     uint32_t *U;             // [N] upper bound of the record slots of the environment
-    int32_t item_stride;
+    int32_t item_stride;     // capacity of the item list = N * item_stride
     // wave allocation
     uint32_t *rec_base;      // [N] first arena slot of the environment's segment
-    uint32_t *item_pre;      // [N+1] exclusive prefix of n_items over the wave (indexed by environment)
     uint32_t *cnt;           // [N][2] slots used from the bottom (small) and from the top (large) of the segment
+    uint32_t *cntA;          // [N][2] the same after the occluder phase (what the second phase has to bin and draw)
     uint32_t *ctl;           // [C_NCTL]
     // arena
     uint4 *recs;             // [arena_slots][4]
@@ -82,12 +85,19 @@ struct PipeParams {
     uint32_t arena_slots;
     // K3 output
     uint32_t *tile_off;      // [N][T * NBUCKET + 1] exclusive offsets into the environment's refs
+    uint32_t *n_large;       // [N] large entries of the phase that was binned last
     uint32_t *tasks;         // [NCLASS][N * T] raster tasks (env * T + tile) per cost class
     int32_t tiles_x, tiles_y, T;
     float bucket_off, bucket_scale;   // bucket = clamp(int((bucket_off - log2(qmax)) * bucket_scale), 0, NBUCKET - 1)
     int32_t subcull;         // test every 32-triangle sub-cluster of a visible cluster against the frustum
     int32_t big_px;          // records wider or higher than this many pixels take the block path (1..TILE)
     int32_t hiz;             // 0 = no hi-Z rejection (verification)
+    // occluder scheme (two phases of geometry / bin / raster per wave)
+    int32_t occl;            // 1 = on
+    float occl_area;         // a sub-cluster is an occluder if its screen box has this many pixels per triangle
+    unsigned long long *keys;   // [N][T][256] tile keys between the two raster phases
+    uint32_t *hizb;          // [N][H/4][W/8] bits of the largest depth per 8x4-pixel block after the occluder phase
+    uint32_t *hizt;          // [N][T] the same per tile
 };
 
 template <bool COOP, typename T>
@@ -187,30 +197,30 @@ __device__ __forceinline__ void env_setup(const PipeParams &PP, int env, const E
 
 // ------------------------------------------------------------------------------------------------
 // wave allocation, by one whole CTA: starting at environment e_first, as many consecutive environments as fit
-// the arena get their segment (exclusive scan of U) and their range of the wave's flat item index space; the
-// wave's cursors and per-environment counters are reset.  ctl[C_WAVE_E0 .. C_WAVE_E1) is the wave.
+// the arena get their segment (exclusive scan of U); the wave's cursors and per-environment counters are
+// reset.  ctl[C_WAVE_E0 .. C_WAVE_E1) is the wave.
 // ------------------------------------------------------------------------------------------------
 __device__ void alloc_wave(const PipeParams &PP, uint32_t e_first) {
-    __shared__ uint32_t s_wu[32], s_wi[32];
-    __shared__ uint32_t s_run_u, s_run_i, s_end, s_fin_i;
+    __shared__ uint32_t s_wu[32];
+    __shared__ uint32_t s_run_u, s_end;
     const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t N = (uint32_t)PP.g.N;
-    if (tid == 0) { s_run_u = 0; s_run_i = 0; s_end = N; s_fin_i = 0; }
+    if (tid == 0) { s_run_u = 0; s_end = N; }
     __syncthreads();
     for (uint32_t c0 = e_first; c0 < N; c0 += NT) {
         const uint32_t e = c0 + tid;
-        const uint32_t u = e < N ? __ldcg(&PP.U[e]) : 0u, ni = e < N ? __ldcg(&PP.n_items[e]) : 0u;
-        uint32_t iu = u, ii = ni;
+        const uint32_t u = e < N ? __ldcg(&PP.U[e]) : 0u;
+        uint32_t iu = u;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, iu, d), b = __shfl_up_sync(0xFFFFFFFFu, ii, d);
-            if (lane >= d) { iu += a; ii += b; }
+            const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, iu, d);
+            if (lane >= d) iu += a;
         }
-        if (lane == 31) { s_wu[warp] = iu; s_wi[warp] = ii; }
+        if (lane == 31) s_wu[warp] = iu;
         __syncthreads();
-        uint32_t bu = s_run_u, bi = s_run_i;
-        for (int w = 0; w < warp; ++w) { bu += s_wu[w]; bi += s_wi[w]; }
-        const uint32_t ex_u = bu + iu - u, ex_i = bi + ii - ni;
+        uint32_t bu = s_run_u;
+        for (int w = 0; w < warp; ++w) bu += s_wu[w];
+        const uint32_t ex_u = bu + iu - u;
         // (the first environment of a wave always fits: the host sizes the arena for the largest possible U,
         // and cull_kernel empties an environment that would still exceed it)
         const bool fits = (unsigned long long)ex_u + u <= (unsigned long long)PP.arena_slots || e == e_first;
@@ -219,27 +229,21 @@ __device__ void alloc_wave(const PipeParams &PP, uint32_t e_first) {
         const uint32_t end = s_end;
         if (e < end) {
             PP.rec_base[e] = ex_u;
-            PP.item_pre[e] = ex_i;
             PP.cnt[2 * e] = 0;
             PP.cnt[2 * e + 1] = 0;
+            PP.cntA[2 * e] = 0;
+            PP.cntA[2 * e + 1] = 0;
         }
-        if (e == end) s_fin_i = ex_i;
-        if (tid == NT - 1) { s_run_u = ex_u + u; s_run_i = ex_i + ni; }
+        if (tid == NT - 1) s_run_u = ex_u + u;
         __syncthreads();
         if (end < N) break;   // (uniform) the wave ends inside this chunk
     }
     if (tid == 0) {
-        const uint32_t end = s_end;
-        const uint32_t n_it = end < N ? s_fin_i : s_run_i;
-        PP.item_pre[end] = n_it;
         PP.ctl[C_WAVE_E0] = e_first;
-        PP.ctl[C_WAVE_E1] = end;
-        PP.ctl[C_WAVE_ITEMS] = n_it;
-        PP.ctl[C_GEOM_CUR] = 0;
-        PP.ctl[C_BIN_CUR] = 0;
-        PP.ctl[C_RAST_CUR] = 0;
+        PP.ctl[C_WAVE_E1] = s_end;
+        for (int c = 0; c < 2; ++c) { PP.ctl[C_GEOM_CUR + c] = 0; PP.ctl[C_BIN_CUR + c] = 0; PP.ctl[C_RAST_CUR + c] = 0; }
         PP.ctl[C_WAVES] += 1;
-        for (int c = 0; c < NCLASS; ++c) PP.ctl[C_TASK_CNT + c] = 0;
+        for (int c = 0; c < 2 * NCLASS; ++c) PP.ctl[C_TASK_CNT + c] = 0;
     }
 }
 
@@ -285,10 +289,9 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
     unsigned st_tested = 0, st_drawn = 0;
     constexpr int CCH = 256;                                   // clusters per round
     constexpr int VB_CAP = CCH * GX_MAX_BATCH_PER_CLUSTER;     // batches of the visible clusters of a round
-    __shared__ uint32_t s_vb[VB_CAP], s_vm[VB_CAP], s_vlo[VB_CAP], s_vhi[VB_CAP];
-    __shared__ unsigned s_nvb, s_nitems, s_U;
-    if (tid == 0) { s_nitems = 0; s_U = 0; }
-    uint4 *env_items = PP.items + (size_t)env * (size_t)PP.item_stride;
+    __shared__ uint32_t s_vb[VB_CAP], s_vm[VB_CAP];
+    __shared__ unsigned s_nvb, s_U;
+    if (tid == 0) s_U = 0;
     for (uint32_t c0 = 0; c0 < n_cl; c0 += CCH) {
         if (tid == 0) s_nvb = 0;
         __syncthreads();
@@ -305,15 +308,16 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
                 const uint32_t at = atomicAdd(&s_nvb, nb);
                 for (uint32_t k = 0; k < nb; ++k) {
                     s_vb[at + k] = (s << 24) | (c.batch_off + k);
-                    s_vm[at + k] = 0u; s_vlo[at + k] = 0xFFFFu; s_vhi[at + k] = 0u;
+                    s_vm[at + k] = 0u;
                 }
             }
         }
         __syncthreads();
         const unsigned nvb = s_nvb;
-        // step 2 (K1b), one thread per run of 32 triangles of a listed batch: its AABB against the frustum.  A
-        // surviving run adds its triangle count to U -- four slots per triangle if its box reaches the near
-        // plane (a clipped triangle leaves as up to two pieces of two slots each), one otherwise.
+        // step 2 (K1b), one thread per run of 32 triangles of a listed batch: its AABB against the frustum, and
+        // its class in the occluder scheme (bit r = occluder, bit 8 + r = the rest).  A surviving run adds its
+        // triangle count to U -- four slots per triangle if its box reaches the near plane (a clipped triangle
+        // leaves as up to two pieces of two slots each), one otherwise.
         for (unsigned idx = tid; idx < nvb * GX_SUBS_PER_BATCH; idx += NT) {
             const unsigned v = idx / GX_SUBS_PER_BATCH, r = idx % GX_SUBS_PER_BATCH;
             const uint32_t batch = s_vb[v] & 0xFFFFFFu, s = s_vb[v] >> 24;
@@ -323,33 +327,31 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
             const CamBox bx = cluster_box(sb, es.MV + s * 12);
             const bool sv = !(P.cull && PP.subcull) || box_in_frustum(bx, P.fx, P.fy, P.znear, P.zfar);
             if (sv) {
-                atomicOr(&s_vm[v], 1u << r);
-                atomicMin(&s_vlo[v], sb.batch_off);   // (fields reused: first and last vertex the run references)
-                atomicMax(&s_vhi[v], sb.nbatch);
+                const bool occluder = !PP.occl || sub_is_occluder(bx, P.fx, P.fy, P.W, P.H, P.znear, PP.occl_area);
+                atomicOr(&s_vm[v], (occluder ? 1u : 256u) << r);
                 const unsigned n = (unsigned)min(32, nt - (int)r * 32);
                 atomicAdd(&s_U, (bx.wmin >= P.znear) ? n : 4u * n);
             }
         }
         __syncthreads();
-        // step 3: one work item per batch that has a run left
+        // step 3: one work item per batch that has a run left, appended to the call's list
         for (unsigned v0 = warp * 32; v0 < nvb; v0 += NT) {
             const unsigned v = v0 + lane;
             const bool has = v < nvb && s_vm[v] != 0u;
             const unsigned m = __ballot_sync(0xFFFFFFFFu, has);
             uint32_t base = 0;
-            if (lane == 0 && m) base = atomicAdd(&s_nitems, (unsigned)__popc(m));
+            if (lane == 0 && m) base = atomicAdd(&PP.ctl[C_N_ITEMS], (unsigned)__popc(m));
             base = __shfl_sync(0xFFFFFFFFu, base, 0);
-            if (has) env_items[base + __popc(m & ((1u << lane) - 1u))] = make_uint4(s_vb[v], s_vm[v], s_vlo[v] | (s_vhi[v] << 16), 0u);
+            if (has) PP.items[base + __popc(m & ((1u << lane) - 1u))] = make_uint4(s_vb[v], s_vm[v], (uint32_t)env, 0u);
         }
         __syncthreads();
     }
     __syncthreads();
     __shared__ bool s_last;
     if (tid == 0) {
-        uint32_t u = s_U, ni = s_nitems;
-        if (u > PP.arena_slots) { u = 0; ni = 0; atomicAdd(&PP.ctl[C_BAD_ENVS], 1u); }   // cannot happen: see alloc_wave
-        PP.n_items[env] = ni;
-        PP.U[env] = u;
+        uint32_t u = s_U;
+        if (u > PP.arena_slots) { u = 0; atomicAdd(&PP.ctl[C_BAD_ENVS], 1u); }   // cannot happen: see alloc_wave (the geometry
+        PP.U[env] = u;                                                           // stage skips items of an environment with U = 0)
         atomicAdd(reinterpret_cast<unsigned long long *>(&PP.ctl[C_SUM_U]), (unsigned long long)u);
         atomicMax(&PP.ctl[C_MAX_U], u);
         __threadfence();
@@ -450,10 +452,13 @@ __device__ __forceinline__ void emit_records(const PipeParams &PP, int env, uint
 
 // K2 for one batch, by one warp.  sub_mask: bit r set = pass r of the triangle loop (32 consecutive triangles,
 // one sub-cluster) is drawn; [v_lo, v_hi]: the vertices those passes reference (K1b, cull_kernel).
-template <bool STATS>
+// hzb: in the second phase of the occluder scheme, the environment's per-block hi-Z values of the first phase: a
+// triangle whose nearest vertex is behind every block its pixel box touches is dropped before set-up.
+template <bool COOP, bool STATS>
 __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj, uint32_t batch, const float *MV,
                                            uint32_t slot_id_base, const GeomWarpSmem &ws, int env, uint32_t base, uint32_t U,
-                                           int lane, unsigned sub_mask, int v_lo, int v_hi, unsigned &n_in, unsigned &n_tri) {
+                                           int lane, unsigned sub_mask, int v_lo, int v_hi, const uint32_t *hzb,
+                                           unsigned &n_in, unsigned &n_tri, unsigned &n_hid) {
     const GxParams &P = PP.g;
     const unsigned FULL = 0xFFFFFFFFu;
     const GxBatchDev b = P.batches[batch];
@@ -500,6 +505,15 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                 if (i0 <= i1 && j0 <= j1) {
                     ok = max(Xmax - Xmin, Ymax - Ymin) < NARROW_EXT;
                     slow = !ok;
+                    if (hzb && i1 - i0 < 32 && j1 - j0 < 16) {   // (at most 5 x 5 blocks)
+                        uint32_t zb = 0;
+                        const int bw = P.W >> 3;
+                        for (int by = j0 >> 2; by <= (j1 >> 2); ++by)
+                            for (int bx = i0 >> 3; bx <= (i1 >> 3); ++bx) zb = max(zb, ldi<COOP>(&hzb[by * bw + bx]));
+                        const float qmax = fmaxf(ws.vQ[ix.x], fmaxf(ws.vQ[ix.y], ws.vQ[ix.z]));
+                        // every depth of the triangle is >= 1/qmax (N7, up to a few ulp): hidden iff behind with margin
+                        if (qmax * __uint_as_float(zb) < 1.0f - 1e-5f) { ok = false; slow = false; if (STATS) ++n_hid; }
+                    }
                 }
             } else if (nout < 3) {
                 slow = true;
@@ -628,11 +642,25 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
     __syncwarp();
 }
 
-// The geometry stage: every warp draws items of the wave's flat item index space until it is exhausted.
+// second phase of the occluder scheme: is the box of a run of 32 triangles behind the hi-Z tiles of the first phase?
+// (a function of its own: only 8 lanes of a warp get here, and its registers stay out of the triangle loops)
+template <bool COOP>
+__device__ __forceinline__ bool sub_hidden(const PipeParams &PP, const GxClusterDev &sb, const float *MV, uint32_t e) {
+    float M[12];
+#pragma unroll
+    for (int k = 0; k < 12; ++k) M[k] = ldi<COOP>(&MV[k]);
+    return box_occluded<COOP>(cluster_box(sb, M), PP.hizt + (size_t)e * (size_t)PP.T, PP.tiles_x, PP.g.fx, PP.g.fy, PP.g.W, PP.g.H,
+                              PP.g.znear);
+}
+
+// The geometry stage: every warp draws items of the call's list until it is exhausted; items of environments
+// outside the current wave are skipped.  phase: 0 = every run of the item, 1 = the occluder runs, 2 = the other
+// runs, after a hi-Z test of each run's box against the tiles of the occluder phase.
 // No CTA-level synchronisation.  warp_smem: GEOM_WARP_SMEM bytes of shared memory private to the warp.
-template <bool COOP, bool STATS>
-__device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *warp_smem) {
+template <bool COOP, bool STATS, bool HZ>
+__device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *warp_smem, int phase) {
     const GxParams &P = PP.g;
+    const unsigned FULL = 0xFFFFFFFFu;
     const int lane = threadIdx.x & 31;
     const int K = P.K;
     GeomWarpSmem ws;
@@ -644,42 +672,58 @@ __device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *
     pj.fx = P.fx; pj.fy = P.fy;
     pj.hw = 128.0f * (float)P.W; pj.hh = 128.0f * (float)P.H;
 
-    unsigned st_in = 0, st_tri = 0;
+    unsigned st_in = 0, st_tri = 0, st_hid = 0, st_subhid = 0;
     const uint32_t e0 = ldi<COOP>(&PP.ctl[C_WAVE_E0]), e1 = ldi<COOP>(&PP.ctl[C_WAVE_E1]);
-    const unsigned n_items = ldi<COOP>(&PP.ctl[C_WAVE_ITEMS]);
-    uint32_t e = e0;      // the environment of the previous item: items are drawn in increasing order
+    const unsigned n_items = ldi<COOP>(&PP.ctl[C_N_ITEMS]);
+    uint32_t *cursor = &PP.ctl[C_GEOM_CUR + (phase == 2 ? 1 : 0)];
+    const size_t hzb_stride = (size_t)(P.W >> 3) * (size_t)(P.H >> 2);
     unsigned next = 0;
-    if (lane == 0) next = atomicAdd(&PP.ctl[C_GEOM_CUR], 1u);
-    next = __shfl_sync(0xFFFFFFFFu, next, 0);
+    if (lane == 0) next = atomicAdd(cursor, 1u);
+    next = __shfl_sync(FULL, next, 0);
     while (next < n_items) {
         const unsigned g = next;
-        if (lane == 0) next = atomicAdd(&PP.ctl[C_GEOM_CUR], 1u);   // draw the following item while this one is processed
-        // environment of item g: largest e in [e0, e1) with item_pre[e] <= g (a few steps forward, else bisection)
-        {
-            int steps = 0;
-            while (steps < 4 && e + 1 < e1 && ldi<COOP>(&PP.item_pre[e + 1]) <= g) { ++e; ++steps; }
-            if (e + 1 < e1 && ldi<COOP>(&PP.item_pre[e + 1]) <= g) {
-                uint32_t lo = e + 1, hi = e1 - 1;
-                while (lo < hi) {
-                    const uint32_t mid = (lo + hi + 1) >> 1;
-                    if (ldi<COOP>(&PP.item_pre[mid]) <= g) lo = mid; else hi = mid - 1;
+        if (lane == 0) next = atomicAdd(cursor, 1u);   // draw the following item while this one is processed
+        const uint4 item = ldi<COOP>(&PP.items[g]);
+        const uint32_t e = item.z, s = item.x >> 24, batch = item.x & 0xFFFFFFu;
+        unsigned mask = phase == 0 ? ((item.y | (item.y >> 8)) & 255u) : (phase == 1 ? (item.y & 255u) : ((item.y >> 8) & 255u));
+        const uint32_t U = (e >= e0 && e < e1) ? ldi<COOP>(&PP.U[e]) : 0u;
+        if (mask && U) {
+            const float *MV = PP.env_mv + ((size_t)e * (size_t)(K + 1) + s) * 12;
+            // lanes 0..7: one run each -- its vertex range, and in the second phase the hi-Z test of its box
+            uint32_t vlo = 0xFFFFu, vhi = 0u;
+            bool keep = false;
+            if (lane < GX_SUBS_PER_BATCH && ((mask >> lane) & 1u)) {
+                const GxClusterDev sb = P.subs[(size_t)batch * GX_SUBS_PER_BATCH + lane];
+                keep = true;
+                if (HZ) {
+                    keep = !sub_hidden<COOP>(PP, sb, MV, e);
+                    if (STATS && !keep) ++st_subhid;
                 }
-                e = lo;
+                if (keep) { vlo = sb.batch_off; vhi = sb.nbatch; }   // (fields reused: first and last vertex the run references)
+            }
+            mask = __ballot_sync(FULL, keep);
+            if (mask) {
+                vlo = __reduce_min_sync(FULL, vlo);
+                vhi = __reduce_max_sync(FULL, vhi);
+                geom_batch<COOP, STATS>(PP, pj, batch, MV, ldi<COOP>(&PP.env_idb[(size_t)e * (size_t)(K + 1) + s]), ws, (int)e,
+                                        ldi<COOP>(&PP.rec_base[e]), U, lane, mask, (int)vlo, (int)vhi,
+                                        HZ ? PP.hizb + (size_t)e * hzb_stride : nullptr, st_in, st_tri, st_hid);
             }
         }
-        const uint4 item = ldi<COOP>(&PP.items[(size_t)e * (size_t)PP.item_stride + (g - ldi<COOP>(&PP.item_pre[e]))]);
-        const uint32_t s = item.x >> 24;
-        geom_batch<STATS>(PP, pj, item.x & 0xFFFFFFu, PP.env_mv + ((size_t)e * (size_t)(K + 1) + s) * 12,
-                          ldi<COOP>(&PP.env_idb[(size_t)e * (size_t)(K + 1) + s]), ws, (int)e, ldi<COOP>(&PP.rec_base[e]),
-                          ldi<COOP>(&PP.U[e]), lane, item.y, (int)(item.z & 0xFFFFu), (int)(item.z >> 16), st_in, st_tri);
-        next = __shfl_sync(0xFFFFFFFFu, next, 0);
+        next = __shfl_sync(FULL, next, 0);
     }
     if (STATS) {
 #pragma unroll
-        for (int d = 16; d; d >>= 1) st_tri += __shfl_xor_sync(0xFFFFFFFFu, st_tri, d);
+        for (int d = 16; d; d >>= 1) {
+            st_tri += __shfl_xor_sync(FULL, st_tri, d);
+            st_hid += __shfl_xor_sync(FULL, st_hid, d);
+            st_subhid += __shfl_xor_sync(FULL, st_subhid, d);
+        }
         if (lane == 0) {
             atomicAdd(&P.stats[GX_STAT_TRIS_IN], (unsigned long long)st_in);
             atomicAdd(&P.stats[GX_STAT_TRIS_RASTER], (unsigned long long)st_tri);
+            atomicAdd(&P.stats[GX_STAT_TRIS_HIDDEN], (unsigned long long)st_hid);
+            atomicAdd(&P.stats[GX_STAT_SUBS_HIDDEN], (unsigned long long)st_subhid);
         }
     }
 }
@@ -687,51 +731,121 @@ __device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *
 #ifndef GEOM_MINB
 #define GEOM_MINB 4
 #endif
-template <int WARPS, bool STATS>
-__global__ void __launch_bounds__(WARPS * 32, GEOM_MINB) geom_kernel(const PipeParams PP) {
+template <int WARPS, bool STATS, bool HZ>
+__global__ void __launch_bounds__(WARPS * 32, GEOM_MINB) geom_kernel(const PipeParams PP, int phase) {
     extern __shared__ __align__(16) unsigned char smem[];
-    geom_stage<false, STATS>(PP, smem + (size_t)(threadIdx.x >> 5) * GEOM_WARP_SMEM);
+    geom_stage<false, STATS, HZ>(PP, smem + (size_t)(threadIdx.x >> 5) * GEOM_WARP_SMEM, phase);
 }
 
 
 // ------------------------------------------------------------------------------------------------
-// K3: binning.  One CTA per environment at a time: count -> exclusive scan -> fill of the small records into
-// per-(tile, depth bucket) lists.  s_cnt, s_off: T * NBUCKET words of shared memory each.
+// K3: binning.  One CTA per environment at a time.
+//   small records: count -> exclusive scan -> fill into per-(tile, depth bucket) lists of record indices at the
+//     bottom of the environment's reference area (exact sizes, nothing can overflow);
+//   large records: one 16-byte entry each -- (slot | wide << 31, 64-bit mask of the cells of the frame some pixel
+//     of the triangle can fall in, bits of the largest q) -- sorted front to back by a counting sort over NLB
+//     depth buckets, at the top of the reference area (entry i at uint4 index U - 1 - i).  A cell is a tile
+//     (frames of at most 64 tiles) or 2x2 tiles; a cell is left out when some edge function is negative at all
+//     four corners of it, so a tile only looks at triangles that reach it.
+//   Also files every tile as a raster task under its cost class.
+// phase 0 / 1 bin everything emitted so far, phase 2 what the second geometry phase added (cntA .. cnt).
+// s_cnt, s_off: T * NBUCKET words of shared memory each.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ int depth_bucket(const PipeParams &PP, uint32_t qmax_bits) {
-    const float v = (PP.bucket_off - __log2f(__uint_as_float(qmax_bits))) * PP.bucket_scale;
-    return min(max((int)v, 0), NBUCKET - 1);
+__device__ __forceinline__ int depth_bucket(const PipeParams &PP, uint32_t qmax_bits, int nb, float scale) {
+    const float v = (PP.bucket_off - __log2f(__uint_as_float(qmax_bits))) * scale;
+    return min(max((int)v, 0), nb - 1);
+}
+
+// cells of the frame a large record can touch
+template <bool COOP>
+__device__ __forceinline__ unsigned long long large_mask(const PipeParams &PP, const uint4 *rp, uint32_t bb, bool &wide) {
+    const int cshift = PP.T > 64 ? 5 : 4;                       // log2 of the cell edge in pixels
+    const int cells_x = (PP.g.W + (1 << cshift) - 1) >> cshift;
+    const int i0 = (int)(bb & 255u), j0 = (int)((bb >> 8) & 255u);
+    const int i1 = i0 + (int)((bb >> 16) & 255u), j1 = j0 + (int)(bb >> 24);
+    const uint4 u0 = ldi<COOP>(rp), u1 = ldi<COOP>(rp + 1);
+    const uint32_t flags = ldi<COOP>(reinterpret_cast<const uint32_t *>(rp + 2) + 3) >> 24;
+    wide = (flags & F_WIDE) != 0;
+    unsigned long long m = 0;
+    const int ce = (1 << cshift) - 1;
+    if (!wide) {
+        int sx[3], sy[3], Eo[3];
+        const uint32_t E[3] = {u0.x, u0.y, u0.z}, D[3] = {u0.w, u1.x, u1.y};
+#pragma unroll
+        for (int e = 0; e < 3; ++e) {
+            const int dx = (int)D[e] >> 16, dy = (int)(short)(D[e] & 0xFFFFu);
+            sx[e] = -(dy << 8);
+            sy[e] = dx << 8;
+            // largest value over a cell whose first pixel is the box origin, top-left bias taken off
+            Eo[e] = (int)E[e] - (int)((flags >> e) & 1u) + max(ce * sx[e], 0) + max(ce * sy[e], 0);
+        }
+        for (int cy = j0 >> cshift; cy <= (j1 >> cshift); ++cy)
+            for (int cx = i0 >> cshift; cx <= (i1 >> cshift); ++cx) {
+                // the cell's corner pixels are at most one cell edge outside the box; for cells of 32 pixels the
+                // edge values could leave int32, so those are only tested against the box
+                bool in = true;
+                if (cshift == 4) {
+                    const int ox = (cx << 4) - i0, oy = (cy << 4) - j0;
+#pragma unroll
+                    for (int e = 0; e < 3; ++e) in = in && (Eo[e] + ox * sx[e] + oy * sy[e] >= 0);
+                }
+                if (in) m |= 1ull << (cy * cells_x + cx);
+            }
+    } else {
+        for (int cy = j0 >> cshift; cy <= (j1 >> cshift); ++cy)
+            for (int cx = i0 >> cshift; cx <= (i1 >> cshift); ++cx) m |= 1ull << (cy * cells_x + cx);
+    }
+    return m;
 }
 
 template <bool COOP, bool STATS>
-__device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt, uint32_t *s_off) {
-    __shared__ uint32_t s_env, s_wtot[32], s_ccnt[NCLASS], s_cbase[NCLASS];
+__device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt, uint32_t *s_off, int phase) {
+    __shared__ uint32_t s_env, s_wtot[32], s_ccnt[NCLASS], s_cbase[NCLASS], s_lcnt[NLB], s_loff[NLB];
     const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const int T = PP.T, NK = T * NBUCKET;
+    const int pi = phase == 2 ? 1 : 0;
     const uint32_t e0 = ldi<COOP>(&PP.ctl[C_WAVE_E0]), e1 = ldi<COOP>(&PP.ctl[C_WAVE_E1]);
+    const float sc_small = PP.bucket_scale, sc_large = PP.bucket_scale * (float)NLB / (float)NBUCKET;
     for (;;) {
         __syncthreads();
-        if (tid == 0) s_env = e0 + atomicAdd(&PP.ctl[C_BIN_CUR], 1u);
+        if (tid == 0) s_env = e0 + atomicAdd(&PP.ctl[C_BIN_CUR + pi], 1u);
         __syncthreads();
         const uint32_t env = s_env;
         if (env >= e1) break;
         const uint32_t ns = ldi<COOP>(&PP.cnt[2 * env]), nl = ldi<COOP>(&PP.cnt[2 * env + 1]);
+        const uint32_t s_lo = phase == 2 ? ldi<COOP>(&PP.cntA[2 * env]) : 0u, l_lo = phase == 2 ? ldi<COOP>(&PP.cntA[2 * env + 1]) : 0u;
+        const uint32_t U = ldi<COOP>(&PP.U[env]);
         const size_t base = ldi<COOP>(&PP.rec_base[env]);
         const uint2 *ebb = PP.bbs + base;
+        const uint4 *env_recs = PP.recs + base * 4;
         uint32_t *erefs = PP.refs + 4 * base;
+        uint4 *elarge = reinterpret_cast<uint4 *>(erefs);
         for (int k = tid; k < NK; k += NT) s_cnt[k] = 0;
         if (tid < NCLASS) s_ccnt[tid] = 0;
+        if (tid < NLB) s_lcnt[tid] = 0;
         __syncthreads();
-        // count
-        for (uint32_t s = tid; s < ns; s += NT) {
+        // count: small records per (tile, bucket), large records per bucket (slot U - 1 - k is the k-th large record)
+        for (uint32_t s = s_lo + tid; s < ns; s += NT) {
             const uint2 b = ldi<COOP>(&ebb[s]);
             if (b.x == BB_SKIP) continue;
             const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
             const int i1 = i0 + (int)((b.x >> 16) & 255u), j1 = j0 + (int)(b.x >> 24);
-            const int bk = depth_bucket(PP, b.y);
+            const int bk = depth_bucket(PP, b.y, NBUCKET, sc_small);
             for (int ty = j0 >> 4; ty <= (j1 >> 4); ++ty)
                 for (int tx = i0 >> 4; tx <= (i1 >> 4); ++tx) atomicAdd(&s_cnt[(ty * PP.tiles_x + tx) * NBUCKET + bk], 1u);
         }
+        for (uint32_t k = l_lo + tid; k < nl; k += NT) {
+            const uint2 b = ldi<COOP>(&ebb[U - 1 - k]);
+            if (b.x != BB_SKIP) atomicAdd(&s_lcnt[depth_bucket(PP, b.y, NLB, sc_large)], 1u);
+        }
+        __syncthreads();
+        if (tid == 0) {
+            uint32_t run = 0;
+            for (int k = 0; k < NLB; ++k) { s_loff[k] = run; run += s_lcnt[k]; s_lcnt[k] = 0; }
+            s_wtot[31] = run;   // (number of large entries; read below after the next barrier)
+        }
+        __syncthreads();
+        const uint32_t n_large = s_wtot[31];
         __syncthreads();
         // exclusive scan over (tile, bucket); thread t takes tile t's buckets
         uint32_t run = 0;
@@ -756,16 +870,16 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
                 uint32_t *g_off = PP.tile_off + (size_t)env * (size_t)(NK + 1) + (size_t)t * NBUCKET;
 #pragma unroll
                 for (int k = 0; k < NBUCKET; ++k) { s_off[t * NBUCKET + k] = ex; g_off[k] = ex; s_cnt[t * NBUCKET + k] = 0; ex += v[k]; }
-                // the tile's raster task, filed under its cost class: refs of the tile, plus the large records
-                // every tile of the environment scans
-                const uint32_t cost = sum + (nl >> 2) + 8u;
+                // the tile's raster task, filed under its cost class: references of the tile, plus a share of the
+                // large records
+                const uint32_t cost = sum + (n_large >> 2) + 8u;
                 const int c = min(NCLASS - 1, 28 - __clz((int)cost));
                 v[0] = (uint32_t)c | (atomicAdd(&s_ccnt[c], 1u) << 8);
             }
             run += tot;
             __syncthreads();
             if (t0 + NT >= T) {   // last chunk: reserve this environment's range of every class list
-                if (tid < NCLASS && s_ccnt[tid]) s_cbase[tid] = atomicAdd(&PP.ctl[C_TASK_CNT + tid], s_ccnt[tid]);
+                if (tid < NCLASS && s_ccnt[tid]) s_cbase[tid] = atomicAdd(&PP.ctl[C_TASK_CNT + pi * NCLASS + tid], s_ccnt[tid]);
                 __syncthreads();
             }
             // (T <= NT in every supported frame size, so the class bases are ready for the tile written below)
@@ -776,30 +890,45 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
         }
         if (tid == 0) {
             PP.tile_off[(size_t)env * (size_t)(NK + 1) + NK] = run;
-            if (STATS) atomicAdd(&PP.g.stats[GX_STAT_REFS], (unsigned long long)run);
+            PP.n_large[env] = n_large;
+            if (phase == 1) { PP.cntA[2 * env] = ns; PP.cntA[2 * env + 1] = nl; }
+            if (STATS) {
+                atomicAdd(&PP.g.stats[GX_STAT_REFS], (unsigned long long)run);
+                atomicAdd(&PP.g.stats[GX_STAT_LARGE], (unsigned long long)n_large);
+            }
         }
         __syncthreads();
         // fill
-        for (uint32_t s = tid; s < ns; s += NT) {
+        for (uint32_t s = s_lo + tid; s < ns; s += NT) {
             const uint2 b = ldi<COOP>(&ebb[s]);
             if (b.x == BB_SKIP) continue;
             const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
             const int i1 = i0 + (int)((b.x >> 16) & 255u), j1 = j0 + (int)(b.x >> 24);
-            const int bk = depth_bucket(PP, b.y);
+            const int bk = depth_bucket(PP, b.y, NBUCKET, sc_small);
             for (int ty = j0 >> 4; ty <= (j1 >> 4); ++ty)
                 for (int tx = i0 >> 4; tx <= (i1 >> 4); ++tx) {
                     const int key = (ty * PP.tiles_x + tx) * NBUCKET + bk;
                     erefs[s_off[key] + atomicAdd(&s_cnt[key], 1u)] = s;
                 }
         }
+        for (uint32_t k = l_lo + tid; k < nl; k += NT) {
+            const uint32_t slot = U - 1 - k;
+            const uint2 b = ldi<COOP>(&ebb[slot]);
+            if (b.x == BB_SKIP) continue;
+            const int bk = depth_bucket(PP, b.y, NLB, sc_large);
+            bool wide;
+            const unsigned long long m = large_mask<COOP>(PP, env_recs + (size_t)slot * 4, b.x, wide);
+            const uint32_t at = s_loff[bk] + atomicAdd(&s_lcnt[bk], 1u);
+            elarge[U - 1 - at] = make_uint4(slot | (wide ? 0x80000000u : 0u), (uint32_t)m, (uint32_t)(m >> 32), b.y);
+        }
     }
 }
 
 template <bool STATS>
-__global__ void __launch_bounds__(256) bin_kernel(const PipeParams PP) {
+__global__ void __launch_bounds__(256) bin_kernel(const PipeParams PP, int phase) {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t *s_cnt = reinterpret_cast<uint32_t *>(smem);
-    bin_stage<false, STATS>(PP, s_cnt, s_cnt + PP.T * NBUCKET);
+    bin_stage<false, STATS>(PP, s_cnt, s_cnt + PP.T * NBUCKET, phase);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -814,14 +943,23 @@ enum { R_E0 = 0, R_E1, R_E2,   // E_e at the (clipped) box origin
        R_BB,                   // x | y << 4 | (w-1) << 8 | (h-1) << 12 | bias bits << 16   (tile-relative)
        R_SLOT,                 // slot of the record in the environment's segment
        REC_WORDS };
+// staged record of the large path (same SoA area)
+enum { L_E0 = 0, L_E1, L_E2,      // E_e - bias_e at the tile's first pixel
+       L_SX0, L_SX1, L_SX2,       // step of E_e per pixel in x
+       L_SY0, L_SY1, L_SY2,       // ... in y
+       L_Q0, L_Q1, L_Q2, L_FA, L_ID, L_SLOT,
+       L_CLIP,                    // cx0 | cy0 << 4 | cx1 << 8 | cy1 << 12 | bias bits << 16: the record's box inside the tile
+       LREC_WORDS };
+constexpr int STAGE_WORDS = (int)LREC_WORDS > (int)REC_WORDS ? (int)LREC_WORDS : (int)REC_WORDS;
 
 struct RastWarpSmem {
     unsigned long long *fb;   // [256] keys: depth bits << 32 | record slot; KEY_BG = background
-    uint32_t *rec;            // [REC_WORDS * 32]
+    uint32_t *rec;            // [STAGE_WORDS * 32]
     uint32_t *fq;             // [FQ_CAP] covered fragments: r | x << 5 | y << 9 (relative to the record's clipped box)
     uint32_t *hz;             // [8] bits of the largest stored depth per 8x4-pixel block; 0xFFFFFFFF = background shows
+    uint32_t *pend;           // [64] small records that passed the hi-Z test and wait for a full group
 };
-constexpr int RAST_WARP_SMEM = 256 * 8 + REC_WORDS * 32 * 4 + FQ_CAP * 4 + 8 * 4;
+constexpr int RAST_WARP_SMEM = 256 * 8 + STAGE_WORDS * 32 * 4 + FQ_CAP * 4 + 8 * 4 + 64 * 4;
 
 // key of pixel (x, y) of the tile: bit 3 of the column XORed with bit 0 of the row, so that an 8x4 block of
 // 64-bit keys touches every bank exactly twice (the minimum) and 4-aligned runs of a row stay contiguous
@@ -848,61 +986,97 @@ __device__ __forceinline__ void key_min_rec(unsigned long long *slot, uint32_t d
 }
 
 // ---- large records: pixel-parallel over the tile's eight 8x4-pixel blocks ---------------------------------
-// Lanes 0..7 classify one block each: rejected if some edge function is negative at all four corners (its
-// largest corner value is), if the block misses the record's box, or if the record's nearest depth is behind
-// the block's hi-Z value.  The surviving blocks are drawn one after the other, one pixel per lane; the lane
-// owns the pixel's key, so N9 is a plain compare and store, and the block's hi-Z value is the warp maximum
-// of the stored depths afterwards.
-template <bool COOP, bool STATS>
-__device__ __forceinline__ void draw_large(const PipeParams &PP, const RastWarpSmem &ws, const uint4 *env_recs, uint32_t slot,
-                                           int x0, int y0, int lane, unsigned &n_frag, unsigned &n_blk) {
-    const unsigned FULL = 0xFFFFFFFFu;
+// The tile's large records are set up one per lane into the staging area (edge values at the tile's first pixel,
+// steps, 1/w, the box inside the tile).  Then four records at a time, lane = (record, block): a block is rejected
+// if some edge function is negative at all four corners (its largest corner value is), if it misses the record's
+// box, or if the record's nearest depth is behind the block's hi-Z value.  The surviving (record, block) pairs
+// are drawn one after the other, one pixel per lane; the lane owns the pixel's key, so N9 is a plain compare and
+// store, and the block's hi-Z value is the warp maximum of the stored depths afterwards.
+template <bool COOP>
+__device__ __forceinline__ void stage_large(const RastWarpSmem &ws, const uint4 *env_recs, uint32_t slot, int pos, int x0, int y0) {
     const uint4 *rp = env_recs + (size_t)slot * 4;
     const uint4 u0 = ldi<COOP>(rp), u1 = ldi<COOP>(rp + 1), u2 = ldi<COOP>(rp + 2);
-    const uint32_t flags = u2.w >> 24, bb = u1.z, id2 = u1.w;
+    const uint32_t flags = u2.w >> 24, bb = u1.z;
     const int i0 = (int)(bb & 255u), j0 = (int)((bb >> 8) & 255u);
     const int cx0 = max(i0, x0) - x0, cx1 = min(i0 + (int)((bb >> 16) & 255u), x0 + TILE - 1) - x0;
     const int cy0 = max(j0, y0) - y0, cy1 = min(j0 + (int)(bb >> 24), y0 + TILE - 1) - y0;
-    const float q0 = __uint_as_float(u2.x), q1 = __uint_as_float(u2.y), q2 = __uint_as_float(u2.z);
-    const float qmax = fmaxf(q0, fmaxf(q1, q2));
+    const uint32_t E[3] = {u0.x, u0.y, u0.z}, D[3] = {u0.w, u1.x, u1.y};
+#pragma unroll
+    for (int e = 0; e < 3; ++e) {
+        const int dx = (int)D[e] >> 16, dy = (int)(short)(D[e] & 0xFFFFu);
+        const int sx = -(dy << 8), sy = dx << 8;
+        ws.rec[(L_SX0 + e) * 32 + pos] = (uint32_t)sx;
+        ws.rec[(L_SY0 + e) * 32 + pos] = (uint32_t)sy;
+        ws.rec[(L_E0 + e) * 32 + pos] = (uint32_t)((int)E[e] + (y0 - j0) * sy + (x0 - i0) * sx - (int)((flags >> e) & 1u));
+    }
+    ws.rec[L_Q0 * 32 + pos] = u2.x; ws.rec[L_Q1 * 32 + pos] = u2.y; ws.rec[L_Q2 * 32 + pos] = u2.z;
+    ws.rec[L_FA * 32 + pos] = __float_as_uint((float)(int)(u0.x + u0.y + u0.z));   // E_0 + E_1 + E_2 = A at any pixel
+    ws.rec[L_ID * 32 + pos] = u1.w;
+    ws.rec[L_SLOT * 32 + pos] = slot;
+    ws.rec[L_CLIP * 32 + pos] = (uint32_t)cx0 | ((uint32_t)cy0 << 4) | ((uint32_t)cx1 << 8) | ((uint32_t)cy1 << 12) | ((flags & (uint32_t)F_BIAS) << 16);
+}
+
+template <bool COOP, bool STATS>
+__device__ __forceinline__ void draw_staged_large(const PipeParams &PP, const RastWarpSmem &ws, const uint4 *env_recs, int ns,
+                                                  int lane, unsigned &n_frag, unsigned &n_blk) {
+    const unsigned FULL = 0xFFFFFFFFu;
     const float zfar = PP.g.zfar;
     const int b8 = lane & 7, bxo8 = (b8 & 1) * 8, byo8 = (b8 >> 1) * 4;
     const int lx = lane & 7, ly = lane >> 3;
-    bool rej = bxo8 > cx1 || bxo8 + 7 < cx0 || byo8 > cy1 || byo8 + 3 < cy0;
-    if (PP.hiz) rej = rej || (qmax * __uint_as_float(ws.hz[b8]) < 1.0f - 1e-5f);
-
-    if (!(flags & F_WIDE)) {
-        int sx[3], sy[3], Et[3], bias[3];
-        const uint32_t E[3] = {u0.x, u0.y, u0.z}, D[3] = {u0.w, u1.x, u1.y};
+    for (int r0 = 0; r0 < ns; r0 += 4) {
+        const int rr = r0 + (lane >> 3);
+        bool rej = rr >= ns;
+        if (!rej) {
+            const uint32_t clip = ws.rec[L_CLIP * 32 + rr];
+            const int cx0 = (int)(clip & 15u), cy0 = (int)((clip >> 4) & 15u), cx1 = (int)((clip >> 8) & 15u), cy1 = (int)((clip >> 12) & 15u);
+            rej = bxo8 > cx1 || bxo8 + 7 < cx0 || byo8 > cy1 || byo8 + 3 < cy0;
+            if (PP.hiz) {
+                const float qm = fmaxf(__uint_as_float(ws.rec[L_Q0 * 32 + rr]), fmaxf(__uint_as_float(ws.rec[L_Q1 * 32 + rr]), __uint_as_float(ws.rec[L_Q2 * 32 + rr])));
+                rej = rej || (qm * __uint_as_float(ws.hz[b8]) < 1.0f - 1e-5f);
+            }
 #pragma unroll
-        for (int e = 0; e < 3; ++e) {
-            const int dx = (int)D[e] >> 16, dy = (int)(short)(D[e] & 0xFFFFu);
-            sx[e] = -(dy << 8);
-            sy[e] = dx << 8;
-            bias[e] = (int)((flags >> e) & 1u);
-            Et[e] = (int)E[e] + (y0 - j0) * sy[e] + (x0 - i0) * sx[e] - bias[e];   // at the tile's first pixel, bias taken off
+            for (int e = 0; e < 3; ++e) {
+                const int sx = (int)ws.rec[(L_SX0 + e) * 32 + rr], sy = (int)ws.rec[(L_SY0 + e) * 32 + rr];
+                const int mx = (int)ws.rec[(L_E0 + e) * 32 + rr] + bxo8 * sx + byo8 * sy + max(7 * sx, 0) + max(3 * sy, 0);
+                rej = rej || mx < 0;
+            }
         }
-        const float fA = (float)(int)(u0.x + u0.y + u0.z);   // E_0 + E_1 + E_2 = A at any pixel
-#pragma unroll
-        for (int e = 0; e < 3; ++e) {
-            const int mx = Et[e] + bxo8 * sx[e] + byo8 * sy[e] + max(7 * sx[e], 0) + max(3 * sy[e], 0);
-            rej = rej || mx < 0;
-        }
-        unsigned live = __ballot_sync(FULL, lane < 8 && !rej);
-        int Ep[3];
-#pragma unroll
-        for (int e = 0; e < 3; ++e) Ep[e] = Et[e] + lx * sx[e] + ly * sy[e];
+        unsigned live = __ballot_sync(FULL, !rej);
+        int cur = -1;
+        int Ep[3] = {0, 0, 0}, sx[3] = {0, 0, 0}, sy[3] = {0, 0, 0}, bias[3] = {0, 0, 0}, cx0 = 0, cy0 = 0, cx1 = 0, cy1 = 0;
+        float q0 = 0.f, q1 = 0.f, q2 = 0.f, fA = 0.f, qmax = 0.f;
+        uint32_t slot = 0, id2 = 0;
         while (live) {
-            const int b = __ffs((int)live) - 1;
+            const int bit = __ffs((int)live) - 1;
             live &= live - 1u;
+            const int rec = r0 + (bit >> 3), b = bit & 7;
+            if (rec != cur) {   // (uniform)
+                cur = rec;
+                const uint32_t clip = ws.rec[L_CLIP * 32 + rec];
+                cx0 = (int)(clip & 15u); cy0 = (int)((clip >> 4) & 15u); cx1 = (int)((clip >> 8) & 15u); cy1 = (int)((clip >> 12) & 15u);
+#pragma unroll
+                for (int e = 0; e < 3; ++e) {
+                    sx[e] = (int)ws.rec[(L_SX0 + e) * 32 + rec];
+                    sy[e] = (int)ws.rec[(L_SY0 + e) * 32 + rec];
+                    Ep[e] = (int)ws.rec[(L_E0 + e) * 32 + rec] + lx * sx[e] + ly * sy[e];
+                    bias[e] = (int)((clip >> (16 + e)) & 1u);
+                }
+                q0 = __uint_as_float(ws.rec[L_Q0 * 32 + rec]); q1 = __uint_as_float(ws.rec[L_Q1 * 32 + rec]); q2 = __uint_as_float(ws.rec[L_Q2 * 32 + rec]);
+                qmax = fmaxf(q0, fmaxf(q1, q2));
+                fA = __uint_as_float(ws.rec[L_FA * 32 + rec]);
+                slot = ws.rec[L_SLOT * 32 + rec];
+                id2 = ws.rec[L_ID * 32 + rec];
+            }
+            // the block's hi-Z value may have moved since the record was listed
+            if (PP.hiz && qmax * __uint_as_float(ws.hz[b]) < 1.0f - 1e-5f) continue;
             const int bxo = (b & 1) * 8, byo = (b >> 1) * 4;
             const int px = bxo + lx, py = byo + ly;
             const int E0 = Ep[0] + bxo * sx[0] + byo * sy[0], E1 = Ep[1] + bxo * sx[1] + byo * sy[1],
                       E2 = Ep[2] + bxo * sx[2] + byo * sy[2];
             const bool cov = px >= cx0 && px <= cx1 && py >= cy0 && py <= cy1 && (E0 | E1 | E2) >= 0;
             unsigned long long *kp = &ws.fb[fb_idx(px, py)];
-            const unsigned long long cur = *kp;
-            uint32_t nd = (uint32_t)(cur >> 32);
+            const unsigned long long ck = *kp;
+            uint32_t nd = (uint32_t)(ck >> 32);
             if (cov) {
                 const float f0 = (float)(E0 + bias[0]), f1 = (float)(E1 + bias[1]), f2 = (float)(E2 + bias[2]);
                 const float num = fmaf(f2, q2, fmaf(f1, q1, f0 * q0));
@@ -910,52 +1084,72 @@ __device__ __forceinline__ void draw_large(const PipeParams &PP, const RastWarpS
                 if (!(depth > zfar)) {
                     const uint32_t d = __float_as_uint(depth);
                     bool win = d < nd;
-                    if (d == nd) win = id2 < ldi<COOP>(reinterpret_cast<const uint32_t *>(env_recs + (size_t)(uint32_t)cur * 4) + 7);
+                    if (d == nd) win = id2 < ldi<COOP>(reinterpret_cast<const uint32_t *>(env_recs + (size_t)(uint32_t)ck * 4) + 7);
                     if (win) { *kp = ((unsigned long long)d << 32) | slot; nd = d; }
                 }
             }
             const uint32_t zb = __reduce_max_sync(FULL, nd);
             if (lane == 0) ws.hz[b] = zb;
+            __syncwarp();
             if (STATS) { n_frag += cov ? 1u : 0u; n_blk += lane == 0 ? 1u : 0u; }
         }
-    } else {
-        Tri t;
-        t.X[0] = (int)u0.x; t.X[1] = (int)u0.y; t.X[2] = (int)u0.z;
-        t.Y[0] = (int)u0.w; t.Y[1] = (int)u1.x; t.Y[2] = (int)u1.y;
-        t.q[0] = q0; t.q[1] = q1; t.q[2] = q2;
-        t.id2 = id2;
-        Edges E;
-        edge_setup(t, area2(t), E);   // orientation-normalised by the geometry stage: area > 0
-        {
-            const long long pxo = (long long)(((x0 + bxo8) << 8) + 128), pyo = (long long)(((y0 + byo8) << 8) + 128);
+    }
+    __syncwarp();
+}
+
+// a wide record (edge functions need int64): straight from its record, block by block
+template <bool COOP, bool STATS>
+__device__ __noinline__ void draw_wide(const PipeParams &PP, const RastWarpSmem &ws, const uint4 *env_recs, uint32_t slot,
+                                       int x0, int y0, int lane, unsigned &n_frag, unsigned &n_blk) {
+    const unsigned FULL = 0xFFFFFFFFu;
+    const uint4 *rp = env_recs + (size_t)slot * 4;
+    const uint4 u0 = ldi<COOP>(rp), u1 = ldi<COOP>(rp + 1), u2 = ldi<COOP>(rp + 2);
+    const uint32_t bb = u1.z, id2 = u1.w;
+    const int i0 = (int)(bb & 255u), j0 = (int)((bb >> 8) & 255u);
+    const int cx0 = max(i0, x0) - x0, cx1 = min(i0 + (int)((bb >> 16) & 255u), x0 + TILE - 1) - x0;
+    const int cy0 = max(j0, y0) - y0, cy1 = min(j0 + (int)(bb >> 24), y0 + TILE - 1) - y0;
+    const float zfar = PP.g.zfar;
+    const int b8 = lane & 7, bxo8 = (b8 & 1) * 8, byo8 = (b8 >> 1) * 4;
+    const int lx = lane & 7, ly = lane >> 3;
+    Tri t;
+    t.X[0] = (int)u0.x; t.X[1] = (int)u0.y; t.X[2] = (int)u0.z;
+    t.Y[0] = (int)u0.w; t.Y[1] = (int)u1.x; t.Y[2] = (int)u1.y;
+    t.q[0] = __uint_as_float(u2.x); t.q[1] = __uint_as_float(u2.y); t.q[2] = __uint_as_float(u2.z);
+    t.id2 = id2;
+    const float qmax = fmaxf(t.q[0], fmaxf(t.q[1], t.q[2]));
+    bool rej = bxo8 > cx1 || bxo8 + 7 < cx0 || byo8 > cy1 || byo8 + 3 < cy0;
+    if (PP.hiz) rej = rej || (qmax * __uint_as_float(ws.hz[b8]) < 1.0f - 1e-5f);
+    Edges E;
+    edge_setup(t, area2(t), E);   // orientation-normalised by the geometry stage: area > 0
+    {
+        const long long pxo = (long long)(((x0 + bxo8) << 8) + 128), pyo = (long long)(((y0 + byo8) << 8) + 128);
 #pragma unroll
-            for (int e = 0; e < 3; ++e) {
-                const long long Eb = (long long)E.dx[e] * (pyo - E.Ya[e]) - (long long)E.dy[e] * (pxo - E.Xa[e]) - E.bias[e];
-                const long long sx = -(long long)E.dy[e] * 256, sy = (long long)E.dx[e] * 256;
-                const long long mx = Eb + max(7 * sx, 0ll) + max(3 * sy, 0ll);
-                rej = rej || mx < 0;
-            }
+        for (int e = 0; e < 3; ++e) {
+            const long long Eb = (long long)E.dx[e] * (pyo - E.Ya[e]) - (long long)E.dy[e] * (pxo - E.Xa[e]) - E.bias[e];
+            const long long sx = -(long long)E.dy[e] * 256, sy = (long long)E.dx[e] * 256;
+            const long long mx = Eb + max(7 * sx, 0ll) + max(3 * sy, 0ll);
+            rej = rej || mx < 0;
         }
-        unsigned live = __ballot_sync(FULL, lane < 8 && !rej);
-        while (live) {
-            const int b = __ffs((int)live) - 1;
-            live &= live - 1u;
-            const int px = (b & 1) * 8 + lx, py = (b >> 1) * 4 + ly;
-            float f[3], num, depth;
-            const bool cov = px >= cx0 && px <= cx1 && py >= cy0 && py <= cy1 && cover_depth(E, t.q, x0 + px, y0 + py, f, num, depth);
-            unsigned long long *kp = &ws.fb[fb_idx(px, py)];
-            const unsigned long long cur = *kp;
-            uint32_t nd = (uint32_t)(cur >> 32);
-            if (cov && !(depth > zfar)) {
-                const uint32_t d = __float_as_uint(depth);
-                bool win = d < nd;
-                if (d == nd) win = id2 < ldi<COOP>(reinterpret_cast<const uint32_t *>(env_recs + (size_t)(uint32_t)cur * 4) + 7);
-                if (win) { *kp = ((unsigned long long)d << 32) | slot; nd = d; }
-            }
-            const uint32_t zb = __reduce_max_sync(FULL, nd);
-            if (lane == 0) ws.hz[b] = zb;
-            if (STATS) { n_frag += cov ? 1u : 0u; n_blk += lane == 0 ? 1u : 0u; }
+    }
+    unsigned live = __ballot_sync(FULL, lane < 8 && !rej);
+    while (live) {
+        const int b = __ffs((int)live) - 1;
+        live &= live - 1u;
+        const int px = (b & 1) * 8 + lx, py = (b >> 1) * 4 + ly;
+        float f[3], num, depth;
+        const bool cov = px >= cx0 && px <= cx1 && py >= cy0 && py <= cy1 && cover_depth(E, t.q, x0 + px, y0 + py, f, num, depth);
+        unsigned long long *kp = &ws.fb[fb_idx(px, py)];
+        const unsigned long long ck = *kp;
+        uint32_t nd = (uint32_t)(ck >> 32);
+        if (cov && !(depth > zfar)) {
+            const uint32_t d = __float_as_uint(depth);
+            bool win = d < nd;
+            if (d == nd) win = id2 < ldi<COOP>(reinterpret_cast<const uint32_t *>(env_recs + (size_t)(uint32_t)ck * 4) + 7);
+            if (win) { *kp = ((unsigned long long)d << 32) | slot; nd = d; }
         }
+        const uint32_t zb = __reduce_max_sync(FULL, nd);
+        if (lane == 0) ws.hz[b] = zb;
+        if (STATS) { n_frag += cov ? 1u : 0u; n_blk += lane == 0 ? 1u : 0u; }
     }
     __syncwarp();
 }
@@ -1025,31 +1219,17 @@ __device__ __forceinline__ void shade_queue(const RastWarpSmem &ws, int qn, floa
 }
 
 // K3 (inside the tile): the clipped boxes of the group's records are cut into slots of SW pixels of one row.
-// Returns the lane's exclusive prefix of slot counts (Pex, record = lane) and the group's total.  A record
-// whose nearest vertex is behind the hi-Z value of every block its box touches gets no slots.
+// Returns the lane's exclusive prefix of slot counts (Pex, record = lane) and the group's total.
 template <int SW>
-__device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int lane, bool use_hz, int &Pex, unsigned &skip,
-                                           unsigned &n_culled) {
+__device__ __forceinline__ int group_slots(const RastWarpSmem &ws, int nrec, int lane, int &Pex, unsigned &skip) {
     const unsigned FULL = 0xFFFFFFFFu;
     int ns = 0;
-    bool culled = false;
     if (lane < nrec) {
         const uint32_t bb = ws.rec[R_BB * 32 + lane];
-        const int x = (int)(bb & 15u), y = (int)((bb >> 4) & 15u);
         const int w = (int)((bb >> 8) & 15u) + 1, h = (int)((bb >> 12) & 15u) + 1;
         ns = h * ((w + SW - 1) / SW);
-        if (use_hz) {
-            uint32_t zb = 0;
-            for (int by = y >> 2; by <= ((y + h - 1) >> 2); ++by)
-                for (int bx = x >> 3; bx <= ((x + w - 1) >> 3); ++bx) zb = max(zb, ws.hz[by * 2 + bx]);
-            const float qmax = fmaxf(__uint_as_float(ws.rec[(R_Q0 + 0) * 32 + lane]),
-                                     fmaxf(__uint_as_float(ws.rec[(R_Q0 + 1) * 32 + lane]),
-                                           __uint_as_float(ws.rec[(R_Q0 + 2) * 32 + lane])));
-            // every depth of the triangle is >= 1/qmax (N7, up to a few ulp): hidden iff 1/qmax > zmax with margin
-            if (qmax * __uint_as_float(zb) < 1.0f - 1e-5f) { ns = 0; culled = true; ++n_culled; }
-        }
     }
-    skip = __ballot_sync(FULL, culled || lane >= nrec);   // records without slots: the slot walk steps over them
+    skip = __ballot_sync(FULL, lane >= nrec);   // records without slots: the slot walk steps over them
     int inc = ns;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -1216,25 +1396,34 @@ __device__ __forceinline__ uint32_t resolve_rec(const uint4 *env_recs, uint32_t 
 }
 
 // The raster stage: every warp draws tile tasks, heaviest class first, until none is left.
+// phase 0: clear, draw, resolve (K5).  phase 1 (occluder phase): clear, draw, leave the tile's keys and its hi-Z
+// values in global memory.  phase 2: reload the keys, draw what the second geometry phase added, resolve.
 // warp_smem: RAST_WARP_SMEM bytes of shared memory private to the warp.
-template <bool COOP, bool STATS>
+template <bool COOP, bool STATS, int PHASE>
 __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char *warp_smem) {
+    constexpr int phase = PHASE;
     const GxParams &P = PP.g;
     const unsigned FULL = 0xFFFFFFFFu;
     constexpr int SW = 4;
     const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u;
     const int W = P.W, npix = P.W * P.H, T = PP.T, NK = T * NBUCKET;
+    const int pi = phase == 2 ? 1 : 0;
     RastWarpSmem ws;
     ws.fb = reinterpret_cast<unsigned long long *>(warp_smem);
     ws.rec = reinterpret_cast<uint32_t *>(warp_smem + 256 * 8);
-    ws.fq = ws.rec + REC_WORDS * 32;
+    ws.fq = ws.rec + STAGE_WORDS * 32;
     ws.hz = ws.fq + FQ_CAP;
+    ws.pend = ws.hz + 8;
     const bool want_rgb = P.rgb != nullptr || P.obs != nullptr;
-    unsigned st_frag = 0, st_culled = 0, st_blk = 0;
+    unsigned st_frag = 0, st_culled = 0, st_blk = 0, st_ldraw = 0;
+    const int cshift = T > 64 ? 1 : 0;                      // a cell of the large records' masks is 1 or 2x2 tiles
+    const int cells_x = (PP.tiles_x + cshift) >> cshift;
+    const int hzb_w = W >> 3;
 
     // class list boundaries: tasks are drawn from the heaviest class down
     uint32_t cnt_c = 0;
-    if (lane < NCLASS) cnt_c = ldi<COOP>(&PP.ctl[C_TASK_CNT + (NCLASS - 1 - lane)]);   // lane l holds class NCLASS-1-l
+    if (lane < NCLASS) cnt_c = ldi<COOP>(&PP.ctl[C_TASK_CNT + pi * NCLASS + (NCLASS - 1 - lane)]);   // lane l holds class NCLASS-1-l
     uint32_t inc_c = cnt_c;
 #pragma unroll
     for (int d = 1; d < NCLASS; d <<= 1) {
@@ -1246,7 +1435,7 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
 
     for (;;) {
         uint32_t k = 0;
-        if (lane == 0) k = atomicAdd(&PP.ctl[C_RAST_CUR], 1u);
+        if (lane == 0) k = atomicAdd(&PP.ctl[C_RAST_CUR + pi], 1u);
         k = __shfl_sync(FULL, k, 0);
         if (k >= n_tasks) break;
         // class of task k: first lane whose inclusive prefix exceeds k
@@ -1261,60 +1450,113 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
         const uint4 *env_recs = PP.recs + base * 4;
         const uint2 *ebb = PP.bbs + base;
         const uint32_t *erefs = PP.refs + 4 * base;
-        const uint32_t U = ldi<COOP>(&PP.U[env]), nl = ldi<COOP>(&PP.cnt[2 * env + 1]);
+        const uint4 *elarge = reinterpret_cast<const uint4 *>(erefs);
+        const uint32_t U = ldi<COOP>(&PP.U[env]), nl = ldi<COOP>(&PP.n_large[env]);
+        uint4 *gkeys = reinterpret_cast<uint4 *>(PP.keys + (size_t)task * 256);
+        uint32_t *ghzb = PP.hizb + (size_t)env * (size_t)hzb_w * (size_t)(P.H >> 2);
 
-        // ---- clear the tile ------------------------------------------------------------------------
+        // ---- clear the tile, or take it over from the occluder phase -------------------------------------
         {
             uint4 *f4 = reinterpret_cast<uint4 *>(ws.fb);
-            const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+            if (phase == 2) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) f4[i * 32 + lane] = ones;
-            if (lane < 8) ws.hz[lane] = 0xFFFFFFFFu;
+                for (int i = 0; i < 4; ++i) f4[i * 32 + lane] = __ldcg(&gkeys[i * 32 + lane]);
+                if (lane < 8) ws.hz[lane] = __ldcg(&ghzb[(ty * 4 + (lane >> 1)) * hzb_w + tx * 2 + (lane & 1)]);
+            } else {
+                const uint4 ones = make_uint4(0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu, 0xFFFFFFFFu);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) f4[i * 32 + lane] = ones;
+                if (lane < 8) ws.hz[lane] = 0xFFFFFFFFu;
+            }
         }
         __syncwarp();
 
-        // ---- large records: every tile scans the environment's list (top of the segment) -----------------
-        for (uint32_t c0 = 0; c0 < nl; c0 += 32) {
-            const uint32_t s = U - nl + c0 + lane;
-            bool ov = false;
-            if (c0 + lane < nl) {
-                const uint2 b = ldi<COOP>(&ebb[s]);
-                if (b.x != BB_SKIP) {
-                    const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
-                    const int i1 = i0 + (int)((b.x >> 16) & 255u), j1 = j0 + (int)(b.x >> 24);
-                    ov = i0 < x0 + TILE && i1 >= x0 && j0 < y0 + TILE && j1 >= y0;
+        // ---- large records of the environment, front to back: those whose mask has this tile's cell ----------
+        {
+            const int cell = (ty >> cshift) * cells_x + (tx >> cshift);
+            for (uint32_t c0 = 0; c0 < nl; c0 += 32) {
+                bool ov = false;
+                uint4 en = make_uint4(0u, 0u, 0u, 0u);
+                if (c0 + lane < nl) {
+                    en = ldi<COOP>(&elarge[U - 1 - (c0 + lane)]);
+                    ov = (((cell < 32 ? en.y : en.z) >> (cell & 31)) & 1u) != 0u;
+                    if (ov && cshift) {   // (cells of 2x2 tiles: the record's box against this tile)
+                        const uint32_t bb = ldi<COOP>(&ebb[en.x & 0x7FFFFFFFu]).x;
+                        const int i0 = (int)(bb & 255u), j0 = (int)((bb >> 8) & 255u);
+                        const int i1 = i0 + (int)((bb >> 16) & 255u), j1 = j0 + (int)(bb >> 24);
+                        ov = i0 < x0 + TILE && i1 >= x0 && j0 < y0 + TILE && j1 >= y0;
+                    }
                     if (ov && PP.hiz) {   // behind everything drawn so far in every block of the tile?
                         uint32_t tz = 0;
 #pragma unroll
                         for (int i = 0; i < 8; ++i) tz = max(tz, ws.hz[i]);
-                        ov = !(__uint_as_float(b.y) * __uint_as_float(tz) < 1.0f - 1e-5f);
+                        ov = !(__uint_as_float(en.w) * __uint_as_float(tz) < 1.0f - 1e-5f);
                         if (STATS && !ov) ++st_culled;
                     }
                 }
-            }
-            unsigned m = __ballot_sync(FULL, ov);
-            while (m) {
-                const int src = __ffs((int)m) - 1;
-                m &= m - 1u;
-                draw_large<COOP, STATS>(PP, ws, env_recs, __shfl_sync(FULL, s, src), x0, y0, lane, st_frag, st_blk);
+                const unsigned mw = __ballot_sync(FULL, ov && (en.x >> 31));
+                const unsigned mn = __ballot_sync(FULL, ov && !(en.x >> 31));
+                if (mn) {
+                    if (ov && !(en.x >> 31)) stage_large<COOP>(ws, env_recs, en.x, __popc(mn & lt), x0, y0);
+                    __syncwarp();
+                    if (STATS) st_ldraw += lane == 0 ? (unsigned)__popc(mn) : 0u;
+                    draw_staged_large<COOP, STATS>(PP, ws, env_recs, __popc(mn), lane, st_frag, st_blk);
+                }
+                unsigned m = mw;
+                while (m) {
+                    const int src = __ffs((int)m) - 1;
+                    m &= m - 1u;
+                    if (STATS) st_ldraw += lane == 0 ? 1u : 0u;
+                    draw_wide<COOP, STATS>(PP, ws, env_recs, __shfl_sync(FULL, en.x, src) & 0x7FFFFFFFu, x0, y0, lane, st_frag, st_blk);
+                }
             }
         }
 
         // ---- small records of the tile, nearest bucket first ---------------------------------------------
+        // The references are tested against the hi-Z values of the blocks their box touches before the record is
+        // loaded; the survivors wait in `pend` until a full group of 32 can be drawn.
         {
             const uint32_t *toff = PP.tile_off + (size_t)env * (size_t)(NK + 1) + (size_t)tile * NBUCKET;
             const uint32_t r_begin = ldi<COOP>(&toff[0]), r_end = ldi<COOP>(&toff[NBUCKET]);
-            for (uint32_t r0 = r_begin; r0 < r_end; r0 += 32) {
-                const int nrec = (int)min(32u, r_end - r0);
+            int np = 0;
+            for (uint32_t r0 = r_begin; r0 < r_end || np > 0; r0 += 32) {
+                if (r0 < r_end) {
+                    const bool have = r0 + lane < r_end;
+                    const uint32_t slot = have ? ldi<COOP>(&erefs[r0 + lane]) : 0u;
+                    bool keep = have;
+                    if (have && PP.hiz) {
+                        const uint2 b = ldi<COOP>(&ebb[slot]);
+                        const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
+                        const int x = max(i0, x0) - x0, y = max(j0, y0) - y0;
+                        const int x1 = min(i0 + (int)((b.x >> 16) & 255u), x0 + TILE - 1) - x0, y1 = min(j0 + (int)(b.x >> 24), y0 + TILE - 1) - y0;
+                        uint32_t zb = 0;
+                        for (int by = y >> 2; by <= (y1 >> 2); ++by)
+                            for (int bx = x >> 3; bx <= (x1 >> 3); ++bx) zb = max(zb, ws.hz[by * 2 + bx]);
+                        // every depth of the triangle is >= 1/qmax (N7, up to a few ulp): hidden iff 1/qmax > zmax with margin
+                        keep = !(__uint_as_float(b.y) * __uint_as_float(zb) < 1.0f - 1e-5f);
+                        if (STATS && !keep) ++st_culled;
+                    }
+                    const unsigned mk = __ballot_sync(FULL, keep);
+                    if (keep) ws.pend[np + __popc(mk & lt)] = slot;
+                    np += __popc(mk);
+                    __syncwarp();
+                    if (np < 32 && r0 + 32 < r_end) continue;
+                }
+                if (np == 0) break;
+                const int nrec = min(np, 32);
                 const bool have = lane < nrec;
-                const uint32_t slot = have ? ldi<COOP>(&erefs[r0 + lane]) : 0u;
+                const uint32_t slot = have ? ws.pend[lane] : 0u;
+                const uint32_t carry = (32 + lane < np) ? ws.pend[32 + lane] : 0u;
+                __syncwarp();
+                if (32 + lane < np) ws.pend[lane] = carry;
+                np -= nrec;
                 load_group<COOP>(ws, env_recs, slot, have, x0, y0, lane);
                 int Pex;
                 unsigned skip;
-                const int Tn = group_slots<SW>(ws, nrec, lane, PP.hiz != 0, Pex, skip, st_culled);
+                const int Tn = group_slots<SW>(ws, nrec, lane, Pex, skip);
                 if (Tn) raster_slots<COOP, STATS, SW>(ws, Pex, skip, Tn, P.zfar, env_recs, lane, st_frag);
                 // hi-Z values follow the small records too: cheap, and dense small geometry hides a lot
-                if (PP.hiz && r0 + 32 < r_end) {
+                if (PP.hiz && (r0 + 32 < r_end || np > 0)) {
 #pragma unroll
                     for (int b = 0; b < 8; ++b) {
                         const uint32_t d = (uint32_t)(ws.fb[fb_idx((b & 1) * 8 + (lane & 7), (b >> 1) * 4 + (lane >> 3))] >> 32);
@@ -1326,6 +1568,24 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
             }
         }
         __syncwarp();
+
+        if (phase == 1) {
+            // ---- occluder phase: the keys and the hi-Z values go to global memory ---------------------------
+            const uint4 *f4 = reinterpret_cast<const uint4 *>(ws.fb);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) __stcg(&gkeys[i * 32 + lane], f4[i * 32 + lane]);
+            uint32_t tz = 0;
+#pragma unroll
+            for (int b = 0; b < 8; ++b) {
+                const uint32_t d = (uint32_t)(ws.fb[fb_idx((b & 1) * 8 + (lane & 7), (b >> 1) * 4 + (lane >> 3))] >> 32);
+                const uint32_t zb = __reduce_max_sync(FULL, d);
+                if (lane == b) __stcg(&ghzb[(ty * 4 + (b >> 1)) * hzb_w + tx * 2 + (b & 1)], zb);
+                tz = max(tz, zb);
+            }
+            if (lane == 0) __stcg(&PP.hizt[(size_t)env * (size_t)T + tile], tz);
+            __syncwarp();
+            continue;
+        }
 
         // ---- K5: resolve the winners, write RGB / depth / id as 16-byte stores ----------------------------
 #pragma unroll 1
@@ -1383,11 +1643,13 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
             st_frag += __shfl_xor_sync(FULL, st_frag, d);
             st_culled += __shfl_xor_sync(FULL, st_culled, d);
             st_blk += __shfl_xor_sync(FULL, st_blk, d);
+            st_ldraw += __shfl_xor_sync(FULL, st_ldraw, d);
         }
         if (lane == 0) {
             atomicAdd(&P.stats[GX_STAT_FRAGMENTS], (unsigned long long)st_frag);
             atomicAdd(&P.stats[GX_STAT_RECORDS_OCCLUDED], (unsigned long long)st_culled);
             atomicAdd(&P.stats[GX_STAT_BLOCKS_DRAWN], (unsigned long long)st_blk);
+            atomicAdd(&P.stats[GX_STAT_LARGE_DRAWS], (unsigned long long)st_ldraw);
         }
     }
 }
@@ -1395,10 +1657,10 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
 #ifndef RAST_MINB
 #define RAST_MINB 4
 #endif
-template <int WARPS, bool STATS>
+template <int WARPS, bool STATS, int PHASE>
 __global__ void __launch_bounds__(WARPS * 32, RAST_MINB) raster_kernel(const PipeParams PP) {
     extern __shared__ __align__(16) unsigned char smem[];
-    raster_stage<false, STATS>(PP, smem + (size_t)(threadIdx.x >> 5) * RAST_WARP_SMEM);
+    raster_stage<false, STATS, PHASE>(PP, smem + (size_t)(threadIdx.x >> 5) * RAST_WARP_SMEM);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -1425,12 +1687,17 @@ __global__ void __launch_bounds__(TAIL_WARPS * 32, 2) tail_kernel(const PipePara
         grid.sync();   // every CTA has read the end of the previous wave before it moves
         if (blockIdx.x == 0) alloc_wave(PP, e_next);
         grid.sync();
-        geom_stage<true, STATS>(PP, smem + (size_t)warp * GEOM_WARP_SMEM);
-        grid.sync();
-        bin_stage<true, STATS>(PP, reinterpret_cast<uint32_t *>(smem), reinterpret_cast<uint32_t *>(smem) + PP.T * NBUCKET);
-        grid.sync();
-        raster_stage<true, STATS>(PP, smem + (size_t)warp * RAST_WARP_SMEM);
-        grid.sync();
+        for (int phase = PP.occl ? 1 : 0; phase <= (PP.occl ? 2 : 0); ++phase) {
+            if (phase == 2 && PP.hiz) geom_stage<true, STATS, true>(PP, smem + (size_t)warp * GEOM_WARP_SMEM, phase);
+            else geom_stage<true, STATS, false>(PP, smem + (size_t)warp * GEOM_WARP_SMEM, phase);
+            grid.sync();
+            bin_stage<true, STATS>(PP, reinterpret_cast<uint32_t *>(smem), reinterpret_cast<uint32_t *>(smem) + PP.T * NBUCKET, phase);
+            grid.sync();
+            if (phase == 0) raster_stage<true, STATS, 0>(PP, smem + (size_t)warp * RAST_WARP_SMEM);
+            else if (phase == 1) raster_stage<true, STATS, 1>(PP, smem + (size_t)warp * RAST_WARP_SMEM);
+            else raster_stage<true, STATS, 2>(PP, smem + (size_t)warp * RAST_WARP_SMEM);
+            grid.sync();
+        }
     }
 }
 

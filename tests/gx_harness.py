@@ -51,7 +51,8 @@ def render_gpu(wl, want_id=True, want_rgb=None, cull=1, stats=False, scene=None,
         if stats:
             out["stats"] = {k: gx.gx_get_stat(scene, k) for k in
                             ("clusters_tested", "clusters_drawn", "triangles_in", "triangles_raster", "fragments",
-                             "records_occluded", "blocks_drawn", "tile_refs", "waves", "sum_slots", "max_env_slots",
+                             "records_occluded", "blocks_drawn", "tile_refs", "triangles_hidden", "subclusters_hidden",
+                             "large_records", "large_draws", "waves", "sum_slots", "max_env_slots",
                              "bad_ids", "launches")}
         return out
     finally:

@@ -105,17 +105,21 @@ def test_cull_is_conservative(oracle_mod):
     """N10: the image with frustum culling of clusters and sub-clusters and with hi-Z rejection in the tiles equals
     the image with all of them off, bit for bit."""
     wl = gen.make_config(1, n_envs=16)
-    a = render_gpu(wl, cull=1, stats=True)
+    a = render_gpu(wl, cull=1, stats=True, options=dict(occlusion=0))
+    a2 = render_gpu(wl, cull=1, stats=True)     # occluder scheme (default at this frame size)
     b = render_gpu(wl, cull=0, stats=True, options=dict(hiz=0))
     c = render_gpu(wl, cull=1, stats=True, options=dict(subcull=0))
     d = render_gpu(wl, cull=1, stats=True, options=dict(hiz=0))
     for k in ("rgb", "depth", "id"):
         assert np.array_equal(a[k], b[k]), k
+        assert np.array_equal(a2[k], b[k]), k
         assert np.array_equal(c[k], b[k]), k
         assert np.array_equal(d[k], b[k]), k
     assert a["stats"]["clusters_drawn"] < b["stats"]["clusters_drawn"]
     assert b["stats"]["clusters_drawn"] == b["stats"]["clusters_tested"]
-    assert a["stats"]["triangles_raster"] == b["stats"]["triangles_raster"]     # culling only drops what covers nothing
+    assert a["stats"]["triangles_raster"] == b["stats"]["triangles_raster"]     # frustum culling only drops what covers nothing
+    assert a2["stats"]["triangles_raster"] < a["stats"]["triangles_raster"]     # the occluder scheme drops hidden triangles too
+    assert a2["stats"]["triangles_in"] < a["stats"]["triangles_in"]
     assert a["stats"]["triangles_in"] < c["stats"]["triangles_in"] < b["stats"]["triangles_in"]
     assert a["stats"]["records_occluded"] > 0 and d["stats"]["records_occluded"] == 0
     assert a["stats"]["fragments"] < d["stats"]["fragments"]
@@ -131,7 +135,9 @@ def test_waves_and_option_variants(oracle_mod):
     ref = render_gpu(wl, stats=True)
     rep = compare(o, ref)
     assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, rep
-    assert ref["stats"]["waves"] == 1 and ref["stats"]["launches"] == 5 and ref["stats"]["bad_ids"] == 0
+    # cull + 2 x (geometry, bin, raster) + tail: the occluder scheme is on by default for 128x128 frames
+    assert ref["stats"]["waves"] == 1 and ref["stats"]["launches"] == 8 and ref["stats"]["bad_ids"] == 0
+    assert ref["stats"]["subclusters_hidden"] > 0 and ref["stats"]["triangles_hidden"] > 0
     assert ref["stats"]["max_env_slots"] * wl.N >= ref["stats"]["sum_slots"] > ref["stats"]["triangles_raster"]
     per_env = ref["stats"]["max_env_slots"]
     variants = {
@@ -144,15 +150,24 @@ def test_waves_and_option_variants(oracle_mod):
         "no hi-Z": dict(hiz=0),
         "no sub-cluster culling": dict(subcull=0),
         "no hi-Z, blocks from 2 px, 2 environments per wave": dict(hiz=0, big_px=2, arena_slots=2 * per_env),
+        "single pass (no occluder phase)": dict(occlusion=0),
+        "single pass, 1 environment per wave": dict(occlusion=0, arena_slots=1),
+        "every sub-cluster an occluder": dict(occl_area=0),
+        "no sub-cluster an occluder (but those at the near plane)": dict(occl_area=1 << 20),
+        "occluders from 8 px per triangle, 3 environments per wave": dict(occl_area=8, arena_slots=3 * per_env),
     }
     for name, opts in variants.items():
         g = render_gpu(wl, stats=True, options=opts)
         for k in ("rgb", "depth", "id"):
             assert np.array_equal(ref[k], g[k]), (name, k)
-        if name == "arena for 1 environment":
-            assert g["stats"]["waves"] == wl.N, g["stats"]
-        if name.startswith("arena for ~3") or name == "arena by budget":
+        if name == "arena for 1 environment":      # (the arena never shrinks below the largest possible environment)
+            assert g["stats"]["waves"] >= 3, g["stats"]
+        if name == "arena by budget":
             assert 1 < g["stats"]["waves"] < wl.N, g["stats"]
+        if name.startswith("single pass"):
+            assert g["stats"]["subclusters_hidden"] == 0 and g["stats"]["triangles_hidden"] == 0
+        if name == "single pass (no occluder phase)":
+            assert g["stats"]["launches"] == 5
         if name == "block path for every record":
             assert g["stats"]["tile_refs"] == 0 and g["stats"]["blocks_drawn"] > ref["stats"]["blocks_drawn"]
     assert ref["stats"]["records_occluded"] > 0 and ref["stats"]["tile_refs"] > 0
