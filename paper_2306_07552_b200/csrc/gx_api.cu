@@ -529,14 +529,16 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     size_t off = 64;
     const size_t o_U = off; off += n;
     const size_t o_base = off; off += n;
-    const size_t o_cnt = off; off += 2 * n;
-    const size_t o_cntA = off; off += 2 * n;
+    const size_t o_cnt = off; off += n;
+    const size_t o_cntA = off; off += n;
     const size_t o_nl = off; off += n;
     const size_t o_idb = off; off += n * k1;
     const size_t o_mv = off; off += n * k1 * 12;
     const size_t o_toff = off; off += n * NK1;
     const size_t o_tasks = off; off += (size_t)gx::NCLASS * n * (size_t)PP.T;
-    const size_t o_hizt = off; off += PP.occl ? n * (size_t)PP.T : 0;
+    PP.hz_stride = 0;
+    for (int w = PP.tiles_x, h = PP.tiles_y;; w = (w + 1) >> 1, h = (h + 1) >> 1) { PP.hz_stride += w * h; if (w == 1 && h == 1) break; }
+    const size_t o_hizt = off; off += PP.occl ? n * (size_t)PP.hz_stride : 0;
     const size_t o_hizb = off; off += PP.occl ? n * (size_t)PP.T * 8 : 0;
     off = (off + 3) & ~(size_t)3;
     const size_t o_items = off; off += 4 * n * (size_t)PP.item_stride;
@@ -553,6 +555,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     sc->last_stream = stream;
     if (st) GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
     GX_CUDA(cudaMemsetAsync(PP.ctl, 0, 64 * sizeof(uint32_t), stream));
+    if (PP.occl) GX_CUDA(cudaMemsetAsync(PP.hizt, 0, n * (size_t)PP.hz_stride * sizeof(uint32_t), stream));
     if ((rc = mark(sc, stream, 0)) != GX_OK) return rc;
 
     // K1: one CTA per environment: 4 warps for small scenes, 16 where an environment has thousands of sub-clusters

@@ -271,13 +271,14 @@ __device__ __forceinline__ bool sub_is_occluder(const CamBox &b, float fx, float
     return wpx * hpx >= occl_area * 32.0f;
 }
 
-// Occlusion test of a sub-cluster's camera-space box against the per-tile hi-Z values of the occluder phase
-// (hizt: bits of the largest stored depth per 16x16-pixel tile, 0xFFFFFFFF where background shows): true only if
-// every fragment the box can produce is strictly behind what is already drawn at every pixel it can touch, so
-// that it can never win N9 and the image stays bit-identical (N10).
+// Occlusion test of a sub-cluster's camera-space box against the hi-Z pyramid of the occluder phase (hz: bits of
+// the largest stored depth per 16x16-pixel tile, 0xFFFFFFFF where background shows; then the same per 2x2 tiles,
+// 4x4 tiles, ... level after level): true only if every fragment the box can produce is strictly behind what is
+// already drawn at every pixel it can touch, so that it can never win N9 and the image stays bit-identical (N10).
+// The level is the finest one at which the box's pixel range spans at most 2x2 entries.
 template <bool COOP>
-__device__ __forceinline__ bool box_occluded(const CamBox &b, const uint32_t *hizt, int tiles_x, float fx, float fy, int W, int H,
-                                             float znear) {
+__device__ __forceinline__ bool box_occluded(const CamBox &b, const uint32_t *hz, int tiles_x, int tiles_y, float fx, float fy,
+                                             int W, int H, float znear) {
     if (!(b.wmin >= znear)) return false;   // reaches the near plane: no screen bound
     const float xl = b.cx - b.ex, xh = b.cx + b.ex, yl = b.cy - b.ey, yh = b.cy + b.ey;
     const float iw0 = 1.0f / b.wmin, iw1 = 1.0f / b.wmax;
@@ -285,13 +286,20 @@ __device__ __forceinline__ bool box_occluded(const CamBox &b, const uint32_t *hi
     const float nyl = fy * yl * (yl >= 0.0f ? iw1 : iw0), nyh = fy * yh * (yh >= 0.0f ? iw0 : iw1);
     // pixel range, padded by one pixel for the 1/256 snap and the float error of the box arithmetic
     const float fW = (float)W, fH = (float)H;
-    const int pxl = (int)fminf(fmaxf(floorf((nxl * 0.5f + 0.5f) * fW) - 1.0f, 0.0f), fW - 1.0f);
-    const int pxh = (int)fminf(fmaxf(floorf((nxh * 0.5f + 0.5f) * fW) + 1.0f, 0.0f), fW - 1.0f);
-    const int pyl = (int)fminf(fmaxf(floorf((-nyh * 0.5f + 0.5f) * fH) - 1.0f, 0.0f), fH - 1.0f);
-    const int pyh = (int)fminf(fmaxf(floorf((-nyl * 0.5f + 0.5f) * fH) + 1.0f, 0.0f), fH - 1.0f);
-    uint32_t zb = 0;
-    for (int ty = pyl >> 4; ty <= (pyh >> 4); ++ty)
-        for (int tx = pxl >> 4; tx <= (pxh >> 4); ++tx) zb = max(zb, COOP ? __ldcg(&hizt[ty * tiles_x + tx]) : __ldg(&hizt[ty * tiles_x + tx]));
+    int tx0 = (int)fminf(fmaxf(floorf((nxl * 0.5f + 0.5f) * fW) - 1.0f, 0.0f), fW - 1.0f) >> 4;
+    int tx1 = (int)fminf(fmaxf(floorf((nxh * 0.5f + 0.5f) * fW) + 1.0f, 0.0f), fW - 1.0f) >> 4;
+    int ty0 = (int)fminf(fmaxf(floorf((-nyh * 0.5f + 0.5f) * fH) - 1.0f, 0.0f), fH - 1.0f) >> 4;
+    int ty1 = (int)fminf(fmaxf(floorf((-nyl * 0.5f + 0.5f) * fH) + 1.0f, 0.0f), fH - 1.0f) >> 4;
+    int off = 0, w = tiles_x, h = tiles_y;
+    while (tx1 - tx0 > 1 || ty1 - ty0 > 1) {
+        off += w * h;
+        w = (w + 1) >> 1; h = (h + 1) >> 1;
+        tx0 >>= 1; tx1 >>= 1; ty0 >>= 1; ty1 >>= 1;
+    }
+    const uint32_t *p = hz + off;
+    const int a00 = ty0 * w + tx0, a01 = ty0 * w + tx1, a10 = ty1 * w + tx0, a11 = ty1 * w + tx1;
+    const uint32_t zb = COOP ? max(max(__ldcg(&p[a00]), __ldcg(&p[a01])), max(__ldcg(&p[a10]), __ldcg(&p[a11])))
+                             : max(max(__ldg(&p[a00]), __ldg(&p[a01])), max(__ldg(&p[a10]), __ldg(&p[a11])));
     return b.wmin * (1.0f - 1e-4f) > __uint_as_float(zb);   // (background: NaN, the comparison is false)
 }
 

@@ -75,8 +75,8 @@ struct PipeParams {
     int32_t item_stride;     // capacity of the item list = N * item_stride
     // wave allocation
     uint32_t *rec_base;      // [N] first arena slot of the environment's segment
-    uint32_t *cnt;           // [N][2] slots used from the bottom (small) and from the top (large) of the segment
-    uint32_t *cntA;          // [N][2] the same after the occluder phase (what the second phase has to bin and draw)
+    uint32_t *cnt;           // [N] slots used of the segment
+    uint32_t *cntA;          // [N] the same after the occluder phase (the second phase bins and draws what came later)
     uint32_t *ctl;           // [C_NCTL]
     // arena
     uint4 *recs;             // [arena_slots][4]
@@ -97,7 +97,9 @@ struct PipeParams {
     float occl_area;         // a sub-cluster is an occluder if its screen box has this many pixels per triangle
     unsigned long long *keys;   // [N][T][256] tile keys between the two raster phases
     uint32_t *hizb;          // [N][H/4][W/8] bits of the largest depth per 8x4-pixel block after the occluder phase
-    uint32_t *hizt;          // [N][T] the same per tile
+    uint32_t *hizt;          // [N][hz_stride] the same per tile, then per 2x2 tiles, 4x4 tiles, ... up to one value for the
+                             //   frame (levels above the first are zeroed before the call and built with atomicMax)
+    int32_t hz_stride;
 };
 
 template <bool COOP, typename T>
@@ -229,10 +231,8 @@ __device__ void alloc_wave(const PipeParams &PP, uint32_t e_first) {
         const uint32_t end = s_end;
         if (e < end) {
             PP.rec_base[e] = ex_u;
-            PP.cnt[2 * e] = 0;
-            PP.cnt[2 * e + 1] = 0;
-            PP.cntA[2 * e] = 0;
-            PP.cntA[2 * e + 1] = 0;
+            PP.cnt[e] = 0;
+            PP.cntA[e] = 0;
         }
         if (tid == NT - 1) s_run_u = ex_u + u;
         __syncthreads();
@@ -414,33 +414,18 @@ __device__ __forceinline__ bool narrow_setup(int X[3], int Y[3], float q[3], int
     return true;
 }
 
-// One record per lane at most (kind 0 = none, 1 = small, 2 = large; pair = a colour slot follows): the warp
-// reserves its slots with one atomic per end of the segment -- small records grow from the bottom, large ones
-// from the top -- and every lane stores its 64 (or 128) bytes and the (box, qmax) word of the side array.
-// cnt_small + cnt_large <= U by construction of U (cull_kernel), so the two ends never meet.
-__device__ __forceinline__ void emit_records(const PipeParams &PP, int env, uint32_t base, uint32_t U, int lane, int kind,
-                                             bool pair, const uint32_t w[14], const float (*oc)[3], uint32_t qmax_bits) {
-    const unsigned FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
-    const unsigned ms = __ballot_sync(FULL, kind == 1), ml = __ballot_sync(FULL, kind == 2), mp = __ballot_sync(FULL, pair);
-    if ((ms | ml) == 0u) return;
-    uint32_t bs = 0, bl = 0;
-    if (lane == 0) {
-        if (ms) bs = atomicAdd(&PP.cnt[2 * env], (unsigned)(__popc(ms) + __popc(ms & mp)));
-        if (ml) bl = atomicAdd(&PP.cnt[2 * env + 1], (unsigned)(__popc(ml) + __popc(ml & mp)));
-    }
-    bs = __shfl_sync(FULL, bs, 0);
-    bl = __shfl_sync(FULL, bl, 0);
-    if (kind == 0) return;
-    uint32_t slot;
-    if (kind == 1) slot = bs + (uint32_t)(__popc(ms & lt) + __popc(ms & mp & lt));
-    else slot = U - (bl + (uint32_t)(__popc(ml & lt) + __popc(ml & mp & lt))) - (pair ? 2u : 1u);
-    const size_t at = (size_t)base + slot;
+// One record: 64 bytes at slot `at` of the arena (128 with the colour slot of a near-clipped piece) and the (box,
+// qmax) word of the side array; bit 31 of the second word marks a record of the large path (box of big_px pixels
+// or more, or int64 edge functions).
+constexpr uint32_t BB_LARGE = 0x80000000u;
+__device__ __forceinline__ void store_record(const PipeParams &PP, size_t at, bool large, bool pair, const uint32_t w[14],
+                                             const float (*oc)[3], uint32_t qmax_bits) {
     uint4 *dst = PP.recs + at * 4;
     dst[0] = make_uint4(w[0], w[1], w[2], w[3]);
     dst[1] = make_uint4(w[4], w[5], w[6], w[7]);
     dst[2] = make_uint4(w[8], w[9], w[10], w[11]);
     dst[3] = make_uint4(w[12], w[13], 0u, 0u);
-    PP.bbs[at] = make_uint2(w[6], qmax_bits);
+    PP.bbs[at] = make_uint2(w[6], qmax_bits | (large ? BB_LARGE : 0u));
     if (pair) {
         dst[4] = make_uint4(0u, 0u, 0u, 0u);
         dst[5] = make_uint4(0u, 0u, 0u, __float_as_uint(oc[0][0]));
@@ -448,6 +433,20 @@ __device__ __forceinline__ void emit_records(const PipeParams &PP, int env, uint
         dst[7] = make_uint4(__float_as_uint(oc[1][2]), __float_as_uint(oc[2][0]), __float_as_uint(oc[2][1]), __float_as_uint(oc[2][2]));
         PP.bbs[at + 1] = make_uint2(BB_SKIP, 0u);
     }
+}
+
+// One record per lane at most (kind 0 = none, 1 = small, 2 = large; pair = a colour slot follows): the warp
+// reserves its slots with one atomic.  (Slots used <= U by construction of U, cull_kernel.)
+__device__ __forceinline__ void emit_records(const PipeParams &PP, int env, uint32_t base, int lane, int kind,
+                                             bool pair, const uint32_t w[14], const float (*oc)[3], uint32_t qmax_bits) {
+    const unsigned FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
+    const unsigned m = __ballot_sync(FULL, kind != 0), mp = __ballot_sync(FULL, pair);
+    if (m == 0u) return;
+    uint32_t bs = 0;
+    if (lane == 0) bs = atomicAdd(&PP.cnt[env], (unsigned)(__popc(m) + __popc(m & mp)));
+    bs = __shfl_sync(FULL, bs, 0);
+    if (kind == 0) return;
+    store_record(PP, (size_t)base + bs + (uint32_t)(__popc(m & lt) + __popc(m & mp & lt)), kind == 2, pair, w, oc, qmax_bits);
 }
 
 // K2 for one batch, by one warp.  sub_mask: bit r set = pass r of the triangle loop (32 consecutive triangles,
@@ -527,7 +526,12 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
     }
     __syncwarp();
 
-    // K2c: set-up of the narrow survivors, 32 at a time
+    // K2c: set-up of the narrow survivors, 32 at a time.  Their slots are reserved with one atomic for the batch;
+    // what zero-area triangles leave unused is marked as skipped.
+    uint32_t bs0 = 0;
+    if (lane == 0 && nsurv) bs0 = atomicAdd(&PP.cnt[env], (unsigned)nsurv);
+    bs0 = __shfl_sync(FULL, bs0, 0);
+    int used = 0;
     for (int g0 = 0; g0 < nsurv; g0 += 32) {
         const bool have = g0 + lane < nsurv;
         uint32_t w[14];
@@ -557,8 +561,11 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                 if (STATS) ++n_tri;
             }
         }
-        emit_records(PP, env, base, U, lane, kind, false, w, nullptr, qmax_bits);
+        const unsigned mg = __ballot_sync(FULL, kind != 0);
+        if (kind) store_record(PP, (size_t)base + bs0 + (uint32_t)(used + __popc(mg & lt)), kind == 2, false, w, nullptr, qmax_bits);
+        used += __popc(mg);
     }
+    for (int k = used + lane; k < nsurv; k += 32) PP.bbs[(size_t)base + bs0 + (uint32_t)k] = make_uint2(BB_SKIP, 0u);
 
     // slow path: wide triangles and near-plane straddlers (N4), piece by piece
     for (int g = 0; g < nslow; g += 32) {
@@ -636,7 +643,7 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                     }
                 }
             }
-            emit_records(PP, env, base, U, lane, kind, pair, w, oc, qmax_bits);
+            emit_records(PP, env, base, lane, kind, pair, w, oc, qmax_bits);
         }
     }
     __syncwarp();
@@ -649,8 +656,8 @@ __device__ __forceinline__ bool sub_hidden(const PipeParams &PP, const GxCluster
     float M[12];
 #pragma unroll
     for (int k = 0; k < 12; ++k) M[k] = ldi<COOP>(&MV[k]);
-    return box_occluded<COOP>(cluster_box(sb, M), PP.hizt + (size_t)e * (size_t)PP.T, PP.tiles_x, PP.g.fx, PP.g.fy, PP.g.W, PP.g.H,
-                              PP.g.znear);
+    return box_occluded<COOP>(cluster_box(sb, M), PP.hizt + (size_t)e * (size_t)PP.hz_stride, PP.tiles_x, PP.tiles_y, PP.g.fx, PP.g.fy,
+                              PP.g.W, PP.g.H, PP.g.znear);
 }
 
 // The geometry stage: every warp draws items of the call's list until it is exhausted; items of environments
@@ -742,7 +749,7 @@ __global__ void __launch_bounds__(WARPS * 32, GEOM_MINB) geom_kernel(const PipeP
 // K3: binning.  One CTA per environment at a time.
 //   small records: count -> exclusive scan -> fill into per-(tile, depth bucket) lists of record indices at the
 //     bottom of the environment's reference area (exact sizes, nothing can overflow);
-//   large records: one 16-byte entry each -- (slot | wide << 31, 64-bit mask of the cells of the frame some pixel
+//   large records (bit 31 of the second word of the side array): one 16-byte entry each -- (slot | wide << 31, 64-bit mask of the cells of the frame some pixel
 //     of the triangle can fall in, bits of the largest q) -- sorted front to back by a counting sort over NLB
 //     depth buckets, at the top of the reference area (entry i at uint4 index U - 1 - i).  A cell is a tile
 //     (frames of at most 64 tiles) or 2x2 tiles; a cell is left out when some edge function is negative at all
@@ -812,8 +819,8 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
         __syncthreads();
         const uint32_t env = s_env;
         if (env >= e1) break;
-        const uint32_t ns = ldi<COOP>(&PP.cnt[2 * env]), nl = ldi<COOP>(&PP.cnt[2 * env + 1]);
-        const uint32_t s_lo = phase == 2 ? ldi<COOP>(&PP.cntA[2 * env]) : 0u, l_lo = phase == 2 ? ldi<COOP>(&PP.cntA[2 * env + 1]) : 0u;
+        const uint32_t ns = ldi<COOP>(&PP.cnt[env]);
+        const uint32_t s_lo = phase == 2 ? ldi<COOP>(&PP.cntA[env]) : 0u;
         const uint32_t U = ldi<COOP>(&PP.U[env]);
         const size_t base = ldi<COOP>(&PP.rec_base[env]);
         const uint2 *ebb = PP.bbs + base;
@@ -824,19 +831,16 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
         if (tid < NCLASS) s_ccnt[tid] = 0;
         if (tid < NLB) s_lcnt[tid] = 0;
         __syncthreads();
-        // count: small records per (tile, bucket), large records per bucket (slot U - 1 - k is the k-th large record)
+        // count: small records per (tile, bucket), large records per bucket
         for (uint32_t s = s_lo + tid; s < ns; s += NT) {
             const uint2 b = ldi<COOP>(&ebb[s]);
             if (b.x == BB_SKIP) continue;
+            if (b.y & BB_LARGE) { atomicAdd(&s_lcnt[depth_bucket(PP, b.y & ~BB_LARGE, NLB, sc_large)], 1u); continue; }
             const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
             const int i1 = i0 + (int)((b.x >> 16) & 255u), j1 = j0 + (int)(b.x >> 24);
             const int bk = depth_bucket(PP, b.y, NBUCKET, sc_small);
             for (int ty = j0 >> 4; ty <= (j1 >> 4); ++ty)
                 for (int tx = i0 >> 4; tx <= (i1 >> 4); ++tx) atomicAdd(&s_cnt[(ty * PP.tiles_x + tx) * NBUCKET + bk], 1u);
-        }
-        for (uint32_t k = l_lo + tid; k < nl; k += NT) {
-            const uint2 b = ldi<COOP>(&ebb[U - 1 - k]);
-            if (b.x != BB_SKIP) atomicAdd(&s_lcnt[depth_bucket(PP, b.y, NLB, sc_large)], 1u);
         }
         __syncthreads();
         if (tid == 0) {
@@ -891,7 +895,7 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
         if (tid == 0) {
             PP.tile_off[(size_t)env * (size_t)(NK + 1) + NK] = run;
             PP.n_large[env] = n_large;
-            if (phase == 1) { PP.cntA[2 * env] = ns; PP.cntA[2 * env + 1] = nl; }
+            if (phase == 1) PP.cntA[env] = ns;
             if (STATS) {
                 atomicAdd(&PP.g.stats[GX_STAT_REFS], (unsigned long long)run);
                 atomicAdd(&PP.g.stats[GX_STAT_LARGE], (unsigned long long)n_large);
@@ -902,6 +906,15 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
         for (uint32_t s = s_lo + tid; s < ns; s += NT) {
             const uint2 b = ldi<COOP>(&ebb[s]);
             if (b.x == BB_SKIP) continue;
+            if (b.y & BB_LARGE) {
+                const uint32_t qb = b.y & ~BB_LARGE;
+                const int bk = depth_bucket(PP, qb, NLB, sc_large);
+                bool wide;
+                const unsigned long long m = large_mask<COOP>(PP, env_recs + (size_t)s * 4, b.x, wide);
+                const uint32_t at = s_loff[bk] + atomicAdd(&s_lcnt[bk], 1u);
+                elarge[U - 1 - at] = make_uint4(s | (wide ? 0x80000000u : 0u), (uint32_t)m, (uint32_t)(m >> 32), qb);
+                continue;
+            }
             const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
             const int i1 = i0 + (int)((b.x >> 16) & 255u), j1 = j0 + (int)(b.x >> 24);
             const int bk = depth_bucket(PP, b.y, NBUCKET, sc_small);
@@ -910,16 +923,6 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
                     const int key = (ty * PP.tiles_x + tx) * NBUCKET + bk;
                     erefs[s_off[key] + atomicAdd(&s_cnt[key], 1u)] = s;
                 }
-        }
-        for (uint32_t k = l_lo + tid; k < nl; k += NT) {
-            const uint32_t slot = U - 1 - k;
-            const uint2 b = ldi<COOP>(&ebb[slot]);
-            if (b.x == BB_SKIP) continue;
-            const int bk = depth_bucket(PP, b.y, NLB, sc_large);
-            bool wide;
-            const unsigned long long m = large_mask<COOP>(PP, env_recs + (size_t)slot * 4, b.x, wide);
-            const uint32_t at = s_loff[bk] + atomicAdd(&s_lcnt[bk], 1u);
-            elarge[U - 1 - at] = make_uint4(slot | (wide ? 0x80000000u : 0u), (uint32_t)m, (uint32_t)(m >> 32), b.y);
         }
     }
 }
@@ -1582,7 +1585,16 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
                 if (lane == b) __stcg(&ghzb[(ty * 4 + (b >> 1)) * hzb_w + tx * 2 + (b & 1)], zb);
                 tz = max(tz, zb);
             }
-            if (lane == 0) __stcg(&PP.hizt[(size_t)env * (size_t)T + tile], tz);
+            if (lane == 0) {
+                uint32_t *hp = PP.hizt + (size_t)env * (size_t)PP.hz_stride;
+                __stcg(&hp[tile], tz);
+                int off = T, w = PP.tiles_x, h = PP.tiles_y;
+                for (int l = 1; w > 1 || h > 1; ++l) {
+                    w = (w + 1) >> 1; h = (h + 1) >> 1;
+                    atomicMax(&hp[off + (ty >> l) * w + (tx >> l)], tz);
+                    off += w * h;
+                }
+            }
             __syncwarp();
             continue;
         }
