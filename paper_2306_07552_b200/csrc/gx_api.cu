@@ -82,7 +82,7 @@ struct GxScene {
     int max_smem_optin = 0;
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
     // options (gx_set_option)
-    int opt_cull = 1, opt_subcull = 1, opt_stats = 0, opt_hiz = 1, opt_big_px = gx::TILE;
+    int opt_cull = 1, opt_subcull = 1, opt_stats = 0, opt_hiz = 1, opt_big_px = 24;
     int opt_occlusion = -1;             // occluder scheme: 1 on, 0 off, -1 automatic (on for frames of at least 8192 pixels)
     int opt_occl_area = 64;             // pixels per triangle of a sub-cluster's screen box that make it an occluder
     int64_t opt_pool_bytes = 0;         // arena budget; 0 = 4 GB
@@ -374,7 +374,7 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
         return GX_OK;
     }
     if (!strcmp(name, "big_px")) {
-        if (value < 1 || value > gx::TILE) return fail(GX_ERR_INVALID_ARG, "big_px must be in [1, %d]", gx::TILE);
+        if (value < 1 || value > 2 * gx::TILE) return fail(GX_ERR_INVALID_ARG, "big_px must be in [1, %d]", 2 * gx::TILE);   // (a box below 32 pixels touches at most 3x3 tiles)
         sc->opt_big_px = (int)value;
         return GX_OK;
     }

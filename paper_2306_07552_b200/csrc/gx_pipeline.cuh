@@ -807,9 +807,10 @@ __device__ __forceinline__ unsigned long long large_mask(const PipeParams &PP, c
 
 template <bool COOP, bool STATS>
 __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt, uint32_t *s_off, int phase) {
-    __shared__ uint32_t s_env, s_wtot[32], s_ccnt[NCLASS], s_cbase[NCLASS], s_lcnt[NLB], s_loff[NLB];
+    constexpr int LCAP = 1536;   // large records listed in shared memory between the two passes
+    __shared__ uint32_t s_env, s_wtot[32], s_ccnt[NCLASS], s_cbase[NCLASS], s_lcnt[NLB], s_loff[NLB], s_nl, s_llist[LCAP];
     const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5;
-    const int T = PP.T, NK = T * NBUCKET;
+    const int T = PP.T, NK = T * NBUCKET;     // (T <= NT in every supported frame size: thread t takes tile t)
     const int pi = phase == 2 ? 1 : 0;
     const uint32_t e0 = ldi<COOP>(&PP.ctl[C_WAVE_E0]), e1 = ldi<COOP>(&PP.ctl[C_WAVE_E1]);
     const float sc_small = PP.bucket_scale, sc_large = PP.bucket_scale * (float)NLB / (float)NBUCKET;
@@ -827,35 +828,46 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
         const uint4 *env_recs = PP.recs + base * 4;
         uint32_t *erefs = PP.refs + 4 * base;
         uint4 *elarge = reinterpret_cast<uint4 *>(erefs);
-        for (int k = tid; k < NK; k += NT) s_cnt[k] = 0;
-        if (tid < NCLASS) s_ccnt[tid] = 0;
-        if (tid < NLB) s_lcnt[tid] = 0;
-        __syncthreads();
-        // count: small records per (tile, bucket), large records per bucket
-        for (uint32_t s = s_lo + tid; s < ns; s += NT) {
-            const uint2 b = ldi<COOP>(&ebb[s]);
-            if (b.x == BB_SKIP) continue;
-            if (b.y & BB_LARGE) { atomicAdd(&s_lcnt[depth_bucket(PP, b.y & ~BB_LARGE, NLB, sc_large)], 1u); continue; }
-            const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
-            const int i1 = i0 + (int)((b.x >> 16) & 255u), j1 = j0 + (int)(b.x >> 24);
-            const int bk = depth_bucket(PP, b.y, NBUCKET, sc_small);
-            for (int ty = j0 >> 4; ty <= (j1 >> 4); ++ty)
-                for (int tx = i0 >> 4; tx <= (i1 >> 4); ++tx) atomicAdd(&s_cnt[(ty * PP.tiles_x + tx) * NBUCKET + bk], 1u);
-        }
-        __syncthreads();
-        if (tid == 0) {
-            uint32_t run = 0;
-            for (int k = 0; k < NLB; ++k) { s_loff[k] = run; run += s_lcnt[k]; s_lcnt[k] = 0; }
-            s_wtot[31] = run;   // (number of large entries; read below after the next barrier)
-        }
-        __syncthreads();
-        const uint32_t n_large = s_wtot[31];
-        __syncthreads();
-        // exclusive scan over (tile, bucket); thread t takes tile t's buckets
-        uint32_t run = 0;
-        for (int t0 = 0; t0 < T; t0 += NT) {
-            const int t = t0 + tid;
-            uint32_t v[NBUCKET], sum = 0;
+        // Records of the small path reference every tile their box touches: at most 2x2 tiles for boxes below 16
+        // pixels, so 4 words per slot always hold them; boxes up to big_px (< 32) pixels can touch 3x3.  If the exact
+        // count of a first attempt does not fit the environment's reference area, the boxes of 16 pixels and more
+        // join the large records and the count is taken again (which then fits by the 2x2 argument).
+        bool mid_large = false;
+        uint32_t n_large = 0, run = 0, sum = 0;
+        auto is_large = [&](const uint2 &b) {
+            return (b.y & BB_LARGE) != 0u || (mid_large && ((b.x >> 16) & 255u) >= 16u) || (mid_large && (b.x >> 24) >= 16u);
+        };
+        for (int attempt = 0; attempt < 2; ++attempt) {
+            for (int k = tid; k < NK; k += NT) s_cnt[k] = 0;
+            if (tid < NLB) s_lcnt[tid] = 0;
+            if (tid == 0) s_nl = 0;
+            __syncthreads();
+            // count: small records per (tile, bucket), large records per bucket
+            for (uint32_t s = s_lo + tid; s < ns; s += NT) {
+                const uint2 b = ldi<COOP>(&ebb[s]);
+                if (b.x == BB_SKIP) continue;
+                if (is_large(b)) {   // listed, so that the second pass works on them with every lane
+                    atomicAdd(&s_lcnt[depth_bucket(PP, b.y & ~BB_LARGE, NLB, sc_large)], 1u);
+                    const uint32_t k = atomicAdd(&s_nl, 1u);
+                    if (k < (uint32_t)LCAP) s_llist[k] = s;
+                    continue;
+                }
+                const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
+                const int i1 = i0 + (int)((b.x >> 16) & 255u), j1 = j0 + (int)(b.x >> 24);
+                const int bk = depth_bucket(PP, b.y, NBUCKET, sc_small);
+                for (int ty = j0 >> 4; ty <= (j1 >> 4); ++ty)
+                    for (int tx = i0 >> 4; tx <= (i1 >> 4); ++tx) atomicAdd(&s_cnt[(ty * PP.tiles_x + tx) * NBUCKET + bk], 1u);
+            }
+            __syncthreads();
+            n_large = s_nl;
+            if (tid == 0) {
+                uint32_t r = 0;
+                for (int k = 0; k < NLB; ++k) { s_loff[k] = r; r += s_lcnt[k]; s_lcnt[k] = 0; }
+            }
+            // exclusive scan over (tile, bucket); thread t takes tile t's buckets
+            const int t = tid;
+            uint32_t v[NBUCKET];
+            sum = 0;
 #pragma unroll
             for (int k = 0; k < NBUCKET; ++k) { v[k] = t < T ? s_cnt[t * NBUCKET + k] : 0u; sum += v[k]; }
             uint32_t inc = sum;
@@ -866,32 +878,33 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
             }
             if (lane == 31) s_wtot[warp] = inc;
             __syncthreads();
-            uint32_t ex = run + inc - sum;
+            uint32_t ex = inc - sum;
             for (int w = 0; w < warp; ++w) ex += s_wtot[w];
-            uint32_t tot = 0;
-            for (int w = 0; w < (NT >> 5); ++w) tot += s_wtot[w];
+            run = 0;
+            for (int w = 0; w < (NT >> 5); ++w) run += s_wtot[w];
             if (t < T) {
                 uint32_t *g_off = PP.tile_off + (size_t)env * (size_t)(NK + 1) + (size_t)t * NBUCKET;
 #pragma unroll
                 for (int k = 0; k < NBUCKET; ++k) { s_off[t * NBUCKET + k] = ex; g_off[k] = ex; s_cnt[t * NBUCKET + k] = 0; ex += v[k]; }
-                // the tile's raster task, filed under its cost class: references of the tile, plus a share of the
-                // large records
-                const uint32_t cost = sum + (n_large >> 2) + 8u;
-                const int c = min(NCLASS - 1, 28 - __clz((int)cost));
-                v[0] = (uint32_t)c | (atomicAdd(&s_ccnt[c], 1u) << 8);
             }
-            run += tot;
             __syncthreads();
-            if (t0 + NT >= T) {   // last chunk: reserve this environment's range of every class list
-                if (tid < NCLASS && s_ccnt[tid]) s_cbase[tid] = atomicAdd(&PP.ctl[C_TASK_CNT + pi * NCLASS + tid], s_ccnt[tid]);
-                __syncthreads();
-            }
-            // (T <= NT in every supported frame size, so the class bases are ready for the tile written below)
-            if (t < T) {
-                const uint32_t c = v[0] & 255u, pos = v[0] >> 8;
-                PP.tasks[(size_t)c * (size_t)PP.g.N * (size_t)T + s_cbase[c] + pos] = env * (uint32_t)T + (uint32_t)t;
-            }
+            if ((unsigned long long)run + 4ull * n_large <= 4ull * U) break;   // (uniform) the references fit
+            mid_large = true;
         }
+        // every tile is a raster task, filed under its cost class: references of the tile, plus a share of the
+        // large records
+        if (tid < NCLASS) s_ccnt[tid] = 0;
+        __syncthreads();
+        uint32_t my_class = 0, my_pos = 0;
+        if (tid < T) {
+            const uint32_t cost = sum + (n_large >> 2) + 8u;
+            my_class = (uint32_t)min(NCLASS - 1, 28 - __clz((int)cost));
+            my_pos = atomicAdd(&s_ccnt[my_class], 1u);
+        }
+        __syncthreads();
+        if (tid < NCLASS && s_ccnt[tid]) s_cbase[tid] = atomicAdd(&PP.ctl[C_TASK_CNT + pi * NCLASS + tid], s_ccnt[tid]);
+        __syncthreads();
+        if (tid < T) PP.tasks[(size_t)my_class * (size_t)PP.g.N * (size_t)T + s_cbase[my_class] + my_pos] = env * (uint32_t)T + (uint32_t)tid;
         if (tid == 0) {
             PP.tile_off[(size_t)env * (size_t)(NK + 1) + NK] = run;
             PP.n_large[env] = n_large;
@@ -901,18 +914,21 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
                 atomicAdd(&PP.g.stats[GX_STAT_LARGE], (unsigned long long)n_large);
             }
         }
-        __syncthreads();
         // fill
+        const bool listed = n_large <= (uint32_t)LCAP;
+        auto fill_large = [&](uint32_t s, const uint2 &b) {
+            const uint32_t qb = b.y & ~BB_LARGE;
+            const int bk = depth_bucket(PP, qb, NLB, sc_large);
+            bool wide;
+            const unsigned long long m = large_mask<COOP>(PP, env_recs + (size_t)s * 4, b.x, wide);
+            const uint32_t at = s_loff[bk] + atomicAdd(&s_lcnt[bk], 1u);
+            elarge[U - 1 - at] = make_uint4(s | (wide ? 0x80000000u : 0u), (uint32_t)m, (uint32_t)(m >> 32), qb);
+        };
         for (uint32_t s = s_lo + tid; s < ns; s += NT) {
             const uint2 b = ldi<COOP>(&ebb[s]);
             if (b.x == BB_SKIP) continue;
-            if (b.y & BB_LARGE) {
-                const uint32_t qb = b.y & ~BB_LARGE;
-                const int bk = depth_bucket(PP, qb, NLB, sc_large);
-                bool wide;
-                const unsigned long long m = large_mask<COOP>(PP, env_recs + (size_t)s * 4, b.x, wide);
-                const uint32_t at = s_loff[bk] + atomicAdd(&s_lcnt[bk], 1u);
-                elarge[U - 1 - at] = make_uint4(s | (wide ? 0x80000000u : 0u), (uint32_t)m, (uint32_t)(m >> 32), qb);
+            if (is_large(b)) {
+                if (!listed) fill_large(s, b);
                 continue;
             }
             const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
@@ -924,6 +940,11 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
                     erefs[s_off[key] + atomicAdd(&s_cnt[key], 1u)] = s;
                 }
         }
+        if (listed)
+            for (uint32_t k = tid; k < n_large; k += NT) {
+                const uint32_t s = s_llist[k];
+                fill_large(s, ldi<COOP>(&ebb[s]));
+            }
     }
 }
 

@@ -292,6 +292,34 @@ def test_random_soup_large_triangles(oracle_mod):
     assert (o["id"][o["id"] != BG] < 300).all()        # lower id wins every exact tie
 
 
+def test_reference_area_fallback(oracle_mod):
+    """Records of 17..31 pixels reference up to 3x3 tiles; when the exact count does not fit the environment's
+    reference area (4 words per record slot) the bin stage sends them down the large path instead.  300 stacked
+    triangles whose boxes all span pixels 15..45 of a 64x64 frame (9 tiles each, no slot to spare) force that;
+    big_px = 16 never needs it.  All three renders equal the oracle."""
+    nt, W = 300, 64
+    pos = np.zeros((nt * 3, 3), np.float32)
+    for i in range(nt):
+        d = 2.0 + 0.01 * i
+        for k, (px, py) in enumerate(((15.3, 15.3), (45.7, 15.3), (15.3, 45.7))):
+            pos[3 * i + k] = ((px / 32.0 - 1.0) * d, -(py / 32.0 - 1.0) * d, -d)
+    rng = np.random.Generator(np.random.Philox(key=[78, 100]))
+    col = rng.integers(0, 256, (nt * 3, 3)).astype(np.uint8)
+    m = gen.Mesh(pos, col, np.arange(nt * 3, dtype=np.uint32).reshape(nt, 3))
+    cam = np.eye(4, dtype=np.float32).reshape(1, 16)
+    wl = gen.Workload("stack", W, W, 1.0, 1.0, 0.1, 20.0, [m], [], np.zeros(1, np.int32), cam,
+                      np.zeros((1, 0), np.int32), np.zeros((1, 0, 16), np.float32))
+    o = oracle_mod.render(wl)
+    for opts in ({"hiz": 0}, {"hiz": 0, "big_px": 16}, {}):
+        g = render_gpu(wl, stats=True, options=opts)
+        rep = compare(o, g)
+        assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, (opts, rep)
+        if opts == {"hiz": 0}:                       # fell back: every record on the large path, no tile references
+            assert g["stats"]["tile_refs"] == 0 and g["stats"]["large_records"] == nt, g["stats"]
+        if opts.get("big_px") == 16:
+            assert g["stats"]["large_records"] == nt
+
+
 def test_argument_errors():
     import torch
     from paper_2306_07552_b200 import binding as gx
