@@ -117,10 +117,11 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def load_workload(cfg: int, n_envs: int):
+def load_workload(cfg: int, n_envs: int, rank: int = 0):
+    """Rank r renders its own environments: ids r*n .. (r+1)*n - 1 of the config's recipe (weak scaling)."""
     from paper_2306_07552_b200 import gen
-    wl = gen.make_config(cfg, n_envs=n_envs or None)
-    return wl
+    n = n_envs or gen.CONFIG_SHAPES[cfg][1]
+    return gen.make_config(cfg, env_ids=rank * n + np.arange(n), beyond=rank > 0)
 
 
 def workload_name(cfg: int, wl) -> str:
@@ -145,8 +146,13 @@ def time_oracle(wl, budget_s: float = 15.0):
     for _ in range(reps):
         oracle.render(sample, n_threads=cores)
     dt = time.perf_counter() - t0
+    # the same oracle on one core, on a smaller sample (about 3 s)
+    S1 = int(min(S, max(4, rate / cores * 3.0)))
+    one = wl.subset(np.arange(S1))
+    t1 = time.perf_counter(); oracle.render(one, n_threads=1); dt1 = time.perf_counter() - t1
     return {"value": S * reps / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"first {S} of {wl.N} envs x {reps} passes, {dt:.1f} s wall, OpenMP over envs"}
+            "sample": f"first {S} of {wl.N} envs x {reps} passes, {dt:.1f} s wall, OpenMP over envs",
+            "value_1core": S1 / dt1, "sample_1core": f"first {S1} envs, 1 thread, {dt1:.1f} s wall"}
 
 
 def run_reference(args):
@@ -192,6 +198,10 @@ def run_gx(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the render path has no CPU fallback)")
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
+    if torch.cuda.device_count() <= local:
+        raise SystemExit(f"bench.py: rank {rank} needs cuda:{local} but only {torch.cuda.device_count()} device(s) are visible")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
@@ -207,7 +217,7 @@ def run_gx(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = load_workload(args.config, args.envs)
+    wl = load_workload(args.config, args.envs, rank)
     N, K, H, W = wl.N, wl.K, wl.height, wl.width
     scene = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, local)
     for o in args.opt:
@@ -257,6 +267,11 @@ def run_gx(args):
     total_ms = float(sum(ms))
     launches = gx.gx_get_stat(scene, "launches")
     total_ms_max = sharding.max_over_ranks(total_ms, dev)        # time of the job = the slowest rank's
+    per_rank_ms = [total_ms / args.steps]
+    if world > 1:
+        t_all = [torch.zeros(1, dtype=torch.float64, device=dev) for _ in range(world)]
+        dist.all_gather(t_all, torch.tensor([total_ms / args.steps], dtype=torch.float64, device=dev))
+        per_rank_ms = [float(t.item()) for t in t_all]
     ms_per_step = total_ms_max / args.steps
     value = world * N * args.steps / (total_ms_max * 1e-3)
 
@@ -304,40 +319,47 @@ def run_gx(args):
     bytes_per_launch = float(b["total"].sum())
     kernels_ms = {k: v * 1e-6 / max(timed_calls, 1) for k, v in kernel_ns.items()}
     kernel_ms = sum(kernels_ms.values()) if timed_calls else total_ms / args.steps
-    achieved = bytes_per_launch / (kernel_ms * 1e-3) / 1e9
-    traffic = None      # DRAM bytes per launch of all our kernels, from the committed ncu capture of this workload
+    step_ms = total_ms / args.steps                       # this rank's step, memsets and launch gaps included
+    achieved = bytes_per_launch / (step_ms * 1e-3) / 1e9
+    achieved_kernels = bytes_per_launch / (kernel_ms * 1e-3) / 1e9
+    # DRAM bytes per launch of all our kernels: not measured in this run (ncu replays kernels); taken from the
+    # committed ncu capture of the same workload, whose header names the commit it was captured at
+    traffic, traffic_src = None, None
     try:
         import csv
-        with open(os.path.join(ROOT, "profiles", "r1g_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as f:
             rows = [r for r in csv.DictReader(f) if int(r["workload_config"]) == args.config]
-        if rows and not args.opt and not args.envs:
+        if rows and not args.opt and not args.envs and not args.obs:
             traffic = float(sum(int(r["dram_bytes_per_launch"]) for r in rows))
+            traffic_src = "profiles/r2_traffic.csv (ncu --set full capture; commit in profiles/r2_pipeline_ncu.md)"
     except Exception:
         pass
     dom = max(kernels_ms, key=kernels_ms.get) if timed_calls else "raster"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": traffic, "peak_source": peak_src,
-                "kernel": "gx pipeline: cull_kernel + geom_kernel + bin_kernel + raster_kernel + tail_kernel",
-                "kernel_ms": kernel_ms, "kernels_ms": kernels_ms,
+                "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                "kernel": "gx pipeline: cull_kernel + 2 x (geom_kernel + bin_kernel + raster_kernel) + tail_kernel",
+                "step_ms": step_ms, "kernel_ms": kernel_ms, "kernels_ms": kernels_ms,
+                "achieved_over_kernel_ms": achieved_kernels, "frac_over_kernel_ms": achieved_kernels / peak,
                 "dominant_kernel": {"name": "gx::" + dom + "_kernel", "ms": kernels_ms.get(dom),
                                     "share_of_kernel_time": (kernels_ms.get(dom, 0.0) / kernel_ms) if kernel_ms else None},
                 "algorithmic_bytes_per_launch": bytes_per_launch,
                 "bytes_per_env": {k: float(b[k].mean()) for k in ("cull", "geom", "out", "total")},
                 "post_cull_tris_per_env": float(b["tris"].mean()),
                 "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
-                "note": "issue-bound, not DRAM-bound: see DESIGN.md section 7"}
+                "note": "frac = algorithmic bytes / whole step time; issue- and latency-bound, not DRAM-bound: DESIGN.md section 7"}
     cpu = None if args.no_cpu_baseline else time_oracle(wl)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_name(args.config, wl), "envs_per_gpu": N, "width": W, "height": H,
+        "config": {"workload": workload_name(args.config, wl), "envs_per_gpu": N, "env_ids": f"rank r renders ids r*{N} .. (r+1)*{N}-1", "width": W, "height": H,
                    "instances_per_env": K, "tris_per_env": float(wl.tris_per_env().mean()),
                    "outputs": "obs f16 [N,4,H,W] (gx_render_batch_obs)" if args.obs else
                               ("depth f32" if wl.depth_only else "rgb u8 + depth f32"),
                    "l2": "256 MB buffer written between timed iterations (untimed)",
                    "arithmetic": "f32 vertex stage, i32/i64 fixed-point coverage, f32 depth/colour"},
-        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches) * args.steps,
+        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches) * args.steps * world,
+        "ms_per_step_per_rank": per_rank_ms,
         "roofline": roofline, "cpu_baseline": cpu,
     }
     print(json.dumps(out), flush=True)
@@ -350,6 +372,15 @@ def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under torchrun: start one rank per GPU ourselves; refuse rather than quietly run on fewer devices
+        import torch
+        from paper_2306_07552_b200 import build as gx_build, sharding
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but only {have} CUDA device(s) are visible")
+        gx_build.build()
+        sharding.spawn_ranks(args.gpus, run_gx, (args,))
     else:
         run_gx(args)
 

@@ -606,16 +606,18 @@ def _config_rooms(cfg: int, env_ids: np.ndarray) -> Workload:
                     dict(scene_info=[i for _, i in scenes]))
 
 
-def make_config(cfg: int, n_envs: Optional[int] = None, env_ids: Optional[Sequence[int]] = None) -> Workload:
+def make_config(cfg: int, n_envs: Optional[int] = None, env_ids: Optional[Sequence[int]] = None,
+                beyond: bool = False) -> Workload:
     """Workload `cfg` (0-4) of BASELINE.json.  n_envs: first n environments; env_ids: explicit subset
     (each environment is generated from its own stream, so a subset equals the same rows of the full
-    config)."""
+    config).  beyond: allow environment ids past the config's N -- more environments of the same
+    recipe, e.g. rank r of a weak-scaling run renders ids r*N .. (r+1)*N - 1."""
     if cfg not in CONFIG_SHAPES:
         raise ValueError(f"unknown config {cfg}")
     N = CONFIG_SHAPES[cfg][1]
     if env_ids is None:
         env_ids = np.arange(N if n_envs is None else min(n_envs, N))
     env_ids = np.asarray(env_ids, np.int64)
-    if env_ids.size and (env_ids.min() < 0 or env_ids.max() >= N):
+    if env_ids.size and (env_ids.min() < 0 or (env_ids.max() >= N and not beyond) or env_ids.max() >= 2 ** 40):
         raise ValueError("env id out of range")
     return _config0(env_ids) if cfg == 0 else _config_rooms(cfg, env_ids)

@@ -40,3 +40,24 @@ def gather_shards(local, n: int):
     out = [torch.empty_like(buf) for _ in range(world)]
     dist.all_gather(out, buf)
     return torch.cat([o[:e - b] for o, (b, e) in zip(out, sizes)], dim=0)
+
+
+def _rank_main(rank: int, world: int, port: int, target, args) -> None:
+    import os
+    os.environ.update({"RANK": str(rank), "LOCAL_RANK": str(rank), "WORLD_SIZE": str(world),
+                       "MASTER_ADDR": "127.0.0.1", "MASTER_PORT": str(port)})
+    target(*args)
+
+
+def spawn_ranks(world: int, target, args=()) -> None:
+    """Start `world` processes on this node, one per GPU, each with the RANK / LOCAL_RANK / WORLD_SIZE /
+    MASTER_* environment torchrun would give it, run target(*args) in every one and wait for all of them
+    (what `bench.py --gpus N` does when it was not started under torchrun).  Raises if a rank fails."""
+    import socket
+    import torch.multiprocessing as mp
+    if world < 1:
+        raise ValueError("world must be >= 1")
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    mp.spawn(_rank_main, args=(world, port, target, tuple(args)), nprocs=world, join=True)

@@ -64,3 +64,42 @@ def test_two_rank_sharded_render_matches_single(tmp_path, oracle_mod):
     assert np.array_equal(got["id"], ref["id"])
     assert np.array_equal(got["rgb"], ref["rgb"])
     assert float(got["t"]) == 11.0
+
+
+def _stub_rank(out_dir):
+    """What bench.py's ranks do around the render step, with a stub step: read the torchrun-style environment,
+    join the process group, reduce a per-rank time with max, pick this rank's environments."""
+    sys.path.insert(0, ROOT)
+    import torch.distributed as dist
+    from paper_2306_07552_b200.sharding import max_over_ranks
+    rank, world, local = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"]), int(os.environ["LOCAL_RANK"])
+    assert os.environ["MASTER_ADDR"] == "127.0.0.1" and local == rank
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        import bench
+        wl = bench.load_workload(0, 2, rank)           # rank r renders environments 2r, 2r+1 of the recipe
+        t = max_over_ranks(1.0 + rank)
+        with open(os.path.join(out_dir, f"rank{rank}.txt"), "w") as f:
+            f.write(f"{world} {t} {' '.join(str(int(i)) for i in wl.env_ids)}")
+    finally:
+        dist.destroy_process_group()
+
+
+def test_spawn_ranks_gives_each_rank_its_environment(tmp_path):
+    """sharding.spawn_ranks is what `bench.py --gpus N` uses when it is not started by torchrun."""
+    from paper_2306_07552_b200.sharding import spawn_ranks
+    spawn_ranks(2, _stub_rank, (str(tmp_path),))
+    got = [open(os.path.join(str(tmp_path), f"rank{r}.txt")).read().split() for r in range(2)]
+    assert got[0] == ["2", "2.0", "0", "1"] and got[1] == ["2", "2.0", "2", "3"]
+
+
+def test_bench_refuses_more_gpus_than_visible():
+    """`bench.py --gpus 2` must not quietly run on fewer devices (no CUDA device at all in the CPU test run)."""
+    import subprocess
+    import torch
+    if torch.cuda.device_count() >= 2:
+        pytest.skip("needs a box with fewer than 2 GPUs")
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode != 0 and "--gpus 2" in (r.stderr + r.stdout)
