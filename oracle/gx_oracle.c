@@ -30,6 +30,12 @@
  * double-precision ray casting (N8), order/id permutation invariants (N9), full-scan == bbox (N6).
  * Parity unpinned: exact RGB value where perspective correction matters beyond +-1 LSB of the
  * double-precision ray caster.
+ *
+ * Also here (end of the file): N11, the packed float16 observation, and N12, the scene-graph update (forward
+ * kinematics of the robot, Table 5) that produces the camera and link transforms
+ * the renderer reads.  N12 pins: its own sine / cosine against float64 and the exact values at 0; closed forms
+ * (joints at 0 with dyadic offsets, a quarter turn about each axis, a prismatic joint, base yaw); random
+ * chains against a float64 composition; parent / child and held-object identities.
  */
 #include <math.h>
 #include <stdint.h>
@@ -438,4 +444,124 @@ int gx_oracle_pack_obs(const uint8_t *rgb /* [N,H,W,3] */, const float *depth /*
 /* binary32 -> binary16 of an array: exposes or_half_rn to its pins */
 void gx_oracle_half_rn(const float *in, uint16_t *out, size_t n) {
     for (size_t k = 0; k < n; ++k) out[k] = or_half_rn(in[k]);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * N12: scene-graph update -- forward kinematics from base pose and joint positions to the link, camera and
+ * held-object transforms the renderer reads (N12; "we use forward kinematics
+ * to compute the position of the robot's articulated links", "Scene graph updates are communicated
+ * ... to the ... renderer", Table 5 PAPER.md:416 "Render Setup").  Plain loops, one environment after the
+ * other, link after link in index order (a parent always has a smaller index than its child).
+ * All operations are IEEE binary32; fmaf is the single-rounding fused multiply-add; nothing is contracted.
+ * ------------------------------------------------------------------------------------------------ */
+
+/* N12a: sine and cosine in binary32: Cody-Waite reduction by multiples of pi/2 in two steps, then the degree-7 /
+ * degree-8 polynomials on [-pi/4, pi/4] evaluated by Horner's rule with fmaf, then the quadrant. */
+static void n12_sincos(float x, float *s_out, float *c_out) {
+    const float k = rintf(x * 0.636619772f);               /* nearest multiple of pi/2 */
+    float r = fmaf(-k, 1.57079625f, x);                    /* pi/2 = 1.57079625 + 7.54978942e-08 (+ ...) */
+    r = fmaf(-k, 7.54978942e-08f, r);
+    const float z = r * r;
+    float ps = fmaf(z, -1.9515295891e-4f, 8.3321608736e-3f);
+    ps = fmaf(z, ps, -1.6666654611e-1f);
+    const float sn = fmaf(r * z, ps, r);                   /* sin r */
+    float pc = fmaf(z, 2.443315711809948e-5f, -1.388731625493765e-3f);
+    pc = fmaf(z, pc, 4.166664568298827e-2f);
+    const float cs = fmaf(z * z, pc, fmaf(-0.5f, z, 1.0f)); /* cos r */
+    const int q = (int)k & 3;                              /* two's complement: also right for negative k */
+    float s = (q & 1) ? cs : sn, c = (q & 1) ? sn : cs;
+    if (q == 1 || q == 2) c = -c;
+    if (q >= 2) s = -s;
+    *s_out = s;
+    *c_out = c;
+}
+
+/* affine product C = A * B of two 3x4 matrices (rows of 4, implicit last row 0 0 0 1), the operation order of N2 */
+static void n12_mul(const float *A, const float *B, float *C) {
+    for (int i = 0; i < 3; ++i) {
+        for (int j = 0; j < 3; ++j)
+            C[i * 4 + j] = fmaf(A[i * 4 + 2], B[8 + j], fmaf(A[i * 4 + 1], B[4 + j], A[i * 4] * B[j]));
+        C[i * 4 + 3] = fmaf(A[i * 4 + 2], B[11], fmaf(A[i * 4 + 1], B[7], fmaf(A[i * 4], B[3], A[i * 4 + 3])));
+    }
+}
+
+/* N12b: joint transform.  type 0 fixed: identity; 1 revolute about the unit axis a by theta (Rodrigues);
+ * 2 prismatic along a by theta. */
+static void n12_joint(int type, const float *a, float theta, float *J) {
+    for (int k = 0; k < 12; ++k) J[k] = (k % 5 == 0) ? 1.0f : 0.0f;
+    if (type == 1) {
+        float s, c;
+        n12_sincos(theta, &s, &c);
+        const float t = 1.0f - c;
+        J[0] = fmaf(t * a[0], a[0], c);
+        J[1] = fmaf(t * a[0], a[1], -(s * a[2]));
+        J[2] = fmaf(t * a[0], a[2], s * a[1]);
+        J[4] = fmaf(t * a[1], a[0], s * a[2]);
+        J[5] = fmaf(t * a[1], a[1], c);
+        J[6] = fmaf(t * a[1], a[2], -(s * a[0]));
+        J[8] = fmaf(t * a[2], a[0], -(s * a[1]));
+        J[9] = fmaf(t * a[2], a[1], s * a[0]);
+        J[10] = fmaf(t * a[2], a[2], c);
+    } else if (type == 2) {
+        J[3] = theta * a[0];
+        J[7] = theta * a[1];
+        J[11] = theta * a[2];
+    }
+}
+
+typedef struct {
+    int32_t parent;      /* index of the parent link, -1 = the base */
+    int32_t joint_type;  /* 0 fixed, 1 revolute, 2 prismatic */
+    float axis[3];       /* unit joint axis in the joint frame */
+    float origin[12];    /* 3x4: joint frame in the parent link's frame */
+} GxOracleLink;
+
+static void n12_store44(float *dst, const float *M) {
+    for (int k = 0; k < 12; ++k) dst[k] = M[k];
+    dst[12] = 0.0f; dst[13] = 0.0f; dst[14] = 0.0f; dst[15] = 1.0f;
+}
+
+/* N12c.  base_pose [N,3] = (x, z, yaw): the base stands on the ground plane y = 0 and turns about +Y.
+ * W_base = Ry(yaw) with translation (x, 0, z); W_l = W_parent(l) * (origin_l * J_l(joint_pos[n][l])).
+ * Writes inst_xform[n][link_slot0 + l] = W_l (4x4 row-major), cam_pose[n] = W_camera_link * cam_mount, and, where
+ * held_slot[n] >= 0, inst_xform[n][held_slot[n]] = W_ee_link * held_xform[n].  Other slots are left alone.
+ * Returns 0, or -1 on bad arguments. */
+int gx_oracle_fk(const GxOracleLink *links, int32_t L, int32_t camera_link, const float *cam_mount /* [12] */, int32_t ee_link,
+                 int32_t N, int32_t K, int32_t link_slot0, const float *base_pose, const float *joint_pos /* [N,L] */,
+                 const int32_t *held_slot /* [N] or NULL */, const float *held_xform /* [N,12] or NULL */,
+                 float *cam_pose /* [N,16] */, float *inst_xform /* [N,K,16] */) {
+    if (!links || L <= 0 || L > 64 || N <= 0 || !base_pose || !joint_pos || !cam_pose || !cam_mount) return -1;
+    if (camera_link < -1 || camera_link >= L || ee_link < -1 || ee_link >= L) return -1;
+    if (link_slot0 < 0 || link_slot0 + L > K || (K > 0 && !inst_xform)) return -1;
+    for (int l = 0; l < L; ++l)
+        if (links[l].parent < -1 || links[l].parent >= l) return -1;
+    for (int n = 0; n < N; ++n) {
+        float W[65][12];   /* W[0] = base, W[l + 1] = link l */
+        float s, c;
+        n12_sincos(base_pose[3 * n + 2], &s, &c);
+        const float B[12] = {c, 0.0f, s, base_pose[3 * n], 0.0f, 1.0f, 0.0f, 0.0f, -s, 0.0f, c, base_pose[3 * n + 1]};
+        for (int k = 0; k < 12; ++k) W[0][k] = B[k];
+        for (int l = 0; l < L; ++l) {
+            float J[12], Loc[12];
+            n12_joint(links[l].joint_type, links[l].axis, joint_pos[(size_t)n * L + l], J);
+            n12_mul(links[l].origin, J, Loc);
+            n12_mul(W[links[l].parent + 1], Loc, W[l + 1]);
+            n12_store44(inst_xform + ((size_t)n * K + link_slot0 + l) * 16, W[l + 1]);
+        }
+        float Cm[12];
+        n12_mul(W[camera_link + 1], cam_mount, Cm);
+        n12_store44(cam_pose + (size_t)n * 16, Cm);
+        if (held_slot && held_xform && held_slot[n] >= 0) {
+            if (held_slot[n] >= K) return -1;
+            float Hm[12];
+            n12_mul(W[ee_link + 1], held_xform + (size_t)n * 12, Hm);
+            n12_store44(inst_xform + ((size_t)n * K + held_slot[n]) * 16, Hm);
+        }
+    }
+    return 0;
+}
+
+/* N12a alone, for its pins */
+void gx_oracle_sincos(const float *x, float *s, float *c, size_t n) {
+    for (size_t i = 0; i < n; ++i) n12_sincos(x[i], &s[i], &c[i]);
 }

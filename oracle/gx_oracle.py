@@ -170,3 +170,49 @@ def half_rn(x: np.ndarray) -> np.ndarray:
     L.gx_oracle_half_rn.restype = None
     L.gx_oracle_half_rn(_p(x), _p(out), C.c_size_t(x.size))
     return out
+
+
+class _Link(C.Structure):
+    _fields_ = [("parent", C.c_int32), ("joint_type", C.c_int32), ("axis", C.c_float * 3), ("origin", C.c_float * 12)]
+
+
+def sincos(x: np.ndarray):
+    """N12a: the definition's own binary32 sine and cosine."""
+    L = _load()
+    x = np.ascontiguousarray(x, np.float32)
+    s, c = np.empty_like(x), np.empty_like(x)
+    L.gx_oracle_sincos.restype = None
+    L.gx_oracle_sincos(_p(x), _p(s), _p(c), C.c_size_t(x.size))
+    return s, c
+
+
+def fk(robot, base_pose, joint_pos, K: int, link_slot0: int, inst_xform: Optional[np.ndarray] = None,
+       held_slot: Optional[np.ndarray] = None, held_xform: Optional[np.ndarray] = None):
+    """N12: forward kinematics.  robot: any object with parent [L], joint_type [L], axis [L,3], origin [L,12],
+    camera_link, cam_mount [12], ee_link (gen.Robot).  Returns (cam_pose [N,16], inst_xform [N,K,16])."""
+    lib = _load()
+    Ln = len(robot.parent)
+    links = (_Link * Ln)()
+    for l in range(Ln):
+        links[l].parent = int(robot.parent[l])
+        links[l].joint_type = int(robot.joint_type[l])
+        for k in range(3):
+            links[l].axis[k] = float(np.float32(robot.axis[l][k]))
+        for k in range(12):
+            links[l].origin[k] = float(np.float32(np.asarray(robot.origin[l]).reshape(12)[k]))
+    base_pose = np.ascontiguousarray(base_pose, np.float32)
+    joint_pos = np.ascontiguousarray(joint_pos, np.float32)
+    N = base_pose.shape[0]
+    assert base_pose.shape == (N, 3) and joint_pos.shape == (N, Ln)
+    xf = np.zeros((N, K, 16), np.float32) if inst_xform is None else np.array(inst_xform, np.float32, copy=True).reshape(N, K, 16)
+    cam = np.empty((N, 16), np.float32)
+    mount = np.ascontiguousarray(robot.cam_mount, np.float32).reshape(12)
+    hs = None if held_slot is None else np.ascontiguousarray(held_slot, np.int32)
+    hx = None if held_xform is None else np.ascontiguousarray(held_xform, np.float32).reshape(N, 12)
+    lib.gx_oracle_fk.restype = C.c_int
+    rc = lib.gx_oracle_fk(links, C.c_int32(Ln), C.c_int32(int(robot.camera_link)), _p(mount), C.c_int32(int(robot.ee_link)),
+                          C.c_int32(N), C.c_int32(K), C.c_int32(link_slot0), _p(base_pose), _p(joint_pos), _p(hs), _p(hx),
+                          _p(cam), _p(xf))
+    if rc != 0:
+        raise ValueError("gx_oracle_fk: bad arguments")
+    return cam, xf

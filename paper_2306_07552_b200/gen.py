@@ -43,6 +43,20 @@ class Mesh:
 
 
 @dataclass
+class Robot:
+    """Description of an articulated robot for the scene-graph update (N12): data only.  Link l hangs off
+    link parent[l] < l (-1 = the base); origin[l] is the joint frame in the parent's frame (3x4), joint_type 0
+    fixed / 1 revolute / 2 prismatic about or along the unit vector axis[l]."""
+    parent: np.ndarray       # [L] int32
+    joint_type: np.ndarray   # [L] int32
+    axis: np.ndarray         # [L,3] float32
+    origin: np.ndarray       # [L,12] float32
+    camera_link: int         # link the head camera is mounted on (-1 = the base)
+    cam_mount: np.ndarray    # [12] float32: camera frame in that link's frame
+    ee_link: int             # end-effector link (carries the held object)
+
+
+@dataclass
 class Workload:
     name: str
     width: int
@@ -621,3 +635,33 @@ def make_config(cfg: int, n_envs: Optional[int] = None, env_ids: Optional[Sequen
     if env_ids.size and (env_ids.min() < 0 or (env_ids.max() >= N and not beyond) or env_ids.max() >= 2 ** 40):
         raise ValueError("env id out of range")
     return _config0(env_ids) if cfg == 0 else _config_rooms(cfg, env_ids)
+
+
+def robot_proxy() -> Robot:
+    """The 5-link robot proxy of the room configs as a kinematic chain (stands in for the paper's Fetch: mobile
+    base, lift, arm, head camera): base box -> torso (prismatic lift along +Y) -> upper arm
+    (revolute about X at the shoulder) -> forearm (revolute about X at the elbow) -> hand (revolute about Y);
+    the head camera sits on the torso at 1.2 m and looks along -Z, pitched down a little."""
+    def T(x, y, z):
+        return [1, 0, 0, x, 0, 1, 0, y, 0, 0, 1, z]
+    parent = np.array([-1, 0, 1, 2, 3], np.int32)
+    joint_type = np.array([0, 2, 1, 1, 1], np.int32)
+    axis = np.array([[0, 1, 0], [0, 1, 0], [1, 0, 0], [1, 0, 0], [0, 1, 0]], np.float32)
+    origin = np.array([T(0, 0.25, 0), T(0, 0.45, 0), T(0.2, 0.25, -0.15), T(0, 0, -0.35), T(0, 0, -0.3)], np.float32)
+    p = np.float32(-0.2)   # camera pitch about X
+    mount = np.array([1, 0, 0, 0, 0, np.cos(p), -np.sin(p), 0.5, 0, np.sin(p), np.cos(p), -0.1], np.float32)
+    return Robot(parent, joint_type, axis, origin, 1, mount, 4)
+
+
+def robot_states(robot: Robot, n: int, seed: int = 0):
+    """Seeded per-environment robot state: base_pose [n,3] = (x, z, yaw), joint_pos [n,L], held_slot [n] (-1 = hand
+    empty), held_xform [n,12] (held object in the end-effector frame)."""
+    g = _rng(9, seed)
+    L = len(robot.parent)
+    base = np.stack([g.uniform(1, 11, n), g.uniform(1, 11, n), g.uniform(-np.pi, np.pi, n)], axis=1).astype(np.float32)
+    joints = g.uniform(-1.2, 1.2, (n, L)).astype(np.float32)
+    joints[:, robot.joint_type == 2] = g.uniform(0.0, 0.4, (n, int((robot.joint_type == 2).sum()))).astype(np.float32)
+    held = np.where(g.uniform(0, 1, n) < 0.5, 0, -1).astype(np.int32)
+    hx = np.tile(np.array([1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, -0.12], np.float32), (n, 1))
+    hx[:, 3] = g.uniform(-0.02, 0.02, n).astype(np.float32)
+    return base, joints, held, hx
