@@ -275,6 +275,40 @@ def run_gx(args):
     ms_per_step = total_ms_max / args.steps
     value = world * N * args.steps / (total_ms_max * 1e-3)
 
+    # ---- scene-graph update (N12) + render: the robot's links and the camera come from gx_update_transforms --------
+    fk = None
+    if K >= 5 and not args.obs:
+        from paper_2306_07552_b200 import gen as _gen
+        robot = _gen.robot_proxy()
+        gx.gx_set_robot(scene, robot)
+        st = _gen.robot_states(robot, N, seed=rank)
+        st[0][:, :2] = wl.cam_pose.reshape(N, 4, 4)[:, [0, 2], 3]      # stand where the config's camera stood
+        d_st = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in st]
+        d_cam2, d_xf2 = d_in[1].clone(), d_in[3].clone()
+
+        def fk_only():
+            gx.gx_update_transforms(scene, N, K, K - 5, d_st[0], d_st[1], d_st[2], d_st[3], d_cam2, d_xf2, stream)
+
+        def fk_render():
+            fk_only()
+            gx.gx_render_batch(scene, cam, N, K, d_in[0], d_cam2, d_in[2], d_xf2, rgb, depth, None, stream)
+        res = {}
+        for name, fn in (("fk_ms", fk_only), ("fk_plus_render_ms", fk_render)):
+            for _ in range(3):
+                fn()
+            torch.cuda.synchronize()
+            evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+            for a, b in evs:
+                flush.zero_()
+                a.record(); fn(); b.record()
+            torch.cuda.synchronize()
+            res[name] = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        fk = dict(res, links=5, note="gx_update_transforms (N12: base pose + joint positions -> link, camera and held-object "
+                  "transforms) then gx_render_batch on the same stream; the paper's CPU 'Render Setup' is 0.77 ms @128 envs, "
+                  "1.47 ms @512 (Table 5, another machine)")
+        step()      # leave the handle's history and the images as the render-only step made them
+        torch.cuda.synchronize()
+
     # ---- e2e: host buffers in, host buffers out, through gx_render_batch_host -------------------------
     e2e = None
     if not args.no_e2e and not args.obs:
@@ -359,7 +393,7 @@ def run_gx(args):
                    "l2": "256 MB buffer written between timed iterations (untimed)",
                    "arithmetic": "f32 vertex stage, i32/i64 fixed-point coverage, f32 depth/colour"},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches) * args.steps * world,
-        "ms_per_step_per_rank": per_rank_ms,
+        "ms_per_step_per_rank": per_rank_ms, "scene_graph_update": fk,
         "roofline": roofline, "cpu_baseline": cpu,
     }
     print(json.dumps(out), flush=True)

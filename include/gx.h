@@ -90,7 +90,7 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
  * NaN/Inf inputs and out-of-range env_scene/inst_mesh values are precondition violations: the image is
  * undefined, but no out-of-bounds write occurs for in-range ids.
  * Errors: INVALID_ARG (null handle/camera/required pointer, N <= 0, K < 0, K > GX_MAX_INSTANCES, width or
- * height not a positive multiple of 16, znear <= 0, zfar <= znear), UNSUPPORTED (width or height > 128),
+ * height not a positive multiple of 16, znear <= 0, zfar <= znear), UNSUPPORTED (width or height > 256),
  * OOM, CUDA.
  */
 int gx_render_batch(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K, const int32_t *env_scene,
@@ -115,7 +115,7 @@ int gx_render_batch_obs(GxScene *scene, const GxCamera *camera, int32_t N, int32
 
 /*
  * gx_render_batch_host -- the same operation with every array argument in HOST memory (pageable or
- * pinned): copies the inputs to the device, renders in sub-batches of 512 environments while the images of
+ * pinned): copies the inputs to the device, renders in sub-batches of 64..256 environments while the images of
  * the previous sub-batch are copied back on a second stream, and synchronises before returning.  This is the
  * end-to-end entry point bench.py times for its "e2e" figure.
  */
@@ -124,24 +124,57 @@ int gx_render_batch_host(GxScene *scene, const GxCamera *camera, int32_t N, int3
                          uint8_t *rgb_out, float *depth_out, uint32_t *id_out);
 
 /*
+ * GxLink, gx_set_robot, gx_update_transforms -- the scene-graph update on the GPU: forward kinematics from the
+ * per-environment base pose and joint positions to the link, camera and held-object transforms, written straight
+ * into the arrays gx_render_batch reads ("we use forward kinematics to compute the position of the robot's
+ * articulated links"; "Scene graph updates are communicated from our physics simulation to the ...
+ * renderer"; it replaces the CPU "Render Setup" stage of Table 5).  The paper gives no
+ * robot format or arithmetic; N12 fixes both (binary32, own sine / cosine, Rodrigues joints, the affine
+ * product order of N2).
+ *
+ * gx_set_robot: links [n_links] HOST array, copied.  Link l hangs off link parent < l (-1 = the base); origin is the
+ *   joint frame in the parent link's frame (3x4 row-major, rigid); joint_type 0 fixed, 1 revolute about, 2 prismatic
+ *   along the unit vector axis (joint frame).  camera_link / cam_mount [12]: the link the camera rides on (-1 = the
+ *   base) and the camera frame in that link's frame; ee_link: the link that carries a held object (-1 = the base).
+ *   Errors: INVALID_ARG (NULL, n_links outside [1, 64], a parent that does not precede its link, a joint type
+ *   outside 0..2, link indices out of range), OOM, CUDA.
+ * gx_update_transforms: all arrays are DEVICE pointers, caller-owned; rows of 16 floats must be 16-byte aligned.
+ *   base_pose  [N,3]     float32 in   x, z, yaw: the base stands on the ground plane y = 0 and turns about +Y
+ *   joint_pos  [N,L]     float32 in   one position per link (radians or metres; ignored for fixed joints)
+ *   held_slot  [N]       int32   in   instance slot of the object in the gripper, -1 = none; NULL = no held objects
+ *   held_xform [N,12]    float32 in   the held object's pose in the end-effector link's frame (3x4); NULL with held_slot
+ *   cam_pose   [N,16]    float32 out  camera-to-world of every environment
+ *   inst_xform [N,K,16]  float32 i/o  slots link_slot0 .. link_slot0 + L - 1 receive the link transforms, slot
+ *                                     held_slot[n] the held object's; every other slot is left as it is
+ *   The call only enqueues one kernel on cuda_stream; a gx_render_batch enqueued after it on the same stream sees
+ *   the new transforms.  Errors: INVALID_ARG (no robot set, NULL arrays, N <= 0, link slots outside [0, K)), CUDA.
+ */
+typedef struct {
+    int32_t parent;
+    int32_t joint_type;
+    float axis[3];
+    float origin[12];
+} GxLink;
+int gx_set_robot(GxScene *scene, const GxLink *links, int32_t n_links, int32_t camera_link, const float *cam_mount,
+                 int32_t ee_link);
+int gx_update_transforms(GxScene *scene, int32_t N, int32_t K, int32_t link_slot0, const float *base_pose,
+                         const float *joint_pos, const int32_t *held_slot, const float *held_xform, float *cam_pose,
+                         float *inst_xform, void *cuda_stream);
+
+/*
  * gx_set_option -- tuning / verification switches of a handle.  Unknown names and out-of-range values return
  * INVALID_ARG.  Every switch leaves the images bit-identical (tested); they only move time around.
- *   "cull"         0|1 (1)   per-environment frustum culling of clusters and 32-triangle sub-clusters (K1).
- *   "subcull"      0|1 (1)   the sub-cluster test in the geometry kernel.
- *   "path"         0|1 (0)   0 = cull / geometry / raster kernels over a triangle-record pool;
- *                            1 = the single-kernel renderer (also the pass that renders environments whose
- *                            records overflow their pool segment).
- *   "bands"        0|1|2|4 (0 = automatic: 2 for frames above 64 KB of keys) raster tasks per frame.
- *   "occlusion"    0..3 (1)  occluder scheme: 0 = one pass; 2 = the sub-clusters whose triangles are
- *                            big on screen are drawn first, the others are culled against their hi-Z tiles and
- *                            drawn in a second pass; 3 = the far big ones wait for a middle pass; 1 = automatic
- *                            (2 passes for frames of >= 8192 pixels and batches of >= 512 environments).
- *   "occl_area"    (64)      screen-box pixels per triangle from which a sub-cluster counts as big.
- *   "occluder_pct" 1..100 (50) three passes only: share of the visible clusters, nearest first, that are "near".
- *   "pool_slots"   narrow record slots per (environment, band); 0 = max(2048, 4*W*H/bands).
- *   "pool_bytes"   record pool budget, which bounds the environments per pass; 0 = 8 GB.
- *   "big_slots", "chunk_slots"  raster pass B: a group of more than big_slots 4-pixel slots is drawn in chunks
- *                            of chunk_slots (512, 128).
+ *   "cull"         0|1 (1)   per-environment frustum culling of clusters (K1).
+ *   "subcull"      0|1 (1)   the same test for every run of 32 triangles of a visible cluster.
+ *   "hiz"          0|1 (1)   hi-Z rejection (in the tiles, and with it the occluder scheme).
+ *   "occlusion"    -1|0|1 (-1) occluder scheme: the runs whose triangles are big on screen go through
+ *                            geometry / bin / raster first, the others are culled against the hi-Z values that
+ *                            leaves (per run and per triangle) and follow in a second phase.  -1 = automatic: on
+ *                            for frames of at least 8192 pixels.
+ *   "occl_area"    (64)      screen-box pixels per triangle from which a run counts as big.
+ *   "big_px"       1..32 (24) records whose pixel box is at least this wide or high take the large (block) path.
+ *   "pool_bytes"   budget of the record arena, which bounds the environments per wave; 0 = 4 GB.
+ *   "arena_slots"  force the arena size in record slots (tests: several waves); 0 = automatic.
  *   "stats"        0|1 (0)   count what gx_get_stat reports (slower kernels).
  *   "timing"       0|1 (0)   1 starts (and resets), 0 stops recording CUDA events around every kernel of
  *                            subsequent gx_render_batch calls on their stream.
@@ -151,12 +184,14 @@ int gx_set_option(GxScene *scene, const char *name, int64_t value);
 /*
  * gx_get_stat -- counters of the most recent gx_render_batch on this handle ("stats" = 1); synchronises the
  * stream the call ran on.  Names: "clusters_tested", "clusters_drawn", "triangles_in" (triangles of drawn
- * sub-clusters), "triangles_raster" (survived clip, zero-area and pixel-centre bounding-box rejection),
- * "fragments" (pixel-centre hits before the depth test), "overflow_envs" (environments rendered by the overflow
- * pass), "clusters_occluded", "records_occluded" (occluder scheme), "max_env_records", "p50_env_records"
- * (records per raster task, last chunk), "launches" (kernels launched by the call).
- * With "timing": "timed_calls" and "ns_cull", "ns_geom", "ns_order", "ns_raster", "ns_fallback" = nanoseconds
- * spent in each kernel class, summed over the calls since timing was started.
+ * runs), "triangles_raster" (survived clip, zero-area and pixel-centre bounding-box rejection and the hi-Z test of
+ * the second phase), "triangles_hidden", "subclusters_hidden" (dropped by the hi-Z tests of the second phase),
+ * "fragments" (pixel-centre hits that reached the depth test), "records_occluded" (references dropped by hi-Z in
+ * the tiles), "blocks_drawn", "large_records", "large_draws", "tile_refs", "waves", "sum_slots", "max_env_slots"
+ * (record slot bounds), "bad_ids" (out-of-range mesh ids treated as empty slots), "launches" (kernels launched by
+ * the call), "arena_bytes".
+ * With "timing": "timed_calls" and "ns_cull", "ns_geom", "ns_bin", "ns_raster", "ns_tail" = nanoseconds spent in
+ * each kernel class, summed over the calls since timing was started.
  * Unknown names return INVALID_ARG; *out receives the value.
  */
 int gx_get_stat(GxScene *scene, const char *name, int64_t *out);

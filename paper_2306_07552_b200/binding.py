@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgx.so")
 GX_OK, GX_ERR_INVALID_ARG, GX_ERR_CUDA, GX_ERR_OOM, GX_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 GX_BACKGROUND_ID = 0xFFFFFFFF
 EXPORTS = ("gx_create_scene", "gx_render_batch", "gx_render_batch_host", "gx_set_option", "gx_get_stat",
-           "gx_render_batch_obs", "gx_destroy", "gx_last_error")
+           "gx_render_batch_obs", "gx_set_robot", "gx_update_transforms", "gx_destroy", "gx_last_error")
 
 
 class GxMesh(C.Structure):
@@ -30,6 +30,10 @@ class GxMesh(C.Structure):
 class GxCamera(C.Structure):
     _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float),
                 ("znear", C.c_float), ("zfar", C.c_float)]
+
+
+class GxLink(C.Structure):
+    _fields_ = [("parent", C.c_int32), ("joint_type", C.c_int32), ("axis", C.c_float * 3), ("origin", C.c_float * 12)]
 
 
 class GxError(RuntimeError):
@@ -51,7 +55,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.gx_last_error.restype = C.c_char_p
         L.gx_destroy.restype = None
-        for n in EXPORTS[:6]:
+        for n in EXPORTS[:8]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -129,6 +133,33 @@ def gx_render_batch_host(scene, camera: GxCamera, N: int, K: int, env_scene, cam
                                       _host(inst_mesh, np.int32), _host(inst_xform, np.float32),
                                       _host(rgb_out, np.uint8), _host(depth_out, np.float32),
                                       _host(id_out, np.uint32)))
+
+
+def gx_set_robot(scene, robot) -> None:
+    """robot: an object with parent [L], joint_type [L], axis [L,3], origin [L,12], camera_link, cam_mount [12],
+    ee_link (gen.Robot); host data, copied."""
+    L = len(robot.parent)
+    links = (GxLink * L)()
+    for l in range(L):
+        links[l].parent = int(robot.parent[l])
+        links[l].joint_type = int(robot.joint_type[l])
+        ax = np.asarray(robot.axis[l], np.float32)
+        og = np.asarray(robot.origin[l], np.float32).reshape(12)
+        for k in range(3):
+            links[l].axis[k] = float(ax[k])
+        for k in range(12):
+            links[l].origin[k] = float(og[k])
+    mount = np.ascontiguousarray(robot.cam_mount, np.float32).reshape(12)
+    _check(lib().gx_set_robot(scene, links, C.c_int32(L), C.c_int32(int(robot.camera_link)), C.c_void_p(mount.ctypes.data),
+                              C.c_int32(int(robot.ee_link))))
+
+
+def gx_update_transforms(scene, N: int, K: int, link_slot0: int, base_pose, joint_pos, held_slot, held_xform, cam_pose,
+                         inst_xform, cuda_stream: int = 0) -> None:
+    """All arrays are device tensors / addresses; enqueues on cuda_stream and returns."""
+    _check(lib().gx_update_transforms(scene, C.c_int32(N), C.c_int32(K), C.c_int32(link_slot0), _dev(base_pose), _dev(joint_pos),
+                                      _dev(held_slot), _dev(held_xform), _dev(cam_pose), _dev(inst_xform),
+                                      C.c_void_p(cuda_stream)))
 
 
 def gx_set_option(scene, name: str, value: int) -> None:

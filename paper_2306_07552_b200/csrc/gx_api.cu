@@ -11,6 +11,7 @@
 
 #include "../../include/gx.h"
 #include "gx_pipeline.cuh"
+#include "gx_fk.cuh"
 
 namespace {
 
@@ -111,6 +112,10 @@ struct GxScene {
     // launch configurations, resolved once per kernel instantiation (occupancy queries are not free)
     struct Plan { const void *fn; size_t smem; int per_sm; };
     std::vector<Plan> plans;
+    // robot description (gx_set_robot)
+    gx::FkLink *fk_links = nullptr;
+    int fk_L = 0, fk_camera_link = -1, fk_ee_link = -1;
+    float fk_mount[12] = {1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0};
     // staging for gx_render_batch_host
     DevBuf<int32_t> h_env_scene, h_inst_mesh;
     DevBuf<float> h_cam_pose, h_inst_xform, h_depth;
@@ -340,6 +345,7 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->clusters);
     cudaFree(sc->meshes);
     cudaFree(sc->stats);
+    cudaFree(sc->fk_links);
     sc->arena_recs.release(); sc->arena_bbs.release(); sc->arena_refs.release(); sc->scratch.release();
     for (cudaEvent_t e : sc->t_ev) cudaEventDestroy(e);
     if (sc->h_ctl) cudaFreeHost(sc->h_ctl);
@@ -646,6 +652,55 @@ int gx_render_batch_obs(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, 
     if (!obs_out) return fail(GX_ERR_INVALID_ARG, "obs_out is required");
     return render_impl(sc, cam, N, K, env_scene, cam_pose, inst_mesh, inst_xform, nullptr, nullptr, nullptr, obs_out, depth_min,
                        depth_max, cuda_stream);
+}
+
+int gx_set_robot(GxScene *sc, const GxLink *links, int32_t n_links, int32_t camera_link, const float *cam_mount, int32_t ee_link) {
+    if (!sc || !links || !cam_mount) return fail(GX_ERR_INVALID_ARG, "NULL argument");
+    if (n_links <= 0 || n_links > gx::FK_MAX_LINKS) return fail(GX_ERR_INVALID_ARG, "n_links must be in [1, %d], got %d", gx::FK_MAX_LINKS, n_links);
+    if (camera_link < -1 || camera_link >= n_links || ee_link < -1 || ee_link >= n_links)
+        return fail(GX_ERR_INVALID_ARG, "camera_link and ee_link must be in [-1, n_links)");
+    std::vector<gx::FkLink> h((size_t)n_links);
+    for (int l = 0; l < n_links; ++l) {
+        if (links[l].parent < -1 || links[l].parent >= l) return fail(GX_ERR_INVALID_ARG, "link %d: parent %d must precede it (or be -1)", l, links[l].parent);
+        if (links[l].joint_type < 0 || links[l].joint_type > 2) return fail(GX_ERR_INVALID_ARG, "link %d: joint_type %d", l, links[l].joint_type);
+        h[l].parent = links[l].parent;
+        h[l].joint_type = links[l].joint_type;
+        memcpy(h[l].axis, links[l].axis, sizeof(h[l].axis));
+        memcpy(h[l].origin, links[l].origin, sizeof(h[l].origin));
+    }
+    DeviceGuard guard(sc->device);
+    if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
+    if (sc->fk_links) { cudaFree(sc->fk_links); sc->fk_links = nullptr; sc->fk_L = 0; }
+    GX_CUDA(cudaMalloc(&sc->fk_links, (size_t)n_links * sizeof(gx::FkLink)));
+    GX_CUDA(cudaMemcpy(sc->fk_links, h.data(), (size_t)n_links * sizeof(gx::FkLink), cudaMemcpyHostToDevice));
+    sc->fk_L = n_links;
+    sc->fk_camera_link = camera_link;
+    sc->fk_ee_link = ee_link;
+    memcpy(sc->fk_mount, cam_mount, sizeof(sc->fk_mount));
+    return GX_OK;
+}
+
+int gx_update_transforms(GxScene *sc, int32_t N, int32_t K, int32_t link_slot0, const float *base_pose, const float *joint_pos,
+                         const int32_t *held_slot, const float *held_xform, float *cam_pose, float *inst_xform, void *cuda_stream) {
+    if (!sc) return fail(GX_ERR_INVALID_ARG, "NULL scene");
+    if (!sc->fk_links) return fail(GX_ERR_INVALID_ARG, "no robot: call gx_set_robot first");
+    if (N <= 0 || K < 0 || K > GX_MAX_INSTANCES) return fail(GX_ERR_INVALID_ARG, "bad N or K");
+    if (!base_pose || !joint_pos || !cam_pose || !inst_xform) return fail(GX_ERR_INVALID_ARG, "NULL array argument");
+    if ((held_slot == nullptr) != (held_xform == nullptr)) return fail(GX_ERR_INVALID_ARG, "held_slot and held_xform go together");
+    if (held_slot && sc->fk_ee_link < -1) return fail(GX_ERR_INVALID_ARG, "no end-effector link");
+    if (link_slot0 < 0 || link_slot0 + sc->fk_L > K) return fail(GX_ERR_INVALID_ARG, "link slots [%d, %d) do not fit K = %d", link_slot0, link_slot0 + sc->fk_L, K);
+    DeviceGuard guard(sc->device);
+    if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
+    gx::FkParams P;
+    P.links = sc->fk_links; P.L = sc->fk_L; P.camera_link = sc->fk_camera_link; P.ee_link = sc->fk_ee_link;
+    memcpy(P.cam_mount, sc->fk_mount, sizeof(P.cam_mount));
+    P.N = N; P.K = K; P.link_slot0 = link_slot0;
+    P.base_pose = base_pose; P.joint_pos = joint_pos; P.held_slot = held_slot; P.held_xform = held_xform;
+    P.cam_pose = cam_pose; P.inst_xform = inst_xform;
+    constexpr int FW = 4;
+    gx::fk_kernel<FW><<<(N + FW - 1) / FW, FW * 32, 0, (cudaStream_t)cuda_stream>>>(P);
+    GX_CUDA(cudaGetLastError());
+    return GX_OK;
 }
 
 int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,

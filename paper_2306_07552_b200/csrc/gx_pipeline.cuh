@@ -1593,7 +1593,7 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
         }
         __syncwarp();
 
-        if (phase == 1) {
+        if constexpr (PHASE == 1) {
             // ---- occluder phase: the keys and the hi-Z values go to global memory ---------------------------
             const uint4 *f4 = reinterpret_cast<const uint4 *>(ws.fb);
 #pragma unroll
@@ -1617,8 +1617,7 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
                 }
             }
             __syncwarp();
-            continue;
-        }
+        } else {
 
         // ---- K5: resolve the winners, write RGB / depth / id as 16-byte stores ----------------------------
 #pragma unroll 1
@@ -1666,6 +1665,7 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
                     *reinterpret_cast<uint4 *>(dst) = make_uint4(o[0], o[1], o[2], o[3]);
                 }
             }
+        }
         }
         __syncwarp();
     }
