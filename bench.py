@@ -332,8 +332,21 @@ def run_gx(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
         h2d = sum(a.nbytes for a in h_in)
         d2h = N * H * W * (4 if wl.depth_only else 7)
+        # the box's pinned device-to-host ceiling for the same bytes, for context
+        raw_d = torch.empty(d2h, dtype=torch.uint8, device=dev)
+        raw_h = torch.empty(d2h, dtype=torch.uint8).pin_memory()
+        for _ in range(2):
+            raw_h.copy_(raw_d, non_blocking=True)
+        torch.cuda.synchronize()
+        t1 = time.perf_counter()
+        for _ in range(5):
+            raw_h.copy_(raw_d, non_blocking=True)
+        torch.cuda.synchronize()
+        raw_gbs = d2h * 5 / (time.perf_counter() - t1) / 1e9
+        del raw_d, raw_h
         e2e = {"value": world * N * n_e2e / float(t.item()), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
                "d2h_bytes_per_step": int(d2h), "steps": n_e2e,
+               "d2h_gbs_achieved": d2h * n_e2e / float(t.item()) / 1e9, "d2h_gbs_bare_copy": raw_gbs,
                "note": "gx_render_batch_host: pinned host inputs -> device, render, RGBD -> pinned host, sync"}
         # the e2e images must be the device-path images
         assert np.array_equal(p_depth.numpy().view(np.uint32), depth.cpu().numpy().view(np.uint32))

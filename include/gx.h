@@ -115,7 +115,7 @@ int gx_render_batch_obs(GxScene *scene, const GxCamera *camera, int32_t N, int32
 
 /*
  * gx_render_batch_host -- the same operation with every array argument in HOST memory (pageable or
- * pinned): copies the inputs to the device, renders in sub-batches of 64..256 environments while the images of
+ * pinned): copies the inputs to the device, renders in three sub-batches (option "host_sub") while the images of
  * the previous sub-batch are copied back on a second stream, and synchronises before returning.  This is the
  * end-to-end entry point bench.py times for its "e2e" figure.
  */
@@ -175,6 +175,7 @@ int gx_update_transforms(GxScene *scene, int32_t N, int32_t K, int32_t link_slot
  *   "big_px"       1..32 (24) records whose pixel box is at least this wide or high take the large (block) path.
  *   "pool_bytes"   budget of the record arena, which bounds the environments per wave; 0 = 4 GB.
  *   "arena_slots"  force the arena size in record slots (tests: several waves); 0 = automatic.
+ *   "host_sub"     environments per sub-batch of gx_render_batch_host; 0 = a third of the batch.
  *   "stats"        0|1 (0)   count what gx_get_stat reports (slower kernels).
  *   "timing"       0|1 (0)   1 starts (and resets), 0 stops recording CUDA events around every kernel of
  *                            subsequent gx_render_batch calls on their stream.

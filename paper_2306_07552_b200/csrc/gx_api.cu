@@ -84,6 +84,7 @@ struct GxScene {
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
     // options (gx_set_option)
     int opt_cull = 1, opt_subcull = 1, opt_stats = 0, opt_hiz = 1, opt_big_px = 24;
+    int opt_host_sub = 0;               // gx_render_batch_host: environments per sub-batch; 0 = automatic
     int opt_occlusion = -1;             // occluder scheme: 1 on, 0 off, -1 automatic (on for frames of at least 8192 pixels)
     int opt_occl_area = 64;             // pixels per triangle of a sub-cluster's screen box that make it an occluder
     int64_t opt_pool_bytes = 0;         // arena budget; 0 = 4 GB
@@ -100,6 +101,7 @@ struct GxScene {
     bool ctl_pending = false;
     int ctl_N = 0;
     double hist_u_per_env = 0.0;
+    int hist_waves = 1;                 // waves the last call needed (the host launches that many rounds of the stage kernels)
     // kernel timing (option "timing"): CUDA events recorded on the caller's stream around every kernel
     int opt_timing = 0;
     std::vector<cudaEvent_t> t_ev;      // recorded marks, in order
@@ -369,6 +371,11 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
         if (value) { sc->t_used = 0; sc->t_calls = 0; sc->t_full = false; }
         return GX_OK;
     }
+    if (!strcmp(name, "host_sub")) {
+        if (value < 0) return fail(GX_ERR_INVALID_ARG, "host_sub must be >= 0");
+        sc->opt_host_sub = (int)value;
+        return GX_OK;
+    }
     if (!strcmp(name, "occlusion")) {
         if (value < -1 || value > 1) return fail(GX_ERR_INVALID_ARG, "occlusion must be -1 (automatic), 0 or 1");
         sc->opt_occlusion = (int)value;
@@ -506,6 +513,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     if (sc->ctl_pending && cudaEventQuery(sc->ev_ctl) == cudaSuccess) {
         const uint64_t sum = (uint64_t)sc->h_ctl[gx::C_SUM_U] | ((uint64_t)sc->h_ctl[gx::C_SUM_U + 1] << 32);
         sc->hist_u_per_env = std::max(sc->hist_u_per_env, (double)sum / (double)std::max(sc->ctl_N, 1));
+        sc->hist_waves = (int)std::min<uint32_t>(std::max<uint32_t>(sc->h_ctl[gx::C_WAVES], 1u), 256u);
         sc->ctl_pending = false;
     }
     cudaGetLastError();   // (cudaErrorNotReady of the query is not an error)
@@ -534,6 +542,8 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     PP.item_stride = (int32_t)std::max<size_t>((size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches, 1);
     size_t off = 64;
     const size_t o_U = off; off += n;
+    const size_t o_nitems = off; off += n;
+    const size_t o_cpre = off; off += n + 1;
     const size_t o_base = off; off += n;
     const size_t o_cnt = off; off += n;
     const size_t o_cntA = off; off += n;
@@ -548,14 +558,16 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     const size_t o_hizb = off; off += PP.occl ? n * (size_t)PP.T * 8 : 0;
     off = (off + 3) & ~(size_t)3;
     const size_t o_items = off; off += 4 * n * (size_t)PP.item_stride;
+    const size_t o_witems = off; off += 4 * n * (size_t)PP.item_stride;
     const size_t o_keys = off; off += PP.occl ? n * (size_t)P.W * (size_t)P.H * 2 : 0;
     if ((rc = sc->scratch.reserve(off)) != GX_OK) return rc;
     uint32_t *sp = sc->scratch.p;
-    PP.ctl = sp; PP.U = sp + o_U; PP.rec_base = sp + o_base;
+    PP.ctl = sp; PP.U = sp + o_U; PP.n_items = sp + o_nitems; PP.item_pre = sp + o_cpre; PP.rec_base = sp + o_base;
     PP.cnt = sp + o_cnt; PP.cntA = sp + o_cntA; PP.n_large = sp + o_nl; PP.env_idb = sp + o_idb;
     PP.env_mv = reinterpret_cast<float *>(sp + o_mv);
     PP.tile_off = sp + o_toff; PP.tasks = sp + o_tasks; PP.hizt = sp + o_hizt; PP.hizb = sp + o_hizb;
     PP.items = reinterpret_cast<uint4 *>(sp + o_items);
+    PP.wave_items = reinterpret_cast<uint4 *>(sp + o_witems);
     PP.keys = reinterpret_cast<unsigned long long *>(sp + o_keys);
 
     sc->last_stream = stream;
@@ -578,6 +590,19 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
         if ((rc = mark(sc, stream, 1)) != GX_OK) return rc;
     }
     int launches = 1;
+    // one round of the stage kernels per wave the previous call on this handle needed (its batch is the best guess
+    // for this one), plus one when there were several; whatever is still left goes to the cooperative tail kernel
+    const int rounds = sc->hist_waves > 1 ? sc->hist_waves + 1 : 1;
+    for (int round = 0; round < rounds; ++round) {
+    if (round > 0) {
+        gx::wave_kernel<<<1, 256, 0, stream>>>(PP);
+        GX_CUDA(cudaGetLastError());
+        ++launches;
+    }
+    gx::pack_kernel<<<std::min(std::max(N / 8, 1), 4 * sc->num_sms), 256, 0, stream>>>(PP);
+    GX_CUDA(cudaGetLastError());
+    if ((rc = mark(sc, stream, round > 0 ? 5 : 1)) != GX_OK) return rc;
+    ++launches;
     for (int phase = PP.occl ? 1 : 0; phase <= (PP.occl ? 2 : 0); ++phase) {
         // K2: persistent independent warps
         {
@@ -616,6 +641,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
             if ((rc = mark(sc, stream, 4)) != GX_OK) return rc;
         }
         launches += 3;
+    }
     }
     // the tail: later waves, on the device (exits at once when the first wave took every environment)
     {
@@ -729,10 +755,11 @@ int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K,
         GX_CUDA(cudaMemcpyAsync(sc->h_inst_mesh.p, inst_mesh, nk * 4, cudaMemcpyHostToDevice, st));
         GX_CUDA(cudaMemcpyAsync(sc->h_inst_xform.p, inst_xform, nk * 64, cudaMemcpyHostToDevice, st));
     }
-    // render in sub-batches and copy each one's images back on a second stream while the next one renders: the
-    // device-to-host copy of RGBD over PCIe takes several times longer than the rendering, so the sub-batches are
-    // small (the first render and the last copy are the only parts not overlapped)
-    const int sub = std::max(64, std::min(256, (N + 7) / 8));
+    // render in sub-batches and copy each one's images back on a second stream while the next one renders.  The
+    // device-to-host copy of RGBD over PCIe takes about twice as long as the rendering, and a render call has a
+    // fixed cost of a few hundred microseconds, so three sub-batches are the best split measured on cfg 2
+    // (time = first render + the whole copy): 2.76 ms against 2.09 ms for the bare copy at 56 GB/s.
+    const int sub = sc->opt_host_sub > 0 ? sc->opt_host_sub : std::max(64, (N + 2) / 3);
     size_t n_sub = 0;
     for (int e0 = 0; e0 < N; e0 += sub, ++n_sub) {
         const int n = std::min(sub, N - e0);

@@ -60,7 +60,7 @@ enum { F_BIAS = 7, F_FLOATCOL = 8, F_WIDE = 16 };
 // control words (device): cursors and the current wave
 // (cursors and task counts exist once per phase of the occluder scheme: index 0 = single pass or occluder phase, 1 = second phase)
 enum { C_WAVE_E0 = 0, C_WAVE_E1, C_GEOM_CUR, C_BIN_CUR = C_GEOM_CUR + 2, C_RAST_CUR = C_BIN_CUR + 2, C_CULL_DONE = C_RAST_CUR + 2,
-       C_N_ITEMS, C_SUM_U /* 64-bit: two words, even index */, C_WAVES = C_SUM_U + 2, C_MAX_U, C_BAD_ENVS, C_TASK_CNT = 16,
+       C_WAVE_ITEMS, C_SUM_U /* 64-bit: two words, even index */, C_WAVES = C_SUM_U + 2, C_MAX_U, C_BAD_ENVS, C_TASK_CNT = 16,
        C_NCTL = C_TASK_CNT + 2 * NCLASS };
 static_assert(C_SUM_U % 2 == 0 && C_BAD_ENVS < C_TASK_CNT, "control word layout");
 
@@ -69,10 +69,14 @@ struct PipeParams {
     // environment table and K1 output
     float *env_mv;           // [N][K+1][12] model-view per slot
     uint32_t *env_idb;       // [N][K+1] first triangle id per slot
-    uint4 *items;            // [ctl[C_N_ITEMS]] one flat list for the call: (slot << 24 | batch, runs of 32 triangles
-                             //   to draw: occluder class | the rest << 8, environment, unused)
+    uint4 *items;            // [N][item_stride]: (slot << 24 | batch, runs of 32 triangles to draw: occluder class |
+                             //   the rest << 8, unused, unused)
+    uint32_t *n_items;       // [N]
+    uint32_t *item_pre;      // [N+1] exclusive prefix of n_items over the environments of the wave
+    uint4 *wave_items;       // [ctl[C_WAVE_ITEMS]] the items of the wave's environments in one list, the environment in
+                             //   the third word (pack_stage), which is what the geometry stage hands out
     uint32_t *U;             // [N] upper bound of the record slots of the environment
-    int32_t item_stride;     // capacity of the item list = N * item_stride
+    int32_t item_stride;
     // wave allocation
     uint32_t *rec_base;      // [N] first arena slot of the environment's segment
     uint32_t *cnt;           // [N] slots used of the segment
@@ -203,26 +207,27 @@ __device__ __forceinline__ void env_setup(const PipeParams &PP, int env, const E
 // reset.  ctl[C_WAVE_E0 .. C_WAVE_E1) is the wave.
 // ------------------------------------------------------------------------------------------------
 __device__ void alloc_wave(const PipeParams &PP, uint32_t e_first) {
-    __shared__ uint32_t s_wu[32];
-    __shared__ uint32_t s_run_u, s_end;
+    __shared__ uint32_t s_wu[32], s_wi[32];
+    __shared__ uint32_t s_run_u, s_run_i, s_end, s_fin_i;
     const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t N = (uint32_t)PP.g.N;
-    if (tid == 0) { s_run_u = 0; s_end = N; }
+    if (tid == 0) { s_run_u = 0; s_run_i = 0; s_end = N; s_fin_i = 0; }
     __syncthreads();
     for (uint32_t c0 = e_first; c0 < N; c0 += NT) {
         const uint32_t e = c0 + tid;
         const uint32_t u = e < N ? __ldcg(&PP.U[e]) : 0u;
-        uint32_t iu = u;
+        const uint32_t ni = e < N && u ? __ldcg(&PP.n_items[e]) : 0u;   // (U = 0: nothing to draw)
+        uint32_t iu = u, ii = ni;
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
-            const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, iu, d);
-            if (lane >= d) iu += a;
+            const uint32_t a = __shfl_up_sync(0xFFFFFFFFu, iu, d), b = __shfl_up_sync(0xFFFFFFFFu, ii, d);
+            if (lane >= d) { iu += a; ii += b; }
         }
-        if (lane == 31) s_wu[warp] = iu;
+        if (lane == 31) { s_wu[warp] = iu; s_wi[warp] = ii; }
         __syncthreads();
-        uint32_t bu = s_run_u;
-        for (int w = 0; w < warp; ++w) bu += s_wu[w];
-        const uint32_t ex_u = bu + iu - u;
+        uint32_t bu = s_run_u, bi = s_run_i;
+        for (int w = 0; w < warp; ++w) { bu += s_wu[w]; bi += s_wi[w]; }
+        const uint32_t ex_u = bu + iu - u, ex_i = bi + ii - ni;
         // (the first environment of a wave always fits: the host sizes the arena for the largest possible U,
         // and cull_kernel empties an environment that would still exceed it)
         const bool fits = (unsigned long long)ex_u + u <= (unsigned long long)PP.arena_slots || e == e_first;
@@ -231,16 +236,21 @@ __device__ void alloc_wave(const PipeParams &PP, uint32_t e_first) {
         const uint32_t end = s_end;
         if (e < end) {
             PP.rec_base[e] = ex_u;
+            PP.item_pre[e] = ex_i;
             PP.cnt[e] = 0;
             PP.cntA[e] = 0;
         }
-        if (tid == NT - 1) s_run_u = ex_u + u;
+        if (e == end) s_fin_i = ex_i;
+        if (tid == NT - 1) { s_run_u = ex_u + u; s_run_i = ex_i + ni; }
         __syncthreads();
         if (end < N) break;   // (uniform) the wave ends inside this chunk
     }
     if (tid == 0) {
+        const uint32_t end = s_end, n_ch = end < N ? s_fin_i : s_run_i;
+        PP.item_pre[end] = n_ch;
+        PP.ctl[C_WAVE_ITEMS] = n_ch;
         PP.ctl[C_WAVE_E0] = e_first;
-        PP.ctl[C_WAVE_E1] = s_end;
+        PP.ctl[C_WAVE_E1] = end;
         for (int c = 0; c < 2; ++c) { PP.ctl[C_GEOM_CUR + c] = 0; PP.ctl[C_BIN_CUR + c] = 0; PP.ctl[C_RAST_CUR + c] = 0; }
         PP.ctl[C_WAVES] += 1;
         for (int c = 0; c < 2 * NCLASS; ++c) PP.ctl[C_TASK_CNT + c] = 0;
@@ -290,8 +300,9 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
     constexpr int CCH = 256;                                   // clusters per round
     constexpr int VB_CAP = CCH * GX_MAX_BATCH_PER_CLUSTER;     // batches of the visible clusters of a round
     __shared__ uint32_t s_vb[VB_CAP], s_vm[VB_CAP];
-    __shared__ unsigned s_nvb, s_U;
-    if (tid == 0) s_U = 0;
+    __shared__ unsigned s_nvb, s_U, s_nitems;
+    if (tid == 0) { s_U = 0; s_nitems = 0; }
+    uint4 *env_items = PP.items + (size_t)env * (size_t)PP.item_stride;
     for (uint32_t c0 = 0; c0 < n_cl; c0 += CCH) {
         if (tid == 0) s_nvb = 0;
         __syncthreads();
@@ -334,15 +345,15 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
             }
         }
         __syncthreads();
-        // step 3: one work item per batch that has a run left, appended to the call's list
+        // step 3: one work item per batch that has a run left, appended to the environment's list
         for (unsigned v0 = warp * 32; v0 < nvb; v0 += NT) {
             const unsigned v = v0 + lane;
             const bool has = v < nvb && s_vm[v] != 0u;
             const unsigned m = __ballot_sync(0xFFFFFFFFu, has);
             uint32_t base = 0;
-            if (lane == 0 && m) base = atomicAdd(&PP.ctl[C_N_ITEMS], (unsigned)__popc(m));
+            if (lane == 0 && m) base = atomicAdd(&s_nitems, (unsigned)__popc(m));
             base = __shfl_sync(0xFFFFFFFFu, base, 0);
-            if (has) PP.items[base + __popc(m & ((1u << lane) - 1u))] = make_uint4(s_vb[v], s_vm[v], (uint32_t)env, 0u);
+            if (has) env_items[base + __popc(m & ((1u << lane) - 1u))] = make_uint4(s_vb[v], s_vm[v], 0u, 0u);
         }
         __syncthreads();
     }
@@ -351,7 +362,8 @@ __global__ void __launch_bounds__(WARPS * 32) cull_kernel(const PipeParams PP) {
     if (tid == 0) {
         uint32_t u = s_U;
         if (u > PP.arena_slots) { u = 0; atomicAdd(&PP.ctl[C_BAD_ENVS], 1u); }   // cannot happen: see alloc_wave (the geometry
-        PP.U[env] = u;                                                           // stage skips items of an environment with U = 0)
+        PP.U[env] = u;                                                           // stage never sees an environment with U = 0)
+        PP.n_items[env] = s_nitems;
         atomicAdd(reinterpret_cast<unsigned long long *>(&PP.ctl[C_SUM_U]), (unsigned long long)u);
         atomicMax(&PP.ctl[C_MAX_U], u);
         __threadfence();
@@ -680,8 +692,7 @@ __device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *
     pj.hw = 128.0f * (float)P.W; pj.hh = 128.0f * (float)P.H;
 
     unsigned st_in = 0, st_tri = 0, st_hid = 0, st_subhid = 0;
-    const uint32_t e0 = ldi<COOP>(&PP.ctl[C_WAVE_E0]), e1 = ldi<COOP>(&PP.ctl[C_WAVE_E1]);
-    const unsigned n_items = ldi<COOP>(&PP.ctl[C_N_ITEMS]);
+    const unsigned n_items = ldi<COOP>(&PP.ctl[C_WAVE_ITEMS]);
     uint32_t *cursor = &PP.ctl[C_GEOM_CUR + (phase == 2 ? 1 : 0)];
     const size_t hzb_stride = (size_t)(P.W >> 3) * (size_t)(P.H >> 2);
     unsigned next = 0;
@@ -690,11 +701,12 @@ __device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *
     while (next < n_items) {
         const unsigned g = next;
         if (lane == 0) next = atomicAdd(cursor, 1u);   // draw the following item while this one is processed
-        const uint4 item = ldi<COOP>(&PP.items[g]);
+        const uint4 item = ldi<COOP>(&PP.wave_items[g]);
         const uint32_t e = item.z, s = item.x >> 24, batch = item.x & 0xFFFFFFu;
+        const uint32_t U = ldi<COOP>(&PP.U[e]), rbase = ldi<COOP>(&PP.rec_base[e]);
+        {
         unsigned mask = phase == 0 ? ((item.y | (item.y >> 8)) & 255u) : (phase == 1 ? (item.y & 255u) : ((item.y >> 8) & 255u));
-        const uint32_t U = (e >= e0 && e < e1) ? ldi<COOP>(&PP.U[e]) : 0u;
-        if (mask && U) {
+        if (mask) {
             const float *MV = PP.env_mv + ((size_t)e * (size_t)(K + 1) + s) * 12;
             // lanes 0..7: one run each -- its vertex range, and in the second phase the hi-Z test of its box
             uint32_t vlo = 0xFFFFu, vhi = 0u;
@@ -713,9 +725,10 @@ __device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *
                 vlo = __reduce_min_sync(FULL, vlo);
                 vhi = __reduce_max_sync(FULL, vhi);
                 geom_batch<COOP, STATS>(PP, pj, batch, MV, ldi<COOP>(&PP.env_idb[(size_t)e * (size_t)(K + 1) + s]), ws, (int)e,
-                                        ldi<COOP>(&PP.rec_base[e]), U, lane, mask, (int)vlo, (int)vhi,
+                                        rbase, U, lane, mask, (int)vlo, (int)vhi,
                                         HZ ? PP.hizb + (size_t)e * hzb_stride : nullptr, st_in, st_tri, st_hid);
             }
+        }
         }
         next = __shfl_sync(FULL, next, 0);
     }
@@ -1687,6 +1700,40 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
     }
 }
 
+// The items of the wave's environments, copied into one list with the environment in the third word: the geometry
+// stage then needs no search to know whose item it drew.  One warp per environment at a time.
+template <bool COOP>
+__device__ __forceinline__ void pack_stage(const PipeParams &PP) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t e0 = ldi<COOP>(&PP.ctl[C_WAVE_E0]), e1 = ldi<COOP>(&PP.ctl[C_WAVE_E1]);
+    const uint32_t warps = gridDim.x * (blockDim.x >> 5), w = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    for (uint32_t e = e0 + w; e < e1; e += warps) {
+        const uint32_t at = ldi<COOP>(&PP.item_pre[e]), n = ldi<COOP>(&PP.item_pre[e + 1]) - at;
+        const uint4 *src = PP.items + (size_t)e * (size_t)PP.item_stride;
+        for (uint32_t i = lane; i < n; i += 32) {
+            const uint4 it = ldi<COOP>(&src[i]);
+            PP.wave_items[at + i] = make_uint4(it.x, it.y, e, 0u);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) pack_kernel(const PipeParams PP) { pack_stage<false>(PP); }
+
+// the next wave, as a kernel of its own (one CTA): the host launches it, followed by the stage kernels, once for every
+// wave the previous call needed, so that later waves run at full occupancy too; when no environment is left the wave
+// is empty and the stage kernels that follow exit at once
+__global__ void __launch_bounds__(256) wave_kernel(const PipeParams PP) {
+    const uint32_t e_next = __ldcg(&PP.ctl[C_WAVE_E1]);
+    if (e_next < (uint32_t)PP.g.N) {
+        alloc_wave(PP, e_next);
+    } else if (threadIdx.x == 0) {
+        PP.ctl[C_WAVE_E0] = e_next;
+        PP.ctl[C_WAVE_ITEMS] = 0;
+        for (int c = 0; c < 2; ++c) { PP.ctl[C_GEOM_CUR + c] = 0; PP.ctl[C_BIN_CUR + c] = 0; PP.ctl[C_RAST_CUR + c] = 0; }
+        for (int c = 0; c < 2 * NCLASS; ++c) PP.ctl[C_TASK_CNT + c] = 0;
+    }
+}
+
 #ifndef RAST_MINB
 #define RAST_MINB 4
 #endif
@@ -1719,6 +1766,8 @@ __global__ void __launch_bounds__(TAIL_WARPS * 32, 2) tail_kernel(const PipePara
         if (e_next >= (uint32_t)PP.g.N) break;
         grid.sync();   // every CTA has read the end of the previous wave before it moves
         if (blockIdx.x == 0) alloc_wave(PP, e_next);
+        grid.sync();
+        pack_stage<true>(PP);
         grid.sync();
         for (int phase = PP.occl ? 1 : 0; phase <= (PP.occl ? 2 : 0); ++phase) {
             if (phase == 2 && PP.hiz) geom_stage<true, STATS, true>(PP, smem + (size_t)warp * GEOM_WARP_SMEM, phase);
