@@ -98,6 +98,15 @@ int gx_render_batch(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K
                     float *depth_out, uint32_t *id_out, void *cuda_stream);
 
 /*
+ * gx_reserve -- allocate (or grow) everything the handle needs for calls of this shape now, so that the render calls
+ * that follow never allocate: the record arena (option "pool_bytes": at most an eighth of the device's memory and
+ * 16 GB by default; what does not fit is rendered in further waves) and the per-call tables.  Optional: the first
+ * gx_render_batch of a shape does the same.  "arena_bytes" and "scratch_bytes" of gx_get_stat tell what is held.
+ * Errors: INVALID_ARG, OOM, CUDA.
+ */
+int gx_reserve(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K);
+
+/*
  * gx_render_batch_obs -- the same rasterisation, written as the packed observation tensor the policy reads
  * ("directly consumed by PyTorch GPU-based batch DNN inference"; the visual encoder takes RGBD,
  * PAPER.md:141, Table 3).  The paper is silent on the layout and normalisation; N11 fixes them:
@@ -170,10 +179,11 @@ int gx_update_transforms(GxScene *scene, int32_t N, int32_t K, int32_t link_slot
  *   "occlusion"    -1|0|1 (-1) occluder scheme: the runs whose triangles are big on screen go through
  *                            geometry / bin / raster first, the others are culled against the hi-Z values that
  *                            leaves (per run and per triangle) and follow in a second phase.  -1 = automatic: on
- *                            for frames of at least 8192 pixels.
+ *                            for frames of at least 4096 pixels.
  *   "occl_area"    (64)      screen-box pixels per triangle from which a run counts as big.
  *   "big_px"       1..32 (24) records whose pixel box is at least this wide or high take the large (block) path.
- *   "pool_bytes"   budget of the record arena, which bounds the environments per wave; 0 = 4 GB.
+ *   "pool_bytes"   budget of the record arena, which bounds the environments per wave; 0 = an eighth of the
+ *                            device's memory, at most 16 GB.
  *   "arena_slots"  force the arena size in record slots (tests: several waves); 0 = automatic.
  *   "host_sub"     environments per sub-batch of gx_render_batch_host; 0 = a third of the batch.
  *   "stats"        0|1 (0)   count what gx_get_stat reports (slower kernels).
@@ -190,7 +200,7 @@ int gx_set_option(GxScene *scene, const char *name, int64_t value);
  * "fragments" (pixel-centre hits that reached the depth test), "records_occluded" (references dropped by hi-Z in
  * the tiles), "blocks_drawn", "large_records", "large_draws", "tile_refs", "waves", "sum_slots", "max_env_slots"
  * (record slot bounds), "bad_ids" (out-of-range mesh ids treated as empty slots), "launches" (kernels launched by
- * the call), "arena_bytes".
+ * the call), "arena_bytes", "scratch_bytes".
  * With "timing": "timed_calls" and "ns_cull", "ns_geom", "ns_bin", "ns_raster", "ns_tail" = nanoseconds spent in
  * each kernel class, summed over the calls since timing was started.
  * Unknown names return INVALID_ARG; *out receives the value.

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libgx.so")
 GX_OK, GX_ERR_INVALID_ARG, GX_ERR_CUDA, GX_ERR_OOM, GX_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 GX_BACKGROUND_ID = 0xFFFFFFFF
 EXPORTS = ("gx_create_scene", "gx_render_batch", "gx_render_batch_host", "gx_set_option", "gx_get_stat",
-           "gx_render_batch_obs", "gx_set_robot", "gx_update_transforms", "gx_destroy", "gx_last_error")
+           "gx_render_batch_obs", "gx_set_robot", "gx_update_transforms", "gx_reserve", "gx_destroy", "gx_last_error")
 
 
 class GxMesh(C.Structure):
@@ -55,7 +55,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.gx_last_error.restype = C.c_char_p
         L.gx_destroy.restype = None
-        for n in EXPORTS[:8]:
+        for n in EXPORTS[:9]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -160,6 +160,10 @@ def gx_update_transforms(scene, N: int, K: int, link_slot0: int, base_pose, join
     _check(lib().gx_update_transforms(scene, C.c_int32(N), C.c_int32(K), C.c_int32(link_slot0), _dev(base_pose), _dev(joint_pos),
                                       _dev(held_slot), _dev(held_xform), _dev(cam_pose), _dev(inst_xform),
                                       C.c_void_p(cuda_stream)))
+
+
+def gx_reserve(scene, camera: GxCamera, N: int, K: int) -> None:
+    _check(lib().gx_reserve(scene, C.byref(camera), C.c_int32(N), C.c_int32(K)))
 
 
 def gx_set_option(scene, name: str, value: int) -> None:

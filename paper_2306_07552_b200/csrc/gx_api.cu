@@ -81,6 +81,7 @@ struct GxScene {
     uint32_t max_dyn_nt = 0, max_static_nt = 0;
     uint32_t max_static_batches = 0, max_dyn_batches = 0;   // largest number of batches in any static / dynamic mesh
     int max_smem_optin = 0;
+    int64_t default_pool_bytes = (int64_t)4 << 30;   // arena budget: an eighth of the device's memory, at most 16 GB
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
     // options (gx_set_option)
     int opt_cull = 1, opt_subcull = 1, opt_stats = 0, opt_hiz = 1, opt_big_px = 24;
@@ -309,6 +310,7 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
     if (rc == GX_OK) {
         sc->num_sms = prop.multiProcessorCount;
         sc->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
+        sc->default_pool_bytes = std::min<int64_t>((int64_t)16 << 30, (int64_t)(prop.totalGlobalMem / 8));
     }
     if (rc == GX_OK) rc = upload(sc->verts, verts);
     if (rc == GX_OK) rc = upload(sc->tris, tris);
@@ -409,6 +411,7 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
     if (!strcmp(name, "launches")) { *out = sc->last_launches; return GX_OK; }
     if (!strcmp(name, "timed_calls")) { *out = sc->t_calls; return GX_OK; }
     if (!strcmp(name, "arena_bytes")) { *out = (int64_t)(sc->arena_slots * 88); return GX_OK; }
+    if (!strcmp(name, "scratch_bytes")) { *out = (int64_t)(sc->scratch.n * sizeof(uint32_t)); return GX_OK; }
     if (!strncmp(name, "ns_", 3)) {   // nanoseconds per kernel class, summed over the calls since "timing" was set
         static const char *kinds[6] = {"", "cull", "geom", "bin", "raster", "tail"};
         int kind = 0;
@@ -457,6 +460,81 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
     return fail(GX_ERR_INVALID_ARG, "unknown stat '%s'", name);
 }
 
+// Arena and scratch for a call of this shape: allocates (or grows) what the handle owns and fills the pointers of
+// PP.  PP.g.{N,K,W,H}, PP.T, PP.tiles_x/y and PP.occl must be set.  Allocation happens only when something has to
+// grow (it may synchronise the device); gx_reserve does it ahead of the first render call.
+static int setup_buffers(GxScene *sc, gx::PipeParams &PP, unsigned long long worst_tris) {
+    GxParams &P = PP.g;
+    const int N = P.N, K = P.K;
+    int rc;
+    // ---- arena: record slots shared by the environments of a wave ------------------------------------
+    // An environment's segment is sized by U, the bound cull_kernel computes; the arena must hold the largest
+    // possible U (four slots per triangle: everything clipped by the near plane into two pieces with float
+    // colours), so that a wave always has room for at least one environment.  Beyond that it is sized from the
+    // history of earlier calls (mean U per environment, read back asynchronously) or, on the first call, from a
+    // default of 48 Ki slots per environment, and capped by the budget; what does not fit goes to later waves.
+    if (sc->ctl_pending && cudaEventQuery(sc->ev_ctl) == cudaSuccess) {
+        const uint64_t sum = (uint64_t)sc->h_ctl[gx::C_SUM_U] | ((uint64_t)sc->h_ctl[gx::C_SUM_U + 1] << 32);
+        sc->hist_u_per_env = std::max(sc->hist_u_per_env, (double)sum / (double)std::max(sc->ctl_N, 1));
+        sc->hist_waves = (int)std::min<uint32_t>(std::max<uint32_t>(sc->h_ctl[gx::C_WAVES], 1u), 256u);
+        sc->ctl_pending = false;
+    }
+    cudaGetLastError();   // (cudaErrorNotReady of the query is not an error)
+    const uint64_t worst_env = 4ull * worst_tris + 64;
+    const int64_t budget = sc->opt_pool_bytes > 0 ? sc->opt_pool_bytes : sc->default_pool_bytes;
+    uint64_t want;
+    if (sc->opt_arena_slots > 0) want = (uint64_t)sc->opt_arena_slots;
+    else {
+        const double per_env = sc->hist_u_per_env > 0.0 ? 1.25 * sc->hist_u_per_env + 1024.0 : (double)std::min<uint64_t>(worst_env, 49152);
+        want = std::min<uint64_t>((uint64_t)(per_env * N), (uint64_t)N * worst_env);
+        want = std::min<uint64_t>(want, (uint64_t)budget / 88);
+    }
+    want = std::min<uint64_t>(std::max<uint64_t>(want, worst_env), 0xFFFFFF00ull);
+    if (want > sc->arena_slots) {
+        if ((rc = sc->arena_recs.reserve((size_t)want * 4)) != GX_OK) return rc;
+        if ((rc = sc->arena_bbs.reserve((size_t)want)) != GX_OK) return rc;
+        if ((rc = sc->arena_refs.reserve((size_t)want * 4)) != GX_OK) return rc;
+        sc->arena_slots = (size_t)want;
+    }
+    PP.recs = sc->arena_recs.p; PP.bbs = sc->arena_bbs.p; PP.refs = sc->arena_refs.p;
+    PP.arena_slots = (uint32_t)(sc->opt_arena_slots > 0 ? std::max<uint64_t>((uint64_t)sc->opt_arena_slots, worst_env) : sc->arena_slots);
+
+    // ---- scratch words: ctl | U | rec_base | cnt | cntA | n_large | env_idb | env_mv | tile_off | tasks | hizt | hizb | items | keys
+    const size_t n = (size_t)N, k1 = (size_t)K + 1, NK1 = (size_t)PP.T * gx::NBUCKET + 1;
+    PP.item_stride = (int32_t)std::max<size_t>((size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches, 1);
+    size_t off = 64;
+    const size_t o_U = off; off += n;
+    const size_t o_nitems = off; off += n;
+    const size_t o_cpre = off; off += n + 1;
+    const size_t o_base = off; off += n;
+    const size_t o_cnt = off; off += n;
+    const size_t o_cntA = off; off += n;
+    const size_t o_nl = off; off += n;
+    const size_t o_idb = off; off += n * k1;
+    const size_t o_mv = off; off += n * k1 * 12;
+    const size_t o_toff = off; off += n * NK1;
+    const size_t o_tasks = off; off += (size_t)gx::NCLASS * n * (size_t)PP.T;
+    PP.hz_stride = 0;
+    for (int w = PP.tiles_x, h = PP.tiles_y;; w = (w + 1) >> 1, h = (h + 1) >> 1) { PP.hz_stride += w * h; if (w == 1 && h == 1) break; }
+    const size_t o_hizt = off; off += PP.occl ? n * (size_t)PP.hz_stride : 0;
+    const size_t o_hizb = off; off += PP.occl ? n * (size_t)PP.T * 8 : 0;
+    off = (off + 3) & ~(size_t)3;
+    const size_t o_items = off; off += 4 * n * (size_t)PP.item_stride;
+    const size_t o_witems = off; off += 4 * n * (size_t)PP.item_stride;
+    const size_t o_keys = off; off += PP.occl ? n * (size_t)P.W * (size_t)P.H * 2 : 0;
+    if ((rc = sc->scratch.reserve(off)) != GX_OK) return rc;
+    uint32_t *sp = sc->scratch.p;
+    PP.ctl = sp; PP.U = sp + o_U; PP.n_items = sp + o_nitems; PP.item_pre = sp + o_cpre; PP.rec_base = sp + o_base;
+    PP.cnt = sp + o_cnt; PP.cntA = sp + o_cntA; PP.n_large = sp + o_nl; PP.env_idb = sp + o_idb;
+    PP.env_mv = reinterpret_cast<float *>(sp + o_mv);
+    PP.tile_off = sp + o_toff; PP.tasks = sp + o_tasks; PP.hizt = sp + o_hizt; PP.hizb = sp + o_hizb;
+    PP.items = reinterpret_cast<uint4 *>(sp + o_items);
+    PP.wave_items = reinterpret_cast<uint4 *>(sp + o_witems);
+    PP.keys = reinterpret_cast<unsigned long long *>(sp + o_keys);
+
+    return GX_OK;
+}
+
 static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
                        const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,
                        float *depth_out, uint32_t *id_out, uint16_t *obs_out, float obs_dmin, float obs_dmax,
@@ -501,79 +579,15 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     PP.subcull = sc->opt_subcull;
     PP.big_px = sc->opt_big_px;
     PP.hiz = sc->opt_hiz;
-    PP.occl = sc->opt_hiz && (sc->opt_occlusion == 1 || (sc->opt_occlusion < 0 && P.W * P.H >= 8192)) ? 1 : 0;
+    PP.occl = sc->opt_hiz && (sc->opt_occlusion == 1 || (sc->opt_occlusion < 0 && P.W * P.H >= 4096)) ? 1 : 0;
     PP.occl_area = (float)sc->opt_occl_area;
 
-    // ---- arena: record slots shared by the environments of a wave ------------------------------------
-    // An environment's segment is sized by U, the bound cull_kernel computes; the arena must hold the largest
-    // possible U (four slots per triangle: everything clipped by the near plane into two pieces with float
-    // colours), so that a wave always has room for at least one environment.  Beyond that it is sized from the
-    // history of earlier calls (mean U per environment, read back asynchronously) or, on the first call, from a
-    // default of 48 Ki slots per environment, and capped by the budget; what does not fit goes to later waves.
-    if (sc->ctl_pending && cudaEventQuery(sc->ev_ctl) == cudaSuccess) {
-        const uint64_t sum = (uint64_t)sc->h_ctl[gx::C_SUM_U] | ((uint64_t)sc->h_ctl[gx::C_SUM_U + 1] << 32);
-        sc->hist_u_per_env = std::max(sc->hist_u_per_env, (double)sum / (double)std::max(sc->ctl_N, 1));
-        sc->hist_waves = (int)std::min<uint32_t>(std::max<uint32_t>(sc->h_ctl[gx::C_WAVES], 1u), 256u);
-        sc->ctl_pending = false;
-    }
-    cudaGetLastError();   // (cudaErrorNotReady of the query is not an error)
-    const uint64_t worst_env = 4ull * worst_tris + 64;
-    const int64_t budget = sc->opt_pool_bytes > 0 ? sc->opt_pool_bytes : (int64_t)4 << 30;
-    uint64_t want;
-    if (sc->opt_arena_slots > 0) want = (uint64_t)sc->opt_arena_slots;
-    else {
-        const double per_env = sc->hist_u_per_env > 0.0 ? 1.25 * sc->hist_u_per_env + 1024.0 : (double)std::min<uint64_t>(worst_env, 49152);
-        want = std::min<uint64_t>((uint64_t)(per_env * N), (uint64_t)N * worst_env);
-        want = std::min<uint64_t>(want, (uint64_t)budget / 88);
-    }
-    want = std::min<uint64_t>(std::max<uint64_t>(want, worst_env), 0xFFFFFF00ull);
     int rc;
-    if (want > sc->arena_slots) {
-        if ((rc = sc->arena_recs.reserve((size_t)want * 4)) != GX_OK) return rc;
-        if ((rc = sc->arena_bbs.reserve((size_t)want)) != GX_OK) return rc;
-        if ((rc = sc->arena_refs.reserve((size_t)want * 4)) != GX_OK) return rc;
-        sc->arena_slots = (size_t)want;
-    }
-    PP.recs = sc->arena_recs.p; PP.bbs = sc->arena_bbs.p; PP.refs = sc->arena_refs.p;
-    PP.arena_slots = (uint32_t)(sc->opt_arena_slots > 0 ? std::max<uint64_t>((uint64_t)sc->opt_arena_slots, worst_env) : sc->arena_slots);
-
-    // ---- scratch words: ctl | U | rec_base | cnt | cntA | n_large | env_idb | env_mv | tile_off | tasks | hizt | hizb | items | keys
-    const size_t n = (size_t)N, k1 = (size_t)K + 1, NK1 = (size_t)PP.T * gx::NBUCKET + 1;
-    PP.item_stride = (int32_t)std::max<size_t>((size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches, 1);
-    size_t off = 64;
-    const size_t o_U = off; off += n;
-    const size_t o_nitems = off; off += n;
-    const size_t o_cpre = off; off += n + 1;
-    const size_t o_base = off; off += n;
-    const size_t o_cnt = off; off += n;
-    const size_t o_cntA = off; off += n;
-    const size_t o_nl = off; off += n;
-    const size_t o_idb = off; off += n * k1;
-    const size_t o_mv = off; off += n * k1 * 12;
-    const size_t o_toff = off; off += n * NK1;
-    const size_t o_tasks = off; off += (size_t)gx::NCLASS * n * (size_t)PP.T;
-    PP.hz_stride = 0;
-    for (int w = PP.tiles_x, h = PP.tiles_y;; w = (w + 1) >> 1, h = (h + 1) >> 1) { PP.hz_stride += w * h; if (w == 1 && h == 1) break; }
-    const size_t o_hizt = off; off += PP.occl ? n * (size_t)PP.hz_stride : 0;
-    const size_t o_hizb = off; off += PP.occl ? n * (size_t)PP.T * 8 : 0;
-    off = (off + 3) & ~(size_t)3;
-    const size_t o_items = off; off += 4 * n * (size_t)PP.item_stride;
-    const size_t o_witems = off; off += 4 * n * (size_t)PP.item_stride;
-    const size_t o_keys = off; off += PP.occl ? n * (size_t)P.W * (size_t)P.H * 2 : 0;
-    if ((rc = sc->scratch.reserve(off)) != GX_OK) return rc;
-    uint32_t *sp = sc->scratch.p;
-    PP.ctl = sp; PP.U = sp + o_U; PP.n_items = sp + o_nitems; PP.item_pre = sp + o_cpre; PP.rec_base = sp + o_base;
-    PP.cnt = sp + o_cnt; PP.cntA = sp + o_cntA; PP.n_large = sp + o_nl; PP.env_idb = sp + o_idb;
-    PP.env_mv = reinterpret_cast<float *>(sp + o_mv);
-    PP.tile_off = sp + o_toff; PP.tasks = sp + o_tasks; PP.hizt = sp + o_hizt; PP.hizb = sp + o_hizb;
-    PP.items = reinterpret_cast<uint4 *>(sp + o_items);
-    PP.wave_items = reinterpret_cast<uint4 *>(sp + o_witems);
-    PP.keys = reinterpret_cast<unsigned long long *>(sp + o_keys);
-
+    if ((rc = setup_buffers(sc, PP, worst_tris)) != GX_OK) return rc;
     sc->last_stream = stream;
     if (st) GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
     GX_CUDA(cudaMemsetAsync(PP.ctl, 0, 64 * sizeof(uint32_t), stream));
-    if (PP.occl) GX_CUDA(cudaMemsetAsync(PP.hizt, 0, n * (size_t)PP.hz_stride * sizeof(uint32_t), stream));
+    if (PP.occl) GX_CUDA(cudaMemsetAsync(PP.hizt, 0, (size_t)N * (size_t)PP.hz_stride * sizeof(uint32_t), stream));
     if ((rc = mark(sc, stream, 0)) != GX_OK) return rc;
 
     // K1: one CTA per environment: 4 warps for small scenes, 16 where an environment has thousands of sub-clusters
@@ -662,6 +676,22 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     sc->last_launches = launches + 1;
     if (sc->opt_timing && !sc->t_full) ++sc->t_calls;
     return GX_OK;
+}
+
+int gx_reserve(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K) {
+    if (!sc || !cam) return fail(GX_ERR_INVALID_ARG, "NULL scene or camera");
+    if (N <= 0 || K < 0 || K > GX_MAX_INSTANCES) return fail(GX_ERR_INVALID_ARG, "bad N or K");
+    if (cam->width <= 0 || cam->height <= 0 || cam->width % 16 || cam->height % 16 || cam->width > GX_MAX_FRAME || cam->height > GX_MAX_FRAME)
+        return fail(GX_ERR_INVALID_ARG, "width and height must be positive multiples of 16 up to %d", GX_MAX_FRAME);
+    DeviceGuard guard(sc->device);
+    if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
+    gx::PipeParams PP;
+    memset(&PP, 0, sizeof(PP));
+    PP.g.N = N; PP.g.K = K; PP.g.W = cam->width; PP.g.H = cam->height;
+    PP.tiles_x = cam->width / gx::TILE; PP.tiles_y = cam->height / gx::TILE; PP.T = PP.tiles_x * PP.tiles_y;
+    PP.occl = sc->opt_hiz && (sc->opt_occlusion == 1 || (sc->opt_occlusion < 0 && cam->width * cam->height >= 4096)) ? 1 : 0;
+    const unsigned long long worst_tris = (unsigned long long)sc->max_static_nt + (unsigned long long)K * sc->max_dyn_nt;
+    return setup_buffers(sc, PP, worst_tris);
 }
 
 int gx_render_batch(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,

@@ -320,6 +320,27 @@ def test_reference_area_fallback(oracle_mod):
             assert g["stats"]["large_records"] == nt
 
 
+def test_reserve_then_no_growth(oracle_mod):
+    """gx_reserve sizes the arena and the tables for a call shape ahead of time: the render calls that follow leave
+    "arena_bytes" and "scratch_bytes" unchanged (ADVICE: no hidden allocation in the steady state), and the budget
+    option bounds the arena."""
+    from paper_2306_07552_b200 import binding as gx
+    wl = gen.make_config(1, n_envs=24)
+    sc = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, 0)
+    try:
+        gx.gx_set_option(sc, "pool_bytes", 256 << 20)
+        gx.gx_reserve(sc, gx.camera_of(wl), wl.N, wl.K)
+        a0, s0 = gx.gx_get_stat(sc, "arena_bytes"), gx.gx_get_stat(sc, "scratch_bytes")
+        assert 0 < a0 <= (256 << 20) + 88 * (4 * 71600 + 64) and s0 > 0
+        o = oracle_mod.render(wl)
+        for _ in range(3):
+            g = render_gpu(wl, scene=sc)
+            assert compare(o, g)["id_mismatch"] == 0
+            assert gx.gx_get_stat(sc, "arena_bytes") == a0 and gx.gx_get_stat(sc, "scratch_bytes") == s0
+    finally:
+        gx.gx_destroy(sc)
+
+
 def test_argument_errors():
     import torch
     from paper_2306_07552_b200 import binding as gx
