@@ -200,7 +200,7 @@ int gx_set_option(GxScene *scene, const char *name, int64_t value);
  * "fragments" (pixel-centre hits that reached the depth test), "records_occluded" (references dropped by hi-Z in
  * the tiles), "blocks_drawn", "large_records", "large_draws", "tile_refs", "waves", "sum_slots", "max_env_slots"
  * (record slot bounds), "bad_ids" (out-of-range mesh ids treated as empty slots), "launches" (kernels launched by
- * the call), "arena_bytes", "scratch_bytes".
+ * the call), "arena_bytes", "scratch_bytes", "bound_violations" (the kernels' own index checks in the stats build: always 0).
  * With "timing": "timed_calls" and "ns_cull", "ns_geom", "ns_bin", "ns_raster", "ns_tail" = nanoseconds spent in
  * each kernel class, summed over the calls since timing was started.
  * Unknown names return INVALID_ARG; *out receives the value.

@@ -447,7 +447,7 @@ int gx_get_stat(GxScene *sc, const char *name, int64_t *out) {
     }
     static const char *names[GX_NSTAT] = {"clusters_tested", "clusters_drawn", "triangles_in", "triangles_raster",
                                           "fragments", "records_occluded", "blocks_drawn", "tile_refs", "triangles_hidden",
-                                          "subclusters_hidden", "large_records", "large_draws"};
+                                          "subclusters_hidden", "large_records", "large_draws", "bound_violations"};
     for (int k = 0; k < GX_NSTAT; ++k)
         if (!strcmp(name, names[k])) {
             DeviceGuard guard(sc->device);

@@ -449,7 +449,8 @@ __device__ __forceinline__ void store_record(const PipeParams &PP, size_t at, bo
 
 // One record per lane at most (kind 0 = none, 1 = small, 2 = large; pair = a colour slot follows): the warp
 // reserves its slots with one atomic.  (Slots used <= U by construction of U, cull_kernel.)
-__device__ __forceinline__ void emit_records(const PipeParams &PP, int env, uint32_t base, int lane, int kind,
+template <bool STATS>
+__device__ __forceinline__ void emit_records(const PipeParams &PP, int env, uint32_t base, uint32_t U, int lane, int kind,
                                              bool pair, const uint32_t w[14], const float (*oc)[3], uint32_t qmax_bits) {
     const unsigned FULL = 0xFFFFFFFFu, lt = (1u << lane) - 1u;
     const unsigned m = __ballot_sync(FULL, kind != 0), mp = __ballot_sync(FULL, pair);
@@ -458,7 +459,9 @@ __device__ __forceinline__ void emit_records(const PipeParams &PP, int env, uint
     if (lane == 0) bs = atomicAdd(&PP.cnt[env], (unsigned)(__popc(m) + __popc(m & mp)));
     bs = __shfl_sync(FULL, bs, 0);
     if (kind == 0) return;
-    store_record(PP, (size_t)base + bs + (uint32_t)(__popc(m & lt) + __popc(m & mp & lt)), kind == 2, pair, w, oc, qmax_bits);
+    const uint32_t slot = bs + (uint32_t)(__popc(m & lt) + __popc(m & mp & lt));
+    if (STATS && slot + (pair ? 1u : 0u) >= U) atomicAdd(&PP.g.stats[GX_STAT_VIOLATIONS], 1ull);   // (own bounds check)
+    store_record(PP, (size_t)base + slot, kind == 2, pair, w, oc, qmax_bits);
 }
 
 // K2 for one batch, by one warp.  sub_mask: bit r set = pass r of the triangle loop (32 consecutive triangles,
@@ -574,6 +577,7 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
             }
         }
         const unsigned mg = __ballot_sync(FULL, kind != 0);
+        if (STATS && kind && bs0 + (uint32_t)(used + __popc(mg & lt)) >= U) atomicAdd(&P.stats[GX_STAT_VIOLATIONS], 1ull);   // (own bounds check)
         if (kind) store_record(PP, (size_t)base + bs0 + (uint32_t)(used + __popc(mg & lt)), kind == 2, false, w, nullptr, qmax_bits);
         used += __popc(mg);
     }
@@ -655,7 +659,7 @@ __device__ __forceinline__ void geom_batch(const PipeParams &PP, const Proj &pj,
                     }
                 }
             }
-            emit_records(PP, env, base, lane, kind, pair, w, oc, qmax_bits);
+            emit_records<STATS>(PP, env, base, U, lane, kind, pair, w, oc, qmax_bits);
         }
     }
     __syncwarp();
@@ -935,6 +939,7 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
             bool wide;
             const unsigned long long m = large_mask<COOP>(PP, env_recs + (size_t)s * 4, b.x, wide);
             const uint32_t at = s_loff[bk] + atomicAdd(&s_lcnt[bk], 1u);
+            if (STATS && (at >= n_large || s >= ns)) atomicAdd(&PP.g.stats[GX_STAT_VIOLATIONS], 1ull);   // (own bounds check)
             elarge[U - 1 - at] = make_uint4(s | (wide ? 0x80000000u : 0u), (uint32_t)m, (uint32_t)(m >> 32), qb);
         };
         for (uint32_t s = s_lo + tid; s < ns; s += NT) {
@@ -950,7 +955,9 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
             for (int ty = j0 >> 4; ty <= (j1 >> 4); ++ty)
                 for (int tx = i0 >> 4; tx <= (i1 >> 4); ++tx) {
                     const int key = (ty * PP.tiles_x + tx) * NBUCKET + bk;
-                    erefs[s_off[key] + atomicAdd(&s_cnt[key], 1u)] = s;
+                    const uint32_t at = s_off[key] + atomicAdd(&s_cnt[key], 1u);
+                    if (STATS && (unsigned long long)at + 4ull * n_large >= 4ull * U) atomicAdd(&PP.g.stats[GX_STAT_VIOLATIONS], 1ull);   // (own bounds check)
+                    erefs[at] = s;
                 }
         }
         if (listed)
@@ -1561,7 +1568,8 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
                     const bool have = r0 + lane < r_end;
                     const uint32_t slot = have ? ldi<COOP>(&erefs[r0 + lane]) : 0u;
                     bool keep = have;
-                    if (have && PP.hiz) {
+                    if (STATS && have && slot >= U) { atomicAdd(&P.stats[GX_STAT_VIOLATIONS], 1ull); keep = false; }   // (own bounds check)
+                    if (keep && PP.hiz) {
                         const uint2 b = ldi<COOP>(&ebb[slot]);
                         const int i0 = (int)(b.x & 255u), j0 = (int)((b.x >> 8) & 255u);
                         const int x = max(i0, x0) - x0, y = max(j0, y0) - y0;

@@ -61,4 +61,4 @@ struct GxParams {
 
 enum { GX_STAT_CLUSTERS_TESTED = 0, GX_STAT_CLUSTERS_DRAWN, GX_STAT_TRIS_IN, GX_STAT_TRIS_RASTER,
        GX_STAT_FRAGMENTS, GX_STAT_RECORDS_OCCLUDED, GX_STAT_BLOCKS_DRAWN, GX_STAT_REFS, GX_STAT_TRIS_HIDDEN,
-       GX_STAT_SUBS_HIDDEN, GX_STAT_LARGE, GX_STAT_LARGE_DRAWS, GX_NSTAT };
+       GX_STAT_SUBS_HIDDEN, GX_STAT_LARGE, GX_STAT_LARGE_DRAWS, GX_STAT_VIOLATIONS, GX_NSTAT };

@@ -52,8 +52,9 @@ def render_gpu(wl, want_id=True, want_rgb=None, cull=1, stats=False, scene=None,
             out["stats"] = {k: gx.gx_get_stat(scene, k) for k in
                             ("clusters_tested", "clusters_drawn", "triangles_in", "triangles_raster", "fragments",
                              "records_occluded", "blocks_drawn", "tile_refs", "triangles_hidden", "subclusters_hidden",
-                             "large_records", "large_draws", "waves", "sum_slots", "max_env_slots",
+                             "large_records", "large_draws", "bound_violations", "waves", "sum_slots", "max_env_slots",
                              "bad_ids", "launches")}
+            assert out["stats"]["bound_violations"] == 0, out["stats"]     # the kernels' own bounds checks (stats build)
         return out
     finally:
         if own:
