@@ -85,6 +85,7 @@ struct GxScene {
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
     // options (gx_set_option)
     int opt_cull = 1, opt_subcull = 1, opt_stats = 0, opt_hiz = 1, opt_big_px = 24;
+    int opt_bin_threads = 0;
     int opt_host_sub = 0;               // gx_render_batch_host: environments per sub-batch; 0 = automatic
     int opt_occlusion = -1;             // occluder scheme: 1 on, 0 off, -1 automatic (on for frames of at least 8192 pixels)
     int opt_occl_area = 64;             // pixels per triangle of a sub-cluster's screen box that make it an occluder
@@ -113,7 +114,7 @@ struct GxScene {
     int last_launches = 0;
     cudaStream_t last_stream = nullptr;
     // launch configurations, resolved once per kernel instantiation (occupancy queries are not free)
-    struct Plan { const void *fn; size_t smem; int per_sm; };
+    struct Plan { const void *fn; size_t smem; int threads; int per_sm; };
     std::vector<Plan> plans;
     // robot description (gx_set_robot)
     gx::FkLink *fk_links = nullptr;
@@ -228,12 +229,12 @@ int upload(T *&dst, const std::vector<T> &src) {
 // blocks per SM of a kernel at a block size and dynamic shared memory size; sets the opt-in attribute once
 int plan_of(GxScene *sc, const void *fn, int threads, size_t smem, int *per_sm) {
     for (const GxScene::Plan &p : sc->plans)
-        if (p.fn == fn && p.smem == smem) { *per_sm = p.per_sm; return GX_OK; }
+        if (p.fn == fn && p.smem == smem && p.threads == threads) { *per_sm = p.per_sm; return GX_OK; }
     GX_CUDA(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int n = 0;
     GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, threads, smem));
     if (n < 1) return fail(GX_ERR_UNSUPPORTED, "kernel does not fit: %zu bytes of shared memory", smem);
-    sc->plans.push_back({fn, smem, n});
+    sc->plans.push_back({fn, smem, threads, n});
     *per_sm = n;
     return GX_OK;
 }
@@ -371,6 +372,11 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
     if (!strcmp(name, "timing")) {   // 1 = start (and reset) the per-kernel event timing, 0 = stop recording
         sc->opt_timing = value != 0;
         if (value) { sc->t_used = 0; sc->t_calls = 0; sc->t_full = false; }
+        return GX_OK;
+    }
+    if (!strcmp(name, "bin_threads")) {   // (development)
+        if (value != 0 && value != 256 && value != 512 && value != 1024) return fail(GX_ERR_INVALID_ARG, "bin_threads must be 0, 256, 512 or 1024");
+        sc->opt_bin_threads = (int)value;
         return GX_OK;
     }
     if (!strcmp(name, "host_sub")) {
@@ -636,8 +642,10 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
             auto bk = st ? gx::bin_kernel<true> : gx::bin_kernel<false>;
             const size_t bsmem = (size_t)2 * PP.T * gx::NBUCKET * 4;
             int per_sm = 0;
-            if ((rc = plan_of(sc, (const void *)bk, 256, bsmem, &per_sm)) != GX_OK) return rc;
-            bk<<<std::min(N, sc->num_sms * per_sm), 256, bsmem, stream>>>(PP, phase);
+            // (thread t of the CTA owns tile t in the scan, so a CTA has at least T = 256 threads at the largest frame)
+            const int bthreads = sc->opt_bin_threads ? sc->opt_bin_threads : 512;
+            if ((rc = plan_of(sc, (const void *)bk, bthreads, bsmem, &per_sm)) != GX_OK) return rc;
+            bk<<<std::min(N, sc->num_sms * per_sm), bthreads, bsmem, stream>>>(PP, phase);
             GX_CUDA(cudaGetLastError());
             if ((rc = mark(sc, stream, 3)) != GX_OK) return rc;
         }
