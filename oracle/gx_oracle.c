@@ -36,6 +36,8 @@
  * the renderer reads.  N12 pins: its own sine / cosine against float64 and the exact values at 0; closed forms
  * (joints at 0 with dyadic offsets, a quarter turn about each axis, a prismatic joint, base yaw); random
  * chains against a float64 composition; parent / child and held-object identities.
+ * And N13, the batch collision queries of the kinematic simulator (spheres against column grids and oriented boxes,
+ * PAPER.md:111-119, App. G): pins in tests/test_collide_pins.py (closed forms, boundary cases, float64 brute force).
  */
 #include <math.h>
 #include <stdint.h>
@@ -564,4 +566,95 @@ int gx_oracle_fk(const GxOracleLink *links, int32_t L, int32_t camera_link, cons
 /* N12a alone, for its pins */
 void gx_oracle_sincos(const float *x, float *s, float *c, size_t n) {
     for (size_t i = 0; i < n; ++i) n12_sincos(x[i], &s[i], &c[i]);
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * N13: batch collision queries of the kinematic simulator (N13; PAPER.md:111-119 and
+ * Appendix G): every sphere of the robot against the static scene's column grid of its radius
+ * and against the oriented boxes of the resting movable objects.  The paper's regular grids and its layer cache
+ * are accelerations that do not change the answer, so the oracle is the plain definition: nearest column, linear
+ * search of its layers from the first; every object, one after the other.  All operations binary32.
+ * ------------------------------------------------------------------------------------------------ */
+typedef struct {
+    float x0, z0;            /* world position of column (0, 0) */
+    float spacing;           /* 0.03 m in the paper */
+    int32_t nx, nz;
+    const uint32_t *col_off; /* [nx*nz + 1] first layer of column iz*nx + ix */
+    const float *layers;     /* [..][2] lo, hi: free heights of the sphere CENTRE (the radius is baked in) */
+} GxOracleColumnGrid;
+
+typedef struct {
+    int32_t link;            /* link the sphere is attached to (>= 0) */
+    int32_t radius_class;    /* index into radii[] */
+    float centre[3];         /* in the link's frame */
+} GxOracleSphere;
+
+/* object-space box of a mesh: centre 0.5f*(min+max), half extent 0.5f*(max-min) of its vertex positions */
+static void n13_mesh_box(const OrMesh *m, float *ctr, float *half) {
+    float lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+    for (uint32_t v = 0; v < m->nv; ++v)
+        for (int a = 0; a < 3; ++a) {
+            const float p = m->positions[3 * (size_t)v + a];
+            if (v == 0 || p < lo[a]) lo[a] = p;
+            if (v == 0 || p > hi[a]) hi[a] = p;
+        }
+    for (int a = 0; a < 3; ++a) { ctr[a] = 0.5f * (lo[a] + hi[a]); half[a] = 0.5f * (hi[a] - lo[a]); }
+}
+
+/* out_static[n][s] = 1 if sphere s of environment n is in obstructed space of its column grid (or outside the grid),
+ * out_object[n][s] = lowest instance slot in [obj_slot0, obj_slot0 + n_obj) whose box the sphere overlaps (distance
+ * from the centre to the box <= radius), skipping empty slots and held_slot[n]; -1 if none.
+ * grids: [n_static][n_radii].  Sphere centres: W_link * centre with W_link = inst_xform[n][link_slot0 + link].
+ * Returns 0, or -1 on bad arguments. */
+int gx_oracle_collide(const OrMesh *dyn_meshes, int32_t n_dyn, const GxOracleColumnGrid *grids, int32_t n_static,
+                      int32_t n_radii, const float *radii, const GxOracleSphere *spheres, int32_t S, int32_t N, int32_t K,
+                      const int32_t *env_scene, const int32_t *inst_mesh, const float *inst_xform, int32_t link_slot0,
+                      int32_t obj_slot0, int32_t n_obj, const int32_t *held_slot /* [N] or NULL */, uint8_t *out_static,
+                      int32_t *out_object) {
+    if (!grids || !radii || !spheres || S <= 0 || N <= 0 || !env_scene || !inst_xform || !out_static || !out_object) return -1;
+    if (obj_slot0 < 0 || n_obj < 0 || obj_slot0 + n_obj > K || (n_obj > 0 && (!inst_mesh || !dyn_meshes))) return -1;
+    for (int n = 0; n < N; ++n) {
+        if (env_scene[n] < 0 || env_scene[n] >= n_static) return -1;
+        for (int s = 0; s < S; ++s) {
+            const GxOracleSphere *sp = &spheres[s];
+            if (sp->link < 0 || link_slot0 + sp->link >= K || sp->radius_class < 0 || sp->radius_class >= n_radii) return -1;
+            const float *Wl = inst_xform + ((size_t)n * K + link_slot0 + sp->link) * 16;
+            float c[3];
+            for (int i = 0; i < 3; ++i)   /* N3's order */
+                c[i] = fmaf(Wl[i * 4 + 2], sp->centre[2], fmaf(Wl[i * 4 + 1], sp->centre[1], fmaf(Wl[i * 4], sp->centre[0], Wl[i * 4 + 3])));
+            /* static scene: nearest column, then its layers */
+            const GxOracleColumnGrid *g = &grids[(size_t)env_scene[n] * n_radii + sp->radius_class];
+            const float fx = rintf((c[0] - g->x0) / g->spacing), fz = rintf((c[2] - g->z0) / g->spacing);
+            int hit = 1;
+            if (fx >= 0.0f && fx < (float)g->nx && fz >= 0.0f && fz < (float)g->nz) {
+                const size_t col = (size_t)(int)fz * g->nx + (size_t)(int)fx;
+                for (uint32_t l = g->col_off[col]; l < g->col_off[col + 1]; ++l)
+                    if (g->layers[2 * (size_t)l] <= c[1] && c[1] <= g->layers[2 * (size_t)l + 1]) { hit = 0; break; }
+            }
+            out_static[(size_t)n * S + s] = (uint8_t)hit;
+            /* resting movable objects: every slot, lowest overlapping one */
+            const float r = radii[sp->radius_class], r2 = r * r;
+            int found = -1;
+            for (int k = obj_slot0; k < obj_slot0 + n_obj && found < 0; ++k) {
+                const int mesh = inst_mesh[(size_t)n * K + k];
+                if (mesh < 0 || (held_slot && held_slot[n] == k)) continue;
+                if (mesh >= n_dyn) return -1;
+                float bc[3], bh[3];
+                n13_mesh_box(&dyn_meshes[mesh], bc, bh);
+                const float *M = inst_xform + ((size_t)n * K + k) * 16;
+                const float d[3] = {c[0] - M[3], c[1] - M[7], c[2] - M[11]};
+                float e[3];
+                for (int i = 0; i < 3; ++i) {
+                    const float loc = fmaf(M[8 + i], d[2], fmaf(M[4 + i], d[1], M[i] * d[0]));   /* R^T d */
+                    const float rel = loc - bc[i];
+                    const float q = fminf(fmaxf(rel, -bh[i]), bh[i]);
+                    e[i] = rel - q;
+                }
+                const float dist2 = fmaf(e[2], e[2], fmaf(e[1], e[1], e[0] * e[0]));
+                if (dist2 <= r2) found = k;
+            }
+            out_object[(size_t)n * S + s] = found;
+        }
+    }
+    return 0;
 }

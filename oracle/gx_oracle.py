@@ -216,3 +216,52 @@ def fk(robot, base_pose, joint_pos, K: int, link_slot0: int, inst_xform: Optiona
     if rc != 0:
         raise ValueError("gx_oracle_fk: bad arguments")
     return cam, xf
+
+
+class _ColumnGrid(C.Structure):
+    _fields_ = [("x0", C.c_float), ("z0", C.c_float), ("spacing", C.c_float), ("nx", C.c_int32), ("nz", C.c_int32),
+                ("col_off", C.c_void_p), ("layers", C.c_void_p)]
+
+
+class _Sphere(C.Structure):
+    _fields_ = [("link", C.c_int32), ("radius_class", C.c_int32), ("centre", C.c_float * 3)]
+
+
+def collide(dyn_meshes, grids, radii, spheres, env_scene, inst_mesh, inst_xform, link_slot0: int, obj_slot0: int,
+            n_obj: int, held_slot: Optional[np.ndarray] = None):
+    """N13: batch collision queries.  grids: [n_static][n_radii] objects with x0, z0, spacing, nx, nz, col_off, layers
+    (gen.ColumnGrid); spheres: objects with link, radius_class, centre.  Returns (static [N,S] uint8, object [N,S] int32)."""
+    lib = _load()
+    dm, keep = _meshes(dyn_meshes)
+    n_static, n_radii = len(grids), len(radii)
+    garr = (_ColumnGrid * (n_static * n_radii))()
+    for i, row in enumerate(grids):
+        assert len(row) == n_radii
+        for j, g in enumerate(row):
+            off = np.ascontiguousarray(g.col_off, np.uint32)
+            lay = np.ascontiguousarray(g.layers, np.float32).reshape(-1, 2)
+            keep += [off, lay]
+            garr[i * n_radii + j] = _ColumnGrid(float(g.x0), float(g.z0), float(g.spacing), int(g.nx), int(g.nz),
+                                                off.ctypes.data, lay.ctypes.data)
+    S = len(spheres)
+    sarr = (_Sphere * S)()
+    for i, s in enumerate(spheres):
+        sarr[i].link = int(s.link)
+        sarr[i].radius_class = int(s.radius_class)
+        for k in range(3):
+            sarr[i].centre[k] = float(np.float32(s.centre[k]))
+    rad = np.ascontiguousarray(radii, np.float32)
+    env_scene = np.ascontiguousarray(env_scene, np.int32)
+    inst_mesh = np.ascontiguousarray(inst_mesh, np.int32)
+    inst_xform = np.ascontiguousarray(inst_xform, np.float32)
+    N, K = inst_mesh.shape
+    hs = None if held_slot is None else np.ascontiguousarray(held_slot, np.int32)
+    out_s = np.empty((N, S), np.uint8)
+    out_o = np.empty((N, S), np.int32)
+    lib.gx_oracle_collide.restype = C.c_int
+    rc = lib.gx_oracle_collide(dm, C.c_int32(len(dyn_meshes)), garr, C.c_int32(n_static), C.c_int32(n_radii), _p(rad), sarr,
+                               C.c_int32(S), C.c_int32(N), C.c_int32(K), _p(env_scene), _p(inst_mesh), _p(inst_xform),
+                               C.c_int32(link_slot0), C.c_int32(obj_slot0), C.c_int32(n_obj), _p(hs), _p(out_s), _p(out_o))
+    if rc != 0:
+        raise ValueError("gx_oracle_collide: bad arguments")
+    return out_s, out_o

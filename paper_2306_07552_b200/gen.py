@@ -665,3 +665,121 @@ def robot_states(robot: Robot, n: int, seed: int = 0):
     hx = np.tile(np.array([1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, -0.12], np.float32), (n, 1))
     hx[:, 3] = g.uniform(-0.02, 0.02, n).astype(np.float32)
     return base, joints, held, hx
+
+
+# ----------------------------------------------------------------------------------------------
+# collision queries (N13; Appendix G): column grids, robot spheres, resting objects
+# ----------------------------------------------------------------------------------------------
+
+SPHERE_RADII = (0.015, 0.05, 0.12)      # the paper's sphere-radius working set
+COLUMN_SPACING = 0.03
+
+
+@dataclass
+class ColumnGrid:
+    """Free space of one static scene for one sphere radius: a dense array of columns in the XZ plane, each a
+    list of layers (lo, hi) of heights the sphere's CENTRE may take.  Data only."""
+    x0: float
+    z0: float
+    spacing: float
+    nx: int
+    nz: int
+    col_off: np.ndarray      # [nx*nz + 1] uint32, column iz*nx + ix
+    layers: np.ndarray       # [n,2] float32
+
+
+@dataclass
+class Sphere:
+    link: int
+    radius_class: int
+    centre: Tuple[float, float, float]
+
+
+_grid_cache: Dict = {}
+
+
+def column_grid(cfg: int, scene: int, radius: float, extent: Optional[Tuple[float, float, float, float]] = None) -> ColumnGrid:
+    """The column grid of a procedural apartment (stands in for the paper's offline pass over a ReplicaCAD scene with
+    Habitat 2.0 sphere queries): a column is closed within radius + 5 cm of a wall; furniture whose
+    footprint comes within the radius blocks the heights [0, top + radius], or, for every third piece (a 'table'),
+    only [0.7 top - radius, top + radius]; the floor and the ceiling bound what is left.  extent = (x0, z0, x1, z1)
+    restricts the grid to a window (tests)."""
+    key = (cfg, scene, radius, extent)
+    if key in _grid_cache:
+        return _grid_cache[key]
+    n_tris = CONFIG_SHAPES[cfg][5]
+    info = _scenes(cfg, scene + 1, n_tris)[scene][1]
+    boxes, segs = info["boxes"], info["segs"]
+    x0, z0, x1, z1 = extent if extent is not None else (0.0, 0.0, FOOT, FOOT)
+    nx, nz = int(round((x1 - x0) / COLUMN_SPACING)) + 1, int(round((z1 - z0) / COLUMN_SPACING)) + 1
+    col_off = np.zeros(nx * nz + 1, np.uint32)
+    layers: List[Tuple[float, float]] = []
+    table = (np.arange(len(boxes)) % 3) == 2
+    for iz in range(nz):
+        px = x0 + COLUMN_SPACING * np.arange(nx)
+        pz = np.full(nx, z0 + COLUMN_SPACING * iz)
+        wall = _dist_segs(px, pz, segs).min(-1) < radius + 0.05
+        near = _dist_boxes(px, pz, boxes) < radius                     # [nx, B]
+        for ix in range(nx):
+            if not wall[ix]:
+                blocked = [(0.7 * boxes[b, 5] - radius if table[b] else -1.0, boxes[b, 5] + radius) for b in np.flatnonzero(near[ix])]
+                lo = radius
+                for b0, b1 in sorted(blocked):
+                    if b0 > lo:
+                        layers.append((lo, b0))
+                    lo = max(lo, b1)
+                if HEIGHT - radius > lo:
+                    layers.append((lo, HEIGHT - radius))
+            col_off[iz * nx + ix + 1] = len(layers)
+    g = ColumnGrid(float(np.float32(x0)), float(np.float32(z0)), float(np.float32(COLUMN_SPACING)), nx, nz, col_off,
+                   np.asarray(layers, np.float32).reshape(-1, 2))
+    _grid_cache[key] = g
+    return g
+
+
+def robot_spheres(robot: Robot) -> List[Sphere]:
+    """Spheres of the robot proxy (the paper authors them by hand for Fetch): big ones fill the base
+    and the torso, medium and small ones run along the arm links and the hand."""
+    out = [Sphere(0, 2, (dx, 0.0, dz)) for dx in (-0.12, 0.12) for dz in (-0.12, 0.12)]
+    out += [Sphere(1, 2, (0.0, dy, 0.0)) for dy in (-0.15, 0.05, 0.25)]
+    out += [Sphere(2, 1, (0.0, 0.0, -d)) for d in (0.0, 0.09, 0.18, 0.27)]
+    out += [Sphere(3, 1, (0.0, 0.0, -d)) for d in (0.04, 0.12, 0.20, 0.28)]
+    out += [Sphere(4, 0, (dx, 0.0, -d)) for d in (0.02, 0.08, 0.14, 0.20) for dx in (-0.02, 0.02)]
+    assert all(0 <= s.link < len(robot.parent) for s in out)
+    return out
+
+
+def collision_world(n_envs: int, seed: int = 0, cfg: int = 1, extent: Optional[Tuple[float, float, float, float]] = None):
+    """A batch of collision queries shaped like the paper's step (1 target + 29 distractor objects
+    per episode; App. G): the robot proxy with its spheres in n_envs environments of one apartment, 30 resting
+    box-shaped objects per environment (three meshes of different extents, rigid random poses on the floor near
+    the robot or further away), the hand holding object 0 in half of them.  Returns a dict of plain arrays."""
+    g = _rng(10, seed)
+    robot = robot_proxy()
+    base, joints, held, hx = robot_states(robot, n_envs, seed=seed)
+    if extent is not None:
+        base[:, 0] = g.uniform(extent[0] + 0.3, extent[2] - 0.3, n_envs).astype(np.float32)
+        base[:, 1] = g.uniform(extent[1] + 0.3, extent[3] - 0.3, n_envs).astype(np.float32)
+    meshes = [box_mesh(d, (1, 1, 1), _rng(10, 100 + i)) for i, d in enumerate(((0.06, 0.18, 0.06), (0.16, 0.08, 0.10), (0.09, 0.09, 0.22)))]
+    n_obj, L = 30, len(robot.parent)
+    K = n_obj + L
+    inst_mesh = np.full((n_envs, K), -1, np.int32)
+    inst_mesh[:, :n_obj] = g.integers(0, 3, (n_envs, n_obj))
+    inst_mesh[:, 7] = -1                                                  # an empty slot among the objects
+    xf = np.tile(np.eye(4, dtype=np.float32).reshape(16), (n_envs, K, 1))
+    for n in range(n_envs):
+        for k in range(n_obj):
+            near = g.uniform() < 0.5
+            rad = g.uniform(0.2, 0.9) if near else g.uniform(1.0, 4.0)
+            ang = g.uniform(0, 2 * np.pi)
+            yaw, tilt = g.uniform(0, 2 * np.pi), (g.uniform(-0.5, 0.5) if g.uniform() < 0.3 else 0.0)
+            cy, sy, ct, st = np.cos(yaw), np.sin(yaw), np.cos(tilt), np.sin(tilt)
+            R = np.array([[cy, 0, sy], [0, 1, 0], [-sy, 0, cy]]) @ np.array([[1, 0, 0], [0, ct, -st], [0, st, ct]])
+            M = np.eye(4)
+            M[:3, :3] = R
+            M[:3, 3] = [base[n, 0] + rad * np.cos(ang), g.uniform(0.03, 1.3), base[n, 1] + rad * np.sin(ang)]
+            xf[n, k] = M.astype(np.float32).reshape(16)
+    held_slot = np.where(held >= 0, 0, -1).astype(np.int32)
+    return dict(robot=robot, spheres=robot_spheres(robot), radii=np.asarray(SPHERE_RADII, np.float32), dyn_meshes=meshes,
+                base_pose=base, joint_pos=joints, held_slot=held_slot, held_xform=hx, inst_mesh=inst_mesh, inst_xform=xf,
+                env_scene=np.zeros(n_envs, np.int32), K=K, link_slot0=n_obj, obj_slot0=0, n_obj=n_obj, cfg=cfg)
