@@ -54,6 +54,9 @@ def parse_args():
     ap.add_argument("--obs", action="store_true",
                     help="time gx_render_batch_obs (packed [N,4,H,W] float16 observation, DESIGN.md N11) instead of "
                          "gx_render_batch; device timing only")
+    ap.add_argument("--collide", action="store_true",
+                    help="also time the batch collision queries (gx_collide_batch, DESIGN.md N13) on this rank's environments; "
+                         "building the column grids on the host takes about half a minute")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="gx_set_option before rendering (development: e.g. --opt occlusion=0)")
     return ap.parse_args()
@@ -309,6 +312,50 @@ def run_gx(args):
         step()      # leave the handle's history and the images as the render-only step made them
         torch.cuda.synchronize()
 
+    # ---- batch collision queries (N13): the robot's spheres against column grids and resting objects -------------
+    collide = None
+    if args.collide:
+        from paper_2306_07552_b200 import gen as _gen
+        ext = (2.0, 2.0, 10.0, 10.0)
+        grids = [[_gen.column_grid(1, 0, r, ext) for r in _gen.SPHERE_RADII]]
+        cw = _gen.collision_world(N, seed=rank, extent=ext)
+        room = _gen.Mesh(np.zeros((3, 3), np.float32), np.zeros((3, 3), np.uint8), np.array([[0, 1, 2]], np.uint32))
+        sc2 = gx.gx_create_scene([room], cw["dyn_meshes"], local)
+        gx.gx_set_robot(sc2, cw["robot"])
+        gx.gx_set_collision_world(sc2, grids, cw["radii"], cw["spheres"])
+        t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        c_in = [t(cw[k]) for k in ("base_pose", "joint_pos", "held_slot", "held_xform", "env_scene", "inst_mesh")]
+        c_xf, c_cam = t(cw["inst_xform"].astype(np.float32)), torch.zeros((N, 16), dtype=torch.float32, device=dev)
+        S = len(cw["spheres"])
+        o_s, o_o = torch.zeros((N, S), dtype=torch.uint8, device=dev), torch.zeros((N, S), dtype=torch.int32, device=dev)
+
+        def fk_collide():
+            gx.gx_update_transforms(sc2, N, cw["K"], cw["link_slot0"], c_in[0], c_in[1], c_in[2], c_in[3], c_cam, c_xf, stream)
+            gx.gx_collide_batch(sc2, N, cw["K"], c_in[4], c_in[5], c_xf, cw["link_slot0"], 0, cw["n_obj"], c_in[2], o_s, o_o, stream)
+        for _ in range(3):
+            fk_collide()
+        torch.cuda.synchronize()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for a, b in evs:
+            flush.zero_()
+            a.record(); fk_collide(); b.record()
+        torch.cuda.synchronize()
+        ms_c = float(np.mean([a.elapsed_time(b) for a, b in evs]))
+        import oracle as _oracle
+        _oracle.build()
+        t0 = time.perf_counter()
+        _, xfo = _oracle.fk(cw["robot"], cw["base_pose"], cw["joint_pos"], cw["K"], cw["link_slot0"], inst_xform=cw["inst_xform"],
+                            held_slot=cw["held_slot"], held_xform=cw["held_xform"])
+        so, oo = _oracle.collide(cw["dyn_meshes"], grids, cw["radii"], cw["spheres"], cw["env_scene"], cw["inst_mesh"], xfo,
+                                 cw["link_slot0"], 0, cw["n_obj"], cw["held_slot"])
+        cpu_ms = 1e3 * (time.perf_counter() - t0)
+        assert np.array_equal(so, o_s.cpu().numpy()) and np.array_equal(oo, o_o.cpu().numpy())
+        collide = {"fk_plus_collide_ms": ms_c, "sphere_queries_per_s": N * S / (ms_c * 1e-3), "spheres_per_env": S,
+                   "objects_per_env": cw["n_obj"], "columns_per_grid": grids[0][0].nx * grids[0][0].nz,
+                   "oracle_ms_1core": cpu_ms, "static_hit_rate": float(so.mean()), "object_hit_rate": float((oo >= 0).mean()),
+                   "note": "gx_update_transforms + gx_collide_batch (N13) for every environment of the batch; equal to the oracle's answer"}
+        gx.gx_destroy(sc2)
+
     # ---- e2e: host buffers in, host buffers out, through gx_render_batch_host -------------------------
     e2e = None
     if not args.no_e2e and not args.obs:
@@ -406,7 +453,7 @@ def run_gx(args):
                    "l2": "256 MB buffer written between timed iterations (untimed)",
                    "arithmetic": "f32 vertex stage, i32/i64 fixed-point coverage, f32 depth/colour"},
         "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches) * args.steps * world,
-        "ms_per_step_per_rank": per_rank_ms, "scene_graph_update": fk,
+        "ms_per_step_per_rank": per_rank_ms, "scene_graph_update": fk, "collision_queries": collide,
         "roofline": roofline, "cpu_baseline": cpu,
     }
     print(json.dumps(out), flush=True)

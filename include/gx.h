@@ -171,6 +171,47 @@ int gx_update_transforms(GxScene *scene, int32_t N, int32_t K, int32_t link_slot
                          float *inst_xform, void *cuda_stream);
 
 /*
+ * GxColumnGrid, GxSphere, gx_set_collision_world, gx_collide_batch -- the batch collision queries of the kinematic
+ * simulator on the GPU ("This new candidate pose for the robot is tested for overlap (penetration) with
+ * the environment"; PAPER.md:111-119 and Appendix G): every sphere of the robot against the static
+ * scene's column grid of its radius and against the oriented boxes of the resting movable objects.  The paper gives
+ * the structures but no layout or arithmetic; N13 fixes both.  Its layer cache and its four offset regular
+ * grids are accelerations of the same answer for a CPU; here every sphere tests all boxes of its environment.
+ *
+ * gx_set_collision_world: HOST arrays, copied.  grids [n_static * n_radii], grid (scene s, radius class c) at
+ *   s * n_radii + c: columns in the XZ plane at `spacing` (0.03 m in the paper), column (ix, iz) at
+ *   col_off[iz * nx + ix] .. col_off[iz * nx + ix + 1] of `layers`, a layer = (lo, hi), the heights the CENTRE of a
+ *   sphere of that radius may take (both inclusive).  radii [n_radii]: the sphere-radius working set ({0.015, 0.05,
+ *   0.12} in the paper).  spheres [n_spheres]: link index (>= 0), radius class, centre in the link's frame.
+ *   Errors: INVALID_ARG, UNSUPPORTED (more than 2^32 columns or layers), OOM, CUDA.
+ * gx_collide_batch: DEVICE arrays.  Sphere centres are W_link * centre with W_link = inst_xform[n][link_slot0 + link]
+ *   (what gx_update_transforms wrote).  The box of instance slot k is the object-space bounding box of its mesh
+ *   under inst_xform[n][k], which must be rigid.
+ *   out_static [N, n_spheres] uint8: 1 if the sphere is in obstructed space of its column grid or outside the grid.
+ *   out_object [N, n_spheres] int32: the lowest slot in [obj_slot0, obj_slot0 + n_obj) whose box the sphere overlaps
+ *   (distance from the centre to the box <= radius), skipping empty slots and held_slot[n] (NULL = nothing held); -1
+ *   if none.  Enqueues one kernel on cuda_stream.  Errors: INVALID_ARG (no collision world, NULL arrays, slots outside
+ *   [0, K)), CUDA.
+ */
+typedef struct {
+    float x0, z0;
+    float spacing;
+    int32_t nx, nz;
+    const uint32_t *col_off;
+    const float *layers;
+} GxColumnGrid;
+typedef struct {
+    int32_t link;
+    int32_t radius_class;
+    float centre[3];
+} GxSphere;
+int gx_set_collision_world(GxScene *scene, const GxColumnGrid *grids, int32_t n_radii, const float *radii,
+                           const GxSphere *spheres, int32_t n_spheres);
+int gx_collide_batch(GxScene *scene, int32_t N, int32_t K, const int32_t *env_scene, const int32_t *inst_mesh,
+                     const float *inst_xform, int32_t link_slot0, int32_t obj_slot0, int32_t n_obj,
+                     const int32_t *held_slot, uint8_t *out_static, int32_t *out_object, void *cuda_stream);
+
+/*
  * gx_set_option -- tuning / verification switches of a handle.  Unknown names and out-of-range values return
  * INVALID_ARG.  Every switch leaves the images bit-identical (tested); they only move time around.
  *   "cull"         0|1 (1)   per-environment frustum culling of clusters (K1).

@@ -19,7 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libgx.so")
 GX_OK, GX_ERR_INVALID_ARG, GX_ERR_CUDA, GX_ERR_OOM, GX_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 GX_BACKGROUND_ID = 0xFFFFFFFF
 EXPORTS = ("gx_create_scene", "gx_render_batch", "gx_render_batch_host", "gx_set_option", "gx_get_stat",
-           "gx_render_batch_obs", "gx_set_robot", "gx_update_transforms", "gx_reserve", "gx_destroy", "gx_last_error")
+           "gx_render_batch_obs", "gx_set_robot", "gx_update_transforms", "gx_reserve", "gx_set_collision_world",
+           "gx_collide_batch", "gx_destroy", "gx_last_error")
 
 
 class GxMesh(C.Structure):
@@ -34,6 +35,15 @@ class GxCamera(C.Structure):
 
 class GxLink(C.Structure):
     _fields_ = [("parent", C.c_int32), ("joint_type", C.c_int32), ("axis", C.c_float * 3), ("origin", C.c_float * 12)]
+
+
+class GxColumnGrid(C.Structure):
+    _fields_ = [("x0", C.c_float), ("z0", C.c_float), ("spacing", C.c_float), ("nx", C.c_int32), ("nz", C.c_int32),
+                ("col_off", C.c_void_p), ("layers", C.c_void_p)]
+
+
+class GxSphere(C.Structure):
+    _fields_ = [("link", C.c_int32), ("radius_class", C.c_int32), ("centre", C.c_float * 3)]
 
 
 class GxError(RuntimeError):
@@ -55,7 +65,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.gx_last_error.restype = C.c_char_p
         L.gx_destroy.restype = None
-        for n in EXPORTS[:9]:
+        for n in EXPORTS[:11]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -160,6 +170,39 @@ def gx_update_transforms(scene, N: int, K: int, link_slot0: int, base_pose, join
     _check(lib().gx_update_transforms(scene, C.c_int32(N), C.c_int32(K), C.c_int32(link_slot0), _dev(base_pose), _dev(joint_pos),
                                       _dev(held_slot), _dev(held_xform), _dev(cam_pose), _dev(inst_xform),
                                       C.c_void_p(cuda_stream)))
+
+
+def gx_set_collision_world(scene, grids, radii, spheres) -> None:
+    """grids: [n_static][n_radii] objects with x0, z0, spacing, nx, nz, col_off, layers (gen.ColumnGrid); spheres:
+    objects with link, radius_class, centre (gen.Sphere); host data, copied."""
+    n_radii = len(radii)
+    keep = []
+    arr = (GxColumnGrid * (len(grids) * n_radii))()
+    for i, row in enumerate(grids):
+        if len(row) != n_radii:
+            raise ValueError("one column grid per (scene, radius)")
+        for j, g in enumerate(row):
+            off = np.ascontiguousarray(g.col_off, np.uint32)
+            lay = np.ascontiguousarray(g.layers, np.float32).reshape(-1, 2)
+            keep += [off, lay]
+            arr[i * n_radii + j] = GxColumnGrid(float(g.x0), float(g.z0), float(g.spacing), int(g.nx), int(g.nz),
+                                                off.ctypes.data, lay.ctypes.data if lay.size else None)
+    sph = (GxSphere * len(spheres))()
+    for i, s in enumerate(spheres):
+        sph[i].link = int(s.link)
+        sph[i].radius_class = int(s.radius_class)
+        for k in range(3):
+            sph[i].centre[k] = float(np.float32(s.centre[k]))
+    rad = np.ascontiguousarray(radii, np.float32)
+    _check(lib().gx_set_collision_world(scene, arr, C.c_int32(n_radii), C.c_void_p(rad.ctypes.data), sph, C.c_int32(len(spheres))))
+
+
+def gx_collide_batch(scene, N: int, K: int, env_scene, inst_mesh, inst_xform, link_slot0: int, obj_slot0: int, n_obj: int,
+                     held_slot, out_static, out_object, cuda_stream: int = 0) -> None:
+    """All arrays are device tensors / addresses; enqueues on cuda_stream and returns."""
+    _check(lib().gx_collide_batch(scene, C.c_int32(N), C.c_int32(K), _dev(env_scene), _dev(inst_mesh), _dev(inst_xform),
+                                  C.c_int32(link_slot0), C.c_int32(obj_slot0), C.c_int32(n_obj), _dev(held_slot), _dev(out_static),
+                                  _dev(out_object), C.c_void_p(cuda_stream)))
 
 
 def gx_reserve(scene, camera: GxCamera, N: int, K: int) -> None:

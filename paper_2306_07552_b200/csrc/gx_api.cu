@@ -12,6 +12,7 @@
 #include "../../include/gx.h"
 #include "gx_pipeline.cuh"
 #include "gx_fk.cuh"
+#include "gx_collide.cuh"
 
 namespace {
 
@@ -120,6 +121,14 @@ struct GxScene {
     gx::FkLink *fk_links = nullptr;
     int fk_L = 0, fk_camera_link = -1, fk_ee_link = -1;
     float fk_mount[12] = {1, 0, 0, 0, 0, 1, 0, 0, 0, 0, 1, 0};
+    // collision world (gx_set_collision_world)
+    float4 *mesh_box = nullptr;          // [n_dyn][2] object-space box of every dynamic mesh (centre, half extent)
+    gx::ColGridDev *cg_grids = nullptr;
+    uint32_t *cg_col_off = nullptr;
+    float2 *cg_layers = nullptr;
+    float *cg_radii = nullptr;
+    gx::SphereDev *cg_spheres = nullptr;
+    int cg_n_radii = 0, cg_S = 0, cg_max_link = -1;
     // staging for gx_render_batch_host
     DevBuf<int32_t> h_env_scene, h_inst_mesh;
     DevBuf<float> h_cam_pose, h_inst_xform, h_depth;
@@ -319,6 +328,28 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
     if (rc == GX_OK) rc = upload(sc->subs, subs);
     if (rc == GX_OK) rc = upload(sc->clusters, clusters);
     if (rc == GX_OK) rc = upload(sc->meshes, meshes);
+    if (rc == GX_OK) {   // N13: object-space box of every dynamic mesh, in binary32 as the definition says
+        std::vector<float4> boxes((size_t)std::max(n_dyn, 1) * 2, make_float4(0.f, 0.f, 0.f, 0.f));
+        for (int i = 0; i < n_dyn; ++i) {
+            const GxMesh &m = dyn_meshes[i];
+            float lo[3] = {0.f, 0.f, 0.f}, hi[3] = {0.f, 0.f, 0.f};
+            for (uint32_t v = 0; v < m.nv; ++v)
+                for (int a = 0; a < 3; ++a) {
+                    const float pv = m.positions[3 * (size_t)v + a];
+                    if (v == 0 || pv < lo[a]) lo[a] = pv;
+                    if (v == 0 || pv > hi[a]) hi[a] = pv;
+                }
+            float c[3], h[3];
+            for (int a = 0; a < 3; ++a) {
+                volatile float sum = lo[a] + hi[a], dif = hi[a] - lo[a];   // (binary32 results, whatever the host compiler keeps in registers)
+                c[a] = 0.5f * sum;
+                h[a] = 0.5f * dif;
+            }
+            boxes[2 * (size_t)i] = make_float4(c[0], c[1], c[2], 0.f);
+            boxes[2 * (size_t)i + 1] = make_float4(h[0], h[1], h[2], 0.f);
+        }
+        rc = upload(sc->mesh_box, boxes);
+    }
     if (rc == GX_OK) {
         auto alloc = [&]() -> int {
             GX_CUDA(cudaMalloc(&sc->stats, GX_NSTAT * sizeof(unsigned long long)));
@@ -351,6 +382,8 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->meshes);
     cudaFree(sc->stats);
     cudaFree(sc->fk_links);
+    cudaFree(sc->mesh_box); cudaFree(sc->cg_grids); cudaFree(sc->cg_col_off); cudaFree(sc->cg_layers); cudaFree(sc->cg_radii);
+    cudaFree(sc->cg_spheres);
     sc->arena_recs.release(); sc->arena_bbs.release(); sc->arena_refs.release(); sc->scratch.release();
     for (cudaEvent_t e : sc->t_ev) cudaEventDestroy(e);
     if (sc->h_ctl) cudaFreeHost(sc->h_ctl);
@@ -763,6 +796,76 @@ int gx_update_transforms(GxScene *sc, int32_t N, int32_t K, int32_t link_slot0, 
     P.cam_pose = cam_pose; P.inst_xform = inst_xform;
     constexpr int FW = 4;
     gx::fk_kernel<FW><<<(N + FW - 1) / FW, FW * 32, 0, (cudaStream_t)cuda_stream>>>(P);
+    GX_CUDA(cudaGetLastError());
+    return GX_OK;
+}
+
+int gx_set_collision_world(GxScene *sc, const GxColumnGrid *grids, int32_t n_radii, const float *radii, const GxSphere *spheres,
+                           int32_t n_spheres) {
+    if (!sc || !grids || !radii || !spheres) return fail(GX_ERR_INVALID_ARG, "NULL argument");
+    if (n_radii <= 0 || n_radii > 16 || n_spheres <= 0 || n_spheres > 4096) return fail(GX_ERR_INVALID_ARG, "bad n_radii or n_spheres");
+    const size_t ng = (size_t)sc->n_static * (size_t)n_radii;
+    std::vector<gx::ColGridDev> hg(ng);
+    std::vector<uint32_t> hoff;
+    std::vector<float2> hlay;
+    for (size_t i = 0; i < ng; ++i) {
+        const GxColumnGrid &g = grids[i];
+        if (g.nx <= 0 || g.nz <= 0 || !(g.spacing > 0.0f) || !g.col_off || (unsigned long long)g.nx * g.nz >= (1ull << 30))
+            return fail(GX_ERR_INVALID_ARG, "column grid %zu: bad size, spacing or NULL col_off", i);
+        const size_t nc = (size_t)g.nx * g.nz;
+        const uint32_t nl = g.col_off[nc];
+        if (nl && !g.layers) return fail(GX_ERR_INVALID_ARG, "column grid %zu: NULL layers", i);
+        for (size_t c = 0; c < nc; ++c)
+            if (g.col_off[c] > g.col_off[c + 1]) return fail(GX_ERR_INVALID_ARG, "column grid %zu: col_off not ascending", i);
+        if (hoff.size() + nc + 1 >= 0xFFFFFFFFull || hlay.size() + nl >= 0xFFFFFFFFull) return fail(GX_ERR_UNSUPPORTED, "column grids too large");
+        hg[i] = {g.x0, g.z0, g.spacing, g.nx, g.nz, (uint32_t)hoff.size(), (uint32_t)hlay.size(), 0u};
+        hoff.insert(hoff.end(), g.col_off, g.col_off + nc + 1);
+        for (uint32_t l = 0; l < nl; ++l) hlay.push_back(make_float2(g.layers[2 * (size_t)l], g.layers[2 * (size_t)l + 1]));
+    }
+    std::vector<gx::SphereDev> hs((size_t)n_spheres);
+    int max_link = -1;
+    for (int i = 0; i < n_spheres; ++i) {
+        if (spheres[i].link < 0 || spheres[i].radius_class < 0 || spheres[i].radius_class >= n_radii)
+            return fail(GX_ERR_INVALID_ARG, "sphere %d: bad link or radius class", i);
+        hs[i] = {spheres[i].link, spheres[i].radius_class, spheres[i].centre[0], spheres[i].centre[1], spheres[i].centre[2]};
+        max_link = std::max(max_link, spheres[i].link);
+    }
+    DeviceGuard guard(sc->device);
+    if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
+    cudaFree(sc->cg_grids); cudaFree(sc->cg_col_off); cudaFree(sc->cg_layers); cudaFree(sc->cg_radii); cudaFree(sc->cg_spheres);
+    sc->cg_grids = nullptr; sc->cg_col_off = nullptr; sc->cg_layers = nullptr; sc->cg_radii = nullptr; sc->cg_spheres = nullptr;
+    sc->cg_S = 0;
+    int rc;
+    std::vector<float> hr(radii, radii + n_radii);
+    if ((rc = upload(sc->cg_grids, hg)) != GX_OK || (rc = upload(sc->cg_col_off, hoff)) != GX_OK || (rc = upload(sc->cg_layers, hlay)) != GX_OK ||
+        (rc = upload(sc->cg_radii, hr)) != GX_OK || (rc = upload(sc->cg_spheres, hs)) != GX_OK)
+        return rc;
+    sc->cg_n_radii = n_radii;
+    sc->cg_S = n_spheres;
+    sc->cg_max_link = max_link;
+    return GX_OK;
+}
+
+int gx_collide_batch(GxScene *sc, int32_t N, int32_t K, const int32_t *env_scene, const int32_t *inst_mesh, const float *inst_xform,
+                     int32_t link_slot0, int32_t obj_slot0, int32_t n_obj, const int32_t *held_slot, uint8_t *out_static,
+                     int32_t *out_object, void *cuda_stream) {
+    if (!sc) return fail(GX_ERR_INVALID_ARG, "NULL scene");
+    if (!sc->cg_S) return fail(GX_ERR_INVALID_ARG, "no collision world: call gx_set_collision_world first");
+    if (N <= 0 || K <= 0 || K > GX_MAX_INSTANCES) return fail(GX_ERR_INVALID_ARG, "bad N or K");
+    if (!env_scene || !inst_xform || !out_static || !out_object || (n_obj > 0 && !inst_mesh)) return fail(GX_ERR_INVALID_ARG, "NULL array argument");
+    if (link_slot0 < 0 || link_slot0 + sc->cg_max_link >= K) return fail(GX_ERR_INVALID_ARG, "link slots do not fit K = %d", K);
+    if (obj_slot0 < 0 || n_obj < 0 || obj_slot0 + n_obj > K) return fail(GX_ERR_INVALID_ARG, "object slots [%d, %d) do not fit K = %d", obj_slot0, obj_slot0 + n_obj, K);
+    DeviceGuard guard(sc->device);
+    if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
+    gx::CollideParams P;
+    P.grids = sc->cg_grids; P.col_off = sc->cg_col_off; P.layers = sc->cg_layers; P.radii = sc->cg_radii; P.spheres = sc->cg_spheres;
+    P.mesh_box = sc->mesh_box;
+    P.n_static = sc->n_static; P.n_radii = sc->cg_n_radii; P.n_dyn = sc->n_dyn; P.S = sc->cg_S;
+    P.N = N; P.K = K; P.link_slot0 = link_slot0; P.obj_slot0 = obj_slot0; P.n_obj = n_obj;
+    P.env_scene = env_scene; P.inst_mesh = inst_mesh; P.inst_xform = inst_xform; P.held_slot = held_slot;
+    P.out_static = out_static; P.out_object = out_object;
+    constexpr int CW = 4;
+    gx::collide_kernel<CW><<<(N + CW - 1) / CW, CW * 32, 0, (cudaStream_t)cuda_stream>>>(P);
     GX_CUDA(cudaGetLastError());
     return GX_OK;
 }
