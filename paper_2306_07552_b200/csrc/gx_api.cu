@@ -408,7 +408,7 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
         return GX_OK;
     }
     if (!strcmp(name, "bin_threads")) {   // (development)
-        if (value != 0 && value != 256 && value != 512 && value != 1024) return fail(GX_ERR_INVALID_ARG, "bin_threads must be 0, 256, 512 or 1024");
+        if (value != 0 && value != 256 && value != 512) return fail(GX_ERR_INVALID_ARG, "bin_threads must be 0, 256 or 512");
         sc->opt_bin_threads = (int)value;
         return GX_OK;
     }

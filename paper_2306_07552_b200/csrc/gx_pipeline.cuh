@@ -969,7 +969,7 @@ __device__ __forceinline__ void bin_stage(const PipeParams &PP, uint32_t *s_cnt,
 }
 
 template <bool STATS>
-__global__ void __launch_bounds__(256) bin_kernel(const PipeParams PP, int phase) {
+__global__ void __launch_bounds__(512) bin_kernel(const PipeParams PP, int phase) {
     extern __shared__ __align__(16) unsigned char smem[];
     uint32_t *s_cnt = reinterpret_cast<uint32_t *>(smem);
     bin_stage<false, STATS>(PP, s_cnt, s_cnt + PP.T * NBUCKET, phase);
