@@ -227,6 +227,9 @@ int gx_collide_batch(GxScene *scene, int32_t N, int32_t K, const int32_t *env_sc
  *                            device's memory, at most 16 GB.
  *   "arena_slots"  force the arena size in record slots (tests: several waves); 0 = automatic.
  *   "host_sub"     environments per sub-batch of gx_render_batch_host; 0 = a third of the batch.
+ *   "ctas_per_sm"  0..8 (0 = as many as fit) CTAs per SM of the persistent geometry and raster kernels, for callers
+ *                            that run other kernels beside the renderer.
+ *   "bin_threads"  0|256|512 (0 = 512) threads per CTA of the bin kernel.
  *   "stats"        0|1 (0)   count what gx_get_stat reports (slower kernels).
  *   "timing"       0|1 (0)   1 starts (and resets), 0 stops recording CUDA events around every kernel of
  *                            subsequent gx_render_batch calls on their stream.

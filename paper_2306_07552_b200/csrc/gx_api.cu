@@ -87,6 +87,8 @@ struct GxScene {
     // options (gx_set_option)
     int opt_cull = 1, opt_subcull = 1, opt_stats = 0, opt_hiz = 1, opt_big_px = 24;
     int opt_bin_threads = 0;
+    int opt_max_rounds = 0;             // rounds of stage kernels the host launches at most (0 = no limit; 1 = later waves all in the tail kernel)
+    int opt_ctas_per_sm = 0;            // persistent kernels: CTAs per SM (0 = as many as fit); smaller when two handles share the GPU
     int opt_host_sub = 0;               // gx_render_batch_host: environments per sub-batch; 0 = automatic
     int opt_occlusion = -1;             // occluder scheme: 1 on, 0 off, -1 automatic (on for frames of at least 8192 pixels)
     int opt_occl_area = 64;             // pixels per triangle of a sub-cluster's screen box that make it an occluder
@@ -407,6 +409,16 @@ int gx_set_option(GxScene *sc, const char *name, int64_t value) {
         if (value) { sc->t_used = 0; sc->t_calls = 0; sc->t_full = false; }
         return GX_OK;
     }
+    if (!strcmp(name, "ctas_per_sm")) {
+        if (value < 0 || value > 8) return fail(GX_ERR_INVALID_ARG, "ctas_per_sm must be in [0, 8]");
+        sc->opt_ctas_per_sm = (int)value;
+        return GX_OK;
+    }
+    if (!strcmp(name, "max_rounds")) {   // (development / tests)
+        if (value < 0) return fail(GX_ERR_INVALID_ARG, "max_rounds must be >= 0");
+        sc->opt_max_rounds = (int)value;
+        return GX_OK;
+    }
     if (!strcmp(name, "bin_threads")) {   // (development)
         if (value != 0 && value != 256 && value != 512) return fail(GX_ERR_INVALID_ARG, "bin_threads must be 0, 256 or 512");
         sc->opt_bin_threads = (int)value;
@@ -645,7 +657,8 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     int launches = 1;
     // one round of the stage kernels per wave the previous call on this handle needed (its batch is the best guess
     // for this one), plus one when there were several; whatever is still left goes to the cooperative tail kernel
-    const int rounds = sc->hist_waves > 1 ? sc->hist_waves + 1 : 1;
+    int rounds = sc->hist_waves > 1 ? sc->hist_waves + 1 : 1;
+    if (sc->opt_max_rounds > 0) rounds = std::min(rounds, sc->opt_max_rounds);
     for (int round = 0; round < rounds; ++round) {
     if (round > 0) {
         gx::wave_kernel<<<1, 256, 0, stream>>>(PP);
@@ -666,6 +679,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
             const size_t gsmem = (size_t)GW * gx::GEOM_WARP_SMEM;
             int per_sm = 0;
             if ((rc = plan_of(sc, (const void *)gk, GW * 32, gsmem, &per_sm)) != GX_OK) return rc;
+            if (sc->opt_ctas_per_sm) per_sm = std::min(per_sm, sc->opt_ctas_per_sm);
             gk<<<sc->num_sms * per_sm, GW * 32, gsmem, stream>>>(PP, phase);
             GX_CUDA(cudaGetLastError());
             if ((rc = mark(sc, stream, 2)) != GX_OK) return rc;
@@ -691,6 +705,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
             const size_t rsmem = (size_t)RW * gx::RAST_WARP_SMEM;
             int per_sm = 0;
             if ((rc = plan_of(sc, (const void *)rk, RW * 32, rsmem, &per_sm)) != GX_OK) return rc;
+            if (sc->opt_ctas_per_sm) per_sm = std::min(per_sm, sc->opt_ctas_per_sm);
             rk<<<sc->num_sms * per_sm, RW * 32, rsmem, stream>>>(PP);
             GX_CUDA(cudaGetLastError());
             if ((rc = mark(sc, stream, 4)) != GX_OK) return rc;

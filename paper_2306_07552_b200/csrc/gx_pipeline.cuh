@@ -1765,7 +1765,7 @@ __host__ __device__ inline size_t tail_smem_bytes(int T) {
 }
 
 template <bool STATS>
-__global__ void __launch_bounds__(TAIL_WARPS * 32, 2) tail_kernel(const PipeParams PP) {
+__global__ void __launch_bounds__(TAIL_WARPS * 32, 3) tail_kernel(const PipeParams PP) {
     extern __shared__ __align__(16) unsigned char smem[];
     cg::grid_group grid = cg::this_grid();
     const int warp = threadIdx.x >> 5;

@@ -155,6 +155,9 @@ def test_waves_and_option_variants(oracle_mod):
         "every sub-cluster an occluder": dict(occl_area=0),
         "no sub-cluster an occluder (but those at the near plane)": dict(occl_area=1 << 20),
         "occluders from 8 px per triangle, 3 environments per wave": dict(occl_area=8, arena_slots=3 * per_env),
+        "two CTAs per SM, bin CTAs of 256 threads": dict(ctas_per_sm=2, bin_threads=256),
+        "large path from 16 px": dict(big_px=16),
+        "large path from 32 px": dict(big_px=32),
     }
     for name, opts in variants.items():
         g = render_gpu(wl, stats=True, options=opts)
