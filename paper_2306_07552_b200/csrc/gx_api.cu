@@ -572,6 +572,7 @@ static int setup_buffers(GxScene *sc, gx::PipeParams &PP, unsigned long long wor
     off = (off + 3) & ~(size_t)3;
     const size_t o_items = off; off += 4 * n * (size_t)PP.item_stride;
     const size_t o_witems = off; off += 4 * n * (size_t)PP.item_stride;
+    const size_t o_witems2 = off; off += PP.occl ? 4 * n * (size_t)PP.item_stride : 0;
     const size_t o_keys = off; off += PP.occl ? n * (size_t)P.W * (size_t)P.H * 2 : 0;
     if ((rc = sc->scratch.reserve(off)) != GX_OK) return rc;
     uint32_t *sp = sc->scratch.p;
@@ -581,6 +582,7 @@ static int setup_buffers(GxScene *sc, gx::PipeParams &PP, unsigned long long wor
     PP.tile_off = sp + o_toff; PP.tasks = sp + o_tasks; PP.hizt = sp + o_hizt; PP.hizb = sp + o_hizb;
     PP.items = reinterpret_cast<uint4 *>(sp + o_items);
     PP.wave_items = reinterpret_cast<uint4 *>(sp + o_witems);
+    PP.wave_items2 = reinterpret_cast<uint4 *>(sp + o_witems2);
     PP.keys = reinterpret_cast<unsigned long long *>(sp + o_keys);
 
     return GX_OK;
@@ -670,6 +672,13 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     if ((rc = mark(sc, stream, round > 0 ? 5 : 1)) != GX_OK) return rc;
     ++launches;
     for (int phase = PP.occl ? 1 : 0; phase <= (PP.occl ? 2 : 0); ++phase) {
+        if (phase == 2) {   // the runs of the second phase against the hi-Z pyramid of the first, densely
+            auto ck = st ? gx::cull2_kernel<true> : gx::cull2_kernel<false>;
+            ck<<<sc->num_sms * 4, 256, 0, stream>>>(PP);
+            GX_CUDA(cudaGetLastError());
+            if ((rc = mark(sc, stream, 1)) != GX_OK) return rc;
+            ++launches;
+        }
         // K2: persistent independent warps
         {
             constexpr int GW = 8;

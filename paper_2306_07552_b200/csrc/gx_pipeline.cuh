@@ -60,7 +60,8 @@ enum { F_BIAS = 7, F_FLOATCOL = 8, F_WIDE = 16 };
 // control words (device): cursors and the current wave
 // (cursors and task counts exist once per phase of the occluder scheme: index 0 = single pass or occluder phase, 1 = second phase)
 enum { C_WAVE_E0 = 0, C_WAVE_E1, C_GEOM_CUR, C_BIN_CUR = C_GEOM_CUR + 2, C_RAST_CUR = C_BIN_CUR + 2, C_CULL_DONE = C_RAST_CUR + 2,
-       C_WAVE_ITEMS, C_SUM_U /* 64-bit: two words, even index */, C_WAVES = C_SUM_U + 2, C_MAX_U, C_BAD_ENVS, C_TASK_CNT = 16,
+       C_WAVE_ITEMS, C_SUM_U /* 64-bit: two words, even index */, C_WAVES = C_SUM_U + 2, C_MAX_U, C_BAD_ENVS, C_WAVE_ITEMS2,
+       C_TASK_CNT = 16,
        C_NCTL = C_TASK_CNT + 2 * NCLASS };
 static_assert(C_SUM_U % 2 == 0 && C_BAD_ENVS < C_TASK_CNT, "control word layout");
 
@@ -75,6 +76,8 @@ struct PipeParams {
     uint32_t *item_pre;      // [N+1] exclusive prefix of n_items over the environments of the wave
     uint4 *wave_items;       // [ctl[C_WAVE_ITEMS]] the items of the wave's environments in one list, the environment in
                              //   the third word (pack_stage), which is what the geometry stage hands out
+    uint4 *wave_items2;      // [ctl[C_WAVE_ITEMS2]] second phase of the occluder scheme: the items that still have a run
+                             //   after the hi-Z test of every run's box (cull2_stage); second word = those runs
     uint32_t *U;             // [N] upper bound of the record slots of the environment
     int32_t item_stride;
     // wave allocation
@@ -249,6 +252,7 @@ __device__ void alloc_wave(const PipeParams &PP, uint32_t e_first) {
         const uint32_t end = s_end, n_ch = end < N ? s_fin_i : s_run_i;
         PP.item_pre[end] = n_ch;
         PP.ctl[C_WAVE_ITEMS] = n_ch;
+        PP.ctl[C_WAVE_ITEMS2] = 0;
         PP.ctl[C_WAVE_E0] = e_first;
         PP.ctl[C_WAVE_E1] = end;
         for (int c = 0; c < 2; ++c) { PP.ctl[C_GEOM_CUR + c] = 0; PP.ctl[C_BIN_CUR + c] = 0; PP.ctl[C_RAST_CUR + c] = 0; }
@@ -695,8 +699,9 @@ __device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *
     pj.fx = P.fx; pj.fy = P.fy;
     pj.hw = 128.0f * (float)P.W; pj.hh = 128.0f * (float)P.H;
 
-    unsigned st_in = 0, st_tri = 0, st_hid = 0, st_subhid = 0;
-    const unsigned n_items = ldi<COOP>(&PP.ctl[C_WAVE_ITEMS]);
+    unsigned st_in = 0, st_tri = 0, st_hid = 0;
+    const unsigned n_items = ldi<COOP>(&PP.ctl[phase == 2 ? C_WAVE_ITEMS2 : C_WAVE_ITEMS]);
+    const uint4 *items = phase == 2 ? PP.wave_items2 : PP.wave_items;
     uint32_t *cursor = &PP.ctl[C_GEOM_CUR + (phase == 2 ? 1 : 0)];
     const size_t hzb_stride = (size_t)(P.W >> 3) * (size_t)(P.H >> 2);
     unsigned next = 0;
@@ -705,27 +710,20 @@ __device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *
     while (next < n_items) {
         const unsigned g = next;
         if (lane == 0) next = atomicAdd(cursor, 1u);   // draw the following item while this one is processed
-        const uint4 item = ldi<COOP>(&PP.wave_items[g]);
+        const uint4 item = ldi<COOP>(&items[g]);
         const uint32_t e = item.z, s = item.x >> 24, batch = item.x & 0xFFFFFFu;
         const uint32_t U = ldi<COOP>(&PP.U[e]), rbase = ldi<COOP>(&PP.rec_base[e]);
         {
-        unsigned mask = phase == 0 ? ((item.y | (item.y >> 8)) & 255u) : (phase == 1 ? (item.y & 255u) : ((item.y >> 8) & 255u));
+        unsigned mask = phase == 0 ? ((item.y | (item.y >> 8)) & 255u) : (item.y & 255u);   // (phase 2: the runs cull2_stage left)
         if (mask) {
             const float *MV = PP.env_mv + ((size_t)e * (size_t)(K + 1) + s) * 12;
-            // lanes 0..7: one run each -- its vertex range, and in the second phase the hi-Z test of its box
+            // lanes 0..7: one run each -- its vertex range
             uint32_t vlo = 0xFFFFu, vhi = 0u;
-            bool keep = false;
             if (lane < GX_SUBS_PER_BATCH && ((mask >> lane) & 1u)) {
                 const GxClusterDev sb = P.subs[(size_t)batch * GX_SUBS_PER_BATCH + lane];
-                keep = true;
-                if (HZ) {
-                    keep = !sub_hidden<COOP>(PP, sb, MV, e);
-                    if (STATS && !keep) ++st_subhid;
-                }
-                if (keep) { vlo = sb.batch_off; vhi = sb.nbatch; }   // (fields reused: first and last vertex the run references)
+                vlo = sb.batch_off; vhi = sb.nbatch;   // (fields reused: first and last vertex the run references)
             }
-            mask = __ballot_sync(FULL, keep);
-            if (mask) {
+            {
                 vlo = __reduce_min_sync(FULL, vlo);
                 vhi = __reduce_max_sync(FULL, vhi);
                 geom_batch<COOP, STATS>(PP, pj, batch, MV, ldi<COOP>(&PP.env_idb[(size_t)e * (size_t)(K + 1) + s]), ws, (int)e,
@@ -741,13 +739,11 @@ __device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *
         for (int d = 16; d; d >>= 1) {
             st_tri += __shfl_xor_sync(FULL, st_tri, d);
             st_hid += __shfl_xor_sync(FULL, st_hid, d);
-            st_subhid += __shfl_xor_sync(FULL, st_subhid, d);
         }
         if (lane == 0) {
             atomicAdd(&P.stats[GX_STAT_TRIS_IN], (unsigned long long)st_in);
             atomicAdd(&P.stats[GX_STAT_TRIS_RASTER], (unsigned long long)st_tri);
             atomicAdd(&P.stats[GX_STAT_TRIS_HIDDEN], (unsigned long long)st_hid);
-            atomicAdd(&P.stats[GX_STAT_SUBS_HIDDEN], (unsigned long long)st_subhid);
         }
     }
 }
@@ -1708,6 +1704,58 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
     }
 }
 
+// Second phase of the occluder scheme, before its geometry: one thread per (item of the wave, run of 32 triangles):
+// the box of every run that was not an occluder is tested against the hi-Z pyramid the first raster phase left
+// (sub_hidden); items that keep a run are appended, with those runs as their mask, to the second item list.  Dense
+// (all lanes busy, 8 per item), so that the geometry stage never sees what is hidden.
+template <bool COOP, bool STATS>
+__device__ __forceinline__ void cull2_stage(const PipeParams &PP) {
+    __shared__ unsigned s_cnt, s_base;
+    const GxParams &P = PP.g;
+    const unsigned FULL = 0xFFFFFFFFu;
+    const int tid = threadIdx.x, lane = tid & 31, r = lane & 7, sub = lane >> 3;
+    const int K = P.K;
+    const unsigned n_items = ldi<COOP>(&PP.ctl[C_WAVE_ITEMS]);
+    const unsigned per_cta = blockDim.x >> 3;                           // items per CTA and round (8 threads each)
+    unsigned st_hid = 0;
+    for (unsigned g0 = blockIdx.x * per_cta; g0 < n_items; g0 += gridDim.x * per_cta) {   // (uniform per CTA)
+        const unsigned g = g0 + (tid >> 3);
+        uint4 item = make_uint4(0u, 0u, 0u, 0u);
+        bool keep = false;
+        if (g < n_items) {
+            item = ldi<COOP>(&PP.wave_items[g]);
+            if ((item.y >> (8 + r)) & 1u) {
+                const uint32_t batch = item.x & 0xFFFFFFu, s = item.x >> 24, e = item.z;
+                const GxClusterDev sb = P.subs[(size_t)batch * GX_SUBS_PER_BATCH + r];
+                keep = !PP.hiz || !sub_hidden<COOP>(PP, sb, PP.env_mv + ((size_t)e * (size_t)(K + 1) + s) * 12, e);
+                if (STATS && !keep) ++st_hid;
+            }
+        }
+        const unsigned m = __ballot_sync(FULL, keep);
+        const unsigned mine = (m >> (sub * 8)) & 255u;                 // the runs this lane's item keeps
+        const bool lead = r == 0 && mine != 0u;
+        const unsigned ml = __ballot_sync(FULL, lead);
+        // one reservation per CTA and round
+        if (tid == 0) s_cnt = 0;
+        __syncthreads();
+        unsigned wbase = 0;
+        if (lane == 0 && ml) wbase = atomicAdd(&s_cnt, (unsigned)__popc(ml));
+        wbase = __shfl_sync(FULL, wbase, 0);
+        __syncthreads();
+        if (tid == 0 && s_cnt) s_base = atomicAdd(&PP.ctl[C_WAVE_ITEMS2], s_cnt);
+        __syncthreads();
+        if (lead) PP.wave_items2[s_base + wbase + __popc(ml & ((1u << lane) - 1u))] = make_uint4(item.x, mine, item.z, 0u);
+    }
+    if (STATS) {
+#pragma unroll
+        for (int d = 16; d; d >>= 1) st_hid += __shfl_xor_sync(FULL, st_hid, d);
+        if (lane == 0 && st_hid) atomicAdd(&P.stats[GX_STAT_SUBS_HIDDEN], (unsigned long long)st_hid);
+    }
+}
+
+template <bool STATS>
+__global__ void __launch_bounds__(256) cull2_kernel(const PipeParams PP) { cull2_stage<false, STATS>(PP); }
+
 // The items of the wave's environments, copied into one list with the environment in the third word: the geometry
 // stage then needs no search to know whose item it drew.  One warp per environment at a time.
 template <bool COOP>
@@ -1737,6 +1785,7 @@ __global__ void __launch_bounds__(256) wave_kernel(const PipeParams PP) {
     } else if (threadIdx.x == 0) {
         PP.ctl[C_WAVE_E0] = e_next;
         PP.ctl[C_WAVE_ITEMS] = 0;
+        PP.ctl[C_WAVE_ITEMS2] = 0;
         for (int c = 0; c < 2; ++c) { PP.ctl[C_GEOM_CUR + c] = 0; PP.ctl[C_BIN_CUR + c] = 0; PP.ctl[C_RAST_CUR + c] = 0; }
         for (int c = 0; c < 2 * NCLASS; ++c) PP.ctl[C_TASK_CNT + c] = 0;
     }
@@ -1778,6 +1827,10 @@ __global__ void __launch_bounds__(TAIL_WARPS * 32, 3) tail_kernel(const PipePara
         pack_stage<true>(PP);
         grid.sync();
         for (int phase = PP.occl ? 1 : 0; phase <= (PP.occl ? 2 : 0); ++phase) {
+            if (phase == 2) {
+                cull2_stage<true, STATS>(PP);
+                grid.sync();
+            }
             if (phase == 2 && PP.hiz) geom_stage<true, STATS, true>(PP, smem + (size_t)warp * GEOM_WARP_SMEM, phase);
             else geom_stage<true, STATS, false>(PP, smem + (size_t)warp * GEOM_WARP_SMEM, phase);
             grid.sync();
