@@ -712,10 +712,10 @@ __device__ __forceinline__ void geom_stage(const PipeParams &PP, unsigned char *
         if (lane == 0) next = atomicAdd(cursor, 1u);   // draw the following item while this one is processed
         const uint4 item = ldi<COOP>(&items[g]);
         const uint32_t e = item.z, s = item.x >> 24, batch = item.x & 0xFFFFFFu;
-        const uint32_t U = ldi<COOP>(&PP.U[e]), rbase = ldi<COOP>(&PP.rec_base[e]);
         {
         unsigned mask = phase == 0 ? ((item.y | (item.y >> 8)) & 255u) : (item.y & 255u);   // (phase 2: the runs cull2_stage left)
         if (mask) {
+            const uint32_t U = ldi<COOP>(&PP.U[e]), rbase = ldi<COOP>(&PP.rec_base[e]);
             const float *MV = PP.env_mv + ((size_t)e * (size_t)(K + 1) + s) * 12;
             // lanes 0..7: one run each -- its vertex range
             uint32_t vlo = 0xFFFFu, vhi = 0u;
