@@ -1444,7 +1444,13 @@ __device__ __forceinline__ void raster_stage(const PipeParams &PP, unsigned char
     constexpr int phase = PHASE;
     const GxParams &P = PP.g;
     const unsigned FULL = 0xFFFFFFFFu;
-    constexpr int SW = 4;
+#ifndef GX_SW1
+#define GX_SW1 8
+#endif
+#ifndef GX_SW2
+#define GX_SW2 4
+#endif
+    constexpr int SW = PHASE == 2 ? GX_SW2 : GX_SW1;   // pixels per slot of the slot walk (the occluder phase has the bigger boxes)
     const int lane = threadIdx.x & 31;
     const unsigned lt = (1u << lane) - 1u;
     const int W = P.W, npix = P.W * P.H, T = PP.T, NK = T * NBUCKET;
