@@ -23,6 +23,7 @@ def _check(oracle_mod, wl, **kw):
     rep = compare(o, g, check_rgb=not wl.depth_only)
     assert rep["id_mismatch"] == 0, rep
     assert rep["depth_bits_differ"] == 0, rep
+    assert rep["rgb_differ"] == 0, rep       # N8 is implemented verbatim: not just within +-1 LSB, the same bytes
     return o, g, rep
 
 
