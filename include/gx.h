@@ -86,7 +86,10 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
  *   cuda_stream: a cudaStream_t (NULL = legacy default stream).
  * The call only enqueues work on the stream and returns; outputs are valid in stream order (the zero-copy
  * hand-off of PAPER.md:91).  Scratch inside the handle grows on demand; growing may synchronise the device,
- * steady state does not.  Same inputs give bit-identical outputs, independent of how N is sharded.
+ * steady state does not.  The call may be captured into a CUDA graph (cudaStreamBeginCapture on cuda_stream) once
+ * the handle holds its buffers for this shape (gx_reserve, or one plain call): inside a capture it allocates
+ * nothing and reads nothing back, and returns UNSUPPORTED if it would have to; replays read the input arrays and
+ * write the output arrays the captured call was given.  Same inputs give bit-identical outputs, independent of how N is sharded.
  * NaN/Inf inputs and out-of-range env_scene/inst_mesh values are precondition violations: the image is
  * undefined, but no out-of-bounds write occurs for in-range ids.
  * Errors: INVALID_ARG (null handle/camera/required pointer, N <= 0, K < 0, K > GX_MAX_INSTANCES, width or

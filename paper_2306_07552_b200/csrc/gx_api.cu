@@ -104,6 +104,7 @@ struct GxScene {
     uint32_t *h_ctl = nullptr;          // pinned host copy of the control words of the last call
     cudaEvent_t ev_ctl = nullptr;
     bool ctl_pending = false;
+    bool capturing = false;             // the current call's stream is being captured into a CUDA graph
     int ctl_N = 0;
     double hist_u_per_env = 0.0;
     int hist_waves = 1;                 // waves the last call needed (the host launches that many rounds of the stage kernels)
@@ -524,7 +525,7 @@ static int setup_buffers(GxScene *sc, gx::PipeParams &PP, unsigned long long wor
     // colours), so that a wave always has room for at least one environment.  Beyond that it is sized from the
     // history of earlier calls (mean U per environment, read back asynchronously) or, on the first call, from a
     // default of 48 Ki slots per environment, and capped by the budget; what does not fit goes to later waves.
-    if (sc->ctl_pending && cudaEventQuery(sc->ev_ctl) == cudaSuccess) {
+    if (!sc->capturing && sc->ctl_pending && cudaEventQuery(sc->ev_ctl) == cudaSuccess) {
         const uint64_t sum = (uint64_t)sc->h_ctl[gx::C_SUM_U] | ((uint64_t)sc->h_ctl[gx::C_SUM_U + 1] << 32);
         sc->hist_u_per_env = std::max(sc->hist_u_per_env, (double)sum / (double)std::max(sc->ctl_N, 1));
         sc->hist_waves = (int)std::min<uint32_t>(std::max<uint32_t>(sc->h_ctl[gx::C_WAVES], 1u), 256u);
@@ -541,6 +542,9 @@ static int setup_buffers(GxScene *sc, gx::PipeParams &PP, unsigned long long wor
         want = std::min<uint64_t>(want, (uint64_t)budget / 88);
     }
     want = std::min<uint64_t>(std::max<uint64_t>(want, worst_env), 0xFFFFFF00ull);
+    if (want > sc->arena_slots && sc->capturing) want = sc->arena_slots;   // (no allocation inside a capture: more waves instead)
+    if (sc->capturing && sc->arena_slots < worst_env)
+        return fail(GX_ERR_UNSUPPORTED, "the arena cannot hold one environment of this shape: call gx_reserve (or render once) before capturing the call into a CUDA graph");
     if (want > sc->arena_slots) {
         if ((rc = sc->arena_recs.reserve((size_t)want * 4)) != GX_OK) return rc;
         if ((rc = sc->arena_bbs.reserve((size_t)want)) != GX_OK) return rc;
@@ -574,6 +578,8 @@ static int setup_buffers(GxScene *sc, gx::PipeParams &PP, unsigned long long wor
     const size_t o_witems = off; off += 4 * n * (size_t)PP.item_stride;
     const size_t o_witems2 = off; off += PP.occl ? 4 * n * (size_t)PP.item_stride : 0;
     const size_t o_keys = off; off += PP.occl ? n * (size_t)P.W * (size_t)P.H * 2 : 0;
+    if (off > sc->scratch.n && sc->capturing)
+        return fail(GX_ERR_UNSUPPORTED, "the handle's tables would have to grow during stream capture: call gx_reserve for this shape first");
     if ((rc = sc->scratch.reserve(off)) != GX_OK) return rc;
     uint32_t *sp = sc->scratch.p;
     PP.ctl = sp; PP.U = sp + o_U; PP.n_items = sp + o_nitems; PP.item_pre = sp + o_cpre; PP.rec_base = sp + o_base;
@@ -636,6 +642,14 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
     PP.occl_area = (float)sc->opt_occl_area;
 
     int rc;
+    {   // inside a stream capture (CUDA graph) nothing may be allocated and nothing is read back: the buffers must be
+        // there already (gx_reserve, or one ordinary call of the same shape), and the graph replays the rounds of
+        // stage kernels the handle's history asks for at capture time (the tail kernel still renders any wave beyond)
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        GX_CUDA(cudaStreamIsCapturing(stream, &cs));
+        sc->capturing = cs == cudaStreamCaptureStatusActive;
+        if (sc->capturing && sc->opt_timing) return fail(GX_ERR_UNSUPPORTED, "option \"timing\" cannot be used during stream capture");
+    }
     if ((rc = setup_buffers(sc, PP, worst_tris)) != GX_OK) return rc;
     sc->last_stream = stream;
     if (st) GX_CUDA(cudaMemsetAsync(sc->stats, 0, GX_NSTAT * sizeof(unsigned long long), stream));
@@ -732,7 +746,7 @@ static int render_impl(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, c
         GX_CUDA(cudaLaunchCooperativeKernel((const void *)tk, dim3((unsigned)(sc->num_sms * per_sm)), dim3(gx::TAIL_WARPS * 32), args, tsmem, stream));
         if ((rc = mark(sc, stream, 5)) != GX_OK) return rc;
     }
-    if (!sc->ctl_pending) {   // (a read-back still in flight keeps its buffer)
+    if (!sc->ctl_pending && !sc->capturing) {   // (a read-back still in flight keeps its buffer)
         GX_CUDA(cudaMemcpyAsync(sc->h_ctl, PP.ctl, gx::C_NCTL * sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
         GX_CUDA(cudaEventRecord(sc->ev_ctl, stream));
         sc->ctl_pending = true;
@@ -750,6 +764,7 @@ int gx_reserve(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K) {
         return fail(GX_ERR_INVALID_ARG, "width and height must be positive multiples of 16 up to %d", GX_MAX_FRAME);
     DeviceGuard guard(sc->device);
     if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
+    sc->capturing = false;
     gx::PipeParams PP;
     memset(&PP, 0, sizeof(PP));
     PP.g.N = N; PP.g.K = K; PP.g.W = cam->width; PP.g.H = cam->height;

@@ -345,6 +345,52 @@ def test_reserve_then_no_growth(oracle_mod):
         gx.gx_destroy(sc)
 
 
+def test_cuda_graph_capture_and_replay(oracle_mod):
+    """gx_render_batch can be captured into a CUDA graph once the handle holds its buffers (gx_reserve or one plain
+    call): inside the capture it allocates nothing and reads nothing back; replays give the oracle's images, also
+    with new poses written into the same input tensors and with an arena so small that the captured call needs
+    several waves (host rounds and the cooperative tail kernel inside the graph)."""
+    import torch
+    from paper_2306_07552_b200 import binding as gx
+    wl = gen.make_config(1, n_envs=16)
+    wl2 = gen.make_config(1, env_ids=np.arange(16, 32))
+    o1, o2 = oracle_mod.render(wl), oracle_mod.render(wl2)
+    dev = torch.device("cuda:0")
+    for opts in ({}, {"arena_slots": 1}):
+        sc = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, 0)
+        try:
+            for k, v in opts.items():
+                gx.gx_set_option(sc, k, v)
+            cam = gx.camera_of(wl)
+            N, K, H, W = wl.N, wl.K, wl.height, wl.width
+            t = lambda a, ty: torch.from_numpy(np.ascontiguousarray(a, ty)).to(dev)
+            d = [t(wl.env_scene, np.int32), t(wl.cam_pose, np.float32), t(wl.inst_mesh, np.int32), t(wl.inst_xform, np.float32)]
+            rgb = torch.zeros((N, H, W, 3), dtype=torch.uint8, device=dev)
+            depth = torch.zeros((N, H, W), dtype=torch.float32, device=dev)
+            ids = torch.zeros((N, H, W), dtype=torch.int32, device=dev)
+            g, s = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+            if not opts:     # without buffers the capture is refused, and the refusal leaves the capture usable
+                with pytest.raises(gx.GxError):
+                    with torch.cuda.graph(torch.cuda.CUDAGraph(), stream=s):
+                        gx.gx_render_batch(sc, cam, N, K, d[0], d[1], d[2], d[3], rgb, depth, ids, torch.cuda.current_stream().cuda_stream)
+            gx.gx_reserve(sc, cam, N, K)
+            with torch.cuda.graph(g, stream=s):
+                gx.gx_render_batch(sc, cam, N, K, d[0], d[1], d[2], d[3], rgb, depth, ids, torch.cuda.current_stream().cuda_stream)
+            for o, w in ((o1, wl), (o2, wl2), (o1, wl)):
+                d[0].copy_(t(w.env_scene, np.int32)); d[1].copy_(t(w.cam_pose, np.float32))
+                d[2].copy_(t(w.inst_mesh, np.int32)); d[3].copy_(t(w.inst_xform, np.float32))
+                depth.fill_(-1.0)
+                g.replay()
+                torch.cuda.synchronize()
+                got = dict(rgb=rgb.cpu().numpy(), depth=depth.cpu().numpy(), id=ids.cpu().numpy().view(np.uint32))
+                rep = compare(o, got)
+                assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0 and rep["rgb_differ"] == 0, (opts, rep)
+            if opts:
+                assert gx.gx_get_stat(sc, "waves") > 1
+        finally:
+            gx.gx_destroy(sc)
+
+
 def test_argument_errors():
     import torch
     from paper_2306_07552_b200 import binding as gx
