@@ -15,7 +15,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libgx.so")
 SOURCES = ["gx_api.cu"]
-DEPS = ["gx_api.cu", "gx_math.cuh", "gx_pipeline.cuh", "gx_types.h", os.path.join("..", "..", "include", "gx.h")]
+DEPS = ["gx_api.cu", "gx_math.cuh", "gx_pipeline.cuh", "gx_fk.cuh", "gx_collide.cuh", "gx_types.h",
+        os.path.join("..", "..", "include", "gx.h")]
 NVCC_FLAGS = ["-shared", "-Xcompiler", "-fPIC", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3",
               "-fmad=false", "-std=c++17", "-cudart", "static"]
 
