@@ -13,8 +13,10 @@ the max over ranks.
 
 Prints ONE JSON line (rank 0).  `value` = env-frames/s, device timed; `e2e` = the same metric through
 gx_render_batch_host with pinned HOST buffers (H2D of poses/transforms and D2H of RGBD inside the timed
-region); `roofline` = algorithmic bytes (accounting.py: culled geometry + RGBD out) / render-kernel time
-against the measured HBM copy peak; `cpu_baseline` = the CPU oracle on this box's host cores.
+region); `roofline` = algorithmic bytes (accounting.py: culled geometry + RGBD out) / step time against the
+measured HBM copy peak; `cpu_baseline` = the CPU oracle on this box's host cores; `scene_graph_update` = the
+forward-kinematics call (N12) alone and followed by the render; `--collide` adds the collision queries (N13).
+`--gpus N` without torchrun starts N ranks itself (one per GPU) and refuses if fewer devices are visible.
 
 --impl reference times the oracle itself (this tier's reference arm): each step renders a bounded sample
 of the same workload on the host cores.
@@ -409,9 +411,10 @@ def run_gx(args):
         return
 
     # ---- roofline: algorithmic bytes of the whole path / time of the path's kernels -----------------------
-    # The algorithmic bytes (accounting.py) belong to the whole hot path K1..K5, which is four kernels per step
-    # (cull, geometry, raster order, raster) plus the overflow pass; `achieved` divides by the sum of their
-    # event-timed durations.  The dominant kernel (raster) and every kernel's share are reported beside it.
+    # The algorithmic bytes (accounting.py) belong to the whole hot path K1..K5, which is ten launches per step (cull,
+    # pack, geometry / bin / raster of the occluder phase, cull2, geometry / bin / raster of the second phase, tail);
+    # `achieved` divides by the whole step time, the sum of the event-timed kernels is reported beside it, and so are
+    # the dominant kernel (raster) and every kernel class's share.
     peak, peak_src = measured_peak()
     b = accounting.env_bytes(wl)
     bytes_per_launch = float(b["total"].sum())
