@@ -425,13 +425,14 @@ def run_gx(args):
     achieved_kernels = bytes_per_launch / (kernel_ms * 1e-3) / 1e9
     # DRAM bytes per launch of all our kernels: not measured in this run (ncu replays kernels); taken from the
     # committed ncu capture of the same workload, whose header names the commit it was captured at
-    traffic, traffic_src = None, None
+    traffic, traffic_src, warp_inst = None, None, None
     try:
         import csv
         with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as f:
             rows = [r for r in csv.DictReader(f) if int(r["workload_config"]) == args.config]
         if rows and not args.opt and not args.envs and not args.obs:
             traffic = float(sum(int(r["dram_bytes_per_launch"]) for r in rows))
+            warp_inst = float(sum(int(r["warp_instructions"]) for r in rows))
             traffic_src = "profiles/r2_traffic.csv (ncu --set full capture; commit in profiles/r2_pipeline_ncu.md)"
     except Exception:
         pass
@@ -448,6 +449,14 @@ def run_gx(args):
                 "post_cull_tris_per_env": float(b["tris"].mean()),
                 "frac_of_nominal_8TBs": achieved / NOMINAL_HBM_GBS,
                 "note": "frac = algorithmic bytes / whole step time; issue- and latency-bound, not DRAM-bound: DESIGN.md section 7"}
+    if warp_inst:
+        # what actually binds the path: instruction issue.  Peak = SMs x 4 schedulers x SM clock
+        # (one warp instruction per scheduler and cycle); the count is the ncu figure of the committed capture.
+        sm_mhz = (clk.summary().get("sm_mhz") or 1965.0)
+        issue_peak = torch.cuda.get_device_properties(dev).multi_processor_count * 4 * sm_mhz * 1e6
+        roofline["issue"] = {"bound": "alu", "warp_instructions_per_call": warp_inst, "achieved": warp_inst / (step_ms * 1e-3),
+                             "peak": issue_peak, "unit": "warp-instructions/s", "frac": warp_inst / (step_ms * 1e-3) / issue_peak,
+                             "source": traffic_src}
     cpu = None if args.no_cpu_baseline else time_oracle(wl)
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
