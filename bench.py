@@ -56,6 +56,9 @@ def parse_args():
     ap.add_argument("--obs", action="store_true",
                     help="time gx_render_batch_obs (packed [N,4,H,W] float16 observation, DESIGN.md N11) instead of "
                          "gx_render_batch; device timing only")
+    ap.add_argument("--frame", type=int, nargs=2, default=None, metavar=("W", "H"),
+                    help="render the config's scenes at another frame size (multiples of 16 up to 256; fx = fy * H / W): the "
+                         "larger sensors of PAPER.md Table 1; not the headline workload")
     ap.add_argument("--collide", action="store_true",
                     help="also time the batch collision queries (gx_collide_batch, DESIGN.md N13) on this rank's environments; "
                          "building the column grids on the host takes about half a minute")
@@ -129,9 +132,20 @@ def load_workload(cfg: int, n_envs: int, rank: int = 0):
     return gen.make_config(cfg, env_ids=rank * n + np.arange(n), beyond=rank > 0)
 
 
+def reframe(wl, frame):
+    if frame:
+        wl.width, wl.height = int(frame[0]), int(frame[1])
+        wl.fy = 1.0
+        wl.fx = wl.height / wl.width
+        wl.name += f" at {wl.width}x{wl.height}"
+    return wl
+
+
 def workload_name(cfg: int, wl) -> str:
     from paper_2306_07552_b200 import gen
-    return f"configs[{cfg}]: {gen.CONFIG_SHAPES[cfg][0]}" + ("" if wl.N == gen.CONFIG_SHAPES[cfg][1] else f" (first {wl.N} envs)")
+    shape = gen.CONFIG_SHAPES[cfg]
+    return (f"configs[{cfg}]: {shape[0]}" + ("" if wl.N == shape[1] else f" (first {wl.N} envs)") +
+            ("" if (wl.width, wl.height) == (shape[2], shape[3]) else f" rendered at {wl.width}x{wl.height}"))
 
 
 def time_oracle(wl, budget_s: float = 15.0):
@@ -166,7 +180,7 @@ def run_reference(args):
         return
     import oracle
     oracle.build()
-    wl = load_workload(args.config, args.envs)
+    wl = reframe(load_workload(args.config, args.envs), args.frame)
     cores = len(os.sched_getaffinity(0))
     probe = wl.subset(np.arange(min(wl.N, 2 * cores)))
     t0 = time.perf_counter(); oracle.render(probe, n_threads=cores); rate = probe.N / (time.perf_counter() - t0)
@@ -222,7 +236,7 @@ def run_gx(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    wl = load_workload(args.config, args.envs, rank)
+    wl = reframe(load_workload(args.config, args.envs, rank), args.frame)
     N, K, H, W = wl.N, wl.K, wl.height, wl.width
     scene = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, local)
     for o in args.opt:
