@@ -101,6 +101,53 @@ int gx_render_batch(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K
                     float *depth_out, uint32_t *id_out, void *cuda_stream);
 
 /*
+ * gx_render_batch_noalloc -- gx_render_batch for callers that must not enter the CUDA allocator while they render.
+ *
+ * Who that is: gx_render_batch and gx_reserve obtain the record arena and the per-call tables with cudaMalloc (and
+ * give them back with cudaFree when they have to grow).  That is unusable where the renderer is a guest on a device
+ * whose memory another component has already claimed -- a simulation worker inside a training process whose tensor
+ * allocator holds all remaining device memory, so that a cudaMalloc of the arena fails or takes memory the policy's
+ * next batch needs -- and where the render call runs beside other streams (the policy's inference):
+ * cudaMalloc and cudaFree wait for the whole device, so one growing render call stalls every stream of the process.
+ * Such callers own their inputs and outputs (they pass them here as usual) but have no way to own the renderer's
+ * intermediate memory, which has no public layout.
+ *
+ * What it does instead: the arena and the tables are carved out of one array of GX_NOALLOC_SCRATCH_BYTES bytes that
+ * is part of the library's device image (a file-scope __device__ array; every GPU that uses libgx.so holds these
+ * bytes from the time the library's kernels are loaded on it until the process exits, whether or not this entry
+ * point is ever called).  K1 (cull_kernel) runs as in gx_render_batch with its tables in that array; K2-K5 run as
+ * one cooperative kernel, a variant of the tail kernel of gx_render_batch that starts at the first environment and
+ * renders the batch in as many waves as the arena left in the array requires.  The images are the same, bit for bit
+ * (tests/test_zz_no_alloc.py); a call is slower than gx_render_batch when it needs several waves.
+ *
+ * Arguments, stream semantics and results exactly as gx_render_batch.  The options "cull", "subcull", "hiz",
+ * "occlusion", "occl_area", "big_px" and "ctas_per_sm" apply; "stats", "timing", "pool_bytes" and "arena_slots" do not, and
+ * gx_get_stat keeps describing the last gx_render_batch.  The scene handle still comes from gx_create_scene, which
+ * allocates (meshes are uploaded once, at start-up, before the device's memory is handed to anyone else).
+ *   The call itself uses no cudaMalloc, cudaMallocAsync, cudaFree or other allocating routine, on any path.
+ *   Limit: the tables of the call shape (about 150 KB per environment at 128x128 with 25 instance slots; 8 bytes per
+ *   pixel plus the work-item lists) and an arena for at least the largest environment the scene can produce
+ *   (88 bytes x (4 x (largest static mesh + K x largest dynamic mesh, in triangles) + 64)) must fit
+ *   GX_NOALLOC_SCRATCH_BYTES together; e.g. up to about 250 environments of a 50k-triangle scene with 25 slots of
+ *   1k-triangle meshes at 128x128.  A shape beyond that returns UNSUPPORTED and the message names the bytes needed
+ *   and the bytes there are; nothing is enqueued.
+ *   First call on a device: looks up the array's device address and the launch shape of the cooperative kernel for
+ *   that device and keeps them for the process's lifetime (no allocation; a few driver queries).  Make that first
+ *   call outside any stream capture.
+ *   Sharing: every call on a device, from every handle and every thread, uses the same array.  The call clears the
+ *   words that must start at zero (control words, the hi-Z pyramid) on cuda_stream itself and overwrites everything
+ *   else before reading it, so the previous call's contents never show; but two calls whose GPU work overlaps (two
+ *   streams, two threads, two handles) race on the array and give undefined images.  Order them on one stream or
+ *   with events.  gx_render_batch does not use the array and may overlap with it.
+ * Errors: as gx_render_batch, plus UNSUPPORTED (shape beyond the array; device ordinal >= 64; device without
+ * cooperative launch).
+ */
+#define GX_NOALLOC_SCRATCH_BYTES (64u << 20)
+int gx_render_batch_noalloc(GxScene *scene, const GxCamera *camera, int32_t N, int32_t K, const int32_t *env_scene,
+                            const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform, uint8_t *rgb_out,
+                            float *depth_out, uint32_t *id_out, void *cuda_stream);
+
+/*
  * gx_reserve -- allocate (or grow) everything the handle needs for calls of this shape now, so that the render calls
  * that follow never allocate: the record arena (option "pool_bytes": at most an eighth of the device's memory and
  * 16 GB by default; what does not fit is rendered in further waves) and the per-call tables.  Optional: the first

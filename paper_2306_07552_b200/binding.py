@@ -18,9 +18,10 @@ LIB_PATH = os.path.join(_HERE, "libgx.so")
 
 GX_OK, GX_ERR_INVALID_ARG, GX_ERR_CUDA, GX_ERR_OOM, GX_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 GX_BACKGROUND_ID = 0xFFFFFFFF
+GX_NOALLOC_SCRATCH_BYTES = 64 << 20
 EXPORTS = ("gx_create_scene", "gx_render_batch", "gx_render_batch_host", "gx_set_option", "gx_get_stat",
            "gx_render_batch_obs", "gx_set_robot", "gx_update_transforms", "gx_reserve", "gx_set_collision_world",
-           "gx_collide_batch", "gx_destroy", "gx_last_error")
+           "gx_collide_batch", "gx_render_batch_noalloc", "gx_destroy", "gx_last_error")
 
 
 class GxMesh(C.Structure):
@@ -65,7 +66,7 @@ def lib():
         L = C.CDLL(LIB_PATH)
         L.gx_last_error.restype = C.c_char_p
         L.gx_destroy.restype = None
-        for n in EXPORTS[:11]:
+        for n in EXPORTS[:-2]:
             getattr(L, n).restype = C.c_int
         _lib = L
     return _lib
@@ -125,6 +126,16 @@ def gx_render_batch(scene, camera: GxCamera, N: int, K: int, env_scene, cam_pose
     _check(lib().gx_render_batch(scene, C.byref(camera), C.c_int32(N), C.c_int32(K), _dev(env_scene), _dev(cam_pose),
                                  _dev(inst_mesh), _dev(inst_xform), _dev(rgb_out), _dev(depth_out), _dev(id_out),
                                  C.c_void_p(cuda_stream)))
+
+
+def gx_render_batch_noalloc(scene, camera: GxCamera, N: int, K: int, env_scene, cam_pose, inst_mesh, inst_xform,
+                            rgb_out, depth_out, id_out=None, cuda_stream: int = 0) -> None:
+    """gx_render_batch for callers that must not let the library call cudaMalloc / cudaFree (include/gx.h): same
+    arguments and images, intermediate memory from the library's built-in GX_NOALLOC_SCRATCH_BYTES array; raises
+    GxError(GX_ERR_UNSUPPORTED) for shapes beyond it.  Calls on one device must not overlap on the GPU."""
+    _check(lib().gx_render_batch_noalloc(scene, C.byref(camera), C.c_int32(N), C.c_int32(K), _dev(env_scene),
+                                         _dev(cam_pose), _dev(inst_mesh), _dev(inst_xform), _dev(rgb_out),
+                                         _dev(depth_out), _dev(id_out), C.c_void_p(cuda_stream)))
 
 
 def gx_render_batch_obs(scene, camera: GxCamera, N: int, K: int, env_scene, cam_pose, inst_mesh, inst_xform, obs_out,

@@ -4,6 +4,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <unordered_map>
@@ -966,3 +967,202 @@ int gx_render_batch_host(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K,
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
+// gx_render_batch_noalloc (include/gx.h): the render path for callers that must not enter the CUDA allocator.
+// Everything gx_render_batch keeps in cudaMalloc'ed buffers of the handle (record arena, per-call tables) lives in
+// the array below instead, which belongs to the library's device image: it exists on every GPU that loads these
+// kernels, from module load to process exit, and no call ever allocates or frees it.
+// ------------------------------------------------------------------------------------------------
+namespace {
+
+// The scratch.  In HOST code this name is only a handle for the runtime's symbol calls -- it is not a device address,
+// and a kernel handed `g_noalloc_scratch` from the host would fault (or, on a system where the GPU can reach host
+// memory, quietly use host memory).  The host gets the real address once per device from cudaGetSymbolAddress
+// (noalloc_device_setup) and passes that to the kernels inside PipeParams.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[GX_NOALLOC_SCRATCH_BYTES];
+
+// K2-K5 over the whole batch as ONE cooperative kernel: tail_kernel's wave loop (gx_pipeline.cuh), except that it
+// starts at environment 0 instead of where the host-launched first wave ended.  cull_kernel has run before it on the
+// same stream (U, item lists and model-view tables are in the scratch); its own allocation of a first wave is simply
+// redone here.
+__global__ void __launch_bounds__(gx::TAIL_WARPS * 32, 3) noalloc_waves_kernel(const gx::PipeParams PP) {
+    using namespace gx;
+    extern __shared__ __align__(16) unsigned char smem[];
+    cg::grid_group grid = cg::this_grid();
+    const int warp = threadIdx.x >> 5;
+    uint32_t e_next = 0;
+    while (e_next < (uint32_t)PP.g.N) {
+        grid.sync();   // every CTA has read the end of the previous wave before the control words change
+        if (blockIdx.x == 0) alloc_wave(PP, e_next);
+        grid.sync();
+        pack_stage<true>(PP);
+        grid.sync();
+        for (int phase = PP.occl ? 1 : 0; phase <= (PP.occl ? 2 : 0); ++phase) {
+            if (phase == 2) {
+                cull2_stage<true, false>(PP);
+                grid.sync();
+            }
+            if (phase == 2 && PP.hiz) geom_stage<true, false, true>(PP, smem + (size_t)warp * GEOM_WARP_SMEM, phase);
+            else geom_stage<true, false, false>(PP, smem + (size_t)warp * GEOM_WARP_SMEM, phase);
+            grid.sync();
+            bin_stage<true, false>(PP, reinterpret_cast<uint32_t *>(smem), reinterpret_cast<uint32_t *>(smem) + PP.T * NBUCKET, phase);
+            grid.sync();
+            if (phase == 0) raster_stage<true, false, 0>(PP, smem + (size_t)warp * RAST_WARP_SMEM);
+            else if (phase == 1) raster_stage<true, false, 1>(PP, smem + (size_t)warp * RAST_WARP_SMEM);
+            else raster_stage<true, false, 2>(PP, smem + (size_t)warp * RAST_WARP_SMEM);
+            grid.sync();
+        }
+        e_next = __ldcg(&PP.ctl[C_WAVE_E1]);
+    }
+}
+
+// What the first call on a device finds out and every later call reuses.  Plain static storage: nothing is allocated.
+constexpr int NOALLOC_MAX_DEVICES = 64;
+struct NoallocDevice {
+    bool ready = false;
+    unsigned char *base = nullptr;   // device address of g_noalloc_scratch on this device
+    int ctas_per_sm = 0;             // co-resident CTAs of noalloc_waves_kernel at its largest shared-memory size
+};
+NoallocDevice g_noalloc_dev[NOALLOC_MAX_DEVICES];
+std::mutex g_noalloc_mutex;
+
+// Once per device, with that device current (the caller's DeviceGuard): the array's address on THIS device -- each
+// device has its own copy of the array at its own address -- and the cooperative kernel's launch shape.
+int noalloc_device_setup(int device, NoallocDevice **out) {
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES)
+        return fail(GX_ERR_UNSUPPORTED, "gx_render_batch_noalloc supports device ordinals below %d, got %d", NOALLOC_MAX_DEVICES, device);
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    NoallocDevice &d = g_noalloc_dev[device];
+    if (!d.ready) {
+        int coop = 0;
+        GX_CUDA(cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device));
+        if (!coop) return fail(GX_ERR_UNSUPPORTED, "device %d cannot launch cooperative kernels", device);
+        void *p = nullptr;
+        GX_CUDA(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+        if (!p || ((uintptr_t)p & 255u)) return fail(GX_ERR_CUDA, "cudaGetSymbolAddress gave %p for the scratch array", p);
+        const size_t smem = gx::tail_smem_bytes((GX_MAX_FRAME / gx::TILE) * (GX_MAX_FRAME / gx::TILE));   // (the largest any frame needs)
+        GX_CUDA(cudaFuncSetAttribute((const void *)noalloc_waves_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int per_sm = 0;
+        GX_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)noalloc_waves_kernel, gx::TAIL_WARPS * 32, smem));
+        if (per_sm < 1) return fail(GX_ERR_UNSUPPORTED, "the cooperative kernel does not fit an SM of device %d", device);
+        d.base = static_cast<unsigned char *>(p);
+        d.ctas_per_sm = per_sm;
+        d.ready = true;
+    }
+    *out = &d;
+    return GX_OK;
+}
+
+}  // namespace
+
+extern "C" int gx_render_batch_noalloc(GxScene *sc, const GxCamera *cam, int32_t N, int32_t K, const int32_t *env_scene,
+                                       const float *cam_pose, const int32_t *inst_mesh, const float *inst_xform,
+                                       uint8_t *rgb_out, float *depth_out, uint32_t *id_out, void *cuda_stream) {
+    if (!sc || !cam) return fail(GX_ERR_INVALID_ARG, "NULL scene or camera");
+    if (N <= 0) return fail(GX_ERR_INVALID_ARG, "N must be positive, got %d", N);
+    if (K < 0 || K > GX_MAX_INSTANCES) return fail(GX_ERR_INVALID_ARG, "K must be in [0, %d], got %d", GX_MAX_INSTANCES, K);
+    if (!env_scene || !cam_pose || !depth_out) return fail(GX_ERR_INVALID_ARG, "env_scene, cam_pose and depth_out are required");
+    if (K > 0 && (!inst_mesh || !inst_xform)) return fail(GX_ERR_INVALID_ARG, "inst_mesh and inst_xform are required when K > 0");
+    if (cam->width <= 0 || cam->height <= 0 || cam->width % 16 || cam->height % 16)
+        return fail(GX_ERR_INVALID_ARG, "width and height must be positive multiples of 16, got %dx%d", cam->width, cam->height);
+    if (!(cam->znear > 0.0f) || !(cam->zfar > cam->znear)) return fail(GX_ERR_INVALID_ARG, "need 0 < znear < zfar");
+    if (!(cam->fx > 0.0f) || !(cam->fy > 0.0f)) return fail(GX_ERR_INVALID_ARG, "fx and fy must be positive");
+    if (cam->width > GX_MAX_FRAME || cam->height > GX_MAX_FRAME)
+        return fail(GX_ERR_UNSUPPORTED, "width and height must be <= %d, got %dx%d", GX_MAX_FRAME, cam->width, cam->height);
+    const unsigned long long worst_tris = (unsigned long long)sc->max_static_nt + (unsigned long long)K * sc->max_dyn_nt;
+    if (worst_tris >= (1ull << 29)) return fail(GX_ERR_UNSUPPORTED, "more than 2^29 triangles per environment");
+    DeviceGuard guard(sc->device);
+    if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);
+    NoallocDevice *dev = nullptr;
+    int rc;
+    if ((rc = noalloc_device_setup(sc->device, &dev)) != GX_OK) return rc;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    gx::PipeParams PP;
+    memset(&PP, 0, sizeof(PP));
+    GxParams &P = PP.g;
+    P.verts = sc->verts; P.tris = sc->tris; P.batches = sc->batches; P.subs = sc->subs; P.clusters = sc->clusters; P.meshes = sc->meshes;
+    P.n_static = sc->n_static; P.n_dyn = sc->n_dyn;
+    P.N = N; P.K = K; P.W = cam->width; P.H = cam->height;
+    P.fx = cam->fx; P.fy = cam->fy; P.znear = cam->znear; P.zfar = cam->zfar;
+    P.env_scene = env_scene; P.cam_pose = cam_pose; P.inst_mesh = inst_mesh; P.inst_xform = inst_xform;
+    P.rgb = rgb_out; P.depth = depth_out; P.id = id_out;
+    P.obs = nullptr; P.obs_dmin = 0.0f; P.obs_dmax = 1.0f; P.obs_range = 1.0f;
+    P.stats = sc->stats;   // (never touched: only the kernels without the statistics are used here)
+    P.cull = sc->opt_cull;
+    PP.tiles_x = P.W / gx::TILE; PP.tiles_y = P.H / gx::TILE; PP.T = PP.tiles_x * PP.tiles_y;
+    PP.bucket_off = -log2f(P.znear);
+    PP.bucket_scale = (float)gx::NBUCKET / log2f(P.zfar / P.znear);
+    PP.subcull = sc->opt_subcull;
+    PP.big_px = sc->opt_big_px;
+    PP.hiz = sc->opt_hiz;
+    PP.occl = sc->opt_hiz && (sc->opt_occlusion == 1 || (sc->opt_occlusion < 0 && P.W * P.H >= 4096)) ? 1 : 0;
+    PP.occl_area = (float)sc->opt_occl_area;
+    PP.item_stride = (int32_t)std::max<size_t>((size_t)sc->max_static_batches + (size_t)K * sc->max_dyn_batches, 1);
+    PP.hz_stride = 0;
+    for (int w = PP.tiles_x, h = PP.tiles_y;; w = (w + 1) >> 1, h = (h + 1) >> 1) { PP.hz_stride += w * h; if (w == 1 && h == 1) break; }
+
+    // ---- carve the array: tables first (the order of setup_buffers), the arena takes what is left ------------
+    const size_t cap = (size_t)GX_NOALLOC_SCRATCH_BYTES;
+    const size_t n = (size_t)N, k1 = (size_t)K + 1, NK1 = (size_t)PP.T * gx::NBUCKET + 1, istr = (size_t)PP.item_stride;
+    size_t off = 0;   // bytes
+    auto take = [&off](size_t bytes) { const size_t at = off; off = (off + bytes + 255) & ~(size_t)255; return at; };   // (N < 2^31 and the factors below keep every product far inside 64 bits)
+    const size_t o_ctl = take(64 * 4);
+    const size_t o_U = take(n * 4), o_nitems = take(n * 4), o_cpre = take((n + 1) * 4), o_base = take(n * 4);
+    const size_t o_cnt = take(n * 4), o_cntA = take(n * 4), o_nl = take(n * 4);
+    const size_t o_idb = take(n * k1 * 4), o_mv = take(n * k1 * 48);
+    const size_t o_toff = take(n * NK1 * 4), o_tasks = take((size_t)gx::NCLASS * n * (size_t)PP.T * 4);
+    const size_t hizt_bytes = PP.occl ? n * (size_t)PP.hz_stride * 4 : 0;
+    const size_t o_hizt = take(hizt_bytes), o_hizb = take(PP.occl ? n * (size_t)PP.T * 32 : 0);
+    const size_t o_items = take(n * istr * 16), o_witems = take(n * istr * 16), o_witems2 = take(PP.occl ? n * istr * 16 : 0);
+    const size_t o_keys = take(PP.occl ? n * (size_t)P.W * (size_t)P.H * 8 : 0);
+    const size_t tables = off;
+    // record slots: 64 bytes of record, 8 of box / depth word, 16 of tile references; the arena must hold the largest
+    // environment the scene can produce (setup_buffers has the reasoning), more only shortens the wave loop
+    const unsigned long long worst_env = 4ull * worst_tris + 64;
+    const unsigned long long need = (unsigned long long)tables + worst_env * 88ull + 3 * 256;
+    if (need > cap)
+        return fail(GX_ERR_UNSUPPORTED, "gx_render_batch_noalloc: N = %d, K = %d at %dx%d needs %llu bytes of scratch (%zu for the tables of "
+                    "the call, the rest for an arena of one worst-case environment of %llu triangles) but the built-in array holds "
+                    "GX_NOALLOC_SCRATCH_BYTES = %zu; render fewer environments per call, or use gx_render_batch where allocation is allowed",
+                    N, K, cam->width, cam->height, need, tables, worst_tris, cap);
+    unsigned long long slots = (cap - tables - 3 * 256) / 88ull;
+    slots = std::min<unsigned long long>(slots, std::min<unsigned long long>((unsigned long long)N * worst_env, 0xFFFFFF00ull));
+    const size_t o_recs = take((size_t)slots * 64), o_bbs = take((size_t)slots * 8), o_refs = take((size_t)slots * 16);
+    if (off > cap) return fail(GX_ERR_UNSUPPORTED, "gx_render_batch_noalloc: internal layout error (%zu > %zu bytes)", off, cap);
+    unsigned char *b = dev->base;
+    PP.ctl = reinterpret_cast<uint32_t *>(b + o_ctl); PP.U = reinterpret_cast<uint32_t *>(b + o_U);
+    PP.n_items = reinterpret_cast<uint32_t *>(b + o_nitems); PP.item_pre = reinterpret_cast<uint32_t *>(b + o_cpre);
+    PP.rec_base = reinterpret_cast<uint32_t *>(b + o_base); PP.cnt = reinterpret_cast<uint32_t *>(b + o_cnt);
+    PP.cntA = reinterpret_cast<uint32_t *>(b + o_cntA); PP.n_large = reinterpret_cast<uint32_t *>(b + o_nl);
+    PP.env_idb = reinterpret_cast<uint32_t *>(b + o_idb); PP.env_mv = reinterpret_cast<float *>(b + o_mv);
+    PP.tile_off = reinterpret_cast<uint32_t *>(b + o_toff); PP.tasks = reinterpret_cast<uint32_t *>(b + o_tasks);
+    PP.hizt = reinterpret_cast<uint32_t *>(b + o_hizt); PP.hizb = reinterpret_cast<uint32_t *>(b + o_hizb);
+    PP.items = reinterpret_cast<uint4 *>(b + o_items); PP.wave_items = reinterpret_cast<uint4 *>(b + o_witems);
+    PP.wave_items2 = reinterpret_cast<uint4 *>(b + o_witems2);
+    PP.keys = reinterpret_cast<unsigned long long *>(b + o_keys);
+    PP.recs = reinterpret_cast<uint4 *>(b + o_recs); PP.bbs = reinterpret_cast<uint2 *>(b + o_bbs);
+    PP.refs = reinterpret_cast<uint32_t *>(b + o_refs);
+    PP.arena_slots = (uint32_t)slots;
+
+    // ---- what must start at zero; everything else in the array is written before it is read -------------------
+    GX_CUDA(cudaMemsetAsync(PP.ctl, 0, 64 * sizeof(uint32_t), stream));
+    if (PP.occl) GX_CUDA(cudaMemsetAsync(PP.hizt, 0, hizt_bytes, stream));
+    // K1, as in gx_render_batch
+    {
+        const size_t csmem = gx::env_smem_bytes(K);
+        if ((size_t)PP.item_stride > 512) gx::cull_kernel<16, false><<<N, 16 * 32, csmem, stream>>>(PP);
+        else gx::cull_kernel<4, false><<<N, 4 * 32, csmem, stream>>>(PP);
+        GX_CUDA(cudaGetLastError());
+    }
+    // K2-K5, all waves
+    {
+        int per_sm = dev->ctas_per_sm;
+        if (sc->opt_ctas_per_sm) per_sm = std::min(per_sm, sc->opt_ctas_per_sm);
+        void *args[1] = {(void *)&PP};
+        GX_CUDA(cudaLaunchCooperativeKernel((const void *)noalloc_waves_kernel, dim3((unsigned)(sc->num_sms * per_sm)),
+                                            dim3(gx::TAIL_WARPS * 32), args, gx::tail_smem_bytes(PP.T), stream));
+    }
+    return GX_OK;
+}
