@@ -89,7 +89,10 @@ int gx_create_scene(const GxMesh *static_meshes, int32_t n_static, const GxMesh 
  * steady state does not.  The call may be captured into a CUDA graph (cudaStreamBeginCapture on cuda_stream) once
  * the handle holds its buffers for this shape (gx_reserve, or one plain call): inside a capture it allocates
  * nothing and reads nothing back, and returns UNSUPPORTED if it would have to; replays read the input arrays and
- * write the output arrays the captured call was given.  Same inputs give bit-identical outputs, independent of how N is sharded.
+ * write the output arrays the captured call was given.  A graph stays valid for the life of the handle: when a later
+ * call makes the handle grow, buffers a captured call used are kept (not freed) until gx_destroy, and the graph goes
+ * on rendering with the arena it was captured with.  A call that fails with OOM while growing leaves the handle
+ * without an arena but usable: the next call allocates again.  Same inputs give bit-identical outputs, independent of how N is sharded.
  * NaN/Inf inputs and out-of-range env_scene/inst_mesh values are precondition violations: the image is
  * undefined, but no out-of-bounds write occurs for in-range ids.
  * Errors: INVALID_ARG (null handle/camera/required pointer, N <= 0, K < 0, K > GX_MAX_INSTANCES, width or

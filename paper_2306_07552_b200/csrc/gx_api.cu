@@ -52,11 +52,17 @@ template <typename T>
 struct DevBuf {
     T *p = nullptr;
     size_t n = 0;
-    int reserve(size_t want) {   // grow only; contents are not kept
+    bool in_graph = false;   // a captured CUDA graph holds this buffer's address
+    // grow only; contents are not kept.  A buffer a graph may still use is not freed but handed to `retired`
+    // (gx_destroy frees that list), so that replaying the graph stays valid
+    int reserve(size_t want, std::vector<void *> *retired = nullptr) {
         if (want <= n) return GX_OK;
-        if (p) cudaFree(p);
+        if (p && in_graph && retired) {
+            try { retired->push_back(p); } catch (const std::bad_alloc &) { return fail(GX_ERR_OOM, "host allocation failed"); }
+        } else if (p) cudaFree(p);
         p = nullptr;
         n = 0;
+        in_graph = false;
         GX_CUDA(cudaMalloc(&p, want * sizeof(T)));
         n = want;
         return GX_OK;
@@ -106,6 +112,7 @@ struct GxScene {
     cudaEvent_t ev_ctl = nullptr;
     bool ctl_pending = false;
     bool capturing = false;             // the current call's stream is being captured into a CUDA graph
+    std::vector<void *> retired;        // buffers a captured graph may still use, replaced by larger ones since; freed by gx_destroy
     int ctl_N = 0;
     double hist_u_per_env = 0.0;
     int hist_waves = 1;                 // waves the last call needed (the host launches that many rounds of the stage kernels)
@@ -389,6 +396,7 @@ void gx_destroy(GxScene *sc) {
     cudaFree(sc->mesh_box); cudaFree(sc->cg_grids); cudaFree(sc->cg_col_off); cudaFree(sc->cg_layers); cudaFree(sc->cg_radii);
     cudaFree(sc->cg_spheres);
     sc->arena_recs.release(); sc->arena_bbs.release(); sc->arena_refs.release(); sc->scratch.release();
+    for (void *q : sc->retired) cudaFree(q);
     for (cudaEvent_t e : sc->t_ev) cudaEventDestroy(e);
     if (sc->h_ctl) cudaFreeHost(sc->h_ctl);
     if (sc->ev_ctl) cudaEventDestroy(sc->ev_ctl);
@@ -546,14 +554,22 @@ static int setup_buffers(GxScene *sc, gx::PipeParams &PP, unsigned long long wor
     if (want > sc->arena_slots && sc->capturing) want = sc->arena_slots;   // (no allocation inside a capture: more waves instead)
     if (sc->capturing && sc->arena_slots < worst_env)
         return fail(GX_ERR_UNSUPPORTED, "the arena cannot hold one environment of this shape: call gx_reserve (or render once) before capturing the call into a CUDA graph");
+    // Buffers whose addresses a captured graph holds are never freed while the handle lives: when one has to grow it is
+    // retired instead, so that replaying the earlier graph stays valid (it keeps the arena it was captured with).
+    std::vector<void *> *keep = &sc->retired;
     if (want > sc->arena_slots) {
-        if ((rc = sc->arena_recs.reserve((size_t)want * 4)) != GX_OK) return rc;
-        if ((rc = sc->arena_bbs.reserve((size_t)want)) != GX_OK) return rc;
-        if ((rc = sc->arena_refs.reserve((size_t)want * 4)) != GX_OK) return rc;
+        // the three arrays grow one by one and any of the allocations can fail: until all of them have the new size the
+        // handle holds no arena at all, so that a later (smaller) call allocates again instead of trusting a stale size
+        sc->arena_slots = 0;
+        if ((rc = sc->arena_recs.reserve((size_t)want * 4, keep)) != GX_OK) return rc;
+        if ((rc = sc->arena_bbs.reserve((size_t)want, keep)) != GX_OK) return rc;
+        if ((rc = sc->arena_refs.reserve((size_t)want * 4, keep)) != GX_OK) return rc;
         sc->arena_slots = (size_t)want;
     }
     PP.recs = sc->arena_recs.p; PP.bbs = sc->arena_bbs.p; PP.refs = sc->arena_refs.p;
-    PP.arena_slots = (uint32_t)(sc->opt_arena_slots > 0 ? std::max<uint64_t>((uint64_t)sc->opt_arena_slots, worst_env) : sc->arena_slots);
+    // (never more than is held: inside a capture the arena does not grow, whatever "arena_slots" asks for)
+    PP.arena_slots = (uint32_t)std::min<uint64_t>(sc->opt_arena_slots > 0 ? std::max<uint64_t>((uint64_t)sc->opt_arena_slots, worst_env) : (uint64_t)sc->arena_slots,
+                                                  (uint64_t)sc->arena_slots);
 
     // ---- scratch words: ctl | U | rec_base | cnt | cntA | n_large | env_idb | env_mv | tile_off | tasks | hizt | hizb | items | keys
     const size_t n = (size_t)N, k1 = (size_t)K + 1, NK1 = (size_t)PP.T * gx::NBUCKET + 1;
@@ -581,7 +597,9 @@ static int setup_buffers(GxScene *sc, gx::PipeParams &PP, unsigned long long wor
     const size_t o_keys = off; off += PP.occl ? n * (size_t)P.W * (size_t)P.H * 2 : 0;
     if (off > sc->scratch.n && sc->capturing)
         return fail(GX_ERR_UNSUPPORTED, "the handle's tables would have to grow during stream capture: call gx_reserve for this shape first");
-    if ((rc = sc->scratch.reserve(off)) != GX_OK) return rc;
+    if ((rc = sc->scratch.reserve(off, keep)) != GX_OK) return rc;
+    if (sc->capturing)   // (what this call enqueues is recorded with these addresses)
+        sc->arena_recs.in_graph = sc->arena_bbs.in_graph = sc->arena_refs.in_graph = sc->scratch.in_graph = true;
     uint32_t *sp = sc->scratch.p;
     PP.ctl = sp; PP.U = sp + o_U; PP.n_items = sp + o_nitems; PP.item_pre = sp + o_cpre; PP.rec_base = sp + o_base;
     PP.cnt = sp + o_cnt; PP.cntA = sp + o_cntA; PP.n_large = sp + o_nl; PP.env_idb = sp + o_idb;

@@ -391,6 +391,102 @@ def test_cuda_graph_capture_and_replay(oracle_mod):
             gx.gx_destroy(sc)
 
 
+def test_cuda_graph_survives_growth_of_the_handle(oracle_mod):
+    """A captured call bakes the handle's arena and table addresses into the graph.  Later plain calls that make the
+    handle grow (more environments; a larger arena) must not free what the graph uses: the old buffers are retired
+    until gx_destroy, replaying the earlier graph still gives the oracle's images, and so does a second graph captured
+    after the growth.  Inside a capture "arena_slots" can never hand out more slots than the handle holds."""
+    import torch
+    from paper_2306_07552_b200 import binding as gx
+    wl = gen.make_config(1, n_envs=8)
+    big = gen.make_config(1, n_envs=48)
+    o, ob = oracle_mod.render(wl), oracle_mod.render(big)
+    dev = torch.device("cuda:0")
+    sc = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, 0)
+    try:
+        cam = gx.camera_of(wl)
+        N, K, H, W = wl.N, wl.K, wl.height, wl.width
+        t = lambda a, ty: torch.from_numpy(np.ascontiguousarray(a, ty)).to(dev)
+        d = [t(wl.env_scene, np.int32), t(wl.cam_pose, np.float32), t(wl.inst_mesh, np.int32), t(wl.inst_xform, np.float32)]
+        rgb = torch.zeros((N, H, W, 3), dtype=torch.uint8, device=dev)
+        depth = torch.zeros((N, H, W), dtype=torch.float32, device=dev)
+        ids = torch.zeros((N, H, W), dtype=torch.int32, device=dev)
+        s = torch.cuda.Stream()
+
+        def capture():
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=s):
+                gx.gx_render_batch(sc, cam, N, K, d[0], d[1], d[2], d[3], rgb, depth, ids, torch.cuda.current_stream().cuda_stream)
+            return g
+
+        def replay_ok(g, what):
+            depth.fill_(-1.0); ids.fill_(7); rgb.fill_(9)
+            g.replay()
+            torch.cuda.synchronize()
+            got = dict(rgb=rgb.cpu().numpy(), depth=depth.cpu().numpy(), id=ids.cpu().numpy().view(np.uint32))
+            rep = compare(o, got)
+            assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0 and rep["rgb_differ"] == 0, (what, rep)
+
+        gx.gx_set_option(sc, "arena_slots", 400000)         # a small arena (worst case of one environment: ~300k slots)
+        gx.gx_reserve(sc, cam, N, K)
+        a0, s0 = gx.gx_get_stat(sc, "arena_bytes"), gx.gx_get_stat(sc, "scratch_bytes")
+        g1 = capture()
+        replay_ok(g1, "first graph")
+        # inside a capture the option may ask for more than is held: more waves, never slots past the allocation
+        gx.gx_set_option(sc, "arena_slots", 4000000)
+        g1b = capture()
+        assert gx.gx_get_stat(sc, "arena_bytes") == a0
+        replay_ok(g1b, "graph captured with arena_slots beyond the held arena")
+        # plain calls that grow both the arena and the tables
+        gx.gx_set_option(sc, "arena_slots", 0)
+        for _ in range(2):
+            gb = render_gpu(big, scene=sc)
+            rep = compare(ob, gb)
+            assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0, rep
+        assert gx.gx_get_stat(sc, "arena_bytes") > a0 and gx.gx_get_stat(sc, "scratch_bytes") > s0
+        junk = [torch.full((1 << 26,), 0x7F, dtype=torch.uint8, device=dev) for _ in range(4)]   # reuse whatever was freed
+        replay_ok(g1, "first graph after the handle grew")
+        replay_ok(g1b, "second graph after the handle grew")
+        g2 = capture()
+        replay_ok(g2, "graph captured after the growth")
+        replay_ok(g1, "first graph again")
+        del junk
+    finally:
+        gx.gx_destroy(sc)
+
+
+def test_failed_arena_growth_leaves_the_handle_usable(oracle_mod):
+    """The arena is three arrays that grow one after the other.  When the device runs out of memory in the middle (the
+    first array fits, the second does not) the call returns GX_ERR_OOM and the handle must not keep the old arena
+    size with a missing array: the next, smaller call allocates afresh and renders the oracle's images."""
+    import torch
+    from paper_2306_07552_b200 import binding as gx
+    wl = gen.make_config(1, n_envs=6)
+    o = oracle_mod.render(wl)
+    sc = gx.gx_create_scene(wl.static_meshes, wl.dyn_meshes, 0)
+    try:
+        g = render_gpu(wl, scene=sc)                         # the handle holds an arena and renders
+        assert compare(o, g)["id_mismatch"] == 0
+        torch.cuda.empty_cache()
+        free, _total = torch.cuda.mem_get_info()
+        # 64 + 8 + 16 bytes per slot in three arrays: at free / 70 slots the first (64 B) fits and the second cannot
+        slots = int(free // 70)
+        if slots >= 0xFFFFFF00:
+            pytest.skip("more free device memory than a 2^32-slot arena can use up")
+        gx.gx_set_option(sc, "arena_slots", slots)
+        with pytest.raises(gx.GxError) as ei:
+            render_gpu(wl, scene=sc)
+        assert ei.value.code == gx.GX_ERR_OOM, str(ei.value)
+        assert gx.gx_get_stat(sc, "arena_bytes") == 0        # nothing usable is claimed
+        gx.gx_set_option(sc, "arena_slots", 0)
+        for _ in range(2):
+            g = render_gpu(wl, scene=sc)
+            rep = compare(o, g)
+            assert rep["id_mismatch"] == 0 and rep["depth_bits_differ"] == 0 and rep["rgb_differ"] == 0, rep
+    finally:
+        gx.gx_destroy(sc)
+
+
 def test_argument_errors():
     import torch
     from paper_2306_07552_b200 import binding as gx
