@@ -48,7 +48,7 @@ typedef struct {
 
 /* Pinhole camera shared by all environments of a call. */
 typedef struct {
-    int32_t width, height; /* pixels; multiples of 16; each <= 128 in this build */
+    int32_t width, height; /* pixels; multiples of 16; each <= GX_MAX_FRAME */
     float fx, fy;          /* NDC focal lengths: fy = 1/tan(fovy/2), fx = fy*height/width; 90 deg square: 1 */
     float znear, zfar;     /* metres, 0 < znear < zfar; fragments with view depth > zfar are dropped */
 } GxCamera;
@@ -283,6 +283,9 @@ int gx_collide_batch(GxScene *scene, int32_t N, int32_t K, const int32_t *env_sc
  *   "ctas_per_sm"  0..8 (0 = as many as fit) CTAs per SM of the persistent geometry and raster kernels, for callers
  *                            that run other kernels beside the renderer.
  *   "bin_threads"  0|256|512 (0 = 512) threads per CTA of the bin kernel.
+ *   "max_rounds"   >= 0 (0 = no limit) rounds of stage kernels the host launches per call; with several waves the
+ *                            host launches one round per wave the previous call needed and the cooperative tail kernel
+ *                            renders what is left, so 1 sends every wave after the first to the tail kernel (tests).
  *   "stats"        0|1 (0)   count what gx_get_stat reports (slower kernels).
  *   "timing"       0|1 (0)   1 starts (and resets), 0 stops recording CUDA events around every kernel of
  *                            subsequent gx_render_batch calls on their stream.

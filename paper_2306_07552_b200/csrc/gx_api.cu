@@ -89,7 +89,7 @@ struct GxScene {
     uint32_t max_dyn_nt = 0, max_static_nt = 0;
     uint32_t max_static_batches = 0, max_dyn_batches = 0;   // largest number of batches in any static / dynamic mesh
     int max_smem_optin = 0;
-    int64_t default_pool_bytes = (int64_t)4 << 30;   // arena budget: an eighth of the device's memory, at most 16 GB
+    int64_t default_pool_bytes = (int64_t)4 << 30;   // arena budget: set by gx_create_scene to an eighth of the device's memory, at most 16 GB
     unsigned long long *stats = nullptr;   // device [GX_NSTAT]
     // options (gx_set_option)
     int opt_cull = 1, opt_subcull = 1, opt_stats = 0, opt_hiz = 1, opt_big_px = 24;
@@ -97,9 +97,9 @@ struct GxScene {
     int opt_max_rounds = 0;             // rounds of stage kernels the host launches at most (0 = no limit; 1 = later waves all in the tail kernel)
     int opt_ctas_per_sm = 0;            // persistent kernels: CTAs per SM (0 = as many as fit); smaller when two handles share the GPU
     int opt_host_sub = 0;               // gx_render_batch_host: environments per sub-batch; 0 = automatic
-    int opt_occlusion = -1;             // occluder scheme: 1 on, 0 off, -1 automatic (on for frames of at least 8192 pixels)
+    int opt_occlusion = -1;             // occluder scheme: 1 on, 0 off, -1 automatic (on for frames of at least 4096 pixels)
     int opt_occl_area = 64;             // pixels per triangle of a sub-cluster's screen box that make it an occluder
-    int64_t opt_pool_bytes = 0;         // arena budget; 0 = 4 GB
+    int64_t opt_pool_bytes = 0;         // arena budget; 0 = default_pool_bytes (an eighth of the device's memory, at most 16 GB)
     int64_t opt_arena_slots = 0;        // force the arena size in record slots (tests: several waves); 0 = automatic
     // scratch owned by the handle: grows on demand, never inside a steady-state call
     DevBuf<uint4> arena_recs;
@@ -842,7 +842,6 @@ int gx_update_transforms(GxScene *sc, int32_t N, int32_t K, int32_t link_slot0, 
     if (N <= 0 || K < 0 || K > GX_MAX_INSTANCES) return fail(GX_ERR_INVALID_ARG, "bad N or K");
     if (!base_pose || !joint_pos || !cam_pose || !inst_xform) return fail(GX_ERR_INVALID_ARG, "NULL array argument");
     if ((held_slot == nullptr) != (held_xform == nullptr)) return fail(GX_ERR_INVALID_ARG, "held_slot and held_xform go together");
-    if (held_slot && sc->fk_ee_link < -1) return fail(GX_ERR_INVALID_ARG, "no end-effector link");
     if (link_slot0 < 0 || link_slot0 + sc->fk_L > K) return fail(GX_ERR_INVALID_ARG, "link slots [%d, %d) do not fit K = %d", link_slot0, link_slot0 + sc->fk_L, K);
     DeviceGuard guard(sc->device);
     if (!guard.ok) return fail(GX_ERR_CUDA, "cannot select CUDA device %d", sc->device);

@@ -1,4 +1,4 @@
-// gx_types.h -- device-side data layout shared by the host API (gx_api.cu) and the kernels (gx_kernels.cuh).
+// gx_types.h -- device-side data layout shared by the host API (gx_api.cu) and the kernels (gx_pipeline.cuh).
 // Product code: nothing here is shared with oracle/.
 #pragma once
 #include <cstdint>
