@@ -720,3 +720,85 @@ def test_clip_pieces_tie_goes_to_sub_zero(oracle_mod):
             if found >= 6:
                 break
     assert found >= 6, found
+
+
+def test_colour_rounds_half_to_even(oracle_mod):
+    """N8: `rintf(v)` -- an exact tie goes to the even integer.  floor(v + 0.5) differs at every
+    even m + 1/2, which the +-0.5 bound of test_colour_constant_and_affine cannot see.
+    Construction, every value by hand: a fronto-parallel right triangle at w = 2 (q = 1/2 exactly) with corners
+    v0 = (3, 4.5) px, v1 = (11, 4.5) px, v2 = (3, 12.5) px, so A = 2048 * 2048 = 2^22.  Vertices 0 and 1 carry the
+    colour a, vertex 2 carries a + b with b odd.  On pixel row 8 (centre y = 8.5 px, half way down) the weight of
+    vertex 2 is E_2 / A = 1/2 for every covered pixel, all products and sums are integers below 2^30 with few
+    significant bits (exact in binary32), so v = a + b / 2 = a + m + 1/2 exactly with b = 2 m + 1: the byte must be
+    a + m for even a + m and a + m + 1 for odd a + m."""
+    W = H = 16
+    XY = [[(256 * 3, 256 * 4 + 128), (256 * 11, 256 * 4 + 128), (256 * 3, 256 * 12 + 128)]]
+    row = 8
+    # row 8: covered from x = 3 px to the hypotenuse at x = 3 + 8 * (1 - 1/2) = 7 px: centres 3.5 .. 6.5 (7.5 is outside)
+    cols = [3, 4, 5, 6]
+    checked_even = checked_odd = 0
+    for a in (0, 10, 101):
+        for b0 in range(1, 256 - a, 6):
+            bs = [b for b in (b0, b0 + 2, b0 + 4) if a + b <= 255]
+            while len(bs) < 3:
+                bs.append(bs[-1])
+            col = np.zeros((1, 3, 3), np.float32)
+            col[0, 0, :] = a
+            col[0, 1, :] = a
+            col[0, 2, :] = [a + b for b in bs]
+            for flip in (0, 1):
+                xy = [[XY[0][0], XY[0][2], XY[0][1]]] if flip else XY
+                cc = col[:, [0, 2, 1], :] if flip else col
+                o = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, _soup_from_snapped(xy, W, H, w=2.0, colors=cc), [0])
+                cov = np.nonzero(o["id"][row] == 0)[0]
+                assert list(cov) == cols
+                for ch, b in enumerate(bs):
+                    m = (b - 1) // 2                      # v = a + m + 1/2
+                    lo = a + m
+                    want = lo if lo % 2 == 0 else lo + 1
+                    assert np.all(o["rgb"][row, cols, ch] == want), (a, b, flip, o["rgb"][row, cols, ch], want)
+                    checked_even += lo % 2 == 0
+                    checked_odd += lo % 2 == 1
+    assert checked_even > 50 and checked_odd > 50
+
+
+def test_snap_clamps_at_two_to_the_28(oracle_mod):
+    """N5: X and Y are clamped to +-2^28 before the conversion ('clamp to +-2^28 with fminf/fmaxf').
+    By hand at W = H = 128 (hw = hh = 16384), identity camera, fx = fy = 1, w = 1/8 (q = 8, inside: w >= znear):
+      x = 4096  -> X = 4096 * 8 * 16384 + 16384 = 2^29 + 2^14  -> clamped to  2^28;   x = -4096 -> -2^29 + 2^14 -> -2^28
+      y = 4096  -> Y = -(2^29) + 2^14 -> -2^28;                                        y = -4096 -> +2^28
+      x = 256   -> X = 256 * 8 * 16384 + 16384 = 2^25 + 2^14 = 33570816: large, inside the clamp, exact in binary32
+      x = 2047.875 (= 2^11 - 2^-3) -> X = (2^14 - 1) * 16384 + 16384 = 2^28 exactly: the largest unclamped value."""
+    W = H = 128
+    L = 1 << 28
+    pos = np.array([[4096.0, 4096.0, -0.125], [-4096.0, -4096.0, -0.125], [256.0, -256.0, -0.125],
+                    [2047.875, -2047.875, -0.125], [1.0e6, -1.0e6, -0.125]], np.float32)
+    o = oracle_mod.vertex_stage(W, H, 1.0, 1.0, 0.1, 20.0, _pose("I"), None, pos)
+    assert np.all(o["inside"] == 1)
+    assert list(o["Xi"]) == [L, -L, (1 << 25) + (1 << 14), L, L]
+    assert list(o["Yi"]) == [-L, L, (1 << 25) + (1 << 14), L, L]
+    # the raster path (N5 inside the triangle pipeline) clamps the same way: a triangle with one corner far to the
+    # right, v2 = (x = 4096, y = 0, w = 1/8) -> (2^28, 16384) after the clamp, and two corners on the screen at w = 2.
+    # Its upper edge leaves v0 one sub-pixel above the centres of pixel row 20 and sinks so slowly that where it
+    # crosses that row of centres depends on where v2 ends up: at 2^28 it crosses inside the frame (near column 104),
+    # unclamped (2^29 + 2^14) it would not cross at all, at 2^24 it would cross near column 16.  Expected coverage: the
+    # plain inequality definition in exact integers on the clamped corner.
+    X0, Y0, Y1 = 256 * 10, 256 * 20 + 127, 256 * 100
+    on = _soup_from_snapped([[(X0, Y0), (X0, Y1), (X0, Y1)]], W, H, w=2.0)[0]
+    soup = np.zeros((1, 3, 6), np.float32)
+    soup[0, 0] = on[0]
+    soup[0, 1] = on[1]
+    soup[0, 2] = [4096.0, 0.0, 0.125, 200.0, 200.0, 200.0]
+    r = oracle_mod.raster_soup(W, H, 1.0, 1.0, 0.1, 20.0, soup, [0])
+    got = r["id"] != BG
+    corners = [(X0, Y0), (X0, Y1), (L, 128 * H)]
+    want = np.zeros((H, W), bool)
+    for j in range(H):
+        for i in range(W):
+            want[j, i] = _covered_exact(corners, 256 * i + 128, 256 * j + 128)
+    assert np.array_equal(got, want), int((got != want).sum())
+    # the pin really depends on the clamp value: the other two candidate corners give other images
+    for other in ((1 << 29) + (1 << 14), 1 << 24):
+        alt = [(X0, Y0), (X0, Y1), (other, 128 * H)]
+        assert any(_covered_exact(alt, 256 * i + 128, 256 * 20 + 128) != want[20, i] for i in range(W)), other
+    assert want[20].any() and not want[20].all()
