@@ -586,7 +586,7 @@ typedef struct {
 typedef struct {
     int32_t link;            /* link the sphere is attached to (>= 0) */
     int32_t radius_class;    /* index into radii[] */
-    float centre[3];         /* in the link's frame */
+    float centre[3];         /* in the link's frame (link == -1: in the grasped object's frame) */
 } GxOracleSphere;
 
 /* object-space box of a mesh: centre 0.5f*(min+max), half extent 0.5f*(max-min) of its vertex positions */
@@ -617,8 +617,23 @@ int gx_oracle_collide(const OrMesh *dyn_meshes, int32_t n_dyn, const GxOracleCol
         if (env_scene[n] < 0 || env_scene[n] >= n_static) return -1;
         for (int s = 0; s < S; ++s) {
             const GxOracleSphere *sp = &spheres[s];
-            if (sp->link < 0 || link_slot0 + sp->link >= K || sp->radius_class < 0 || sp->radius_class >= n_radii) return -1;
-            const float *Wl = inst_xform + ((size_t)n * K + link_slot0 + sp->link) * 16;
+            if (sp->link < -1 || (sp->link >= 0 && link_slot0 + sp->link >= K) || sp->radius_class < 0 || sp->radius_class >= n_radii) return -1;
+            /* "we approximate the robot (and the current grasped object, if any) with a set of spheres"
+             * (PAPER.md:111): link == -1 attaches the sphere to the grasped object -- its centre is given in that
+             * object's frame and moves with inst_xform[n][held_slot[n]].  With nothing in the gripper the sphere does
+             * not exist: it reports free space and no object. */
+            int frame = link_slot0 + sp->link;
+            if (sp->link == -1) {
+                const int hs = held_slot ? held_slot[n] : -1;
+                if (hs >= K) return -1;
+                if (hs < 0) {
+                    out_static[(size_t)n * S + s] = 0;
+                    out_object[(size_t)n * S + s] = -1;
+                    continue;
+                }
+                frame = hs;
+            }
+            const float *Wl = inst_xform + ((size_t)n * K + frame) * 16;
             float c[3];
             for (int i = 0; i < 3; ++i)   /* N3's order */
                 c[i] = fmaf(Wl[i * 4 + 2], sp->centre[2], fmaf(Wl[i * 4 + 1], sp->centre[1], fmaf(Wl[i * 4], sp->centre[0], Wl[i * 4 + 3])));

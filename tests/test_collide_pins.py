@@ -184,3 +184,44 @@ def test_bad_arguments(oracle_mod):
     with pytest.raises(ValueError):      # scene index out of range
         oracle_mod.collide([], _open_grid(), [0.05], [gen.Sphere(0, 0, (0, 0, 0))], np.array([1], np.int32),
                            np.full((1, 1), -1, np.int32), np.tile(I44, (1, 1, 1)), 0, 0, 0)
+
+
+def test_spheres_of_the_grasped_object(oracle_mod):
+    """'we approximate the robot (and the current grasped object, if any) with a set of spheres' (PAPER.md:111): a
+    sphere with link == -1 rides on the object in the gripper, inst_xform[n][held_slot[n]].  By hand:
+    column grid with spacing 1, column (ix, iz) free only at height y == iz for ix == 2 (as in the link-transform pin);
+    the held object (slot 1) is turned +90 degrees about Z and stands at (2, 0, 3): its sphere at (3, 0, 0) in the
+    object's frame is at (2, 3, 3) in the world -> free; at (1, 0, 0) -> (2, 1, 3) -> obstructed.  The robot-link sphere
+    (link 0, identity transform in slot 2) at the same local points lands elsewhere: (3, 0, 0) -> column 3, closed.
+    Boxes: slot 0 holds a unit cube at the origin shifted to x = 2.5, so it spans x in [2, 3]; the held sphere at world
+    (2, 3, 3) is far from it; a held sphere at local (0, 0.25, -3) -> world (1.75, 0, 0) is 0.25 from the face x = 2:
+    radius 0.25 touches (inclusive) -> slot 0.  The held object's own box (slot 1) is never reported.
+    With nothing held (held_slot -1, or no held_slot array) the sphere does not exist: (0, -1)."""
+    g = [[_grid(0.0, 0.0, 1.0, 4, 4, [[[(float(iz), float(iz))] if ix == 2 else [] for ix in range(4)] for iz in range(4)])]]
+    cube = _boxmesh((-0.5, -0.5, -0.5), (0.5, 0.5, 0.5))
+    Hm = np.array([[0, -1, 0, 2.0], [1, 0, 0, 0.0], [0, 0, 1, 3.0], [0, 0, 0, 1]], np.float32).reshape(16)
+    box = I44.copy(); box[3] = 2.5
+    K = 3
+    xf = np.stack([box, Hm, I44]).reshape(1, K, 16)
+    im = np.array([[0, 0, -1]], np.int32)
+    sph = [gen.Sphere(-1, 0, (3.0, 0.0, 0.0)), gen.Sphere(-1, 0, (1.0, 0.0, 0.0)), gen.Sphere(0, 0, (3.0, 0.0, 0.0)),
+           gen.Sphere(-1, 0, (0.0, 0.25, -3.0)), gen.Sphere(-1, 0, (0.0, 0.2578125, -3.0)), gen.Sphere(-1, 0, (0.0, 0.0, 0.0))]
+    call = lambda held: oracle_mod.collide([cube], g, [0.25], sph, np.zeros(1, np.int32), im, xf, 2, 0, 2, held)
+    s, o = call(np.array([1], np.int32))
+    # world centres: (2,3,3) free | (2,1,3) column (2,3) wants y == 3 | link sphere (3,0,0): column 3 is closed |
+    # (1.75,0,0) and (1.7421875,0,0): nearest column (2,0), free at y == 0 | (2,0,3): column (2,3) wants y == 3
+    assert list(s[0]) == [0, 1, 1, 0, 0, 1]
+    assert list(o[0]) == [-1, -1, 0, 0, -1, -1]      # link sphere (3,0,0) touches the face x = 3; held: exactly r -> 0, one step beyond -> none;
+    #                                                  the sphere at the held object's own centre never reports slot 1
+    for held in (np.array([-1], np.int32), None):
+        s, o = call(held)
+        assert list(s[0][[0, 1, 3, 4, 5]]) == [0] * 5 and list(o[0][[0, 1, 3, 4, 5]]) == [-1] * 5
+        assert s[0][2] == 1 and o[0][2] == 0         # the robot's own sphere is unaffected
+    # held slot that is also inside the object window but empty in inst_mesh: the transform still carries the sphere
+    im2 = np.array([[0, -1, -1]], np.int32)
+    s, o = oracle_mod.collide([cube], g, [0.25], sph, np.zeros(1, np.int32), im2, xf, 2, 0, 2, np.array([1], np.int32))
+    assert list(s[0]) == [0, 1, 1, 0, 0, 1] and list(o[0]) == [-1, -1, 0, 0, -1, -1]
+    with pytest.raises(ValueError):                  # link below -1
+        oracle_mod.collide([cube], g, [0.25], [gen.Sphere(-2, 0, (0, 0, 0))], np.zeros(1, np.int32), im, xf, 2, 0, 2, None)
+    with pytest.raises(ValueError):                  # held slot beyond K
+        oracle_mod.collide([cube], g, [0.25], sph, np.zeros(1, np.int32), im, xf, 2, 0, 2, np.array([3], np.int32))
