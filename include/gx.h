@@ -235,10 +235,13 @@ int gx_update_transforms(GxScene *scene, int32_t N, int32_t K, int32_t link_slot
  *   s * n_radii + c: columns in the XZ plane at `spacing` (0.03 m in the paper), column (ix, iz) at
  *   col_off[iz * nx + ix] .. col_off[iz * nx + ix + 1] of `layers`, a layer = (lo, hi), the heights the CENTRE of a
  *   sphere of that radius may take (both inclusive).  radii [n_radii]: the sphere-radius working set ({0.015, 0.05,
- *   0.12} in the paper).  spheres [n_spheres]: link index (>= 0), radius class, centre in the link's frame.
+ *   0.12} in the paper).  spheres [n_spheres]: link index (>= 0), radius class, centre in the link's frame; link -1
+ *   puts the sphere on the grasped object ("the robot (and the current grasped object, if any)"): its
+ *   centre is in that object's frame and it moves with inst_xform[n][held_slot[n]].
  *   Errors: INVALID_ARG, UNSUPPORTED (more than 2^32 columns or layers), OOM, CUDA.
  * gx_collide_batch: DEVICE arrays.  Sphere centres are W_link * centre with W_link = inst_xform[n][link_slot0 + link]
- *   (what gx_update_transforms wrote).  The box of instance slot k is the object-space bounding box of its mesh
+ *   (what gx_update_transforms wrote); for a sphere with link -1, W = inst_xform[n][held_slot[n]], and where nothing
+ *   is held (held_slot NULL, or held_slot[n] outside [0, K)) that sphere reports 0 and -1.  The box of instance slot k is the object-space bounding box of its mesh
  *   under inst_xform[n][k], which must be rigid.
  *   out_static [N, n_spheres] uint8: 1 if the sphere is in obstructed space of its column grid or outside the grid.
  *   out_object [N, n_spheres] int32: the lowest slot in [obj_slot0, obj_slot0 + n_obj) whose box the sphere overlaps

@@ -882,7 +882,7 @@ int gx_set_collision_world(GxScene *sc, const GxColumnGrid *grids, int32_t n_rad
     std::vector<gx::SphereDev> hs((size_t)n_spheres);
     int max_link = -1;
     for (int i = 0; i < n_spheres; ++i) {
-        if (spheres[i].link < 0 || spheres[i].radius_class < 0 || spheres[i].radius_class >= n_radii)
+        if (spheres[i].link < -1 || spheres[i].radius_class < 0 || spheres[i].radius_class >= n_radii)   // (-1: on the grasped object)
             return fail(GX_ERR_INVALID_ARG, "sphere %d: bad link or radius class", i);
         hs[i] = {spheres[i].link, spheres[i].radius_class, spheres[i].centre[0], spheres[i].centre[1], spheres[i].centre[2]};
         max_link = std::max(max_link, spheres[i].link);

@@ -18,7 +18,7 @@ struct ColGridDev {          // one (static scene, radius class) column grid
     uint32_t pad;
 };
 
-struct SphereDev { int32_t link, radius_class; float cx, cy, cz; };
+struct SphereDev { int32_t link, radius_class; float cx, cy, cz; };   // link == -1: rides on the grasped object (slot held_slot[n])
 
 struct CollideParams {
     const ColGridDev *grids;     // [n_static * n_radii]
@@ -55,9 +55,15 @@ __global__ void __launch_bounds__(WARPS * 32) collide_kernel(const CollideParams
         const bool have = s < P.S;
         float cx = 0.f, cy = 0.f, cz = 0.f, r2 = 0.f;
         int hit = 1;
+        bool active = have;      // a sphere of the grasped object (link == -1) exists only while something is held
         if (have) {
+            const SphereDev sp0 = P.spheres[s];
+            if (sp0.link < 0) active = held >= 0 && held < P.K;
+            if (!active) hit = 0;
+        }
+        if (active) {
             const SphereDev sp = P.spheres[s];
-            const float *W = xf + (size_t)(P.link_slot0 + sp.link) * 16;
+            const float *W = xf + (size_t)(sp.link < 0 ? held : P.link_slot0 + sp.link) * 16;
             cx = fmaf(W[2], sp.cz, fmaf(W[1], sp.cy, fmaf(W[0], sp.cx, W[3])));      // N3's order
             cy = fmaf(W[6], sp.cz, fmaf(W[5], sp.cy, fmaf(W[4], sp.cx, W[7])));
             cz = fmaf(W[10], sp.cz, fmaf(W[9], sp.cy, fmaf(W[8], sp.cx, W[11])));
@@ -101,7 +107,7 @@ __global__ void __launch_bounds__(WARPS * 32) collide_kernel(const CollideParams
                 }
             }
             __syncwarp();
-            if (have && found < 0) {
+            if (active && found < 0) {
                 for (int k = 0; k < nk; ++k) {
                     const float *o = s_obj[warp][k];
                     if (o[18] == 0.0f) continue;

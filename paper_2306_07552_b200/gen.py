@@ -749,6 +749,12 @@ def robot_spheres(robot: Robot) -> List[Sphere]:
     return out
 
 
+def held_object_spheres() -> List[Sphere]:
+    """Spheres of the object in the gripper ("and the current grasped object, if any"): link -1, centres
+    in the object's own frame; three of the 5 cm class along its vertical axis and one small one off to the side."""
+    return [Sphere(-1, 1, (0.0, dy, 0.0)) for dy in (-0.06, 0.0, 0.06)] + [Sphere(-1, 0, (0.05, 0.0, 0.03))]
+
+
 def collision_world(n_envs: int, seed: int = 0, cfg: int = 1, extent: Optional[Tuple[float, float, float, float]] = None):
     """A batch of collision queries shaped like the paper's step (1 target + 29 distractor objects
     per episode; App. G): the robot proxy with its spheres in n_envs environments of one apartment, 30 resting

@@ -46,6 +46,8 @@ def test_collide_matches_oracle_after_fk(oracle_mod):
     grids = [[gen.column_grid(1, 0, r, ext) for r in gen.SPHERE_RADII]]
     for n, held in ((1, True), (37, True), (1030, False)):      # ragged last block of 4 warps
         w = gen.collision_world(n, seed=n, extent=ext)
+        n_robot = len(w["spheres"])
+        w["spheres"] = w["spheres"] + gen.held_object_spheres()       # link -1: they ride on the grasped object
         hs, hx = (w["held_slot"], w["held_xform"]) if held else (None, None)
         _, xf = oracle_mod.fk(w["robot"], w["base_pose"], w["joint_pos"], w["K"], w["link_slot0"], inst_xform=w["inst_xform"],
                               held_slot=hs, held_xform=hx)
@@ -56,6 +58,11 @@ def test_collide_matches_oracle_after_fk(oracle_mod):
         assert np.array_equal(so, sg) and np.array_equal(oo, og)
         if n > 30:
             assert 0.05 < so.mean() < 0.95 and (oo >= 0).any() and (oo < 0).any()
+        holding = (w["held_slot"] >= 0) if held else np.zeros(n, bool)
+        assert not so[~holding, n_robot:].any() and (oo[~holding, n_robot:] == -1).all()     # nothing held: no such sphere
+        if n == 37:
+            assert holding.any() and so[holding, n_robot:].any() and not so[holding, n_robot:].all()
+            assert not (oo[holding, n_robot:] == 0).any()             # never its own box (slot 0 is the held object)
 
 
 def test_collide_two_scenes_object_windows_and_many_objects(oracle_mod):
@@ -66,7 +73,7 @@ def test_collide_two_scenes_object_windows_and_many_objects(oracle_mod):
     w = gen.collision_world(50, seed=9, extent=(3.5, 3.5, 5.5, 5.5))
     rng = np.random.default_rng(2)
     w["env_scene"] = rng.integers(0, 2, 50).astype(np.int32)
-    w["spheres"] = w["spheres"] + [gen.Sphere(int(rng.integers(0, 5)), int(rng.integers(0, 3)), tuple(rng.uniform(-0.3, 0.3, 3))) for _ in range(13)]
+    w["spheres"] = w["spheres"] + [gen.Sphere(int(rng.integers(-1, 5)), int(rng.integers(0, 3)), tuple(rng.uniform(-0.3, 0.3, 3))) for _ in range(13)]
     # 70 object slots: the 30 of the generator, then 40 more copies jittered
     N, L = 50, 5
     K = 70 + L
