@@ -40,6 +40,22 @@ if ROOT not in sys.path:
 METRIC = "rendered env-frames/sec (RGBD) at 1 B200; HBM-roofline fraction"
 UNIT = "env-frames/s"
 NOMINAL_HBM_GBS = 8000.0        # north_star divides by 8 TB/s
+TRAFFIC_CSV = "r3_traffic.csv"  # ncu capture of DRAM bytes and warp instructions per kernel (profiles/), stamped with csrc_sha16
+
+
+def csrc_sha16() -> str:
+    """Identity of the kernels a profile was taken from: sha256 over every source file under csrc/ (sorted by name)
+    and the nvcc flags, first 16 hex digits.  `python bench.py --csrc-sha` prints it."""
+    import hashlib
+    from paper_2306_07552_b200 import build as gx_build
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(gx_build.CSRC)):
+        if name.endswith((".cu", ".cuh", ".h")):
+            h.update(name.encode())
+            with open(os.path.join(gx_build.CSRC, name), "rb") as f:
+                h.update(f.read())
+    h.update(" ".join(gx_build.NVCC_FLAGS).encode())
+    return h.hexdigest()[:16]
 FALLBACK_HBM_GBS = 6650.0       # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
 
 
@@ -439,17 +455,27 @@ def run_gx(args):
     achieved_kernels = bytes_per_launch / (kernel_ms * 1e-3) / 1e9
     # DRAM bytes per launch of all our kernels: not measured in this run (ncu replays kernels); taken from the
     # committed ncu capture of the same workload, whose header names the commit it was captured at
+    # A capture is only quoted for the kernels it was taken from: every row carries the hash of csrc/ and the build
+    # flags at capture time (csrc_sha16), and when the tree has moved on `traffic` is null and the reason is given.
     traffic, traffic_src, warp_inst = None, None, None
     try:
         import csv
-        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", TRAFFIC_CSV)) as f:
             rows = [r for r in csv.DictReader(f) if int(r["workload_config"]) == args.config]
-        if rows and not args.opt and not args.envs and not args.obs:
+        here = csrc_sha16()
+        if not rows:
+            traffic_src = f"no ncu capture of config {args.config} in profiles/{TRAFFIC_CSV}"
+        elif args.opt or args.envs or args.obs or args.frame:
+            traffic_src = f"profiles/{TRAFFIC_CSV} was captured with the default options and shape, this run differs"
+        elif any(r.get("csrc_sha16") != here for r in rows):
+            traffic_src = (f"stale: profiles/{TRAFFIC_CSV} was captured at csrc_sha16 {rows[0].get('csrc_sha16')}, "
+                           f"this tree is {here}; re-capture (profiles/r3_pipeline_ncu.md has the commands)")
+        else:
             traffic = float(sum(int(r["dram_bytes_per_launch"]) for r in rows))
             warp_inst = float(sum(int(r["warp_instructions"]) for r in rows))
-            traffic_src = "profiles/r2_traffic.csv (ncu --set full capture; commit in profiles/r2_pipeline_ncu.md)"
-    except Exception:
-        pass
+            traffic_src = f"profiles/{TRAFFIC_CSV} (ncu capture of the same csrc_sha16 {here}; commands in profiles/r3_pipeline_ncu.md)"
+    except Exception as e:
+        traffic_src = f"profiles/{TRAFFIC_CSV} unreadable: {e}"
     dom = max(kernels_ms, key=kernels_ms.get) if timed_calls else "raster"
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
@@ -482,7 +508,7 @@ def run_gx(args):
                               ("depth f32" if wl.depth_only else "rgb u8 + depth f32"),
                    "l2": "256 MB buffer written between timed iterations (untimed)",
                    "arithmetic": "f32 vertex stage, i32/i64 fixed-point coverage, f32 depth/colour"},
-        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches) * args.steps * world,
+        "clocks": clk.summary(), "e2e": e2e, "gpu_launches": int(launches) * args.steps * world, "csrc_sha16": csrc_sha16(),
         "ms_per_step_per_rank": per_rank_ms, "scene_graph_update": fk, "collision_queries": collide,
         "roofline": roofline, "cpu_baseline": cpu,
     }
@@ -493,6 +519,9 @@ def run_gx(args):
 
 
 def main():
+    if "--csrc-sha" in sys.argv:
+        print(csrc_sha16())
+        return
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
